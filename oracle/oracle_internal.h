@@ -1,0 +1,64 @@
+/* HMLFC oracle (test infrastructure) -- internal types shared by the oracle's own .c files only. */
+#ifndef HMLFC_ORACLE_INTERNAL_H
+#define HMLFC_ORACLE_INTERNAL_H
+
+#include "hmlfc_oracle.h"
+
+#define ORC_MAX_LEVELS 8
+
+/* per-block record of a plane-channel */
+typedef struct {
+    int32_t mode;  /* 0 subtractive (P = e + R), 1 additive (P = e - R)  -- reading R10 */
+    int32_t dx, dy;
+    int32_t sad;   /* Delta = min(Delta-, Delta+) */
+    int32_t E;     /* energy of the original SRV block: sum |px| */
+    int32_t flags; /* bit0 res, bit1 pred */
+} orc_block;
+
+struct orc_tree {
+    orc_params p;
+    int h;
+    int UL[ORC_MAX_LEVELS + 1], VL[ORC_MAX_LEVELS + 1];
+    int nbx, nby, nblk;
+    /* X[c][L][pv*UL+pu] : int16 [Ht*Ws], L = 0..h ; srv[c][L][...] : L = 0..h-1 */
+    int16_t **X[3][ORC_MAX_LEVELS + 1];
+    int16_t **srv[3][ORC_MAX_LEVELS];
+    orc_block *blk[3][ORC_MAX_LEVELS]; /* [UL*VL][nblk] */
+    int thresholded;
+};
+
+/* ---- stream constants ---- */
+#define ORC_HEADER_BYTES 160
+#define ORC_DIRENT_BYTES 48
+#define ORC_VERSION 1
+
+/* directory entry as parsed */
+typedef struct {
+    int32_t offset;      /* value bias: stored value = offset + BISE value */
+    uint32_t N;
+    uint32_t n_res, n_pred;
+    uint64_t flags_off;  /* bytes from the flags section */
+    uint64_t pay_bitoff; /* bits from the payload section */
+    uint64_t mv_bitoff;  /* bits from the MV section */
+    int32_t layout, m;
+} orc_dirent;
+
+struct orc_stream {
+    orc_params p;
+    int h;
+    int UL[ORC_MAX_LEVELS + 1], VL[ORC_MAX_LEVELS + 1];
+    int nbx, nby, nblk;
+    uint8_t *bytes;
+    size_t len;
+    uint64_t off_rkv, off_dir, off_flags, off_payload, off_mv, total;
+    uint64_t n_pc;
+    orc_dirent *dir;            /* [n_pc] in stream order */
+    uint64_t level_base[ORC_MAX_LEVELS]; /* first directory index of level L */
+    uint32_t **rank_res;        /* [n_pc][nblk+1] exclusive prefix counts (built at open) */
+    uint32_t **rank_pred;       /* same for pred maps (NULL for reference planes) */
+    uint32_t mvN;               /* 2 (2W+1)^2 */
+};
+
+static inline int orc_is_predictive(int pu, int pv) { return ((pu | pv) & 1) != 0; }
+
+#endif
