@@ -1,0 +1,144 @@
+/*
+ * hmlfc.h -- C ABI of the B200-native HMLFC decode + render library (libhmlfc_b200.so).
+ *
+ * The hot path of "HMLFC: Hierarchical Motion-Compensated Light Field Compression for
+ * Interactive Rendering" (arXiv 1902.09396): random-access per-pixel decoding of the
+ * hierarchical, phase-shifted motion-compensated representation (section
+ * 4.8), fused with two-plane (u,v,s,t) novel-view rendering.
+ * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - (u,v) = camera-grid index, U x V views; (s,t) = pixel column/row inside a view, Ws x Ht.
+ *   - All functions return 0 on success or a negative HMLFC_E_* code; no exceptions cross the ABI.
+ *   - Pointers named h_* are HOST pointers, d_* are DEVICE pointers on the device that was
+ *     current when hmlfc_load() ran.  cuda_stream is a cudaStream_t passed as void* (NULL = the
+ *     legacy default stream).
+ *   - decode / render / footprint only ENQUEUE work on cuda_stream and return without
+ *     synchronising; the *_host variants synchronise before returning.
+ *   - The handle is immutable after load apart from its counters; concurrent launches on
+ *     different streams are legal (the out-of-range counter is shared and atomic).
+ */
+#ifndef HMLFC_H
+#define HMLFC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    HMLFC_OK = 0,
+    HMLFC_E_MAGIC = -1,        /* stream does not start with "HMLF"                          */
+    HMLFC_E_TRUNCATED = -2,    /* fewer bytes than the header / directory say                */
+    HMLFC_E_VERSION = -3,      /* stream version is not 1                                    */
+    HMLFC_E_INVALID = -4,      /* null pointer, n < 0, W/H <= 0, ...                          */
+    HMLFC_E_UNSUPPORTED = -5,  /* B not in {2,4,8} or B does not divide Ws/Ht, chroma         */
+                               /* subsampling set, RKV codec != raw, height > 8              */
+    HMLFC_E_CORRUPT = -6,      /* directory inconsistent with the section sizes              */
+    HMLFC_E_NOMEM = -7,        /* host or device allocation failed                           */
+    HMLFC_E_CUDA = -8          /* a CUDA runtime call failed (see hmlfc_last_cuda_error)     */
+};
+
+typedef struct hmlfc_handle hmlfc_handle; /* opaque; owns every device allocation */
+
+/* Stream parameters (header of the compressed stream) and the sizes of its device form. */
+typedef struct {
+    int32_t U, V, Ws, Ht;
+    int32_t height;            /* tree height h ("tree height")              */
+    int32_t block;             /* block size B                                            */
+    int32_t window;            /* search window W: motion vectors lie in [-W, W]^2        */
+    int32_t tau_ref, tau_res;  /* the encoder's two block thresholds       */
+    float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st; /* light slab geometry */
+    uint8_t background[3];     /* colour of rays that miss the slab                       */
+    uint8_t _pad;
+    uint64_t stream_bytes;     /* length of the serialized stream                         */
+    uint64_t device_bytes;     /* bytes resident in HBM after load (all tables)           */
+    uint64_t n_plane_channels; /* SRV plane-channels in the tree                          */
+} hmlfc_info_t;
+
+/* One output camera: a ray basis, not necessarily orthonormal (off-axis frusta are expressible).
+ * Output pixel (i,j) of a W x H view looks along
+ *   D = fwd + ((2(i+.5)/W - 1) tan_half_x) right + ((2(j+.5)/H - 1) tan_half_y) down
+ * from eye, in the light slab's world frame (camera plane z = 0, image plane z = z_st). */
+typedef struct {
+    float eye[3], right[3], down[3], fwd[3];
+    float tan_half_x, tan_half_y;
+    float _pad[2];
+} hmlfc_camera; /* 64 bytes */
+
+/* Algorithmic-bytes accounting of one render or decode batch: every distinct
+ * (plane-channel, block) touched -- including reference blocks reached through motion
+ * vectors -- counts once. */
+typedef struct {
+    int64_t blocks_touched;
+    int64_t flag_bits;       /* 1 bit per touched block of a reference plane, 2 of a predictive one */
+    int64_t payload_bits15;  /* payload bits of touched significant blocks, in units of 1/15 bit    */
+    int64_t mv_bits15;       /* motion-record bits of touched predicted blocks, in 1/15 bit         */
+    int64_t rkv_bytes;       /* distinct top-level RKV samples touched: 1 (Y) or 2 (Co,Cg) bytes    */
+    int64_t out_bytes, in_bytes;
+    double bytes_alg;        /* total bytes                                                          */
+} hmlfc_footprint_t;
+
+/* hmlfc_load -- PAPER.md:293 "the top-level RKV images are decoded and stored in memory",
+ * PAPER.md:296 "the reference SRV images at all the levels are ... loaded into the memory".
+ * Parses the serialized stream (layout: DESIGN.md "Stream format v1"), re-packs it into the
+ * device structure-of-arrays form (flag + rank records, bit-packed BISE payloads and motion
+ * vectors, packed top-level RKVs) and uploads it to the current CUDA device.
+ *   h_stream_bytes : host, read only during the call; the caller may free it afterwards.
+ *   out            : receives the handle; untouched on error.                              */
+int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out);
+
+int hmlfc_info(const hmlfc_handle *h, hmlfc_info_t *out);
+
+/* hmlfc_decode -- PAPER.md:289-293 (decoding procedure) and :309 (random access): for each
+ * coordinate, top-level RKV sample + sum over the levels of the SRV sample (stored block value,
+ * plus or minus the motion-shifted reference-SRV sample for predicted blocks), inverse YCoCg-R,
+ * clamp to [0,255].
+ *   d_coords : device, int32 [n][4] = (u, v, s, t), row-major.
+ *   d_out    : device, uint8 [n][3] RGB.
+ * An out-of-range coordinate writes (0,0,0) and increments the handle's out-of-range counter. */
+int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint8_t *d_out, void *cuda_stream);
+
+/* hmlfc_render -- PAPER.md:73 / :309 / :409: per output pixel, ray -> (u,v,s,t) on the two
+ * planes, 16-tap quadrilinear blend of decoded samples (4 nearest views x 4 nearest pixels,
+ * edge-clamped), rounded to RGB8; rays that miss the slab get the background colour.
+ *   d_cameras : device, hmlfc_camera [n_views].
+ *   d_out     : device, uint8 [n_views][H][W][3], row-major, no padding.                    */
+int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                 void *cuda_stream);
+
+/* End-to-end variants with HOST buffers: copy the inputs to the device, run the same kernels,
+ * copy the result back, synchronise.  Scratch device buffers live in the handle and grow on
+ * demand (so these two calls are not re-entrant on one handle).  Pinned host memory makes
+ * the copies asynchronous DMA; pageable memory works too. */
+int hmlfc_decode_host(hmlfc_handle *h, const int32_t *h_coords, int64_t n, uint8_t *h_out);
+int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, int W, int H, uint8_t *h_out);
+
+/* Synchronous: the number of out-of-range coordinates seen by hmlfc_decode since load. */
+int hmlfc_last_oob_count(const hmlfc_handle *h, int64_t *out);
+
+/* Measurement aid (not on the hot path): marks every block / RKV sample the batch touches with
+ * a kernel, then reduces the marks to the algorithmic-byte count.  Synchronous. */
+int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H,
+                           hmlfc_footprint_t *out);
+int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out);
+
+/* Kernel selection for hmlfc_render: 0 = automatic (default), 1 = one thread per output pixel
+ * (16 independent tap decodes), 2 = tile-shared (a CTA decodes its tile's LF footprint once
+ * into shared memory).  All variants produce identical bytes. */
+int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
+
+/* Number of kernels this library has launched through the handle since load (bench accounting). */
+int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);
+
+void hmlfc_free(hmlfc_handle *h);
+const char *hmlfc_strerror(int code);
+/* cudaError_t of the most recent failed CUDA call made through this handle (0 if none). */
+int hmlfc_last_cuda_error(const hmlfc_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HMLFC_H */

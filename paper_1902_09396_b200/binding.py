@@ -1,0 +1,226 @@
+"""Thin Python binding of libhmlfc_b200.so (include/hmlfc.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing, or a call needs
+a GPU and none is present, the call raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
+
+# every symbol include/hmlfc.h declares
+EXPORTS = (
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant",
+    "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
+)
+
+RENDER_AUTO, RENDER_PIXEL, RENDER_TILED = 0, 1, 2
+
+
+class HmlfcError(RuntimeError):
+    def __init__(self, code, what, detail=""):
+        super().__init__(f"{what}: {detail or code} (code {code})")
+        self.code = code
+
+
+class Info(C.Structure):
+    _fields_ = [
+        ("U", C.c_int32), ("V", C.c_int32), ("Ws", C.c_int32), ("Ht", C.c_int32),
+        ("height", C.c_int32), ("block", C.c_int32), ("window", C.c_int32),
+        ("tau_ref", C.c_int32), ("tau_res", C.c_int32),
+        ("uv_origin", C.c_float * 2), ("uv_step", C.c_float * 2), ("st_origin", C.c_float * 2),
+        ("st_step", C.c_float * 2), ("z_st", C.c_float),
+        ("background", C.c_uint8 * 3), ("_pad", C.c_uint8),
+        ("stream_bytes", C.c_uint64), ("device_bytes", C.c_uint64), ("n_plane_channels", C.c_uint64),
+    ]
+
+
+class Footprint(C.Structure):
+    _fields_ = [
+        ("blocks_touched", C.c_int64), ("flag_bits", C.c_int64), ("payload_bits15", C.c_int64),
+        ("mv_bits15", C.c_int64), ("rkv_bytes", C.c_int64), ("out_bytes", C.c_int64), ("in_bytes", C.c_int64),
+        ("bytes_alg", C.c_double),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA library; fail loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise HmlfcError(-1, "libhmlfc_b200.so not built",
+                         f"{LIB_PATH} is missing; run `python -m paper_1902_09396_b200.build` (there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64 = C.c_void_p, C.c_int64
+    L.hmlfc_load.argtypes, L.hmlfc_load.restype = [vp, C.c_size_t, C.POINTER(vp)], C.c_int
+    L.hmlfc_info.argtypes, L.hmlfc_info.restype = [vp, C.POINTER(Info)], C.c_int
+    L.hmlfc_decode.argtypes, L.hmlfc_decode.restype = [vp, vp, i64, vp, vp], C.c_int
+    L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
+    L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
+    L.hmlfc_render_host.argtypes, L.hmlfc_render_host.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp], C.c_int
+    L.hmlfc_last_oob_count.argtypes, L.hmlfc_last_oob_count.restype = [vp, C.POINTER(i64)], C.c_int
+    L.hmlfc_footprint_render.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(Footprint)]
+    L.hmlfc_footprint_render.restype = C.c_int
+    L.hmlfc_footprint_decode.argtypes, L.hmlfc_footprint_decode.restype = [vp, vp, i64, C.POINTER(Footprint)], C.c_int
+    L.hmlfc_set_render_variant.argtypes, L.hmlfc_set_render_variant.restype = [vp, C.c_int], C.c_int
+    L.hmlfc_launch_count.argtypes, L.hmlfc_launch_count.restype = [vp, C.POINTER(i64)], C.c_int
+    L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
+    L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
+    L.hmlfc_last_cuda_error.argtypes, L.hmlfc_last_cuda_error.restype = [vp], C.c_int
+    _lib = L
+    return L
+
+
+def _check(rc, what, handle=None):
+    if rc != 0:
+        detail = lib().hmlfc_strerror(rc).decode()
+        if handle is not None and rc == -8:
+            detail += f" (cudaError {lib().hmlfc_last_cuda_error(handle)})"
+        raise HmlfcError(rc, what, detail)
+
+
+def _require_cuda():
+    import torch
+
+    if not torch.cuda.is_available():
+        raise HmlfcError(-8, "no CUDA device", "the HMLFC hot path runs only on the GPU (there is no CPU fallback)")
+    return torch
+
+
+def _stream_ptr(stream):
+    torch = _require_cuda()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Handle:
+    """Owns one loaded stream on the current CUDA device."""
+
+    def __init__(self, ptr):
+        self._h = ptr
+        self.info = Info()
+        _check(lib().hmlfc_info(self._h, C.byref(self.info)), "hmlfc_info")
+
+    def free(self):
+        if self._h:
+            lib().hmlfc_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def hmlfc_load(stream_bytes: bytes) -> Handle:
+    """Upload a serialized HMLFC stream to the current CUDA device (include/hmlfc.h: hmlfc_load)."""
+    _require_cuda().cuda.current_device()  # make sure a context exists on the current device
+    buf = np.frombuffer(stream_bytes, dtype=np.uint8)
+    out = C.c_void_p()
+    _check(lib().hmlfc_load(buf.ctypes.data_as(C.c_void_p), buf.size, C.byref(out)), "hmlfc_load")
+    return Handle(out)
+
+
+def hmlfc_decode(h: Handle, coords, out=None, stream=None):
+    """coords: CUDA int32 tensor [n][4] = (u,v,s,t); returns CUDA uint8 tensor [n][3]."""
+    torch = _require_cuda()
+    assert coords.is_cuda and coords.dtype == torch.int32 and coords.is_contiguous() and coords.shape[-1] == 4
+    n = coords.numel() // 4
+    if out is None:
+        out = torch.empty((n, 3), dtype=torch.uint8, device=coords.device)
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == 3 * n
+    _check(lib().hmlfc_decode(h._h, C.c_void_p(coords.data_ptr()), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
+           "hmlfc_decode", h._h)
+    return out
+
+
+def hmlfc_render(h: Handle, cameras, W: int, H: int, out=None, stream=None):
+    """cameras: CUDA float32 tensor [n_views][16]; returns CUDA uint8 tensor [n_views][H][W][3]."""
+    torch = _require_cuda()
+    assert cameras.is_cuda and cameras.dtype == torch.float32 and cameras.is_contiguous() and cameras.shape[-1] == 16
+    n = cameras.numel() // 16
+    if out is None:
+        out = torch.empty((n, H, W, 3), dtype=torch.uint8, device=cameras.device)
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * H * W * 3
+    _check(lib().hmlfc_render(h._h, C.c_void_p(cameras.data_ptr()), n, W, H, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
+           "hmlfc_render", h._h)
+    return out
+
+
+def hmlfc_decode_host(h: Handle, coords: np.ndarray, out: np.ndarray = None) -> np.ndarray:
+    """End-to-end decode with HOST buffers (numpy, ideally backed by pinned memory)."""
+    _require_cuda()
+    assert coords.dtype == np.int32 and coords.flags.c_contiguous and coords.shape[-1] == 4
+    n = coords.size // 4
+    if out is None:
+        out = np.empty((n, 3), dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.flags.c_contiguous and out.size == 3 * n
+    _check(lib().hmlfc_decode_host(h._h, coords.ctypes.data_as(C.c_void_p), n, out.ctypes.data_as(C.c_void_p)),
+           "hmlfc_decode_host", h._h)
+    return out
+
+
+def hmlfc_render_host(h: Handle, cameras: np.ndarray, W: int, H: int, out: np.ndarray = None) -> np.ndarray:
+    """End-to-end render with HOST buffers (numpy, ideally backed by pinned memory)."""
+    _require_cuda()
+    assert cameras.dtype == np.float32 and cameras.flags.c_contiguous and cameras.shape[-1] == 16
+    n = cameras.size // 16
+    if out is None:
+        out = np.empty((n, H, W, 3), dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.flags.c_contiguous and out.size == n * H * W * 3
+    _check(lib().hmlfc_render_host(h._h, cameras.ctypes.data_as(C.c_void_p), n, W, H, out.ctypes.data_as(C.c_void_p)),
+           "hmlfc_render_host", h._h)
+    return out
+
+
+def hmlfc_last_oob_count(h: Handle) -> int:
+    v = C.c_int64()
+    _check(lib().hmlfc_last_oob_count(h._h, C.byref(v)), "hmlfc_last_oob_count", h._h)
+    return v.value
+
+
+def hmlfc_footprint_render(h: Handle, cameras, W: int, H: int) -> dict:
+    torch = _require_cuda()
+    assert cameras.is_cuda and cameras.dtype == torch.float32 and cameras.is_contiguous()
+    fp = Footprint()
+    torch.cuda.synchronize()
+    _check(lib().hmlfc_footprint_render(h._h, C.c_void_p(cameras.data_ptr()), cameras.numel() // 16, W, H, C.byref(fp)),
+           "hmlfc_footprint_render", h._h)
+    return fp.as_dict()
+
+
+def hmlfc_footprint_decode(h: Handle, coords) -> dict:
+    torch = _require_cuda()
+    assert coords.is_cuda and coords.dtype == torch.int32 and coords.is_contiguous()
+    fp = Footprint()
+    torch.cuda.synchronize()
+    _check(lib().hmlfc_footprint_decode(h._h, C.c_void_p(coords.data_ptr()), coords.numel() // 4, C.byref(fp)),
+           "hmlfc_footprint_decode", h._h)
+    return fp.as_dict()
+
+
+def hmlfc_set_render_variant(h: Handle, variant: int):
+    _check(lib().hmlfc_set_render_variant(h._h, variant), "hmlfc_set_render_variant")
+
+
+def hmlfc_launch_count(h: Handle) -> int:
+    v = C.c_int64()
+    _check(lib().hmlfc_launch_count(h._h, C.byref(v)), "hmlfc_launch_count")
+    return v.value
+
+
+def hmlfc_free(h: Handle):
+    h.free()

@@ -1,0 +1,278 @@
+// C ABI of libhmlfc_b200.so (include/hmlfc.h): stream parsing, device upload, kernel dispatch.
+// The stream byte layout parsed here is DESIGN.md "Stream format v1"; this parser is written
+// from that document and shares no code with the oracle's.
+#include "../../include/hmlfc.h"
+#include "hmlfc_kernels.cuh"
+#include "hmlfc_tables.h"
+
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace hmlfc;
+
+struct hmlfc_handle {
+    DevStream ds{};
+    hmlfc_info_t info{};
+    int device = 0;
+    // device allocations
+    uint4 *d_pc = nullptr;
+    uint4 *d_flagrec = nullptr;
+    uint32_t *d_pay = nullptr;
+    uint32_t *d_mv = nullptr;
+    short4 *d_rkv = nullptr;
+    uint32_t *d_bits15 = nullptr;       // per plane-channel BISE bits/value in 1/15 bit (footprint only)
+    unsigned long long *d_oob = nullptr;
+    uint64_t n_pc = 0;
+    uint32_t mv_bits15 = 0;
+    // scratch of the *_host entry points
+    void *d_in = nullptr;
+    size_t d_in_cap = 0;
+    uint8_t *d_outbuf = nullptr;
+    size_t d_out_cap = 0;
+    cudaStream_t host_stream = nullptr;
+    int render_variant = 0;
+    mutable std::atomic<long long> launches{0};
+    mutable std::atomic<int> last_cuda_error{0};
+};
+
+namespace {
+
+int cuda_fail(const hmlfc_handle *h, cudaError_t e)
+{
+    if (h) h->last_cuda_error.store((int)e);
+    return HMLFC_E_CUDA;
+}
+
+#define CU(h, call)                                            \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) return cuda_fail((h), e__);    \
+    } while (0)
+
+void release(hmlfc_handle *h)
+{
+    if (!h) return;
+    cudaFree(h->d_pc); cudaFree(h->d_flagrec); cudaFree(h->d_pay); cudaFree(h->d_mv); cudaFree(h->d_rkv);
+    cudaFree(h->d_bits15); cudaFree(h->d_oob); cudaFree(h->d_in); cudaFree(h->d_outbuf);
+    if (h->host_stream) cudaStreamDestroy(h->host_stream);
+    delete h;
+}
+
+template <typename T>
+cudaError_t upload(T **dst, const void *src, size_t bytes, size_t slack, uint64_t *total)
+{
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(dst), bytes + slack);
+    if (e != cudaSuccess) return e;
+    if (slack && (e = cudaMemset(reinterpret_cast<uint8_t *>(*dst) + bytes, 0, slack)) != cudaSuccess) return e;
+    if (bytes && (e = cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+    *total += bytes + slack;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *hmlfc_strerror(int code)
+{
+    switch (code) {
+    case HMLFC_OK: return "ok";
+    case HMLFC_E_MAGIC: return "bad magic: not an HMLF stream";
+    case HMLFC_E_TRUNCATED: return "truncated stream";
+    case HMLFC_E_VERSION: return "unsupported stream version";
+    case HMLFC_E_INVALID: return "invalid argument";
+    case HMLFC_E_UNSUPPORTED: return "unsupported stream parameter";
+    case HMLFC_E_CORRUPT: return "corrupt stream directory";
+    case HMLFC_E_NOMEM: return "out of memory";
+    case HMLFC_E_CUDA: return "CUDA runtime error";
+    default: return "unknown error";
+    }
+}
+
+int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
+{
+    if (!h_stream_bytes || !out) return HMLFC_E_INVALID;
+    HostTables T;
+    int rc = build_tables(h_stream_bytes, len, T);
+    if (rc != HMLFC_OK) return rc;
+    hmlfc_handle *h = new (std::nothrow) hmlfc_handle();
+    if (!h) return HMLFC_E_NOMEM;
+    h->ds = T.ds;
+    h->info = T.info;
+    h->n_pc = T.n_pc;
+    h->mv_bits15 = T.mv_bits15;
+    const uint8_t *s = static_cast<const uint8_t *>(h_stream_bytes);
+
+    cudaError_t ce;
+    uint64_t dev_bytes = 0;
+    if ((ce = cudaGetDevice(&h->device)) != cudaSuccess ||
+        (ce = upload(&h->d_pc, T.pc.data(), T.pc.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_flagrec, T.flagrec.data(), T.flagrec.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_pay, s + T.off_pay, (size_t)(T.off_mv - T.off_pay), 16, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_mv, s + T.off_mv, (size_t)(T.total - T.off_mv), 16, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_rkv, T.rkv.data(), T.rkv.size() * sizeof(short4), 0, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_bits15, T.bits15.data(), T.bits15.size() * sizeof(uint32_t), 0, &dev_bytes)) != cudaSuccess ||
+        (ce = cudaMalloc(reinterpret_cast<void **>(&h->d_oob), sizeof(unsigned long long))) != cudaSuccess ||
+        (ce = cudaMemset(h->d_oob, 0, sizeof(unsigned long long))) != cudaSuccess ||
+        (ce = cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking)) != cudaSuccess) {
+        const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
+        release(h);
+        return code;
+    }
+    DevStream &D = h->ds;
+    D.pc = h->d_pc; D.flagrec = h->d_flagrec; D.pay = h->d_pay; D.mv = h->d_mv; D.rkv = h->d_rkv;
+    h->info.device_bytes = dev_bytes;
+    *out = h;
+    return HMLFC_OK;
+}
+
+int hmlfc_info(const hmlfc_handle *h, hmlfc_info_t *out)
+{
+    if (!h || !out) return HMLFC_E_INVALID;
+    *out = h->info;
+    return HMLFC_OK;
+}
+
+int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint8_t *d_out, void *cuda_stream)
+{
+    if (!h || n < 0 || (n > 0 && (!d_coords || !d_out))) return HMLFC_E_INVALID;
+    int nl = 0;
+    CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    h->launches += nl;
+    return HMLFC_OK;
+}
+
+int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                 void *cuda_stream)
+{
+    if (!h || n_views < 0 || W <= 0 || H <= 0 || n_views > 65535 || (n_views > 0 && (!d_cameras || !d_out))) return HMLFC_E_INVALID;
+    static_assert(sizeof(hmlfc_camera) == sizeof(Camera) && sizeof(Camera) == 64, "camera layout");
+    int nl = 0;
+    const Camera *cams = reinterpret_cast<const Camera *>(d_cameras);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (h->render_variant == 1)
+        CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
+    else
+        CU(h, launch_render_tiled(h->ds, cams, n_views, W, H, d_out, st, &nl));
+    h->launches += nl;
+    return HMLFC_OK;
+}
+
+static int ensure(hmlfc_handle *h, void **buf, size_t *cap, size_t need)
+{
+    if (need <= *cap) return HMLFC_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr; *cap = 0;
+    cudaError_t e = cudaMalloc(buf, need);
+    if (e != cudaSuccess) { h->last_cuda_error.store((int)e); return e == cudaErrorMemoryAllocation ? HMLFC_E_NOMEM : HMLFC_E_CUDA; }
+    *cap = need;
+    return HMLFC_OK;
+}
+
+int hmlfc_decode_host(hmlfc_handle *h, const int32_t *h_coords, int64_t n, uint8_t *h_out)
+{
+    if (!h || n < 0 || (n > 0 && (!h_coords || !h_out))) return HMLFC_E_INVALID;
+    if (n == 0) return HMLFC_OK;
+    int rc;
+    if ((rc = ensure(h, &h->d_in, &h->d_in_cap, (size_t)n * 16)) != HMLFC_OK) return rc;
+    if ((rc = ensure(h, reinterpret_cast<void **>(&h->d_outbuf), &h->d_out_cap, (size_t)n * 3 + 4)) != HMLFC_OK) return rc;
+    CU(h, cudaMemcpyAsync(h->d_in, h_coords, (size_t)n * 16, cudaMemcpyHostToDevice, h->host_stream));
+    if ((rc = hmlfc_decode(h, static_cast<const int32_t *>(h->d_in), n, h->d_outbuf, h->host_stream)) != HMLFC_OK) return rc;
+    CU(h, cudaMemcpyAsync(h_out, h->d_outbuf, (size_t)n * 3, cudaMemcpyDeviceToHost, h->host_stream));
+    CU(h, cudaStreamSynchronize(h->host_stream));
+    return HMLFC_OK;
+}
+
+int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, int W, int H, uint8_t *h_out)
+{
+    if (!h || n_views < 0 || W <= 0 || H <= 0 || (n_views > 0 && (!h_cameras || !h_out))) return HMLFC_E_INVALID;
+    if (n_views == 0) return HMLFC_OK;
+    const size_t out_bytes = (size_t)n_views * W * H * 3;
+    int rc;
+    if ((rc = ensure(h, &h->d_in, &h->d_in_cap, (size_t)n_views * sizeof(hmlfc_camera))) != HMLFC_OK) return rc;
+    if ((rc = ensure(h, reinterpret_cast<void **>(&h->d_outbuf), &h->d_out_cap, out_bytes + 4)) != HMLFC_OK) return rc;
+    CU(h, cudaMemcpyAsync(h->d_in, h_cameras, (size_t)n_views * sizeof(hmlfc_camera), cudaMemcpyHostToDevice, h->host_stream));
+    if ((rc = hmlfc_render(h, static_cast<const hmlfc_camera *>(h->d_in), n_views, W, H, h->d_outbuf, h->host_stream)) != HMLFC_OK) return rc;
+    CU(h, cudaMemcpyAsync(h_out, h->d_outbuf, out_bytes, cudaMemcpyDeviceToHost, h->host_stream));
+    CU(h, cudaStreamSynchronize(h->host_stream));
+    return HMLFC_OK;
+}
+
+int hmlfc_last_oob_count(const hmlfc_handle *h, int64_t *out)
+{
+    if (!h || !out) return HMLFC_E_INVALID;
+    unsigned long long v = 0;
+    CU(h, cudaDeviceSynchronize());
+    CU(h, cudaMemcpy(&v, h->d_oob, sizeof(v), cudaMemcpyDeviceToHost));
+    *out = (int64_t)v;
+    return HMLFC_OK;
+}
+
+static int footprint_common(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, const int32_t *d_coords,
+                            int64_t n, hmlfc_footprint_t *out)
+{
+    const DevStream &D = h->ds;
+    const size_t blk_words = ((size_t)h->n_pc * (size_t)D.nblk + 31) / 32 + 1;
+    const size_t rkv_words = ((size_t)D.UH * D.VH * D.Ht * D.Ws + 31) / 32 + 1;
+    FootprintMarks mk{nullptr, nullptr};
+    FootprintTotals *d_tot = nullptr, tot{};
+    int rc = HMLFC_OK;
+    cudaError_t e;
+    if ((e = cudaMalloc(reinterpret_cast<void **>(&mk.blk), blk_words * 4)) != cudaSuccess ||
+        (e = cudaMalloc(reinterpret_cast<void **>(&mk.rkv), rkv_words * 4)) != cudaSuccess ||
+        (e = cudaMalloc(reinterpret_cast<void **>(&d_tot), sizeof(FootprintTotals))) != cudaSuccess ||
+        (e = cudaMemset(mk.blk, 0, blk_words * 4)) != cudaSuccess || (e = cudaMemset(mk.rkv, 0, rkv_words * 4)) != cudaSuccess ||
+        (e = cudaMemset(d_tot, 0, sizeof(FootprintTotals))) != cudaSuccess ||
+        (e = d_cameras ? launch_footprint_render(D, reinterpret_cast<const Camera *>(d_cameras), n_views, W, H, mk, nullptr)
+                       : launch_footprint_decode(D, d_coords, n, mk, nullptr)) != cudaSuccess ||
+        (e = launch_footprint_reduce(D, h->n_pc, h->d_bits15, h->mv_bits15, mk, d_tot, nullptr)) != cudaSuccess ||
+        (e = cudaMemcpy(&tot, d_tot, sizeof(tot), cudaMemcpyDeviceToHost)) != cudaSuccess)
+        rc = cuda_fail(h, e);
+    cudaFree(mk.blk); cudaFree(mk.rkv); cudaFree(d_tot);
+    if (rc != HMLFC_OK) return rc;
+    out->blocks_touched = (int64_t)tot.blocks;
+    out->flag_bits = (int64_t)tot.flag_bits;
+    out->payload_bits15 = (int64_t)tot.payload_bits15;
+    out->mv_bits15 = (int64_t)tot.mv_bits15;
+    out->rkv_bytes = (int64_t)tot.rkv_samples * 5;  // Y 1 byte + Co, Cg 2 bytes each
+    if (d_cameras) { out->out_bytes = (int64_t)n_views * W * H * 3; out->in_bytes = (int64_t)n_views * 64; }
+    else { out->out_bytes = n * 3; out->in_bytes = n * 16; }
+    out->bytes_alg = ((double)out->flag_bits + (double)(out->payload_bits15 + out->mv_bits15) / 15.0) / 8.0 +
+                     (double)out->rkv_bytes + (double)out->out_bytes + (double)out->in_bytes;
+    return HMLFC_OK;
+}
+
+int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, hmlfc_footprint_t *out)
+{
+    if (!h || !out || !d_cameras || n_views <= 0 || n_views > 65535 || W <= 0 || H <= 0) return HMLFC_E_INVALID;
+    return footprint_common(h, d_cameras, n_views, W, H, nullptr, 0, out);
+}
+
+int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out)
+{
+    if (!h || !out || !d_coords || n <= 0) return HMLFC_E_INVALID;
+    return footprint_common(h, nullptr, 0, 0, 0, d_coords, n, out);
+}
+
+int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
+{
+    if (!h || variant < 0 || variant > 2) return HMLFC_E_INVALID;
+    h->render_variant = variant;
+    return HMLFC_OK;
+}
+
+int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out)
+{
+    if (!h || !out) return HMLFC_E_INVALID;
+    *out = h->launches.load();
+    return HMLFC_OK;
+}
+
+int hmlfc_last_cuda_error(const hmlfc_handle *h) { return h ? h->last_cuda_error.load() : 0; }
+
+void hmlfc_free(hmlfc_handle *h) { release(h); }
+
+}  // extern "C"

@@ -1,0 +1,298 @@
+// Device-side data layout and per-sample decode of the HMLFC representation (sm_100a).
+//
+// What is computed: PAPER.md:289-293 (section 4.8.1, decoding procedure) and :309 (random access):
+//   sample(u,v,s,t,c) = topRKV_c[v>>h][u>>h][t][s] + sum_{L<h} SRV_L[(u>>L, v>>L)](s,t)
+//   SRV_L[p](s,t)     = stored_p(s,t)                                   p reference plane
+//                     = stored_p(s,t) +- stored_r(s+dx, t+dy)           p predictive, block predicted
+// with r the cluster's reference plane, (mode,dx,dy) the block's BISE-coded motion record
+// (PAPER.md:276), stored_*(.) = 0 where the block is insignificant or outside the
+// image, then inverse YCoCg-R and clamp.  Readings: DESIGN.md R7-R19.
+//
+// HBM layout (built by hmlfc_load):
+//   pc[]       one 16-byte descriptor per SRV plane-channel: {flag record base, payload word base,
+//              MV word base, offset:16 | layout:2 | m:4 | predictive:1}; the three channels of a
+//              plane are adjacent (48 bytes)
+//   flagrec[]  one 16-byte record per 32 blocks of a plane-channel: {res bits, res rank before,
+//              pred bits, pred rank before} -- flag test and rank come from ONE 128-bit load
+//   pay[], mv[] bit-packed BISE strings as streamed (LSB-first 32-bit words), addressed in O(1)
+//   rkv[]      top-level RKVs as short4 {Y, Co, Cg, 0} per sample: one 64-bit load per sample
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#ifdef HMLFC_HOST_DEBUG
+#define HMLFC_DEV __host__ __device__ inline
+#else
+#define HMLFC_DEV __device__ __forceinline__
+#endif
+
+namespace hmlfc {
+
+constexpr int kMaxLevels = 8;
+
+struct LevelDesc {
+    int32_t UL, VL;    // planes per row / rows of level L
+    uint32_t pc_base;  // index of the level's first plane-channel descriptor
+    uint32_t _pad;
+};
+
+struct DevStream {
+    int32_t U, V, Ws, Ht, h, B, logB, W;
+    int32_t nbx, nby, nblk, fgroups;  // blocks per row / column / plane; 32-block groups per plane-channel
+    int32_t UH, VH;                   // top-level RKV grid
+    uint32_t nd, nd2, nd_magic;       // 2W+1, (2W+1)^2, ceil(2^32 / nd)
+    uint32_t mv_layout, mv_m;         // BISE layout of the motion records, N = 2 (2W+1)^2
+    uint32_t _pad0;
+    LevelDesc lev[kMaxLevels];
+    const uint4 *pc;
+    const uint4 *flagrec;
+    const uint32_t *pay;
+    const uint32_t *mv;
+    const short4 *rkv;
+    float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
+    uint8_t bg[4];
+};
+
+// ---------------------------------------------------------------- small helpers
+template <typename T>
+HMLFC_DEV T ldg(const T *p)
+{
+#if defined(__CUDA_ARCH__)
+    return __ldg(p);
+#else
+    return *p;
+#endif
+}
+
+HMLFC_DEV uint32_t funnel_r(uint32_t lo, uint32_t hi, uint32_t sh)
+{
+#if defined(__CUDA_ARCH__)
+    return __funnelshift_r(lo, hi, sh);
+#else
+    return (uint32_t)(((((uint64_t)hi) << 32) | lo) >> (sh & 31));
+#endif
+}
+
+HMLFC_DEV uint32_t popc(uint32_t x)
+{
+#if defined(__CUDA_ARCH__)
+    return (uint32_t)__popc(x);
+#else
+    return (uint32_t)__builtin_popcount(x);
+#endif
+}
+
+HMLFC_DEV uint32_t umulhi(uint32_t a, uint32_t b)
+{
+#if defined(__CUDA_ARCH__)
+    return __umulhi(a, b);
+#else
+    return (uint32_t)(((uint64_t)a * b) >> 32);
+#endif
+}
+
+// descriptor fields
+HMLFC_DEV int pc_offset(uint32_t w) { return (int)(int16_t)(w & 0xFFFFu); }
+HMLFC_DEV uint32_t pc_layout(uint32_t w) { return (w >> 16) & 3u; }
+HMLFC_DEV uint32_t pc_m(uint32_t w) { return (w >> 18) & 15u; }
+HMLFC_DEV uint32_t pc_is_pred(uint32_t w) { return (w >> 22) & 1u; }
+
+// ---------------------------------------------------------------- BISE decode_at
+// Bit string = LSB-first 32-bit words.  plain: value i at bit i*m.  trit: group g = i/5 at bit
+// g*(8+5m): 8-bit T = sum t_k 3^k then five m-bit fields.  quint: group g = i/3 at bit g*(7+3m):
+// 7-bit Q = sum q_k 5^k then three m-bit fields.  value = digit * 2^m + low.  (R15)
+HMLFC_DEV uint32_t bise_decode_at(const uint32_t *__restrict__ w, uint32_t i, uint32_t layout, uint32_t m)
+{
+    if (layout == 0u) {
+        uint32_t bit = i * m;
+        uint32_t idx = bit >> 5;
+        uint32_t v = funnel_r(ldg(w + idx), ldg(w + idx + 1), bit & 31u);
+        return v & ((1u << m) - 1u);
+    }
+    uint32_t g, k, gb, hb;
+    if (layout == 1u) { g = i / 5u; k = i - 5u * g; hb = 8u; gb = g * (8u + 5u * m); }
+    else              { g = i / 3u; k = i - 3u * g; hb = 7u; gb = g * (7u + 3u * m); }
+    uint32_t idx = gb >> 5, sh = gb & 31u;
+    // a group spans at most 8 + 5*10 = 58 bits from bit sh <= 31: three words cover it
+    uint32_t w0 = ldg(w + idx), w1 = ldg(w + idx + 1), w2 = ldg(w + idx + 2);
+    uint32_t head = funnel_r(w0, w1, sh) & ((1u << hb) - 1u);
+    uint32_t p = sh + hb + k * m;
+    uint32_t a = p < 32u ? w0 : (p < 64u ? w1 : w2);
+    uint32_t b = p < 32u ? w1 : (p < 64u ? w2 : 0u);
+    uint32_t low = funnel_r(a, b, p & 31u) & ((1u << m) - 1u);
+    uint32_t digit;
+    if (layout == 1u) {
+        // floor(T / 3^k) for T < 256 by multiply-shift, then mod 3
+        uint32_t mul = k == 0u ? 65536u : k == 1u ? 21846u : k == 2u ? 7282u : k == 3u ? 2428u : 810u;
+        uint32_t x = (head * mul) >> 16;
+        digit = x - 3u * ((x * 171u) >> 9);
+    } else {
+        uint32_t mul = k == 0u ? 65536u : k == 1u ? 13108u : 2622u;
+        uint32_t x = (head * mul) >> 16;
+        digit = x - 5u * ((x * 205u) >> 10);
+    }
+    return (digit << m) | low;
+}
+
+// stored value of a plane-channel at pixel (x,y) given its descriptor and the block's flag record
+HMLFC_DEV int stored_value(const DevStream &S, uint4 d, uint4 fr, uint32_t bit, int kin)
+{
+    if (!(fr.x & bit)) return 0;
+    uint32_t rank = fr.y + popc(fr.x & (bit - 1u));
+    uint32_t i = (rank << (2 * S.logB)) + (uint32_t)kin;
+    return pc_offset(d.w) + (int)bise_decode_at(S.pay + d.y, i, pc_layout(d.w), pc_m(d.w));
+}
+
+// reference-plane sample at (rx,ry): 0 outside the image (R8) or in an insignificant block
+HMLFC_DEV int reference_value(const DevStream &S, uint4 d, int rx, int ry)
+{
+    if ((unsigned)rx >= (unsigned)S.Ws || (unsigned)ry >= (unsigned)S.Ht) return 0;
+    int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+    uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+    int kin = ((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1));
+    return stored_value(S, d, fr, 1u << (b & 31), kin);
+}
+
+// motion record r = mode*nd^2 + (dy+W)*nd + (dx+W)  (R16)
+HMLFC_DEV void mv_unpack(const DevStream &S, uint32_t r, int &mode, int &dx, int &dy)
+{
+    mode = r >= S.nd2;
+    uint32_t rem = r - (mode ? S.nd2 : 0u);
+    uint32_t q = umulhi(rem, S.nd_magic);  // exact floor(rem / nd) for rem < 2^16
+    dy = (int)q - S.W;
+    dx = (int)(rem - q * S.nd) - S.W;
+}
+
+// (Y, Co, Cg) of light-field sample (u,v,s=x,t=y); coordinates must be in range
+HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int acc[3])
+{
+    const int h = S.h;
+    size_t ri = ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)y) * (size_t)S.Ws + (size_t)x;
+    short4 r = ldg(S.rkv + ri);
+    acc[0] = r.x; acc[1] = r.y; acc[2] = r.z;
+    const int b = (y >> S.logB) * S.nbx + (x >> S.logB);
+    const uint32_t bit = 1u << (b & 31);
+    const uint32_t fg = (uint32_t)(b >> 5);
+    const int kin = ((y & (S.B - 1)) << S.logB) + (x & (S.B - 1));
+#pragma unroll 1
+    for (int L = 0; L < h; ++L) {
+        const int pu = u >> L, pv = v >> L;
+        const LevelDesc lv = S.lev[L];
+        const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
+        const uint32_t rbase = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
+        const bool predictive = ((pu | pv) & 1) != 0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            uint4 d = ldg(S.pc + base + c);
+            uint4 fr = ldg(S.flagrec + d.x + fg);
+            int e = stored_value(S, d, fr, bit, kin);
+            if (predictive && (fr.z & bit)) {
+                uint32_t mi = fr.w + popc(fr.z & (bit - 1u));
+                uint32_t rec = bise_decode_at(S.mv + d.z, mi, S.mv_layout, S.mv_m);
+                int mode, dx, dy;
+                mv_unpack(S, rec, mode, dx, dy);
+                int q = reference_value(S, ldg(S.pc + rbase + c), x + dx, y + dy);
+                e += mode ? -q : q;  // R10: subtractive P = e + R, additive P = e - R
+            }
+            acc[c] += e;
+        }
+    }
+}
+
+// inverse YCoCg-R (arithmetic shifts = floor) and clamp to [0,255]; returns R | G<<8 | B<<16
+HMLFC_DEV uint32_t ycocg_to_rgb8(const int acc[3])
+{
+    int t = acc[0] - (acc[2] >> 1);
+    int G = acc[2] + t;
+    int Bl = t - (acc[1] >> 1);
+    int R = Bl + acc[1];
+    R = min(max(R, 0), 255);
+    G = min(max(G, 0), 255);
+    Bl = min(max(Bl, 0), 255);
+    return (uint32_t)R | ((uint32_t)G << 8) | ((uint32_t)Bl << 16);
+}
+
+HMLFC_DEV uint32_t decode_rgb8(const DevStream &S, int u, int v, int x, int y)
+{
+    int acc[3];
+    decode_ycocg(S, u, v, x, y, acc);
+    return ycocg_to_rgb8(acc);
+}
+
+// ---------------------------------------------------------------- ray set-up
+// Strict IEEE fp32, fixed operation order, no FMA contraction: __fmul_rn/__fadd_rn/__fdiv_rn are
+// never fused by the compiler, so hit/miss and floor() agree bit for bit with the oracle.
+struct Camera {
+    float eye[3], right[3], down[3], fwd[3];
+    float tan_half_x, tan_half_y;
+    float _pad[2];
+};
+
+struct Ray {
+    float u, v, s, t;
+    bool hit;
+};
+
+#if defined(__CUDA_ARCH__)
+#define HMLFC_MUL(a, b) __fmul_rn((a), (b))
+#define HMLFC_ADD(a, b) __fadd_rn((a), (b))
+#define HMLFC_SUB(a, b) __fsub_rn((a), (b))
+#define HMLFC_DIV(a, b) __fdiv_rn((a), (b))
+#else
+#define HMLFC_MUL(a, b) ((a) * (b))
+#define HMLFC_ADD(a, b) ((a) + (b))
+#define HMLFC_SUB(a, b) ((a) - (b))
+#define HMLFC_DIV(a, b) ((a) / (b))
+#endif
+
+HMLFC_DEV Ray ray_setup(const DevStream &S, const Camera &cam, int W, int H, int i, int j)
+{
+    Ray r;
+    r.hit = false;
+    r.u = r.v = r.s = r.t = 0.0f;
+    float fi = HMLFC_ADD((float)i, 0.5f), fj = HMLFC_ADD((float)j, 0.5f);
+    float px = HMLFC_MUL(HMLFC_SUB(HMLFC_DIV(HMLFC_MUL(2.0f, fi), (float)W), 1.0f), cam.tan_half_x);
+    float py = HMLFC_MUL(HMLFC_SUB(HMLFC_DIV(HMLFC_MUL(2.0f, fj), (float)H), 1.0f), cam.tan_half_y);
+    float Dx = HMLFC_ADD(HMLFC_ADD(cam.fwd[0], HMLFC_MUL(px, cam.right[0])), HMLFC_MUL(py, cam.down[0]));
+    float Dy = HMLFC_ADD(HMLFC_ADD(cam.fwd[1], HMLFC_MUL(px, cam.right[1])), HMLFC_MUL(py, cam.down[1]));
+    float Dz = HMLFC_ADD(HMLFC_ADD(cam.fwd[2], HMLFC_MUL(px, cam.right[2])), HMLFC_MUL(py, cam.down[2]));
+    if (!(Dz > 0.0f)) return r;
+    float l0 = HMLFC_DIV(HMLFC_SUB(0.0f, cam.eye[2]), Dz);
+    float l1 = HMLFC_DIV(HMLFC_SUB(S.z_st, cam.eye[2]), Dz);
+    float uw = HMLFC_ADD(cam.eye[0], HMLFC_MUL(l0, Dx));
+    float vw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l0, Dy));
+    float sw = HMLFC_ADD(cam.eye[0], HMLFC_MUL(l1, Dx));
+    float tw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l1, Dy));
+    float u = HMLFC_DIV(HMLFC_SUB(uw, S.uv_origin[0]), S.uv_step[0]);
+    float v = HMLFC_DIV(HMLFC_SUB(vw, S.uv_origin[1]), S.uv_step[1]);
+    float s = HMLFC_DIV(HMLFC_SUB(sw, S.st_origin[0]), S.st_step[0]);
+    float t = HMLFC_DIV(HMLFC_SUB(tw, S.st_origin[1]), S.st_step[1]);
+    if (!(u >= 0.0f && u <= (float)(S.U - 1) && v >= 0.0f && v <= (float)(S.V - 1) && s >= 0.0f &&
+          s <= (float)(S.Ws - 1) && t >= 0.0f && t <= (float)(S.Ht - 1)))
+        return r;
+    r.hit = true;
+    r.u = u; r.v = v; r.s = s; r.t = t;
+    return r;
+}
+
+// 16-tap enumeration: base indices, +1 neighbours clamped to the edge, fractional weights
+struct Taps {
+    int u0, u1, v0, v1, s0, s1, t0, t1;
+    float fu, fv, fs, ft;
+};
+
+HMLFC_DEV Taps tap_setup(const DevStream &S, const Ray &r)
+{
+    Taps k;
+    float u0 = floorf(r.u), v0 = floorf(r.v), s0 = floorf(r.s), t0 = floorf(r.t);
+    k.fu = HMLFC_SUB(r.u, u0); k.fv = HMLFC_SUB(r.v, v0); k.fs = HMLFC_SUB(r.s, s0); k.ft = HMLFC_SUB(r.t, t0);
+    k.u0 = (int)u0; k.v0 = (int)v0; k.s0 = (int)s0; k.t0 = (int)t0;
+    k.u1 = min(k.u0 + 1, S.U - 1);
+    k.v1 = min(k.v0 + 1, S.V - 1);
+    k.s1 = min(k.s0 + 1, S.Ws - 1);
+    k.t1 = min(k.t0 + 1, S.Ht - 1);
+    return k;
+}
+
+}  // namespace hmlfc

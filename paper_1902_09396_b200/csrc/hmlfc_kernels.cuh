@@ -1,0 +1,32 @@
+// Launchers of the HMLFC kernels (definitions in hmlfc_kernels.cu / hmlfc_render_tiled.cu).
+#pragma once
+
+#include "hmlfc_device.cuh"
+
+namespace hmlfc {
+
+// marks written by the footprint kernels
+struct FootprintMarks {
+    uint32_t *blk;  // [n_pc * nblk] bits
+    uint32_t *rkv;  // [UH * VH * Ht * Ws] bits
+};
+
+struct FootprintTotals {
+    unsigned long long blocks, flag_bits, payload_bits15, mv_bits15, rkv_samples;
+};
+
+cudaError_t launch_decode(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
+                          unsigned long long *d_oob, cudaStream_t st, int *n_launches);
+cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
+                                cudaStream_t st, int *n_launches);
+cudaError_t launch_render_tiled(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
+                                cudaStream_t st, int *n_launches);
+cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,
+                                    FootprintMarks marks, cudaStream_t st);
+cudaError_t launch_footprint_decode(const DevStream &S, const int32_t *d_coords, int64_t n, FootprintMarks marks,
+                                    cudaStream_t st);
+// bits15[k] = BISE bits per value of plane-channel k in units of 1/15 bit
+cudaError_t launch_footprint_reduce(const DevStream &S, uint64_t n_pc, const uint32_t *d_bits15, uint32_t mv_bits15,
+                                    FootprintMarks marks, FootprintTotals *d_totals, cudaStream_t st);
+
+}  // namespace hmlfc

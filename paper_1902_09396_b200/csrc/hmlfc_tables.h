@@ -1,0 +1,190 @@
+// Host-side parsing of a serialized HMLFC stream into the device structure-of-arrays tables.
+// Written from DESIGN.md "Stream format v1"; shares no code with the oracle's parser.
+#pragma once
+
+#include "../../include/hmlfc.h"
+#include "hmlfc_device.cuh"
+
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace hmlfc {
+
+struct HostTables {
+    DevStream ds{};  // device pointers left null; hmlfc_load fills them after the upload
+    hmlfc_info_t info{};
+    std::vector<uint4> pc, flagrec;
+    std::vector<uint32_t> bits15;  // per plane-channel BISE bits/value in 1/15 bit (footprint only)
+    std::vector<short4> rkv;
+    uint64_t n_pc = 0, off_pay = 0, off_mv = 0, total = 0;
+    uint32_t mv_bits15 = 0;
+};
+
+namespace tables_detail {
+
+inline uint32_t rd16(const uint8_t *p) { return (uint32_t)p[0] | ((uint32_t)p[1] << 8); }
+inline uint32_t rd32(const uint8_t *p) { return rd16(p) | (rd16(p + 2) << 16); }
+inline uint64_t rd64(const uint8_t *p) { return (uint64_t)rd32(p) | ((uint64_t)rd32(p + 4) << 32); }
+inline float rdf(const uint8_t *p) { uint32_t u = rd32(p); float f; memcpy(&f, &u, 4); return f; }
+
+constexpr size_t kHeaderBytes = 160, kDirentBytes = 48;
+
+// BISE layout rule (R15): cheapest bits/value of plain / trit / quint; ties in that order.
+inline void bise_layout(uint32_t N, uint32_t *layout, uint32_t *m)
+{
+    if (N <= 1) { *layout = 0; *m = 0; return; }
+    uint32_t b = 0, mt = 0, mq = 0;
+    while ((1ull << b) < N) ++b;
+    while ((3ull << mt) < N) ++mt;
+    while ((5ull << mq) < N) ++mq;
+    uint32_t cp = 15 * b, ct = 24 + 15 * mt, cq = 35 + 15 * mq;
+    *layout = 0; *m = b;
+    uint32_t best = cp;
+    if (ct < best) { best = ct; *layout = 1; *m = mt; }
+    if (cq < best) { *layout = 2; *m = mq; }
+}
+
+inline uint32_t bise_bits15(uint32_t layout, uint32_t m) { return layout == 0 ? 15 * m : layout == 1 ? 24 + 15 * m : 35 + 15 * m; }
+
+inline uint64_t bise_nbits(uint32_t layout, uint32_t m, uint64_t count)
+{
+    if (layout == 0) return count * m;
+    if (layout == 1) return ((count + 4) / 5) * (8 + 5 * m);
+    return ((count + 2) / 3) * (7 + 3 * m);
+}
+
+inline uint32_t popcount32(uint32_t x)
+{
+    x = x - ((x >> 1) & 0x55555555u);
+    x = (x & 0x33333333u) + ((x >> 2) & 0x33333333u);
+    return (((x + (x >> 4)) & 0x0F0F0F0Fu) * 0x01010101u) >> 24;
+}
+
+}  // namespace tables_detail
+
+// Validates the stream and fills T.  Returns HMLFC_OK or a negative HMLFC_E_* code.
+inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
+{
+    using namespace tables_detail;
+    const uint8_t *s = static_cast<const uint8_t *>(h_stream_bytes);
+    if (len < 8) return HMLFC_E_TRUNCATED;
+    if (memcmp(s, "HMLF", 4) != 0) return HMLFC_E_MAGIC;
+    if (rd16(s + 4) != 1) return HMLFC_E_VERSION;
+    if (len < kHeaderBytes) return HMLFC_E_TRUNCATED;
+
+    hmlfc_info_t &I = T.info;
+    I.U = (int32_t)rd32(s + 8); I.V = (int32_t)rd32(s + 12); I.Ws = (int32_t)rd32(s + 16); I.Ht = (int32_t)rd32(s + 20);
+    I.height = (int32_t)rd32(s + 24); I.block = (int32_t)rd32(s + 28); I.window = (int32_t)rd32(s + 32);
+    const uint32_t n_channels = rd32(s + 36);
+    I.tau_ref = (int32_t)rd32(s + 40); I.tau_res = (int32_t)rd32(s + 44);
+    const uint8_t colour_id = s[48], chroma = s[49], rkv_codec = s[50];
+    I.background[0] = s[52]; I.background[1] = s[53]; I.background[2] = s[54];
+    I.uv_origin[0] = rdf(s + 56); I.uv_origin[1] = rdf(s + 60); I.uv_step[0] = rdf(s + 64); I.uv_step[1] = rdf(s + 68);
+    I.st_origin[0] = rdf(s + 72); I.st_origin[1] = rdf(s + 76); I.st_step[0] = rdf(s + 80); I.st_step[1] = rdf(s + 84);
+    I.z_st = rdf(s + 88);
+    const uint64_t n_pc_hdr = rd64(s + 104);
+    const uint64_t off_rkv = rd64(s + 112), off_dir = rd64(s + 120), off_flags = rd64(s + 128);
+    const uint64_t off_pay = rd64(s + 136), off_mv = rd64(s + 144), total = rd64(s + 152);
+
+    if (rd16(s + 6) != kHeaderBytes) return HMLFC_E_CORRUPT;
+    if (I.U < 1 || I.V < 1 || I.Ws < 1 || I.Ht < 1 || I.height < 1 || I.window < 0) return HMLFC_E_CORRUPT;
+    if (n_channels != 3 || colour_id != 1 || chroma != 0 || rkv_codec != 0) return HMLFC_E_UNSUPPORTED;
+    if (I.height > kMaxLevels || I.window > 64) return HMLFC_E_UNSUPPORTED;
+    if (!(I.block == 2 || I.block == 4 || I.block == 8) || (I.Ws % I.block) || (I.Ht % I.block)) return HMLFC_E_UNSUPPORTED;
+    if ((uint64_t)I.U * I.V > (1u << 24) || (uint64_t)I.Ws * I.Ht > (1u << 26)) return HMLFC_E_UNSUPPORTED;
+    if (len < total) return HMLFC_E_TRUNCATED;
+
+    DevStream &D = T.ds;
+    D.U = I.U; D.V = I.V; D.Ws = I.Ws; D.Ht = I.Ht; D.h = I.height; D.B = I.block; D.W = I.window;
+    D.logB = I.block == 2 ? 1 : I.block == 4 ? 2 : 3;
+    D.nbx = I.Ws / I.block; D.nby = I.Ht / I.block; D.nblk = D.nbx * D.nby; D.fgroups = (D.nblk + 31) / 32;
+    D.nd = 2u * I.window + 1u; D.nd2 = D.nd * D.nd;
+    D.nd_magic = D.nd == 1 ? 0xFFFFFFFFu : (uint32_t)((0x100000000ull + D.nd - 1) / D.nd);
+    bise_layout(2u * D.nd2, &D.mv_layout, &D.mv_m);
+    T.mv_bits15 = bise_bits15(D.mv_layout, D.mv_m);
+    for (int i = 0; i < 2; ++i) {
+        D.uv_origin[i] = I.uv_origin[i]; D.uv_step[i] = I.uv_step[i];
+        D.st_origin[i] = I.st_origin[i]; D.st_step[i] = I.st_step[i];
+    }
+    D.z_st = I.z_st;
+    D.bg[0] = I.background[0]; D.bg[1] = I.background[1]; D.bg[2] = I.background[2]; D.bg[3] = 0;
+
+    // level table: the stream lists levels top-down (L = h-1 .. 0), planes row-major, channel innermost
+    uint64_t n_pc = 0;
+    for (int L = I.height - 1; L >= 0; --L) {
+        D.lev[L].UL = (I.U + (1 << L) - 1) >> L;
+        D.lev[L].VL = (I.V + (1 << L) - 1) >> L;
+        D.lev[L].pc_base = (uint32_t)n_pc;
+        n_pc += (uint64_t)D.lev[L].UL * D.lev[L].VL * 3;
+    }
+    D.UH = (I.U + (1 << I.height) - 1) >> I.height;
+    D.VH = (I.V + (1 << I.height) - 1) >> I.height;
+    const uint64_t npx = (uint64_t)I.Ws * I.Ht, n_top = (uint64_t)D.UH * D.VH;
+    if (n_pc != n_pc_hdr || n_pc * (uint64_t)D.fgroups > 0xFFFFFFFFull) return HMLFC_E_CORRUPT;
+    if (off_rkv != kHeaderBytes || off_dir < off_rkv + n_top * npx * 5 || off_flags < off_dir + n_pc * kDirentBytes ||
+        off_pay < off_flags || off_mv < off_pay || total < off_mv)
+        return HMLFC_E_CORRUPT;
+    const uint64_t flags_len = off_pay - off_flags, pay_bits = (off_mv - off_pay) * 8, mv_bits = (total - off_mv) * 8;
+    if (pay_bits / 32 > 0xFFFFFFF0ull || mv_bits / 32 > 0xFFFFFFF0ull) return HMLFC_E_UNSUPPORTED;
+    T.n_pc = n_pc; T.off_pay = off_pay; T.off_mv = off_mv; T.total = total;
+    I.n_plane_channels = n_pc;
+    I.stream_bytes = total;
+
+    try {
+        T.pc.resize(n_pc);
+        T.bits15.resize(n_pc);
+        T.flagrec.resize(n_pc * (uint64_t)D.fgroups);
+        T.rkv.resize(n_top * npx);
+    } catch (const std::bad_alloc &) {
+        return HMLFC_E_NOMEM;
+    }
+
+    // descriptors + flag/rank records
+    const uint64_t fbytes = (uint64_t)D.fgroups * 4;
+    const uint32_t BB = (uint32_t)(I.block * I.block);
+    uint64_t k = 0;
+    for (int L = I.height - 1; L >= 0; --L)
+        for (int pv = 0; pv < D.lev[L].VL; ++pv)
+            for (int pu = 0; pu < D.lev[L].UL; ++pu)
+                for (int c = 0; c < 3; ++c, ++k) {
+                    const uint8_t *e = s + off_dir + k * kDirentBytes;
+                    const int32_t offset = (int32_t)rd32(e);
+                    const uint32_t N = rd32(e + 4), n_res = rd32(e + 8), n_pred = rd32(e + 12);
+                    const uint64_t foff = rd64(e + 16), pboff = rd64(e + 24), mboff = rd64(e + 32);
+                    const bool is_pred = ((pu | pv) & 1) != 0;
+                    uint32_t layout, m;
+                    bise_layout(N, &layout, &m);
+                    if (N < 1 || N > 4096 || offset < -32768 || offset > 32767 || e[40] != layout || e[41] != m ||
+                        e[42] != (is_pred ? 1 : 0) || (pboff & 31) || (mboff & 31) || (foff & 3) ||
+                        foff + fbytes * (is_pred ? 2 : 1) > flags_len ||
+                        pboff + bise_nbits(layout, m, (uint64_t)n_res * BB) > pay_bits ||
+                        mboff + bise_nbits(D.mv_layout, D.mv_m, n_pred) > mv_bits || (!is_pred && n_pred != 0))
+                        return HMLFC_E_CORRUPT;
+                    T.pc[k] = make_uint4((uint32_t)(k * (uint64_t)D.fgroups), (uint32_t)(pboff / 32), (uint32_t)(mboff / 32),
+                                         ((uint32_t)offset & 0xFFFFu) | (layout << 16) | (m << 18) | ((is_pred ? 1u : 0u) << 22));
+                    T.bits15[k] = bise_bits15(layout, m);
+                    const uint8_t *fres = s + off_flags + foff;
+                    const uint8_t *fprd = fres + fbytes;
+                    uint32_t rr = 0, rp = 0;
+                    for (int g = 0; g < D.fgroups; ++g) {
+                        uint32_t wr = rd32(fres + 4 * g), wp = is_pred ? rd32(fprd + 4 * g) : 0u;
+                        if (g == D.fgroups - 1 && (D.nblk & 31)) {  // ignore padding bits
+                            const uint32_t mask = (1u << (D.nblk & 31)) - 1u;
+                            wr &= mask; wp &= mask;
+                        }
+                        T.flagrec[k * (uint64_t)D.fgroups + g] = make_uint4(wr, rr, wp, rp);
+                        rr += popcount32(wr);
+                        rp += popcount32(wp);
+                    }
+                    if (rr != n_res || rp != n_pred) return HMLFC_E_CORRUPT;
+                }
+
+    // top-level RKVs: Y uint8 planes, then Co and Cg int16 LE planes -> short4 {Y, Co, Cg, 0} per sample
+    const uint8_t *py = s + off_rkv, *pco = py + n_top * npx, *pcg = pco + n_top * npx * 2;
+    for (uint64_t i = 0; i < n_top * npx; ++i)
+        T.rkv[i] = make_short4((short)py[i], (short)(int16_t)rd16(pco + 2 * i), (short)(int16_t)rd16(pcg + 2 * i), 0);
+    return HMLFC_OK;
+}
+
+}  // namespace hmlfc

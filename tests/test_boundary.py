@@ -1,0 +1,88 @@
+"""CPU checks of the C-ABI boundary: the library loads, exports every symbol include/hmlfc.h declares,
+rejects malformed streams before touching CUDA, and refuses to compute without a GPU."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_1902_09396_b200 as pkg
+    from paper_1902_09396_b200 import build
+
+    build.build()  # nvcc cross-compiles for sm_100a without a GPU
+    return pkg
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "hmlfc.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(hmlfc_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(P):
+    L = P.lib()
+    declared = _declared_symbols()
+    assert len(declared) >= 14
+    for name in declared:
+        assert hasattr(L, name), f"{name} declared in include/hmlfc.h but not exported"
+    assert sorted(P.EXPORTS) == declared
+
+
+def test_library_is_built_for_sm_100a(P):
+    import subprocess
+
+    out = subprocess.run(["cuobjdump", "-lelf", P.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
+    cfg, lf, data, info, s = enc("cfg1_lossy")
+    L = P.lib()
+
+    def load(blob):
+        buf = np.frombuffer(bytes(blob), dtype=np.uint8)
+        out = C.c_void_p()
+        return L.hmlfc_load(buf.ctypes.data_as(C.c_void_p), buf.size, C.byref(out)), out
+
+    bad_magic = bytearray(data)
+    bad_magic[1] ^= 0x40
+    bad_version = bytearray(data)
+    bad_version[4] = 9
+    chroma = bytearray(data)
+    chroma[49] = 1
+    bad_block = bytearray(data)
+    bad_block[28] = 3
+    bad_dir = bytearray(data)
+    off_dir = int.from_bytes(data[120:128], "little")
+    bad_dir[off_dir + 8] ^= 0x01  # n_res of the first plane-channel no longer matches its flag map
+    cases = [(bad_magic, -1), (data[:6], -2), (data[:100], -2), (data[:len(data) // 2], -2), (bad_version, -3),
+             (chroma, -5), (bad_block, -5), (bad_dir, -6)]
+    for blob, code in cases:
+        rc, out = load(blob)
+        assert rc == code and not out.value, (rc, code)
+    assert L.hmlfc_load(None, 0, None) == -4
+    assert b"magic" in L.hmlfc_strerror(-1) and b"truncated" in L.hmlfc_strerror(-2)
+
+
+def test_entry_points_validate_arguments(P):
+    L = P.lib()
+    assert L.hmlfc_decode(None, None, 0, None, None) == -4
+    assert L.hmlfc_render(None, None, 0, 1, 1, None, None) == -4
+    assert L.hmlfc_info(None, None) == -4
+    L.hmlfc_free(None)  # no-op
+
+
+def test_no_cpu_fallback(P, enc):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    cfg, lf, data, info, s = enc("cfg1_lossy")
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_load(data)

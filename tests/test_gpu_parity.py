@@ -1,0 +1,199 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element.
+
+Decoded pixels must be bit-exact; rendered views within max|delta| <= 1 on the 8-bit scale
+(BASELINE.json north_star).  Streams and expected values come from the oracle only.
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+TOL_VIEW = 1  # max |delta| on the 8-bit scale, north_star
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_1902_09396_b200 as pkg
+
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    return pkg
+
+
+_handles = {}
+
+
+def _loaded(P, enc, name):
+    if name not in _handles:
+        cfg, lf, data, info, s = enc(name)
+        _handles[name] = P.hmlfc_load(data)
+    return _handles[name]
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ---------------------------------------------------------------- decode: bit-exact
+def test_decode_cfg1_every_pixel_lossless(P, enc):
+    cfg, lf, data, info, s = enc("cfg1")
+    h = _loaded(P, enc, "cfg1")
+    coords = wl.all_coords(cfg)
+    out = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
+    assert np.array_equal(out, s.decode(coords))
+    assert np.array_equal(out.reshape(lf.shape), lf)  # zero-threshold round trip reproduces the input
+
+
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4"])
+def test_decode_every_pixel_matches_oracle(P, enc, name):
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    coords = wl.all_coords(cfg)
+    out = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
+    assert np.array_equal(out.reshape(lf.shape), info["p1"])      # = the encoder's own reconstruction
+    rc = wl.random_coords(cfg, 100_003)                           # ragged: not a multiple of the block size
+    assert np.array_equal(P.hmlfc_decode(h, _dev(rc)).cpu().numpy(), s.decode(rc))
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 255, 257, 1000])
+def test_decode_ragged_sizes_and_unaligned_output(P, enc, n):
+    cfg, lf, data, info, s = enc("mini3")
+    h = _loaded(P, enc, "mini3")
+    rc = wl.random_coords(cfg, max(n, 1), seed_offset=n)[:n]
+    expect = s.decode(rc) if n else np.zeros((0, 3), np.uint8)
+    assert np.array_equal(P.hmlfc_decode(h, _dev(rc).reshape(-1, 4)).cpu().numpy(), expect)
+    if n:
+        buf = torch.full((3 * n + 8,), 0xAB, dtype=torch.uint8, device="cuda")
+        out = buf[1:1 + 3 * n]                                     # 1-byte offset: byte-store path
+        P.hmlfc_decode(h, _dev(rc), out=out)
+        assert np.array_equal(out.cpu().numpy().reshape(n, 3), expect)
+        assert buf[0].item() == 0xAB and buf[1 + 3 * n].item() == 0xAB
+
+
+def test_decode_out_of_range_is_black_and_counted(P, enc):
+    cfg, lf, data, info, s = enc("cfg1_lossy")
+    h = P.hmlfc_load(data)
+    coords = np.array([[0, 0, 0, 0], [8, 0, 0, 0], [0, -1, 0, 0], [0, 0, 64, 0], [0, 0, 0, 64], [7, 7, 63, 63]], dtype=np.int32)
+    out = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
+    exp, oob = s.decode(coords, return_oob=True)
+    assert np.array_equal(out, exp) and P.hmlfc_last_oob_count(h) == oob == 4
+    P.hmlfc_free(h)
+
+
+def test_decode_host_entry_point(P, enc):
+    cfg, lf, data, info, s = enc("mini4")
+    h = _loaded(P, enc, "mini4")
+    rc = wl.random_coords(cfg, 20_001)
+    assert np.array_equal(P.hmlfc_decode_host(h, rc), s.decode(rc))
+
+
+# ---------------------------------------------------------------- render: <= 1 LSB
+def _check_views(P, h, s, cams, W, H):
+    expect = s.render(cams, W, H)
+    outs = {}
+    for variant in (P.RENDER_PIXEL, P.RENDER_TILED):
+        P.hmlfc_set_render_variant(h, variant)
+        got = P.hmlfc_render(h, _dev(cams), W, H).cpu().numpy()
+        d = np.abs(got.astype(np.int16) - expect.astype(np.int16))
+        assert d.max() <= TOL_VIEW, (variant, int(d.max()), int((d > TOL_VIEW).sum()))
+        assert (d > 0).mean() < 1e-3  # rounding-boundary cases only
+        outs[variant] = got
+    P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_TILED])  # the two kernels agree byte for byte
+    return expect
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4"])
+def test_render_matches_oracle(P, enc, name):
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    _check_views(P, h, s, wl.camera_path(cfg), cfg.out_w, cfg.out_h)
+
+
+@pytest.mark.parametrize("W,H", [(61, 37), (32, 8), (33, 9), (1, 1), (130, 5)])
+def test_render_ragged_output_sizes(P, enc, W, H):
+    cfg, lf, data, info, s = enc("mini2")
+    h = _loaded(P, enc, "mini2")
+    _check_views(P, h, s, wl.camera_path(cfg, n_views=2, out_w=W, out_h=H), W, H)
+
+
+def test_render_grid_camera_reproduces_decoded_view(P, enc):
+    cfg, lf, data, info, s = enc("cfg1_lossy")
+    h = _loaded(P, enc, "cfg1_lossy")
+    cams = np.stack([wl.grid_camera(cfg, 3, 5), wl.grid_camera(cfg, 0, 7)])
+    got = P.hmlfc_render(h, _dev(cams), cfg.Ws, cfg.Ht).cpu().numpy()
+    assert np.array_equal(got[0], info["p1"][5, 3]) and np.array_equal(got[1], info["p1"][7, 0])
+
+
+def test_render_minification_takes_the_fallback_path_and_misses_get_background(P, enc):
+    # a wide frustum on a tiny output: footprints of a tile span the whole light field (box > patch),
+    # and the border rays miss the slab
+    cfg, lf, data, info, s = enc("mini2")
+    h = _loaded(P, enc, "mini2")
+    cam = wl.camera_path(cfg, n_views=1, out_w=40, out_h=24)
+    cam[:, 12:14] *= 2.2
+    expect = _check_views(P, h, s, cam, 40, 24)
+    assert (expect.reshape(-1, 3) == 0).all(1).any() and expect.any()
+
+
+def test_render_host_entry_point(P, enc):
+    cfg, lf, data, info, s = enc("mini3")
+    h = _loaded(P, enc, "mini3")
+    cams = wl.camera_path(cfg)
+    got = P.hmlfc_render_host(h, cams, cfg.out_w, cfg.out_h)
+    assert np.abs(got.astype(int) - s.render(cams, cfg.out_w, cfg.out_h).astype(int)).max() <= TOL_VIEW
+
+
+# ---------------------------------------------------------------- accounting
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini4"])
+def test_footprint_equals_oracle_stats(P, enc, name):
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    cams = wl.camera_path(cfg)
+    fp = P.hmlfc_footprint_render(h, _dev(cams), cfg.out_w, cfg.out_h)
+    st = s.stats_render(cams, cfg.out_w, cfg.out_h)
+    for k in ("blocks_touched", "flag_bits", "payload_bits15", "mv_bits15", "rkv_bytes", "out_bytes", "in_bytes"):
+        assert fp[k] == st[k], k
+    assert abs(fp["bytes_alg"] - st["bytes_alg"]) < 1e-6 * st["bytes_alg"]
+    rc = wl.random_coords(cfg, 5000)
+    fpd, std = P.hmlfc_footprint_decode(h, _dev(rc)), s.stats_decode(rc)
+    for k in ("blocks_touched", "flag_bits", "payload_bits15", "mv_bits15", "rkv_bytes"):
+        assert fpd[k] == std[k], k
+
+
+def test_info_and_launch_count(P, enc):
+    cfg, lf, data, info, s = enc("mini2")
+    h = P.hmlfc_load(data)
+    i = h.info
+    assert (i.U, i.V, i.Ws, i.Ht, i.height, i.block, i.window) == (cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, 4, 16)
+    assert i.stream_bytes == len(data) and 0 < i.device_bytes < 3 * len(data)
+    n0 = P.hmlfc_launch_count(h)
+    P.hmlfc_decode(h, _dev(wl.random_coords(cfg, 10)))
+    P.hmlfc_render(h, _dev(wl.camera_path(cfg)), 32, 8)
+    torch.cuda.synchronize()
+    assert P.hmlfc_launch_count(h) - n0 == 2
+    P.hmlfc_free(h)
+
+
+# ---------------------------------------------------------------- full size, bench configuration (cfg2)
+def test_cfg2_full_size_sampled_parity(P, enc):
+    """BASELINE.json configs[1] at full size, in the launch configuration bench.py times: 64 views of
+    512x512 in one launch; four whole views and 2*10^6 random coordinates compared with the oracle."""
+    import oracle as orc
+    from oracle import streams
+
+    cfg, data, info = streams.get_stream("cfg2")
+    s = orc.Stream(data)
+    h = P.hmlfc_load(data)
+    cams = wl.camera_path(cfg)
+    got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
+    for k in (0, 21, 42, 63):
+        d = np.abs(got[k].astype(np.int16) - s.render(cams[k:k + 1], cfg.out_w, cfg.out_h)[0].astype(np.int16))
+        assert d.max() <= TOL_VIEW
+    rc = wl.random_coords(cfg, 2_000_000)
+    assert np.array_equal(P.hmlfc_decode(h, _dev(rc)).cpu().numpy(), s.decode(rc))
+    assert 38.0 < info["psnr"] < 42.0  # "quantisation set for ~40 dB"
+    P.hmlfc_free(h)
