@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py -- HMLFC decode + fused render hot path on B200 (contract: see DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: hmlfc_render of the
+configuration's view batch (ray set-up, tap enumeration, tree-walk decode with motion
+re-compensation, inverse colour, quadrilinear blend, RGB8 store -- SURVEY.md 8(a) S1-S9) in ONE kernel
+launch.  The second half of BASELINE.json's metric, decoded LF pixels/s (hmlfc_decode on seeded uniformly
+random coordinates), is timed in the same run and reported under "decode".
+
+Inputs: the seeded synthetic light field of the configuration (workloads/), encoded ONCE, before any timed
+region, by the oracle's encoder (oracle/streams.py; the encoder is outside the hot path this repo builds).
+The timed product path calls only the C-ABI library; the oracle is executed again only for the
+"cpu_baseline" object and for `--impl reference`.
+
+N > 1 (torchrun): the path shards with no exchange step -- every rank holds the stream and renders its own
+batch of views (weak scaling); value = views of all ranks / max-over-ranks device time.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_FLUSH_BYTES = 512 << 20  # > 126 MB L2
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and clock-event reasons of one GPU while the timed region runs."""
+
+    REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4),
+               ("hw_power_brake", 0x80), ("applications_clocks", 0x2))
+
+    def __init__(self, index, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev)
+                for name, bit in self.REASONS:
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def _physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def _get_stream(name, rank, world, barrier):
+    """Rank 0 encodes (oracle encoder, input preparation) into the on-disk cache; the others read it."""
+    from oracle import streams
+
+    if world == 1 or rank == 0:
+        out = streams.get_stream(name)
+        barrier()
+        return out
+    barrier()
+    return streams.get_stream(name)
+
+
+def _oracle_views_sample(stream, cams, W, H, budget_s, max_views):
+    """Render views one by one with the oracle (all host cores) until budget_s is used."""
+    t0 = time.perf_counter()
+    n = 0
+    while n < max_views:
+        stream.render(cams[n % len(cams)][None], W, H)
+        n += 1
+        if time.perf_counter() - t0 >= budget_s:
+            break
+    return n, time.perf_counter() - t0
+
+
+def run_reference(args, cfg_name):
+    """--impl reference: the oracle as it stands, on the host cores; each step = a bounded sample of the batch."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as orc
+    import workloads as wl
+    from oracle import streams
+
+    cfg, data, info = streams.get_stream(cfg_name)
+    s = orc.Stream(data)
+    cams = wl.camera_path(cfg)
+    cores = os.cpu_count() or 1
+    W, H = cfg.out_w, cfg.out_h
+    # size the per-step sample from one view so the whole run ends within a few minutes
+    t0 = time.perf_counter()
+    s.render(cams[:1], W, H)
+    t_view = time.perf_counter() - t0
+    per_step = int(max(1, min(cfg.n_views, round(6.0 / max(t_view, 1e-3)))))
+    for k in range(args.warmup):
+        s.render(cams[k % len(cams)][None], W, H)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        idx = [(k * per_step + i) % len(cams) for i in range(per_step)]
+        s.render(cams[idx], W, H)
+    dt = time.perf_counter() - t0
+    value = args.steps * per_step / dt
+    sample = f"{per_step} of the batch's {cfg.n_views} views ({W}x{H}) per step, OpenMP over {cores} threads"
+    line = {
+        "impl": "reference", "metric": "rendered_views_per_s", "value": value, "unit": "views/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": _config_dict(cfg, info, "n/a (CPU)"),
+        "cpu_baseline": {"value": value, "unit": "views/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "views/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def _config_dict(cfg, info, l2_policy):
+    return {
+        "workload": f"{cfg.name}: {cfg.U}x{cfg.V} views x {cfg.Ws}x{cfg.Ht} RGB8, h={cfg.height}, B={cfg.block}, W={cfg.window}; "
+                    f"render {cfg.n_views} views of {cfg.out_w}x{cfg.out_h} per step on the seeded circular camera path",
+        "stream_bytes": info["stream_bytes"], "stream_bpp": round(info["bpp"], 4), "psnr_db": round(info["psnr"], 3),
+        "tau_res": info["tau_res"], "views_per_step": cfg.n_views, "out_w": cfg.out_w, "out_h": cfg.out_h,
+        "l2": l2_policy,
+    }
+
+
+def run_ours(args, cfg_name):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1902_09396_b200 as P
+    import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the HMLFC hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    cfg, data, info = _get_stream(cfg_name, rank, world, barrier)
+    h = P.hmlfc_load(data)
+    W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
+    # weak scaling: every rank renders a full batch, each on its own arc of the camera circle
+    cams_np = wl.camera_path(cfg, seed_offset=rank)
+    cams = torch.from_numpy(cams_np).cuda()
+    out = torch.empty((V, H, W, 3), dtype=torch.uint8, device="cuda")
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        P.hmlfc_render(h, cams, W, H, out=out, stream=stream)
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            flush.fill_(1)
+            fn()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        torch.cuda.synchronize()
+        for a, b in ev:
+            flush.fill_(1)          # evict the stream and the previous output from L2 (outside the events)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    # ---- the timed region: K steps of the fused render kernel, inputs resident in HBM
+    n0 = P.hmlfc_launch_count(h)
+    with ClockSampler(_physical_gpu_index(local_rank)) as clk:
+        ms = timed(step, args.steps, args.warmup)
+    launches = P.hmlfc_launch_count(h) - n0 - args.warmup
+    total_ms = float(sum(ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    views_per_s = world * V * args.steps / (total_ms * 1e-3)
+
+    # ---- decode leg: seeded uniformly random LF coordinates (inputs larger than L2)
+    n_dec = cfg.n_decode
+    coords = torch.from_numpy(wl.random_coords(cfg, n_dec, seed_offset=rank)).cuda()
+    dec_out = torch.empty((n_dec, 3), dtype=torch.uint8, device="cuda")
+    dec_ms = timed(lambda: P.hmlfc_decode(h, coords, out=dec_out, stream=stream), max(3, min(args.steps, 10)), 3)
+    dec_total = float(sum(dec_ms))
+    if world > 1:
+        t = torch.tensor([dec_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dec_total = float(t.item())
+    dec_px_per_s = world * n_dec * len(dec_ms) / (dec_total * 1e-3)
+
+    # ---- end to end through the C ABI with HOST (pinned) buffers: cameras H2D + views D2H inside the timed region
+    cams_pin = torch.from_numpy(cams_np).pin_memory()
+    out_pin = torch.empty((V, H, W, 3), dtype=torch.uint8).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        P.hmlfc_render_host(h, cams_pin.numpy(), W, H, out=out_pin.numpy())
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        P.hmlfc_render_host(h, cams_pin.numpy(), W, H, out=out_pin.numpy())   # synchronises before returning
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_views_per_s = world * V * e2e_steps / e2e_s
+    assert torch.equal(out_pin.cuda(), out), "host entry point and device entry point disagree"
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel: algorithmic bytes per launch / average launch time
+        peak, peak_src = _peaks()
+        fp = P.hmlfc_footprint_render(h, cams, W, H)
+        kernel_ms = float(np.mean(ms))
+        achieved = fp["bytes_alg"] / (kernel_ms * 1e-3) / 1e9
+        fpd = P.hmlfc_footprint_decode(h, coords)
+        dec_kernel_ms = float(np.mean(dec_ms))
+        dec_achieved = fpd["bytes_alg"] / (dec_kernel_ms * 1e-3) / 1e9
+        roofline = {
+            "bound": "hbm", "kernel": "render_tiled_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": _traffic_from_profiles("render"), "peak_source": peak_src,
+            "bytes_alg_per_launch": fp["bytes_alg"], "out_bytes": fp["out_bytes"],
+            "compressed_bytes_touched": fp["bytes_alg"] - fp["out_bytes"] - fp["in_bytes"],
+            "kernel_ms": kernel_ms, "frac_of_8TBs": achieved / 8000.0,
+        }
+        decode = {
+            "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
+            "roofline": {"bound": "hbm", "kernel": "decode_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
+                         "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
+                         "traffic": _traffic_from_profiles("decode")},
+        }
+        # ---- the oracle timed beside it, on a bounded sample of the same batch
+        import oracle as orc
+
+        s = orc.Stream(data)
+        cores = os.cpu_count() or 1
+        n_cpu, cpu_s = _oracle_views_sample(s, cams_np, W, H, args.cpu_budget, V)
+        cpu = {"value": n_cpu / cpu_s, "unit": "views/s", "cores": cores, "kind": "oracle",
+               "sample": f"{n_cpu} of the batch's {V} views ({W}x{H}), one at a time, OpenMP over {cores} threads, {cpu_s:.1f} s"}
+        line = {
+            "metric": "rendered_views_per_s", "value": views_per_s, "unit": "views/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": _config_dict(cfg, info, f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB fill)"),
+            "e2e": {"value": e2e_views_per_s, "unit": "views/s", "h2d_bytes_per_step": int(cams_np.nbytes),
+                    "d2h_bytes_per_step": int(out_pin.numel()), "steps": e2e_steps},
+            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "decode": decode,
+            "output_px_per_s": views_per_s * W * H, "clocks": clk.summary(),
+            "device_bytes": int(h.info.device_bytes),
+            "paper_context": "~200 fps at 512x512 on a GTX-980, Lego Knights (PAPER.md:409): another machine and light field, not the target",
+        }
+        print(json.dumps(line), flush=True)
+    P.hmlfc_free(h)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _traffic_from_profiles(which):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture, if any."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as fh:
+                return json.load(fh).get(which)
+        except Exception:
+            return None
+    return None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg2")
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args, args.config)
+    else:
+        run_ours(args, args.config)
+
+
+if __name__ == "__main__":
+    main()
