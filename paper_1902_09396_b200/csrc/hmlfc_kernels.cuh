@@ -21,6 +21,10 @@ cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_
                                 cudaStream_t st, int *n_launches);
 cudaError_t launch_render_tiled(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
                                 cudaStream_t st, int *n_launches);
+cudaError_t launch_render_blocks(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
+                                 cudaStream_t st, int *n_launches);
+// opts the block-centric kernel into its dynamic shared-memory size on the current device (call once per device)
+cudaError_t configure_render_blocks();
 cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,
                                     FootprintMarks marks, cudaStream_t st);
 cudaError_t launch_footprint_decode(const DevStream &S, const int32_t *d_coords, int64_t n, FootprintMarks marks,

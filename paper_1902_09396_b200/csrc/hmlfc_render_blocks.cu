@@ -1,0 +1,452 @@
+// Fused decode + render kernel, block-centric variant (sm_100a) -- the default of hmlfc_render.
+//
+// PAPER.md:289-293 (decoding procedure): "collect the required BISE compressed SRV blocks from the
+// top level to the bottom level.  Using the block indices, we infer whether a block belongs to the
+// predictive SRV images ... The motion vector values for the corresponding block are decoded" and
+// "As a block of pixels are decoded, our method benefits any LF rendering scheme by
+// providing fast access to neighboring pixels for interpolation".
+//
+// One CTA renders a 32 x TH tile of one output view.  The work of the tree walk is organised the
+// way the paper states it -- per BLOCK, not per sample -- and compacted so that the expensive
+// steps run on full warps over non-empty blocks only (at ~40 dB 70-90% of the blocks are empty):
+//   A   ray set-up per pixel; bounding box of the tile's 16-tap footprints in (u,v,s,t);
+//   S   the box's SRV planes: per level L the rectangle of planes (u>>L, v>>L) -- level >= 1 planes
+//       are shared by the 2^L x 2^L views below them, so each is visited once per tile;
+//   B1  one thread per (plane, channel, block) item: ONE 128-bit flag/rank record load, test the
+//       res / pred bits; non-empty items are appended to a compact record list in shared memory;
+//   B2  one thread per non-empty record: decode the block's motion record once (BISE), clip the
+//       block against the footprint box and append one task per needed value;
+//   B3  one thread per value task: BISE decode_at of the stored value, motion re-compensation from
+//       the reference SRV (flag/rank + BISE decode_at), written to a per-plane int16 accumulator;
+//   B4  one thread per (view, sample) of the box: top-level RKV + the h per-level terms, inverse
+//       YCoCg-R, clamp -> RGB8 patch in shared memory;
+//   C   every pixel gathers its 16 taps from the patch, blends in fp32, coalesced 32-bit stores.
+// If the box exceeds the shared-memory capacities (strong minification) the CTA falls back to 16
+// direct sample decodes per pixel.  All paths produce identical bytes.
+#include "hmlfc_kernels.cuh"
+
+namespace hmlfc {
+
+namespace {
+
+constexpr int kTW = 32;
+constexpr int kMaxSlots = 48;    // SRV planes of one tile's footprint, all levels
+constexpr int kMaxViews = 16;    // views of one tile's footprint
+constexpr int kAccCap = 2560;    // (plane, sample) accumulators of 4 x int16
+constexpr int kRecCap = 448;     // non-empty (plane, channel, block) records
+constexpr int kTaskCap = 6144;   // value tasks (uint16)
+constexpr int kPatchCap = 3072;  // (view, sample) RGB8 entries (aliases the task list)
+constexpr int kMaxItems = 32768;
+
+// digits of the packed trit / quint words: trit T -> t0 | t1<<2 | .. | t4<<8, quint Q -> q0 | q1<<3 | q2<<6
+struct DigitLut {
+    uint16_t v[384];
+};
+
+constexpr DigitLut make_digit_lut()
+{
+    DigitLut l{};
+    for (int T = 0; T < 256; ++T) {
+        int x = T, p = 0;
+        for (int k = 0; k < 5; ++k) { p |= (x % 3) << (2 * k); x /= 3; }
+        l.v[T] = (uint16_t)p;
+    }
+    for (int Q = 0; Q < 128; ++Q) {
+        int x = Q, p = 0;
+        for (int k = 0; k < 3; ++k) { p |= (x % 5) << (3 * k); x /= 5; }
+        l.v[256 + Q] = (uint16_t)p;
+    }
+    return l;
+}
+
+__device__ const DigitLut g_digit_lut = make_digit_lut();
+
+struct TileCtx {
+    int u0, v0, s0, t0;          // minima of the footprint box
+    int nu, nv, ns, nt;          // extents
+    int bx0, by0, nbw, nbh;      // block box
+    int nsamp, nblkbox, nviews, nslots, nitems;
+    uint32_t m_nblkbox, m_nbw, m_nsamp, m_ns, m_nu;  // magic multipliers: n / d = umulhi(n, m) (m == 0: d == 1)
+    int mode;                    // 0: no ray hits, 1: block path, 2: direct fallback
+    int lvl_base[kMaxLevels], lvl_pu0[kMaxLevels], lvl_pv0[kMaxLevels], lvl_nu[kMaxLevels];
+    int n_rec, n_task, overflow;
+};
+
+__device__ __forceinline__ uint32_t magic_of(uint32_t d) { return d <= 1u ? 0u : (uint32_t)(0x100000000ull / d) + 1u; }
+__device__ __forceinline__ uint32_t fdiv(uint32_t n, uint32_t m) { return m ? __umulhi(n, m) : n; }
+
+// bits [pos, pos+n) of an LSB-first 32-bit word string, n <= 16
+__device__ __forceinline__ uint32_t bits_at(const uint32_t *__restrict__ w, uint32_t pos, uint32_t n)
+{
+    const uint32_t *p = w + (pos >> 5);
+    return __funnelshift_r(__ldg(p), __ldg(p + 1), pos & 31u) & ((1u << n) - 1u);
+}
+
+// BISE decode_at (layout in DESIGN.md section 4) with the digit tables in shared memory
+__device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint32_t i, uint32_t layout, uint32_t m,
+                                            const uint16_t *__restrict__ lut)
+{
+    if (layout == 0u) return bits_at(w, i * m, m);
+    const bool trit = layout == 1u;
+    const uint32_t G = trit ? 5u : 3u, hb = trit ? 8u : 7u;
+    const uint32_t g = trit ? (__umulhi(i, 0xCCCCCCCDu) >> 2) : (__umulhi(i, 0xAAAAAAABu) >> 1);
+    const uint32_t k = i - G * g;
+    const uint32_t gb = g * (hb + G * m);
+    const uint32_t head = bits_at(w, gb, hb);
+    const uint32_t low = bits_at(w, gb + hb + k * m, m);
+    const uint32_t dig = ((uint32_t)lut[(trit ? 0u : 256u) + head] >> (k * (trit ? 2u : 3u))) & (trit ? 3u : 7u);
+    return (dig << m) | low;
+}
+
+__device__ __forceinline__ uint32_t blend16(const Taps &k, const uint32_t (&p)[16])
+{
+    // p[a*4 + b]: a = view (bit0 u, bit1 v), b = pixel (bit0 s, bit1 t)
+    const float ws0 = 1.0f - k.fs, wt0 = 1.0f - k.ft, wu0 = 1.0f - k.fu, wv0 = 1.0f - k.fv;
+    const float wst[4] = {ws0 * wt0, k.fs * wt0, ws0 * k.ft, k.fs * k.ft};
+    const float wuv[4] = {wu0 * wv0, k.fu * wv0, wu0 * k.fv, k.fu * k.fv};
+    float acc[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        float C[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const uint32_t rgb = p[a * 4 + b];
+            // byte -> float without the conversion pipe: 0x4B000000 | byte is the float 2^23 + byte
+            const float r = __uint_as_float(__byte_perm(rgb, 0x4B000000u, 0x7440)) - 8388608.0f;
+            const float g = __uint_as_float(__byte_perm(rgb, 0x4B000000u, 0x7441)) - 8388608.0f;
+            const float bl = __uint_as_float(__byte_perm(rgb, 0x4B000000u, 0x7442)) - 8388608.0f;
+            C[0] = fmaf(wst[b], r, C[0]);
+            C[1] = fmaf(wst[b], g, C[1]);
+            C[2] = fmaf(wst[b], bl, C[2]);
+        }
+        acc[0] = fmaf(wuv[a], C[0], acc[0]);
+        acc[1] = fmaf(wuv[a], C[1], acc[1]);
+        acc[2] = fmaf(wuv[a], C[2], acc[2]);
+    }
+    const uint32_t r = (uint32_t)min(max(__float2int_rd(acc[0] + 0.5f), 0), 255);
+    const uint32_t g = (uint32_t)min(max(__float2int_rd(acc[1] + 0.5f), 0), 255);
+    const uint32_t b = (uint32_t)min(max(__float2int_rd(acc[2] + 0.5f), 0), 255);
+    return r | (g << 8) | (b << 16);
+}
+
+template <int TH>
+struct Smem {
+    TileCtx cx;
+    int red[TH][8];
+    uint32_t stage[TH][24];
+    uint4 slotinfo[kMaxSlots];               // {pc index of channel 0, pc index of the reference plane's channel 0, level, predictive}
+    uint8_t vslot[kMaxViews][kMaxLevels];    // accumulator slot of view's plane at level L
+    uint16_t lut[384];
+    uint4 rec[kRecCap][2];
+    unsigned long long acc[kAccCap];         // 4 x int16 {Y, Co, Cg, -} per (slot, sample)
+    union {
+        uint16_t task[kTaskCap];
+        uint32_t patch[kPatchCap];
+    } tp;
+};
+
+template <int TH>
+__global__ void __launch_bounds__(kTW *TH)
+render_blocks_kernel(const DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned)
+{
+    constexpr int NT = kTW * TH;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem<TH> &sm = *reinterpret_cast<Smem<TH> *>(smem_raw);
+    TileCtx &cx = sm.cx;
+
+    const int lane = threadIdx.x, wy = threadIdx.y;
+    const int tid = wy * kTW + lane;
+    const int i = blockIdx.x * kTW + lane;
+    const int j = blockIdx.y * TH + wy;
+    const int view = blockIdx.z;
+    const bool valid = i < W && j < H;
+
+    // ---------------------------------------------------------------- phase A: rays and the footprint box
+    Ray r;
+    r.hit = false;
+    Taps k;
+    if (valid) {
+        const Camera cam = cams[view];
+        r = ray_setup(S, cam, W, H, i, j);
+    }
+    int lo[4] = {0x7fffffff, 0x7fffffff, 0x7fffffff, 0x7fffffff}, hi[4] = {-1, -1, -1, -1};
+    if (r.hit) {
+        k = tap_setup(S, r);
+        lo[0] = k.u0; lo[1] = k.v0; lo[2] = k.s0; lo[3] = k.t0;
+        hi[0] = k.u1; hi[1] = k.v1; hi[2] = k.s1; hi[3] = k.t1;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        lo[q] = __reduce_min_sync(0xffffffffu, lo[q]);
+        hi[q] = __reduce_max_sync(0xffffffffu, hi[q]);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { sm.red[wy][q] = lo[q]; sm.red[wy][4 + q] = hi[q]; }
+    }
+    for (int q = tid; q < 192; q += NT) reinterpret_cast<uint32_t *>(sm.lut)[q] = reinterpret_cast<const uint32_t *>(g_digit_lut.v)[q];
+    __syncthreads();
+    if (tid == 0) {
+        int L4[4], H4[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            L4[q] = sm.red[0][q]; H4[q] = sm.red[0][4 + q];
+            for (int w = 1; w < TH; ++w) { L4[q] = min(L4[q], sm.red[w][q]); H4[q] = max(H4[q], sm.red[w][4 + q]); }
+        }
+        cx.n_rec = 0; cx.n_task = 0; cx.overflow = 0;
+        if (H4[0] < 0) {
+            cx.mode = 0;
+        } else {
+            cx.u0 = L4[0]; cx.v0 = L4[1]; cx.s0 = L4[2]; cx.t0 = L4[3];
+            cx.nu = H4[0] - L4[0] + 1; cx.nv = H4[1] - L4[1] + 1; cx.ns = H4[2] - L4[2] + 1; cx.nt = H4[3] - L4[3] + 1;
+            cx.bx0 = L4[2] >> S.logB; cx.by0 = L4[3] >> S.logB;
+            cx.nbw = (H4[2] >> S.logB) - cx.bx0 + 1; cx.nbh = (H4[3] >> S.logB) - cx.by0 + 1;
+            const long long nsamp = (long long)cx.ns * cx.nt, nviews = (long long)cx.nu * cx.nv;
+            int nslots = 0;
+            for (int L = 0; L < S.h; ++L) {
+                const int pu0 = L4[0] >> L, pv0 = L4[1] >> L;
+                const int nuL = (H4[0] >> L) - pu0 + 1, nvL = (H4[1] >> L) - pv0 + 1;
+                cx.lvl_base[L] = nslots; cx.lvl_pu0[L] = pu0; cx.lvl_pv0[L] = pv0; cx.lvl_nu[L] = nuL;
+                nslots = min(nslots + nuL * nvL, 1 << 20);
+            }
+            const long long nblkbox = (long long)cx.nbw * cx.nbh;
+            const long long nitems = (long long)nslots * 3 * nblkbox;
+            const bool fits = nviews <= kMaxViews && nslots <= kMaxSlots && (long long)nslots * nsamp <= kAccCap &&
+                              nviews * nsamp <= kPatchCap && nitems <= kMaxItems;
+            cx.mode = fits ? 1 : 2;
+            cx.nsamp = (int)min(nsamp, 1LL << 20); cx.nviews = (int)min(nviews, 1LL << 20); cx.nslots = nslots;
+            cx.nblkbox = (int)min(nblkbox, 1LL << 20); cx.nitems = (int)min(nitems, 1LL << 30);
+            cx.m_nblkbox = magic_of((uint32_t)cx.nblkbox); cx.m_nbw = magic_of((uint32_t)cx.nbw);
+            cx.m_nsamp = magic_of((uint32_t)cx.nsamp); cx.m_ns = magic_of((uint32_t)cx.ns); cx.m_nu = magic_of((uint32_t)cx.nu);
+        }
+    }
+    __syncthreads();
+    const int mode = cx.mode;
+
+    uint32_t rgb = (uint32_t)S.bg[0] | ((uint32_t)S.bg[1] << 8) | ((uint32_t)S.bg[2] << 16);
+    if (mode == 1) {
+        const int nsamp = cx.nsamp, ns = cx.ns, nu = cx.nu, nslots = cx.nslots, h = S.h;
+        // ---------------------------------------------------------------- S: plane slots, view -> slot table, zero the accumulators
+        for (int s = tid; s < nslots; s += NT) {
+            int L = 0;
+            while (L + 1 < h && s >= cx.lvl_base[L + 1]) ++L;
+            const int jj = s - cx.lvl_base[L], nuL = cx.lvl_nu[L];
+            const int pv = cx.lvl_pv0[L] + jj / nuL, pu = cx.lvl_pu0[L] + jj % nuL;
+            const LevelDesc lv = S.lev[L];
+            sm.slotinfo[s] = make_uint4(lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u,
+                                        lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u, (uint32_t)L,
+                                        (uint32_t)((pu | pv) & 1));
+        }
+        for (int q = tid; q < cx.nviews * h; q += NT) {
+            const int vw = q / h, L = q - vw * h;
+            const int iv = vw / nu, iu = vw - iv * nu;
+            sm.vslot[vw][L] = (uint8_t)(cx.lvl_base[L] + (((cx.v0 + iv) >> L) - cx.lvl_pv0[L]) * cx.lvl_nu[L] +
+                                        (((cx.u0 + iu) >> L) - cx.lvl_pu0[L]));
+        }
+        for (int q = tid; q < nslots * nsamp; q += NT) sm.acc[q] = 0ull;
+        __syncthreads();
+
+        // ---------------------------------------------------------------- B1: classify (plane, channel, block) items
+        const int nitems = cx.nitems;
+        for (int base = 0; base < nitems; base += NT) {
+            const int it = base + tid;
+            bool keep = false;
+            uint4 r0, r1;
+            if (it < nitems) {
+                const uint32_t sc = fdiv((uint32_t)it, cx.m_nblkbox), blk = (uint32_t)it - sc * (uint32_t)cx.nblkbox;
+                const uint32_t slot = sc / 3u, c = sc - 3u * slot;
+                const uint32_t jb = fdiv(blk, cx.m_nbw), ib = blk - jb * (uint32_t)cx.nbw;
+                const uint4 si = sm.slotinfo[slot];
+                const uint4 d = ldg(S.pc + si.x + c);
+                const int bx = cx.bx0 + (int)ib, by = cx.by0 + (int)jb;
+                const int b = by * S.nbx + bx;
+                const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+                const uint32_t bit = 1u << (b & 31);
+                const bool res = (fr.x & bit) != 0u, pred = si.w && (fr.z & bit);
+                keep = res || pred;
+                r0 = make_uint4(d.y, res ? ((fr.y + popc(fr.x & (bit - 1u))) << (2 * S.logB)) : 0xFFFFFFFFu, d.w,
+                                pred ? (fr.w + popc(fr.z & (bit - 1u))) : 0xFFFFFFFFu);
+                r1 = make_uint4(d.z, si.y + c, (uint32_t)bx | ((uint32_t)by << 16), slot | (c << 16));
+            }
+            const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+            if (bal) {
+                int wbase = 0;
+                if (lane == 0) wbase = atomicAdd(&cx.n_rec, (int)popc(bal));
+                wbase = __shfl_sync(0xffffffffu, wbase, 0);
+                if (keep) {
+                    const int idx = wbase + (int)popc(bal & ((1u << lane) - 1u));
+                    if (idx < kRecCap) { sm.rec[idx][0] = r0; sm.rec[idx][1] = r1; }
+                    else cx.overflow = 1;
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---------------------------------------------------------------- B2: motion records, clip to the box, emit value tasks
+        const int nrec = min(cx.n_rec, kRecCap);
+        const bool ovf1 = cx.overflow != 0;
+        if (!ovf1) {
+            const int s0 = cx.s0, t0 = cx.t0, s1 = cx.s0 + cx.ns - 1, t1 = cx.t0 + cx.nt - 1, B = S.B;
+            for (int base = 0; base < nrec; base += NT) {
+                const int rr = base + tid;
+                int cnt = 0, xa = 0, xb = -1, ya = 0, yb = -1, x0 = 0, y0 = 0;
+                if (rr < nrec) {
+                    const uint4 r0 = sm.rec[rr][0], r1 = sm.rec[rr][1];
+                    uint32_t mvp = 0u;
+                    if (r0.w != 0xFFFFFFFFu) {
+                        const uint32_t rec = bise_at(S.mv + r1.x, r0.w, S.mv_layout, S.mv_m, sm.lut);
+                        int md, dx, dy;
+                        mv_unpack(S, rec, md, dx, dy);
+                        mvp = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+                    }
+                    sm.rec[rr][0].w = mvp;
+                    x0 = (int)(r1.z & 0xFFFFu) << S.logB; y0 = (int)(r1.z >> 16) << S.logB;
+                    xa = max(x0, s0); xb = min(x0 + B - 1, s1); ya = max(y0, t0); yb = min(y0 + B - 1, t1);
+                    cnt = (xb - xa + 1) * (yb - ya + 1);
+                }
+                // warp-inclusive scan of cnt, one atomic per warp
+                int inc = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += n;
+                }
+                const int tot = __shfl_sync(0xffffffffu, inc, 31);
+                if (tot) {
+                    int wbase = 0;
+                    if (lane == 0) wbase = atomicAdd(&cx.n_task, tot);
+                    wbase = __shfl_sync(0xffffffffu, wbase, 0);
+                    int o = wbase + inc - cnt;
+                    if (o + cnt > kTaskCap) { if (cnt) cx.overflow = 1; }
+                    else
+                        for (int y = ya; y <= yb; ++y)
+                            for (int x = xa; x <= xb; ++x) sm.tp.task[o++] = (uint16_t)((rr << 6) | (((y - y0) << S.logB) + (x - x0)));
+                }
+            }
+        }
+        __syncthreads();
+
+        if (cx.overflow == 0) {
+            // ---------------------------------------------------------------- B3: one stored / re-compensated value per task
+            const int ntask = cx.n_task;
+            int16_t *acc16 = reinterpret_cast<int16_t *>(sm.acc);
+            for (int t = tid; t < ntask; t += NT) {
+                const uint32_t task = sm.tp.task[t];
+                const uint32_t rr = task >> 6, kin = task & 63u;
+                const uint4 r0 = sm.rec[rr][0], r1 = sm.rec[rr][1];
+                const int x = ((int)(r1.z & 0xFFFFu) << S.logB) + (int)(kin & (uint32_t)(S.B - 1));
+                const int y = ((int)(r1.z >> 16) << S.logB) + (int)(kin >> S.logB);
+                int e = 0;
+                if (r0.y != 0xFFFFFFFFu) e = pc_offset(r0.z) + (int)bise_at(S.pay + r0.x, r0.y + kin, pc_layout(r0.z), pc_m(r0.z), sm.lut);
+                if (r0.w) {
+                    const int rx = x + (int)((r0.w >> 8) & 0xFFu) - S.W, ry = y + (int)(r0.w & 0xFFu) - S.W;
+                    int q = 0;
+                    if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {
+                        const uint4 d = ldg(S.pc + r1.y);
+                        const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+                        const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+                        const uint32_t bit = 1u << (b & 31);
+                        if (fr.x & bit) {
+                            const uint32_t ii = ((fr.y + popc(fr.x & (bit - 1u))) << (2 * S.logB)) +
+                                                (uint32_t)(((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1)));
+                            q = pc_offset(d.w) + (int)bise_at(S.pay + d.y, ii, pc_layout(d.w), pc_m(d.w), sm.lut);
+                        }
+                    }
+                    e += (r0.w & 0x10000u) ? -q : q;  // R10: subtractive P = e + R, additive P = e - R
+                }
+                const int samp = (y - cx.t0) * ns + (x - cx.s0);
+                acc16[(((int)(r1.w & 0xFFFFu) * nsamp + samp) << 2) + (int)(r1.w >> 16)] = (int16_t)e;
+            }
+            __syncthreads();
+
+            // ---------------------------------------------------------------- B4: RKV + per-level terms -> RGB8 patch
+            const int ncell = cx.nviews * nsamp;
+            for (int q = tid; q < ncell; q += NT) {
+                const uint32_t vw = fdiv((uint32_t)q, cx.m_nsamp), samp = (uint32_t)q - vw * (uint32_t)nsamp;
+                const uint32_t iv = fdiv(vw, cx.m_nu), iu = vw - iv * (uint32_t)nu;
+                const uint32_t it = fdiv(samp, cx.m_ns), is = samp - it * (uint32_t)ns;
+                const int u = cx.u0 + (int)iu, v = cx.v0 + (int)iv, x = cx.s0 + (int)is, y = cx.t0 + (int)it;
+                const size_t ri = ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)y) * (size_t)S.Ws + (size_t)x;
+                const short4 rk = ldg(S.rkv + ri);
+                int a[3] = {rk.x, rk.y, rk.z};
+                for (int L = 0; L < h; ++L) {
+                    const unsigned long long w = sm.acc[(int)sm.vslot[vw][L] * nsamp + (int)samp];
+                    a[0] += (int)(int16_t)(w & 0xFFFFull);
+                    a[1] += (int)(int16_t)((w >> 16) & 0xFFFFull);
+                    a[2] += (int)(int16_t)((w >> 32) & 0xFFFFull);
+                }
+                sm.tp.patch[q] = ycocg_to_rgb8(a);
+            }
+            __syncthreads();
+
+            // ---------------------------------------------------------------- C: gather + blend
+            if (r.hit) {
+                uint32_t p[16];
+                const int plane = nsamp;
+                const int bu[2] = {k.u0 - cx.u0, k.u1 - cx.u0}, bv[2] = {k.v0 - cx.v0, k.v1 - cx.v0};
+                const int bs[2] = {k.s0 - cx.s0, k.s1 - cx.s0}, bt[2] = {k.t0 - cx.t0, k.t1 - cx.t0};
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    const int vbase = (bv[a >> 1] * nu + bu[a & 1]) * plane;
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) p[a * 4 + b] = sm.tp.patch[vbase + bt[b >> 1] * ns + bs[b & 1]];
+                }
+                rgb = blend16(k, p);
+            }
+        }
+    }
+    if ((mode == 2 || (mode == 1 && cx.overflow != 0)) && r.hit) {
+        // ---------------------------------------------------------------- fallback: 16 direct sample decodes
+        uint32_t p[16];
+#pragma unroll 1
+        for (int a = 0; a < 16; ++a)
+            p[a] = decode_rgb8(S, (a & 4) ? k.u1 : k.u0, (a & 8) ? k.v1 : k.v0, (a & 1) ? k.s1 : k.s0, (a & 2) ? k.t1 : k.t0);
+        rgb = blend16(k, p);
+    }
+
+    // ---------------------------------------------------------------- store: 96 contiguous bytes per tile row
+    const int i0 = blockIdx.x * kTW;
+    const bool fast = out_aligned && (i0 + kTW <= W) && (j < H);
+    uint8_t *rowp = out + 3 * (((size_t)view * H + (size_t)min(j, H - 1)) * (size_t)W + (size_t)i0);
+    if (fast) {
+        uint8_t *sb = reinterpret_cast<uint8_t *>(sm.stage[wy]);
+        sb[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
+        sb[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
+        sb[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
+        __syncwarp();
+        if (lane < 24) reinterpret_cast<uint32_t *>(rowp)[lane] = sm.stage[wy][lane];
+    } else if (valid) {
+        uint8_t *o = rowp + 3 * lane;
+        o[0] = (uint8_t)(rgb & 0xFF);
+        o[1] = (uint8_t)((rgb >> 8) & 0xFF);
+        o[2] = (uint8_t)((rgb >> 16) & 0xFF);
+    }
+}
+
+template <int TH>
+cudaError_t launch_t(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st)
+{
+    const size_t smem = sizeof(Smem<TH>);
+    dim3 block(kTW, TH), grid((W + kTW - 1) / kTW, (H + TH - 1) / TH, n_views);
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0 && (W % 4) == 0) ? 1 : 0;
+    render_blocks_kernel<TH><<<grid, block, smem, st>>>(S, d_cams, W, H, d_out, aligned);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t configure_render_blocks()
+{
+    return cudaFuncSetAttribute(render_blocks_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<8>));
+}
+
+cudaError_t launch_render_blocks(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
+                                 cudaStream_t st, int *n_launches)
+{
+    if (n_views == 0) return cudaSuccess;
+    cudaError_t e = launch_t<8>(S, d_cams, n_views, W, H, d_out, st);
+    if (n_launches) *n_launches += 1;
+    return e;
+}
+
+}  // namespace hmlfc
