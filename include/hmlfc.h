@@ -125,11 +125,13 @@ int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n
                            hmlfc_footprint_t *out);
 int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out);
 
-/* Kernel selection for hmlfc_render: 0 = automatic (default; currently 3), 1 = one thread per
+/* Kernel selection for hmlfc_render: 0 = automatic (default; currently 4), 1 = one thread per
  * output pixel (16 independent tap decodes), 2 = sample-shared tile (a CTA decodes every LF sample
  * of its tile's footprint once into shared memory), 3 = block-centric tile (per tile: classify the
  * footprint's blocks, decode motion records once per block, evaluate only non-empty blocks on full
- * warps, share level >= 1 planes between the tile's views).  All variants produce identical bytes. */
+ * warps, share level >= 1 planes between the tile's views), 4 = the same block-centric pipeline run by
+ * ONE WARP per 16x8 tile out of a private shared-memory workspace (no CTA barriers).  All variants
+ * produce identical bytes. */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Number of kernels this library has launched through the handle since load (bench accounting). */

@@ -118,7 +118,7 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
         (ce = cudaMalloc(reinterpret_cast<void **>(&h->d_oob), sizeof(unsigned long long))) != cudaSuccess ||
         (ce = cudaMemset(h->d_oob, 0, sizeof(unsigned long long))) != cudaSuccess ||
         (ce = cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking)) != cudaSuccess ||
-        (ce = configure_render_blocks()) != cudaSuccess) {
+        (ce = configure_render_blocks()) != cudaSuccess || (ce = configure_render_warp()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
@@ -158,8 +158,10 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 2)
         CU(h, launch_render_tiled(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else
+    else if (h->render_variant == 3)
         CU(h, launch_render_blocks(h->ds, cams, n_views, W, H, d_out, st, &nl));
+    else
+        CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 5 ? 1 : 0));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -262,7 +264,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 3) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 5) return HMLFC_E_INVALID;
     h->render_variant = variant;
     return HMLFC_OK;
 }

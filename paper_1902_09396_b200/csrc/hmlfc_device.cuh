@@ -51,6 +51,8 @@ struct DevStream {
     const uint32_t *mv;
     const short4 *rkv;
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
+    float uv_inv[2], st_inv[2];  // 1 / step where that is exact (step a power of two), see pow2_mask
+    uint32_t pow2_mask;          // bit 0..3: uv_step[0], uv_step[1], st_step[0], st_step[1] is a power of two
     uint8_t bg[4];
 };
 
@@ -246,14 +248,28 @@ struct Ray {
 #define HMLFC_DIV(a, b) ((a) / (b))
 #endif
 
+// x / step.  When step is a power of two, x * (1/step) is the same correctly rounded real number, so
+// the multiplication is bit-identical to the IEEE division the definition asks for.
+HMLFC_DEV float div_step(float x, float step, float inv, bool pow2) { return pow2 ? HMLFC_MUL(x, inv) : HMLFC_DIV(x, step); }
+
+// screen coordinate of pixel column / row i of an n-pixel-wide view: ((2 (i + 0.5)) / n - 1) tan_half
+HMLFC_DEV float ray_screen(float tan_half, int n, int i)
+{
+    return HMLFC_MUL(HMLFC_SUB(HMLFC_DIV(HMLFC_MUL(2.0f, HMLFC_ADD((float)i, 0.5f)), (float)n), 1.0f), tan_half);
+}
+
+HMLFC_DEV Ray ray_from_screen(const DevStream &S, const Camera &cam, float px, float py);
+
 HMLFC_DEV Ray ray_setup(const DevStream &S, const Camera &cam, int W, int H, int i, int j)
+{
+    return ray_from_screen(S, cam, ray_screen(cam.tan_half_x, W, i), ray_screen(cam.tan_half_y, H, j));
+}
+
+HMLFC_DEV Ray ray_from_screen(const DevStream &S, const Camera &cam, float px, float py)
 {
     Ray r;
     r.hit = false;
     r.u = r.v = r.s = r.t = 0.0f;
-    float fi = HMLFC_ADD((float)i, 0.5f), fj = HMLFC_ADD((float)j, 0.5f);
-    float px = HMLFC_MUL(HMLFC_SUB(HMLFC_DIV(HMLFC_MUL(2.0f, fi), (float)W), 1.0f), cam.tan_half_x);
-    float py = HMLFC_MUL(HMLFC_SUB(HMLFC_DIV(HMLFC_MUL(2.0f, fj), (float)H), 1.0f), cam.tan_half_y);
     float Dx = HMLFC_ADD(HMLFC_ADD(cam.fwd[0], HMLFC_MUL(px, cam.right[0])), HMLFC_MUL(py, cam.down[0]));
     float Dy = HMLFC_ADD(HMLFC_ADD(cam.fwd[1], HMLFC_MUL(px, cam.right[1])), HMLFC_MUL(py, cam.down[1]));
     float Dz = HMLFC_ADD(HMLFC_ADD(cam.fwd[2], HMLFC_MUL(px, cam.right[2])), HMLFC_MUL(py, cam.down[2]));
@@ -264,10 +280,10 @@ HMLFC_DEV Ray ray_setup(const DevStream &S, const Camera &cam, int W, int H, int
     float vw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l0, Dy));
     float sw = HMLFC_ADD(cam.eye[0], HMLFC_MUL(l1, Dx));
     float tw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l1, Dy));
-    float u = HMLFC_DIV(HMLFC_SUB(uw, S.uv_origin[0]), S.uv_step[0]);
-    float v = HMLFC_DIV(HMLFC_SUB(vw, S.uv_origin[1]), S.uv_step[1]);
-    float s = HMLFC_DIV(HMLFC_SUB(sw, S.st_origin[0]), S.st_step[0]);
-    float t = HMLFC_DIV(HMLFC_SUB(tw, S.st_origin[1]), S.st_step[1]);
+    float u = div_step(HMLFC_SUB(uw, S.uv_origin[0]), S.uv_step[0], S.uv_inv[0], S.pow2_mask & 1u);
+    float v = div_step(HMLFC_SUB(vw, S.uv_origin[1]), S.uv_step[1], S.uv_inv[1], S.pow2_mask & 2u);
+    float s = div_step(HMLFC_SUB(sw, S.st_origin[0]), S.st_step[0], S.st_inv[0], S.pow2_mask & 4u);
+    float t = div_step(HMLFC_SUB(tw, S.st_origin[1]), S.st_step[1], S.st_inv[1], S.pow2_mask & 8u);
     if (!(u >= 0.0f && u <= (float)(S.U - 1) && v >= 0.0f && v <= (float)(S.V - 1) && s >= 0.0f &&
           s <= (float)(S.Ws - 1) && t >= 0.0f && t <= (float)(S.Ht - 1)))
         return r;

@@ -25,6 +25,10 @@ cudaError_t launch_render_blocks(const DevStream &S, const Camera *d_cams, int n
                                  cudaStream_t st, int *n_launches);
 // opts the block-centric kernel into its dynamic shared-memory size on the current device (call once per device)
 cudaError_t configure_render_blocks();
+// shape 0: 16 x 8 tiles (4 pixels per lane), 1: 8 x 8 tiles (2 pixels per lane)
+cudaError_t launch_render_warp(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
+                               int *n_launches, int shape);
+cudaError_t configure_render_warp();
 cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,
                                     FootprintMarks marks, cudaStream_t st);
 cudaError_t launch_footprint_decode(const DevStream &S, const int32_t *d_coords, int64_t n, FootprintMarks marks,

@@ -5,6 +5,7 @@
 #include "../../include/hmlfc.h"
 #include "hmlfc_device.cuh"
 
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -93,6 +94,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     if (I.height > kMaxLevels || I.window > 64) return HMLFC_E_UNSUPPORTED;
     if (!(I.block == 2 || I.block == 4 || I.block == 8) || (I.Ws % I.block) || (I.Ht % I.block)) return HMLFC_E_UNSUPPORTED;
     if ((uint64_t)I.U * I.V > (1u << 24) || (uint64_t)I.Ws * I.Ht > (1u << 26)) return HMLFC_E_UNSUPPORTED;
+    if (I.U > 4096 || I.V > 4096 || I.Ws > 16384 || I.Ht > 16384) return HMLFC_E_UNSUPPORTED;  // packed tap indices
     if (len < total) return HMLFC_E_TRUNCATED;
 
     DevStream &D = T.ds;
@@ -108,6 +110,14 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
         D.st_origin[i] = I.st_origin[i]; D.st_step[i] = I.st_step[i];
     }
     D.z_st = I.z_st;
+    D.pow2_mask = 0;
+    for (int i = 0; i < 4; ++i) {  // a step whose reciprocal is exact lets the kernels multiply instead of divide
+        const float step = i < 2 ? I.uv_step[i] : I.st_step[i - 2];
+        int e = 0;
+        const bool pow2 = std::isnormal(step) && std::frexp(step, &e) == 0.5f && std::isnormal(1.0f / step);
+        (i < 2 ? D.uv_inv[i] : D.st_inv[i - 2]) = pow2 ? 1.0f / step : 0.0f;
+        if (pow2) D.pow2_mask |= 1u << i;
+    }
     D.bg[0] = I.background[0]; D.bg[1] = I.background[1]; D.bg[2] = I.background[2]; D.bg[3] = 0;
 
     // level table: the stream lists levels top-down (L = h-1 .. 0), planes row-major, channel innermost
