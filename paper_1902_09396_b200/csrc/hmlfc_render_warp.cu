@@ -19,10 +19,12 @@
 //       res / pred bits; non-empty items are compacted (ballot) into a record list;
 //   B2  one lane per record: decode the block's motion record once (BISE), clip the block against
 //       the footprint box, emit one task per needed value (warp scan);
+//   R   one lane per (view, sample) cell of the box: the top-level RKV sample initialises the cell's
+//       (Y, Co, Cg) accumulator in shared memory;
 //   B3  one lane per value task: BISE decode_at of the stored value, motion re-compensation from
-//       the reference SRV (flag/rank + BISE decode_at), written to a per-plane int16 accumulator;
-//   B4  one lane per (view, sample) of the box: top-level RKV + the h per-level terms, inverse
-//       YCoCg-R, clamp -> float RGB patch;
+//       the reference SRV (flag/rank + BISE decode_at), added (shared-memory atomics) to the cell of
+//       every view of the box that lies below the plane;
+//   B4  one lane per cell, in place: inverse YCoCg-R, clamp -> float RGB;
 //   C   every pixel gathers its 16 taps from the patch (128-bit loads), blends with packed fp32 FMAs,
 //       and the lane's 4 pixels leave as three 32-bit stores.
 // A tile whose footprint exceeds the workspace is split by rows (8 -> 4 -> 2 -> 1); a single row that
@@ -41,14 +43,13 @@ constexpr int kMaxItems = 8192;
 
 // Compile-time shape of one instantiation: tile = (4 PPL) x 8 output pixels per warp, and the capacities of the
 // warp's shared-memory workspace.
-template <int PPL_, int WARPS_, int ACC_, int REC_, int TASK_, int CELL_, int MINB_>
+template <int PPL_, int WARPS_, int REC_, int TASK_, int CELL_, int MINB_>
 struct Cfg {
     static constexpr int kPPL = PPL_, kTileW = 4 * PPL_;
     static constexpr int kWarps = WARPS_;   // warps (= tiles) per CTA
-    static constexpr int kAccCap = ACC_;    // (plane, sample) accumulators of 4 x int16
     static constexpr int kRecCap = REC_;    // non-empty (plane, channel, block) records per chunk
     static constexpr int kTaskCap = TASK_;  // value tasks per chunk
-    static constexpr int kCellCap = CELL_;  // (view, sample) float4 patch entries (aliases records + tasks)
+    static constexpr int kCellCap = CELL_;  // (view, sample) cells: int4 accumulators, then float4 RGB in place
     static constexpr int kMinBlocks = MINB_;
 };
 
@@ -102,6 +103,22 @@ __device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint
     return (dig << m) | low;
 }
 
+// The same decode without control flow (plain = groups of one value with an empty digit word): every lane of a
+// warp issues the same loads, so independent decodes overlap and lanes with different layouts do not serialise.
+__device__ __forceinline__ uint32_t bise_at_uniform(const uint32_t *__restrict__ w, uint32_t i, uint32_t layout, uint32_t m,
+                                                    const uint16_t *__restrict__ lut)
+{
+    const bool plain = layout == 0u, trit = layout == 1u;
+    const uint32_t G = plain ? 1u : (trit ? 5u : 3u), hb = plain ? 0u : (trit ? 8u : 7u);
+    const uint32_t g = plain ? i : (trit ? (__umulhi(i, 0xCCCCCCCDu) >> 2) : (__umulhi(i, 0xAAAAAAABu) >> 1));
+    const uint32_t k = i - G * g;
+    const uint32_t gb = g * (hb + G * m);
+    const uint32_t head = bits_at(w, gb, hb);  // plain: 0 bits -> 0, and the quint table maps 0 to digit 0
+    const uint32_t low = bits_at(w, gb + hb + k * m, m);
+    const uint32_t dig = ((uint32_t)lut[(trit ? 0u : 256u) + head] >> (k * (trit ? 2u : 3u))) & (trit ? 3u : 7u);
+    return (dig << m) | low;
+}
+
 template <class C>
 struct Queues {
     uint4 rec[C::kRecCap][2];
@@ -110,13 +127,12 @@ struct Queues {
 
 template <class C>
 struct WarpWs {
-    unsigned long long acc[C::kAccCap];  // 4 x int16 {Y, Co, Cg, -} per (slot, sample)
     union {
-        Queues<C> q;
-        float4 patch[C::kCellCap];       // {R, G, B, 0} per (view, sample)
-    } tp;
-    uint4 slotinfo[kMaxSlots];        // {pc index of channel 0, pc index of the reference plane's channel 0, level, predictive}
-    uint8_t vslot[kMaxViews][kMaxLevels];  // accumulator slot of a view's plane at level L
+        int4 acc[C::kCellCap];      // {Y, Co, Cg, -} per (view, sample) while the levels are summed
+        float4 rgb[C::kCellCap];    // {R, G, B, 0} afterwards
+    } cell;
+    Queues<C> q;
+    uint4 slotinfo[kMaxSlots];      // {pc index of channel 0, pc index of the reference plane's channel 0, predictive, views below}
     int lvl_base[kMaxLevels], lvl_pu0[kMaxLevels], lvl_pv0[kMaxLevels], lvl_nu[kMaxLevels];
 };
 
@@ -180,7 +196,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                    int tiles_x, int tiles_per_view)
 {
     constexpr int kPPL = C::kPPL, kTileW = C::kTileW, kWarps = C::kWarps;
-    constexpr int kAccCap = C::kAccCap, kRecCap = C::kRecCap, kTaskCap = C::kTaskCap, kCellCap = C::kCellCap;
+    constexpr int kRecCap = C::kRecCap, kTaskCap = C::kTaskCap, kCellCap = C::kCellCap;
     static_assert(kRecCap >= 32 && (kRecCap << 6) <= 65536 && kTaskCap >= 64, "queue capacities");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint16_t lut[384];
@@ -269,38 +285,49 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
             }
             const int nslots = __shfl_sync(FULL, incl, h - 1);
             const long long nsamp_l = (long long)ns * nt, nviews_l = (long long)nu * nv, nblk_l = (long long)nbw * nbh;
-            const bool fits = nviews_l <= kMaxViews && nslots <= kMaxSlots && nslots * nsamp_l <= kAccCap &&
+            const bool fits = nu <= 8 && nv <= 8 && nviews_l <= kMaxViews && nslots <= kMaxSlots && nbw <= 32 && nbh <= 32 &&
                               nviews_l * nsamp_l <= kCellCap && nslots * 3 * nblk_l <= kMaxItems;
             if (fits) {
                 const int nsamp = (int)nsamp_l, nviews = (int)nviews_l, nblkbox = (int)nblk_l, nitems = nslots * 3 * nblkbox;
-                __syncwarp();  // the previous range's patch reads are complete
+                const int ncell = nviews * nsamp;
+                // magic multipliers for the index decompositions below: lane i computes one, everybody fetches it
+                uint32_t mg = 0u;
+                if (lane < 5) mg = magic_of((uint32_t)(lane == 0 ? nblkbox : lane == 1 ? nbw : lane == 2 ? nsamp : lane == 3 ? ns : nu));
+                const uint32_t m_nblkbox = __shfl_sync(FULL, mg, 0), m_nbw = __shfl_sync(FULL, mg, 1), m_nsamp = __shfl_sync(FULL, mg, 2),
+                               m_ns = __shfl_sync(FULL, mg, 3), m_nu = __shfl_sync(FULL, mg, 4);
+                __syncwarp();  // the previous range's cell reads are complete
                 if (lane < h) { ws.lvl_base[lane] = incl - cntL; ws.lvl_pu0[lane] = pu0; ws.lvl_pv0[lane] = pv0; ws.lvl_nu[lane] = nuL; }
-                for (int q = lane; q < nslots * nsamp; q += 32) ws.acc[q] = 0ull;
+                // ------------------------------------------------------------ R: top-level RKV samples initialise the cells
+                for (int q = lane; q < ncell; q += 32) {
+                    const uint32_t vw = fdiv((uint32_t)q, m_nsamp), samp = (uint32_t)q - vw * (uint32_t)nsamp;
+                    const uint32_t iv = fdiv(vw, m_nu), iu = vw - iv * (uint32_t)nu;
+                    const uint32_t it = fdiv(samp, m_ns), is = samp - it * (uint32_t)ns;
+                    const uint32_t top = (uint32_t)(((bv0 + (int)iv) >> h) * S.UH + ((bu0 + (int)iu) >> h));
+                    const short4 rk = ldg(S.rkv + ((size_t)top * (size_t)S.Ht + (size_t)(bt0 + (int)it)) * (size_t)S.Ws + (size_t)(bs0 + (int)is));
+                    ws.cell.acc[q] = make_int4(rk.x, rk.y, rk.z, 0);
+                }
                 __syncwarp();
-                // ------------------------------------------------------------ S (part 2): slot table, view -> slot table
+                // ------------------------------------------------------------ S (part 2): slot table
                 for (int s = lane; s < nslots; s += 32) {
                     int L = 0;
                     while (L + 1 < h && s >= ws.lvl_base[L + 1]) ++L;
                     const int jj = s - ws.lvl_base[L], n = ws.lvl_nu[L];
-                    const int pv = ws.lvl_pv0[L] + jj / n, pu = ws.lvl_pu0[L] + jj % n;
+                    const int jv = jj / n;
+                    const int pv = ws.lvl_pv0[L] + jv, pu = ws.lvl_pu0[L] + (jj - jv * n);
                     const LevelDesc lv = S.lev[L];
+                    // views of the box below this plane: [iu0, iu1] x [iv0, iv1] relative to (bu0, bv0)
+                    const int iu0 = max(pu << L, bu0) - bu0, iu1 = min(((pu + 1) << L) - 1, bu0 + nu - 1) - bu0;
+                    const int iv0 = max(pv << L, bv0) - bv0, iv1 = min(((pv + 1) << L) - 1, bv0 + nv - 1) - bv0;
                     ws.slotinfo[s] = make_uint4(lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u,
-                                                lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u, (uint32_t)L,
-                                                (uint32_t)((pu | pv) & 1));
-                }
-                for (int q = lane; q < nviews * h; q += 32) {
-                    const int vw = q / h, L = q - vw * h;
-                    const int iv = vw / nu, iu = vw - iv * nu;
-                    ws.vslot[vw][L] = (uint8_t)(ws.lvl_base[L] + (((bv0 + iv) >> L) - ws.lvl_pv0[L]) * ws.lvl_nu[L] +
-                                                (((bu0 + iu) >> L) - ws.lvl_pu0[L]));
+                                                lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u, (uint32_t)((pu | pv) & 1),
+                                                (uint32_t)(iu0 | (iu1 << 3) | (iv0 << 6) | (iv1 << 9)));
                 }
                 __syncwarp();
 
                 // ------------------------------------------------------------ B1..B3, in chunks that fit the record / task queues
-                const uint32_t m_nblkbox = magic_of((uint32_t)nblkbox), m_nbw = magic_of((uint32_t)nbw);
                 const int s1 = bs0 + ns - 1, t1 = bt0 + nt - 1;
                 const int rec_step = min(32, kTaskCap >> (2 * logB));  // records whose tasks always fit one B2 step
-                int16_t *acc16 = reinterpret_cast<int16_t *>(ws.acc);
+                                int *acc32 = reinterpret_cast<int *>(ws.cell.acc);
                 int item_base = 0;
                 while (item_base < nitems) {
                     // -------------------------------------------------------- B1: classify (plane, channel, block) items
@@ -315,20 +342,20 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                             const uint32_t jb = fdiv(blk, m_nbw), ib = blk - jb * (uint32_t)nbw;
                             const uint4 si = ws.slotinfo[slot];
                             const uint4 d = ldg(S.pc + si.x + c);
-                            const int bx = bx0 + (int)ib, by = by0 + (int)jb;
-                            const int b = by * S.nbx + bx;
+                            const int b = (by0 + (int)jb) * S.nbx + bx0 + (int)ib;
                             const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
                             const uint32_t bit = 1u << (b & 31);
-                            const bool res = (fr.x & bit) != 0u, pred = si.w && (fr.z & bit);
+                            const bool res = (fr.x & bit) != 0u, pred = si.z && (fr.z & bit);
                             keep = res || pred;
+                            // own payload base, rank * B^2, descriptor word, rank of the motion record | MV string base, reference pc, -, position
                             r0 = make_uint4(d.y, res ? ((fr.y + popc(fr.x & (bit - 1u))) << (2 * logB)) : 0xFFFFFFFFu, d.w,
                                             pred ? (fr.w + popc(fr.z & (bit - 1u))) : 0xFFFFFFFFu);
-                            r1 = make_uint4(d.z, si.y + c, (uint32_t)bx | ((uint32_t)by << 16), slot | (c << 16));
+                            r1 = make_uint4(d.z, si.y + c, 0u, ib | (jb << 5) | (c << 10) | (si.w << 12));
                         }
                         const uint32_t bal = __ballot_sync(FULL, keep);
                         if (keep) {
                             const int idx = n_rec + (int)popc(bal & ((1u << lane) - 1u));
-                            ws.tp.q.rec[idx][0] = r0; ws.tp.q.rec[idx][1] = r1;
+                            ws.q.rec[idx][0] = r0; ws.q.rec[idx][1] = r1;
                         }
                         n_rec += (int)popc(bal);
                         item_base += 32;
@@ -336,26 +363,30 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                     __syncwarp();
                     int rec_base = 0;
                     while (rec_base < n_rec) {
-                        // ---------------------------------------------------- B2: motion records, clip to the box, emit value tasks
+                        // ---------------------------------------------------- B2: motion record + reference descriptor once per block, emit value tasks
                         int n_task = 0;
                         while (rec_base < n_rec && n_task + (rec_step << (2 * logB)) <= kTaskCap) {
                             const int rr = rec_base + lane;
-                            int cnt = 0, xa = 0, xb = -1, ya = 0, yb = -1, bx_ = 0, by_ = 0;
+                            int cnt = 0, kxa = 0, kxb = -1, kya = 0, kyb = -1;
                             if (lane < rec_step && rr < n_rec) {
-                                const uint4 r0 = ws.tp.q.rec[rr][0], r1 = ws.tp.q.rec[rr][1];
-                                uint32_t mvp = 0u;
+                                const uint4 r0 = ws.q.rec[rr][0], r1 = ws.q.rec[rr][1];
                                 if (r0.w != 0xFFFFFFFFu) {
                                     const uint32_t rec = bise_at(S.mv + r1.x, r0.w, S.mv_layout, S.mv_m, lut);
                                     int md, dx, dy;
                                     mv_unpack(S, rec, md, dx, dy);
-                                    mvp = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+                                    const uint4 d = ldg(S.pc + r1.y);
+                                    ws.q.rec[rr][0].w = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+                                    ws.q.rec[rr][1] = make_uint4(d.x, d.y, d.w, r1.w);
+                                } else {
+                                    ws.q.rec[rr][0].w = 0u;
+                                    ws.q.rec[rr][1] = make_uint4(0u, 0u, 0u, r1.w);  // B3 reads through these unconditionally
                                 }
-                                ws.tp.q.rec[rr][0].w = mvp;
-                                bx_ = (int)(r1.z & 0xFFFFu) << logB; by_ = (int)(r1.z >> 16) << logB;
-                                xa = max(bx_, bs0); xb = min(bx_ + Bm1, s1); ya = max(by_, bt0); yb = min(by_ + Bm1, t1);
-                                cnt = (xb - xa + 1) * (yb - ya + 1);
+                                const int bx_ = (bx0 + (int)(r1.w & 31u)) << logB, by_ = (by0 + (int)((r1.w >> 5) & 31u)) << logB;
+                                kxa = max(bx_, bs0) - bx_; kxb = min(bx_ + Bm1, s1) - bx_;
+                                kya = max(by_, bt0) - by_; kyb = min(by_ + Bm1, t1) - by_;
+                                cnt = (kxb - kxa + 1) * (kyb - kya + 1);
                             }
-                            int inc = cnt;
+                            int inc = cnt;  // warp-inclusive scan: the records' tasks stay contiguous (coherent lanes in B3)
 #pragma unroll
                             for (int o = 1; o < 32; o <<= 1) {
                                 const int n = __shfl_up_sync(FULL, inc, o);
@@ -363,64 +394,58 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                             }
                             int o = n_task + inc - cnt;
                             n_task += __shfl_sync(FULL, inc, 31);
-                            for (int yy = ya; yy <= yb; ++yy)
-                                for (int xx = xa; xx <= xb; ++xx)
-                                    ws.tp.q.task[o++] = (uint16_t)((rr << 6) | (((yy - by_) << logB) + (xx - bx_)));
+                            for (int ky = kya; ky <= kyb; ++ky)
+                                for (int kx = kxa; kx <= kxb; ++kx) ws.q.task[o++] = (uint16_t)((rr << 6) | ((ky << logB) + kx));
                             rec_base += rec_step;
                         }
                         __syncwarp();
                         // ---------------------------------------------------- B3: one stored / re-compensated value per task
                         for (int t = lane; t < n_task; t += 32) {
-                            const uint32_t task = ws.tp.q.task[t];
+                            const uint32_t task = ws.q.task[t];
                             const uint32_t rr = task >> 6, kin = task & 63u;
-                            const uint4 r0 = ws.tp.q.rec[rr][0], r1 = ws.tp.q.rec[rr][1];
-                            const int xx = ((int)(r1.z & 0xFFFFu) << logB) + (int)(kin & (uint32_t)Bm1);
-                            const int yy = ((int)(r1.z >> 16) << logB) + (int)(kin >> logB);
-                            int e = 0;
-                            if (r0.y != 0xFFFFFFFFu)
-                                e = pc_offset(r0.z) + (int)bise_at(S.pay + r0.x, r0.y + kin, pc_layout(r0.z), pc_m(r0.z), lut);
-                            if (r0.w) {
-                                const int rx = xx + (int)((r0.w >> 8) & 0xFFu) - S.W, ryy = yy + (int)(r0.w & 0xFFu) - S.W;
-                                int q = 0;
-                                if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ryy < (unsigned)S.Ht) {
-                                    const uint4 d = ldg(S.pc + r1.y);
-                                    const int b = (ryy >> logB) * S.nbx + (rx >> logB);
-                                    const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
-                                    const uint32_t bit = 1u << (b & 31);
-                                    if (fr.x & bit) {
-                                        const uint32_t ii = ((fr.y + popc(fr.x & (bit - 1u))) << (2 * logB)) +
-                                                            (uint32_t)(((ryy & Bm1) << logB) + (rx & Bm1));
-                                        q = pc_offset(d.w) + (int)bise_at(S.pay + d.y, ii, pc_layout(d.w), pc_m(d.w), lut);
-                                    }
+                            const uint4 r0 = ws.q.rec[rr][0], r1 = ws.q.rec[rr][1];
+                            const int xx = ((bx0 + (int)(r1.w & 31u)) << logB) + (int)(kin & (uint32_t)Bm1);
+                            const int yy = ((by0 + (int)((r1.w >> 5) & 31u)) << logB) + (int)(kin >> logB);
+                            // straight-line: both decodes issue their loads at once (clamped / zero addresses where unused)
+                            const bool own = r0.y != 0xFFFFFFFFu, pred = r0.w != 0u;
+                            const int rx = xx + (int)((r0.w >> 8) & 0xFFu) - S.W, ryy = yy + (int)(r0.w & 0xFFu) - S.W;
+                            const bool inb = pred && (unsigned)rx < (unsigned)S.Ws && (unsigned)ryy < (unsigned)S.Ht;
+                            const int rxc = inb ? rx : 0, ryc = inb ? ryy : 0;
+                            const int b = (ryc >> logB) * S.nbx + (rxc >> logB);
+                            const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                            const uint32_t vown = bise_at_uniform(S.pay + (own ? r0.x : 0u), own ? r0.y + kin : 0u, pc_layout(r0.z), pc_m(r0.z), lut);
+                            const uint32_t bit = 1u << (b & 31);
+                            const bool hasq = inb && (fr.x & bit) != 0u;
+                            const uint32_t ii = ((fr.y + popc(fr.x & (bit - 1u))) << (2 * logB)) + (uint32_t)(((ryc & Bm1) << logB) + (rxc & Bm1));
+                            const uint32_t vref = bise_at_uniform(S.pay + (hasq ? r1.y : 0u), hasq ? ii : 0u, pc_layout(r1.z), pc_m(r1.z), lut);
+                            const int q = hasq ? pc_offset(r1.z) + (int)vref : 0;
+                            // R10: subtractive P = e + R, additive P = e - R
+                            const int e = (own ? pc_offset(r0.z) + (int)vown : 0) + ((r0.w & 0x10000u) ? -q : q);
+                            if (e != 0) {
+                                const int samp = (yy - bt0) * ns + (xx - bs0);
+                                const int c = (int)((r1.w >> 10) & 3u);
+                                const int iu0 = (int)((r1.w >> 12) & 7u), iu1 = (int)((r1.w >> 15) & 7u);
+                                const int iv0 = (int)((r1.w >> 18) & 7u), iv1 = (int)((r1.w >> 21) & 7u);
+                                if (iu0 == iu1 && iv0 == iv1) {  // one view below the plane (always so at level 0)
+                                    atomicAdd(&acc32[(((iv0 * nu + iu0) * nsamp + samp) << 2) + c], e);
+                                } else {
+#pragma unroll 1
+                                    for (int iv = iv0; iv <= iv1; ++iv)
+#pragma unroll 1
+                                        for (int iu = iu0; iu <= iu1; ++iu) atomicAdd(&acc32[(((iv * nu + iu) * nsamp + samp) << 2) + c], e);
                                 }
-                                e += (r0.w & 0x10000u) ? -q : q;  // R10: subtractive P = e + R, additive P = e - R
                             }
-                            const int samp = (yy - bt0) * ns + (xx - bs0);
-                            acc16[(((int)(r1.w & 0xFFFFu) * nsamp + samp) << 2) + (int)(r1.w >> 16)] = (int16_t)e;
                         }
                         __syncwarp();
                     }
                 }
                 {
-                    // -------------------------------------------------------- B4: RKV + per-level terms -> float RGB patch
-                    const uint32_t m_nsamp = magic_of((uint32_t)nsamp), m_ns = magic_of((uint32_t)ns), m_nu = magic_of((uint32_t)nu);
-                    const int ncell = nviews * nsamp;
+                    // -------------------------------------------------------- B4: inverse colour transform, in place -> float RGB
                     for (int q = lane; q < ncell; q += 32) {
-                        const uint32_t vw = fdiv((uint32_t)q, m_nsamp), samp = (uint32_t)q - vw * (uint32_t)nsamp;
-                        const uint32_t iv = fdiv(vw, m_nu), iu = vw - iv * (uint32_t)nu;
-                        const uint32_t it = fdiv(samp, m_ns), is = samp - it * (uint32_t)ns;
-                        const int u = bu0 + (int)iu, v = bv0 + (int)iv, xx = bs0 + (int)is, yy = bt0 + (int)it;
-                        const size_t ri = ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)yy) * (size_t)S.Ws + (size_t)xx;
-                        const short4 rk = ldg(S.rkv + ri);
-                        int a[3] = {rk.x, rk.y, rk.z};
-                        for (int L = 0; L < h; ++L) {
-                            const unsigned long long w = ws.acc[(int)ws.vslot[vw][L] * nsamp + (int)samp];
-                            a[0] += (int)(int16_t)(w & 0xFFFFull);
-                            a[1] += (int)(int16_t)((w >> 16) & 0xFFFFull);
-                            a[2] += (int)(int16_t)((w >> 32) & 0xFFFFull);
-                        }
+                        const int4 w = ws.cell.acc[q];
+                        const int a[3] = {w.x, w.y, w.z};
                         const uint32_t c8 = ycocg_to_rgb8(a);
-                        ws.tp.patch[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
+                        ws.cell.rgb[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
                     }
                     __syncwarp();
 
@@ -434,7 +459,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                                 const int base = (iv * nu + iu) * nsamp + it * ns + is;
                                 const int du = ((pt[p].uv >> 24) & 1u) ? nsamp : 0, dv = ((pt[p].uv >> 25) & 1u) ? nu * nsamp : 0;
                                 const int ds = (int)((pt[p].st >> 28) & 1u), dt = ((pt[p].st >> 29) & 1u) ? ns : 0;
-                                const float4 *patch = ws.tp.patch;
+                                const float4 *patch = ws.cell.rgb;
                                 rgb[p] = blend16(pt[p], [&](int a, int b) {
                                     return patch[base + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0) + ((b & 1) ? ds : 0) + ((b & 2) ? dt : 0)];
                                 });
@@ -485,9 +510,9 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     }
 }
 
-// (pixels per lane, warps per CTA, accumulators, records, tasks, cells, min CTAs per SM)
-using CfgA = Cfg<4, 4, 768, 112, 768, 320, 4>;   // 16 x 8 tiles
-using CfgB = Cfg<2, 4, 384, 64, 512, 176, 8>;    // 8 x 8 tiles
+// (pixels per lane, warps per CTA, records, tasks, cells, min CTAs per SM)
+using CfgA = Cfg<4, 4, 64, 512, 320, 6>;    // 16 x 8 tiles
+using CfgB = Cfg<2, 4, 64, 512, 176, 8>;    // 8 x 8 tiles
 
 template <class C>
 cudaError_t launch_shape(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st)
