@@ -187,7 +187,8 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             uint4 d = ldg(S.pc + base + c);
-            uint4 fr = ldg(S.flagrec + d.x + fg);
+            // the flag record of plane-channel k starts at k * fgroups (= d.x): both loads issue at once
+            uint4 fr = ldg(S.flagrec + (size_t)(base + c) * (size_t)S.fgroups + fg);
             int e = stored_value(S, d, fr, bit, kin);
             if (predictive && (fr.z & bit)) {
                 uint32_t mi = fr.w + popc(fr.z & (bit - 1u));

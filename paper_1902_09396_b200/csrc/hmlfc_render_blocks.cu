@@ -260,7 +260,7 @@ render_blocks_kernel(const DevStream S, const Camera *__restrict__ cams, int W, 
                 const uint4 d = ldg(S.pc + si.x + c);
                 const int bx = cx.bx0 + (int)ib, by = cx.by0 + (int)jb;
                 const int b = by * S.nbx + bx;
-                const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+                const uint4 fr = ldg(S.flagrec + (size_t)(si.x + c) * (size_t)S.fgroups + (size_t)(b >> 5));  // = d.x + ..., without waiting for d
                 const uint32_t bit = 1u << (b & 31);
                 const bool res = (fr.x & bit) != 0u, pred = si.w && (fr.z & bit);
                 keep = res || pred;

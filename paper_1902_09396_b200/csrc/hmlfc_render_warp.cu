@@ -27,8 +27,8 @@
 //   B4  one lane per cell, in place: inverse YCoCg-R, clamp -> float RGB;
 //   C   every pixel gathers its 16 taps from the patch (128-bit loads), blends with packed fp32 FMAs,
 //       and the lane's 4 pixels leave as three 32-bit stores.
-// A tile whose footprint exceeds the workspace is split by rows (8 -> 4 -> 2 -> 1); a single row that
-// still does not fit (strong minification) is rendered by 16 direct sample decodes per pixel.  All
+// A tile whose footprint exceeds the workspace is split by lane ranges (rows 8 -> 4 -> 2 -> 1, half rows, single
+// lanes); a single lane that still does not fit (strong minification) is rendered by 16 direct sample decodes per pixel.  All
 // paths produce identical bytes.
 #include "hmlfc_kernels.cuh"
 
@@ -244,9 +244,11 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
 
     // ---------------------------------------------------------------- row ranges: whole tile first, halved while the footprint does not fit
-    int row0 = 0, span = kTileH;
-    while (row0 < kTileH) {
-        const bool inr = ry >= row0 && ry < row0 + span;
+    // lane ranges: the whole tile (32 lanes) first; a range whose footprint does not fit the workspace is halved
+    // (rows 0-3 | 4-7, row pairs, rows, half rows, single lanes) and the halves are processed one after the other
+    int row0 = 0, span = 32;
+    while (row0 < 32) {
+        const bool inr = lane >= row0 && lane < row0 + span;
         int lo[4] = {0x7fffffff, 0x7fffffff, 0x7fffffff, 0x7fffffff}, hi[4] = {-1, -1, -1, -1};
         if (inr) {
 #pragma unroll
@@ -343,7 +345,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                             const uint4 si = ws.slotinfo[slot];
                             const uint4 d = ldg(S.pc + si.x + c);
                             const int b = (by0 + (int)jb) * S.nbx + bx0 + (int)ib;
-                            const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+                            const uint4 fr = ldg(S.flagrec + (size_t)(si.x + c) * (size_t)S.fgroups + (size_t)(b >> 5));  // = d.x + ..., without waiting for d
                             const uint32_t bit = 1u << (b & 31);
                             const bool res = (fr.x & bit) != 0u, pred = si.z && (fr.z & bit);
                             keep = res || pred;
@@ -479,7 +481,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
             }
         }
         row0 += span;
-        span = row0 & -row0;  // the largest aligned range that starts at row0 (row0 < 8 whenever it is used)
+        span = row0 & -row0;  // the largest aligned range that starts at row0 (row0 < 32 whenever it is used)
     }
 
     // ---------------------------------------------------------------- store: 3 kPPL contiguous bytes per lane
@@ -512,7 +514,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
 
 // (pixels per lane, warps per CTA, records, tasks, cells, min CTAs per SM)
 using CfgA = Cfg<4, 4, 64, 512, 320, 6>;    // 16 x 8 tiles
-using CfgB = Cfg<2, 4, 64, 512, 176, 8>;    // 8 x 8 tiles
+using CfgB = Cfg<2, 4, 64, 512, 256, 7>;    // 8 x 8 tiles
 
 template <class C>
 cudaError_t launch_shape(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st)
