@@ -281,7 +281,7 @@ def run_ours(args, cfg_name):
         dec_kernel_ms = float(np.mean(dec_ms))
         dec_achieved = fpd["bytes_alg"] / (dec_kernel_ms * 1e-3) / 1e9
         roofline = {
-            "bound": "hbm", "kernel": {1: "render_pixel_kernel", 2: "render_tiled_kernel", 3: "render_blocks_kernel"}.get(args.variant, "render_warp_kernel"), "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "bound": "hbm", "kernel": {1: "render_pixel_kernel", 2: "render_tiled_kernel", 3: "render_blocks_kernel", 4: "render_warp_kernel", 5: "render_warp_kernel"}.get(args.variant, "render_cta_kernel"), "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
             "traffic": _traffic_from_profiles("render"), "peak_source": peak_src,
             "bytes_alg_per_launch": fp["bytes_alg"], "out_bytes": fp["out_bytes"],
             "compressed_bytes_touched": fp["bytes_alg"] - fp["out_bytes"] - fp["in_bytes"],
@@ -338,7 +338,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg2")
-    ap.add_argument("--variant", type=int, default=0, help="render kernel: 0 auto, 1 pixel, 2 tiled, 3 blocks, 4 warp (A/B only)")
+    ap.add_argument("--variant", type=int, default=0, help="render kernel: 0 auto (= 6 cta), 1 pixel, 2 tiled, 3 blocks, 4/5 warp (A/B only)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -125,13 +125,11 @@ int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n
                            hmlfc_footprint_t *out);
 int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out);
 
-/* Kernel selection for hmlfc_render: 0 = automatic (default; currently 4), 1 = one thread per
- * output pixel (16 independent tap decodes), 2 = sample-shared tile (a CTA decodes every LF sample
- * of its tile's footprint once into shared memory), 3 = block-centric tile (per tile: classify the
- * footprint's blocks, decode motion records once per block, evaluate only non-empty blocks on full
- * warps, share level >= 1 planes between the tile's views), 4 = the same block-centric pipeline run by
- * ONE WARP per 16x8 tile out of a private shared-memory workspace (no CTA barriers).  All variants
- * produce identical bytes. */
+/* Kernel selection for hmlfc_render (A/B measurements and cross-checks; all variants produce identical
+ * bytes): 0 = automatic (default: 6 for B = 4 streams, else 4), 1 = one thread per output pixel (16
+ * independent tap decodes), 2 = sample-shared tile, 3 = block-centric CTA tile (32 x 8), 4 / 5 = the
+ * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile, 6 = CTA per 32 x 32 tile with
+ * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows). */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Number of kernels this library has launched through the handle since load (bench accounting). */

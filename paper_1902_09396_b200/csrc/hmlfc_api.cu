@@ -111,14 +111,14 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
     if ((ce = cudaGetDevice(&h->device)) != cudaSuccess ||
         (ce = upload(&h->d_pc, T.pc.data(), T.pc.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
         (ce = upload(&h->d_flagrec, T.flagrec.data(), T.flagrec.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
-        (ce = upload(&h->d_pay, s + T.off_pay, (size_t)(T.off_mv - T.off_pay), 16, &dev_bytes)) != cudaSuccess ||
-        (ce = upload(&h->d_mv, s + T.off_mv, (size_t)(T.total - T.off_mv), 16, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_pay, s + T.off_pay, (size_t)(T.off_mv - T.off_pay), 64, &dev_bytes)) != cudaSuccess ||
+        (ce = upload(&h->d_mv, s + T.off_mv, (size_t)(T.total - T.off_mv), 64, &dev_bytes)) != cudaSuccess ||
         (ce = upload(&h->d_rkv, T.rkv.data(), T.rkv.size() * sizeof(short4), 0, &dev_bytes)) != cudaSuccess ||
         (ce = upload(&h->d_bits15, T.bits15.data(), T.bits15.size() * sizeof(uint32_t), 0, &dev_bytes)) != cudaSuccess ||
         (ce = cudaMalloc(reinterpret_cast<void **>(&h->d_oob), sizeof(unsigned long long))) != cudaSuccess ||
         (ce = cudaMemset(h->d_oob, 0, sizeof(unsigned long long))) != cudaSuccess ||
         (ce = cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking)) != cudaSuccess ||
-        (ce = configure_render_blocks()) != cudaSuccess || (ce = configure_render_warp()) != cudaSuccess) {
+        (ce = configure_render_blocks()) != cudaSuccess || (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
@@ -160,8 +160,10 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
         CU(h, launch_render_tiled(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 3)
         CU(h, launch_render_blocks(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else
+    else if (h->render_variant == 4 || h->render_variant == 5 || h->ds.B != 4)
         CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 5 ? 1 : 0));
+    else  // 0 (default) and 6: block-row kernel, written for 4 x 4 blocks
+        CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -264,7 +266,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 5) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 6) return HMLFC_E_INVALID;
     h->render_variant = variant;
     return HMLFC_OK;
 }

@@ -29,6 +29,10 @@ cudaError_t configure_render_blocks();
 cudaError_t launch_render_warp(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
                                int *n_launches, int shape);
 cudaError_t configure_render_warp();
+// CTA per 32 x 32 tile, block-row tasks (B = 4 streams only; returns cudaErrorInvalidValue otherwise)
+cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
+                              int *n_launches);
+cudaError_t configure_render_cta();
 cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,
                                     FootprintMarks marks, cudaStream_t st);
 cudaError_t launch_footprint_decode(const DevStream &S, const int32_t *d_coords, int64_t n, FootprintMarks marks,

@@ -94,7 +94,7 @@ def test_decode_host_entry_point(P, enc):
 def _check_views(P, h, s, cams, W, H):
     expect = s.render(cams, W, H)
     outs = {}
-    for variant in (P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8):
+    for variant in (P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA):
         P.hmlfc_set_render_variant(h, variant)
         got = P.hmlfc_render(h, _dev(cams), W, H).cpu().numpy()
         d = np.abs(got.astype(np.int16) - expect.astype(np.int16))
@@ -106,6 +106,7 @@ def _check_views(P, h, s, cams, W, H):
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_BLOCKS])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP8])
+    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA])
     return expect
 
 
