@@ -39,6 +39,8 @@ constexpr int kPPL = 4;           // consecutive pixels per thread
 constexpr int kMaxV = 4;          // views per axis of one tile's footprint
 constexpr int kMaxViews = kMaxV * kMaxV;
 constexpr int kMaxSlots = 52;     // 16 + 9 + 4 * 6 planes + slack
+constexpr int kMaxChunks = 256;   // 32-cell chunks of the patch
+constexpr int kSpecZero = 1536;   // 16-byte words of the accumulator region zeroed while warp 0 builds the tables
 constexpr int kMinRec = 64;       // smallest record capacity worth starting with
 constexpr uint32_t FULL = 0xffffffffu;
 constexpr uint32_t kNone = 0xFFFFFFFFu;
@@ -72,7 +74,7 @@ __device__ __forceinline__ uint32_t fdiv(uint32_t n, uint32_t m) { return m ? __
 
 struct ViewInfo {   // one view of the tile's (u,v) neighbourhood
     int s0, t0, ns, nt;          // footprint box of the view (ns == 0: no pixel of the tile touches it)
-    int cellbase;                // first (view, sample) cell
+    int cellbase;                // first (view, sample) cell (a multiple of 32: a warp's cells belong to one view)
     uint32_t m_ns;               // magic multiplier of ns
     uint32_t rkv_lo, rkv_hi;     // index of the view's top-level RKV plane * Ht * Ws
 };
@@ -91,6 +93,8 @@ struct Ctl {
     ViewInfo view[kMaxViews];
     SlotInfo slot[kMaxSlots + 1];
     int2 voff[kMaxViews][kMaxLevels];    // accumulator offset / row stride of the view's plane at level L
+    int2 vcb[kMaxViews];                 // {cellbase - t0 * ns - s0, ns}: cell of sample (s,t) = x + t * y + s
+    uint8_t chunkvw[kMaxChunks];         // view of the 32-cell chunk
     int lvl_base[kMaxLevels], lvl_pu0[kMaxLevels], lvl_pv0[kMaxLevels], lvl_nu[kMaxLevels];
     int nviews, nslots, ncell, nacc, nitems, reccap, fits;
     int n_rec, overflow;
@@ -313,19 +317,8 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
         if (!done && nu <= kMaxV && nv <= kMaxV) {
             // -------------------------------------------------------- V: footprint box per view
             // lanes with one common key first (the usual case: one or two rounds per warp), then pixel by pixel
-#pragma unroll 1
-            for (int round = 0; round < 1 + kPPL; ++round) {
-                uint32_t k;
-                int a0, a1, a2, a3;
-                if (round == 0) { k = mixed ? kNone : key; a0 = ls0; a1 = lt0; a2 = ls1; a3 = lt1; }
-                else {
-                    const int p = round - 1;
-                    k = (mixed && inr) ? pt[p].uv : kNone;
-                    const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
-                    a0 = s0; a1 = t0; a2 = s0 + (int)((pt[p].st >> 28) & 1u); a3 = t0 + (int)((pt[p].st >> 29) & 1u);
-                }
+            auto merge_boxes = [&](uint32_t k, int a0, int a1, int a2, int a3) {
                 uint32_t todo = __ballot_sync(FULL, k != kNone);
-                if (round > 0 && todo == 0u) continue;
                 while (todo) {
                     const int leader = __ffs(todo) - 1;
                     const uint32_t kk = __shfl_sync(FULL, k, leader);
@@ -343,6 +336,14 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                     }
                     todo &= ~__ballot_sync(FULL, mine);
                 }
+            };
+            merge_boxes(mixed ? kNone : key, ls0, lt0, ls1, lt1);
+            if (__any_sync(FULL, mixed)) {
+#pragma unroll
+                for (int p = 0; p < kPPL; ++p) {
+                    const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
+                    merge_boxes((mixed && inr) ? pt[p].uv : kNone, s0, t0, s0 + (int)((pt[p].st >> 28) & 1u), t0 + (int)((pt[p].st >> 29) & 1u));
+                }
             }
             __syncthreads();
 
@@ -354,17 +355,20 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                     vs0 = ctl.vbox[lane][0]; vt0 = ctl.vbox[lane][1];
                     vns = ctl.vbox[lane][2] - vs0 + 1; vnt = ctl.vbox[lane][3] - vt0 + 1;
                 }
-                int incl = vns * vnt;
+                const int vcells = (vns * vnt + 31) & ~31;  // whole warps per view
+                int incl = vcells;
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
+                for (int o = 1; o < kMaxViews; o <<= 1) {
                     const int n = __shfl_up_sync(FULL, incl, o);
                     if (lane >= o) incl += n;
                 }
-                const int ncell = __shfl_sync(FULL, incl, 31);
+                const int ncell = __shfl_sync(FULL, incl, kMaxViews - 1);
                 if (lane < kMaxViews) {
                     ViewInfo vi;
                     vi.s0 = vs0; vi.t0 = vt0; vi.ns = vns; vi.nt = vnt;
-                    vi.cellbase = incl - vns * vnt;
+                    vi.cellbase = incl - vcells;
+                    ctl.vcb[lane] = make_int2(vi.cellbase - vt0 * vns - vs0, vns);
+                    for (int c = vi.cellbase >> 5; c < min(incl >> 5, kMaxChunks); ++c) ctl.chunkvw[c] = (uint8_t)lane;
                     vi.m_ns = magic_of((uint32_t)vns);
                     const int iv = lane / nu, iu = lane - iv * nu;
                     const unsigned long long ro = (unsigned long long)(((bv0 + iv) >> h) * S.UH + ((bu0 + iu) >> h)) *
@@ -442,12 +446,17 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                     // accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by the record list (32 bytes each)
                     const long long accbytes = ((long long)accrun * 8 + 15) & ~15LL;
                     const long long rest = (long long)ARENA_BYTES - accbytes;
-                    const bool fits = nslots <= kMaxSlots && rest >= (long long)ncell * 16 && rest >= (long long)kMinRec * 32;
+                    const bool fits = nslots <= kMaxSlots && ncell <= 32 * kMaxChunks && rest >= (long long)ncell * 16 && rest >= (long long)kMinRec * 32;
                     ctl.nviews = nviews; ctl.nslots = nslots; ctl.ncell = ncell; ctl.nacc = accrun; ctl.nitems = itemrun;
                     ctl.reccap = fits ? (int)min(rest / 32, 65535LL) : 0;
                     ctl.fits = fits ? 1 : 0;
                     if (nslots <= kMaxSlots) ctl.slot[nslots].itembase = itemrun;  // sentinel of the item -> slot search
                 }
+            }
+            else {
+                // meanwhile the other warps zero the head of the accumulator region (its size is not known yet)
+                uint4 *z = reinterpret_cast<uint4 *>(arena);
+                for (int q = tid - 32; q < kSpecZero; q += kNT - 32) z[q] = make_uint4(0u, 0u, 0u, 0u);
             }
             __syncthreads();
 
@@ -461,7 +470,7 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                 {
                     uint4 *z = reinterpret_cast<uint4 *>(arena);
                     const int nz = (nacc + 1) >> 1;
-                    for (int q = tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);
+                    for (int q = kSpecZero + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);  // the rest (warps 1..7 zeroed the head during T)
                     for (int q = tid; q < nviews * h; q += kNT) {
                         const int vw = q / h, L = q - vw * h;
                         const int iv = vw / nu, iu = vw - iv * nu;
@@ -612,13 +621,13 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                     __syncthreads();
                     // ------------------------------------------------ B4: top-level RKV + per-level terms -> float RGB patch
                     for (int q = tid; q < ncell; q += kNT) {
-                        int vw = 0;
-                        for (int k2 = 1; k2 < nviews; ++k2) vw += (q >= ctl.view[k2].cellbase) ? 1 : 0;
+                        const int vw = ctl.chunkvw[q >> 5];
                         const ViewInfo vi = ctl.view[vw];
                         const uint32_t local = (uint32_t)(q - vi.cellbase);
                         const uint32_t it = fdiv(local, vi.m_ns), is = local - it * (uint32_t)vi.ns;
+                        if ((int)it >= vi.nt) continue;  // padding of the view's last chunk
                         const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
-                        const short4 rk = ldg(S.rkv + ro + (unsigned long long)(vi.t0 + (int)it) * (unsigned long long)S.Ws + (unsigned long long)(vi.s0 + (int)is));
+                        const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
                         int a[3] = {rk.x, rk.y, rk.z};
                         for (int L = 0; L < h; ++L) {
                             const int2 vo = ctl.voff[vw][L];
@@ -645,9 +654,9 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                                 int vb[4], vs[4];
 #pragma unroll
                                 for (int a = 0; a < 4; ++a) {
-                                    const ViewInfo &vi = ctl.view[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
-                                    vb[a] = vi.cellbase + (t0 - vi.t0) * vi.ns + (s0 - vi.s0);
-                                    vs[a] = dt ? vi.ns : 0;
+                                    const int2 cb = ctl.vcb[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
+                                    vb[a] = cb.x + t0 * cb.y + s0;
+                                    vs[a] = dt ? cb.y : 0;
                                 }
                                 rgb[p] = blend16(pt[p], [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
                             }
@@ -689,8 +698,8 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
     }
 }
 
-constexpr int kArenaBytes = 68 * 1024;
-constexpr int kMinBlocks = 3;
+constexpr int kArenaBytes = 50 * 1024;
+constexpr int kMinBlocks = 4;
 
 }  // namespace
 
