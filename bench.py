@@ -47,7 +47,7 @@ class ClockSampler:
     REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4),
                ("hw_power_brake", 0x80), ("applications_clocks", 0x2))
 
-    def __init__(self, index, period=0.05):
+    def __init__(self, index, period=0.002):
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
@@ -201,6 +201,8 @@ def run_ours(args, cfg_name):
     h = P.hmlfc_load(data)
     if args.variant:
         P.hmlfc_set_render_variant(h, args.variant)
+    if args.decode_variant:
+        P.hmlfc_set_decode_variant(h, args.decode_variant)
     W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
     # weak scaling: every rank renders a full batch, each on its own arc of the camera circle
     cams_np = wl.camera_path(cfg, seed_offset=rank)
@@ -289,7 +291,7 @@ def run_ours(args, cfg_name):
         }
         decode = {
             "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
-            "roofline": {"bound": "hbm", "kernel": "decode_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": "decode_kernel" if args.decode_variant == 1 else "decode_queue_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
                          "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
                          "traffic": _traffic_from_profiles("decode")},
         }
@@ -339,6 +341,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg2")
     ap.add_argument("--variant", type=int, default=0, help="render kernel: 0 auto (= 6 cta), 1 pixel, 2 tiled, 3 blocks, 4/5 warp (A/B only)")
+    ap.add_argument("--decode-variant", type=int, default=0, help="decode kernel: 0 auto (= 2 warp-cooperative), 1 thread per coordinate")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

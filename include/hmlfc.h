@@ -132,6 +132,11 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
  * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows). */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
+/* Kernel selection for hmlfc_decode (identical bytes): 0 = automatic (default: 2), 1 = one thread per
+ * coordinate walks the tree on its own, 2 = warp-cooperative (each lane classifies its coordinate, the
+ * motion-record and BISE value decodes run as 32-wide batches from per-warp task stacks). */
+int hmlfc_set_decode_variant(hmlfc_handle *h, int variant);
+
 /* Number of kernels this library has launched through the handle since load (bench accounting). */
 int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);
 

@@ -15,11 +15,12 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
 RENDER_AUTO, RENDER_PIXEL, RENDER_TILED, RENDER_BLOCKS, RENDER_WARP, RENDER_WARP8, RENDER_CTA = 0, 1, 2, 3, 4, 5, 6
+DECODE_AUTO, DECODE_THREAD, DECODE_QUEUE = 0, 1, 2
 
 
 class HmlfcError(RuntimeError):
@@ -75,6 +76,7 @@ def lib():
     L.hmlfc_footprint_render.restype = C.c_int
     L.hmlfc_footprint_decode.argtypes, L.hmlfc_footprint_decode.restype = [vp, vp, i64, C.POINTER(Footprint)], C.c_int
     L.hmlfc_set_render_variant.argtypes, L.hmlfc_set_render_variant.restype = [vp, C.c_int], C.c_int
+    L.hmlfc_set_decode_variant.argtypes, L.hmlfc_set_decode_variant.restype = [vp, C.c_int], C.c_int
     L.hmlfc_launch_count.argtypes, L.hmlfc_launch_count.restype = [vp, C.POINTER(i64)], C.c_int
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
@@ -214,6 +216,10 @@ def hmlfc_footprint_decode(h: Handle, coords) -> dict:
 
 def hmlfc_set_render_variant(h: Handle, variant: int):
     _check(lib().hmlfc_set_render_variant(h._h, variant), "hmlfc_set_render_variant")
+
+
+def hmlfc_set_decode_variant(h: Handle, variant: int):
+    _check(lib().hmlfc_set_decode_variant(h._h, variant), "hmlfc_set_decode_variant")
 
 
 def hmlfc_launch_count(h: Handle) -> int:

@@ -34,6 +34,7 @@ struct hmlfc_handle {
     size_t d_out_cap = 0;
     cudaStream_t host_stream = nullptr;
     int render_variant = 0;
+    int decode_variant = 0;
     mutable std::atomic<long long> launches{0};
     mutable std::atomic<int> last_cuda_error{0};
 };
@@ -141,7 +142,10 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
 {
     if (!h || n < 0 || (n > 0 && (!d_coords || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    if (h->decode_variant == 1)
+        CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    else
+        CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -268,6 +272,13 @@ int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
     if (!h || variant < 0 || variant > 6) return HMLFC_E_INVALID;
     h->render_variant = variant;
+    return HMLFC_OK;
+}
+
+int hmlfc_set_decode_variant(hmlfc_handle *h, int variant)
+{
+    if (!h || variant < 0 || variant > 2) return HMLFC_E_INVALID;
+    h->decode_variant = variant;
     return HMLFC_OK;
 }
 

@@ -1,0 +1,247 @@
+// hmlfc_decode, warp-cooperative form (sm_100a): the tree walk of 32 random coordinates regrouped into
+// uniform batches of work.
+//
+// What is computed is exactly DESIGN.md section 3: per coordinate and channel
+//   acc = topRKV + sum_L [ stored_p(s,t)  (+|-)  stored_r(s+dx, t+dy) ].
+// For uniformly random coordinates every test of that walk (block significant? block predicted? reference
+// block significant?) is taken by a different subset of the lanes, so a thread-per-coordinate kernel runs
+// with ~8 of 32 lanes active (profiles/r01_cta_cfg2.md).  Here each lane still classifies ITS coordinate
+// (flag record + descriptor of every (level, channel): uniform control flow), but the two expensive steps
+// become tasks on two small per-warp stacks in shared memory:
+//   motion task  {MV word base, record index, reference plane-channel, destination}   -> S6 + S7 address part
+//   value task   {payload word base, value index, offset|layout|m|sign|destination}   -> S5 (BISE decode_at)
+// and are executed 32 at a time by all lanes (the stacks are drained whenever they hold >= 32 tasks, so only
+// the last batch of a warp is partial).  Values are accumulated with shared-memory atomics into the
+// destination's (Y, Co, Cg) cell; the owning lane finishes with the inverse colour transform and the staged
+// 96-byte store.  Integer arithmetic only: bit-exact by construction against the per-thread kernel and the oracle.
+#include "hmlfc_kernels.cuh"
+
+namespace hmlfc {
+
+namespace {
+
+constexpr int kThreads = 256, kWarps = kThreads / 32;
+constexpr int kCap = 64;  // per stack: < 32 left over + <= 32 pushed per round
+
+struct DigitLut {
+    uint16_t v[384];
+};
+
+// digits of the packed trit / quint words: T -> t0 | t1<<2 | .. | t4<<8, Q -> q0 | q1<<3 | q2<<6
+constexpr DigitLut make_digit_lut()
+{
+    DigitLut l{};
+    for (int T = 0; T < 256; ++T) {
+        int x = T, p = 0;
+        for (int k = 0; k < 5; ++k) { p |= (x % 3) << (2 * k); x /= 3; }
+        l.v[T] = (uint16_t)p;
+    }
+    for (int Q = 0; Q < 128; ++Q) {
+        int x = Q, p = 0;
+        for (int k = 0; k < 3; ++k) { p |= (x % 5) << (3 * k); x /= 5; }
+        l.v[256 + Q] = (uint16_t)p;
+    }
+    return l;
+}
+
+__device__ const DigitLut g_dq_digit_lut = make_digit_lut();
+
+struct WarpQ {
+    uint4 vq[kCap];      // value tasks
+    uint4 mq[kCap];      // motion tasks
+    int acc[32 * 4];     // {Y, Co, Cg, -} per coordinate of the warp
+    uint32_t xy[32];     // s | t << 16 of the warp's coordinates
+    uint32_t stage[24];  // the warp's 96 output bytes
+};
+
+// bits [pos, pos+n) of an LSB-first 32-bit word string, n <= 16
+__device__ __forceinline__ uint32_t bits_at(const uint32_t *__restrict__ w, uint32_t pos, uint32_t n)
+{
+    const uint32_t *p = w + (pos >> 5);
+    return __funnelshift_r(__ldg(p), __ldg(p + 1), pos & 31u) & ((1u << n) - 1u);
+}
+
+// BISE decode_at (bit layout in DESIGN.md section 4) without control flow: plain = groups of one
+// value with an empty digit word, so lanes holding tasks of different layouts do not serialise.
+__device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint32_t i, uint32_t layout, uint32_t m,
+                                            const uint16_t *__restrict__ lut)
+{
+    const bool plain = layout == 0u, trit = layout == 1u;
+    const uint32_t G = plain ? 1u : (trit ? 5u : 3u), hb = plain ? 0u : (trit ? 8u : 7u);
+    const uint32_t g = plain ? i : (trit ? (__umulhi(i, 0xCCCCCCCDu) >> 2) : (__umulhi(i, 0xAAAAAAABu) >> 1));
+    const uint32_t k = i - G * g;
+    const uint32_t gb = g * (hb + G * m);
+    const uint32_t head = bits_at(w, gb, hb);  // plain: 0 bits -> 0, and the quint table maps 0 to digit 0
+    const uint32_t low = bits_at(w, gb + hb + k * m, m);
+    const uint32_t dig = ((uint32_t)lut[(trit ? 0u : 256u) + head] >> (k * (trit ? 2u : 3u))) & (trit ? 3u : 7u);
+    return (dig << m) | low;
+}
+
+constexpr uint32_t kSignBit = 1u << 23;  // value task: subtract (additive / "phase-shifted" mode, R10)
+
+// push one task per flagged lane on a warp stack; cnt is warp-uniform
+__device__ __forceinline__ void push(uint4 *stack, int &cnt, bool flag, uint4 task, uint32_t lane_lt)
+{
+    const uint32_t m = __ballot_sync(0xffffffffu, flag);
+    if (flag) stack[cnt + __popc(m & lane_lt)] = task;
+    cnt += __popc(m);
+}
+
+// execute the top n (<= 32) value tasks: S5 of the path
+__device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+{
+    __syncwarp();
+    if (lane < n) {
+        const uint4 t = q.vq[vcnt - n + lane];
+        int val = pc_offset(t.z) + (int)bise_at(S.pay + t.x, t.y, pc_layout(t.z), pc_m(t.z), lut);
+        if (t.z & kSignBit) val = -val;
+        atomicAdd(&q.acc[t.z >> 24], val);
+    }
+    vcnt -= n;
+    __syncwarp();
+}
+
+// execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
+// the reference block is significant, push its value task
+__device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
+                                             uint32_t lane_lt, const uint16_t *lut)
+{
+    __syncwarp();
+    bool has = false;
+    uint4 vt = make_uint4(0u, 0u, 0u, 0u);
+    if (lane < n) {
+        const uint4 t = q.mq[mcnt - n + lane];
+        const uint32_t rec = bise_at(S.mv + t.x, t.y, S.mv_layout, S.mv_m, lut);
+        int mode, dx, dy;
+        mv_unpack(S, rec, mode, dx, dy);
+        const uint32_t xy = q.xy[t.w >> 2];
+        const int rx = (int)(xy & 0xFFFFu) + dx, ry = (int)(xy >> 16) + dy;
+        if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {  // R8: outside the image reads 0
+            const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+            const uint4 rd = ldg(S.pc + t.z);
+            const uint4 fr = ldg(S.flagrec + (size_t)t.z * (size_t)S.fgroups + (size_t)(b >> 5));
+            const uint32_t bit = 1u << (b & 31);
+            has = (fr.x & bit) != 0u;
+            const uint32_t rank = fr.y + (uint32_t)__popc(fr.x & (bit - 1u));
+            const uint32_t kin = (uint32_t)(((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1)));
+            vt = make_uint4(rd.y, (rank << (2 * S.logB)) + kin, (rd.w & 0x3FFFFFu) | (mode ? kSignBit : 0u) | (t.w << 24), 0u);
+        }
+    }
+    mcnt -= n;
+    __syncwarp();
+    push(q.vq, vcnt, has, vt, lane_lt);
+}
+
+__global__ void __launch_bounds__(kThreads)
+decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
+                    unsigned long long *oob, int out_aligned)
+{
+    __shared__ WarpQ wq[kWarps];
+    __shared__ uint16_t lut[384];
+    for (int k = threadIdx.x; k < 384; k += kThreads) lut[k] = g_dq_digit_lut.v[k];
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const uint32_t lane_lt = (1u << lane) - 1u;
+    WarpQ &q = wq[threadIdx.x >> 5];
+    const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const bool present = i < n;
+    int4 c4 = make_int4(0, 0, 0, 0);
+    if (present) c4 = __ldg(coords + i);
+    const bool valid = present && (unsigned)c4.x < (unsigned)S.U && (unsigned)c4.y < (unsigned)S.V &&
+                       (unsigned)c4.z < (unsigned)S.Ws && (unsigned)c4.w < (unsigned)S.Ht;
+    if (present && !valid) atomicAdd(oob, 1ull);
+    const int u = c4.x, v = c4.y, x = c4.z, y = c4.w;
+    const int h = S.h;
+
+    // S3 root term: one 64-bit load; the cell starts at the top-level RKV sample
+    short4 root = make_short4(0, 0, 0, 0);
+    if (valid) root = ldg(S.rkv + ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)y) * (size_t)S.Ws + (size_t)x);
+    q.acc[lane * 4 + 0] = root.x;
+    q.acc[lane * 4 + 1] = root.y;
+    q.acc[lane * 4 + 2] = root.z;
+    q.xy[lane] = (uint32_t)x | ((uint32_t)y << 16);
+
+    const int b = valid ? (y >> S.logB) * S.nbx + (x >> S.logB) : 0;
+    const uint32_t bit = 1u << (b & 31);
+    const size_t fg = (size_t)(b >> 5);
+    const uint32_t kin = (uint32_t)(((y & (S.B - 1)) << S.logB) + (x & (S.B - 1)));
+    int vcnt = 0, mcnt = 0;
+
+#pragma unroll 1
+    for (int L = 0; L < h; ++L) {
+        const int pu = u >> L, pv = v >> L;
+        const LevelDesc lv = S.lev[L];
+        const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
+        const uint32_t rbase = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
+        const bool predictive = ((pu | pv) & 1) != 0;
+        // S4: the three channels' descriptors and flag records, six independent loads
+        uint4 d[3], fr[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            d[c] = fr[c] = make_uint4(0u, 0u, 0u, 0u);
+            if (valid) {
+                d[c] = ldg(S.pc + base + c);
+                fr[c] = ldg(S.flagrec + (size_t)(base + c) * (size_t)S.fgroups + fg);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const uint32_t dest = (uint32_t)(lane * 4 + c);
+            const bool res = (fr[c].x & bit) != 0u;
+            const uint32_t rank = fr[c].y + (uint32_t)__popc(fr[c].x & (bit - 1u));
+            push(q.vq, vcnt, res, make_uint4(d[c].y, (rank << (2 * S.logB)) + kin, (d[c].w & 0x3FFFFFu) | (dest << 24), 0u), lane_lt);
+            if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
+            const bool pred = predictive && (fr[c].z & bit) != 0u;
+            const uint32_t mi = fr[c].w + (uint32_t)__popc(fr[c].z & (bit - 1u));
+            push(q.mq, mcnt, pred, make_uint4(d[c].z, mi, rbase + (uint32_t)c, dest), lane_lt);
+            if (mcnt >= 32) {
+                drain_motion(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
+            }
+        }
+    }
+    if (mcnt > 0) drain_motion(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
+    if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
+    if (vcnt > 0) drain_values(S, q, vcnt, vcnt, lane, lut);
+    __syncwarp();
+
+    // S8: inverse YCoCg-R + clamp, then the warp's 96 bytes as 24 coalesced words
+    uint32_t rgb = 0u;
+    if (valid) {
+        const int acc[3] = {q.acc[lane * 4 + 0], q.acc[lane * 4 + 1], q.acc[lane * 4 + 2]};
+        rgb = ycocg_to_rgb8(acc);
+    }
+    const long long wbase = i - lane;
+    uint8_t *o = out + 3 * wbase;
+    if (out_aligned && wbase + 32 <= n) {
+        uint8_t *sb = reinterpret_cast<uint8_t *>(q.stage);
+        sb[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
+        sb[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
+        sb[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
+        __syncwarp();
+        if (lane < 24) reinterpret_cast<uint32_t *>(o)[lane] = q.stage[lane];
+    } else if (present) {
+        o[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
+        o[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
+        o[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches)
+{
+    if (n == 0) return cudaSuccess;
+    if (S.Ws > 65536 || S.Ht > 65536) return cudaErrorInvalidValue;  // s | t << 16 packing
+    const long long blocks = (n + kThreads - 1) / kThreads;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
+    decode_queue_kernel<<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
+                                                                d_oob, aligned);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace hmlfc
