@@ -224,488 +224,569 @@ __device__ __forceinline__ uint2 bise_row4(const uint32_t *__restrict__ w, uint3
     return make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
 }
 
-template <int ARENA_BYTES, int MINB>
-__global__ void __launch_bounds__(kNT, MINB)
-render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned)
+constexpr int kArenaBytes = 50 * 1024;
+constexpr int kMinBlocks = 4;
+#ifndef HMLFC_EST_SLACK
+#define HMLFC_EST_SLACK 120
+#endif
+constexpr int kEstSlackPct = HMLFC_EST_SLACK;  // the 32 x 32 pass is tried when the estimate is below this share of the arena
+
+// ---------------------------------------------------------------------------------------------------------------
+// Phases T, B1-B4 for the sub-tile whose (u,v) range (ctl.lo / ctl.hi) and per-view footprint boxes (ctl.vbox) are
+// set: builds the tables and, if they fit the arena, the float RGB patch of every (view, sample) cell.  Returns
+// false (CTA-uniform) when the sub-tile does not fit; the caller then splits it.  Called by all 256 threads.
+#ifndef HMLFC_BP_ATTR
+#define HMLFC_BP_ATTR __forceinline__
+#endif
+__device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena)
 {
-    extern __shared__ __align__(16) unsigned char arena[];
-    __shared__ Ctl ctl;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int lx = tid & 7, ly = tid >> 3;
-    const int x0 = blockIdx.x * kTile + lx * kPPL, y = blockIdx.y * kTile + ly;
-    const int view = blockIdx.z;
     const int h = S.h;
+    const int bu0 = ctl.lo[0], bv0 = ctl.lo[1];
+    const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
 
-    for (int q = tid; q < 192; q += kNT)
-        reinterpret_cast<uint32_t *>(ctl.lut)[q] = reinterpret_cast<const uint32_t *>(g_cta_digit_lut.v)[q];
+    // -------------------------------------------------------- T: tables (warp 0)
+    if (warp == 0) {
+        const int nviews = nu * nv;
+        int vs0 = 0, vt0 = 0, vns = 0, vnt = 0;
+        if (lane < nviews && ctl.vbox[lane][2] >= 0) {
+            vs0 = ctl.vbox[lane][0]; vt0 = ctl.vbox[lane][1];
+            vns = ctl.vbox[lane][2] - vs0 + 1; vnt = ctl.vbox[lane][3] - vt0 + 1;
+        }
+        const int vcells = (vns * vnt + 31) & ~31;  // whole warps per view
+        int incl = vcells;
+#pragma unroll
+        for (int o = 1; o < kMaxViews; o <<= 1) {
+            const int n = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += n;
+        }
+        const int ncell = __shfl_sync(FULL, incl, kMaxViews - 1);
+        if (lane < kMaxViews) {
+            ViewInfo vi;
+            vi.s0 = vs0; vi.t0 = vt0; vi.ns = vns; vi.nt = vnt;
+            vi.cellbase = incl - vcells;
+            ctl.vcb[lane] = make_int2(vi.cellbase - vt0 * vns - vs0, vns);
+            for (int c = vi.cellbase >> 5; c < min(incl >> 5, kMaxChunks); ++c) ctl.chunkvw[c] = (uint8_t)lane;
+            vi.m_ns = magic_of((uint32_t)vns);
+            const int iv = lane / nu, iu = lane - iv * nu;
+            const unsigned long long ro = (unsigned long long)(((bv0 + iv) >> h) * S.UH + ((bu0 + iu) >> h)) *
+                                          (unsigned long long)S.Ht * (unsigned long long)S.Ws;
+            vi.rkv_lo = (uint32_t)ro; vi.rkv_hi = (uint32_t)(ro >> 32);
+            ctl.view[lane] = vi;
+        }
+        // per level the rectangle of planes over the views; lane L owns level L
+        int pu0 = 0, pv0 = 0, nuL = 0, cntL = 0;
+        if (lane < h) {
+            pu0 = bu0 >> lane; pv0 = bv0 >> lane;
+            nuL = ((bu0 + nu - 1) >> lane) - pu0 + 1;
+            cntL = nuL * (((bv0 + nv - 1) >> lane) - pv0 + 1);
+        }
+        int lincl = cntL;
+#pragma unroll
+        for (int o = 1; o < kMaxLevels; o <<= 1) {
+            const int n = __shfl_up_sync(FULL, lincl, o);
+            if (lane >= o) lincl += n;
+        }
+        const int nslots = __shfl_sync(FULL, lincl, h - 1);
+        if (lane < h) { ctl.lvl_base[lane] = lincl - cntL; ctl.lvl_pu0[lane] = pu0; ctl.lvl_pv0[lane] = pv0; ctl.lvl_nu[lane] = nuL; }
+        __syncwarp();
+        int accrun = 0, itemrun = 0;
+        if (nslots <= kMaxSlots) {
+            for (int sb = 0; sb < nslots; sb += 32) {
+                const int s = sb + lane;
+                SlotInfo si;
+                si.pc0 = si.refpc0 = 0u; si.pred = 0u;
+                si.s0 = si.t0 = 0; si.ns = 0; si.s1 = si.t1 = -1; si.bx0 = si.by0 = 0; si.nbw = 0; si.nbh = 0;
+                int nsamp = 0;
+                if (s < nslots) {
+                    int L = 0;
+                    while (L + 1 < h && s >= ctl.lvl_base[L + 1]) ++L;
+                    const int jj = s - ctl.lvl_base[L], n = ctl.lvl_nu[L];
+                    const int jv = jj / n;
+                    const int pv = ctl.lvl_pv0[L] + jv, pu = ctl.lvl_pu0[L] + (jj - jv * n);
+                    const LevelDesc lv = S.lev[L];
+                    si.pc0 = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
+                    si.refpc0 = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
+                    si.pred = (uint32_t)((pu | pv) & 1);
+                    // union of the boxes of the views below this plane
+                    const int iu0 = max(pu << L, bu0) - bu0, iu1 = min(((pu + 1) << L) - 1, bu0 + nu - 1) - bu0;
+                    const int iv0 = max(pv << L, bv0) - bv0, iv1 = min(((pv + 1) << L) - 1, bv0 + nv - 1) - bv0;
+                    int a0 = 0x7fffffff, a1 = 0x7fffffff, a2 = -1, a3 = -1;
+                    for (int iv = iv0; iv <= iv1; ++iv)
+                        for (int iu = iu0; iu <= iu1; ++iu) {
+                            const int vw = iv * nu + iu;
+                            if (ctl.vbox[vw][2] >= 0) {
+                                a0 = min(a0, ctl.vbox[vw][0]); a1 = min(a1, ctl.vbox[vw][1]);
+                                a2 = max(a2, ctl.vbox[vw][2]); a3 = max(a3, ctl.vbox[vw][3]);
+                            }
+                        }
+                    if (a2 >= 0) {
+                        si.s0 = a0; si.t0 = a1; si.s1 = a2; si.t1 = a3; si.ns = a2 - a0 + 1;
+                        si.bx0 = a0 >> 2; si.by0 = a1 >> 2;
+                        si.nbw = (a2 >> 2) - si.bx0 + 1; si.nbh = (a3 >> 2) - si.by0 + 1;
+                        nsamp = si.ns * (a3 - a1 + 1);
+                    }
+                }
+                int ai = nsamp, ii = 3 * si.nbh;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n1 = __shfl_up_sync(FULL, ai, o), n2 = __shfl_up_sync(FULL, ii, o);
+                    if (lane >= o) { ai += n1; ii += n2; }
+                }
+                si.accbase = accrun + ai - nsamp;
+                si.itembase = itemrun + ii - 3 * si.nbh;
+                if (s < nslots) ctl.slot[s] = si;
+                accrun += __shfl_sync(FULL, ai, 31);
+                itemrun += __shfl_sync(FULL, ii, 31);
+            }
+        }
+        if (lane == 0) {
+            // accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by the record list (32 bytes each)
+            const long long accbytes = ((long long)accrun * 8 + 15) & ~15LL;
+            const long long rest = (long long)kArenaBytes - accbytes;
+            const bool fits = nslots <= kMaxSlots && ncell <= 32 * kMaxChunks && rest >= (long long)ncell * 16 && rest >= (long long)kMinRec * 32;
+            ctl.nviews = nviews; ctl.nslots = nslots; ctl.ncell = ncell; ctl.nacc = accrun; ctl.nitems = itemrun;
+            ctl.reccap = fits ? (int)min(rest / 32, 65535LL) : 0;
+            ctl.fits = fits ? 1 : 0;
+            if (nslots <= kMaxSlots) ctl.slot[nslots].itembase = itemrun;  // sentinel of the item -> slot search
+        }
+    } else {
+        // meanwhile the other warps zero the head of the accumulator region (its size is not known yet)
+        uint4 *z = reinterpret_cast<uint4 *>(arena);
+        for (int q = tid - 32; q < kSpecZero; q += kNT - 32) z[q] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    __syncthreads();
+    if (!ctl.fits) return false;
 
-    // ---------------------------------------------------------------- A: rays of the thread's 4 pixels
-    PixTaps pt[kPPL];
+    const int nviews = ctl.nviews, ncell = ctl.ncell, nacc = ctl.nacc, nitems = ctl.nitems, reccap = ctl.reccap;
+    uint2 *acc = reinterpret_cast<uint2 *>(arena);
+    unsigned char *region2 = arena + (((size_t)nacc * 8 + 15) & ~(size_t)15);
+    uint4 *rec = reinterpret_cast<uint4 *>(region2);      // [reccap][2]
+    float4 *patch = reinterpret_cast<float4 *>(region2);  // [ncell], after the records are dead
+    // ---------------------------------------------------- zero the accumulators; accumulator offsets of every (view, level)
     {
-        const Camera cam = cams[view];
-        const float pxl = ray_screen(cam.tan_half_x, W, blockIdx.x * kTile + lane);
-        const float pyl = ray_screen(cam.tan_half_y, H, blockIdx.y * kTile + warp * 4 + (lane & 3));
-        const float py = __shfl_sync(FULL, pyl, lane >> 3);
+        uint4 *z = reinterpret_cast<uint4 *>(arena);
+        const int nz = (nacc + 1) >> 1;
+        for (int q = kSpecZero + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);  // the rest (warps 1..7 zeroed the head during T)
+        for (int q = tid; q < nviews * h; q += kNT) {
+            const int vw = q / h, L = q - vw * h;
+            const int iv = vw / nu, iu = vw - iv * nu;
+            const int sidx = ctl.lvl_base[L] + (((bv0 + iv) >> L) - ctl.lvl_pv0[L]) * ctl.lvl_nu[L] + (((bu0 + iu) >> L) - ctl.lvl_pu0[L]);
+            const SlotInfo &sl = ctl.slot[sidx];
+            const ViewInfo &vi = ctl.view[vw];
+            ctl.voff[vw][L] = make_int2(sl.accbase + (vi.t0 - sl.t0) * sl.ns + (vi.s0 - sl.s0), sl.ns);
+        }
+    }
+    // ---------------------------------------------------- B1: one lane per (slot, channel, block row): flag words -> records
+    for (int base = 0; base < nitems; base += kNT) {
+        const int it = base + tid;
+        const bool on = it < nitems;
+        uint4 d = make_uint4(0u, 0u, 0u, 0u);
+        uint32_t refpc = 0u, sc = 0u, pred = 0u;
+        int b0 = 0, b1 = -1, by = 0, rowb = 0;
+        size_t frbase = 0;
+        if (on) {
+            int s = 0;
+            while (it >= ctl.slot[s + 1].itembase) ++s;
+            const SlotInfo &sl = ctl.slot[s];
+            const int r = it - sl.itembase;
+            const int c = r / sl.nbh, jr = r - c * sl.nbh;
+            d = ldg(S.pc + sl.pc0 + c);
+            frbase = (size_t)(sl.pc0 + (uint32_t)c) * (size_t)S.fgroups;  // = d.x, without waiting for d
+            refpc = sl.refpc0 + (uint32_t)c;
+            sc = ((uint32_t)s << 22) | ((uint32_t)c << 28);
+            pred = sl.pred;
+            by = sl.by0 + jr;
+            rowb = by * S.nbx;
+            b0 = rowb + sl.bx0; b1 = b0 + sl.nbw - 1;
+        }
+        const int ng = on ? (b1 >> 5) - (b0 >> 5) + 1 : 0;
+        const int ngmax = __reduce_max_sync(FULL, ng);
+        for (int gi = 0; gi < ngmax; ++gi) {
+            uint32_t resb = 0u, prdb = 0u;
+            uint4 fr = make_uint4(0u, 0u, 0u, 0u);
+            const int g = (b0 >> 5) + gi;
+            if (gi < ng) {
+                fr = ldg(S.flagrec + frbase + (size_t)g);
+                const int lo = max(b0 - (g << 5), 0), hi = min(b1 - (g << 5), 31);
+                const uint32_t mask = (0xFFFFFFFFu >> (31 - hi)) & (0xFFFFFFFFu << lo);
+                resb = fr.x & mask;
+                prdb = pred ? (fr.z & mask) : 0u;
+            }
+            uint32_t any = resb | prdb;
+            const int cnt = (int)popc(any);
+            int inc = cnt;
 #pragma unroll
-        for (int p = 0; p < kPPL; ++p) {
-            const float px = __shfl_sync(FULL, pxl, lx * kPPL + p);
-            pt[p].uv = kNone; pt[p].st = 0u;
-            pt[p].fu = pt[p].fv = pt[p].fs = pt[p].ft = 0.f;
-            if (x0 + p < W && y < H) {
-                const Ray r = ray_from_screen(S, cam, px, py);
-                if (r.hit) {
-                    const Taps k = tap_setup(S, r);
-                    pt[p].uv = (uint32_t)k.u0 | ((uint32_t)k.v0 << 12) | ((uint32_t)(k.u1 - k.u0) << 24) | ((uint32_t)(k.v1 - k.v0) << 25);
-                    pt[p].st = (uint32_t)k.s0 | ((uint32_t)k.t0 << 14) | ((uint32_t)(k.s1 - k.s0) << 28) | ((uint32_t)(k.t1 - k.t0) << 29);
-                    pt[p].fu = k.fu; pt[p].fv = k.fv; pt[p].fs = k.fs; pt[p].ft = k.ft;
+            for (int o = 1; o < 32; o <<= 1) {
+                const int n = __shfl_up_sync(FULL, inc, o);
+                if (lane >= o) inc += n;
+            }
+            const int tot = __shfl_sync(FULL, inc, 31);
+            if (tot == 0) continue;
+            int wbase = 0;
+            if (lane == 31) wbase = atomicAdd(&ctl.n_rec, tot);
+            wbase = __shfl_sync(FULL, wbase, 31);
+            int idx = wbase + inc - cnt;
+            while (any) {
+                const int bp = __ffs(any) - 1;
+                const uint32_t bit = 1u << bp;
+                any &= any - 1u;
+                const bool hr = (resb & bit) != 0u, hp = (prdb & bit) != 0u;
+                if (idx < reccap) {
+                    // own payload base, rank * 16, descriptor word, rank of the motion record | MV string base, reference pc, slot / channel, block position
+                    rec[2 * idx] = make_uint4(d.y, hr ? ((fr.y + popc(fr.x & (bit - 1u))) << 4) : kNone, d.w,
+                                              hp ? (fr.w + popc(fr.z & (bit - 1u))) : kNone);
+                    rec[2 * idx + 1] = make_uint4(d.z, refpc, sc, (uint32_t)((g << 5) + bp - rowb) | ((uint32_t)by << 16));
+                } else {
+                    ctl.overflow = 1;
                 }
+                ++idx;
             }
         }
     }
-    const uint32_t bg = (uint32_t)S.bg[0] | ((uint32_t)S.bg[1] << 8) | ((uint32_t)S.bg[2] << 16);
-    uint32_t rgb[kPPL];
-#pragma unroll
-    for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
-
-    // ---------------------------------------------------------------- row ranges: whole tile first, halved while the tables do not fit
-    int row0 = 0, span = kTile;
-    while (row0 < kTile) {
-        const bool inr = ly >= row0 && ly < row0 + span;
-        __syncthreads();  // the previous range's readers of ctl / the patch are done (and the digit table is loaded)
-        if (tid < kMaxViews) { ctl.vbox[tid][0] = 0x7fffffff; ctl.vbox[tid][1] = 0x7fffffff; ctl.vbox[tid][2] = -1; ctl.vbox[tid][3] = -1; }
-        if (tid < 4) { ctl.lo[tid] = 0x7fffffff; ctl.hi[tid] = -1; }
-        if (tid == 0) { ctl.n_rec = 0; ctl.overflow = 0; ctl.fits = 0; }
-        __syncthreads();
-
-        // ------------------------------------------------------------ lane summary: common (u0, v0, du, dv) key and (s,t) box of the lane's pixels
-        uint32_t key = kNone;
-        bool mixed = false;
-        int ls0 = 0x7fffffff, lt0 = 0x7fffffff, ls1 = -1, lt1 = -1;
-        if (inr) {
-#pragma unroll
-            for (int p = 0; p < kPPL; ++p)
-                if (pt[p].uv != kNone) {
-                    if (key == kNone) key = pt[p].uv;
-                    else if (pt[p].uv != key) mixed = true;
-                    const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
-                    ls0 = min(ls0, s0); ls1 = max(ls1, s0 + (int)((pt[p].st >> 28) & 1u));
-                    lt0 = min(lt0, t0); lt1 = max(lt1, t0 + (int)((pt[p].st >> 29) & 1u));
-                }
-        }
-        {   // (u, v) range of the range's taps
-            int ulo = 0x7fffffff, vlo = 0x7fffffff, uhi = -1, vhi = -1;
-            if (inr) {
-#pragma unroll
-                for (int p = 0; p < kPPL; ++p)
-                    if (pt[p].uv != kNone) {
-                        const int u0 = pt[p].uv & 0xFFF, v0 = (pt[p].uv >> 12) & 0xFFF;
-                        ulo = min(ulo, u0); uhi = max(uhi, u0 + (int)((pt[p].uv >> 24) & 1u));
-                        vlo = min(vlo, v0); vhi = max(vhi, v0 + (int)((pt[p].uv >> 25) & 1u));
-                    }
-            }
-            ulo = __reduce_min_sync(FULL, ulo); vlo = __reduce_min_sync(FULL, vlo);
-            uhi = __reduce_max_sync(FULL, uhi); vhi = __reduce_max_sync(FULL, vhi);
-            if (lane == 0 && uhi >= 0) {
-                atomicMin(&ctl.lo[0], ulo); atomicMin(&ctl.lo[1], vlo);
-                atomicMax(&ctl.hi[0], uhi); atomicMax(&ctl.hi[1], vhi);
-            }
-        }
-        __syncthreads();
-        const int bu0 = ctl.lo[0], bv0 = ctl.lo[1];
-        const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
-        bool done = ctl.hi[0] < 0;  // no ray of the range hits the slab: background only
-        if (!done && nu <= kMaxV && nv <= kMaxV) {
-            // -------------------------------------------------------- V: footprint box per view
-            // lanes with one common key first (the usual case: one or two rounds per warp), then pixel by pixel
-            auto merge_boxes = [&](uint32_t k, int a0, int a1, int a2, int a3) {
-                uint32_t todo = __ballot_sync(FULL, k != kNone);
-                while (todo) {
-                    const int leader = __ffs(todo) - 1;
-                    const uint32_t kk = __shfl_sync(FULL, k, leader);
-                    const bool mine = k == kk;
-                    const int m0 = __reduce_min_sync(FULL, mine ? a0 : 0x7fffffff), m1 = __reduce_min_sync(FULL, mine ? a1 : 0x7fffffff);
-                    const int m2 = __reduce_max_sync(FULL, mine ? a2 : -1), m3 = __reduce_max_sync(FULL, mine ? a3 : -1);
-                    if (lane < 4) {
-                        const int du = (int)((kk >> 24) & 1u), dv = (int)((kk >> 25) & 1u);
-                        const int au = lane & 1, av = lane >> 1;
-                        if ((!au || du) && (!av || dv)) {
-                            const int vw = ((int)((kk >> 12) & 0xFFF) - bv0 + av) * nu + ((int)(kk & 0xFFF) - bu0 + au);
-                            atomicMin(&ctl.vbox[vw][0], m0); atomicMin(&ctl.vbox[vw][1], m1);
-                            atomicMax(&ctl.vbox[vw][2], m2); atomicMax(&ctl.vbox[vw][3], m3);
-                        }
-                    }
-                    todo &= ~__ballot_sync(FULL, mine);
-                }
-            };
-            merge_boxes(mixed ? kNone : key, ls0, lt0, ls1, lt1);
-            if (__any_sync(FULL, mixed)) {
-#pragma unroll
-                for (int p = 0; p < kPPL; ++p) {
-                    const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
-                    merge_boxes((mixed && inr) ? pt[p].uv : kNone, s0, t0, s0 + (int)((pt[p].st >> 28) & 1u), t0 + (int)((pt[p].st >> 29) & 1u));
-                }
-            }
-            __syncthreads();
-
-            // -------------------------------------------------------- T: tables (warp 0)
-            if (warp == 0) {
-                const int nviews = nu * nv;
-                int vs0 = 0, vt0 = 0, vns = 0, vnt = 0;
-                if (lane < nviews && ctl.vbox[lane][2] >= 0) {
-                    vs0 = ctl.vbox[lane][0]; vt0 = ctl.vbox[lane][1];
-                    vns = ctl.vbox[lane][2] - vs0 + 1; vnt = ctl.vbox[lane][3] - vt0 + 1;
-                }
-                const int vcells = (vns * vnt + 31) & ~31;  // whole warps per view
-                int incl = vcells;
-#pragma unroll
-                for (int o = 1; o < kMaxViews; o <<= 1) {
-                    const int n = __shfl_up_sync(FULL, incl, o);
-                    if (lane >= o) incl += n;
-                }
-                const int ncell = __shfl_sync(FULL, incl, kMaxViews - 1);
-                if (lane < kMaxViews) {
-                    ViewInfo vi;
-                    vi.s0 = vs0; vi.t0 = vt0; vi.ns = vns; vi.nt = vnt;
-                    vi.cellbase = incl - vcells;
-                    ctl.vcb[lane] = make_int2(vi.cellbase - vt0 * vns - vs0, vns);
-                    for (int c = vi.cellbase >> 5; c < min(incl >> 5, kMaxChunks); ++c) ctl.chunkvw[c] = (uint8_t)lane;
-                    vi.m_ns = magic_of((uint32_t)vns);
-                    const int iv = lane / nu, iu = lane - iv * nu;
-                    const unsigned long long ro = (unsigned long long)(((bv0 + iv) >> h) * S.UH + ((bu0 + iu) >> h)) *
-                                                  (unsigned long long)S.Ht * (unsigned long long)S.Ws;
-                    vi.rkv_lo = (uint32_t)ro; vi.rkv_hi = (uint32_t)(ro >> 32);
-                    ctl.view[lane] = vi;
-                }
-                // per level the rectangle of planes over the views; lane L owns level L
-                int pu0 = 0, pv0 = 0, nuL = 0, cntL = 0;
-                if (lane < h) {
-                    pu0 = bu0 >> lane; pv0 = bv0 >> lane;
-                    nuL = ((bu0 + nu - 1) >> lane) - pu0 + 1;
-                    cntL = nuL * (((bv0 + nv - 1) >> lane) - pv0 + 1);
-                }
-                int lincl = cntL;
-#pragma unroll
-                for (int o = 1; o < kMaxLevels; o <<= 1) {
-                    const int n = __shfl_up_sync(FULL, lincl, o);
-                    if (lane >= o) lincl += n;
-                }
-                const int nslots = __shfl_sync(FULL, lincl, h - 1);
-                if (lane < h) { ctl.lvl_base[lane] = lincl - cntL; ctl.lvl_pu0[lane] = pu0; ctl.lvl_pv0[lane] = pv0; ctl.lvl_nu[lane] = nuL; }
-                __syncwarp();
-                int accrun = 0, itemrun = 0;
-                if (nslots <= kMaxSlots) {
-                    for (int sb = 0; sb < nslots; sb += 32) {
-                        const int s = sb + lane;
-                        SlotInfo si;
-                        si.pc0 = si.refpc0 = 0u; si.pred = 0u;
-                        si.s0 = si.t0 = 0; si.ns = 0; si.s1 = si.t1 = -1; si.bx0 = si.by0 = 0; si.nbw = 0; si.nbh = 0;
-                        int nsamp = 0;
-                        if (s < nslots) {
-                            int L = 0;
-                            while (L + 1 < h && s >= ctl.lvl_base[L + 1]) ++L;
-                            const int jj = s - ctl.lvl_base[L], n = ctl.lvl_nu[L];
-                            const int jv = jj / n;
-                            const int pv = ctl.lvl_pv0[L] + jv, pu = ctl.lvl_pu0[L] + (jj - jv * n);
-                            const LevelDesc lv = S.lev[L];
-                            si.pc0 = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
-                            si.refpc0 = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
-                            si.pred = (uint32_t)((pu | pv) & 1);
-                            // union of the boxes of the views below this plane
-                            const int iu0 = max(pu << L, bu0) - bu0, iu1 = min(((pu + 1) << L) - 1, bu0 + nu - 1) - bu0;
-                            const int iv0 = max(pv << L, bv0) - bv0, iv1 = min(((pv + 1) << L) - 1, bv0 + nv - 1) - bv0;
-                            int a0 = 0x7fffffff, a1 = 0x7fffffff, a2 = -1, a3 = -1;
-                            for (int iv = iv0; iv <= iv1; ++iv)
-                                for (int iu = iu0; iu <= iu1; ++iu) {
-                                    const int vw = iv * nu + iu;
-                                    if (ctl.vbox[vw][2] >= 0) {
-                                        a0 = min(a0, ctl.vbox[vw][0]); a1 = min(a1, ctl.vbox[vw][1]);
-                                        a2 = max(a2, ctl.vbox[vw][2]); a3 = max(a3, ctl.vbox[vw][3]);
-                                    }
-                                }
-                            if (a2 >= 0) {
-                                si.s0 = a0; si.t0 = a1; si.s1 = a2; si.t1 = a3; si.ns = a2 - a0 + 1;
-                                si.bx0 = a0 >> 2; si.by0 = a1 >> 2;
-                                si.nbw = (a2 >> 2) - si.bx0 + 1; si.nbh = (a3 >> 2) - si.by0 + 1;
-                                nsamp = si.ns * (a3 - a1 + 1);
-                            }
-                        }
-                        int ai = nsamp, ii = 3 * si.nbh;
-#pragma unroll
-                        for (int o = 1; o < 32; o <<= 1) {
-                            const int n1 = __shfl_up_sync(FULL, ai, o), n2 = __shfl_up_sync(FULL, ii, o);
-                            if (lane >= o) { ai += n1; ii += n2; }
-                        }
-                        si.accbase = accrun + ai - nsamp;
-                        si.itembase = itemrun + ii - 3 * si.nbh;
-                        if (s < nslots) ctl.slot[s] = si;
-                        accrun += __shfl_sync(FULL, ai, 31);
-                        itemrun += __shfl_sync(FULL, ii, 31);
-                    }
-                }
-                if (lane == 0) {
-                    // accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by the record list (32 bytes each)
-                    const long long accbytes = ((long long)accrun * 8 + 15) & ~15LL;
-                    const long long rest = (long long)ARENA_BYTES - accbytes;
-                    const bool fits = nslots <= kMaxSlots && ncell <= 32 * kMaxChunks && rest >= (long long)ncell * 16 && rest >= (long long)kMinRec * 32;
-                    ctl.nviews = nviews; ctl.nslots = nslots; ctl.ncell = ncell; ctl.nacc = accrun; ctl.nitems = itemrun;
-                    ctl.reccap = fits ? (int)min(rest / 32, 65535LL) : 0;
-                    ctl.fits = fits ? 1 : 0;
-                    if (nslots <= kMaxSlots) ctl.slot[nslots].itembase = itemrun;  // sentinel of the item -> slot search
-                }
-            }
-            else {
-                // meanwhile the other warps zero the head of the accumulator region (its size is not known yet)
-                uint4 *z = reinterpret_cast<uint4 *>(arena);
-                for (int q = tid - 32; q < kSpecZero; q += kNT - 32) z[q] = make_uint4(0u, 0u, 0u, 0u);
-            }
-            __syncthreads();
-
-            if (ctl.fits) {
-                const int nviews = ctl.nviews, nslots = ctl.nslots, ncell = ctl.ncell, nacc = ctl.nacc, nitems = ctl.nitems, reccap = ctl.reccap;
-                uint2 *acc = reinterpret_cast<uint2 *>(arena);
-                unsigned char *region2 = arena + (((size_t)nacc * 8 + 15) & ~(size_t)15);
-                uint4 *rec = reinterpret_cast<uint4 *>(region2);      // [reccap][2]
-                float4 *patch = reinterpret_cast<float4 *>(region2);  // [ncell], after the records are dead
-                // ---------------------------------------------------- zero the accumulators; accumulator offsets of every (view, level)
-                {
-                    uint4 *z = reinterpret_cast<uint4 *>(arena);
-                    const int nz = (nacc + 1) >> 1;
-                    for (int q = kSpecZero + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);  // the rest (warps 1..7 zeroed the head during T)
-                    for (int q = tid; q < nviews * h; q += kNT) {
-                        const int vw = q / h, L = q - vw * h;
-                        const int iv = vw / nu, iu = vw - iv * nu;
-                        const int sidx = ctl.lvl_base[L] + (((bv0 + iv) >> L) - ctl.lvl_pv0[L]) * ctl.lvl_nu[L] + (((bu0 + iu) >> L) - ctl.lvl_pu0[L]);
-                        const SlotInfo &sl = ctl.slot[sidx];
-                        const ViewInfo &vi = ctl.view[vw];
-                        ctl.voff[vw][L] = make_int2(sl.accbase + (vi.t0 - sl.t0) * sl.ns + (vi.s0 - sl.s0), sl.ns);
-                    }
-                }
-                // ---------------------------------------------------- B1: one lane per (slot, channel, block row): flag words -> records
-                for (int base = 0; base < nitems; base += kNT) {
-                    const int it = base + tid;
-                    const bool on = it < nitems;
-                    uint4 d = make_uint4(0u, 0u, 0u, 0u);
-                    uint32_t refpc = 0u, sc = 0u, pred = 0u;
-                    int b0 = 0, b1 = -1, by = 0, rowb = 0;
-                    size_t frbase = 0;
-                    if (on) {
-                        int s = 0;
-                        while (it >= ctl.slot[s + 1].itembase) ++s;
-                        const SlotInfo &sl = ctl.slot[s];
-                        const int r = it - sl.itembase;
-                        const int c = r / sl.nbh, jr = r - c * sl.nbh;
-                        d = ldg(S.pc + sl.pc0 + c);
-                        frbase = (size_t)(sl.pc0 + (uint32_t)c) * (size_t)S.fgroups;  // = d.x, without waiting for d
-                        refpc = sl.refpc0 + (uint32_t)c;
-                        sc = ((uint32_t)s << 22) | ((uint32_t)c << 28);
-                        pred = sl.pred;
-                        by = sl.by0 + jr;
-                        rowb = by * S.nbx;
-                        b0 = rowb + sl.bx0; b1 = b0 + sl.nbw - 1;
-                    }
-                    const int ng = on ? (b1 >> 5) - (b0 >> 5) + 1 : 0;
-                    const int ngmax = __reduce_max_sync(FULL, ng);
-                    for (int gi = 0; gi < ngmax; ++gi) {
-                        uint32_t resb = 0u, prdb = 0u;
-                        uint4 fr = make_uint4(0u, 0u, 0u, 0u);
-                        const int g = (b0 >> 5) + gi;
-                        if (gi < ng) {
-                            fr = ldg(S.flagrec + frbase + (size_t)g);
-                            const int lo = max(b0 - (g << 5), 0), hi = min(b1 - (g << 5), 31);
-                            const uint32_t mask = (0xFFFFFFFFu >> (31 - hi)) & (0xFFFFFFFFu << lo);
-                            resb = fr.x & mask;
-                            prdb = pred ? (fr.z & mask) : 0u;
-                        }
-                        uint32_t any = resb | prdb;
-                        const int cnt = (int)popc(any);
-                        int inc = cnt;
-#pragma unroll
-                        for (int o = 1; o < 32; o <<= 1) {
-                            const int n = __shfl_up_sync(FULL, inc, o);
-                            if (lane >= o) inc += n;
-                        }
-                        const int tot = __shfl_sync(FULL, inc, 31);
-                        if (tot == 0) continue;
-                        int wbase = 0;
-                        if (lane == 31) wbase = atomicAdd(&ctl.n_rec, tot);
-                        wbase = __shfl_sync(FULL, wbase, 31);
-                        int idx = wbase + inc - cnt;
-                        while (any) {
-                            const int bp = __ffs(any) - 1;
-                            const uint32_t bit = 1u << bp;
-                            any &= any - 1u;
-                            const bool hr = (resb & bit) != 0u, hp = (prdb & bit) != 0u;
-                            if (idx < reccap) {
-                                // own payload base, rank * 16, descriptor word, rank of the motion record | MV string base, reference pc, slot / channel, block position
-                                rec[2 * idx] = make_uint4(d.y, hr ? ((fr.y + popc(fr.x & (bit - 1u))) << 4) : kNone, d.w,
-                                                          hp ? (fr.w + popc(fr.z & (bit - 1u))) : kNone);
-                                rec[2 * idx + 1] = make_uint4(d.z, refpc, sc, (uint32_t)((g << 5) + bp - rowb) | ((uint32_t)by << 16));
-                            } else {
-                                ctl.overflow = 1;
-                            }
-                            ++idx;
-                        }
-                    }
-                }
-                __syncthreads();
-                if (ctl.overflow == 0) {
-                    const int nrec = ctl.n_rec;
-                    // ------------------------------------------------ B2: motion record + reference descriptor, once per block
-                    for (int rr = tid; rr < nrec; rr += kNT) {
-                        const uint4 r0 = rec[2 * rr], r1 = rec[2 * rr + 1];
-                        if (r0.w != kNone) {
-                            const uint32_t mr = bise_at(S.mv + r1.x, r0.w, S.mv_layout, S.mv_m, ctl.lut);
-                            int md, dx, dy;
-                            mv_unpack(S, mr, md, dx, dy);
-                            const uint4 dr = ldg(S.pc + r1.y);
-                            rec[2 * rr].w = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
-                            rec[2 * rr + 1] = make_uint4(dr.x, dr.y, r1.z | (dr.w & 0x3FFFFFu), r1.w);
-                        } else {
-                            rec[2 * rr].w = 0u;
-                            rec[2 * rr + 1] = make_uint4(0u, 0u, r1.z, r1.w);
-                        }
-                    }
-                    __syncthreads();
-                    // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values
-                    int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
-                    for (int t = tid; t < 4 * nrec; t += kNT) {
-                        const int rr = t >> 2, ky = t & 3;
-                        const uint4 r0 = rec[2 * rr], r1 = rec[2 * rr + 1];
-                        const SlotInfo &sl = ctl.slot[(r1.z >> 22) & 63u];
-                        const int yy = (int)((r1.w >> 16) << 2) + ky;
-                        const int st0 = sl.t0, st1 = sl.t1;
-                        if (yy < st0 || yy > st1) continue;
-                        const int xx = (int)((r1.w & 0xFFFFu) << 2);
-                        uint2 own = make_uint2(0u, 0u);
-                        if (r0.y != kNone) own = bise_row4(S.pay + r0.x, r0.y + (uint32_t)(ky << 2), r0.z, ctl.lut);
-                        int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
-                        if (r0.w) {
-                            const int rx = xx + (int)((r0.w >> 8) & 0xFFu) - S.W, ry = yy + (int)(r0.w & 0xFFu) - S.W;
-                            if ((unsigned)ry < (unsigned)S.Ht) {
-                                // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
-                                const int o = rx & 3, bxa = rx >> 2;
-                                const uint32_t i0 = (uint32_t)((ry & 3) << 2);
-                                const int rowb = (ry >> 2) * S.nbx;
-                                uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-                                if ((unsigned)bxa < (unsigned)S.nbx) {
-                                    const int b = rowb + bxa;
-                                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
-                                    const uint32_t bit = 1u << (b & 31);
-                                    if (fr.x & bit) qa = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
-                                }
-                                if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
-                                    const int b = rowb + bxa + 1;
-                                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
-                                    const uint32_t bit = 1u << (b & 31);
-                                    if (fr.x & bit) qb = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
-                                }
-                                // samples o .. o+3 of the 8-sample string qa | qb
-                                uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
-                                if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
-                                const uint32_t sh = (uint32_t)(o & 1) << 4;
-                                const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
-                                const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
-                                // R10: subtractive P = e + R, additive P = e - R
-                                if (r0.w & 0x10000u) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
-                                else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
-                            }
-                        }
-                        const int c = (int)((r1.z >> 28) & 3u);
-                        int16_t *dst = acc16 + (((sl.accbase + (yy - st0) * sl.ns + (xx - sl.s0)) << 2) + c);
-                        const int ss0 = sl.s0, ss1 = sl.s1;
-                        if (xx >= ss0 && xx <= ss1) dst[0] = (int16_t)e0;
-                        if (xx + 1 >= ss0 && xx + 1 <= ss1) dst[4] = (int16_t)e1;
-                        if (xx + 2 >= ss0 && xx + 2 <= ss1) dst[8] = (int16_t)e2;
-                        if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
-                    }
-                    __syncthreads();
-                    // ------------------------------------------------ B4: top-level RKV + per-level terms -> float RGB patch
-                    for (int q = tid; q < ncell; q += kNT) {
-                        const int vw = ctl.chunkvw[q >> 5];
-                        const ViewInfo vi = ctl.view[vw];
-                        const uint32_t local = (uint32_t)(q - vi.cellbase);
-                        const uint32_t it = fdiv(local, vi.m_ns), is = local - it * (uint32_t)vi.ns;
-                        if ((int)it >= vi.nt) continue;  // padding of the view's last chunk
-                        const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
-                        const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
-                        int a[3] = {rk.x, rk.y, rk.z};
-                        for (int L = 0; L < h; ++L) {
-                            const int2 vo = ctl.voff[vw][L];
-                            const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
-                            a[0] += (int)(int16_t)(w.x & 0xFFFFu);
-                            a[1] += (int)w.x >> 16;
-                            a[2] += (int)(int16_t)(w.y & 0xFFFFu);
-                        }
-                        const uint32_t c8 = ycocg_to_rgb8(a);
-                        // the patch aliases the record list: all B3 readers passed the barrier above
-                        patch[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
-                    }
-                    __syncthreads();
-                    // ------------------------------------------------ C: gather + blend
-                    if (inr) {
-#pragma unroll
-                        for (int p = 0; p < kPPL; ++p)
-                            if (pt[p].uv != kNone) {
-                                const int iu = (int)(pt[p].uv & 0xFFF) - bu0, iv = (int)((pt[p].uv >> 12) & 0xFFF) - bv0;
-                                const int s0 = (int)(pt[p].st & 0x3FFF), t0 = (int)((pt[p].st >> 14) & 0x3FFF);
-                                const int du = (int)((pt[p].uv >> 24) & 1u), dv = ((pt[p].uv >> 25) & 1u) ? nu : 0;
-                                const int ds = (int)((pt[p].st >> 28) & 1u), dt = (int)((pt[p].st >> 29) & 1u);
-                                const int vw0 = iv * nu + iu;
-                                int vb[4], vs[4];
-#pragma unroll
-                                for (int a = 0; a < 4; ++a) {
-                                    const int2 cb = ctl.vcb[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
-                                    vb[a] = cb.x + t0 * cb.y + s0;
-                                    vs[a] = dt ? cb.y : 0;
-                                }
-                                rgb[p] = blend16(pt[p], [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
-                            }
-                    }
-                    done = true;
-                }
-            }
-        }
-        if (!done) {
-            if (span > 1) { span >>= 1; continue; }  // halve the row range and try again
-            // -------------------------------------------------------- a single row still too large: 16 direct sample decodes
-            if (inr) {
-#pragma unroll
-                for (int p = 0; p < kPPL; ++p)
-                    if (pt[p].uv != kNone) rgb[p] = direct_pixel(S, pt[p]);
-            }
-        }
-        row0 += span;
-        span = row0 & -row0;  // the largest aligned range that starts at row0
-    }
-
-    // ---------------------------------------------------------------- store: 12 contiguous bytes per thread
-    if (y < H && x0 < W) {
-        uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x0);
-        if (out_aligned && x0 + kPPL <= W) {
-            uint32_t *o32 = reinterpret_cast<uint32_t *>(o);
-            o32[0] = rgb[0] | (rgb[1] << 24);
-            o32[1] = (rgb[1] >> 8) | (rgb[2] << 16);
-            o32[2] = (rgb[2] >> 16) | (rgb[3] << 8);
+    __syncthreads();
+    if (ctl.overflow != 0) return false;
+    const int nrec = ctl.n_rec;
+    // ------------------------------------------------ B2: motion record + reference descriptor, once per block
+    for (int rr = tid; rr < nrec; rr += kNT) {
+        const uint4 r0 = rec[2 * rr], r1 = rec[2 * rr + 1];
+        if (r0.w != kNone) {
+            const uint32_t mr = bise_at(S.mv + r1.x, r0.w, S.mv_layout, S.mv_m, ctl.lut);
+            int md, dx, dy;
+            mv_unpack(S, mr, md, dx, dy);
+            const uint4 dr = ldg(S.pc + r1.y);
+            rec[2 * rr].w = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+            rec[2 * rr + 1] = make_uint4(dr.x, dr.y, r1.z | (dr.w & 0x3FFFFFu), r1.w);
         } else {
-#pragma unroll
-            for (int p = 0; p < kPPL; ++p)
-                if (x0 + p < W) {
-                    o[3 * p + 0] = (uint8_t)(rgb[p] & 0xFF);
-                    o[3 * p + 1] = (uint8_t)((rgb[p] >> 8) & 0xFF);
-                    o[3 * p + 2] = (uint8_t)((rgb[p] >> 16) & 0xFF);
+            rec[2 * rr].w = 0u;
+            rec[2 * rr + 1] = make_uint4(0u, 0u, r1.z, r1.w);
+        }
+    }
+    __syncthreads();
+    // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values
+    int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
+    for (int t = tid; t < 4 * nrec; t += kNT) {
+        const int rr = t >> 2, ky = t & 3;
+        const uint4 r0 = rec[2 * rr], r1 = rec[2 * rr + 1];
+        const SlotInfo &sl = ctl.slot[(r1.z >> 22) & 63u];
+        const int yy = (int)((r1.w >> 16) << 2) + ky;
+        const int st0 = sl.t0, st1 = sl.t1;
+        if (yy < st0 || yy > st1) continue;
+        const int xx = (int)((r1.w & 0xFFFFu) << 2);
+        uint2 own = make_uint2(0u, 0u);
+        if (r0.y != kNone) own = bise_row4(S.pay + r0.x, r0.y + (uint32_t)(ky << 2), r0.z, ctl.lut);
+        int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
+        if (r0.w) {
+            const int rx = xx + (int)((r0.w >> 8) & 0xFFu) - S.W, ry = yy + (int)(r0.w & 0xFFu) - S.W;
+            if ((unsigned)ry < (unsigned)S.Ht) {
+                // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
+                const int o = rx & 3, bxa = rx >> 2;
+                const uint32_t i0 = (uint32_t)((ry & 3) << 2);
+                const int rowb = (ry >> 2) * S.nbx;
+                uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
+                if ((unsigned)bxa < (unsigned)S.nbx) {
+                    const int b = rowb + bxa;
+                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                    const uint32_t bit = 1u << (b & 31);
+                    if (fr.x & bit) qa = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
                 }
+                if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
+                    const int b = rowb + bxa + 1;
+                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                    const uint32_t bit = 1u << (b & 31);
+                    if (fr.x & bit) qb = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
+                }
+                // samples o .. o+3 of the 8-sample string qa | qb
+                uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
+                if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
+                const uint32_t sh = (uint32_t)(o & 1) << 4;
+                const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
+                const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
+                // R10: subtractive P = e + R, additive P = e - R
+                if (r0.w & 0x10000u) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
+                else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
+            }
+        }
+        const int c = (int)((r1.z >> 28) & 3u);
+        int16_t *dst = acc16 + (((sl.accbase + (yy - st0) * sl.ns + (xx - sl.s0)) << 2) + c);
+        const int ss0 = sl.s0, ss1 = sl.s1;
+        if (xx >= ss0 && xx <= ss1) dst[0] = (int16_t)e0;
+        if (xx + 1 >= ss0 && xx + 1 <= ss1) dst[4] = (int16_t)e1;
+        if (xx + 2 >= ss0 && xx + 2 <= ss1) dst[8] = (int16_t)e2;
+        if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
+    }
+    __syncthreads();
+    // ------------------------------------------------ B4: top-level RKV + per-level terms -> float RGB patch
+    for (int q = tid; q < ncell; q += kNT) {
+        const int vw = ctl.chunkvw[q >> 5];
+        const ViewInfo vi = ctl.view[vw];
+        const uint32_t local = (uint32_t)(q - vi.cellbase);
+        const uint32_t it = fdiv(local, vi.m_ns), is = local - it * (uint32_t)vi.ns;
+        if ((int)it >= vi.nt) continue;  // padding of the view's last chunk
+        const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
+        const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
+        int a[3] = {rk.x, rk.y, rk.z};
+        for (int L = 0; L < h; ++L) {
+            const int2 vo = ctl.voff[vw][L];
+            const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
+            a[0] += (int)(int16_t)(w.x & 0xFFFFu);
+            a[1] += (int)w.x >> 16;
+            a[2] += (int)(int16_t)(w.y & 0xFFFFu);
+        }
+        const uint32_t c8 = ycocg_to_rgb8(a);
+        // the patch aliases the record list: all B3 readers passed the barrier above
+        patch[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
+    }
+    __syncthreads();
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pixel mapping of a pass.  ts = 32: the whole tile, thread (tid & 7, tid >> 3) owns 4 consecutive pixels.  ts = 16 /
+// 8: a sub-tile, one pixel per thread (pixel slot 0; ts = 8 uses the first 64 threads).  One code path serves both
+// (slots 1..3 are simply empty in sub-tile passes): the kernel is instruction-cache sensitive, so the phases exist once.
+__device__ __forceinline__ void thread_pixel(int ox, int oy, int ts, int &x0, int &y, int &npix)
+{
+    const int tid = threadIdx.x;
+    if (ts == kTile) { x0 = ox + (tid & 7) * kPPL; y = oy + (tid >> 3); npix = kPPL; }
+    else { const int sh = ts == 16 ? 4 : 3; x0 = ox + (tid & (ts - 1)); y = oy + (tid >> sh); npix = tid < ts * ts ? 1 : 0; }
+}
+
+// ---------------------------------------------------------------- A: rays of the thread's pixels
+__device__ __forceinline__ void setup_rays(const DevStream &S, const Camera &cam, int W, int H, int ox, int oy, int ts, PixTaps (&pt)[kPPL])
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int x0, y, npix;
+    thread_pixel(ox, oy, ts, x0, y, npix);
+    // screen coordinates once per column / row of the tile, shared by shuffles (sub-tiles: each lane its own)
+    const float pxl = ray_screen(cam.tan_half_x, W, ts == kTile ? ox + lane : x0);
+    const float pyl = ray_screen(cam.tan_half_y, H, ts == kTile ? oy + warp * 4 + (lane & 3) : y);
+    const float py = __shfl_sync(FULL, pyl, ts == kTile ? lane >> 3 : lane);
+#pragma unroll
+    for (int p = 0; p < kPPL; ++p) {
+        const float px = __shfl_sync(FULL, pxl, ts == kTile ? (tid & 7) * kPPL + p : lane);
+        pt[p].uv = kNone; pt[p].st = 0u;
+        pt[p].fu = pt[p].fv = pt[p].fs = pt[p].ft = 0.f;
+        if (p < npix && x0 + p < W && y < H) {
+            const Ray r = ray_from_screen(S, cam, px, py);
+            if (r.hit) {
+                const Taps k = tap_setup(S, r);
+                pt[p].uv = (uint32_t)k.u0 | ((uint32_t)k.v0 << 12) | ((uint32_t)(k.u1 - k.u0) << 24) | ((uint32_t)(k.v1 - k.v0) << 25);
+                pt[p].st = (uint32_t)k.s0 | ((uint32_t)k.t0 << 14) | ((uint32_t)(k.s1 - k.s0) << 28) | ((uint32_t)(k.t1 - k.t0) << 29);
+                pt[p].fu = k.fu; pt[p].fv = k.fv; pt[p].fs = k.fs; pt[p].ft = k.ft;
+            }
         }
     }
 }
 
-constexpr int kArenaBytes = 50 * 1024;
-constexpr int kMinBlocks = 4;
+// ---------------------------------------------------------------------------------------------------------------
+// One pass over a (sub-)tile whose rays are set up: footprint boxes (V), tables + decode (build_patch), gather + blend
+// (C).  Returns true (CTA-uniform) when rgb[] holds the pass's pixels (background where the ray misses); false
+// when the tables do not fit the arena and the (sub-)tile must be split.
+__device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, const PixTaps (&pt)[kPPL],
+                                          uint32_t (&rgb)[kPPL])
+{
+    constexpr int PPL = kPPL;
+    const int tid = threadIdx.x, lane = tid & 31;
+    __syncthreads();  // the previous pass's readers of ctl / the patch are done (and the digit table is loaded)
+    if (tid < kMaxViews) { ctl.vbox[tid][0] = 0x7fffffff; ctl.vbox[tid][1] = 0x7fffffff; ctl.vbox[tid][2] = -1; ctl.vbox[tid][3] = -1; }
+    if (tid < 4) { ctl.lo[tid] = 0x7fffffff; ctl.hi[tid] = -1; }
+    if (tid == 0) { ctl.n_rec = 0; ctl.overflow = 0; ctl.fits = 0; }
+    __syncthreads();
+
+    // ------------------------------------------------------------ lane summary: common (u0, v0, du, dv) key and (s,t) box of the lane's pixels
+    uint32_t key = kNone;
+    bool mixed = false;
+    int ls0 = 0x7fffffff, lt0 = 0x7fffffff, ls1 = -1, lt1 = -1;
+    int ulo = 0x7fffffff, vlo = 0x7fffffff, uhi = -1, vhi = -1;
+#pragma unroll
+    for (int p = 0; p < PPL; ++p)
+        if (pt[p].uv != kNone) {
+            if (key == kNone) key = pt[p].uv;
+            else if (pt[p].uv != key) mixed = true;
+            const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
+            ls0 = min(ls0, s0); ls1 = max(ls1, s0 + (int)((pt[p].st >> 28) & 1u));
+            lt0 = min(lt0, t0); lt1 = max(lt1, t0 + (int)((pt[p].st >> 29) & 1u));
+            const int u0 = pt[p].uv & 0xFFF, v0 = (pt[p].uv >> 12) & 0xFFF;
+            ulo = min(ulo, u0); uhi = max(uhi, u0 + (int)((pt[p].uv >> 24) & 1u));
+            vlo = min(vlo, v0); vhi = max(vhi, v0 + (int)((pt[p].uv >> 25) & 1u));
+        }
+    ulo = __reduce_min_sync(FULL, ulo); vlo = __reduce_min_sync(FULL, vlo);
+    uhi = __reduce_max_sync(FULL, uhi); vhi = __reduce_max_sync(FULL, vhi);
+    const int ws0 = __reduce_min_sync(FULL, ls0), wt0 = __reduce_min_sync(FULL, lt0);
+    const int ws1 = __reduce_max_sync(FULL, ls1), wt1 = __reduce_max_sync(FULL, lt1);
+    if (lane == 0 && uhi >= 0) {
+        atomicMin(&ctl.lo[0], ulo); atomicMin(&ctl.lo[1], vlo); atomicMin(&ctl.lo[2], ws0); atomicMin(&ctl.lo[3], wt0);
+        atomicMax(&ctl.hi[0], uhi); atomicMax(&ctl.hi[1], vhi); atomicMax(&ctl.hi[2], ws1); atomicMax(&ctl.hi[3], wt1);
+    }
+    __syncthreads();
+    const int bu0 = ctl.lo[0], bv0 = ctl.lo[1];
+    const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
+    if (ctl.hi[0] < 0) return true;  // no ray of the sub-tile hits the slab: background only
+    if (nu > kMaxV || nv > kMaxV) return false;
+    {
+        // Early exit before the tables are built: from the pass's exact (u,v) range and (s,t) box, cells ~ (2 ns + nu)
+        // (2 nt + nv) (every pixel touches 2 x 2 views) and accumulator samples ~ cells (level 0) + box area x planes
+        // of every level >= 1.  Only a hint (build_patch decides): a pass that is let through and does not fit is
+        // split after the tables are built, one that is split needlessly costs some halo.
+        const int ns = ctl.hi[2] - ctl.lo[2] + 1, nt = ctl.hi[3] - ctl.lo[3] + 1;
+        const int area = ns * nt;
+        const int cells = (2 * ns + nu) * (2 * nt + nv) + 16 * nu * nv;
+        int accs = cells;
+        for (int L = 1; L < S.h; ++L)
+            accs += area * ((((bu0 + nu - 1) >> L) - (bu0 >> L) + 1) * (((bv0 + nv - 1) >> L) - (bv0 >> L) + 1));
+        if (16 * cells + 8 * accs > kArenaBytes * kEstSlackPct / 100) return false;
+    }
+
+    // -------------------------------------------------------- V: footprint box per view
+    // lanes with one common key first (the usual case: one or two rounds per warp), then pixel by pixel
+    auto merge_boxes = [&](uint32_t k, int a0, int a1, int a2, int a3) {
+        uint32_t todo = __ballot_sync(FULL, k != kNone);
+        while (todo) {
+            const int leader = __ffs(todo) - 1;
+            const uint32_t kk = __shfl_sync(FULL, k, leader);
+            const bool mine = k == kk;
+            const int m0 = __reduce_min_sync(FULL, mine ? a0 : 0x7fffffff), m1 = __reduce_min_sync(FULL, mine ? a1 : 0x7fffffff);
+            const int m2 = __reduce_max_sync(FULL, mine ? a2 : -1), m3 = __reduce_max_sync(FULL, mine ? a3 : -1);
+            if (lane < 4) {
+                const int du = (int)((kk >> 24) & 1u), dv = (int)((kk >> 25) & 1u);
+                const int au = lane & 1, av = lane >> 1;
+                if ((!au || du) && (!av || dv)) {
+                    const int vw = ((int)((kk >> 12) & 0xFFF) - bv0 + av) * nu + ((int)(kk & 0xFFF) - bu0 + au);
+                    atomicMin(&ctl.vbox[vw][0], m0); atomicMin(&ctl.vbox[vw][1], m1);
+                    atomicMax(&ctl.vbox[vw][2], m2); atomicMax(&ctl.vbox[vw][3], m3);
+                }
+            }
+            todo &= ~__ballot_sync(FULL, mine);
+        }
+    };
+    merge_boxes(mixed ? kNone : key, ls0, lt0, ls1, lt1);
+    if (PPL > 1 && __any_sync(FULL, mixed)) {
+#pragma unroll
+        for (int p = 0; p < PPL; ++p) {
+            const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
+            merge_boxes(mixed ? pt[p].uv : kNone, s0, t0, s0 + (int)((pt[p].st >> 28) & 1u), t0 + (int)((pt[p].st >> 29) & 1u));
+        }
+    }
+    __syncthreads();
+
+    if (!build_patch(S, ctl, arena)) return false;
+
+    // ------------------------------------------------ C: gather + blend
+    const float4 *patch = reinterpret_cast<const float4 *>(arena + (((size_t)ctl.nacc * 8 + 15) & ~(size_t)15));
+#pragma unroll
+    for (int p = 0; p < PPL; ++p)
+        if (pt[p].uv != kNone) {
+            const int iu = (int)(pt[p].uv & 0xFFF) - bu0, iv = (int)((pt[p].uv >> 12) & 0xFFF) - bv0;
+            const int s0 = (int)(pt[p].st & 0x3FFF), t0 = (int)((pt[p].st >> 14) & 0x3FFF);
+            const int du = (int)((pt[p].uv >> 24) & 1u), dv = ((pt[p].uv >> 25) & 1u) ? nu : 0;
+            const int ds = (int)((pt[p].st >> 28) & 1u), dt = (int)((pt[p].st >> 29) & 1u);
+            const int vw0 = iv * nu + iu;
+            int vb[4], vs[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const int2 cb = ctl.vcb[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
+                vb[a] = cb.x + t0 * cb.y + s0;
+                vs[a] = dt ? cb.y : 0;
+            }
+            rgb[p] = blend16(pt[p], [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
+        }
+    return true;
+}
+
+// ---------------------------------------------------------------- stores
+__device__ __forceinline__ void store4(uint8_t *__restrict__ out, int view, int W, int H, int x0, int y, const uint32_t (&rgb)[4], int out_aligned)
+{
+    if (y >= H || x0 >= W) return;
+    uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x0);
+    if (out_aligned && x0 + 4 <= W) {  // 12 contiguous bytes per thread
+        uint32_t *o32 = reinterpret_cast<uint32_t *>(o);
+        o32[0] = rgb[0] | (rgb[1] << 24);
+        o32[1] = (rgb[1] >> 8) | (rgb[2] << 16);
+        o32[2] = (rgb[2] >> 16) | (rgb[3] << 8);
+    } else {
+#pragma unroll
+        for (int p = 0; p < 4; ++p)
+            if (x0 + p < W) {
+                o[3 * p + 0] = (uint8_t)(rgb[p] & 0xFF);
+                o[3 * p + 1] = (uint8_t)((rgb[p] >> 8) & 0xFF);
+                o[3 * p + 2] = (uint8_t)((rgb[p] >> 16) & 0xFF);
+            }
+    }
+}
+
+// one pixel per lane, 4 consecutive lanes = 4 consecutive pixels of a row: their 12 bytes leave as three 32-bit words
+__device__ __forceinline__ void store1(uint8_t *__restrict__ out, int view, int W, int H, int x, int y, bool active, uint32_t rgb, int out_aligned)
+{
+    const uint32_t nb = __shfl_down_sync(FULL, rgb, 1);
+    if (!active || y >= H || x >= W) return;
+    uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x);
+    if (out_aligned) {  // W % 4 == 0 and x % 4 == lane % 4: the group's 4 pixels are all inside the view
+        const int j = x & 3;
+        if (j < 3) {
+            const uint32_t w = j == 0 ? (rgb | (nb << 24)) : j == 1 ? ((rgb >> 8) | (nb << 16)) : ((rgb >> 16) | (nb << 8));
+            reinterpret_cast<uint32_t *>(o - 3 * j)[j] = w;
+        }
+    } else {
+        o[0] = (uint8_t)(rgb & 0xFF);
+        o[1] = (uint8_t)((rgb >> 8) & 0xFF);
+        o[2] = (uint8_t)((rgb >> 16) & 0xFF);
+    }
+}
+
+__global__ void __launch_bounds__(kNT, kMinBlocks)
+render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned)
+{
+    extern __shared__ __align__(16) unsigned char arena[];
+    __shared__ Ctl ctl;
+    const int tid = threadIdx.x;
+    const int ox = blockIdx.x * kTile, oy = blockIdx.y * kTile;
+    const int view = blockIdx.z;
+
+    for (int q = tid; q < 192; q += kNT)
+        reinterpret_cast<uint32_t *>(ctl.lut)[q] = reinterpret_cast<const uint32_t *>(g_cta_digit_lut.v)[q];
+    const Camera cam = cams[view];
+    const uint32_t bg = (uint32_t)S.bg[0] | ((uint32_t)S.bg[1] << 8) | ((uint32_t)S.bg[2] << 16);
+
+    // ---------------------------------------------------------------- passes: the whole 32 x 32 tile (4 pixels per thread); if it does
+    // not fit, its 16 x 16 quadrants, each split again into 8 x 8 when it does not fit (low
+    // magnification: more light-field samples than output pixels under the tile); an 8 x 8 sub-tile that still does not fit
+    // (strong minification) is rendered by 16 direct sample decodes per pixel
+    int q = -1, r = -1;  // q < 0: whole tile; r < 0: 16 x 16 quadrant q; r = 0..3: its 8 x 8 quadrants
+    while (q < 4) {
+        const int ts = q < 0 ? kTile : (r < 0 ? 16 : 8);
+        const int sx = q < 0 ? ox : ox + (q & 1) * 16 + (r < 0 ? 0 : (r & 1) * 8);
+        const int sy = q < 0 ? oy : oy + (q >> 1) * 16 + (r < 0 ? 0 : (r >> 1) * 8);
+        bool done = true;
+        if (sx < W && sy < H) {
+            PixTaps pt[kPPL];
+            uint32_t rgb[kPPL];
+#pragma unroll
+            for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
+            setup_rays(S, cam, W, H, sx, sy, ts, pt);
+            done = tile_pass(S, ctl, arena, pt, rgb);
+            if (!done && r >= 0) {
+                if (pt[0].uv != kNone) rgb[0] = direct_pixel(S, pt[0]);
+                done = true;
+            }
+            if (done) {
+                int x0, y, npix;
+                thread_pixel(sx, sy, ts, x0, y, npix);
+                if (q < 0) store4(out, view, W, H, x0, y, rgb, out_aligned);
+                else store1(out, view, W, H, x0, y, npix > 0, rgb[0], out_aligned);
+            }
+        }
+        if (q < 0) q = done ? 4 : 0;
+        else if (r < 0) { if (done) ++q; else r = 0; }
+        else if (++r == 4) { r = -1; ++q; }
+    }
+}
 
 }  // namespace
 
 cudaError_t configure_render_cta()
 {
-    return cudaFuncSetAttribute(render_cta_kernel<kArenaBytes, kMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaBytes);
+    return cudaFuncSetAttribute(render_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaBytes);
 }
 
 cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
@@ -716,7 +797,7 @@ cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_vi
     dim3 block(kNT), grid((unsigned)((W + kTile - 1) / kTile), (unsigned)((H + kTile - 1) / kTile), (unsigned)n_views);
     if (grid.y > 65535u) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0 && (W % 4) == 0) ? 1 : 0;
-    render_cta_kernel<kArenaBytes, kMinBlocks><<<grid, block, kArenaBytes, st>>>(S, d_cams, W, H, d_out, aligned);
+    render_cta_kernel<<<grid, block, kArenaBytes, st>>>(S, d_cams, W, H, d_out, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
