@@ -103,6 +103,30 @@ def _physical_gpu_index(local_rank):
     return local_rank
 
 
+def reduce_max(x, world, device="cpu"):
+    """Max over ranks of a per-rank duration (the contract's max-over-ranks timing); identity at world 1."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(x)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank_per_step, steps, world, seconds):
+    """Weak scaling: every rank processes its own batch; value = units of ALL ranks / max-over-ranks time."""
+    return world * units_per_rank_per_step * steps / seconds
+
+
+def rank_cameras(cfg, rank):
+    """The view batch of one rank: its own arc of the seeded circular camera path (no exchange between ranks)."""
+    import workloads as wl
+
+    return wl.camera_path(cfg, seed_offset=rank)
+
+
 def _get_stream(name, rank, world, barrier):
     """Rank 0 encodes (oracle encoder, input preparation) into the on-disk cache; the others read it."""
     from oracle import streams
@@ -205,7 +229,7 @@ def run_ours(args, cfg_name):
         P.hmlfc_set_decode_variant(h, args.decode_variant)
     W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
     # weak scaling: every rank renders a full batch, each on its own arc of the camera circle
-    cams_np = wl.camera_path(cfg, seed_offset=rank)
+    cams_np = rank_cameras(cfg, rank)
     cams = torch.from_numpy(cams_np).cuda()
     out = torch.empty((V, H, W, 3), dtype=torch.uint8, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
@@ -235,24 +259,16 @@ def run_ours(args, cfg_name):
     with ClockSampler(_physical_gpu_index(local_rank)) as clk:
         ms = timed(step, args.steps, args.warmup)
     launches = P.hmlfc_launch_count(h) - n0 - args.warmup
-    total_ms = float(sum(ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    views_per_s = world * V * args.steps / (total_ms * 1e-3)
+    total_ms = reduce_max(sum(ms), world, "cuda")
+    views_per_s = whole_job_rate(V, args.steps, world, total_ms * 1e-3)
 
     # ---- decode leg: seeded uniformly random LF coordinates (inputs larger than L2)
     n_dec = cfg.n_decode
     coords = torch.from_numpy(wl.random_coords(cfg, n_dec, seed_offset=rank)).cuda()
     dec_out = torch.empty((n_dec, 3), dtype=torch.uint8, device="cuda")
     dec_ms = timed(lambda: P.hmlfc_decode(h, coords, out=dec_out, stream=stream), max(3, min(args.steps, 10)), 3)
-    dec_total = float(sum(dec_ms))
-    if world > 1:
-        t = torch.tensor([dec_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dec_total = float(t.item())
-    dec_px_per_s = world * n_dec * len(dec_ms) / (dec_total * 1e-3)
+    dec_total = reduce_max(sum(dec_ms), world, "cuda")
+    dec_px_per_s = whole_job_rate(n_dec, len(dec_ms), world, dec_total * 1e-3)
 
     # ---- end to end through the C ABI with HOST (pinned) buffers: cameras H2D + views D2H inside the timed region
     cams_pin = torch.from_numpy(cams_np).pin_memory()
@@ -265,12 +281,8 @@ def run_ours(args, cfg_name):
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         P.hmlfc_render_host(h, cams_pin.numpy(), W, H, out=out_pin.numpy())   # synchronises before returning
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_views_per_s = world * V * e2e_steps / e2e_s
+    e2e_s = reduce_max(time.perf_counter() - t0, world, "cuda")
+    e2e_views_per_s = whole_job_rate(V, e2e_steps, world, e2e_s)
     assert torch.equal(out_pin.cuda(), out), "host entry point and device entry point disagree"
 
     if rank == 0:
