@@ -296,7 +296,7 @@ def run_ours(args, cfg_name):
         dec_achieved = fpd["bytes_alg"] / (dec_kernel_ms * 1e-3) / 1e9
         roofline = {
             "bound": "hbm", "kernel": {1: "render_pixel_kernel", 2: "render_tiled_kernel", 3: "render_blocks_kernel", 4: "render_warp_kernel", 5: "render_warp_kernel"}.get(args.variant, "render_cta_kernel"), "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": _traffic_from_profiles("render"), "peak_source": peak_src,
+            "traffic": _ncu_from_profiles(cfg.name, "render").get("dram_bytes"), "peak_source": peak_src,
             "bytes_alg_per_launch": fp["bytes_alg"], "out_bytes": fp["out_bytes"],
             "compressed_bytes_touched": fp["bytes_alg"] - fp["out_bytes"] - fp["in_bytes"],
             "kernel_ms": kernel_ms, "frac_of_8TBs": achieved / 8000.0,
@@ -305,8 +305,12 @@ def run_ours(args, cfg_name):
             "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
             "roofline": {"bound": "hbm", "kernel": "decode_kernel" if args.decode_variant == 1 else "decode_queue_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
                          "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
-                         "traffic": _traffic_from_profiles("decode")},
+                         "traffic": _ncu_from_profiles(cfg.name, "decode").get("dram_bytes")},
         }
+        clocks = clk.summary()
+        roofline["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "render").get("warp_inst"), kernel_ms, clocks.get("sm_mhz"))
+        decode["roofline"]["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "decode").get("warp_inst"), dec_kernel_ms,
+                                              clocks.get("sm_mhz"))
         # ---- the oracle timed beside it, on a bounded sample of the same batch
         import oracle as orc
 
@@ -323,7 +327,7 @@ def run_ours(args, cfg_name):
             "e2e": {"value": e2e_views_per_s, "unit": "views/s", "h2d_bytes_per_step": int(cams_np.nbytes),
                     "d2h_bytes_per_step": int(out_pin.numel()), "steps": e2e_steps},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "decode": decode,
-            "output_px_per_s": views_per_s * W * H, "clocks": clk.summary(),
+            "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),
             "paper_context": "~200 fps at 512x512 on a GTX-980, Lego Knights (PAPER.md:409): another machine and light field, not the target",
         }
@@ -333,16 +337,28 @@ def run_ours(args, cfg_name):
         dist.destroy_process_group()
 
 
-def _traffic_from_profiles(which):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture, if any."""
+def _ncu_from_profiles(cfg_name, which):
+    """Per-launch counters of the committed `ncu --set full` capture of this configuration (profiles/traffic.json, written
+    from profiles/*.md): {"dram_bytes": dram__bytes_read.sum + dram__bytes_write.sum, "warp_inst": smsp__inst_executed.sum}
+    or {} when there is no capture for the configuration."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
         try:
             with open(path) as fh:
-                return json.load(fh).get(which)
+                return json.load(fh).get(cfg_name, {}).get(which, {}) or {}
         except Exception:
-            return None
-    return None
+            return {}
+    return {}
+
+
+def _alu_view(warp_inst, kernel_ms, sm_mhz, n_sms=148):
+    """Issue-slot view of a kernel: executed warp-instructions per second against n_sms x 4 schedulers x SM clock."""
+    if not warp_inst or not sm_mhz:
+        return None
+    peak = n_sms * 4 * sm_mhz * 1e6
+    achieved = warp_inst / (kernel_ms * 1e-3)
+    return {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G warp-instr/s", "frac": achieved / peak,
+            "warp_inst_per_launch": warp_inst, "source": "smsp__inst_executed.sum of the committed ncu capture (profiles/)"}
 
 
 def main():
