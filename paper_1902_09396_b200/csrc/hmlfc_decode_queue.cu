@@ -77,6 +77,13 @@ __device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint
     return (dig << m) | low;
 }
 
+// 256-bit load (LDG.E.ENL2.256, sm_100a): two adjacent 16-byte records of a 32-byte aligned pair in one request
+__device__ __forceinline__ void ldg256(const uint4 *__restrict__ p, uint4 &a, uint4 &b)
+{
+    asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+}
+
 constexpr uint32_t kSignBit = 1u << 23;  // value task: subtract (additive / "phase-shifted" mode, R10)
 
 // push one task per flagged lane on a warp stack; cnt is warp-uniform
@@ -119,7 +126,7 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
         if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {  // R8: outside the image reads 0
             const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
             const uint4 rd = ldg(S.pc + t.z);
-            const uint4 fr = ldg(S.flagrec + (size_t)t.z * (size_t)S.fgroups + (size_t)(b >> 5));
+            const uint4 fr = ldg(S.flagrec + flag_index(S, t.z, (uint32_t)(b >> 5)));
             const uint32_t bit = 1u << (b & 31);
             has = (fr.x & bit) != 0u;
             const uint32_t rank = fr.y + (uint32_t)__popc(fr.x & (bit - 1u));
@@ -164,7 +171,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
 
     const int b = valid ? (y >> S.logB) * S.nbx + (x >> S.logB) : 0;
     const uint32_t bit = 1u << (b & 31);
-    const size_t fg = (size_t)(b >> 5);
+    const uint32_t fg = (uint32_t)(b >> 5);
     const uint32_t kin = (uint32_t)(((y & (S.B - 1)) << S.logB) + (x & (S.B - 1)));
     int vcnt = 0, mcnt = 0;
 
@@ -177,13 +184,16 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
         const bool predictive = ((pu | pv) & 1) != 0;
         // S4: the three channels' descriptors and flag records, six independent loads
         uint4 d[3], fr[3];
+        // S4: the three channels' descriptors and their flag records; the records share one 64-byte slot: a 256-bit
+        // load (Y, Co) and a 128-bit load (Cg)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            d[c] = fr[c] = make_uint4(0u, 0u, 0u, 0u);
-            if (valid) {
-                d[c] = ldg(S.pc + base + c);
-                fr[c] = ldg(S.flagrec + (size_t)(base + c) * (size_t)S.fgroups + fg);
-            }
+        for (int c = 0; c < 3; ++c) d[c] = fr[c] = make_uint4(0u, 0u, 0u, 0u);
+        if (valid) {
+            const uint4 *slot = S.flagrec + flag_index(S, base, fg);
+            ldg256(slot, fr[0], fr[1]);
+            fr[2] = ldg(slot + 2);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) d[c] = ldg(S.pc + base + c);
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) {

@@ -13,7 +13,9 @@
 //              MV word base, offset:16 | layout:2 | m:4 | predictive:1}; the three channels of a
 //              plane are adjacent (48 bytes)
 //   flagrec[]  one 16-byte record per 32 blocks of a plane-channel: {res bits, res rank before,
-//              pred bits, pred rank before} -- flag test and rank come from ONE 128-bit load
+//              pred bits, pred rank before} -- flag test and rank come from ONE 128-bit load.  The records of
+//              the three channels of a (plane, group) share one 64-byte slot {Y, Co, Cg, spare}: a random
+//              sample touches one HBM access granule per level instead of three (profiles/r01_cfg5.md)
 //   pay[], mv[] bit-packed BISE strings as streamed (LSB-first 32-bit words), addressed in O(1)
 //   rkv[]      top-level RKVs as short4 {Y, Co, Cg, 0} per sample: one 64-bit load per sample
 #pragma once
@@ -94,6 +96,13 @@ HMLFC_DEV uint32_t umulhi(uint32_t a, uint32_t b)
 #endif
 }
 
+// index of the flag record of plane-channel k (= 3 * plane + channel), 32-block group g; equals pc[k].x + 4 g
+HMLFC_DEV size_t flag_index(const DevStream &S, uint32_t k, uint32_t g)
+{
+    const uint32_t p = umulhi(k, 0xAAAAAAABu) >> 1;  // k / 3
+    return ((size_t)p * (size_t)S.fgroups + (size_t)g) * 4u + (size_t)(k - 3u * p);
+}
+
 // descriptor fields
 HMLFC_DEV int pc_offset(uint32_t w) { return (int)(int16_t)(w & 0xFFFFu); }
 HMLFC_DEV uint32_t pc_layout(uint32_t w) { return (w >> 16) & 3u; }
@@ -151,7 +160,7 @@ HMLFC_DEV int reference_value(const DevStream &S, uint4 d, int rx, int ry)
 {
     if ((unsigned)rx >= (unsigned)S.Ws || (unsigned)ry >= (unsigned)S.Ht) return 0;
     int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
-    uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+    uint4 fr = ldg(S.flagrec + d.x + 4u * (uint32_t)(b >> 5));
     int kin = ((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1));
     return stored_value(S, d, fr, 1u << (b & 31), kin);
 }
@@ -187,8 +196,8 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             uint4 d = ldg(S.pc + base + c);
-            // the flag record of plane-channel k starts at k * fgroups (= d.x): both loads issue at once
-            uint4 fr = ldg(S.flagrec + (size_t)(base + c) * (size_t)S.fgroups + fg);
+            // the flag record's index follows from the plane-channel index (= d.x + 4 fg): both loads issue at once
+            uint4 fr = ldg(S.flagrec + flag_index(S, base + (uint32_t)c, fg));
             int e = stored_value(S, d, fr, bit, kin);
             if (predictive && (fr.z & bit)) {
                 uint32_t mi = fr.w + popc(fr.z & (bit - 1u));

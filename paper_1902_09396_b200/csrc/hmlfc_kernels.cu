@@ -135,7 +135,7 @@ __device__ void touch_sample(const DevStream &S, FootprintMarks mk, int u, int v
             mark_bit(mk.blk, (size_t)(base + c) * (size_t)S.nblk + (size_t)b);
             if (!((pu | pv) & 1)) continue;
             uint4 d = ldg(S.pc + base + c);
-            uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+            uint4 fr = ldg(S.flagrec + d.x + 4u * (uint32_t)(b >> 5));
             if (!(fr.z & bit)) continue;
             uint32_t rec = bise_decode_at(S.mv + d.z, fr.w + popc(fr.z & (bit - 1u)), S.mv_layout, S.mv_m);
             int mode, dx, dy;
@@ -189,7 +189,7 @@ __global__ void footprint_reduce_blocks_kernel(const DevStream S, unsigned long 
         }
         if (marks) {
             uint4 d = ldg(S.pc + k);
-            uint4 fr = ldg(S.flagrec + d.x + g);
+            uint4 fr = ldg(S.flagrec + d.x + 4u * g);
             const bool isp = pc_is_pred(d.w);
             blocks = popc(marks);
             flag_bits = blocks * (isp ? 2u : 1u);

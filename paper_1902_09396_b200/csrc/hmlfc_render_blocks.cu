@@ -260,7 +260,7 @@ render_blocks_kernel(const DevStream S, const Camera *__restrict__ cams, int W, 
                 const uint4 d = ldg(S.pc + si.x + c);
                 const int bx = cx.bx0 + (int)ib, by = cx.by0 + (int)jb;
                 const int b = by * S.nbx + bx;
-                const uint4 fr = ldg(S.flagrec + (size_t)(si.x + c) * (size_t)S.fgroups + (size_t)(b >> 5));  // = d.x + ..., without waiting for d
+                const uint4 fr = ldg(S.flagrec + flag_index(S, si.x + (uint32_t)c, (uint32_t)(b >> 5)));  // = d.x + ..., without waiting for d
                 const uint32_t bit = 1u << (b & 31);
                 const bool res = (fr.x & bit) != 0u, pred = si.w && (fr.z & bit);
                 keep = res || pred;
@@ -344,7 +344,7 @@ render_blocks_kernel(const DevStream S, const Camera *__restrict__ cams, int W, 
                     if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {
                         const uint4 d = ldg(S.pc + r1.y);
                         const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
-                        const uint4 fr = ldg(S.flagrec + d.x + (uint32_t)(b >> 5));
+                        const uint4 fr = ldg(S.flagrec + d.x + 4u * (uint32_t)(b >> 5));
                         const uint32_t bit = 1u << (b & 31);
                         if (fr.x & bit) {
                             const uint32_t ii = ((fr.y + popc(fr.x & (bit - 1u))) << (2 * S.logB)) +

@@ -392,7 +392,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
             const int r = it - sl.itembase;
             const int c = r / sl.nbh, jr = r - c * sl.nbh;
             d = ldg(S.pc + sl.pc0 + c);
-            frbase = (size_t)(sl.pc0 + (uint32_t)c) * (size_t)S.fgroups;  // = d.x, without waiting for d
+            frbase = flag_index(S, sl.pc0 + (uint32_t)c, 0u);  // = d.x, without waiting for d
             refpc = sl.refpc0 + (uint32_t)c;
             sc = ((uint32_t)s << 22) | ((uint32_t)c << 28);
             pred = sl.pred;
@@ -407,7 +407,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
             uint4 fr = make_uint4(0u, 0u, 0u, 0u);
             const int g = (b0 >> 5) + gi;
             if (gi < ng) {
-                fr = ldg(S.flagrec + frbase + (size_t)g);
+                fr = ldg(S.flagrec + frbase + 4u * (size_t)g);
                 const int lo = max(b0 - (g << 5), 0), hi = min(b1 - (g << 5), 31);
                 const uint32_t mask = (0xFFFFFFFFu >> (31 - hi)) & (0xFFFFFFFFu << lo);
                 resb = fr.x & mask;
@@ -486,13 +486,13 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
                 uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
                 if ((unsigned)bxa < (unsigned)S.nbx) {
                     const int b = rowb + bxa;
-                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                    const uint4 fr = ldg(S.flagrec + r1.x + 4u * (uint32_t)(b >> 5));
                     const uint32_t bit = 1u << (b & 31);
                     if (fr.x & bit) qa = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
                 }
                 if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
                     const int b = rowb + bxa + 1;
-                    const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                    const uint4 fr = ldg(S.flagrec + r1.x + 4u * (uint32_t)(b >> 5));
                     const uint32_t bit = 1u << (b & 31);
                     if (fr.x & bit) qb = bise_row4(S.pay + r1.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, r1.z, ctl.lut);
                 }

@@ -345,7 +345,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                             const uint4 si = ws.slotinfo[slot];
                             const uint4 d = ldg(S.pc + si.x + c);
                             const int b = (by0 + (int)jb) * S.nbx + bx0 + (int)ib;
-                            const uint4 fr = ldg(S.flagrec + (size_t)(si.x + c) * (size_t)S.fgroups + (size_t)(b >> 5));  // = d.x + ..., without waiting for d
+                            const uint4 fr = ldg(S.flagrec + flag_index(S, si.x + (uint32_t)c, (uint32_t)(b >> 5)));  // = d.x + ..., without waiting for d
                             const uint32_t bit = 1u << (b & 31);
                             const bool res = (fr.x & bit) != 0u, pred = si.z && (fr.z & bit);
                             keep = res || pred;
@@ -414,7 +414,7 @@ render_warp_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
                             const bool inb = pred && (unsigned)rx < (unsigned)S.Ws && (unsigned)ryy < (unsigned)S.Ht;
                             const int rxc = inb ? rx : 0, ryc = inb ? ryy : 0;
                             const int b = (ryc >> logB) * S.nbx + (rxc >> logB);
-                            const uint4 fr = ldg(S.flagrec + r1.x + (uint32_t)(b >> 5));
+                            const uint4 fr = ldg(S.flagrec + r1.x + 4u * (uint32_t)(b >> 5));
                             const uint32_t vown = bise_at_uniform(S.pay + (own ? r0.x : 0u), own ? r0.y + kin : 0u, pc_layout(r0.z), pc_m(r0.z), lut);
                             const uint32_t bit = 1u << (b & 31);
                             const bool hasq = inb && (fr.x & bit) != 0u;

@@ -144,7 +144,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     try {
         T.pc.resize(n_pc);
         T.bits15.resize(n_pc);
-        T.flagrec.resize(n_pc * (uint64_t)D.fgroups);
+        T.flagrec.assign((n_pc / 3) * (uint64_t)D.fgroups * 4, make_uint4(0u, 0u, 0u, 0u));  // 64-byte slot per (plane, group): Y, Co, Cg, spare
         T.rkv.resize(n_top * npx);
     } catch (const std::bad_alloc &) {
         return HMLFC_E_NOMEM;
@@ -171,7 +171,9 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                         pboff + bise_nbits(layout, m, (uint64_t)n_res * BB) > pay_bits ||
                         mboff + bise_nbits(D.mv_layout, D.mv_m, n_pred) > mv_bits || (!is_pred && n_pred != 0))
                         return HMLFC_E_CORRUPT;
-                    T.pc[k] = make_uint4((uint32_t)(k * (uint64_t)D.fgroups), (uint32_t)(pboff / 32), (uint32_t)(mboff / 32),
+                    const uint64_t frbase = (k / 3) * (uint64_t)D.fgroups * 4 + (k % 3);  // record of group g: frbase + 4 g
+                    if (frbase + 4ull * (uint64_t)D.fgroups > 0xFFFFFFFFull) return HMLFC_E_UNSUPPORTED;
+                    T.pc[k] = make_uint4((uint32_t)frbase, (uint32_t)(pboff / 32), (uint32_t)(mboff / 32),
                                          ((uint32_t)offset & 0xFFFFu) | (layout << 16) | (m << 18) | ((is_pred ? 1u : 0u) << 22));
                     T.bits15[k] = bise_bits15(layout, m);
                     const uint8_t *fres = s + off_flags + foff;
@@ -183,7 +185,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                             const uint32_t mask = (1u << (D.nblk & 31)) - 1u;
                             wr &= mask; wp &= mask;
                         }
-                        T.flagrec[k * (uint64_t)D.fgroups + g] = make_uint4(wr, rr, wp, rp);
+                        T.flagrec[frbase + 4ull * (uint64_t)g] = make_uint4(wr, rr, wp, rp);
                         rr += popcount32(wr);
                         rp += popcount32(wp);
                     }
