@@ -285,6 +285,17 @@ def run_ours(args, cfg_name):
     e2e_views_per_s = whole_job_rate(V, e2e_steps, world, e2e_s)
     assert torch.equal(out_pin.cuda(), out), "host entry point and device entry point disagree"
 
+    # ---- encoder-side leg (SURVEY 8(f) first "next" row): phase-shifted exhaustive search of one level-0 channel
+    sU, sV = min(cfg.U, 16), min(cfg.V, 16)  # at most a 16 x 16 sub-grid of planes per launch
+    srv = torch.from_numpy(wl.srv_like_planes(cfg, sU * sV, seed_offset=rank)).cuda()
+    pairs_np = wl.cluster_pairs(sU, sV)
+    pairs_d = torch.from_numpy(pairs_np).cuda()
+    mv_out = torch.empty((len(pairs_np), cfg.Ht // cfg.block, cfg.Ws // cfg.block, 4), dtype=torch.int32, device="cuda")
+    se_ms = timed(lambda: P.hmlfc_search(srv, pairs_d, cfg.block, cfg.window, out=mv_out, stream=stream), 5, 3)
+    se_total = reduce_max(sum(se_ms), world, "cuda")
+    n_blocks_search = len(pairs_np) * (cfg.Ht // cfg.block) * (cfg.Ws // cfg.block)
+    del srv
+
     if rank == 0:
         # ---- roofline of the dominant kernel: algorithmic bytes per launch / average launch time
         peak, peak_src = _peaks()
@@ -311,6 +322,19 @@ def run_ours(args, cfg_name):
         roofline["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "render").get("warp_inst"), kernel_ms, clocks.get("sm_mhz"))
         decode["roofline"]["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "decode").get("warp_inst"), dec_kernel_ms,
                                               clocks.get("sm_mhz"))
+        # search: 2 exact fp32 adds per sample, mode and offset (Eqs. 1-2): a plain-ALU bound, 128 FP32 lanes per SM
+        nd2 = (2 * cfg.window + 1) ** 2
+        se_adds = n_blocks_search * nd2 * cfg.block * cfg.block * 2 * 2
+        se_kernel_ms = float(np.mean(se_ms))
+        se_peak = 148 * 128 * (clocks.get("sm_mhz") or 1965.0) * 1e6
+        search = {
+            "value": whole_job_rate(n_blocks_search, len(se_ms), world, se_total * 1e-3), "unit": "blocks/s",
+            "blocks_per_launch": n_blocks_search, "pairs": int(len(pairs_np)), "ms_per_launch": se_kernel_ms,
+            "workload": f"level-0 planes of one channel ({sU}x{sV} x {cfg.Ws}x{cfg.Ht}, SRV-like synthetic int16), B={cfg.block}, W={cfg.window}",
+            "roofline": {"bound": "alu", "kernel": "search4_kernel", "achieved": se_adds / (se_kernel_ms * 1e-3) / 1e12,
+                         "peak": se_peak / 1e12, "unit": "T fp32 add/s", "frac": se_adds / (se_kernel_ms * 1e-3) / se_peak,
+                         "peak_source": "148 SMs x 128 FP32 lanes x SM clock (DESIGN.md 9.6)"},
+        }
         # ---- the oracle timed beside it, on a bounded sample of the same batch
         import oracle as orc
 
@@ -326,7 +350,7 @@ def run_ours(args, cfg_name):
             "config": _config_dict(cfg, info, f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB fill)"),
             "e2e": {"value": e2e_views_per_s, "unit": "views/s", "h2d_bytes_per_step": int(cams_np.nbytes),
                     "d2h_bytes_per_step": int(out_pin.numel()), "steps": e2e_steps},
-            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "decode": decode,
+            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "decode": decode, "search": search,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),
             "paper_context": "~200 fps at 512x512 on a GTX-980, Lego Knights (PAPER.md:409): another machine and light field, not the target",

@@ -137,6 +137,20 @@ int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
  * motion-record and BISE value decodes run as 32-wide batches from per-warp task stacks). */
 int hmlfc_set_decode_variant(hmlfc_handle *h, int variant);
 
+/* Encoder side (first "next" row): phase-shifted exhaustive block motion search, PAPER.md:227-248,
+ * Eqs. (1)-(2).  For pair k = (p, r) = d_pairs[k] and every block x block block of plane p, over all motion vectors
+ * (dx, dy) in [-window, window]^2:
+ *     Delta-(dx,dy) = sum |P(x,y) - R(x+dx, y+dy)|,   Delta+(dx,dy) = sum |P(x,y) + R(x+dx, y+dy)|,
+ * R reading 0 outside the image; the result is the minimum over both modes, ties resolved subtractive before additive
+ * ("phase-shifted"), then smallest dy, then smallest dx (R8, R9).
+ *   d_planes  device, int16 [n_planes][Ht][Ws] (SRV images of one level and channel, any order)
+ *   d_pairs   device, int32 [n_pairs][2] = (index of the predictive plane, index of its reference plane)
+ *   d_out     device, int32 [n_pairs][Ht/block][Ws/block][4] = mode (0 subtractive, 1 additive), dx, dy, Delta
+ * Needs no handle (the encoder has no stream yet).  Enqueues on cuda_stream and returns; block in 1..8 must divide
+ * Ws and Ht, window <= 64, n_pairs <= 65535, else HMLFC_E_UNSUPPORTED.  Integer-exact for any int16 input. */
+int hmlfc_search(const int16_t *d_planes, const int32_t *d_pairs, int n_pairs, int Ws, int Ht, int block, int window,
+                 int32_t *d_out, void *cuda_stream);
+
 /* Number of kernels this library has launched through the handle since load (bench accounting). */
 int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);
 

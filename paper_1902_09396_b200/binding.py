@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -77,6 +77,8 @@ def lib():
     L.hmlfc_footprint_decode.argtypes, L.hmlfc_footprint_decode.restype = [vp, vp, i64, C.POINTER(Footprint)], C.c_int
     L.hmlfc_set_render_variant.argtypes, L.hmlfc_set_render_variant.restype = [vp, C.c_int], C.c_int
     L.hmlfc_set_decode_variant.argtypes, L.hmlfc_set_decode_variant.restype = [vp, C.c_int], C.c_int
+    L.hmlfc_search.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
+    L.hmlfc_search.restype = C.c_int
     L.hmlfc_launch_count.argtypes, L.hmlfc_launch_count.restype = [vp, C.POINTER(i64)], C.c_int
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
@@ -220,6 +222,21 @@ def hmlfc_set_render_variant(h: Handle, variant: int):
 
 def hmlfc_set_decode_variant(h: Handle, variant: int):
     _check(lib().hmlfc_set_decode_variant(h._h, variant), "hmlfc_set_decode_variant")
+
+
+def hmlfc_search(planes, pairs, block: int, window: int, out=None, stream=None):
+    """planes: cuda int16 [n_planes][Ht][Ws]; pairs: cuda int32 [n_pairs][2]; returns cuda int32 [n_pairs][Ht/B][Ws/B][4]."""
+    torch = _require_cuda()
+    assert planes.is_cuda and planes.dtype == torch.int16 and planes.is_contiguous() and planes.dim() == 3
+    assert pairs.is_cuda and pairs.dtype == torch.int32 and pairs.is_contiguous() and pairs.dim() == 2 and pairs.shape[1] == 2
+    n_pairs, Ht, Ws = int(pairs.shape[0]), int(planes.shape[1]), int(planes.shape[2])
+    if out is None:
+        out = torch.empty((n_pairs, Ht // max(block, 1), Ws // max(block, 1), 4), dtype=torch.int32, device=planes.device)
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().hmlfc_search(C.c_void_p(planes.data_ptr()), C.c_void_p(pairs.data_ptr()), n_pairs, Ws, Ht, block, window,
+                              C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream)), "hmlfc_search")
+    return out
 
 
 def hmlfc_launch_count(h: Handle) -> int:

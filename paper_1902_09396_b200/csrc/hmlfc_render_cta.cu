@@ -224,8 +224,16 @@ __device__ __forceinline__ uint2 bise_row4(const uint32_t *__restrict__ w, uint3
     return make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
 }
 
-constexpr int kArenaBytes = 50 * 1024;
-constexpr int kMinBlocks = 4;
+#ifndef HMLFC_ARENA_KB
+#define HMLFC_ARENA_KB 68
+#endif
+#ifndef HMLFC_MINB
+#define HMLFC_MINB 3
+#endif
+constexpr int kArenaBytes = HMLFC_ARENA_KB * 1024;  // 3 CTAs per SM: 3 x (68 KB + 6 KB static) of the 228 KB, up to 85 registers per thread.
+// Measured (A/B on cfg2 / cfg3 / cfg4): 4 x 50 KB: 0.865 / 1.034 / 1.073 ms, 3 x 68 KB: 0.858 / 0.971 / 1.064 ms, 2 x 104 KB: 0.968 / 0.837 /
+// 1.228 ms, 5 x 38 KB: 1.062 / 1.218 / 1.321 ms -- the kernel is not occupancy-bound; fewer spills and fewer split tiles win.
+constexpr int kMinBlocks = HMLFC_MINB;
 #ifndef HMLFC_EST_SLACK
 #define HMLFC_EST_SLACK 120
 #endif

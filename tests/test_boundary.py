@@ -76,6 +76,10 @@ def test_entry_points_validate_arguments(P):
     assert L.hmlfc_render(None, None, 0, 1, 1, None, None) == -4
     assert L.hmlfc_info(None, None) == -4
     L.hmlfc_free(None)  # no-op
+    assert L.hmlfc_search(None, None, 1, 8, 8, 4, 1, None, None) == -4      # null pointers
+    assert L.hmlfc_search(None, None, 0, 8, 8, 3, 1, None, None) == -5      # block does not divide the image
+    assert L.hmlfc_search(None, None, 0, 8, 8, 4, 65, None, None) == -5     # window > 64
+    assert L.hmlfc_search(None, None, 0, 8, 8, 4, 16, None, None) == 0      # nothing to do
 
 
 def test_no_cpu_fallback(P, enc):

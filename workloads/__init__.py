@@ -259,6 +259,31 @@ def random_coords(cfg: Config, n=None, seed_offset=0) -> np.ndarray:
     return out
 
 
+def srv_like_planes(cfg: Config, n_planes: int, seed_offset=0) -> np.ndarray:
+    """n_planes signed int16 images [n][Ht][Ws] with the statistics of SRV images (differences of neighbouring views:
+    zero-mean, a few tens in magnitude, locally coherent, each plane a shifted and sometimes sign-inverted copy of a
+    common signal plus noise).  Input of the encoder-side search timing; holds no HMLFC arithmetic."""
+    rng = np.random.Generator(np.random.PCG64(cfg.seed + 3000 + seed_offset))
+    pad = 16
+    base = rng.normal(0.0, 40.0, (cfg.Ht + 2 * pad, cfg.Ws + 2 * pad))
+    for _ in range(2):  # a little spatial coherence
+        base = 0.25 * (base + np.roll(base, 1, 0) + np.roll(base, 1, 1) + np.roll(base, (1, 1), (0, 1))) * 1.6
+    out = np.empty((n_planes, cfg.Ht, cfg.Ws), dtype=np.int16)
+    for k in range(n_planes):
+        dx, dy = rng.integers(-pad, pad + 1, 2)
+        sign = -1.0 if rng.uniform() < 0.45 else 1.0
+        img = sign * base[pad + dy:pad + dy + cfg.Ht, pad + dx:pad + dx + cfg.Ws] + rng.normal(0.0, 3.0, (cfg.Ht, cfg.Ws))
+        out[k] = np.clip(np.rint(img), -510, 510).astype(np.int16)
+    return out
+
+
+def cluster_pairs(UL: int, VL: int) -> np.ndarray:
+    """(predictive plane, reference plane) index pairs of a UL x VL level: the even-even member of every 2 x 2 cluster is
+    the reference of the other members (R5).  int32 [n][2], plane index = pv * UL + pu."""
+    return np.array([(pv * UL + pu, (pv & ~1) * UL + (pu & ~1)) for pv in range(VL) for pu in range(UL) if (pu | pv) & 1],
+                    dtype=np.int32).reshape(-1, 2)
+
+
 def all_coords(cfg: Config) -> np.ndarray:
     """Every LF pixel once, in [V][U][Ht][Ws] order (cfg1's exhaustive decode)."""
     v, u, t, s = np.meshgrid(np.arange(cfg.V), np.arange(cfg.U), np.arange(cfg.Ht), np.arange(cfg.Ws), indexing="ij")
