@@ -124,6 +124,30 @@ def test_render_matches_oracle(P, enc, name):
     _check_views(P, h, s, wl.camera_path(cfg), cfg.out_w, cfg.out_h)
 
 
+@pytest.mark.parametrize("name", ["mini_b2", "mini_b8"])
+def test_other_block_sizes_and_windows(P, enc, name):
+    """B = 2 / 8 and W = 5 / 8 streams (PAPER.md:389-405 sweeps the block size): decode bit-exact, views within 1 LSB, through
+    the automatic kernel choice (the 4 x 4-block CTA kernel does not apply) and the thread-per-pixel kernel."""
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    assert (h.info.block, h.info.window) == (cfg.block, cfg.window)
+    coords = wl.all_coords(cfg)
+    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE):
+        P.hmlfc_set_decode_variant(h, variant)
+        assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy().reshape(lf.shape), info["p1"])
+    P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
+    cams = wl.camera_path(cfg)
+    expect = s.render(cams, cfg.out_w, cfg.out_h)
+    outs = []
+    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_CTA):
+        P.hmlfc_set_render_variant(h, variant)
+        got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
+        assert np.abs(got.astype(np.int16) - expect.astype(np.int16)).max() <= TOL_VIEW, variant
+        outs.append(got)
+    P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
 @pytest.mark.parametrize("W,H", [(61, 37), (32, 8), (33, 9), (1, 1), (130, 5)])
 def test_render_ragged_output_sizes(P, enc, W, H):
     cfg, lf, data, info, s = enc("mini2")

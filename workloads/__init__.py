@@ -59,6 +59,9 @@ CONFIGS = {
     "mini2": Config("mini2", 8, 8, 96, 80, 3, 5, 2, 4.0, None, 48, 200, 136, 3, 50_000, seed=BASE_SEED + 12),
     "mini3": Config("mini3", 5, 5, 64, 48, 3, 4, 2, 6.0, None, 30, 100, 76, 2, 30_000, seed=BASE_SEED + 13),
     "mini4": Config("mini4", 16, 16, 64, 64, 4, 6, 3, 8.0, None, 48, 160, 120, 2, 50_000, seed=BASE_SEED + 14),
+    # other block sizes / search windows (the paper's Table 2 sweeps B = 2, 4, 8)
+    "mini_b2": Config("mini_b2", 4, 4, 48, 40, 2, 4, 1, 3.0, None, 12, 90, 70, 2, 20_000, seed=BASE_SEED + 15, block=2, window=5),
+    "mini_b8": Config("mini_b8", 5, 4, 64, 48, 2, 4, 2, 4.0, None, 160, 120, 88, 2, 20_000, seed=BASE_SEED + 16, block=8, window=8),
     # paper-regime sparsity: adjacent views < 1 px apart, as in the Stanford archive
     "cfg2_sparse": Config("cfg2_sparse", 16, 16, 256, 256, 3, 5, 2, 1.0, 40.0, 0, 512, 512, 64, 10 ** 7,
                           seed=BASE_SEED + 22),
