@@ -54,16 +54,12 @@ struct WarpQ {
     uint32_t stage[24];  // the warp's 96 output bytes
 };
 
-// bits [pos, pos+n) of an LSB-first 32-bit word string, n <= 16
-__device__ __forceinline__ uint32_t bits_at(const uint32_t *__restrict__ w, uint32_t pos, uint32_t n)
-{
-    const uint32_t *p = w + (pos >> 5);
-    return __funnelshift_r(__ldg(p), __ldg(p + 1), pos & 31u) & ((1u << n) - 1u);
-}
-
-// BISE decode_at (bit layout in DESIGN.md section 4) without control flow: plain = groups of one
-// value with an empty digit word, so lanes holding tasks of different layouts do not serialise.
-__device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint32_t i, uint32_t layout, uint32_t m,
+// BISE decode_at (bit layout in DESIGN.md section 4) of value i of the string that starts at word `base`
+// of `words`, without control flow: plain = groups of one value with an empty digit word, so lanes holding tasks of
+// different layouts do not serialise.  A group (<= 58 bits from any bit offset) lies in three consecutive words; they
+// are fetched as TWO aligned 64-bit loads (every lane-load of a random coordinate costs a sector-gather whatever its
+// width, profiles/r01_gather_probe.md), then the digit word and the value's m-bit field are cut out with funnel shifts.
+__device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ words, uint32_t base, uint32_t i, uint32_t layout, uint32_t m,
                                             const uint16_t *__restrict__ lut)
 {
     const bool plain = layout == 0u, trit = layout == 1u;
@@ -71,8 +67,15 @@ __device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ w, uint
     const uint32_t g = plain ? i : (trit ? (__umulhi(i, 0xCCCCCCCDu) >> 2) : (__umulhi(i, 0xAAAAAAABu) >> 1));
     const uint32_t k = i - G * g;
     const uint32_t gb = g * (hb + G * m);
-    const uint32_t head = bits_at(w, gb, hb);  // plain: 0 bits -> 0, and the quint table maps 0 to digit 0
-    const uint32_t low = bits_at(w, gb + hb + k * m, m);
+    const uint32_t wi = base + (gb >> 5), sh = gb & 31u;   // absolute word index of the group's first bit
+    const uint2 *p2 = reinterpret_cast<const uint2 *>(words + (wi & ~1u));
+    const uint2 A = __ldg(p2), B = __ldg(p2 + 1);          // words [wi & ~1, +4): covers wi .. wi + 2 (16 bytes of slack follow the string)
+    const bool odd = (wi & 1u) != 0u;
+    const uint32_t w0 = odd ? A.y : A.x, w1 = odd ? B.x : A.y, w2 = odd ? B.y : B.x;
+    const uint32_t head = __funnelshift_r(w0, w1, sh) & ((1u << hb) - 1u);  // plain: 0 bits -> 0, the quint table maps 0 to digit 0
+    const uint32_t pos = sh + hb + k * m;                  // <= 31 + 8 + 4 * 10: the field ends inside w2
+    const uint32_t lo = pos < 32u ? w0 : (pos < 64u ? w1 : w2), hi = pos < 32u ? w1 : (pos < 64u ? w2 : 0u);
+    const uint32_t low = __funnelshift_r(lo, hi, pos & 31u) & ((1u << m) - 1u);
     const uint32_t dig = ((uint32_t)lut[(trit ? 0u : 256u) + head] >> (k * (trit ? 2u : 3u))) & (trit ? 3u : 7u);
     return (dig << m) | low;
 }
@@ -100,7 +103,7 @@ __device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &
     __syncwarp();
     if (lane < n) {
         const uint4 t = q.vq[vcnt - n + lane];
-        int val = pc_offset(t.z) + (int)bise_at(S.pay + t.x, t.y, pc_layout(t.z), pc_m(t.z), lut);
+        int val = pc_offset(t.z) + (int)bise_at(S.pay, t.x, t.y, pc_layout(t.z), pc_m(t.z), lut);
         if (t.z & kSignBit) val = -val;
         atomicAdd(&q.acc[t.z >> 24], val);
     }
@@ -118,7 +121,7 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
     uint4 vt = make_uint4(0u, 0u, 0u, 0u);
     if (lane < n) {
         const uint4 t = q.mq[mcnt - n + lane];
-        const uint32_t rec = bise_at(S.mv + t.x, t.y, S.mv_layout, S.mv_m, lut);
+        const uint32_t rec = bise_at(S.mv, t.x, t.y, S.mv_layout, S.mv_m, lut);
         int mode, dx, dy;
         mv_unpack(S, rec, mode, dx, dy);
         const uint32_t xy = q.xy[t.w >> 2];
