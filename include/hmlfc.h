@@ -151,6 +151,20 @@ int hmlfc_set_decode_variant(hmlfc_handle *h, int variant);
 int hmlfc_search(const int16_t *d_planes, const int32_t *d_pairs, int n_pairs, int Ws, int Ht, int block, int window,
                  int32_t *d_out, void *cuda_stream);
 
+/* Encoder side, hierarchy build (SURVEY.md 8(f) rank 1 with hmlfc_search): forward YCoCg-R and the RLFC
+ * hierarchy of PAPER.md:200 (section 4.3): 2 x 2 clusters on the camera grid, RKV = uniform mean of the members present
+ * rounded half away from zero, SRV = member - RKV, repeated `height` times.  Level L has U_L x V_L planes,
+ * U_L = ceil(U / 2^L); plane (pu, pv) of a level has index pv * U_L + pu.
+ *   d_lf   device, uint8 [V][U][Ht][Ws][3] RGB8 (4-byte aligned)
+ *   d_srv  device, int16 [3][n_srv_planes][Ht][Ws]: channel (Y, Co, Cg) outermost, then the SRV planes of level 0, level 1, ..
+ *          level height-1 (n_srv_planes = sum_{L<height} U_L V_L)
+ *   d_x    device, int16 [3][n_x_planes][Ht][Ws]: the RKV planes X_1 .. X_height (n_x_planes = sum_{1<=L<=height} U_L V_L);
+ *          the last U_h V_h planes of each channel are the top-level RKVs
+ * hmlfc_hierarchy_sizes (host only) returns the two plane counts.  hmlfc_hierarchy enqueues `height` kernels on cuda_stream and
+ * returns; Ws must be a multiple of 4 (HMLFC_E_UNSUPPORTED), the outputs 8-byte aligned.  Integer-exact. */
+int hmlfc_hierarchy_sizes(int U, int V, int height, int64_t *n_srv_planes, int64_t *n_x_planes);
+int hmlfc_hierarchy(const uint8_t *d_lf, int U, int V, int Ws, int Ht, int height, int16_t *d_srv, int16_t *d_x, void *cuda_stream);
+
 /* Number of kernels this library has launched through the handle since load (bench accounting). */
 int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);
 

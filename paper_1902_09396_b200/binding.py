@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -79,6 +79,10 @@ def lib():
     L.hmlfc_set_decode_variant.argtypes, L.hmlfc_set_decode_variant.restype = [vp, C.c_int], C.c_int
     L.hmlfc_search.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
     L.hmlfc_search.restype = C.c_int
+    L.hmlfc_hierarchy_sizes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
+    L.hmlfc_hierarchy_sizes.restype = C.c_int
+    L.hmlfc_hierarchy.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+    L.hmlfc_hierarchy.restype = C.c_int
     L.hmlfc_launch_count.argtypes, L.hmlfc_launch_count.restype = [vp, C.POINTER(i64)], C.c_int
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
@@ -237,6 +241,31 @@ def hmlfc_search(planes, pairs, block: int, window: int, out=None, stream=None):
     _check(lib().hmlfc_search(C.c_void_p(planes.data_ptr()), C.c_void_p(pairs.data_ptr()), n_pairs, Ws, Ht, block, window,
                               C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream)), "hmlfc_search")
     return out
+
+
+def hmlfc_hierarchy_sizes(U: int, V: int, height: int):
+    """(n_srv_planes, n_x_planes) per channel."""
+    a, b = C.c_int64(), C.c_int64()
+    _check(lib().hmlfc_hierarchy_sizes(U, V, height, C.byref(a), C.byref(b)), "hmlfc_hierarchy_sizes")
+    return a.value, b.value
+
+
+def hmlfc_hierarchy(lf, height: int, srv=None, x=None, stream=None):
+    """lf: cuda uint8 [V][U][Ht][Ws][3]; returns (srv int16 [3][n_srv][Ht][Ws], x int16 [3][n_x][Ht][Ws]) on the device."""
+    torch = _require_cuda()
+    assert lf.is_cuda and lf.dtype == torch.uint8 and lf.is_contiguous() and lf.dim() == 5 and lf.shape[4] == 3
+    V, U, Ht, Ws = (int(v) for v in lf.shape[:4])
+    ns, nx = hmlfc_hierarchy_sizes(U, V, height)
+    if srv is None:
+        srv = torch.empty((3, ns, Ht, Ws), dtype=torch.int16, device=lf.device)
+    if x is None:
+        x = torch.empty((3, nx, Ht, Ws), dtype=torch.int16, device=lf.device)
+    assert srv.is_cuda and srv.dtype == torch.int16 and srv.is_contiguous() and tuple(srv.shape) == (3, ns, Ht, Ws)
+    assert x.is_cuda and x.dtype == torch.int16 and x.is_contiguous() and tuple(x.shape) == (3, nx, Ht, Ws)
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().hmlfc_hierarchy(C.c_void_p(lf.data_ptr()), U, V, Ws, Ht, height, C.c_void_p(srv.data_ptr()),
+                                 C.c_void_p(x.data_ptr()), C.c_void_p(st.cuda_stream)), "hmlfc_hierarchy")
+    return srv, x
 
 
 def hmlfc_launch_count(h: Handle) -> int:

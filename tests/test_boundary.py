@@ -80,6 +80,9 @@ def test_entry_points_validate_arguments(P):
     assert L.hmlfc_search(None, None, 0, 8, 8, 3, 1, None, None) == -5      # block does not divide the image
     assert L.hmlfc_search(None, None, 0, 8, 8, 4, 65, None, None) == -5     # window > 64
     assert L.hmlfc_search(None, None, 0, 8, 8, 4, 16, None, None) == 0      # nothing to do
+    assert L.hmlfc_hierarchy(None, 2, 2, 8, 8, 1, None, None, None) == -4
+    assert P.hmlfc_hierarchy_sizes(17, 17, 3) == (17 * 17 + 9 * 9 + 5 * 5, 9 * 9 + 5 * 5 + 3 * 3)   # 17 -> 9 -> 5 -> 3 (R3)
+    assert P.hmlfc_hierarchy_sizes(16, 16, 3) == (256 + 64 + 16, 64 + 16 + 4)
 
 
 def test_no_cpu_fallback(P, enc):
