@@ -70,6 +70,7 @@ def lib():
         "orc_open": (vp, [vp, C.c_size_t, C.POINTER(C.c_int)]),
         "orc_close": (None, [vp]),
         "orc_stream_params": (C.c_int, [vp, C.POINTER(Params)]),
+        "orc_set_min_level": (C.c_int, [vp, C.c_int]),
         "orc_decode": (i64, [vp, vp, i64, vp, C.c_int]),
         "orc_decode_brute": (i64, [vp, vp, i64, vp]),
         "orc_decode_full": (C.c_int, [vp, vp, C.c_int]),
@@ -269,6 +270,12 @@ class Stream:
 
     def __del__(self):
         self.close()
+
+    def set_min_level(self, min_level):
+        """Progressive decoding: sum only the levels >= min_level (0 = full quality, height = top RKV only)."""
+        rc = lib().orc_set_min_level(self._h, min_level)
+        if rc:
+            raise OracleError(rc, "set_min_level")
 
     def decode(self, coords, nthreads=0, return_oob=False):
         c = np.ascontiguousarray(coords, dtype=np.int32).reshape(-1, 4)

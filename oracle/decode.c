@@ -71,7 +71,7 @@ static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int us
     int acc[3];
     for (int c = 0; c < 3; ++c) {
         int a = rkv_sample(s, c, u >> h, v >> h, x, y);
-        for (int L = h - 1; L >= 0; --L) { /* "from the top level to the bottom level" */
+        for (int L = h - 1; L >= s->min_level; --L) { /* "from the top level to the bottom level"; progressive: stop early (R26) */
             int pu = u >> L, pv = v >> L;
             uint64_t k = pc_index(s, L, pu, pv, c);
             int e = plane_value(s, k, x, y, use_rank);
@@ -111,6 +111,13 @@ static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int us
     rgb[0] = (uint8_t)(r < 0 ? 0 : (r > 255 ? 255 : r));
     rgb[1] = (uint8_t)(g < 0 ? 0 : (g > 255 ? 255 : g));
     rgb[2] = (uint8_t)(b < 0 ? 0 : (b > 255 ? 255 : b));
+}
+
+int orc_set_min_level(orc_stream *s, int min_level)
+{
+    if (!s || min_level < 0 || min_level > s->h) return ORC_E_PARAM;
+    s->min_level = min_level;
+    return ORC_OK;
 }
 
 /* used by render.c */
@@ -213,7 +220,7 @@ static void touch_pixel(stat_ctx *cx, int u, int v, int x, int y)
     for (int c = 0; c < 3; ++c) {
         uint64_t ri = ((uint64_t)c * n_top + (uint64_t)(v >> h) * s->UL[h] + (u >> h)) * npx + (uint64_t)y * s->p.Ws + x;
         if (!cx->rkv_seen[ri]) { cx->rkv_seen[ri] = 1; cx->st.rkv_bytes += (c == 0) ? 1 : 2; }
-        for (int L = 0; L < h; ++L) {
+        for (int L = s->min_level; L < h; ++L) {
             int pu = u >> L, pv = v >> L;
             uint64_t k = pc_index(s, L, pu, pv, c);
             int b = (y / B) * s->nbx + (x / B);

@@ -116,6 +116,10 @@ typedef struct orc_stream orc_stream;
 
 orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err); /* copies bytes */
 void orc_close(orc_stream *s);
+/* Progressive decoding (PAPER.md:57, :183 name the property; :289-293 the top-down traversal it truncates; R26): the
+ * decoder and the renderer sum the top-level RKV and the levels h-1 .. min_level only (0 = everything, h = the top RKV alone), which
+ * yields the representative key view of the level-min_level cluster that contains the view.  Returns ORC_E_PARAM outside [0, h]. */
+int orc_set_min_level(orc_stream *s, int min_level);
 int orc_stream_params(const orc_stream *s, orc_params *out);
 /* P2: per-pixel random access; coords [n][4] = u,v,s,t ; out [n][3] RGB8; out-of-range -> (0,0,0).
  * Returns the number of out-of-range coordinates. */

@@ -57,6 +57,7 @@ struct orc_stream {
     uint32_t **rank_res;        /* [n_pc][nblk+1] exclusive prefix counts (built at open) */
     uint32_t **rank_pred;       /* same for pred maps (NULL for reference planes) */
     uint32_t mvN;               /* 2 (2W+1)^2 */
+    int min_level;              /* progressive decoding (R26): the walk stops above this level; 0 = full quality */
 };
 
 static inline int orc_is_predictive(int pu, int pv) { return ((pu | pv) & 1) != 0; }

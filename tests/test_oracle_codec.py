@@ -277,3 +277,60 @@ def test_psnr_closed_form():
     a = np.full((10, 10, 3), 100, dtype=np.uint8)
     assert abs(orc.psnr(a, a + 1) - 48.130803608679) < 1e-9
     assert orc.psnr(a, a) == float("inf")
+
+
+# ---------------------------------------------------------------- progressive decoding (R26)
+def _ycocg_planes_to_rgb(y, co, cg):
+    t = y.astype(np.int32) - (cg.astype(np.int32) >> 1)
+    g = cg + t
+    b = t - (co.astype(np.int32) >> 1)
+    r = b + co
+    return np.clip(np.stack([r, g, b], axis=-1), 0, 255).astype(np.uint8)
+
+
+def test_progressive_level_of_a_lossless_stream_is_the_cluster_key_view():
+    """tau = 0: stopping the walk above level L yields exactly the representative key view X_L of the level-L cluster that
+    contains the view (PAPER.md:200 defines X_L; the path-sum identity pins it) -- for every L in 0..h, every view."""
+    import workloads as wl
+
+    cfg = wl.CONFIGS["mini3"]                      # odd 5 x 5 grid, h = 3
+    lf = wl.light_field(cfg)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, cfg.window, 0, 0)
+    data, info, tree = orc.encode(lf, p)
+    s = orc.Stream(data)
+    for L in range(cfg.height + 1):
+        s.set_min_level(L)
+        full = s.decode_full()
+        for v in range(cfg.V):
+            for u in range(cfg.U):
+                X = [tree.plane("X", L, u >> L, v >> L, c) for c in range(3)]
+                assert np.array_equal(full[v, u], _ycocg_planes_to_rgb(*X)), (L, u, v)
+        if L == 0:
+            assert np.array_equal(full, lf)
+    with pytest.raises(orc.OracleError):
+        s.set_min_level(cfg.height + 1)
+    with pytest.raises(orc.OracleError):
+        s.set_min_level(-1)
+    tree.close()
+
+
+def test_progressive_top_level_equals_huge_threshold_stream_and_quality_is_monotone(enc):
+    cfg, lf, data, info, s0 = enc("mini2")
+    s = orc.Stream(data)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, cfg.window, 10 ** 6, 10 ** 6)
+    data_top, _, tree = orc.encode(lf, p)           # every block insignificant: only the RKV chain survives
+    tree.close()
+    top_only = orc.Stream(data_top).decode_full()
+    quality, touched = [], []
+    import workloads as wl
+
+    rc = wl.random_coords(cfg, 3000)
+    for L in range(cfg.height + 1):
+        s.set_min_level(L)
+        full = s.decode_full()
+        quality.append(orc.psnr(full, lf))
+        touched.append(s.stats_decode(rc)["blocks_touched"])
+        assert np.array_equal(s.decode(rc), full[rc[:, 1], rc[:, 0], rc[:, 3], rc[:, 2]])   # random access = dense, at every level
+    assert np.array_equal(full, top_only)           # min_level = h
+    assert all(a >= b for a, b in zip(quality, quality[1:])) and quality[0] > quality[-1] + 3.0
+    assert all(a > b for a, b in zip(touched, touched[1:])) and touched[-1] == 0
