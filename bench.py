@@ -227,6 +227,8 @@ def run_ours(args, cfg_name):
         P.hmlfc_set_render_variant(h, args.variant)
     if args.decode_variant:
         P.hmlfc_set_decode_variant(h, args.decode_variant)
+    if args.min_level:
+        P.hmlfc_set_min_level(h, args.min_level)  # progressive decoding: an extra, labelled measurement row (not the headline)
     W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
     # weak scaling: every rank renders a full batch, each on its own arc of the camera circle
     cams_np = rank_cameras(cfg, rank)
@@ -364,6 +366,8 @@ def run_ours(args, cfg_name):
         import oracle as orc
 
         s = orc.Stream(data)
+        if args.min_level:
+            s.set_min_level(args.min_level)
         cores = os.cpu_count() or 1
         n_cpu, cpu_s = _oracle_views_sample(s, cams_np, W, H, args.cpu_budget, V)
         cpu = {"value": n_cpu / cpu_s, "unit": "views/s", "cores": cores, "kind": "oracle",
@@ -394,6 +398,7 @@ def run_ours(args, cfg_name):
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "decode": decode, "search": search, "hierarchy": hierarchy,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),
+            "min_level": args.min_level,
             "paper_context": "~200 fps at 512x512 on a GTX-980, Lego Knights (PAPER.md:409): another machine and light field, not the target",
         }
         print(json.dumps(line), flush=True)
@@ -435,6 +440,7 @@ def main():
     ap.add_argument("--config", default="cfg2")
     ap.add_argument("--variant", type=int, default=0, help="render kernel: 0 auto (= 6 cta), 1 pixel, 2 tiled, 3 blocks, 4/5 warp (A/B only)")
     ap.add_argument("--decode-variant", type=int, default=0, help="decode kernel: 0 auto (= 2 warp-cooperative), 1 thread per coordinate")
+    ap.add_argument("--min-level", type=int, default=0, help="progressive decoding: sum only the levels >= this one (0 = full quality)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -132,6 +132,12 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
  * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows). */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
+/* Progressive decoding (PAPER.md:57, :183 name the property; R26): hmlfc_decode / hmlfc_render sum the top-level RKV and the
+ * levels height-1 .. min_level only -- the walk from the root stops early.  0 (default) = full quality; `height` = the top-level RKV
+ * alone; level L yields the representative key view of the level-L cluster containing the view.  Fewer levels = fewer lookups and
+ * bytes per sample.  Takes effect for launches enqueued afterwards; HMLFC_E_INVALID outside [0, height]. */
+int hmlfc_set_min_level(hmlfc_handle *h, int min_level);
+
 /* Kernel selection for hmlfc_decode (identical bytes): 0 = automatic (default: 2), 1 = one thread per
  * coordinate walks the tree on its own, 2 = warp-cooperative (each lane classifies its coordinate, the
  * motion-record and BISE value decodes run as 32-wide batches from per-warp task stacks). */

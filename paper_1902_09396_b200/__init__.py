@@ -8,5 +8,5 @@ from .binding import (  # noqa: F401
     hmlfc_decode, hmlfc_decode_host, hmlfc_footprint_decode, hmlfc_footprint_render, hmlfc_free,
     hmlfc_last_oob_count, hmlfc_launch_count, hmlfc_load, hmlfc_render, hmlfc_render_host, hmlfc_search,
     hmlfc_hierarchy, hmlfc_hierarchy_sizes,
-    hmlfc_set_decode_variant, hmlfc_set_render_variant, lib,
+    hmlfc_set_decode_variant, hmlfc_set_min_level, hmlfc_set_render_variant, lib,
 )

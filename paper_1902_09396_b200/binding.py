@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -77,6 +77,7 @@ def lib():
     L.hmlfc_footprint_decode.argtypes, L.hmlfc_footprint_decode.restype = [vp, vp, i64, C.POINTER(Footprint)], C.c_int
     L.hmlfc_set_render_variant.argtypes, L.hmlfc_set_render_variant.restype = [vp, C.c_int], C.c_int
     L.hmlfc_set_decode_variant.argtypes, L.hmlfc_set_decode_variant.restype = [vp, C.c_int], C.c_int
+    L.hmlfc_set_min_level.argtypes, L.hmlfc_set_min_level.restype = [vp, C.c_int], C.c_int
     L.hmlfc_search.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp]
     L.hmlfc_search.restype = C.c_int
     L.hmlfc_hierarchy_sizes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(i64), C.POINTER(i64)]
@@ -222,6 +223,10 @@ def hmlfc_footprint_decode(h: Handle, coords) -> dict:
 
 def hmlfc_set_render_variant(h: Handle, variant: int):
     _check(lib().hmlfc_set_render_variant(h._h, variant), "hmlfc_set_render_variant")
+
+
+def hmlfc_set_min_level(h: Handle, min_level: int):
+    _check(lib().hmlfc_set_min_level(h._h, min_level), "hmlfc_set_min_level")
 
 
 def hmlfc_set_decode_variant(h: Handle, variant: int):

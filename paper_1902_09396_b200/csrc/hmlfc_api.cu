@@ -158,7 +158,9 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     int nl = 0;
     const Camera *cams = reinterpret_cast<const Camera *>(d_cameras);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (h->render_variant == 1)
+    // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the CTA kernel
+    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || h->render_variant == 6);
+    if (h->render_variant == 1 || (h->ds.lmin > 0 && !cta_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 2)
         CU(h, launch_render_tiled(h->ds, cams, n_views, W, H, d_out, st, &nl));
@@ -272,6 +274,13 @@ int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
     if (!h || variant < 0 || variant > 6) return HMLFC_E_INVALID;
     h->render_variant = variant;
+    return HMLFC_OK;
+}
+
+int hmlfc_set_min_level(hmlfc_handle *h, int min_level)
+{
+    if (!h || min_level < 0 || min_level > h->ds.h) return HMLFC_E_INVALID;
+    h->ds.lmin = min_level;
     return HMLFC_OK;
 }
 

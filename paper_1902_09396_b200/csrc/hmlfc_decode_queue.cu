@@ -179,7 +179,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     int vcnt = 0, mcnt = 0;
 
 #pragma unroll 1
-    for (int L = 0; L < h; ++L) {
+    for (int L = S.lmin; L < h; ++L) {
         const int pu = u >> L, pv = v >> L;
         const LevelDesc lv = S.lev[L];
         const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;

@@ -45,7 +45,7 @@ struct DevStream {
     int32_t UH, VH;                   // top-level RKV grid
     uint32_t nd, nd2, nd_magic;       // 2W+1, (2W+1)^2, ceil(2^32 / nd)
     uint32_t mv_layout, mv_m;         // BISE layout of the motion records, N = 2 (2W+1)^2
-    uint32_t _pad0;
+    int32_t lmin;                     // progressive decoding (R26): levels below lmin are not summed; 0 = full quality
     LevelDesc lev[kMaxLevels];
     const uint4 *pc;
     const uint4 *flagrec;
@@ -187,7 +187,7 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
     const uint32_t fg = (uint32_t)(b >> 5);
     const int kin = ((y & (S.B - 1)) << S.logB) + (x & (S.B - 1));
 #pragma unroll 1
-    for (int L = 0; L < h; ++L) {
+    for (int L = S.lmin; L < h; ++L) {
         const int pu = u >> L, pv = v >> L;
         const LevelDesc lv = S.lev[L];
         const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;

@@ -126,7 +126,7 @@ __device__ void touch_sample(const DevStream &S, FootprintMarks mk, int u, int v
     mark_bit(mk.rkv, ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)y) * (size_t)S.Ws + (size_t)x);
     const int b = (y >> S.logB) * S.nbx + (x >> S.logB);
     const uint32_t bit = 1u << (b & 31);
-    for (int L = 0; L < h; ++L) {
+    for (int L = S.lmin; L < h; ++L) {
         const int pu = u >> L, pv = v >> L;
         const LevelDesc lv = S.lev[L];
         const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;

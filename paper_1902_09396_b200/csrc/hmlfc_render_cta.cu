@@ -284,7 +284,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         }
         // per level the rectangle of planes over the views; lane L owns level L
         int pu0 = 0, pv0 = 0, nuL = 0, cntL = 0;
-        if (lane < h) {
+        if (lane >= S.lmin && lane < h) {  // progressive decoding: no planes below lmin
             pu0 = bu0 >> lane; pv0 = bv0 >> lane;
             nuL = ((bu0 + nu - 1) >> lane) - pu0 + 1;
             cntL = nuL * (((bv0 + nv - 1) >> lane) - pv0 + 1);
@@ -378,6 +378,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         for (int q = kSpecZero + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);  // the rest (warps 1..7 zeroed the head during T)
         for (int q = tid; q < nviews * h; q += kNT) {
             const int vw = q / h, L = q - vw * h;
+            if (L < S.lmin) continue;
             const int iv = vw / nu, iu = vw - iv * nu;
             const int sidx = ctl.lvl_base[L] + (((bv0 + iv) >> L) - ctl.lvl_pv0[L]) * ctl.lvl_nu[L] + (((bu0 + iu) >> L) - ctl.lvl_pu0[L]);
             const SlotInfo &sl = ctl.slot[sidx];
@@ -534,7 +535,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
         const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
         int a[3] = {rk.x, rk.y, rk.z};
-        for (int L = 0; L < h; ++L) {
+        for (int L = S.lmin; L < h; ++L) {
             const int2 vo = ctl.voff[vw][L];
             const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
             a[0] += (int)(int16_t)(w.x & 0xFFFFu);

@@ -182,6 +182,43 @@ def test_render_host_entry_point(P, enc):
     assert np.abs(got.astype(int) - s.render(cams, cfg.out_w, cfg.out_h).astype(int)).max() <= TOL_VIEW
 
 
+# ---------------------------------------------------------------- progressive decoding (R26)
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini3", "mini4", "mini_b8"])
+def test_progressive_levels_match_oracle(P, enc, name):
+    """hmlfc_set_min_level(L) for every L in 0..h: decode bit-exact, views within 1 LSB (CTA kernel and thread-per-pixel kernel
+    byte-identical), footprint = the oracle's counter; out-of-range levels are rejected."""
+    import oracle as orc
+
+    cfg, lf, data, info, s0 = enc(name)
+    s = orc.Stream(data)
+    h = P.hmlfc_load(data)
+    coords, rc, cams = wl.all_coords(cfg), wl.random_coords(cfg, 4000), wl.camera_path(cfg)
+    for L in range(cfg.height + 1):
+        s.set_min_level(L)
+        P.hmlfc_set_min_level(h, L)
+        expect = s.decode(coords)
+        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE):
+            P.hmlfc_set_decode_variant(h, variant)
+            assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), (L, variant)
+        ref = s.render(cams, cfg.out_w, cfg.out_h)
+        outs = []
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP):   # WARP falls back to the per-pixel kernel when L > 0
+            P.hmlfc_set_render_variant(h, variant)
+            got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
+            assert np.abs(got.astype(np.int16) - ref.astype(np.int16)).max() <= TOL_VIEW, (L, variant)
+            outs.append(got)
+        assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+        P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+        fpd, std = P.hmlfc_footprint_decode(h, _dev(rc)), s.stats_decode(rc)
+        for k in ("blocks_touched", "flag_bits", "payload_bits15", "mv_bits15", "rkv_bytes"):
+            assert fpd[k] == std[k], (L, k)
+    assert fpd["blocks_touched"] == 0   # L = h: the top-level RKV alone
+    for bad in (-1, cfg.height + 1):
+        with pytest.raises(P.HmlfcError):
+            P.hmlfc_set_min_level(h, bad)
+    P.hmlfc_free(h)
+
+
 # ---------------------------------------------------------------- accounting
 @pytest.mark.parametrize("name", ["cfg1_lossy", "mini4"])
 def test_footprint_equals_oracle_stats(P, enc, name):
