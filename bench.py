@@ -293,6 +293,18 @@ def run_ours(args, cfg_name):
     e2e_s = reduce_max(time.perf_counter() - t0, world, "cuda")
     e2e_views_per_s = whole_job_rate(V, e2e_steps, world, e2e_s)
     assert torch.equal(out_pin.cuda(), out), "host entry point and device entry point disagree"
+    # the decode leg end to end: coordinates H2D + kernels + pixels D2H, pipelined in chunks by hmlfc_decode_host
+    coords_pin = coords.cpu().pin_memory()
+    dec_pin = torch.empty((n_dec, 3), dtype=torch.uint8).pin_memory()
+    P.hmlfc_decode_host(h, coords_pin.numpy(), out=dec_pin.numpy())
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(3):
+        P.hmlfc_decode_host(h, coords_pin.numpy(), out=dec_pin.numpy())
+    dec_e2e_s = reduce_max(time.perf_counter() - t0, world, "cuda")
+    assert torch.equal(dec_pin.cuda(), dec_out), "decode: host entry point and device entry point disagree"
+    del coords_pin, dec_pin
 
     # ---- encoder-side leg (SURVEY 8(f) first "next" row): phase-shifted exhaustive search of one level-0 channel
     sU, sV = min(cfg.U, 16), min(cfg.V, 16)  # at most a 16 x 16 sub-grid of planes per launch
@@ -333,6 +345,8 @@ def run_ours(args, cfg_name):
         }
         decode = {
             "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
+            "e2e": {"value": whole_job_rate(n_dec, 3, world, dec_e2e_s), "unit": "LF pixels/s", "h2d_bytes_per_step": 16 * n_dec,
+                    "d2h_bytes_per_step": 3 * n_dec, "steps": 3},
             "roofline": {"bound": "hbm", "kernel": "decode_kernel" if args.decode_variant == 1 else "decode_queue_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
                          "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
                          "traffic": _ncu_from_profiles(cfg.name, "decode").get("dram_bytes")},

@@ -288,6 +288,8 @@ def test_full_size_sampled_parity(P, name):
     P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)   # the unshared thread-per-pixel kernel on the first view
     assert np.array_equal(P.hmlfc_render(h, _dev(cams[:1]), cfg.out_w, cfg.out_h).cpu().numpy()[0], got[0])
     P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+    # the host entry point pipelines the batch in chunks of views over three streams: same bytes as the one launch
+    assert np.array_equal(P.hmlfc_render_host(h, cams, cfg.out_w, cfg.out_h), got)
     del got
 
     rc = wl.random_coords(cfg, cfg.n_decode)
@@ -298,6 +300,8 @@ def test_full_size_sampled_parity(P, name):
     P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
     step = max(1, cfg.n_decode // 2_000_000)
     assert np.array_equal(out[::step].cpu().numpy(), s.decode(rc[::step]))
+    n_host = min(cfg.n_decode, 2_500_001)   # three chunks (2^20, 2^20, ragged rest) through the pipelined host entry point
+    assert np.array_equal(P.hmlfc_decode_host(h, rc[:n_host]), out[:n_host].cpu().numpy())
     assert P.hmlfc_last_oob_count(h) == 0
     target = cfg.target_psnr
     assert target - 2.0 < info["psnr"] < target + 2.0  # "quantisation set for ~40 dB" (45 dB for cfg3)
