@@ -174,6 +174,34 @@ int hmlfc_search(const int16_t *d_planes, const int32_t *d_pairs, int n_pairs, i
 int hmlfc_hierarchy_sizes(int U, int V, int height, int64_t *n_srv_planes, int64_t *n_x_planes);
 int hmlfc_hierarchy(const uint8_t *d_lf, int U, int V, int Ws, int Ht, int height, int16_t *d_srv, int16_t *d_x, void *cuda_stream);
 
+/* Encoder, complete: RGB8 light field on the device -> compressed stream in host memory, every
+ * arithmetic step in CUDA kernels: hmlfc_hierarchy, hmlfc_search for every predictive SRV image of every
+ * level and channel, the replacement step and the two block thresholds (reference block
+ * kept iff sum|block| >= tau_ref; predictive block per `policy`, R13: 0 adaptive, 1 all, 2 literal), BISE packing of
+ * the stored blocks and of the joint motion records, in the BFS order of PAPER.md:276.  The host writes the
+ * header, the raw top-level RKVs and the directory around the device-built sections ("Stream format v1").
+ *   d_lf      device, uint8 [V][U][Ht][Ws][3] RGB8, 4-byte aligned (not modified)
+ *   p         host; block in {2,4,8} dividing Ws and Ht, Ws % 4 == 0, height <= 8, window <= 64 (else HMLFC_E_UNSUPPORTED);
+ *             geometry / background / seed are copied into the header
+ *   h_stream  receives a malloc'ed buffer of *len bytes that hmlfc_load accepts; release it with hmlfc_stream_free
+ *   stats     optional (may be NULL): device time per phase (CUDA events) and block counts
+ * Synchronous (the value ranges must reach the host before the strings can be laid out); allocates and frees its device
+ * scratch (about 2.7 x the raw light field as int16 planes + 16 bytes per predictive block). */
+typedef struct {
+    int32_t U, V, Ws, Ht, height, block, window, tau_ref, tau_res, policy;
+    float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
+    unsigned char background[3], _pad;
+    uint64_t seed;
+} hmlfc_encode_params_t;
+typedef struct {
+    float ms_hierarchy, ms_search, ms_classify, ms_pack;   /* device time of the four phases */
+    int64_t n_plane_channels, n_res_blocks, n_pred_blocks, n_search_blocks;
+    int32_t kernel_launches, cuda_error;
+} hmlfc_encode_stats_t;
+int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
+                 hmlfc_encode_stats_t *stats, void *cuda_stream);
+void hmlfc_stream_free(uint8_t *h_stream);
+
 /* Number of kernels this library has launched through the handle since load (bench accounting). */
 int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);
 

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_stream_free",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -85,6 +85,9 @@ def lib():
     L.hmlfc_hierarchy.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp]
     L.hmlfc_hierarchy.restype = C.c_int
     L.hmlfc_launch_count.argtypes, L.hmlfc_launch_count.restype = [vp, C.POINTER(i64)], C.c_int
+    L.hmlfc_encode.argtypes = [vp, vp, C.POINTER(vp), C.POINTER(C.c_size_t), vp, vp]
+    L.hmlfc_encode.restype = C.c_int
+    L.hmlfc_stream_free.argtypes, L.hmlfc_stream_free.restype = [vp], None
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
     L.hmlfc_last_cuda_error.argtypes, L.hmlfc_last_cuda_error.restype = [vp], C.c_int
@@ -271,6 +274,47 @@ def hmlfc_hierarchy(lf, height: int, srv=None, x=None, stream=None):
     _check(lib().hmlfc_hierarchy(C.c_void_p(lf.data_ptr()), U, V, Ws, Ht, height, C.c_void_p(srv.data_ptr()),
                                  C.c_void_p(x.data_ptr()), C.c_void_p(st.cuda_stream)), "hmlfc_hierarchy")
     return srv, x
+
+
+class EncodeParams(C.Structure):
+    _fields_ = [("U", C.c_int32), ("V", C.c_int32), ("Ws", C.c_int32), ("Ht", C.c_int32), ("height", C.c_int32),
+                ("block", C.c_int32), ("window", C.c_int32), ("tau_ref", C.c_int32), ("tau_res", C.c_int32), ("policy", C.c_int32),
+                ("uv_origin", C.c_float * 2), ("uv_step", C.c_float * 2), ("st_origin", C.c_float * 2), ("st_step", C.c_float * 2),
+                ("z_st", C.c_float), ("background", C.c_ubyte * 3), ("_pad", C.c_ubyte), ("seed", C.c_uint64)]
+
+
+class EncodeStats(C.Structure):
+    _fields_ = [("ms_hierarchy", C.c_float), ("ms_search", C.c_float), ("ms_classify", C.c_float), ("ms_pack", C.c_float),
+                ("n_plane_channels", C.c_int64), ("n_res_blocks", C.c_int64), ("n_pred_blocks", C.c_int64),
+                ("n_search_blocks", C.c_int64), ("kernel_launches", C.c_int32), ("cuda_error", C.c_int32)]
+
+
+def hmlfc_encode(lf, height: int, block: int = 4, window: int = 16, tau_ref: int = 0, tau_res: int = 0, policy: int = 0,
+                 geometry: dict = None, background=(0, 0, 0), seed: int = 0, stream=None):
+    """lf: cuda uint8 [V][U][Ht][Ws][3].  Returns (stream bytes, stats dict): the whole encoder runs in CUDA kernels, the host
+    only lays out the sections.  geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab."""
+    torch = _require_cuda()
+    assert lf.is_cuda and lf.dtype == torch.uint8 and lf.is_contiguous() and lf.dim() == 5 and lf.shape[4] == 3
+    p = EncodeParams()
+    p.V, p.U, p.Ht, p.Ws = (int(v) for v in lf.shape[:4])
+    p.height, p.block, p.window, p.tau_ref, p.tau_res, p.policy = height, block, window, tau_ref, tau_res, policy
+    g = geometry or dict(uv_origin=(0.0, 0.0), uv_step=(1.0, 1.0), st_origin=(0.0, 0.0), st_step=(1.0, 1.0), z_st=1.0)
+    for k in ("uv_origin", "uv_step", "st_origin", "st_step"):
+        getattr(p, k)[0], getattr(p, k)[1] = float(g[k][0]), float(g[k][1])
+    p.z_st = float(g["z_st"])
+    for i in range(3):
+        p.background[i] = background[i]
+    p.seed = seed
+    out, n, stats = C.c_void_p(), C.c_size_t(), EncodeStats()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().hmlfc_encode(C.c_void_p(lf.data_ptr()), C.byref(p), C.byref(out), C.byref(n), C.byref(stats), C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise HmlfcError(rc, "hmlfc_encode", f"{lib().hmlfc_strerror(rc).decode()} (cuda error {stats.cuda_error})")
+    try:
+        data = C.string_at(out, n.value)
+    finally:
+        lib().hmlfc_stream_free(out)
+    return data, {k: getattr(stats, k) for k, _ in EncodeStats._fields_}
 
 
 def hmlfc_launch_count(h: Handle) -> int:

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["hmlfc_api.cu", "hmlfc_kernels.cu", "hmlfc_decode_queue.cu", "hmlfc_search.cu", "hmlfc_hierarchy.cu", "hmlfc_render_tiled.cu", "hmlfc_render_blocks.cu", "hmlfc_render_warp.cu", "hmlfc_render_cta.cu"]
+SOURCES = ["hmlfc_api.cu", "hmlfc_kernels.cu", "hmlfc_decode_queue.cu", "hmlfc_search.cu", "hmlfc_hierarchy.cu", "hmlfc_encode.cu", "hmlfc_render_tiled.cu", "hmlfc_render_blocks.cu", "hmlfc_render_warp.cu", "hmlfc_render_cta.cu"]
 HEADERS = ["hmlfc_device.cuh", "hmlfc_kernels.cuh", "hmlfc_tables.h"]
 LIB = os.path.join(HERE, "libhmlfc_b200.so")
 

@@ -1,0 +1,104 @@
+"""GPU parity of hmlfc_encode (the whole HMLFC encoder in CUDA kernels: colour + hierarchy, phase-shifted search, replacement step,
+two block thresholds, BISE packing, BFS stream order -- PAPER.md:200-276) against the oracle's encoder: the two compressed streams
+must be equal BYTE FOR BYTE (header, top-level RKVs, directory, flag maps, payload strings, motion-vector strings).  The two
+writers share no code; the format is DESIGN.md section 4.  Streams fed to the decode / render tests still come from the oracle only."""
+import struct
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_1902_09396_b200 as pkg
+
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    return pkg
+
+
+def _section(data, off):
+    names = ("rkv", "directory", "flags", "payload", "mv", "end")
+    offs = struct.unpack_from("<6Q", data, 112)
+    where = "header"
+    for n, o in zip(names, offs):
+        if off >= o:
+            where = n
+    return where
+
+
+def _assert_same_stream(got, expect):
+    if got == expect:
+        return
+    a, b = np.frombuffer(got, np.uint8), np.frombuffer(expect, np.uint8)
+    n = min(len(a), len(b))
+    diff = np.nonzero(a[:n] != b[:n])[0]
+    first = int(diff[0]) if len(diff) else n
+    raise AssertionError(f"streams differ: lengths {len(a)} / {len(b)}, {len(diff)} bytes differ, first at {first} "
+                         f"(section {_section(expect, first)}), header offsets {struct.unpack_from('<6Q', expect, 112)}")
+
+
+def _gpu_encode(P, cfg, lf, tau_ref, tau_res, policy=0):
+    return P.hmlfc_encode(torch.from_numpy(lf).cuda(), cfg.height, cfg.block, cfg.window, tau_ref, tau_res, policy,
+                          geometry=wl.geometry(cfg), seed=cfg.seed)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8"])
+def test_encoded_stream_equals_the_oracle_stream(P, enc, name):
+    # cfg1: tau = 0 (every block kept); mini3: odd 5 x 5 grid (partial clusters); mini_b2 / mini_b8: B = 2 / 8, W = 5 / 8
+    cfg, lf, data, info, s = enc(name)
+    got, stats = _gpu_encode(P, cfg, lf, info["tau_ref"], info["tau_res"])
+    _assert_same_stream(got, data)
+    assert stats["n_plane_channels"] == struct.unpack_from("<Q", data, 104)[0]
+    assert stats["kernel_launches"] >= cfg.height + 5
+
+
+@pytest.mark.parametrize("policy", [orc.POLICY_ALL, orc.POLICY_LITERAL])
+@pytest.mark.parametrize("tau", [0, 37, 100000])
+def test_other_policies_and_degenerate_thresholds(P, policy, tau):
+    # tau = 100000: no block survives (empty payload and, under `literal`, empty motion-vector strings)
+    cfg = wl.CONFIGS["mini3"]
+    lf = wl.light_field(cfg)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, cfg.window, tau // 2, tau, policy=policy,
+                        geometry=wl.geometry(cfg), seed=cfg.seed)
+    data, info, tree = orc.encode(lf, p)
+    tree.close()
+    got, _ = _gpu_encode(P, cfg, lf, tau // 2, tau, policy)
+    _assert_same_stream(got, data)
+
+
+def test_encoded_stream_loads_and_decodes_to_the_oracle_reconstruction(P, enc):
+    cfg, lf, data, info, s = enc("mini4")
+    got, _ = _gpu_encode(P, cfg, lf, info["tau_ref"], info["tau_res"])
+    h = P.hmlfc_load(got)
+    coords = wl.all_coords(cfg)
+    out = P.hmlfc_decode(h, torch.from_numpy(coords).cuda()).cpu().numpy()
+    assert np.array_equal(out.reshape(info["p1"].shape), info["p1"])  # = the oracle encoder's own reconstruction (P1)
+    P.hmlfc_free(h)
+
+
+def test_cfg2_full_size_stream_equals_the_oracle_stream(P):
+    """BASELINE.json configs[1] at full size (16 x 16 views of 256 x 256, h = 3, B = 4, W = 16, ~40 dB): 7.5 MB stream."""
+    from oracle import streams
+
+    cfg, data, info = streams.get_stream("cfg2")
+    lf = wl.light_field(cfg)
+    got, stats = _gpu_encode(P, cfg, lf, info["tau_ref"], info["tau_res"])
+    _assert_same_stream(got, data)
+    assert stats["n_search_blocks"] == 3 * (192 + 48 + 12) * 4096
+
+
+def test_invalid_and_unsupported_arguments(P):
+    lf = torch.zeros((2, 2, 16, 16, 3), dtype=torch.uint8, device="cuda")
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_encode(lf, 1, block=3)          # B must be 2, 4 or 8
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_encode(lf, 9)                   # height > 8
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_encode(lf, 1, tau_res=-1)
