@@ -185,8 +185,9 @@ int hmlfc_hierarchy(const uint8_t *d_lf, int U, int V, int Ws, int Ht, int heigh
  *             geometry / background / seed are copied into the header
  *   h_stream  receives a malloc'ed buffer of *len bytes that hmlfc_load accepts; release it with hmlfc_stream_free
  *   stats     optional (may be NULL): device time per phase (CUDA events) and block counts
- * Synchronous (the value ranges must reach the host before the strings can be laid out); allocates and frees its device
- * scratch (about 2.7 x the raw light field as int16 planes + 16 bytes per predictive block). */
+ * Synchronous (the value ranges must reach the host before the strings can be laid out); its device scratch (about 2.7 x the
+ * raw light field as int16 planes + 16 bytes per predictive block) comes from a stream-ordered pool (see
+ * hmlfc_encode_release_scratch). */
 typedef struct {
     int32_t U, V, Ws, Ht, height, block, window, tau_ref, tau_res, policy;
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
@@ -195,12 +196,16 @@ typedef struct {
 } hmlfc_encode_params_t;
 typedef struct {
     float ms_hierarchy, ms_search, ms_classify, ms_pack;   /* device time of the four phases */
+    float ms_wall, ms_assemble;                            /* host wall clock: the whole call; stream assembly + copies to the host */
     int64_t n_plane_channels, n_res_blocks, n_pred_blocks, n_search_blocks;
     int32_t kernel_launches, cuda_error;
 } hmlfc_encode_stats_t;
 int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
                  hmlfc_encode_stats_t *stats, void *cuda_stream);
 void hmlfc_stream_free(uint8_t *h_stream);
+/* hmlfc_encode keeps its device scratch in a stream-ordered memory pool of the current device between calls (a second call
+ * allocates nothing from the driver); this returns it.  Synchronises the device. */
+int hmlfc_encode_release_scratch(void);
 
 /* Number of kernels this library has launched through the handle since load (bench accounting). */
 int hmlfc_launch_count(const hmlfc_handle *h, int64_t *out);

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_stream_free",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -88,6 +88,7 @@ def lib():
     L.hmlfc_encode.argtypes = [vp, vp, C.POINTER(vp), C.POINTER(C.c_size_t), vp, vp]
     L.hmlfc_encode.restype = C.c_int
     L.hmlfc_stream_free.argtypes, L.hmlfc_stream_free.restype = [vp], None
+    L.hmlfc_encode_release_scratch.argtypes, L.hmlfc_encode_release_scratch.restype = [], C.c_int
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
     L.hmlfc_last_cuda_error.argtypes, L.hmlfc_last_cuda_error.restype = [vp], C.c_int
@@ -285,6 +286,7 @@ class EncodeParams(C.Structure):
 
 class EncodeStats(C.Structure):
     _fields_ = [("ms_hierarchy", C.c_float), ("ms_search", C.c_float), ("ms_classify", C.c_float), ("ms_pack", C.c_float),
+                ("ms_wall", C.c_float), ("ms_assemble", C.c_float),
                 ("n_plane_channels", C.c_int64), ("n_res_blocks", C.c_int64), ("n_pred_blocks", C.c_int64),
                 ("n_search_blocks", C.c_int64), ("kernel_launches", C.c_int32), ("cuda_error", C.c_int32)]
 
@@ -315,6 +317,10 @@ def hmlfc_encode(lf, height: int, block: int = 4, window: int = 16, tau_ref: int
     finally:
         lib().hmlfc_stream_free(out)
     return data, {k: getattr(stats, k) for k, _ in EncodeStats._fields_}
+
+
+def hmlfc_encode_release_scratch():
+    _check(lib().hmlfc_encode_release_scratch(), "hmlfc_encode_release_scratch")
 
 
 def hmlfc_launch_count(h: Handle) -> int:

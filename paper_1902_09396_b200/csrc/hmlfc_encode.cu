@@ -23,6 +23,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <chrono>
 #include <vector>
 
 namespace {
@@ -322,10 +323,42 @@ void put64(uint8_t *p, uint64_t v) { for (int i = 0; i < 8; ++i) p[i] = (uint8_t
 void putf(uint8_t *p, float f) { uint32_t u; memcpy(&u, &f, 4); put32(p, u); }
 uint64_t up8(uint64_t x) { return (x + 7) & ~7ull; }
 
+double now_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
+
+// Device scratch from the stream-ordered pool of the device (cudaMallocAsync): after the first call the pool serves the
+// encoder's buffers without going to the driver, and frees do not synchronise the device.
+cudaMemPool_t g_pool[64] = {};
+
+cudaError_t scratch_pool(cudaMemPool_t *out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!g_pool[dev]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if ((e = cudaMemPoolCreate(&g_pool[dev], &props)) != cudaSuccess) return e;
+        uint64_t keep = ~0ull;  // keep freed scratch for the next call (hmlfc_encode_release_scratch returns it)
+        if ((e = cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
+    }
+    *out = g_pool[dev];
+    return cudaSuccess;
+}
+
 struct DevBuf {  // frees on scope exit
     void *p = nullptr;
-    ~DevBuf() { if (p) cudaFree(p); }
-    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 16); }
+    cudaStream_t st = nullptr;
+    ~DevBuf() { if (p) cudaFreeAsync(p, st); }
+    cudaError_t alloc(size_t bytes, cudaStream_t s)
+    {
+        st = s;
+        cudaMemPool_t pool;
+        cudaError_t e = scratch_pool(&pool);
+        return e != cudaSuccess ? e : cudaMallocFromPoolAsync(&p, bytes ? bytes : 16, pool, s);
+    }
     template <typename T> T *as() const { return static_cast<T *>(p); }
 };
 
@@ -339,10 +372,19 @@ struct DevBuf {  // frees on scope exit
 
 extern "C" void hmlfc_stream_free(uint8_t *h_stream) { free(h_stream); }
 
+extern "C" int hmlfc_encode_release_scratch(void)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return HMLFC_E_CUDA;
+    if (g_pool[dev] && (cudaDeviceSynchronize() != cudaSuccess || cudaMemPoolTrimTo(g_pool[dev], 0) != cudaSuccess)) return HMLFC_E_CUDA;
+    return HMLFC_OK;
+}
+
 extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
                             hmlfc_encode_stats_t *stats, void *cuda_stream)
 {
     if (stats) memset(stats, 0, sizeof(*stats));
+    const double t_begin = now_ms();
     if (!d_lf || !p || !h_stream || !len) return HMLFC_E_INVALID;
     const int U = p->U, V = p->V, Ws = p->Ws, Ht = p->Ht, h = p->height, B = p->block, W = p->window;
     if (U < 1 || V < 1 || Ws < 1 || Ht < 1 || h < 1 || p->tau_ref < 0 || p->tau_res < 0 || p->policy < 0 || p->policy > 2) return HMLFC_E_INVALID;
@@ -369,8 +411,8 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
 
     // ---- 1. colour + hierarchy
     DevBuf srv, xk;
-    ENC_CU(srv.alloc((size_t)3 * ns * npx * sizeof(int16_t)));
-    ENC_CU(xk.alloc((size_t)3 * nx * npx * sizeof(int16_t)));
+    ENC_CU(srv.alloc((size_t)3 * ns * npx * sizeof(int16_t), st));
+    ENC_CU(xk.alloc((size_t)3 * nx * npx * sizeof(int16_t), st));
     ENC_CU(cudaEventRecord(ev[0], st));
     int rc = hmlfc_hierarchy(d_lf, U, V, Ws, Ht, h, srv.as<int16_t>(), xk.as<int16_t>(), st);
     if (rc != HMLFC_OK) return rc;
@@ -395,10 +437,10 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
         n_rec += (uint64_t)3 * (pairs[L].size() / 2) * nblk;
     }
     DevBuf rec, dpairs;
-    ENC_CU(rec.alloc((size_t)n_rec * sizeof(int4)));
+    ENC_CU(rec.alloc((size_t)n_rec * sizeof(int4), st));
     size_t pair_words = 0;
     for (int L = 0; L < h; ++L) pair_words += pairs[L].size();
-    ENC_CU(dpairs.alloc(pair_words * sizeof(int32_t)));
+    ENC_CU(dpairs.alloc(pair_words * sizeof(int32_t), st));
     {
         size_t o = 0;
         for (int L = 0; L < h; ++L) {
@@ -440,10 +482,10 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
                     }
     }
     DevBuf dpcs, dflags, dstats, drank;
-    ENC_CU(dpcs.alloc(pcs.size() * sizeof(EncPc)));
-    ENC_CU(dflags.alloc((size_t)flag_words * 4));
-    ENC_CU(dstats.alloc((size_t)n_pc * sizeof(Stats)));
-    ENC_CU(drank.alloc((size_t)n_pc * 2 * fwords * sizeof(uint32_t)));
+    ENC_CU(dpcs.alloc(pcs.size() * sizeof(EncPc), st));
+    ENC_CU(dflags.alloc((size_t)flag_words * 4, st));
+    ENC_CU(dstats.alloc((size_t)n_pc * sizeof(Stats), st));
+    ENC_CU(drank.alloc((size_t)n_pc * 2 * fwords * sizeof(uint32_t), st));
     ENC_CU(cudaMemcpyAsync(dpcs.p, pcs.data(), pcs.size() * sizeof(EncPc), cudaMemcpyHostToDevice, st));
     std::vector<Stats> hstats((size_t)n_pc, Stats{INT_MAX, INT_MIN, 0u, 0u});
     ENC_CU(cudaMemcpyAsync(dstats.p, hstats.data(), hstats.size() * sizeof(Stats), cudaMemcpyHostToDevice, st));
@@ -508,13 +550,13 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
 
     // ---- 6. dense values / records in rank order, then the BISE strings
     DevBuf dpks, dvals, dmvs, dpay, dmvbits, dvjobs, dmjobs;
-    ENC_CU(dpks.alloc(pks.size() * sizeof(EncPack)));
-    ENC_CU(dvals.alloc((size_t)n_vals * sizeof(uint16_t)));
-    ENC_CU(dmvs.alloc((size_t)n_mvs * sizeof(uint32_t)));
-    ENC_CU(dpay.alloc((size_t)(pay_bits / 8 + 8)));
-    ENC_CU(dmvbits.alloc((size_t)(mv_bits / 8 + 8)));
-    ENC_CU(dvjobs.alloc(vjobs.size() * sizeof(PackJob)));
-    ENC_CU(dmjobs.alloc(mjobs.size() * sizeof(PackJob)));
+    ENC_CU(dpks.alloc(pks.size() * sizeof(EncPack), st));
+    ENC_CU(dvals.alloc((size_t)n_vals * sizeof(uint16_t), st));
+    ENC_CU(dmvs.alloc((size_t)n_mvs * sizeof(uint32_t), st));
+    ENC_CU(dpay.alloc((size_t)(pay_bits / 8 + 8), st));
+    ENC_CU(dmvbits.alloc((size_t)(mv_bits / 8 + 8), st));
+    ENC_CU(dvjobs.alloc(vjobs.size() * sizeof(PackJob), st));
+    ENC_CU(dmjobs.alloc(mjobs.size() * sizeof(PackJob), st));
     ENC_CU(cudaMemcpyAsync(dpks.p, pks.data(), pks.size() * sizeof(EncPack), cudaMemcpyHostToDevice, st));
     if (!vjobs.empty()) ENC_CU(cudaMemcpyAsync(dvjobs.p, vjobs.data(), vjobs.size() * sizeof(PackJob), cudaMemcpyHostToDevice, st));
     if (!mjobs.empty()) ENC_CU(cudaMemcpyAsync(dmjobs.p, mjobs.data(), mjobs.size() * sizeof(PackJob), cudaMemcpyHostToDevice, st));
@@ -541,6 +583,7 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
     ENC_CU(cudaGetLastError());
     ENC_CU(cudaEventRecord(ev[5], st));
 
+    const double t_assemble = now_ms();
     // ---- 7. stream assembly on the host (header, raw top-level RKVs, directory) + the three device-built sections
     uint8_t *s = static_cast<uint8_t *>(calloc((size_t)total, 1));
     if (!s) return HMLFC_E_NOMEM;
@@ -586,6 +629,8 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
         cudaEventElapsedTime(&ms, ev[1], ev[2]); stats->ms_search = ms;
         cudaEventElapsedTime(&ms, ev[2], ev[3]); stats->ms_classify = ms;
         cudaEventElapsedTime(&ms, ev[4], ev[5]); stats->ms_pack = ms;
+        stats->ms_wall = (float)(now_ms() - t_begin);
+        stats->ms_assemble = (float)(now_ms() - t_assemble);
         stats->n_plane_channels = (int64_t)n_pc;
         stats->n_res_blocks = (int64_t)tot_res;
         stats->n_pred_blocks = (int64_t)n_mvs;

@@ -45,6 +45,15 @@ constexpr int kMinRec = 64;       // smallest record capacity worth starting wit
 constexpr uint32_t FULL = 0xffffffffu;
 constexpr uint32_t kNone = 0xFFFFFFFFu;
 
+// debug builds (-DHMLFC_PASS_STATS) count the passes of every size and why a pass was split
+#ifdef HMLFC_PASS_STATS
+__device__ unsigned long long g_pass_stats[16];  // [0..2] passes tried at 32/16/8, [3..5] passes done, [6] direct pixels passes, [8..] fail reasons
+#define PASS_STAT(i) do { if (threadIdx.x == 0) atomicAdd(&g_pass_stats[i], 1ull); } while (0)
+#else
+#define PASS_STAT(i) do { } while (0)
+#endif
+
+
 // digits of the packed trit / quint words: trit T -> t0 | t1<<2 | .. | t4<<8, quint Q -> q0 | q1<<3 | q2<<6
 struct DigitLut {
     uint16_t v[384];
@@ -364,7 +373,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         for (int q = tid - 32; q < kSpecZero; q += kNT - 32) z[q] = make_uint4(0u, 0u, 0u, 0u);
     }
     __syncthreads();
-    if (!ctl.fits) return false;
+    if (!ctl.fits) { PASS_STAT(10); return false; }
 
     const int nviews = ctl.nviews, ncell = ctl.ncell, nacc = ctl.nacc, nitems = ctl.nitems, reccap = ctl.reccap;
     uint2 *acc = reinterpret_cast<uint2 *>(arena);
@@ -454,7 +463,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         }
     }
     __syncthreads();
-    if (ctl.overflow != 0) return false;
+    if (ctl.overflow != 0) { PASS_STAT(11); return false; }
     const int nrec = ctl.n_rec;
     // ------------------------------------------------ B2: motion record + reference descriptor, once per block
     for (int rr = tid; rr < nrec; rr += kNT) {
@@ -632,7 +641,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     const int bu0 = ctl.lo[0], bv0 = ctl.lo[1];
     const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
     if (ctl.hi[0] < 0) return true;  // no ray of the sub-tile hits the slab: background only
-    if (nu > kMaxV || nv > kMaxV) return false;
+    if (nu > kMaxV || nv > kMaxV) { PASS_STAT(8); return false; }
     {
         // Early exit before the tables are built: from the pass's exact (u,v) range and (s,t) box, cells ~ (2 ns + nu)
         // (2 nt + nv) (every pixel touches 2 x 2 views) and accumulator samples ~ cells (level 0) + box area x planes
@@ -644,7 +653,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
         int accs = cells;
         for (int L = 1; L < S.h; ++L)
             accs += area * ((((bu0 + nu - 1) >> L) - (bu0 >> L) + 1) * (((bv0 + nv - 1) >> L) - (bv0 >> L) + 1));
-        if (16 * cells + 8 * accs > kArenaBytes * kEstSlackPct / 100) return false;
+        if (16 * cells + 8 * accs > kArenaBytes * kEstSlackPct / 100) { PASS_STAT(9); return false; }
     }
 
     // -------------------------------------------------------- V: footprint box per view
@@ -773,8 +782,11 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
 #pragma unroll
             for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
             setup_rays(S, cam, W, H, sx, sy, ts, pt);
+            PASS_STAT(ts == kTile ? 0 : ts == 16 ? 1 : 2);
             done = tile_pass(S, ctl, arena, pt, rgb);
+            if (done) PASS_STAT(ts == kTile ? 3 : ts == 16 ? 4 : 5);
             if (!done && r >= 0) {
+                PASS_STAT(6);
                 if (pt[0].uv != kNone) rgb[0] = direct_pixel(S, pt[0]);
                 done = true;
             }
@@ -792,6 +804,16 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
 }
 
 }  // namespace
+
+#ifdef HMLFC_PASS_STATS
+extern "C" int hmlfc_debug_pass_stats(unsigned long long *out, int reset)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, g_pass_stats, sizeof(g_pass_stats));
+    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(g_pass_stats, z, sizeof(z)); }
+    return 0;
+}
+#endif
 
 cudaError_t configure_render_cta()
 {

@@ -174,6 +174,15 @@ def test_render_minification_takes_the_fallback_path_and_misses_get_background(P
     assert (expect.reshape(-1, 3) == 0).all(1).any() and expect.any()
 
 
+@pytest.mark.parametrize("name", ["mini2", "mini4"])
+def test_render_eye_on_the_camera_plane(P, enc, name):
+    # SURVEY 8(d) D4 "grid-aligned" batch: eye at z = 0, every ray of a view meets the uv plane at the eye (l0 = 0 exactly),
+    # so a whole view blends the same 4 light-field views
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    _check_views(P, h, s, wl.camera_path(cfg, on_plane=True), cfg.out_w, cfg.out_h)
+
+
 def test_render_host_entry_point(P, enc):
     cfg, lf, data, info, s = enc("mini3")
     h = _loaded(P, enc, "mini3")

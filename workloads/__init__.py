@@ -204,16 +204,18 @@ def _camera(eye, look, tan_half_x, tan_half_y) -> np.ndarray:
     return cam
 
 
-def camera_path(cfg: Config, n_views=None, out_w=None, out_h=None, seed_offset=0, phase=None) -> np.ndarray:
+def camera_path(cfg: Config, n_views=None, out_w=None, out_h=None, seed_offset=0, phase=None, on_plane=False) -> np.ndarray:
     """n_views cameras on the seeded circular path of DESIGN.md "Input recipe":
     eye on a circle of radius 0.25 (U-1) around the uv-rectangle centre at z = -0.25 (U-1), looking at the
-    st-rectangle centre; the frustum covers ~80% of the st rectangle.  Returns float32 [n_views][16]."""
+    st-rectangle centre; the frustum covers ~80% of the st rectangle.  Returns float32 [n_views][16].
+    on_plane: the "grid-aligned" batch of SURVEY 8(d) D4 -- the same circle ON the camera plane (z = 0), so every ray of a
+    view meets the uv plane at the eye and a whole view blends exactly the 4 views around it (best case for sharing)."""
     n_views = cfg.n_views if n_views is None else n_views
     out_w, out_h = out_w or cfg.out_w, out_h or cfg.out_h
     rng = np.random.Generator(np.random.PCG64(cfg.seed + 1000 + seed_offset))
     g = geometry(cfg)
     ccx, ccy = 0.5 * (cfg.U - 1), 0.5 * (cfg.V - 1)
-    rad, ze = 0.25 * (cfg.U - 1), -0.25 * (cfg.U - 1)
+    rad, ze = 0.25 * (cfg.U - 1), (0.0 if on_plane else -0.25 * (cfg.U - 1))
     look = np.array([g["st_origin"][0] + 0.5 * (cfg.Ws - 1) * PITCH, g["st_origin"][1] + 0.5 * (cfg.Ht - 1) * PITCH, g["z_st"]])
     start = rng.uniform(0.0, 2.0 * np.pi) if phase is None else phase
     cams = np.zeros((n_views, 16), dtype=np.float32)
