@@ -239,10 +239,18 @@ __device__ __forceinline__ uint2 bise_row4(const uint32_t *__restrict__ w, uint3
 #ifndef HMLFC_MINB
 #define HMLFC_MINB 3
 #endif
-constexpr int kArenaBytes = HMLFC_ARENA_KB * 1024;  // 3 CTAs per SM: 3 x (68 KB + 6 KB static) of the 228 KB, up to 85 registers per thread.
+constexpr int kArenaDefault = HMLFC_ARENA_KB * 1024;  // 3 CTAs per SM: 3 x (68 KB + 6 KB static) of the 228 KB, up to 85 registers per thread.
 // Measured (A/B on cfg2 / cfg3 / cfg4): 4 x 50 KB: 0.865 / 1.034 / 1.073 ms, 3 x 68 KB: 0.858 / 0.971 / 1.064 ms, 2 x 104 KB: 0.968 / 0.837 /
 // 1.228 ms, 5 x 38 KB: 1.062 / 1.218 / 1.321 ms -- the kernel is not occupancy-bound; fewer spills and fewer split tiles win.
-constexpr int kMinBlocks = HMLFC_MINB;
+constexpr int kMinBlocksDefault = HMLFC_MINB;
+// Second instance for views that look at about as many light-field samples as they have pixels (cfg3: 512^2 views of 512^2 images):
+// 2 CTAs per SM with 104 KB each, so that far fewer tiles have to be split into 16 x 16 / 8 x 8 passes (cfg3: 0.97 -> 0.84 ms).  The
+// launcher picks it from the sizes alone: output pixels per view < 2 x light-field pixels per view (a hint: both give the same bytes).
+#ifndef HMLFC_ARENA_BIG_KB
+#define HMLFC_ARENA_BIG_KB 104
+#endif
+constexpr int kArenaBig = HMLFC_ARENA_BIG_KB * 1024;
+constexpr int kMinBlocksBig = 2;
 #ifndef HMLFC_EST_SLACK
 #define HMLFC_EST_SLACK 120
 #endif
@@ -255,6 +263,7 @@ constexpr int kEstSlackPct = HMLFC_EST_SLACK;  // the 32 x 32 pass is tried when
 #ifndef HMLFC_BP_ATTR
 #define HMLFC_BP_ATTR __forceinline__
 #endif
+template <int kArenaBytes>
 __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -601,6 +610,7 @@ __device__ __forceinline__ void setup_rays(const DevStream &S, const Camera &cam
 // One pass over a (sub-)tile whose rays are set up: footprint boxes (V), tables + decode (build_patch), gather + blend
 // (C).  Returns true (CTA-uniform) when rgb[] holds the pass's pixels (background where the ray misses); false
 // when the tables do not fit the arena and the (sub-)tile must be split.
+template <int kArenaBytes>
 __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, const PixTaps (&pt)[kPPL],
                                           uint32_t (&rgb)[kPPL])
 {
@@ -688,7 +698,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     }
     __syncthreads();
 
-    if (!build_patch(S, ctl, arena)) return false;
+    if (!build_patch<kArenaBytes>(S, ctl, arena)) return false;
 
     // ------------------------------------------------ C: gather + blend
     const float4 *patch = reinterpret_cast<const float4 *>(arena + (((size_t)ctl.nacc * 8 + 15) & ~(size_t)15));
@@ -752,6 +762,7 @@ __device__ __forceinline__ void store1(uint8_t *__restrict__ out, int view, int 
     }
 }
 
+template <int kArenaBytes, int kMinBlocks>
 __global__ void __launch_bounds__(kNT, kMinBlocks)
 render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned)
 {
@@ -783,7 +794,7 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
             for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
             setup_rays(S, cam, W, H, sx, sy, ts, pt);
             PASS_STAT(ts == kTile ? 0 : ts == 16 ? 1 : 2);
-            done = tile_pass(S, ctl, arena, pt, rgb);
+            done = tile_pass<kArenaBytes>(S, ctl, arena, pt, rgb);
             if (done) PASS_STAT(ts == kTile ? 3 : ts == 16 ? 4 : 5);
             if (!done && r >= 0) {
                 PASS_STAT(6);
@@ -817,18 +828,24 @@ extern "C" int hmlfc_debug_pass_stats(unsigned long long *out, int reset)
 
 cudaError_t configure_render_cta()
 {
-    return cudaFuncSetAttribute(render_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaBytes);
+    cudaError_t e = cudaFuncSetAttribute(render_cta_kernel<kArenaDefault, kMinBlocksDefault>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaDefault);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(render_cta_kernel<kArenaBig, kMinBlocksBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaBig);
 }
 
 cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
-                              int *n_launches)
+                              int *n_launches, int arena)
 {
     if (n_views == 0) return cudaSuccess;
     if (S.B != 4) return cudaErrorInvalidValue;  // block-row tasks are written for 4 x 4 blocks; the caller dispatches other sizes elsewhere
     dim3 block(kNT), grid((unsigned)((W + kTile - 1) / kTile), (unsigned)((H + kTile - 1) / kTile), (unsigned)n_views);
     if (grid.y > 65535u) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0 && (W % 4) == 0) ? 1 : 0;
-    render_cta_kernel<<<grid, block, kArenaBytes, st>>>(S, d_cams, W, H, d_out, aligned);
+    // measured (default / big, ms per step): cfg2 0.866 / 0.970, cfg3 0.975 / 0.837, cfg3 with the eye on the camera plane 2.24 / 1.08,
+    // cfg1 0.070 / 0.039
+    const bool big = arena < 0 ? (long long)W * H < 2LL * S.Ws * S.Ht : arena == 1;
+    if (big) render_cta_kernel<kArenaBig, kMinBlocksBig><<<grid, block, kArenaBig, st>>>(S, d_cams, W, H, d_out, aligned);
+    else render_cta_kernel<kArenaDefault, kMinBlocksDefault><<<grid, block, kArenaDefault, st>>>(S, d_cams, W, H, d_out, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
