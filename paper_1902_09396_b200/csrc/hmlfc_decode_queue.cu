@@ -157,7 +157,11 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
     const bool present = i < n;
     int4 c4 = make_int4(0, 0, 0, 0);
+#ifdef HMLFC_DECODE_CS
+    if (present) c4 = __ldcs(coords + i);
+#else
     if (present) c4 = __ldg(coords + i);
+#endif
     const bool valid = present && (unsigned)c4.x < (unsigned)S.U && (unsigned)c4.y < (unsigned)S.V &&
                        (unsigned)c4.z < (unsigned)S.Ws && (unsigned)c4.w < (unsigned)S.Ht;
     if (present && !valid) atomicAdd(oob, 1ull);
@@ -233,7 +237,11 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
         sb[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
         sb[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
         __syncwarp();
+#ifdef HMLFC_DECODE_CS
+        if (lane < 24) __stcs(reinterpret_cast<uint32_t *>(o) + lane, q.stage[lane]);
+#else
         if (lane < 24) reinterpret_cast<uint32_t *>(o)[lane] = q.stage[lane];
+#endif
     } else if (present) {
         o[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
         o[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
