@@ -571,7 +571,9 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
         if (B == 2) COMPACT(2); else if (B == 4) COMPACT(4); else COMPACT(8);
 #undef COMPACT
     }
-    auto pack_grid_x = [](uint64_t groups) { uint64_t g = (groups + kThreads - 1) / kThreads; return (unsigned)(g > 4096 ? 4096 : g); };
+    // grid = (CTAs per string, strings): the strings differ in length, so a string gets at most 32 CTAs that stride over its groups
+    // (a CTA whose first group is beyond the string leaves at once)
+    auto pack_grid_x = [](uint64_t groups) { uint64_t g = (groups + kThreads - 1) / kThreads; return (unsigned)(g > 32 ? 32 : g); };
     for (size_t j0 = 0; j0 < vjobs.size(); j0 += 65535) {
         const unsigned nj = (unsigned)(vjobs.size() - j0 < 65535 ? vjobs.size() - j0 : 65535);
         pack_kernel<uint16_t><<<dim3(pack_grid_x(max_vgroups), nj), kThreads, 0, st>>>(dvals.as<uint16_t>(), dvjobs.as<PackJob>() + j0, dpay.as<uint32_t>());

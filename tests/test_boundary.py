@@ -83,6 +83,19 @@ def test_entry_points_validate_arguments(P):
     assert L.hmlfc_hierarchy(None, 2, 2, 8, 8, 1, None, None, None) == -4
     assert P.hmlfc_hierarchy_sizes(17, 17, 3) == (17 * 17 + 9 * 9 + 5 * 5, 9 * 9 + 5 * 5 + 3 * 3)   # 17 -> 9 -> 5 -> 3 (R3)
     assert P.hmlfc_hierarchy_sizes(16, 16, 3) == (256 + 64 + 16, 64 + 16 + 4)
+    # hmlfc_encode checks its arguments before any CUDA call
+    out, n = C.c_void_p(), C.c_size_t()
+    p = P.EncodeParams()
+    p.U, p.V, p.Ws, p.Ht, p.height, p.block, p.window = 2, 2, 16, 16, 1, 4, 4
+    dummy = C.c_void_p(16)
+    assert L.hmlfc_encode(None, C.byref(p), C.byref(out), C.byref(n), None, None) == -4     # null light field
+    p.block = 3
+    assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -5    # B not in {2, 4, 8}
+    p.block, p.Ws = 4, 18
+    assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -5    # B does not divide Ws
+    p.Ws, p.policy = 16, 3
+    assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -4    # unknown policy
+    L.hmlfc_stream_free(None)  # no-op
 
 
 def test_no_cpu_fallback(P, enc):
