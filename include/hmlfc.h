@@ -129,12 +129,13 @@ int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n
 int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out);
 
 /* Kernel selection for hmlfc_render (A/B measurements and cross-checks; all variants produce identical
- * bytes): 0 = automatic (default: 6 or 7 for B = 4 streams, else 4), 1 = one thread per output pixel (16
+ * bytes): 0 = automatic (default: 6, 7 or 8 for B = 4 streams, else 4), 1 = one thread per output pixel (16
  * independent tap decodes), 2 = sample-shared tile, 3 = block-centric CTA tile (32 x 8), 4 / 5 = the
- * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile, 6 / 7 = CTA per 32 x 32 tile with
+ * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile, 6 / 7 / 8 = CTA per 32 x 32 tile with
  * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows), with a
- * 68 KB (3 CTAs per SM) / 104 KB (2 CTAs per SM) shared-memory arena; the automatic choice takes 7 when a
- * view has fewer than twice the pixels of a light-field image (little magnification: more samples per tile). */
+ * 68 KB (3 CTAs per SM) / 104 KB (2 CTAs per SM) / 50 KB (4 CTAs per SM) shared-memory arena; the automatic
+ * choice takes 7 when a view has fewer than twice the pixels of a light-field image (little magnification:
+ * more samples per tile), 8 when it has at least eight times as many, else 6. */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Progressive decoding (PAPER.md:57, :183 name the property; R26): hmlfc_decode / hmlfc_render sum the top-level RKV and the

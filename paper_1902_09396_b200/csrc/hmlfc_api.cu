@@ -183,7 +183,7 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     const Camera *cams = reinterpret_cast<const Camera *>(d_cameras);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the CTA kernel
-    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || h->render_variant == 6 || h->render_variant == 7);
+    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || (h->render_variant >= 6 && h->render_variant <= 8));
     if (h->render_variant == 1 || (h->ds.lmin > 0 && !cta_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 2)
@@ -192,8 +192,8 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
         CU(h, launch_render_blocks(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 4 || h->render_variant == 5 || h->ds.B != 4)
         CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 5 ? 1 : 0));
-    else  // 0 (default: arena chosen from the sizes), 6 (68 KB arena), 7 (104 KB arena): block-row kernel, written for 4 x 4 blocks
-        CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 6 ? 0 : h->render_variant == 7 ? 1 : -1));
+    else  // 0 (default: arena chosen from the sizes), 6 / 7 / 8 (68 / 104 / 50 KB arena): block-row kernel, written for 4 x 4 blocks
+        CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant >= 6 ? h->render_variant - 6 : -1));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -335,7 +335,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 7) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 8) return HMLFC_E_INVALID;
     h->render_variant = variant;
     return HMLFC_OK;
 }

@@ -33,7 +33,7 @@ cudaError_t launch_render_warp(const DevStream &S, const Camera *d_cams, int n_v
                                int *n_launches, int shape);
 cudaError_t configure_render_warp();
 // CTA per 32 x 32 tile, block-row tasks (B = 4 streams only; returns cudaErrorInvalidValue otherwise)
-// arena: 0 = 3 CTAs x 68 KB per SM, 1 = 2 CTAs x 104 KB, -1 = chosen from the output and light-field sizes
+// arena: 0 = 3 CTAs x 68 KB per SM, 1 = 2 CTAs x 104 KB, 2 = 4 CTAs x 50 KB, -1 = chosen from the output and light-field sizes
 cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
                               int *n_launches, int arena);
 cudaError_t configure_render_cta();

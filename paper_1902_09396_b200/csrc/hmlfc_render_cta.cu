@@ -251,6 +251,9 @@ constexpr int kMinBlocksDefault = HMLFC_MINB;
 #endif
 constexpr int kArenaBig = HMLFC_ARENA_BIG_KB * 1024;
 constexpr int kMinBlocksBig = 2;
+// Third instance for strong magnification (cfg5: 2048^2 views of 640^2 images, a tile looks at few samples): 4 CTAs x 50 KB, <= 64 registers.
+constexpr int kArenaSmall = 50 * 1024;
+constexpr int kMinBlocksSmall = 4;
 #ifndef HMLFC_EST_SLACK
 #define HMLFC_EST_SLACK 120
 #endif
@@ -830,6 +833,7 @@ cudaError_t configure_render_cta()
 {
     cudaError_t e = cudaFuncSetAttribute(render_cta_kernel<kArenaDefault, kMinBlocksDefault>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaDefault);
     if (e != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(render_cta_kernel<kArenaSmall, kMinBlocksSmall>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaSmall)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(render_cta_kernel<kArenaBig, kMinBlocksBig>, cudaFuncAttributeMaxDynamicSharedMemorySize, kArenaBig);
 }
 
@@ -841,10 +845,12 @@ cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_vi
     dim3 block(kNT), grid((unsigned)((W + kTile - 1) / kTile), (unsigned)((H + kTile - 1) / kTile), (unsigned)n_views);
     if (grid.y > 65535u) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0 && (W % 4) == 0) ? 1 : 0;
-    // measured (default / big, ms per step): cfg2 0.866 / 0.970, cfg3 0.975 / 0.837, cfg3 with the eye on the camera plane 2.24 / 1.08,
-    // cfg1 0.070 / 0.039
-    const bool big = arena < 0 ? (long long)W * H < 2LL * S.Ws * S.Ht : arena == 1;
-    if (big) render_cta_kernel<kArenaBig, kMinBlocksBig><<<grid, block, kArenaBig, st>>>(S, d_cams, W, H, d_out, aligned);
+    // measured, ms per step (68 KB x 3 / 104 KB x 2 / 50 KB x 4): cfg2 0.850 / 0.950 / 0.859, cfg3 0.975 / 0.837 / -, cfg3 with the eye on
+    // the camera plane 2.24 / 1.08 / -, cfg4 1.010 / 1.163 / 1.035, cfg5 1.538 / 1.828 / 1.401, cfg1 0.070 / 0.039 / -
+    if (arena < 0) arena = (long long)W * H < 2LL * S.Ws * S.Ht ? 1 : ((long long)W * H >= 8LL * S.Ws * S.Ht ? 2 : 0);
+    const bool big = arena == 1;
+    if (arena == 2) render_cta_kernel<kArenaSmall, kMinBlocksSmall><<<grid, block, kArenaSmall, st>>>(S, d_cams, W, H, d_out, aligned);
+    else if (big) render_cta_kernel<kArenaBig, kMinBlocksBig><<<grid, block, kArenaBig, st>>>(S, d_cams, W, H, d_out, aligned);
     else render_cta_kernel<kArenaDefault, kMinBlocksDefault><<<grid, block, kArenaDefault, st>>>(S, d_cams, W, H, d_out, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();

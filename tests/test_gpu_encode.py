@@ -83,15 +83,27 @@ def test_encoded_stream_loads_and_decodes_to_the_oracle_reconstruction(P, enc):
     P.hmlfc_free(h)
 
 
-def test_cfg2_full_size_stream_equals_the_oracle_stream(P):
-    """BASELINE.json configs[1] at full size (16 x 16 views of 256 x 256, h = 3, B = 4, W = 16, ~40 dB): 7.5 MB stream."""
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_full_size_stream_equals_the_oracle_stream(P, name):
+    """BASELINE.json configs[1..4] at full size: the GPU encoder's stream against the oracle encoder's cached stream (cfg2: 7.5 MB,
+    cfg3: 82 MB, cfg4: 175 MB, cfg5: 1.04 GB).  cfg2 and cfg3 always run; cfg4 / cfg5 when HMLFC_FULL names them (the oracle needs
+    ~75 s / ~8 min on 16 cores for what the GPU encoder does in 0.26 s / 1.6 s; results recorded in profiles/r01_all_configs.md)."""
+    import os
+
     from oracle import streams
 
-    cfg, data, info = streams.get_stream("cfg2")
+    extra = [c for c in os.environ.get("HMLFC_FULL", "").split(",") if c]
+    if name in ("cfg4", "cfg5") and name not in extra:
+        pytest.skip(f"{name}: set HMLFC_FULL={name} (oracle encode takes minutes)")
+    cfg, data, info = streams.get_stream(name)
     lf = wl.light_field(cfg)
     got, stats = _gpu_encode(P, cfg, lf, info["tau_ref"], info["tau_res"])
+    del lf
+    P.hmlfc_encode_release_scratch()
     _assert_same_stream(got, data)
-    assert stats["n_search_blocks"] == 3 * (192 + 48 + 12) * 4096
+    n_pairs = sum((((cfg.U - 1) >> L) + 1) * (((cfg.V - 1) >> L) + 1) - ((((cfg.U - 1) >> L) + 2) // 2) * ((((cfg.V - 1) >> L) + 2) // 2)
+                  for L in range(cfg.height))
+    assert stats["n_search_blocks"] == 3 * n_pairs * (cfg.Ws // cfg.block) * (cfg.Ht // cfg.block)
 
 
 def test_invalid_and_unsupported_arguments(P):

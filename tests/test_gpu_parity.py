@@ -101,7 +101,7 @@ def test_decode_host_entry_point(P, enc):
 def _check_views(P, h, s, cams, W, H):
     expect = s.render(cams, W, H)
     outs = {}
-    for variant in (P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG):
+    for variant in (P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
         P.hmlfc_set_render_variant(h, variant)
         got = P.hmlfc_render(h, _dev(cams), W, H).cpu().numpy()
         d = np.abs(got.astype(np.int16) - expect.astype(np.int16))
@@ -115,6 +115,7 @@ def _check_views(P, h, s, cams, W, H):
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP8])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA_BIG])
+    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA_SMALL])
     return expect
 
 
@@ -212,7 +213,7 @@ def test_progressive_levels_match_oracle(P, enc, name):
             assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), (L, variant)
         ref = s.render(cams, cfg.out_w, cfg.out_h)
         outs = []
-        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG):   # WARP falls back to the per-pixel kernel when L > 0
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):   # WARP falls back to the per-pixel kernel when L > 0
             P.hmlfc_set_render_variant(h, variant)
             got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
             assert np.abs(got.astype(np.int16) - ref.astype(np.int16)).max() <= TOL_VIEW, (L, variant)
@@ -297,7 +298,7 @@ def test_full_size_sampled_parity(P, name):
     assert n_diff < 1e-3 * n_all
     P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)   # the unshared thread-per-pixel kernel on the first view
     assert np.array_equal(P.hmlfc_render(h, _dev(cams[:1]), cfg.out_w, cfg.out_h).cpu().numpy()[0], got[0])
-    for variant in (P.RENDER_CTA, P.RENDER_CTA_BIG):   # both shared-memory configurations of the CTA kernel (the default picks one)
+    for variant in (P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):   # the three shared-memory configurations of the CTA kernel (the default picks one)
         P.hmlfc_set_render_variant(h, variant)
         assert np.array_equal(P.hmlfc_render(h, _dev(cams[:2]), cfg.out_w, cfg.out_h).cpu().numpy(), got[:2])
     P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
