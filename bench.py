@@ -356,6 +356,13 @@ def run_ours(args, cfg_name):
             "oracle_encode_seconds": info.get("encode_seconds"),
             "oracle_note": "the oracle's encode of the same light field on the host cores when the cached stream was made (includes its tau bisection)",
         }
+        if cfg.target_psnr is not None:  # the same with the thresholds found by bisection to the configuration's PSNR target
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            b_bytes, b_stats = P.hmlfc_encode(lf_dev, cfg.height, cfg.block, cfg.window, target_psnr=cfg.target_psnr, **enc_kw)
+            encode["bisection"] = {"ms_wall": 1e3 * (time.perf_counter() - t0), "steps": b_stats["bisection_steps"], "tau_res": b_stats["tau_res"],
+                                   "psnr_db": round(b_stats["psnr"], 4), "stream_equals_oracle_stream": bool(b_bytes == data)}
+            del b_bytes
         del lf_dev, enc_bytes
         P.hmlfc_encode_release_scratch()
 

@@ -202,9 +202,20 @@ typedef struct {
     float ms_wall, ms_assemble;                            /* host wall clock: the whole call; stream assembly + copies to the host */
     int64_t n_plane_channels, n_res_blocks, n_pred_blocks, n_search_blocks;
     int32_t kernel_launches, cuda_error;
+    int64_t sse;                  /* sum of squared RGB differences between the stream's reconstruction and the input */
+    double psnr;                  /* 10 log10(255^2 / (sse / bytes)); +inf when sse = 0 */
+    int32_t tau_ref, tau_res;     /* the thresholds written to the stream */
+    int32_t bisection_steps, _pad;
 } hmlfc_encode_stats_t;
 int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
                  hmlfc_encode_stats_t *stats, void *cuda_stream);
+/* The same with the thresholds chosen for a quality target ("encoding parameters are varied ... to achieve a
+ * similar compression quality"; W3, R24): bisection of tau_res over [0, 4096] with tau_ref = floor(tau_res / 2), at most
+ * max_iter steps, until the PSNR of the reconstruction (what hmlfc_decode returns for the stream, computed by a kernel from the
+ * encoder's planes) is within tol dB of target_psnr; the closest step wins.  p's tau_ref / tau_res are ignored.  Hierarchy and
+ * search run once.  HMLFC_E_INVALID for a negative or non-finite target, tol < 0 or max_iter < 1. */
+int hmlfc_encode_psnr(const uint8_t *d_lf, const hmlfc_encode_params_t *p, double target_psnr, double tol, int max_iter,
+                      uint8_t **h_stream, size_t *len, hmlfc_encode_stats_t *stats, void *cuda_stream);
 void hmlfc_stream_free(uint8_t *h_stream);
 /* hmlfc_encode keeps its device scratch in a stream-ordered memory pool of the current device between calls (a second call
  * allocates nothing from the driver); this returns it.  Synchronises the device. */

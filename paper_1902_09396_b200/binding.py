@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 # every symbol include/hmlfc.h declares
 EXPORTS = (
     "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
-    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
+    "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
@@ -88,6 +88,8 @@ def lib():
     L.hmlfc_encode.argtypes = [vp, vp, C.POINTER(vp), C.POINTER(C.c_size_t), vp, vp]
     L.hmlfc_encode.restype = C.c_int
     L.hmlfc_stream_free.argtypes, L.hmlfc_stream_free.restype = [vp], None
+    L.hmlfc_encode_psnr.argtypes = [vp, vp, C.c_double, C.c_double, C.c_int, C.POINTER(vp), C.POINTER(C.c_size_t), vp, vp]
+    L.hmlfc_encode_psnr.restype = C.c_int
     L.hmlfc_encode_release_scratch.argtypes, L.hmlfc_encode_release_scratch.restype = [], C.c_int
     L.hmlfc_free.argtypes, L.hmlfc_free.restype = [vp], None
     L.hmlfc_strerror.argtypes, L.hmlfc_strerror.restype = [C.c_int], C.c_char_p
@@ -288,13 +290,17 @@ class EncodeStats(C.Structure):
     _fields_ = [("ms_hierarchy", C.c_float), ("ms_search", C.c_float), ("ms_classify", C.c_float), ("ms_pack", C.c_float),
                 ("ms_wall", C.c_float), ("ms_assemble", C.c_float),
                 ("n_plane_channels", C.c_int64), ("n_res_blocks", C.c_int64), ("n_pred_blocks", C.c_int64),
-                ("n_search_blocks", C.c_int64), ("kernel_launches", C.c_int32), ("cuda_error", C.c_int32)]
+                ("n_search_blocks", C.c_int64), ("kernel_launches", C.c_int32), ("cuda_error", C.c_int32),
+                ("sse", C.c_int64), ("psnr", C.c_double), ("tau_ref", C.c_int32), ("tau_res", C.c_int32),
+                ("bisection_steps", C.c_int32), ("_pad", C.c_int32)]
 
 
 def hmlfc_encode(lf, height: int, block: int = 4, window: int = 16, tau_ref: int = 0, tau_res: int = 0, policy: int = 0,
-                 geometry: dict = None, background=(0, 0, 0), seed: int = 0, stream=None):
+                 geometry: dict = None, background=(0, 0, 0), seed: int = 0, stream=None, target_psnr: float = None,
+                 tol: float = 0.25, max_iter: int = 12):
     """lf: cuda uint8 [V][U][Ht][Ws][3].  Returns (stream bytes, stats dict): the whole encoder runs in CUDA kernels, the host
-    only lays out the sections.  geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab."""
+    only lays out the sections.  geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab.
+    target_psnr: let hmlfc_encode_psnr choose the thresholds by bisection (tau_ref / tau_res are then ignored)."""
     torch = _require_cuda()
     assert lf.is_cuda and lf.dtype == torch.uint8 and lf.is_contiguous() and lf.dim() == 5 and lf.shape[4] == 3
     p = EncodeParams()
@@ -309,14 +315,18 @@ def hmlfc_encode(lf, height: int, block: int = 4, window: int = 16, tau_ref: int
     p.seed = seed
     out, n, stats = C.c_void_p(), C.c_size_t(), EncodeStats()
     st = stream if stream is not None else torch.cuda.current_stream()
-    rc = lib().hmlfc_encode(C.c_void_p(lf.data_ptr()), C.byref(p), C.byref(out), C.byref(n), C.byref(stats), C.c_void_p(st.cuda_stream))
+    if target_psnr is None:
+        rc = lib().hmlfc_encode(C.c_void_p(lf.data_ptr()), C.byref(p), C.byref(out), C.byref(n), C.byref(stats), C.c_void_p(st.cuda_stream))
+    else:
+        rc = lib().hmlfc_encode_psnr(C.c_void_p(lf.data_ptr()), C.byref(p), float(target_psnr), float(tol), int(max_iter), C.byref(out),
+                                     C.byref(n), C.byref(stats), C.c_void_p(st.cuda_stream))
     if rc != 0:
         raise HmlfcError(rc, "hmlfc_encode", f"{lib().hmlfc_strerror(rc).decode()} (cuda error {stats.cuda_error})")
     try:
         data = C.string_at(out, n.value)
     finally:
         lib().hmlfc_stream_free(out)
-    return data, {k: getattr(stats, k) for k, _ in EncodeStats._fields_}
+    return data, {k: getattr(stats, k) for k, _ in EncodeStats._fields_ if k != "_pad"}
 
 
 def hmlfc_encode_release_scratch():

@@ -24,6 +24,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <chrono>
+#include <cmath>
 #include <vector>
 
 namespace {
@@ -78,37 +79,18 @@ __device__ __forceinline__ void load_row(const int16_t *__restrict__ p, int (&v)
     }
 }
 
-template <int B>
-__device__ __forceinline__ void store_row(int16_t *__restrict__ p, const int (&v)[B])
-{
-    if constexpr (B % 4 == 0) {
-#pragma unroll
-        for (int q = 0; q < B / 4; ++q) {
-            uint2 w;
-            w.x = ((uint32_t)v[4 * q + 0] & 0xFFFFu) | ((uint32_t)v[4 * q + 1] << 16);
-            w.y = ((uint32_t)v[4 * q + 2] & 0xFFFFu) | ((uint32_t)v[4 * q + 3] << 16);
-            *reinterpret_cast<uint2 *>(p + 4 * q) = w;
-        }
-    } else if constexpr (B == 2) {
-        *reinterpret_cast<uint32_t *>(p) = ((uint32_t)v[0] & 0xFFFFu) | ((uint32_t)v[1] << 16);
-    } else {
-#pragma unroll
-        for (int i = 0; i < B; ++i) p[i] = (int16_t)v[i];
-    }
-}
-
 // ---------------------------------------------------------------------------------------------------------------
 // classify_kernel: one lane per block, one warp per 32-block flag word of one plane-channel.
 //   energy E = sum |SRV block|; reference plane: res = E >= tau_ref;
 //   predictive plane (R13), with Delta = the search's best SAD: adaptive: worth = E >= tau_res, pred = worth and Delta < E,
 //   res = worth and (pred ? Delta : E) >= tau_res; all: pred = 1, res = Delta >= tau_res; literal: pred = res = Delta >= tau_res.
-//   A predicted block is REPLACED IN PLACE by its residual e = P -+ R(x+dx, y+dy) (R10, R8, R12): only
-//   reference planes are read by other blocks, and those are never written.
+//   The stored values of a predicted block are its residual e = P -+ R(x+dx, y+dy) (replacement step; R10, R8,
+//   R12); the SRV planes themselves stay untouched, so the thresholds can be changed and the kernel run again (tau bisection).
 // Outputs: the `res` / `pred` flag words (ballots) straight into the stream's flag section, and per plane-channel the range of
 // the stored values of its `res` blocks and the two block counts.
 template <int B>
 __global__ void __launch_bounds__(kThreads)
-classify_kernel(int16_t *__restrict__ srv, const int4 *__restrict__ rec, const EncPc *__restrict__ pcs, int Ws, int Ht, int nbx,
+classify_kernel(const int16_t *__restrict__ srv, const int4 *__restrict__ rec, const EncPc *__restrict__ pcs, int Ws, int Ht, int nbx,
                 int nblk, int fwords, int tau_ref, int tau_res, int policy, uint32_t *__restrict__ flags, Stats *__restrict__ stats)
 {
     const int k = blockIdx.y;
@@ -122,7 +104,7 @@ classify_kernel(int16_t *__restrict__ srv, const int4 *__restrict__ rec, const E
     int vmin = INT_MAX, vmax = INT_MIN;
     if (b < nblk) {
         const int by = b / nbx, bx = b - by * nbx;
-        int16_t *P = srv + pc.srv_off + (size_t)(by * B) * Ws + bx * B;
+        const int16_t *P = srv + pc.srv_off + (size_t)(by * B) * Ws + bx * B;
         int v[B][B];
         int E = 0;
 #pragma unroll
@@ -157,7 +139,6 @@ classify_kernel(int16_t *__restrict__ srv, const int4 *__restrict__ rec, const E
                         const int q = (x >= 0 && x < Ws && y >= 0 && y < Ht) ? (int)R[(size_t)y * Ws + x] : 0;
                         v[j][i] = r.x ? v[j][i] + q : v[j][i] - q;
                     }
-                    store_row<B>(P + (size_t)j * Ws, v[j]);
                 }
             }
         }
@@ -215,7 +196,7 @@ rank_kernel(const uint32_t *__restrict__ flags, const EncPc *__restrict__ pcs, i
 template <int B>
 __global__ void __launch_bounds__(kThreads)
 compact_kernel(const int16_t *__restrict__ srv, const int4 *__restrict__ rec, const EncPc *__restrict__ pcs, const EncPack *__restrict__ pks,
-               int Ws, int nbx, int nblk, int fwords, int window, const uint32_t *__restrict__ flags, const uint32_t *__restrict__ rank,
+               int Ws, int Ht, int nbx, int nblk, int fwords, int window, const uint32_t *__restrict__ flags, const uint32_t *__restrict__ rank,
                uint16_t *__restrict__ vals, uint32_t *__restrict__ mvs)
 {
     const int k = blockIdx.y;
@@ -228,29 +209,101 @@ compact_kernel(const int16_t *__restrict__ srv, const int4 *__restrict__ rec, co
     const int b = fw * 32 + lane;
     const uint32_t below = (1u << lane) - 1u;
     const uint32_t wres = flags[pc.flag_word + fw];
+    const uint32_t wpred = predictive ? flags[pc.flag_word + fwords + fw] : 0u;
+    const bool pred = (wpred >> lane) & 1u;
+    int4 m = make_int4(0, 0, 0, 0);
+    if (pred) m = rec[pc.rec_off + b];  // mode, dx, dy, Delta
     if ((wres >> lane) & 1u) {
         const int by = b / nbx, bx = b - by * nbx;
         const int16_t *P = srv + pc.srv_off + (size_t)(by * B) * Ws + bx * B;
+        const int16_t *R = srv + pc.ref_off;
         const uint64_t r = (uint64_t)rank[((size_t)k * 2) * fwords + fw] + (uint64_t)__popc(wres & below);
         uint16_t *o = vals + pk.val_base + r * (B * B);
 #pragma unroll
         for (int j = 0; j < B; ++j) {
             int v[B];
             load_row<B>(P + (size_t)j * Ws, v);
+            if (pred) {  // the residual of the replacement step, as in classify_kernel
+                const int y = by * B + j + m.z;
+#pragma unroll
+                for (int i = 0; i < B; ++i) {
+                    const int x = bx * B + i + m.y;
+                    const int q = (x >= 0 && x < Ws && y >= 0 && y < Ht) ? (int)R[(size_t)y * Ws + x] : 0;
+                    v[i] = m.x ? v[i] + q : v[i] - q;
+                }
+            }
 #pragma unroll
             for (int i = 0; i < B; ++i) o[j * B + i] = (uint16_t)(v[i] - pk.offset);
         }
     }
     if (predictive) {
-        const uint32_t wpred = flags[pc.flag_word + fwords + fw];
-        if ((wpred >> lane) & 1u) {
-            const int4 m = rec[pc.rec_off + b];
+        if (pred) {
             const uint32_t nd = (uint32_t)(2 * window + 1);
             const uint64_t r = (uint64_t)rank[((size_t)k * 2 + 1) * fwords + fw] + (uint64_t)__popc(wpred & below);
             mvs[pk.mv_base + r] = (uint32_t)m.x * nd * nd + (uint32_t)(m.z + window) * nd + (uint32_t)(m.y + window);
         }
     }
     (void)nblk;
+}
+
+// reconstruct_sse_kernel: the encoder's own dense reconstruction at the current thresholds (what a decoder
+// makes of the stream) and its squared error against the input, one thread per light-field pixel:
+//   acc_c = X_h + sum_L [ res ? stored : 0 ] + [ pred ? +-R'(x+dx, y+dy) : 0 ],  stored = P (reference / intra) or P -+ R(x+dx, y+dy),
+//   R' = the reference sample AS STORED (0 where its block is insignificant or outside the image), R = the unthresholded one (R12);
+//   then inverse YCoCg-R and clamp (R17, R19).  The sum of squared RGB differences feeds the PSNR of PAPER.md:366 / :375.
+struct RecGeom {
+    int h, U, V, Ws, Ht, nbx, fwords, shiftB;  // block = 1 << shiftB
+    int UL[9];
+    uint32_t kbase[9];                            // first plane-channel (stream order) of level L
+    uint64_t top_off, x_ch;                       // element offset of the top-level RKV planes of channel 0 in d_x; channel stride
+};
+
+__global__ void __launch_bounds__(kThreads)
+reconstruct_sse_kernel(const uint8_t *__restrict__ lf, const int16_t *__restrict__ srv, const int16_t *__restrict__ xk, const int4 *__restrict__ rec,
+                       const EncPc *__restrict__ pcs, const uint32_t *__restrict__ flags, RecGeom G, unsigned long long n_px,
+                       unsigned long long *__restrict__ sse)
+{
+    const unsigned long long g = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
+    unsigned long long err = 0ull;
+    if (g < n_px) {
+        const unsigned long long npx = (unsigned long long)G.Ws * G.Ht;
+        const int view = (int)(g / npx), pix = (int)(g - (unsigned long long)view * npx);
+        const int v = view / G.U, u = view - v * G.U, t = pix / G.Ws, s = pix - t * G.Ws;
+        const int b = (t >> G.shiftB) * G.nbx + (s >> G.shiftB);
+        int a[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            int acc = xk[G.top_off + (uint64_t)c * G.x_ch + (uint64_t)((v >> G.h) * G.UL[G.h] + (u >> G.h)) * npx + pix];
+            for (int L = 0; L < G.h; ++L) {
+                const int pu = u >> L, pv = v >> L;
+                const EncPc pc = pcs[G.kbase[L] + (uint32_t)(pv * G.UL[L] + pu) * 3u + c];
+                const bool res = (flags[pc.flag_word + (b >> 5)] >> (b & 31)) & 1u;
+                const int P = srv[pc.srv_off + pix];
+                int term = res ? P : 0;
+                if (pc.rec_off != kNoRec && ((flags[pc.flag_word + G.fwords + (b >> 5)] >> (b & 31)) & 1u)) {
+                    const int4 m = rec[pc.rec_off + b];
+                    const int x = s + m.y, y = t + m.z;
+                    int q = 0, qs = 0;
+                    if (x >= 0 && x < G.Ws && y >= 0 && y < G.Ht) {
+                        q = srv[pc.ref_off + (size_t)y * G.Ws + x];
+                        const EncPc rp = pcs[G.kbase[L] + (uint32_t)((pv & ~1) * G.UL[L] + (pu & ~1)) * 3u + c];
+                        const int rb = (y >> G.shiftB) * G.nbx + (x >> G.shiftB);
+                        qs = ((flags[rp.flag_word + (rb >> 5)] >> (rb & 31)) & 1u) ? q : 0;
+                    }
+                    term = (res ? (m.x ? P + q : P - q) : 0) + (m.x ? -qs : qs);
+                }
+                acc += term;
+            }
+            a[c] = acc;
+        }
+        const int tt = a[0] - (a[2] >> 1), Gc = a[2] + tt, Bc = tt - (a[1] >> 1), Rc = Bc + a[1];  // inverse YCoCg-R lifting
+        const uint8_t *px = lf + g * 3ull;
+        const int dr = min(max(Rc, 0), 255) - (int)px[0], dg = min(max(Gc, 0), 255) - (int)px[1], db = min(max(Bc, 0), 255) - (int)px[2];
+        err = (unsigned long long)(dr * dr + dg * dg + db * db);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) err += __shfl_xor_sync(FULL, err, o);
+    if ((threadIdx.x & 31) == 0 && err) atomicAdd(sse, err);
 }
 
 // n <= 32 bits of v into an LSB-first 32-bit word string (zero-initialised; neighbouring groups share words)
@@ -380,12 +433,18 @@ extern "C" int hmlfc_encode_release_scratch(void)
     return HMLFC_OK;
 }
 
-extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
-                            hmlfc_encode_stats_t *stats, void *cuda_stream)
+// target_psnr < 0: encode at p's thresholds.  Otherwise ("encoding parameters are varied ... to achieve a similar
+// compression quality"; W3, R24): bisection of tau_res in [0, 4096] with tau_ref = floor(tau_res / 2), at most max_iter
+// steps, until the PSNR of the reconstruction is within tol of the target; the closest step wins.  Hierarchy and search run once
+// (they do not depend on the thresholds, R12); every step is one classify pass + one reconstruction pass.
+static int encode_impl(const uint8_t *d_lf, const hmlfc_encode_params_t *p_in, double target_psnr, double tol, int max_iter,
+                       uint8_t **h_stream, size_t *len, hmlfc_encode_stats_t *stats, void *cuda_stream)
 {
     if (stats) memset(stats, 0, sizeof(*stats));
     const double t_begin = now_ms();
-    if (!d_lf || !p || !h_stream || !len) return HMLFC_E_INVALID;
+    if (!d_lf || !p_in || !h_stream || !len) return HMLFC_E_INVALID;
+    hmlfc_encode_params_t prm = *p_in;
+    hmlfc_encode_params_t *p = &prm;
     const int U = p->U, V = p->V, Ws = p->Ws, Ht = p->Ht, h = p->height, B = p->block, W = p->window;
     if (U < 1 || V < 1 || Ws < 1 || Ht < 1 || h < 1 || p->tau_ref < 0 || p->tau_res < 0 || p->policy < 0 || p->policy > 2) return HMLFC_E_INVALID;
     if (h > 8 || (B != 2 && B != 4 && B != 8) || W < 0 || W > 64 || Ws % B || Ht % B || Ws % 4 || (long long)U * V > (1 << 24))
@@ -487,25 +546,76 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
     ENC_CU(dstats.alloc((size_t)n_pc * sizeof(Stats), st));
     ENC_CU(drank.alloc((size_t)n_pc * 2 * fwords * sizeof(uint32_t), st));
     ENC_CU(cudaMemcpyAsync(dpcs.p, pcs.data(), pcs.size() * sizeof(EncPc), cudaMemcpyHostToDevice, st));
-    std::vector<Stats> hstats((size_t)n_pc, Stats{INT_MAX, INT_MIN, 0u, 0u});
-    ENC_CU(cudaMemcpyAsync(dstats.p, hstats.data(), hstats.size() * sizeof(Stats), cudaMemcpyHostToDevice, st));
+    std::vector<Stats> hstats((size_t)n_pc);
+    const std::vector<Stats> stats0((size_t)n_pc, Stats{INT_MAX, INT_MIN, 0u, 0u});
+    DevBuf dsse;
+    ENC_CU(dsse.alloc(sizeof(unsigned long long), st));
 
-    // ---- 4. thresholds + replacement, ranks; plane-channels in chunks of 65535 (grid.y)
+    // ---- 4. thresholds + replacement; plane-channels in chunks of 65535 (grid.y)
     const unsigned gx = (unsigned)((fwords + kThreads / 32 - 1) / (kThreads / 32));
-    for (uint64_t k0 = 0; k0 < n_pc; k0 += 65535) {
-        const unsigned nk = (unsigned)(n_pc - k0 < 65535 ? n_pc - k0 : 65535);
-        const dim3 grid(gx, nk);
+    auto threshold = [&](int tau_ref, int tau_res) -> cudaError_t {
+        cudaError_t e = cudaMemcpyAsync(dstats.p, stats0.data(), stats0.size() * sizeof(Stats), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return e;
+        for (uint64_t k0 = 0; k0 < n_pc; k0 += 65535) {
+            const unsigned nk = (unsigned)(n_pc - k0 < 65535 ? n_pc - k0 : 65535);
+            const dim3 grid(gx, nk);
 #define CLASSIFY(BB) classify_kernel<BB><<<grid, kThreads, 0, st>>>(srv.as<int16_t>(), rec.as<int4>(), dpcs.as<EncPc>() + k0, Ws, Ht, nbx, nblk, fwords, \
-                                                                    p->tau_ref, p->tau_res, p->policy, dflags.as<uint32_t>(), dstats.as<Stats>() + k0)
-        if (B == 2) CLASSIFY(2); else if (B == 4) CLASSIFY(4); else CLASSIFY(8);
+                                                                    tau_ref, tau_res, p->policy, dflags.as<uint32_t>(), dstats.as<Stats>() + k0)
+            if (B == 2) CLASSIFY(2); else if (B == 4) CLASSIFY(4); else CLASSIFY(8);
 #undef CLASSIFY
+        }
+        return cudaGetLastError();
+    };
+    // squared error of the reconstruction at the thresholds last applied (synchronises)
+    RecGeom geo{};
+    geo.h = h; geo.U = U; geo.V = V; geo.Ws = Ws; geo.Ht = Ht; geo.nbx = nbx; geo.fwords = fwords; geo.shiftB = B == 2 ? 1 : (B == 4 ? 2 : 3);
+    {
+        uint32_t kb = 0;
+        for (int L = h - 1; L >= 0; --L) { geo.kbase[L] = kb; kb += (uint32_t)(UL[L] * VL[L]) * 3u; }
+        for (int L = 0; L <= h; ++L) geo.UL[L] = UL[L];
+        geo.top_off = (uint64_t)(nx - n_top) * npx; geo.x_ch = (uint64_t)nx * npx;
     }
+    const unsigned long long n_lf_px = (unsigned long long)U * V * npx;
+    auto measure_sse = [&](unsigned long long *out) -> cudaError_t {
+        cudaError_t e = cudaMemsetAsync(dsse.p, 0, sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return e;
+        reconstruct_sse_kernel<<<(unsigned)((n_lf_px + kThreads - 1) / kThreads), kThreads, 0, st>>>(d_lf, srv.as<int16_t>(), xk.as<int16_t>(), rec.as<int4>(),
+                                                                                                     dpcs.as<EncPc>(), dflags.as<uint32_t>(), geo, n_lf_px,
+                                                                                                     dsse.as<unsigned long long>());
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        if ((e = cudaMemcpyAsync(out, dsse.p, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return e;
+        return cudaStreamSynchronize(st);
+    };
+    auto psnr_of = [&](unsigned long long se) -> double {  // 10 log10(255^2 / MSE) over all RGB bytes
+        if (se == 0ull) return INFINITY;
+        return 10.0 * log10(255.0 * 255.0 / ((double)se / (double)(n_lf_px * 3ull)));
+    };
+    int n_steps = 0;
+    unsigned long long sse = 0ull;
+    if (target_psnr >= 0.0) {
+        int lo = 0, hi = 4096, best_tau = -1;
+        double best_q = 0.0;
+        for (int it = 0; it < max_iter; ++it) {
+            const int mid = (lo + hi) / 2;
+            ENC_CU(threshold(mid / 2, mid));
+            ENC_CU(measure_sse(&sse));
+            ++n_steps;
+            const double q = psnr_of(sse);
+            if (best_tau < 0 || fabs(q - target_psnr) < fabs(best_q - target_psnr)) { best_tau = mid; best_q = q; }
+            if (fabs(q - target_psnr) <= tol || hi - lo <= 1) break;
+            if (q > target_psnr) lo = mid; else hi = mid;
+        }
+        prm.tau_res = best_tau;
+        prm.tau_ref = best_tau / 2;
+    }
+    ENC_CU(threshold(p->tau_ref, p->tau_res));
     rank_kernel<<<(unsigned)((2 * n_pc + kThreads / 32 - 1) / (kThreads / 32)), kThreads, 0, st>>>(dflags.as<uint32_t>(), dpcs.as<EncPc>(), (int)n_pc, fwords,
                                                                                                   drank.as<uint32_t>());
     ENC_CU(cudaGetLastError());
     ENC_CU(cudaEventRecord(ev[3], st));
     ENC_CU(cudaMemcpyAsync(hstats.data(), dstats.p, hstats.size() * sizeof(Stats), cudaMemcpyDeviceToHost, st));
     ENC_CU(cudaStreamSynchronize(st));
+    ENC_CU(measure_sse(&sse));  // quality of the stream about to be written
 
     // ---- 5. directory: value range -> BISE layout, string positions
     uint32_t mv_layout, mv_m;
@@ -566,7 +676,7 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
     for (uint64_t k0 = 0; k0 < n_pc; k0 += 65535) {
         const unsigned nk = (unsigned)(n_pc - k0 < 65535 ? n_pc - k0 : 65535);
         const dim3 grid(gx, nk);
-#define COMPACT(BB) compact_kernel<BB><<<grid, kThreads, 0, st>>>(srv.as<int16_t>(), rec.as<int4>(), dpcs.as<EncPc>() + k0, dpks.as<EncPack>() + k0, Ws, nbx, nblk, \
+#define COMPACT(BB) compact_kernel<BB><<<grid, kThreads, 0, st>>>(srv.as<int16_t>(), rec.as<int4>(), dpcs.as<EncPc>() + k0, dpks.as<EncPack>() + k0, Ws, Ht, nbx, nblk, \
                                                                   fwords, W, dflags.as<uint32_t>(), drank.as<uint32_t>() + k0 * 2 * fwords, dvals.as<uint16_t>(), dmvs.as<uint32_t>())
         if (B == 2) COMPACT(2); else if (B == 4) COMPACT(4); else COMPACT(8);
 #undef COMPACT
@@ -633,6 +743,11 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
         cudaEventElapsedTime(&ms, ev[4], ev[5]); stats->ms_pack = ms;
         stats->ms_wall = (float)(now_ms() - t_begin);
         stats->ms_assemble = (float)(now_ms() - t_assemble);
+        stats->sse = (int64_t)sse;
+        stats->psnr = psnr_of(sse);
+        stats->tau_ref = p->tau_ref;
+        stats->tau_res = p->tau_res;
+        stats->bisection_steps = n_steps;
         stats->n_plane_channels = (int64_t)n_pc;
         stats->n_res_blocks = (int64_t)tot_res;
         stats->n_pred_blocks = (int64_t)n_mvs;
@@ -647,4 +762,20 @@ extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p,
     *h_stream = s;
     *len = (size_t)total;
     return HMLFC_OK;
+}
+
+extern "C" int hmlfc_encode(const uint8_t *d_lf, const hmlfc_encode_params_t *p, uint8_t **h_stream, size_t *len,
+                            hmlfc_encode_stats_t *stats, void *cuda_stream)
+{
+    return encode_impl(d_lf, p, -1.0, 0.0, 0, h_stream, len, stats, cuda_stream);
+}
+
+extern "C" int hmlfc_encode_psnr(const uint8_t *d_lf, const hmlfc_encode_params_t *p, double target_psnr, double tol, int max_iter,
+                                 uint8_t **h_stream, size_t *len, hmlfc_encode_stats_t *stats, void *cuda_stream)
+{
+    if (!(target_psnr >= 0.0) || !(tol >= 0.0) || max_iter < 1 || !std::isfinite(target_psnr)) {
+        if (stats) memset(stats, 0, sizeof(*stats));
+        return HMLFC_E_INVALID;
+    }
+    return encode_impl(d_lf, p, target_psnr, tol, max_iter, h_stream, len, stats, cuda_stream);
 }

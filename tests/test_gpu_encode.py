@@ -57,6 +57,10 @@ def test_encoded_stream_equals_the_oracle_stream(P, enc, name):
     _assert_same_stream(got, data)
     assert stats["n_plane_channels"] == struct.unpack_from("<Q", data, 104)[0]
     assert stats["kernel_launches"] >= cfg.height + 5
+    # the encoder's own reconstruction error (a kernel over its planes) = the oracle's P1 reconstruction error, exactly
+    sse = int(((info["p1"].astype(np.int64) - lf.astype(np.int64)) ** 2).sum())
+    assert stats["sse"] == sse and (stats["tau_ref"], stats["tau_res"]) == (info["tau_ref"], info["tau_res"])
+    assert stats["psnr"] == info["psnr"] or abs(stats["psnr"] - info["psnr"]) < 1e-9
 
 
 @pytest.mark.parametrize("policy", [orc.POLICY_ALL, orc.POLICY_LITERAL])
@@ -106,6 +110,33 @@ def test_full_size_stream_equals_the_oracle_stream(P, name):
     assert stats["n_search_blocks"] == 3 * n_pairs * (cfg.Ws // cfg.block) * (cfg.Ht // cfg.block)
 
 
+@pytest.mark.parametrize("name,target", [("mini2", 38.0), ("mini3", 43.5), ("mini_b8", 36.0), ("cfg1", 120.0)])
+def test_threshold_bisection_to_a_psnr_target_reproduces_the_oracle(P, name, target):
+    # PAPER.md:375; the oracle's encode(lf, p, target) bisects tau_res on its P1 reconstruction; hmlfc_encode_psnr must take the same
+    # decisions (same PSNR values, same steps) and write the same stream.  cfg1 at 120 dB: unreachable, ends at the smallest tau
+    cfg = wl.CONFIGS[name]
+    lf = wl.light_field(cfg)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, cfg.window, 0, 0, geometry=wl.geometry(cfg), seed=cfg.seed)
+    data, info, tree = orc.encode(lf, p, target)
+    tree.close()
+    got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), cfg.height, cfg.block, cfg.window, geometry=wl.geometry(cfg), seed=cfg.seed,
+                                target_psnr=target)
+    assert (stats["tau_ref"], stats["tau_res"]) == (info["tau_ref"], info["tau_res"])
+    assert stats["psnr"] == info["psnr"] or abs(stats["psnr"] - info["psnr"]) < 1e-9
+    assert 1 <= stats["bisection_steps"] <= 12
+    _assert_same_stream(got, data)
+
+
+def test_cfg2_bisection_to_40_db_reproduces_the_cached_oracle_stream(P):
+    from oracle import streams
+
+    cfg, data, info = streams.get_stream("cfg2")
+    got, stats = P.hmlfc_encode(torch.from_numpy(wl.light_field(cfg)).cuda(), cfg.height, cfg.block, cfg.window, geometry=wl.geometry(cfg),
+                                seed=cfg.seed, target_psnr=cfg.target_psnr)
+    assert stats["tau_res"] == info["tau_res"] and abs(stats["psnr"] - info["psnr"]) < 1e-9
+    _assert_same_stream(got, data)
+
+
 def test_invalid_and_unsupported_arguments(P):
     lf = torch.zeros((2, 2, 16, 16, 3), dtype=torch.uint8, device="cuda")
     with pytest.raises(P.HmlfcError):
@@ -114,3 +145,7 @@ def test_invalid_and_unsupported_arguments(P):
         P.hmlfc_encode(lf, 9)                   # height > 8
     with pytest.raises(P.HmlfcError):
         P.hmlfc_encode(lf, 1, tau_res=-1)
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_encode(lf, 1, target_psnr=-3.0)
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_encode(lf, 1, target_psnr=40.0, max_iter=0)
