@@ -49,9 +49,10 @@ def _gpu_encode(P, cfg, lf, tau_ref, tau_res, policy=0):
                           geometry=wl.geometry(cfg), seed=cfg.seed)
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8", "mini_h8", "mini_w64"])
 def test_encoded_stream_equals_the_oracle_stream(P, enc, name):
-    # cfg1: tau = 0 (every block kept); mini3: odd 5 x 5 grid (partial clusters); mini_b2 / mini_b8: B = 2 / 8, W = 5 / 8
+    # cfg1: tau = 0 (every block kept); mini3: odd 5 x 5 grid (partial clusters); mini_b2 / mini_b8: B = 2 / 8, W = 5 / 8; mini_h8 / mini_w64:
+    # the format's limits, tree height 8 and search window 64
     cfg, lf, data, info, s = enc(name)
     got, stats = _gpu_encode(P, cfg, lf, info["tau_ref"], info["tau_res"])
     _assert_same_stream(got, data)

@@ -47,7 +47,7 @@ def test_decode_cfg1_every_pixel_lossless(P, enc):
     assert np.array_equal(out.reshape(lf.shape), lf)  # zero-threshold round trip reproduces the input
 
 
-@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4"])
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"])
 def test_decode_every_pixel_matches_oracle(P, enc, name):
     cfg, lf, data, info, s = enc(name)
     h = _loaded(P, enc, name)
@@ -119,7 +119,7 @@ def _check_views(P, h, s, cams, W, H):
     return expect
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"])
 def test_render_matches_oracle(P, enc, name):
     cfg, lf, data, info, s = enc(name)
     h = _loaded(P, enc, name)

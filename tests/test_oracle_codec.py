@@ -73,7 +73,7 @@ def test_huge_thresholds_leave_only_the_rkv_chain():
 
 
 # ---------------------------------------------------------------- pin 3: P1 = P2
-@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4"])
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"])
 def test_stream_decode_equals_encoder_reconstruction(enc, name):
     cfg, lf, data, info, s = enc(name)
     assert np.array_equal(s.decode_full(), info["p1"])

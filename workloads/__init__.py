@@ -62,6 +62,10 @@ CONFIGS = {
     # other block sizes / search windows (the paper's Table 2 sweeps B = 2, 4, 8)
     "mini_b2": Config("mini_b2", 4, 4, 48, 40, 2, 4, 1, 3.0, None, 12, 90, 70, 2, 20_000, seed=BASE_SEED + 15, block=2, window=5),
     "mini_b8": Config("mini_b8", 5, 4, 64, 48, 2, 4, 2, 4.0, None, 160, 120, 88, 2, 20_000, seed=BASE_SEED + 16, block=8, window=8),
+    # the limits of the stream format: tree height 8 (levels 6x5 -> 3x3 -> 2x2 -> 1x1 x 5: a cluster of one
+    # plane has SRV = 0 at every level above) and search window 64 (129 x 129 offsets, wider than the image)
+    "mini_h8": Config("mini_h8", 6, 5, 32, 24, 8, 3, 1, 3.0, None, 24, 72, 56, 2, 20_000, seed=BASE_SEED + 17, window=4),
+    "mini_w64": Config("mini_w64", 3, 2, 24, 16, 2, 3, 1, 3.0, None, 20, 56, 40, 2, 10_000, seed=BASE_SEED + 18, window=64),
     # paper-regime sparsity: adjacent views < 1 px apart, as in the Stanford archive
     "cfg2_sparse": Config("cfg2_sparse", 16, 16, 256, 256, 3, 5, 2, 1.0, 40.0, 0, 512, 512, 64, 10 ** 7,
                           seed=BASE_SEED + 22),
