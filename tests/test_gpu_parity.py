@@ -185,6 +185,28 @@ def test_render_eye_on_the_camera_plane(P, enc, name):
     _check_views(P, h, s, wl.camera_path(cfg, on_plane=True), cfg.out_w, cfg.out_h)
 
 
+def test_concurrent_launches_on_several_streams_share_one_handle(P, enc):
+    # the handle is immutable after load (include/hmlfc.h): launches enqueued on different CUDA streams may overlap
+    cfg, lf, data, info, s = enc("mini4")
+    h = _loaded(P, enc, "mini4")
+    cams = [_dev(wl.camera_path(cfg, n_views=4, seed_offset=k)) for k in range(3)]
+    coords = _dev(wl.random_coords(cfg, 40_000))
+    serial = [P.hmlfc_render(h, c, cfg.out_w, cfg.out_h).clone() for c in cams]
+    serial_dec = P.hmlfc_decode(h, coords).clone()
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    outs = [torch.empty_like(serial[0]) for _ in range(3)]
+    dec = torch.empty_like(serial_dec)
+    for rep in range(5):
+        for k in range(3):
+            P.hmlfc_render(h, cams[k], cfg.out_w, cfg.out_h, out=outs[k], stream=streams[k])
+        P.hmlfc_decode(h, coords, out=dec, stream=streams[3])
+    torch.cuda.synchronize()
+    for k in range(3):
+        assert torch.equal(outs[k], serial[k])
+    assert torch.equal(dec, serial_dec)
+
+
 def test_render_host_entry_point(P, enc):
     cfg, lf, data, info, s = enc("mini3")
     h = _loaded(P, enc, "mini3")
