@@ -44,6 +44,47 @@ __device__ __forceinline__ unsigned long long make_key(float sad, int mode, int 
            ((unsigned long long)dyi << 8) | (unsigned long long)dxi;
 }
 
+// One task: the block's 4 x 4 samples against NOFF consecutive dx offsets at one dy, both modes; returns the task's minimum key in
+// the order (SAD, mode, dx): subtractive sums first, strict comparisons keep the first (offset 0 of a chunk always exists).
+// NOFF + 3 window samples per row come from (NOFF + 3 + 3) / 4 128-bit shared loads.
+template <int NOFF>
+__device__ __forceinline__ unsigned long long task_min(const float *__restrict__ prow, const float *__restrict__ wrow, int stride, int nvalid,
+                                                       int dyi, int chunk)
+{
+    constexpr int NLD = (NOFF + 3 + 3) / 4;
+    float sm[NOFF], sp[NOFF];
+#pragma unroll
+    for (int d = 0; d < NOFF; ++d) sm[d] = sp[d] = 0.f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const float4 p4 = *reinterpret_cast<const float4 *>(prow + j * (kTBX * 4));
+        const float p[4] = {p4.x, p4.y, p4.z, p4.w};
+        const float4 *row = reinterpret_cast<const float4 *>(wrow + (size_t)j * stride);
+        float r[4 * NLD];
+#pragma unroll
+        for (int q = 0; q < NLD; ++q) {
+            const float4 v = row[q];
+            r[4 * q + 0] = v.x; r[4 * q + 1] = v.y; r[4 * q + 2] = v.z; r[4 * q + 3] = v.w;
+        }
+#pragma unroll
+        for (int d = 0; d < NOFF; ++d)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                sm[d] += fabsf(p[i] - r[d + i]);  // Eq. (1)
+                sp[d] += fabsf(p[i] + r[d + i]);  // Eq. (2)
+            }
+    }
+    float bs = sm[0];
+    int bi = 0;
+#pragma unroll
+    for (int d = 1; d < NOFF; ++d)
+        if (d < nvalid && sm[d] < bs) { bs = sm[d]; bi = d; }
+#pragma unroll
+    for (int d = 0; d < NOFF; ++d)
+        if (d < nvalid && sp[d] < bs) { bs = sp[d]; bi = 16 + d; }
+    return make_key(bs, bi >> 4, dyi, chunk * kChunk + (bi & 15));
+}
+
 #ifndef HMLFC_SEARCH_MINB
 #define HMLFC_SEARCH_MINB 4
 #endif
@@ -80,47 +121,22 @@ search4_kernel(const int16_t *__restrict__ planes, const int2 *__restrict__ pair
     if (tid < kTBX * kTBY) best[tid] = ~0ull;
     __syncthreads();
 
-    const int per_block = nd * nchunks, ntasks = kTBX * kTBY * per_block;
+    // Tasks in the order (chunk, dy, block): the 32 lanes of a warp work on the tile's 32 blocks at one (dy, chunk), so the chunk --
+    // and with it the number of valid offsets -- is warp-uniform.  The last chunk holds nd - 12 (nchunks - 1) offsets (9 for W = 16):
+    // it runs the same body instantiated for 9 offsets and 12 window samples instead of computing 12 and discarding 3.
+    const int per_chunk = kTBX * kTBY * nd, ntasks = per_chunk * nchunks;
+    const int nlast = nd - (nchunks - 1) * kChunk;
     for (int t = tid; t < ntasks; t += kThreads) {
-        const int blk = t / per_block, rem = t - blk * per_block;
-        const int dyi = rem / nchunks, chunk = rem - dyi * nchunks;
+        const int chunk = t / per_chunk, rem = t - chunk * per_chunk;
+        const int dyi = rem / (kTBX * kTBY), blk = rem - dyi * (kTBX * kTBY);
         const int bxl = blk & (kTBX - 1), byl = blk / kTBX;
         if (blockIdx.x * kTBX + bxl >= nbx || blockIdx.y * kTBY + byl >= nby) continue;
-        float sm[kChunk], sp[kChunk];
-#pragma unroll
-        for (int d = 0; d < kChunk; ++d) sm[d] = sp[d] = 0.f;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const float4 p4 = *reinterpret_cast<const float4 *>(ptile + (byl * 4 + j) * (kTBX * 4) + bxl * 4);
-            const float p[4] = {p4.x, p4.y, p4.z, p4.w};
-            // window row of image row y0 + byl*4 + j + dy; column of image column x0 + bxl*4 + dx, dx = chunk*12 - W + d
-            const float4 *row = reinterpret_cast<const float4 *>(win + (size_t)(byl * 4 + j + dyi) * stride + bxl * 4 + chunk * kChunk);
-            float r[16];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const float4 v = row[k];
-                r[4 * k + 0] = v.x; r[4 * k + 1] = v.y; r[4 * k + 2] = v.z; r[4 * k + 3] = v.w;
-            }
-#pragma unroll
-            for (int d = 0; d < kChunk; ++d)
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    sm[d] += fabsf(p[i] - r[d + i]);  // Eq. (1)
-                    sp[d] += fabsf(p[i] + r[d + i]);  // Eq. (2)
-                }
-        }
-        // the task's minimum in the order (SAD, mode, dx): subtractive sums first, strict comparisons keep the first
-        // (offset 0 of a chunk always exists); one 64-bit key per task
-        const int nvalid = nd - chunk * kChunk;
-        float bs = sm[0];
-        int bi = 0;
-#pragma unroll
-        for (int d = 1; d < kChunk; ++d)
-            if (d < nvalid && sm[d] < bs) { bs = sm[d]; bi = d; }
-#pragma unroll
-        for (int d = 0; d < kChunk; ++d)
-            if (d < nvalid && sp[d] < bs) { bs = sp[d]; bi = 16 + d; }
-        const unsigned long long k = make_key(bs, bi >> 4, dyi, chunk * kChunk + (bi & 15));
+        const float *prow = ptile + (byl * 4) * (kTBX * 4) + bxl * 4;
+        // window row of image row y0 + byl*4 + j + dy; column of image column x0 + bxl*4 + dx, dx = chunk*12 - W + d
+        const float *wrow = win + (size_t)(byl * 4 + dyi) * stride + bxl * 4 + chunk * kChunk;
+        unsigned long long k;
+        if (chunk == nchunks - 1 && nlast == 9) k = task_min<9>(prow, wrow, stride, 9, dyi, chunk);
+        else k = task_min<kChunk>(prow, wrow, stride, chunk == nchunks - 1 ? nlast : kChunk, dyi, chunk);
         atomicMin(&best[blk], k);
     }
     __syncthreads();
