@@ -126,6 +126,10 @@ search4_kernel(const int16_t *__restrict__ planes, const int2 *__restrict__ pair
     // it runs the same body instantiated for 9 offsets and 12 window samples instead of computing 12 and discarding 3.
     const int per_chunk = kTBX * kTBY * nd, ntasks = per_chunk * nchunks;
     const int nlast = nd - (nchunks - 1) * kChunk;
+    // kThreads is a multiple of the 32 blocks of a tile: all tasks of a thread belong to ONE block (blk = tid mod 32), so the thread
+    // keeps its minimum key in registers and publishes it once
+    static_assert(kThreads % (kTBX * kTBY) == 0, "a thread's tasks must stay on one block");
+    unsigned long long kbest = ~0ull;
     for (int t = tid; t < ntasks; t += kThreads) {
         const int chunk = t / per_chunk, rem = t - chunk * per_chunk;
         const int dyi = rem / (kTBX * kTBY), blk = rem - dyi * (kTBX * kTBY);
@@ -137,8 +141,9 @@ search4_kernel(const int16_t *__restrict__ planes, const int2 *__restrict__ pair
         unsigned long long k;
         if (chunk == nchunks - 1 && nlast == 9) k = task_min<9>(prow, wrow, stride, 9, dyi, chunk);
         else k = task_min<kChunk>(prow, wrow, stride, chunk == nchunks - 1 ? nlast : kChunk, dyi, chunk);
-        atomicMin(&best[blk], k);
+        kbest = k < kbest ? k : kbest;
     }
+    if (kbest != ~0ull) atomicMin(&best[tid & (kTBX * kTBY - 1)], kbest);
     __syncthreads();
     if (tid < kTBX * kTBY) {
         const int bx = blockIdx.x * kTBX + (tid & (kTBX - 1)), by = blockIdx.y * kTBY + tid / kTBX;
