@@ -27,7 +27,7 @@ namespace hmlfc {
 
 namespace {
 
-constexpr int kTBX = 8, kTBY = 4;  // blocks per CTA tile
+constexpr int kTBX = 8, kTBY = 8;  // blocks per CTA tile
 constexpr int kChunk = 12;         // dx offsets per task
 constexpr int kThreads = 256;
 
