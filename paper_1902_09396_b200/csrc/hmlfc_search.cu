@@ -12,12 +12,13 @@
 // 2^24, so fp32 adds are exact, |x| is a free source modifier of FADD, and the FP32 pipe has twice the lanes of the
 // INT32 pipe on this SM.  The result is bit-identical to the integer definition.
 //
-// One CTA searches a tile of 8 x 4 blocks of one (P, R) pair.  The reference window of the tile (tile + W on every
+// One CTA searches a tile of 8 x 8 blocks of one (P, R) pair.  The reference window of the tile (tile + W on every
 // side, zero outside the image) and the tile of P are staged in shared memory as floats.  A task = (block, dy, chunk
 // of 12 consecutive dx): the thread reads, per block row, 16 consecutive window samples with four 128-bit shared
-// loads and updates 12 + 12 running sums held in registers (192 FADDs per 4 shared loads); its best key goes to the
-// block's 64-bit shared-memory minimum.  Row stride = 4 mod 32 words and chunk = 12 make the 128-bit loads of every
-// quarter-warp bank-conflict free.  Block sizes other than 4 take a plain warp-per-block kernel.
+// loads and updates 12 + 12 running sums held in registers (192 FADDs per 4 shared loads).  Tasks are ordered
+// (chunk, dy, block): a warp's lanes work on 32 neighbouring blocks at one (dy, chunk) -- consecutive 128-bit loads --
+// and every task of a thread belongs to one block, whose minimum key the thread keeps in registers.  Block sizes
+// other than 4 take a plain warp-per-block kernel.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
