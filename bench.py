@@ -415,32 +415,35 @@ def run_ours(args, cfg_name):
             "roofline": {"bound": "hbm", "kernel": "level0_kernel + levelL_kernel", "achieved": hi_bytes / (hi_kernel_ms * 1e-3) / 1e9,
                          "peak": peak, "unit": "GB/s", "frac": hi_bytes / (hi_kernel_ms * 1e-3) / 1e9 / peak, "bytes_alg_per_call": int(hi_bytes)},
         }
-        # ---- the oracle timed beside it, on a bounded sample of the same batch
-        import oracle as orc
+        cpu = None  # the oracle is timed beside the GPU on rank 0 at N = 1 only (other ranks would idle at the next barrier)
+        if world == 1:
+            # ---- the oracle timed beside it, on a bounded sample of the same batch
+            import oracle as orc
 
-        s = orc.Stream(data)
-        if args.min_level:
-            s.set_min_level(args.min_level)
-        cores = os.cpu_count() or 1
-        n_cpu, cpu_s = _oracle_views_sample(s, cams_np, W, H, args.cpu_budget, V)
-        cpu = {"value": n_cpu / cpu_s, "unit": "views/s", "cores": cores, "kind": "oracle",
-               "sample": f"{n_cpu} of the batch's {V} views ({W}x{H}), one at a time, OpenMP over {cores} threads, {cpu_s:.1f} s"}
-        # the oracle's random-access decoder on a sample of the same coordinate list: all cores, then one thread
-        n_s = min(n_dec, 2_000_000)
-        sample_coords = coords[:n_s].cpu().numpy()
-        t0 = time.perf_counter()
-        s.decode(sample_coords)
-        t_all = time.perf_counter() - t0
-        n_1 = max(1, n_s // 16)
-        t0 = time.perf_counter()
-        s.decode(sample_coords[:n_1], nthreads=1)
-        t_one = time.perf_counter() - t0
-        decode["cpu_baseline"] = {"value": n_s / t_all, "unit": "LF pixels/s", "cores": cores, "kind": "oracle",
-                                  "sample": f"the first {n_s} of the {n_dec} coordinates, OpenMP over {cores} threads, {t_all:.2f} s",
-                                  "single_thread": {"value": n_1 / t_one, "sample": f"the first {n_1} coordinates, {t_one:.2f} s"}}
-        t0 = time.perf_counter()
-        s.render(cams_np[:1], W, H, nthreads=1)
-        cpu["single_thread"] = {"value": 1.0 / (time.perf_counter() - t0), "sample": f"1 view ({W}x{H}), one thread"}
+            s = orc.Stream(data)
+            if args.min_level:
+                s.set_min_level(args.min_level)
+            cores = os.cpu_count() or 1
+            n_cpu, cpu_s = _oracle_views_sample(s, cams_np, W, H, args.cpu_budget, V)
+            cpu = {"value": n_cpu / cpu_s, "unit": "views/s", "cores": cores, "kind": "oracle",
+                   "sample": f"{n_cpu} of the batch's {V} views ({W}x{H}), one at a time, OpenMP over {cores} threads, {cpu_s:.1f} s"}
+            # the oracle's random-access decoder on a sample of the same coordinate list: all cores, then one thread
+            n_s = min(n_dec, 2_000_000)
+            sample_coords = coords[:n_s].cpu().numpy()
+            t0 = time.perf_counter()
+            s.decode(sample_coords)
+            t_all = time.perf_counter() - t0
+            n_1 = max(1, n_s // 16)
+            t0 = time.perf_counter()
+            s.decode(sample_coords[:n_1], nthreads=1)
+            t_one = time.perf_counter() - t0
+            decode["cpu_baseline"] = {"value": n_s / t_all, "unit": "LF pixels/s", "cores": cores, "kind": "oracle",
+                                      "sample": f"the first {n_s} of the {n_dec} coordinates, OpenMP over {cores} threads, {t_all:.2f} s",
+                                      "single_thread": {"value": n_1 / t_one, "sample": f"the first {n_1} coordinates, {t_one:.2f} s"}}
+            t0 = time.perf_counter()
+            s.render(cams_np[:1], W, H, nthreads=1)
+            cpu["single_thread"] = {"value": 1.0 / (time.perf_counter() - t0), "sample": f"1 view ({W}x{H}), one thread"}
+
         line = {
             "metric": "rendered_views_per_s", "value": views_per_s, "unit": "views/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
