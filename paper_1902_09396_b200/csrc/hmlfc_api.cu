@@ -258,7 +258,8 @@ int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_view
     // Chunks of whole views, about 6 MB of output and at least 2048 tiles (several waves of CTAs) each; batches below 24 MB go
     // as one launch (the copy is short and small launches have a longer tail).  Measured on cfg2 (64 views of 512 x 512 = 50 MB
     // per call; bare copy 0.93 ms, kernel 0.86 ms): one launch 1.79 ms, 6 MB chunks 1.20 ms, 3 MB 1.37 ms, 0.75 MB 1.92 ms
-    // (host-side enqueue cost per chunk); cfg3 (16 views = 12.6 MB, kernel 0.97 ms) is slower in chunks.
+    // (host-side enqueue cost per chunk); cfg3 (16 views = 12.6 MB, kernel 0.97 ms) is slower in chunks.  With the chunks' kernels
+    // alternating between two streams (below): cfg2 1.09 ms, cfg4 (16 views of 1024 x 1024) 1.50 -> 1.21 ms.
     const size_t tiles = (size_t)((W + 31) / 32) * (size_t)((H + 31) / 32);
     size_t per = (((size_t)6 << 20) + view_bytes - 1) / view_bytes;
     if (per * tiles < 2048) per = (2048 + tiles - 1) / tiles;
@@ -266,11 +267,15 @@ int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_view
     if (((size_t)n_views + per - 1) / per > (size_t)hmlfc_handle::kMaxChunks) per = ((size_t)n_views + hmlfc_handle::kMaxChunks - 1) / hmlfc_handle::kMaxChunks;
     const hmlfc_camera *d_cams = static_cast<const hmlfc_camera *>(h->d_in);
     CU(h, cudaMemcpyAsync(h->d_in, h_cameras, (size_t)n_views * sizeof(hmlfc_camera), cudaMemcpyHostToDevice, h->host_stream));
+    // the chunks' kernels alternate between two streams, so the last, partial wave of CTAs of one chunk overlaps the first of the next
+    CU(h, cudaEventRecord(h->ev_in[0], h->host_stream));
+    CU(h, cudaStreamWaitEvent(h->in_stream, h->ev_in[0], 0));
     int c = 0;
     for (int v = 0; v < n_views; v += (int)per, ++c) {
         const int m = (n_views - v < (int)per) ? n_views - v : (int)per;
-        if ((rc = hmlfc_render(h, d_cams + v, m, W, H, h->d_outbuf + (size_t)v * view_bytes, h->host_stream)) != HMLFC_OK) { sync_pipeline(h); return rc; }
-        CU(h, cudaEventRecord(h->ev_done[c], h->host_stream));
+        cudaStream_t ks = (c & 1) ? h->in_stream : h->host_stream;
+        if ((rc = hmlfc_render(h, d_cams + v, m, W, H, h->d_outbuf + (size_t)v * view_bytes, ks)) != HMLFC_OK) { sync_pipeline(h); return rc; }
+        CU(h, cudaEventRecord(h->ev_done[c], ks));
         CU(h, cudaStreamWaitEvent(h->out_stream, h->ev_done[c], 0));
         CU(h, cudaMemcpyAsync(h_out + (size_t)v * view_bytes, h->d_outbuf + (size_t)v * view_bytes, (size_t)m * view_bytes, cudaMemcpyDeviceToHost, h->out_stream));
     }
