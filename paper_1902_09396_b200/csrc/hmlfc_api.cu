@@ -255,15 +255,16 @@ int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_view
     int rc;
     if ((rc = ensure(h, &h->d_in, &h->d_in_cap, (size_t)n_views * sizeof(hmlfc_camera))) != HMLFC_OK) return rc;
     if ((rc = ensure(h, reinterpret_cast<void **>(&h->d_outbuf), &h->d_out_cap, out_bytes + 4)) != HMLFC_OK) return rc;
-    // Chunks of whole views, about 6 MB of output and at least 2048 tiles (several waves of CTAs) each; batches below 24 MB go
+    // Chunks of whole views, about 6 MB of output and at least 2048 tiles (several waves of CTAs) each; batches below 12 MB go
     // as one launch (the copy is short and small launches have a longer tail).  Measured on cfg2 (64 views of 512 x 512 = 50 MB
     // per call; bare copy 0.93 ms, kernel 0.86 ms): one launch 1.79 ms, 6 MB chunks 1.20 ms, 3 MB 1.37 ms, 0.75 MB 1.92 ms
     // (host-side enqueue cost per chunk); cfg3 (16 views = 12.6 MB, kernel 0.97 ms) is slower in chunks.  With the chunks' kernels
-    // alternating between two streams (below): cfg2 1.09 ms, cfg4 (16 views of 1024 x 1024) 1.50 -> 1.21 ms.
+    // alternating between two streams (below): cfg2 1.09 ms, cfg4 (16 views of 1024 x 1024) 1.50 -> 1.21 ms, cfg3 in two chunks
+    // 1.06 -> 0.96 ms.
     const size_t tiles = (size_t)((W + 31) / 32) * (size_t)((H + 31) / 32);
     size_t per = (((size_t)6 << 20) + view_bytes - 1) / view_bytes;
     if (per * tiles < 2048) per = (2048 + tiles - 1) / tiles;
-    if (out_bytes < ((size_t)24 << 20)) per = (size_t)n_views;
+    if (out_bytes < ((size_t)12 << 20)) per = (size_t)n_views;
     if (((size_t)n_views + per - 1) / per > (size_t)hmlfc_handle::kMaxChunks) per = ((size_t)n_views + hmlfc_handle::kMaxChunks - 1) / hmlfc_handle::kMaxChunks;
     const hmlfc_camera *d_cams = static_cast<const hmlfc_camera *>(h->d_in);
     CU(h, cudaMemcpyAsync(h->d_in, h_cameras, (size_t)n_views * sizeof(hmlfc_camera), cudaMemcpyHostToDevice, h->host_stream));
