@@ -285,6 +285,17 @@ def run_ours(args, cfg_name):
     dec_total = reduce_max(sum(dec_ms), world, "cuda")
     dec_px_per_s = whole_job_rate(n_dec, len(dec_ms), world, dec_total * 1e-3)
 
+    # ---- dense decode: whole views (coordinates generated in the kernel), up to 2^27 light-field pixels per launch
+    n_dv = max(1, min(cfg.U * cfg.V, (1 << 27) // (cfg.Ws * cfg.Ht)))
+    dv_rng = np.random.Generator(np.random.PCG64(cfg.seed + 3000 + rank))
+    dv_ids = dv_rng.permutation(cfg.U * cfg.V)[:n_dv]
+    dv_views = torch.from_numpy(np.stack([dv_ids % cfg.U, dv_ids // cfg.U], axis=1).astype(np.int32)).cuda()
+    dv_out = torch.empty((n_dv, cfg.Ht, cfg.Ws, 3), dtype=torch.uint8, device="cuda")
+    dv_ms = timed(lambda: P.hmlfc_decode_views(h, dv_views, out=dv_out, stream=stream), max(3, min(args.steps, 10)), 3)
+    dv_total = reduce_max(sum(dv_ms), world, "cuda")
+    dv_px = n_dv * cfg.Ws * cfg.Ht
+    del dv_out
+
     # ---- end to end through the C ABI with HOST (pinned) buffers: cameras H2D + views D2H inside the timed region
     cams_pin = torch.from_numpy(cams_np).pin_memory()
     out_pin = torch.empty((V, H, W, 3), dtype=torch.uint8).pin_memory()
@@ -453,6 +464,9 @@ def run_ours(args, cfg_name):
                     "d2h_bytes_per_step": int(out_pin.numel()), "steps": e2e_steps},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "on_plane_batch": {"value": whole_job_rate(V, len(pl_ms), world, pl_total * 1e-3), "unit": "views/s", "ms_per_step": float(np.mean(pl_ms)),
                                "workload": "the same camera circle on the camera plane z = 0 (SURVEY 8(d) D4: every view blends exactly 4 light-field views)"},
+            "decode_views": {"value": whole_job_rate(dv_px, len(dv_ms), world, dv_total * 1e-3), "unit": "LF pixels/s", "n_views": int(n_dv),
+                             "pixels_per_launch": int(dv_px), "ms_per_launch": float(np.mean(dv_ms)),
+                             "workload": "hmlfc_decode_views: every pixel of a seeded random set of whole views (coordinates generated in the kernel)"},
             "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),

@@ -101,6 +101,15 @@ int hmlfc_info(const hmlfc_handle *h, hmlfc_info_t *out);
  * An out-of-range coordinate writes (0,0,0) and increments the handle's out-of-range counter. */
 int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint8_t *d_out, void *cuda_stream);
 
+/* hmlfc_decode_views -- the same decoding procedure for WHOLE views: every pixel of view (u, v) = d_views[k], in
+ * row-major order ("parallel decompression of different pixel values"; the dense counterpart of hmlfc_decode: no
+ * 16-byte coordinate per sample is read, neighbouring lanes decode neighbouring pixels).
+ *   d_views : device, int32 [n_views][2] = (u, v).
+ *   d_out   : device, uint8 [n_views][Ht][Ws][3] RGB.
+ * A view outside the camera grid is written black and every pixel of it counted as out of range.  Progressive decoding
+ * (hmlfc_set_min_level) applies.  Asynchronous like hmlfc_decode. */
+int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_views, uint8_t *d_out, void *cuda_stream);
+
 /* hmlfc_render -- PAPER.md:73 / :309 / :409: per output pixel, ray -> (u,v,s,t) on the two
  * planes, 16-tap quadrilinear blend of decoded samples (4 nearest views x 4 nearest pixels,
  * edge-clamped), rounded to RGB8; rays that miss the slab get the background colour.

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 
 # every symbol include/hmlfc.h declares
 EXPORTS = (
-    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
     "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
@@ -68,6 +68,7 @@ def lib():
     L.hmlfc_load.argtypes, L.hmlfc_load.restype = [vp, C.c_size_t, C.POINTER(vp)], C.c_int
     L.hmlfc_info.argtypes, L.hmlfc_info.restype = [vp, C.POINTER(Info)], C.c_int
     L.hmlfc_decode.argtypes, L.hmlfc_decode.restype = [vp, vp, i64, vp, vp], C.c_int
+    L.hmlfc_decode_views.argtypes, L.hmlfc_decode_views.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
     L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
     L.hmlfc_render_host.argtypes, L.hmlfc_render_host.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp], C.c_int
@@ -159,6 +160,20 @@ def hmlfc_decode(h: Handle, coords, out=None, stream=None):
     assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == 3 * n
     _check(lib().hmlfc_decode(h._h, C.c_void_p(coords.data_ptr()), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
            "hmlfc_decode", h._h)
+    return out
+
+
+def hmlfc_decode_views(h: Handle, views, out=None, stream=None):
+    """views: CUDA int32 tensor [n][2] = (u,v); returns CUDA uint8 tensor [n][Ht][Ws][3] (every pixel of every listed view)."""
+    torch = _require_cuda()
+    assert views.is_cuda and views.dtype == torch.int32 and views.is_contiguous() and views.shape[-1] == 2
+    n = views.numel() // 2
+    Ht, Ws = h.info.Ht, h.info.Ws
+    if out is None:
+        out = torch.empty((n, Ht, Ws, 3), dtype=torch.uint8, device=views.device)
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * Ht * Ws * 3
+    _check(lib().hmlfc_decode_views(h._h, C.c_void_p(views.data_ptr()), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
+           "hmlfc_decode_views", h._h)
     return out
 
 

@@ -174,6 +174,15 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
     return HMLFC_OK;
 }
 
+int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_views, uint8_t *d_out, void *cuda_stream)
+{
+    if (!h || n_views < 0 || (n_views > 0 && (!d_views || !d_out))) return HMLFC_E_INVALID;
+    int nl = 0;
+    CU(h, launch_decode_views(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    h->launches += nl;
+    return HMLFC_OK;
+}
+
 int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
                  void *cuda_stream)
 {

@@ -142,6 +142,9 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
     push(q.vq, vcnt, has, vt, lane_lt);
 }
 
+// kDense: the coordinates are not read but generated -- sample i is pixel i mod (Ws Ht) (row-major) of view views[i / (Ws Ht)]
+// (hmlfc_decode_views: whole views, no 16-byte coordinate per sample, neighbouring lanes in neighbouring pixels).
+template <bool kDense>
 __global__ void __launch_bounds__(kThreads)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
@@ -157,11 +160,22 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
     const bool present = i < n;
     int4 c4 = make_int4(0, 0, 0, 0);
+    if (kDense) {
+        if (present) {
+            const long long npx = (long long)S.Ws * S.Ht;
+            const long long view = i / npx;
+            const int pix = (int)(i - view * npx);
+            const int2 uv = __ldg(reinterpret_cast<const int2 *>(coords) + view);
+            const int y = pix / S.Ws;
+            c4 = make_int4(uv.x, uv.y, pix - y * S.Ws, y);
+        }
+    } else {
 #ifdef HMLFC_DECODE_CS
-    if (present) c4 = __ldcs(coords + i);
+        if (present) c4 = __ldcs(coords + i);
 #else
-    if (present) c4 = __ldg(coords + i);
+        if (present) c4 = __ldg(coords + i);
 #endif
+    }
     const bool valid = present && (unsigned)c4.x < (unsigned)S.U && (unsigned)c4.y < (unsigned)S.V &&
                        (unsigned)c4.z < (unsigned)S.Ws && (unsigned)c4.w < (unsigned)S.Ht;
     if (present && !valid) atomicAdd(oob, 1ull);
@@ -259,8 +273,22 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
-                                                                d_oob, aligned);
+    decode_queue_kernel<false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
+                                                                       d_oob, aligned);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
+                                cudaStream_t st, int *n_launches)
+{
+    if (n_views == 0) return cudaSuccess;
+    if (S.Ws > 65536 || S.Ht > 65536) return cudaErrorInvalidValue;
+    const long long n = (long long)n_views * S.Ws * S.Ht;
+    const long long blocks = (n + kThreads - 1) / kThreads;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
+    decode_queue_kernel<true><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

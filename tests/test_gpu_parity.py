@@ -90,6 +90,26 @@ def test_decode_out_of_range_is_black_and_counted(P, enc):
     P.hmlfc_free(h)
 
 
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini3", "mini_b8", "mini_h8"])
+def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
+    # hmlfc_decode_views: whole views, coordinates generated in the kernel; every view of the light field (shuffled order, one repeated)
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    rng = np.random.default_rng(5)
+    order = rng.permutation(cfg.U * cfg.V)
+    views = np.stack([order % cfg.U, order // cfg.U], axis=1).astype(np.int32)
+    views = np.concatenate([views, views[:1]])
+    got = P.hmlfc_decode_views(h, _dev(views)).cpu().numpy()
+    for k, (u, v) in enumerate(views):
+        assert np.array_equal(got[k], info["p1"][v, u]), (name, u, v)
+    assert P.hmlfc_decode_views(h, _dev(views[:0])).numel() == 0
+    # a view outside the grid is black and counted
+    before = P.hmlfc_last_oob_count(h)
+    bad = P.hmlfc_decode_views(h, _dev(np.array([[cfg.U, 0], [0, 0]], dtype=np.int32))).cpu().numpy()
+    assert not bad[0].any() and np.array_equal(bad[1], info["p1"][0, 0])
+    assert P.hmlfc_last_oob_count(h) - before == cfg.Ws * cfg.Ht
+
+
 def test_decode_host_entry_point(P, enc):
     cfg, lf, data, info, s = enc("mini4")
     h = _loaded(P, enc, "mini4")
