@@ -120,13 +120,14 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
 
 /* End-to-end variants with HOST buffers: copy the inputs to the device, run the same kernels,
  * copy the result back, synchronise.  Scratch device buffers live in the handle and grow on
- * demand (so these two calls are not re-entrant on one handle).  The work is pipelined in
+ * demand (so these calls are not re-entrant on one handle).  The work is pipelined in
  * chunks (whole views / >= 2^20 coordinates) over three streams of the handle, so the input
  * copy of one chunk, the kernel of the previous and the result copy of the one before overlap
  * (hmlfc_render_host alternates its chunks' kernels between two streams so that their last waves overlap);
  * the bytes written equal those of one whole-batch call.  Pinned host memory makes the copies
  * asynchronous DMA; pageable memory works too (the copies then serialise). */
 int hmlfc_decode_host(hmlfc_handle *h, const int32_t *h_coords, int64_t n, uint8_t *h_out);
+int hmlfc_decode_views_host(hmlfc_handle *h, const int32_t *h_views, int64_t n_views, uint8_t *h_out);
 int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, int W, int H, uint8_t *h_out);
 
 /* Synchronous: the number of out-of-range coordinates seen by hmlfc_decode since load. */

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 
 # every symbol include/hmlfc.h declares
 EXPORTS = (
-    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_render", "hmlfc_decode_host", "hmlfc_render_host",
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_render", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
     "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
@@ -71,6 +71,7 @@ def lib():
     L.hmlfc_decode_views.argtypes, L.hmlfc_decode_views.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
     L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
+    L.hmlfc_decode_views_host.argtypes, L.hmlfc_decode_views_host.restype = [vp, vp, i64, vp], C.c_int
     L.hmlfc_render_host.argtypes, L.hmlfc_render_host.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp], C.c_int
     L.hmlfc_last_oob_count.argtypes, L.hmlfc_last_oob_count.restype = [vp, C.POINTER(i64)], C.c_int
     L.hmlfc_footprint_render.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(Footprint)]
@@ -200,6 +201,20 @@ def hmlfc_decode_host(h: Handle, coords: np.ndarray, out: np.ndarray = None) -> 
     assert out.dtype == np.uint8 and out.flags.c_contiguous and out.size == 3 * n
     _check(lib().hmlfc_decode_host(h._h, coords.ctypes.data_as(C.c_void_p), n, out.ctypes.data_as(C.c_void_p)),
            "hmlfc_decode_host", h._h)
+    return out
+
+
+def hmlfc_decode_views_host(h: Handle, views: np.ndarray, out: np.ndarray = None) -> np.ndarray:
+    """End-to-end dense decode with HOST buffers: views int32 [n][2] = (u,v) -> uint8 [n][Ht][Ws][3]."""
+    _require_cuda()
+    assert views.dtype == np.int32 and views.flags.c_contiguous and views.shape[-1] == 2
+    n = views.size // 2
+    Ht, Ws = h.info.Ht, h.info.Ws
+    if out is None:
+        out = np.empty((n, Ht, Ws, 3), dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.flags.c_contiguous and out.size == n * Ht * Ws * 3
+    _check(lib().hmlfc_decode_views_host(h._h, views.ctypes.data_as(C.c_void_p), n, out.ctypes.data_as(C.c_void_p)),
+           "hmlfc_decode_views_host", h._h)
     return out
 
 

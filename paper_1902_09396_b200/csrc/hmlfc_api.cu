@@ -255,6 +255,33 @@ int hmlfc_decode_host(hmlfc_handle *h, const int32_t *h_coords, int64_t n, uint8
     return sync_pipeline(h);
 }
 
+int hmlfc_decode_views_host(hmlfc_handle *h, const int32_t *h_views, int64_t n_views, uint8_t *h_out)
+{
+    if (!h || n_views < 0 || (n_views > 0 && (!h_views || !h_out))) return HMLFC_E_INVALID;
+    if (n_views == 0) return HMLFC_OK;
+    const size_t view_bytes = (size_t)h->ds.Ws * h->ds.Ht * 3;
+    int rc;
+    if ((rc = ensure(h, &h->d_in, &h->d_in_cap, (size_t)n_views * 8)) != HMLFC_OK) return rc;
+    if ((rc = ensure(h, reinterpret_cast<void **>(&h->d_outbuf), &h->d_out_cap, (size_t)n_views * view_bytes + 4)) != HMLFC_OK) return rc;
+    // chunks of whole views, about 6 MB of pixels each; kernels alternate between two streams, result copies on a third
+    int64_t per = (int64_t)((((size_t)6 << 20) + view_bytes - 1) / view_bytes);
+    if ((n_views + per - 1) / per > hmlfc_handle::kMaxChunks) per = (n_views + hmlfc_handle::kMaxChunks - 1) / hmlfc_handle::kMaxChunks;
+    const int32_t *d_views = static_cast<const int32_t *>(h->d_in);
+    CU(h, cudaMemcpyAsync(h->d_in, h_views, (size_t)n_views * 8, cudaMemcpyHostToDevice, h->host_stream));
+    CU(h, cudaEventRecord(h->ev_in[0], h->host_stream));
+    CU(h, cudaStreamWaitEvent(h->in_stream, h->ev_in[0], 0));
+    int c = 0;
+    for (int64_t v = 0; v < n_views; v += per, ++c) {
+        const int64_t m = (n_views - v < per) ? n_views - v : per;
+        cudaStream_t ks = (c & 1) ? h->in_stream : h->host_stream;
+        if ((rc = hmlfc_decode_views(h, d_views + 2 * v, m, h->d_outbuf + (size_t)v * view_bytes, ks)) != HMLFC_OK) { sync_pipeline(h); return rc; }
+        CU(h, cudaEventRecord(h->ev_done[c], ks));
+        CU(h, cudaStreamWaitEvent(h->out_stream, h->ev_done[c], 0));
+        CU(h, cudaMemcpyAsync(h_out + (size_t)v * view_bytes, h->d_outbuf + (size_t)v * view_bytes, (size_t)m * view_bytes, cudaMemcpyDeviceToHost, h->out_stream));
+    }
+    return sync_pipeline(h);
+}
+
 int hmlfc_render_host(hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, int W, int H, uint8_t *h_out)
 {
     if (!h || n_views < 0 || W <= 0 || H <= 0 || (n_views > 0 && (!h_cameras || !h_out))) return HMLFC_E_INVALID;

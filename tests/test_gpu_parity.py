@@ -103,6 +103,7 @@ def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
     for k, (u, v) in enumerate(views):
         assert np.array_equal(got[k], info["p1"][v, u]), (name, u, v)
     assert P.hmlfc_decode_views(h, _dev(views[:0])).numel() == 0
+    assert np.array_equal(P.hmlfc_decode_views_host(h, views), got)   # host buffers, pipelined in chunks of views
     # a view outside the grid is black and counted
     before = P.hmlfc_last_oob_count(h)
     bad = P.hmlfc_decode_views(h, _dev(np.array([[cfg.U, 0], [0, 0]], dtype=np.int32))).cpu().numpy()
