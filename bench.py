@@ -412,6 +412,13 @@ def run_ours(args, cfg_name):
                          "traffic": _ncu_from_profiles(cfg.name, "decode").get("dram_bytes")},
         }
         clocks = clk.summary()
+        # the bound that binds hmlfc_decode on an L2-resident stream: random 32-byte sector gathers served by the L2
+        dsec = _ncu_from_profiles(cfg.name, "decode").get("l2_read_sectors")
+        gpeak = _ncu_top("gather_peak").get("l2_g_sectors_per_s")
+        if dsec and gpeak and info["stream_bytes"] < (96 << 20):
+            decode["roofline"]["gather"] = {"bound": "l2-sector-gather", "achieved": dsec / (dec_kernel_ms * 1e-3) / 1e9, "peak": gpeak,
+                                            "unit": "G sectors/s", "frac": dsec / (dec_kernel_ms * 1e-3) / 1e9 / gpeak, "sectors_per_launch": dsec,
+                                            "source": "lts__t_sectors_srcunit_tex_op_read.sum of the committed ncu capture; peak = gather_probe (profiles/r01_gather_probe.md)"}
         roofline["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "render").get("warp_inst"), kernel_ms, clocks.get("sm_mhz"))
         decode["roofline"]["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "decode").get("warp_inst"), dec_kernel_ms,
                                               clocks.get("sm_mhz"))
@@ -503,6 +510,15 @@ def _ncu_from_profiles(cfg_name, which):
         except Exception:
             return {}
     return {}
+
+
+def _ncu_top(key):
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as fh:
+            return json.load(fh).get(key, {}) or {}
+    except Exception:
+        return {}
 
 
 def _alu_view(warp_inst, kernel_ms, sm_mhz, n_sms=148):
