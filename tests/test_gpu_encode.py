@@ -150,3 +150,41 @@ def test_invalid_and_unsupported_arguments(P):
         P.hmlfc_encode(lf, 1, target_psnr=-3.0)
     with pytest.raises(P.HmlfcError):
         P.hmlfc_encode(lf, 1, target_psnr=40.0, max_iter=0)
+
+
+@pytest.mark.parametrize("U,V,Ws,Ht,h,B,W", [(1, 1, 8, 4, 1, 4, 16), (2, 1, 8, 8, 1, 4, 3), (1, 3, 12, 8, 2, 2, 2), (3, 3, 16, 8, 3, 8, 1), (2, 2, 4, 4, 1, 4, 0)])
+def test_degenerate_shapes(P, U, V, Ws, Ht, h, B, W):
+    """One view (no predictive plane at all), one row / column of views, one block per image, a window far wider than the image, W = 0
+    (prediction from the co-located block only): encoder stream equal to the oracle's, and the decode of every pixel through the GPU-
+    encoded stream equal to the oracle's decode."""
+    from conftest import random_lf
+
+    lf = random_lf(np.random.default_rng(U * 100 + V * 10 + B), U, V, Ws, Ht)
+    for tau in (0, 25):
+        p = orc.make_params(U, V, Ws, Ht, h, B, W, tau // 2, tau, seed=7)
+        data, info, tree = orc.encode(lf, p)
+        tree.close()
+        got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), h, B, W, tau // 2, tau, seed=7)
+        _assert_same_stream(got, data)
+        hd = P.hmlfc_load(got)
+        views = np.array([[u, v] for v in range(V) for u in range(U)], dtype=np.int32)
+        dec = P.hmlfc_decode_views(hd, torch.from_numpy(views).cuda()).cpu().numpy().reshape(V, U, Ht, Ws, 3)
+        assert np.array_equal(dec, orc.Stream(data).decode_full())
+        if tau == 0:
+            assert np.array_equal(dec, lf)  # lossless round trip (north_star pin 1)
+        # a camera ON the camera plane (so that a 1-view-wide grid is hit at all), looking at the centre of the image plane
+        ex, ey = 0.4 * (U - 1), 0.3 * (V - 1)
+        cam = np.zeros((1, 16), dtype=np.float32)
+        cam[0, 0:3] = (ex, ey, 0.0)
+        cam[0, 3:6], cam[0, 6:9] = (1, 0, 0), (0, 1, 0)
+        cam[0, 9:12] = ((Ws - 1) / 2 - ex, (Ht - 1) / 2 - ey, 1.0)
+        cam[0, 12:14] = (0.45 * Ws, 0.45 * Ht)
+        ref = orc.Stream(data).render(cam, 40, 24)
+        assert ref.any()
+        outs = []
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+            P.hmlfc_set_render_variant(hd, variant)
+            outs.append(P.hmlfc_render(hd, torch.from_numpy(cam).cuda(), 40, 24).cpu().numpy())
+            assert np.abs(outs[-1].astype(int) - ref.astype(int)).max() <= 1, variant
+            assert np.array_equal(outs[-1], outs[0])
+        P.hmlfc_free(hd)
