@@ -247,7 +247,7 @@ compact_kernel(const int16_t *__restrict__ srv, const int4 *__restrict__ rec, co
 }
 
 // reconstruct_sse_kernel: the encoder's own dense reconstruction at the current thresholds (what a decoder
-// makes of the stream) and its squared error against the input, one thread per light-field pixel:
+// makes of the stream) and its squared error against the input:
 //   acc_c = X_h + sum_L [ res ? stored : 0 ] + [ pred ? +-R'(x+dx, y+dy) : 0 ],  stored = P (reference / intra) or P -+ R(x+dx, y+dy),
 //   R' = the reference sample AS STORED (0 where its block is insignificant or outside the image), R = the unthresholded one (R12);
 //   then inverse YCoCg-R and clamp (R17, R19).  The sum of squared RGB differences feeds the PSNR of PAPER.md:366 / :375.
@@ -258,48 +258,62 @@ struct RecGeom {
     uint64_t top_off, x_ch;                       // element offset of the top-level RKV planes of channel 0 in d_x; channel stride
 };
 
+// One thread per block-row segment (B consecutive pixels of one block row of one view): the plane-channel descriptor, the flag words
+// and the motion record of a (level, channel) are fetched once per B pixels.
+template <int B>
 __global__ void __launch_bounds__(kThreads)
 reconstruct_sse_kernel(const uint8_t *__restrict__ lf, const int16_t *__restrict__ srv, const int16_t *__restrict__ xk, const int4 *__restrict__ rec,
-                       const EncPc *__restrict__ pcs, const uint32_t *__restrict__ flags, RecGeom G, unsigned long long n_px,
+                       const EncPc *__restrict__ pcs, const uint32_t *__restrict__ flags, RecGeom G, unsigned long long n_seg,
                        unsigned long long *__restrict__ sse)
 {
     const unsigned long long g = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
     unsigned long long err = 0ull;
-    if (g < n_px) {
+    if (g < n_seg) {
         const unsigned long long npx = (unsigned long long)G.Ws * G.Ht;
-        const int view = (int)(g / npx), pix = (int)(g - (unsigned long long)view * npx);
-        const int v = view / G.U, u = view - v * G.U, t = pix / G.Ws, s = pix - t * G.Ws;
-        const int b = (t >> G.shiftB) * G.nbx + (s >> G.shiftB);
-        int a[3];
+        const unsigned long long seg_per_view = npx / B;
+        const int view = (int)(g / seg_per_view), seg = (int)(g - (unsigned long long)view * seg_per_view);
+        const int v = view / G.U, u = view - v * G.U, t = seg / G.nbx, bx = seg - t * G.nbx, s0 = bx * B;
+        const int b = (t >> G.shiftB) * G.nbx + bx;
+        const int pix = t * G.Ws + s0;
+        int a[3][B];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            int acc = xk[G.top_off + (uint64_t)c * G.x_ch + (uint64_t)((v >> G.h) * G.UL[G.h] + (u >> G.h)) * npx + pix];
+            load_row<B>(xk + G.top_off + (uint64_t)c * G.x_ch + (uint64_t)((v >> G.h) * G.UL[G.h] + (u >> G.h)) * npx + pix, a[c]);
             for (int L = 0; L < G.h; ++L) {
                 const int pu = u >> L, pv = v >> L;
                 const EncPc pc = pcs[G.kbase[L] + (uint32_t)(pv * G.UL[L] + pu) * 3u + c];
                 const bool res = (flags[pc.flag_word + (b >> 5)] >> (b & 31)) & 1u;
-                const int P = srv[pc.srv_off + pix];
-                int term = res ? P : 0;
+                int P[B];
+                load_row<B>(srv + pc.srv_off + pix, P);
                 if (pc.rec_off != kNoRec && ((flags[pc.flag_word + G.fwords + (b >> 5)] >> (b & 31)) & 1u)) {
                     const int4 m = rec[pc.rec_off + b];
-                    const int x = s + m.y, y = t + m.z;
-                    int q = 0, qs = 0;
-                    if (x >= 0 && x < G.Ws && y >= 0 && y < G.Ht) {
-                        q = srv[pc.ref_off + (size_t)y * G.Ws + x];
-                        const EncPc rp = pcs[G.kbase[L] + (uint32_t)((pv & ~1) * G.UL[L] + (pu & ~1)) * 3u + c];
-                        const int rb = (y >> G.shiftB) * G.nbx + (x >> G.shiftB);
-                        qs = ((flags[rp.flag_word + (rb >> 5)] >> (rb & 31)) & 1u) ? q : 0;
+                    const uint64_t rflag = pcs[G.kbase[L] + (uint32_t)((pv & ~1) * G.UL[L] + (pu & ~1)) * 3u + c].flag_word;
+                    const int y = t + m.z;
+#pragma unroll
+                    for (int i = 0; i < B; ++i) {
+                        const int x = s0 + i + m.y;
+                        int q = 0, qs = 0;
+                        if (x >= 0 && x < G.Ws && y >= 0 && y < G.Ht) {
+                            q = srv[pc.ref_off + (size_t)y * G.Ws + x];
+                            const int rb = (y >> G.shiftB) * G.nbx + (x >> G.shiftB);
+                            qs = ((flags[rflag + (rb >> 5)] >> (rb & 31)) & 1u) ? q : 0;
+                        }
+                        a[c][i] += (res ? (m.x ? P[i] + q : P[i] - q) : 0) + (m.x ? -qs : qs);
                     }
-                    term = (res ? (m.x ? P + q : P - q) : 0) + (m.x ? -qs : qs);
+                } else if (res) {
+#pragma unroll
+                    for (int i = 0; i < B; ++i) a[c][i] += P[i];
                 }
-                acc += term;
             }
-            a[c] = acc;
         }
-        const int tt = a[0] - (a[2] >> 1), Gc = a[2] + tt, Bc = tt - (a[1] >> 1), Rc = Bc + a[1];  // inverse YCoCg-R lifting
-        const uint8_t *px = lf + g * 3ull;
-        const int dr = min(max(Rc, 0), 255) - (int)px[0], dg = min(max(Gc, 0), 255) - (int)px[1], db = min(max(Bc, 0), 255) - (int)px[2];
-        err = (unsigned long long)(dr * dr + dg * dg + db * db);
+        const uint8_t *px = lf + ((unsigned long long)view * npx + pix) * 3ull;
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            const int tt = a[0][i] - (a[2][i] >> 1), Gc = a[2][i] + tt, Bc = tt - (a[1][i] >> 1), Rc = Bc + a[1][i];  // inverse YCoCg-R lifting
+            const int dr = min(max(Rc, 0), 255) - (int)px[3 * i], dg = min(max(Gc, 0), 255) - (int)px[3 * i + 1],
+                      db = min(max(Bc, 0), 255) - (int)px[3 * i + 2];
+            err += (unsigned long long)(dr * dr + dg * dg + db * db);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) err += __shfl_xor_sync(FULL, err, o);
@@ -579,9 +593,12 @@ static int encode_impl(const uint8_t *d_lf, const hmlfc_encode_params_t *p_in, d
     auto measure_sse = [&](unsigned long long *out) -> cudaError_t {
         cudaError_t e = cudaMemsetAsync(dsse.p, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return e;
-        reconstruct_sse_kernel<<<(unsigned)((n_lf_px + kThreads - 1) / kThreads), kThreads, 0, st>>>(d_lf, srv.as<int16_t>(), xk.as<int16_t>(), rec.as<int4>(),
-                                                                                                     dpcs.as<EncPc>(), dflags.as<uint32_t>(), geo, n_lf_px,
-                                                                                                     dsse.as<unsigned long long>());
+        const unsigned long long n_seg = n_lf_px / (unsigned long long)B;
+        const unsigned gs = (unsigned)((n_seg + kThreads - 1) / kThreads);
+#define RECON(BB) reconstruct_sse_kernel<BB><<<gs, kThreads, 0, st>>>(d_lf, srv.as<int16_t>(), xk.as<int16_t>(), rec.as<int4>(), dpcs.as<EncPc>(), \
+                                                                     dflags.as<uint32_t>(), geo, n_seg, dsse.as<unsigned long long>())
+        if (B == 2) RECON(2); else if (B == 4) RECON(4); else RECON(8);
+#undef RECON
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         if ((e = cudaMemcpyAsync(out, dsse.p, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return e;
         return cudaStreamSynchronize(st);
