@@ -188,3 +188,26 @@ def test_degenerate_shapes(P, U, V, Ws, Ht, h, B, W):
             assert np.abs(outs[-1].astype(int) - ref.astype(int)).max() <= 1, variant
             assert np.array_equal(outs[-1], outs[0])
         P.hmlfc_free(hd)
+
+
+def test_more_than_65535_plane_channels(P):
+    """160 x 160 views of 4 x 4 pixels, h = 2: 96,000 plane-channels, more than one grid.y's worth -- the encoder's kernels run in
+    chunks of 65,535 plane-channels.  Stream equal to the oracle's; every view decodes to the oracle's decode."""
+    U = V = 160
+    rng = np.random.default_rng(11)
+    base = rng.integers(0, 256, (V + 4, U + 4, 3)).astype(np.float64)
+    lf = np.empty((V, U, 4, 4, 3), dtype=np.uint8)
+    for t in range(4):
+        for s in range(4):  # neighbouring views are shifted copies of one image: inter-view coherence
+            lf[:, :, t, s] = np.clip(base[t:t + V, s:s + U] + rng.normal(0, 3.0, (V, U, 3)), 0, 255).astype(np.uint8)
+    p = orc.make_params(U, V, 4, 4, 2, 4, 1, 6, 12, seed=3)
+    data, info, tree = orc.encode(lf, p)
+    tree.close()
+    assert struct.unpack_from("<Q", data, 104)[0] == 96000
+    got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), 2, 4, 1, 6, 12, seed=3)
+    _assert_same_stream(got, data)
+    h = P.hmlfc_load(got)
+    views = np.array([[u, v] for v in range(V) for u in range(U)], dtype=np.int32)
+    dec = P.hmlfc_decode_views(h, torch.from_numpy(views).cuda()).cpu().numpy().reshape(V, U, 4, 4, 3)
+    assert np.array_equal(dec, orc.Stream(data).decode_full())
+    P.hmlfc_free(h)
