@@ -200,14 +200,32 @@ def test_more_than_65535_plane_channels(P):
     for t in range(4):
         for s in range(4):  # neighbouring views are shifted copies of one image: inter-view coherence
             lf[:, :, t, s] = np.clip(base[t:t + V, s:s + U] + rng.normal(0, 3.0, (V, U, 3)), 0, 255).astype(np.uint8)
-    p = orc.make_params(U, V, 4, 4, 2, 4, 1, 6, 12, seed=3)
+    geo = dict(uv_origin=(0.0, 0.0), uv_step=(0.02, 0.02), st_origin=(0.0, 0.0), st_step=(1.0, 1.0), z_st=1.0)  # a dense camera grid
+    p = orc.make_params(U, V, 4, 4, 2, 4, 1, 6, 12, geometry=geo, seed=3)
     data, info, tree = orc.encode(lf, p)
     tree.close()
     assert struct.unpack_from("<Q", data, 104)[0] == 96000
-    got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), 2, 4, 1, 6, 12, seed=3)
+    got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), 2, 4, 1, 6, 12, geometry=geo, seed=3)
     _assert_same_stream(got, data)
     h = P.hmlfc_load(got)
     views = np.array([[u, v] for v in range(V) for u in range(U)], dtype=np.int32)
     dec = P.hmlfc_decode_views(h, torch.from_numpy(views).cuda()).cpu().numpy().reshape(V, U, 4, 4, 3)
     assert np.array_equal(dec, orc.Stream(data).decode_full())
+    # a camera behind the camera plane: every 32 x 32 output tile spans dozens of views (more than the CTA kernel's 4 x 4 per pass),
+    # so the tile is split down to direct decodes; all render kernels agree with the oracle and with one another
+    cam = np.zeros((1, 16), dtype=np.float32)
+    cam[0, 0:3] = (1.6, 1.55, -40.0)
+    cam[0, 3:6], cam[0, 6:9] = (1, 0, 0), (0, 1, 0)
+    cam[0, 9:12] = ((1.5 - 1.6) / 41.0, (1.5 - 1.55) / 41.0, 1.0)
+    cam[0, 12:14] = (1.4 / 41.0, 1.4 / 41.0)
+    s_or = orc.Stream(data)
+    ref = s_or.render(cam, 96, 64)
+    assert ref.any()
+    first = None
+    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+        P.hmlfc_set_render_variant(h, variant)
+        out = P.hmlfc_render(h, torch.from_numpy(cam).cuda(), 96, 64).cpu().numpy()
+        assert np.abs(out.astype(int) - ref.astype(int)).max() <= 1, variant
+        first = out if first is None else first
+        assert np.array_equal(out, first)
     P.hmlfc_free(h)
