@@ -178,7 +178,11 @@ int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_
 {
     if (!h || n_views < 0 || (n_views > 0 && (!d_views || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    CU(h, launch_decode_views(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    // B = 4 streams: one lane per block-row segment; other block sizes (and decode variant 1 / 2, for cross-checks): one lane per pixel
+    if (h->ds.B == 4 && h->decode_variant == 0)
+        CU(h, launch_decode_rows(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    else
+        CU(h, launch_decode_views(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     h->launches += nl;
     return HMLFC_OK;
 }

@@ -23,6 +23,9 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
 // whole views: d_views = int32 [n_views][2] = (u, v); d_out = uint8 [n_views][Ht][Ws][3]; coordinates are generated in the kernel
 cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
                                 cudaStream_t st, int *n_launches);
+// the same for B = 4 streams: one lane per block-row segment (hmlfc_render_cta.cu)
+cudaError_t launch_decode_rows(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
+                               cudaStream_t st, int *n_launches);
 cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
                                 cudaStream_t st, int *n_launches);
 cudaError_t launch_render_tiled(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,

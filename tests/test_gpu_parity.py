@@ -90,7 +90,7 @@ def test_decode_out_of_range_is_black_and_counted(P, enc):
     P.hmlfc_free(h)
 
 
-@pytest.mark.parametrize("name", ["cfg1_lossy", "mini3", "mini_b8", "mini_h8"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b8", "mini_h8", "mini_w64"])
 def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
     # hmlfc_decode_views: whole views, coordinates generated in the kernel; every view of the light field (shuffled order, one repeated)
     cfg, lf, data, info, s = enc(name)
@@ -104,6 +104,9 @@ def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
         assert np.array_equal(got[k], info["p1"][v, u]), (name, u, v)
     assert P.hmlfc_decode_views(h, _dev(views[:0])).numel() == 0
     assert np.array_equal(P.hmlfc_decode_views_host(h, views), got)   # host buffers, pipelined in chunks of views
+    P.hmlfc_set_decode_variant(h, P.DECODE_QUEUE)   # the lane-per-pixel kernel (the default for B = 4 is one lane per block-row segment)
+    assert np.array_equal(P.hmlfc_decode_views(h, _dev(views)).cpu().numpy(), got)
+    P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
     # a view outside the grid is black and counted
     before = P.hmlfc_last_oob_count(h)
     bad = P.hmlfc_decode_views(h, _dev(np.array([[cfg.U, 0], [0, 0]], dtype=np.int32))).cpu().numpy()
@@ -254,6 +257,10 @@ def test_progressive_levels_match_oracle(P, enc, name):
         for variant in (P.DECODE_THREAD, P.DECODE_QUEUE):
             P.hmlfc_set_decode_variant(h, variant)
             assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), (L, variant)
+        # whole views at this level: the block-row kernel (B = 4) / the lane-per-pixel kernel; all_coords is in [V][U][Ht][Ws] order
+        P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
+        all_views = np.array([[u, v] for v in range(cfg.V) for u in range(cfg.U)], dtype=np.int32)
+        assert np.array_equal(P.hmlfc_decode_views(h, _dev(all_views)).cpu().numpy().reshape(-1, 3), expect), L
         ref = s.render(cams, cfg.out_w, cfg.out_h)
         outs = []
         for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):   # WARP falls back to the per-pixel kernel when L > 0
