@@ -483,6 +483,11 @@ def run_ours(args, cfg_name):
                                "workload": "the same camera circle on the camera plane z = 0 (SURVEY 8(d) D4: every view blends exactly 4 light-field views)"},
             "decode_views": {"value": whole_job_rate(dv_px, len(dv_ms), world, dv_total * 1e-3), "unit": "LF pixels/s", "n_views": int(n_dv),
                              "pixels_per_launch": int(dv_px), "ms_per_launch": float(np.mean(dv_ms)),
+                             "roofline": {"bound": "hbm", "kernel": "decode_rows_kernel" if cfg.block == 4 else "decode_queue_kernel<dense>",
+                                          "achieved": (3 * dv_px + 8 * n_dv + info["stream_bytes"]) / (float(np.mean(dv_ms)) * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                                          "frac": (3 * dv_px + 8 * n_dv + info["stream_bytes"]) / (float(np.mean(dv_ms)) * 1e-3) / 1e9 / peak,
+                                          "bytes_alg_per_launch": int(3 * dv_px + 8 * n_dv + info["stream_bytes"]),
+                                          "note": "algorithmic bytes = output + view list + the whole compressed stream once (exact when every view is decoded, else an upper bound)"},
                              "e2e": {"value": whole_job_rate(dv_px, 3, world, dv_e2e_s), "unit": "LF pixels/s", "h2d_bytes_per_step": 8 * int(n_dv),
                                      "d2h_bytes_per_step": 3 * int(dv_px), "steps": 3},
                              "workload": "hmlfc_decode_views: every pixel of a seeded random set of whole views (coordinates generated in the kernel)"},
