@@ -107,7 +107,8 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
  *   d_views : device, int32 [n_views][2] = (u, v).
  *   d_out   : device, uint8 [n_views][Ht][Ws][3] RGB.
  * A view outside the camera grid is written black and every pixel of it counted as out of range.  Progressive decoding
- * (hmlfc_set_min_level) applies.  Asynchronous like hmlfc_decode. */
+ * (hmlfc_set_min_level) applies.  Asynchronous like hmlfc_decode.  B = 4 streams run one lane per block-row segment (4 pixels);
+ * other block sizes, and any stream after hmlfc_set_decode_variant(h, 1 or 2), one lane per pixel -- identical bytes. */
 int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_views, uint8_t *d_out, void *cuda_stream);
 
 /* hmlfc_render -- PAPER.md:73 / :309 / :409: per output pixel, ray -> (u,v,s,t) on the two
