@@ -229,3 +229,57 @@ def test_more_than_65535_plane_channels(P):
         first = out if first is None else first
         assert np.array_equal(out, first)
     P.hmlfc_free(h)
+
+
+def test_randomised_shapes_and_parameters(P):
+    """150 seeded random small light fields (grid 1..6 x 1..6, images of 1..6 x 1..5 blocks, B in {2,4,8}, h 1..4, W 0..9, thresholds 0..120,
+    all three policies): GPU encoder stream = oracle stream; GPU decode of every view (dense kernels) and of shuffled coordinates (both
+    decode kernels) = oracle decode; one on-plane view through every render kernel within 1 LSB of the oracle and byte-identical."""
+    from conftest import random_lf
+
+    rng = np.random.default_rng(20260411)
+    for case in range(150):
+        B = int(rng.choice([2, 4, 8]))
+        U, V = int(rng.integers(1, 7)), int(rng.integers(1, 7))
+        Ws, Ht = B * int(rng.integers(1, 7)), B * int(rng.integers(1, 6))
+        if Ws % 4:
+            Ws *= 2  # hmlfc_hierarchy needs Ws % 4 == 0
+        h, W, tau, policy = int(rng.integers(1, 5)), int(rng.integers(0, 10)), int(rng.integers(0, 121)), int(rng.integers(0, 3))
+        tag = (case, U, V, Ws, Ht, h, B, W, tau, policy)
+        lf = random_lf(rng, U, V, Ws, Ht, smooth=bool(case & 1))
+        p = orc.make_params(U, V, Ws, Ht, h, B, W, tau // 2, tau, policy=policy, seed=case)
+        data, info, tree = orc.encode(lf, p)
+        tree.close()
+        got, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), h, B, W, tau // 2, tau, policy, seed=case)
+        assert got == data, tag
+        s = orc.Stream(data)
+        full = s.decode_full()
+        hd = P.hmlfc_load(got)
+        views = np.array([[u, v] for v in range(V) for u in range(U)], dtype=np.int32)
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE):
+            P.hmlfc_set_decode_variant(hd, variant)
+            dec = P.hmlfc_decode_views(hd, torch.from_numpy(views).cuda()).cpu().numpy().reshape(V, U, Ht, Ws, 3)
+            assert np.array_equal(dec, full), tag
+        coords = np.stack([a.ravel() for a in np.meshgrid(np.arange(U), np.arange(V), np.arange(Ws), np.arange(Ht), indexing="ij")], 1).astype(np.int32)
+        coords = coords[rng.permutation(len(coords))]
+        expect = full[coords[:, 1], coords[:, 0], coords[:, 3], coords[:, 2]]
+        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE):
+            P.hmlfc_set_decode_variant(hd, variant)
+            assert np.array_equal(P.hmlfc_decode(hd, torch.from_numpy(coords).cuda()).cpu().numpy(), expect), tag
+        P.hmlfc_set_decode_variant(hd, P.DECODE_AUTO)
+        cam = np.zeros((1, 16), dtype=np.float32)
+        ex, ey = float(rng.uniform(0, max(U - 1, 0))), float(rng.uniform(0, max(V - 1, 0)))
+        cam[0, 0:3] = (ex, ey, 0.0)
+        cam[0, 3:6], cam[0, 6:9] = (1, 0, 0), (0, 1, 0)
+        cam[0, 9:12] = ((Ws - 1) / 2 - ex, (Ht - 1) / 2 - ey, 1.0)
+        cam[0, 12:14] = (0.55 * Ws, 0.55 * Ht)   # a little wider than the image plane: the border rays miss
+        ref = s.render(cam, 45, 37)
+        first = None
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG,
+                        P.RENDER_CTA_SMALL):
+            P.hmlfc_set_render_variant(hd, variant)
+            out = P.hmlfc_render(hd, torch.from_numpy(cam).cuda(), 45, 37).cpu().numpy()
+            assert np.abs(out.astype(int) - ref.astype(int)).max() <= 1, (tag, variant)
+            first = out if first is None else first
+            assert np.array_equal(out, first), (tag, variant)
+        P.hmlfc_free(hd)
