@@ -370,3 +370,53 @@ def test_full_size_sampled_parity(P, name):
     target = cfg.target_psnr
     assert target - 2.0 < info["psnr"] < target + 2.0  # "quantisation set for ~40 dB" (45 dB for cfg3)
     P.hmlfc_free(h)
+
+
+def test_randomised_cameras_levels_and_geometries(P):
+    """60 seeded random cases: small light fields (3..8 x 3..8 views of 16..48-pixel images, B = 4, h 1..3) with a random light-slab
+    geometry, three rotated off-plane cameras each (random eye, look-at, field of view, output size; many rays miss), a random
+    progressive level: every render kernel configuration within 1 LSB of the oracle and byte-identical to the thread-per-pixel kernel."""
+    import oracle as orc
+    from conftest import random_lf
+
+    rng = np.random.default_rng(190209396)
+    hit = []
+    for case in range(60):
+        U, V = int(rng.integers(3, 9)), int(rng.integers(3, 9))
+        Ws, Ht = 4 * int(rng.integers(4, 13)), 4 * int(rng.integers(4, 13))
+        h, W, tau = int(rng.integers(1, 4)), int(rng.integers(1, 9)), int(rng.integers(0, 60))
+        step_u, step_v = float(rng.uniform(0.2, 1.0)) * Ws / (2 * U), float(rng.uniform(0.2, 1.0)) * Ht / (2 * V)
+        z_st = float(rng.uniform(0.3, 2.0)) * Ws
+        geo = dict(uv_origin=(float(rng.uniform(-3, 3)), float(rng.uniform(-3, 3))), uv_step=(step_u, step_v),
+                   st_origin=(float(rng.uniform(-5, 5)), float(rng.uniform(-5, 5))), st_step=(float(rng.uniform(0.5, 2.0)), float(rng.uniform(0.5, 2.0))),
+                   z_st=z_st)
+        lf = random_lf(rng, U, V, Ws, Ht)
+        p = orc.make_params(U, V, Ws, Ht, h, 4, W, tau // 2, tau, geometry=geo, seed=case)
+        data, info, tree = orc.encode(lf, p)
+        tree.close()
+        s = orc.Stream(data)
+        hd = P.hmlfc_load(data)
+        L = int(rng.integers(0, h + 1))
+        s.set_min_level(L)
+        P.hmlfc_set_min_level(hd, L)
+        uc = (geo["uv_origin"][0] + 0.5 * (U - 1) * step_u, geo["uv_origin"][1] + 0.5 * (V - 1) * step_v)
+        sc = (geo["st_origin"][0] + 0.5 * (Ws - 1) * geo["st_step"][0], geo["st_origin"][1] + 0.5 * (Ht - 1) * geo["st_step"][1])
+        cams = []
+        for _ in range(3):
+            eye = (uc[0] + rng.uniform(-0.35, 0.35) * U * step_u, uc[1] + rng.uniform(-0.35, 0.35) * V * step_v, -float(rng.uniform(0.0, 0.8)) * z_st)
+            look = (sc[0] + rng.uniform(-0.3, 0.3) * Ws * geo["st_step"][0], sc[1] + rng.uniform(-0.3, 0.3) * Ht * geo["st_step"][1], z_st)
+            d = float(np.linalg.norm(np.array(look) - np.array(eye)))
+            th = float(rng.uniform(0.1, 0.5)) * Ws * geo["st_step"][0] / d
+            cams.append(wl._camera(eye, look, th, th * float(rng.uniform(0.6, 1.4))))
+        cams = np.stack(cams)
+        Wo, Ho = int(rng.integers(20, 100)), int(rng.integers(20, 80))
+        ref = s.render(cams, Wo, Ho)
+        hit.append(float(ref.reshape(-1, 3).any(1).mean()))
+        outs = {}
+        for variant in (P.RENDER_PIXEL, P.RENDER_AUTO, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+            P.hmlfc_set_render_variant(hd, variant)
+            outs[variant] = P.hmlfc_render(hd, _dev(cams), Wo, Ho).cpu().numpy()
+            assert np.abs(outs[variant].astype(int) - ref.astype(int)).max() <= TOL_VIEW, (case, variant, L)
+            assert np.array_equal(outs[variant], outs[P.RENDER_PIXEL]), (case, variant, L)
+        P.hmlfc_free(hd)
+    assert np.mean(hit) > 0.2 and np.mean(np.array(hit) < 0.98) > 0.5   # the cameras see the light field, and most frames also have misses
