@@ -306,6 +306,17 @@ def run_ours(args, cfg_name):
     assert torch.equal(dv_pin.cuda(), dv_out), "decode_views: host entry point and device entry point disagree"
     del dv_out, dv_pin
 
+    # ---- random access at block granularity: as many pixels as the decode leg, in whole B x B blocks at seeded random positions
+    n_blk = max(1, n_dec // (cfg.block * cfg.block))
+    brng = np.random.Generator(np.random.PCG64(cfg.seed + 4000 + rank))
+    blk_np = np.stack([brng.integers(0, cfg.U, n_blk), brng.integers(0, cfg.V, n_blk), brng.integers(0, cfg.Ws // cfg.block, n_blk),
+                       brng.integers(0, cfg.Ht // cfg.block, n_blk)], axis=1).astype(np.int32)
+    blk_d = torch.from_numpy(blk_np).cuda()
+    blk_out = torch.empty((n_blk, cfg.block, cfg.block, 3), dtype=torch.uint8, device="cuda")
+    blk_ms = timed(lambda: P.hmlfc_decode_blocks(h, blk_d, out=blk_out, stream=stream), max(3, min(args.steps, 10)), 3)
+    blk_total = reduce_max(sum(blk_ms), world, "cuda")
+    del blk_out, blk_d
+
     # ---- end to end through the C ABI with HOST (pinned) buffers: cameras H2D + views D2H inside the timed region
     cams_pin = torch.from_numpy(cams_np).pin_memory()
     out_pin = torch.empty((V, H, W, 3), dtype=torch.uint8).pin_memory()
@@ -491,6 +502,9 @@ def run_ours(args, cfg_name):
                              "e2e": {"value": whole_job_rate(dv_px, 3, world, dv_e2e_s), "unit": "LF pixels/s", "h2d_bytes_per_step": 8 * int(n_dv),
                                      "d2h_bytes_per_step": 3 * int(dv_px), "steps": 3},
                              "workload": "hmlfc_decode_views: every pixel of a seeded random set of whole views (coordinates generated in the kernel)"},
+            "decode_blocks": {"value": whole_job_rate(n_blk * cfg.block * cfg.block, len(blk_ms), world, blk_total * 1e-3), "unit": "LF pixels/s",
+                              "blocks_per_launch": int(n_blk), "ms_per_launch": float(np.mean(blk_ms)),
+                              "workload": f"hmlfc_decode_blocks: {n_blk} whole {cfg.block} x {cfg.block} blocks at seeded uniformly random (u, v, bx, by)"},
             "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),

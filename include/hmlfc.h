@@ -111,6 +111,14 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
  * other block sizes, and any stream after hmlfc_set_decode_variant(h, 1 or 2), one lane per pixel -- identical bytes. */
 int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_views, uint8_t *d_out, void *cuda_stream);
 
+/* hmlfc_decode_blocks -- random access at the granularity the paper decodes at ("As a block of pixels are decoded, our
+ * method benefits any LF rendering scheme by providing fast access to neighboring pixels"): whole B x B blocks.
+ *   d_blocks : device, int32 [n][4] = (u, v, bx, by): block column / row inside view (u, v), 0 <= bx < Ws/B, 0 <= by < Ht/B.
+ *   d_out    : device, uint8 [n][B][B][3] RGB (row-major inside the block).
+ * A block outside the light field is written black and its B^2 pixels counted as out of range.  Progressive decoding applies.
+ * Asynchronous like hmlfc_decode; B = 4 streams run one lane per block row, others one lane per pixel -- identical bytes. */
+int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, void *cuda_stream);
+
 /* hmlfc_render -- PAPER.md:73 / :309 / :409: per output pixel, ray -> (u,v,s,t) on the two
  * planes, 16-tap quadrilinear blend of decoded samples (4 nearest views x 4 nearest pixels,
  * edge-clamped), rounded to RGB8; rays that miss the slab get the background colour.

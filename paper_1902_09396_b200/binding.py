@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 
 # every symbol include/hmlfc.h declares
 EXPORTS = (
-    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_render", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_decode_blocks", "hmlfc_render", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
     "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
@@ -69,6 +69,7 @@ def lib():
     L.hmlfc_info.argtypes, L.hmlfc_info.restype = [vp, C.POINTER(Info)], C.c_int
     L.hmlfc_decode.argtypes, L.hmlfc_decode.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_decode_views.argtypes, L.hmlfc_decode_views.restype = [vp, vp, i64, vp, vp], C.c_int
+    L.hmlfc_decode_blocks.argtypes, L.hmlfc_decode_blocks.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
     L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
     L.hmlfc_decode_views_host.argtypes, L.hmlfc_decode_views_host.restype = [vp, vp, i64, vp], C.c_int
@@ -175,6 +176,19 @@ def hmlfc_decode_views(h: Handle, views, out=None, stream=None):
     assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * Ht * Ws * 3
     _check(lib().hmlfc_decode_views(h._h, C.c_void_p(views.data_ptr()), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
            "hmlfc_decode_views", h._h)
+    return out
+
+
+def hmlfc_decode_blocks(h: Handle, blocks, out=None, stream=None):
+    """blocks: CUDA int32 tensor [n][4] = (u,v,bx,by); returns CUDA uint8 tensor [n][B][B][3]."""
+    torch = _require_cuda()
+    assert blocks.is_cuda and blocks.dtype == torch.int32 and blocks.is_contiguous() and blocks.shape[-1] == 4
+    n, B = blocks.numel() // 4, h.info.block
+    if out is None:
+        out = torch.empty((n, B, B, 3), dtype=torch.uint8, device=blocks.device)
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * B * B * 3
+    _check(lib().hmlfc_decode_blocks(h._h, C.c_void_p(blocks.data_ptr()), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
+           "hmlfc_decode_blocks", h._h)
     return out
 
 

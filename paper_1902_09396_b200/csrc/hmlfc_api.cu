@@ -187,6 +187,18 @@ int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_
     return HMLFC_OK;
 }
 
+int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, void *cuda_stream)
+{
+    if (!h || n_blocks < 0 || (n_blocks > 0 && (!d_blocks || !d_out))) return HMLFC_E_INVALID;
+    int nl = 0;
+    if (h->ds.B == 4 && h->decode_variant == 0)
+        CU(h, launch_decode_block_rows(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    else
+        CU(h, launch_decode_blocks(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    h->launches += nl;
+    return HMLFC_OK;
+}
+
 int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
                  void *cuda_stream)
 {

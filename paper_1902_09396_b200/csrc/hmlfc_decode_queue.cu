@@ -144,7 +144,7 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
 
 // kDense: the coordinates are not read but generated -- sample i is pixel i mod (Ws Ht) (row-major) of view views[i / (Ws Ht)]
 // (hmlfc_decode_views: whole views, no 16-byte coordinate per sample, neighbouring lanes in neighbouring pixels).
-template <bool kDense>
+template <int kDense>  // 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
 __global__ void __launch_bounds__(kThreads)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
@@ -160,7 +160,17 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
     const bool present = i < n;
     int4 c4 = make_int4(0, 0, 0, 0);
-    if (kDense) {
+    if (kDense == 2) {
+        if (present) {
+            const int bb = S.B * S.B;
+            const long long blk = i / bb;
+            const int k = (int)(i - blk * bb);
+            const int4 q = __ldg(coords + blk);
+            const int ky = k >> S.logB;
+            c4 = make_int4(q.x, q.y, q.z * S.B + (k - (ky << S.logB)), q.w * S.B + ky);
+            if ((unsigned)q.z >= (unsigned)S.nbx || (unsigned)q.w >= (unsigned)S.nby) c4.z = -1;
+        }
+    } else if (kDense == 1) {
         if (present) {
             const long long npx = (long long)S.Ws * S.Ht;
             const long long view = i / npx;
@@ -273,8 +283,22 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
+    decode_queue_kernel<0><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
                                                                        d_oob, aligned);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode_blocks(const DevStream &S, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, unsigned long long *d_oob,
+                                 cudaStream_t st, int *n_launches)
+{
+    if (n_blocks == 0) return cudaSuccess;
+    if (S.Ws > 65536 || S.Ht > 65536) return cudaErrorInvalidValue;
+    const long long n = (long long)n_blocks * S.B * S.B;
+    const long long blocks = (n + kThreads - 1) / kThreads;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
+    decode_queue_kernel<2><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_blocks), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -288,7 +312,7 @@ cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int6
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<true><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
+    decode_queue_kernel<1><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

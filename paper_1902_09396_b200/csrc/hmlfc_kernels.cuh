@@ -26,6 +26,11 @@ cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int6
 // the same for B = 4 streams: one lane per block-row segment (hmlfc_render_cta.cu)
 cudaError_t launch_decode_rows(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
                                cudaStream_t st, int *n_launches);
+// whole B x B blocks: d_blocks = int32 [n][4] = (u, v, bx, by); d_out = uint8 [n][B][B][3]; lane per pixel (any B) / per block row (B = 4)
+cudaError_t launch_decode_blocks(const DevStream &S, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, unsigned long long *d_oob,
+                                 cudaStream_t st, int *n_launches);
+cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, unsigned long long *d_oob,
+                                     cudaStream_t st, int *n_launches);
 cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
                                 cudaStream_t st, int *n_launches);
 cudaError_t launch_render_tiled(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,

@@ -823,6 +823,9 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
 // per-row decode as phase B3 -- flag / rank record once per (level, channel), the row's 4 stored values from one pass over two
 // 64-bit BISE windows, the motion record once, the motion-compensated reference row from at most two reference blocks -- without
 // the shared-memory tables of the render kernel: whole views need no footprint.  PAPER.md:289-293; DESIGN.md section 3.
+// kBlocks (hmlfc_decode_blocks): the segments are the 4 rows of arbitrary 4 x 4 blocks (u, v, bx, by) = blocks[g / 4] -- random access at
+// the granularity the paper decodes at ("As a block of pixels are decoded ...") -- written as [n][4][4][3].
+template <bool kBlocks>
 __global__ void __launch_bounds__(kNT)
 decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__ views, long long n_seg, uint8_t *__restrict__ out,
                    unsigned long long *__restrict__ oob, int out_aligned)
@@ -833,14 +836,25 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
     __syncthreads();
     const long long g = (long long)blockIdx.x * kNT + threadIdx.x;
     if (g >= n_seg) return;
-    const long long seg_per_view = (long long)S.nbx * S.Ht;
-    const long long view = g / seg_per_view;
-    const int seg = (int)(g - view * seg_per_view);
-    const int t = seg / S.nbx, bx = seg - t * S.nbx, s0 = bx << 2;
-    const int2 uv = __ldg(views + view);
-    const int u = uv.x, v = uv.y, h = S.h;
+    long long view = 0;
+    int t, bx, u, v;
+    bool in_range;
+    if (kBlocks) {
+        const int4 q = __ldg(reinterpret_cast<const int4 *>(views) + (g >> 2));
+        u = q.x; v = q.y; bx = q.z; t = (q.w << 2) + (int)(g & 3);
+        in_range = (unsigned)u < (unsigned)S.U && (unsigned)v < (unsigned)S.V && (unsigned)q.z < (unsigned)S.nbx && (unsigned)q.w < (unsigned)S.nby;
+    } else {
+        const long long seg_per_view = (long long)S.nbx * S.Ht;
+        view = g / seg_per_view;
+        const int seg = (int)(g - view * seg_per_view);
+        t = seg / S.nbx; bx = seg - t * S.nbx;
+        const int2 uv = __ldg(views + view);
+        u = uv.x; v = uv.y;
+        in_range = (unsigned)u < (unsigned)S.U && (unsigned)v < (unsigned)S.V;
+    }
+    const int s0 = bx << 2, h = S.h;
     uint32_t rgb[4] = {0u, 0u, 0u, 0u};
-    if ((unsigned)u < (unsigned)S.U && (unsigned)v < (unsigned)S.V) {
+    if (in_range) {
         int a[3][4];
         {
             const short4 *r = S.rkv + ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)t) * (size_t)S.Ws + (size_t)s0;
@@ -909,7 +923,7 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
     } else {
         atomicAdd(oob, 4ull);
     }
-    uint8_t *o = out + 3 * (((size_t)view * (size_t)S.Ht + (size_t)t) * (size_t)S.Ws + (size_t)s0);
+    uint8_t *o = kBlocks ? out + 12 * (size_t)g : out + 3 * (((size_t)view * (size_t)S.Ht + (size_t)t) * (size_t)S.Ws + (size_t)s0);
     if (out_aligned) {
         uint32_t *o32 = reinterpret_cast<uint32_t *>(o);
         o32[0] = rgb[0] | (rgb[1] << 24);
@@ -936,7 +950,21 @@ cudaError_t launch_decode_rows(const DevStream &S, const int32_t *d_views, int64
     const long long blocks = (n_seg + kNT - 1) / kNT;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_rows_kernel<<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    decode_rows_kernel<false><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, unsigned long long *d_oob,
+                                     cudaStream_t st, int *n_launches)
+{
+    if (n_blocks == 0) return cudaSuccess;
+    if (S.B != 4) return cudaErrorInvalidValue;
+    const long long n_seg = (long long)n_blocks * 4;
+    const long long blocks = (n_seg + kNT - 1) / kNT;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
+    decode_rows_kernel<true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

@@ -114,6 +114,31 @@ def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
     assert P.hmlfc_last_oob_count(h) - before == cfg.Ws * cfg.Ht
 
 
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8", "mini_h8"])
+def test_decode_blocks_random_access_at_block_granularity(P, enc, name):
+    # hmlfc_decode_blocks: whole B x B blocks at seeded random (u, v, bx, by), ragged counts; = the oracle's decode of their pixels
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    B = cfg.block
+    rng = np.random.default_rng(17)
+    for n in (0, 1, 63, 64, 65, 5003):
+        blocks = np.stack([rng.integers(0, cfg.U, n), rng.integers(0, cfg.V, n), rng.integers(0, cfg.Ws // B, n),
+                           rng.integers(0, cfg.Ht // B, n)], axis=1).astype(np.int32)
+        jj, ii = np.meshgrid(np.arange(B), np.arange(B), indexing="ij")
+        coords = np.stack([np.repeat(blocks[:, 0], B * B), np.repeat(blocks[:, 1], B * B),
+                           (blocks[:, 2:3] * B + ii.ravel()[None]).ravel(), (blocks[:, 3:4] * B + jj.ravel()[None]).ravel()], axis=1).astype(np.int32)
+        expect = s.decode(coords).reshape(n, B, B, 3)
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE):
+            P.hmlfc_set_decode_variant(h, variant)
+            assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy(), expect), (name, n, variant)
+    P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
+    before = P.hmlfc_last_oob_count(h)
+    bad = np.array([[0, 0, cfg.Ws // B, 0], [0, cfg.V, 0, 0], [1, 1, 1, 1]], dtype=np.int32)
+    got = P.hmlfc_decode_blocks(h, _dev(bad)).cpu().numpy()
+    assert not got[0].any() and not got[1].any() and np.array_equal(got[2], info["p1"][1, 1, B:2 * B, B:2 * B])
+    assert P.hmlfc_last_oob_count(h) - before == 2 * B * B
+
+
 def test_decode_host_entry_point(P, enc):
     cfg, lf, data, info, s = enc("mini4")
     h = _loaded(P, enc, "mini4")
