@@ -266,6 +266,12 @@ def test_randomised_shapes_and_parameters(P):
         for variant in (P.DECODE_THREAD, P.DECODE_QUEUE):
             P.hmlfc_set_decode_variant(hd, variant)
             assert np.array_equal(P.hmlfc_decode(hd, torch.from_numpy(coords).cuda()).cpu().numpy(), expect), tag
+        blocks = np.stack([a.ravel() for a in np.meshgrid(np.arange(U), np.arange(V), np.arange(Ws // B), np.arange(Ht // B), indexing="ij")], 1).astype(np.int32)
+        blocks = blocks[rng.permutation(len(blocks))]
+        bexp = np.stack([full[b[1], b[0], b[3] * B:(b[3] + 1) * B, b[2] * B:(b[2] + 1) * B] for b in blocks])
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE):
+            P.hmlfc_set_decode_variant(hd, variant)
+            assert np.array_equal(P.hmlfc_decode_blocks(hd, torch.from_numpy(blocks).cuda()).cpu().numpy(), bexp), tag
         P.hmlfc_set_decode_variant(hd, P.DECODE_AUTO)
         cam = np.zeros((1, 16), dtype=np.float32)
         ex, ey = float(rng.uniform(0, max(U - 1, 0))), float(rng.uniform(0, max(V - 1, 0)))
