@@ -872,7 +872,7 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
             const uint32_t pc0 = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
             const uint32_t refpc0 = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
             const bool predictive = ((pu | pv) & 1) != 0;
-#pragma unroll 1
+#pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const uint4 d = ldg(S.pc + pc0 + c);
                 const uint4 fr = ldg(S.flagrec + d.x + 4u * g32);
