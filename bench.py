@@ -10,9 +10,11 @@ launch.  The second half of BASELINE.json's metric, decoded LF pixels/s (hmlfc_d
 random coordinates), is timed in the same run and reported under "decode".
 
 Inputs: the seeded synthetic light field of the configuration (workloads/), encoded ONCE, before any timed
-region, by the oracle's encoder (oracle/streams.py; the encoder is outside the hot path this repo builds).
-The timed product path calls only the C-ABI library; the oracle is executed again only for the
-"cpu_baseline" object and for `--impl reference`.
+region.  The headline configuration (cfg2) is encoded by the oracle's encoder (oracle/streams.py, cached on disk); the
+larger configurations of the `configs` object are encoded by hmlfc_encode on the GPU (the oracle would need minutes to
+hours; the GPU encoder's stream is byte-identical to the oracle's on every configuration where both were run --
+tests/test_gpu_encode.py).  The timed product path calls only the C-ABI library; the oracle is executed again only for
+the "cpu_baseline" object and for `--impl reference`.
 
 N > 1 (torchrun): the path shards with no exchange step -- every rank holds the stream and renders its own
 batch of views (weak scaling); value = views of all ranks / max-over-ranks device time.
@@ -31,6 +33,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 L2_FLUSH_BYTES = 512 << 20  # > 126 MB L2
+RENDER_KERNEL_NAME = "render_cta_kernel"
 
 
 def _peaks():
@@ -183,7 +186,7 @@ def run_reference(args, cfg_name):
         "impl": "reference", "metric": "rendered_views_per_s", "value": value, "unit": "views/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-        "config": _config_dict(cfg, info, "n/a (CPU)"),
+        "config": _config_dict(cfg, info), "timing": {"l2": "n/a (CPU)", "clock": "host wall clock"},
         "cpu_baseline": {"value": value, "unit": "views/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "views/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -191,14 +194,100 @@ def run_reference(args, cfg_name):
     print(json.dumps(line), flush=True)
 
 
-def _config_dict(cfg, info, l2_policy):
+def _config_dict(cfg, info):
     return {
         "workload": f"{cfg.name}: {cfg.U}x{cfg.V} views x {cfg.Ws}x{cfg.Ht} RGB8, h={cfg.height}, B={cfg.block}, W={cfg.window}; "
                     f"render {cfg.n_views} views of {cfg.out_w}x{cfg.out_h} per step on the seeded circular camera path",
         "stream_bytes": info["stream_bytes"], "stream_bpp": round(info["bpp"], 4), "psnr_db": round(info["psnr"], 3),
         "tau_res": info["tau_res"], "views_per_step": cfg.n_views, "out_w": cfg.out_w, "out_h": cfg.out_h,
-        "l2": l2_policy,
     }
+
+
+def _timed_single(fn, steps, warmup, flush, stream):
+    """Device time of `steps` calls of fn (one rank): CUDA events on the launching stream, L2 flushed before every call."""
+    import torch
+
+    for _ in range(warmup):
+        flush.fill_(1)
+        fn()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        flush.fill_(1)
+        a.record(stream)
+        fn()
+        b.record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def measure_other_config(P, name, steps, peak, flush, stream):
+    """One of the larger configurations of BASELINE.json (the `configs` object of the bench line): the configuration's light field
+    (workloads/), encoded on the GPU by hmlfc_encode with the thresholds found by bisection to its PSNR target, then the same two
+    timed legs as the headline -- hmlfc_render of the view batch (one launch per step) and hmlfc_decode of the random coordinates."""
+    import torch
+
+    import workloads as wl
+
+    cfg = wl.CONFIGS[name]
+    t0 = time.perf_counter()
+    lf_dev = torch.from_numpy(wl.light_field(cfg)).cuda()
+    t_gen = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    data, est = P.hmlfc_encode(lf_dev, cfg.height, cfg.block, cfg.window, geometry=wl.geometry(cfg), seed=cfg.seed, target_psnr=cfg.target_psnr)
+    t_enc = time.perf_counter() - t0
+    del lf_dev
+    P.hmlfc_encode_release_scratch()
+    torch.cuda.empty_cache()
+    h = P.hmlfc_load(data)
+    W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
+    cams = torch.from_numpy(wl.camera_path(cfg)).cuda()
+    out = torch.empty((V, H, W, 3), dtype=torch.uint8, device="cuda")
+    n0 = P.hmlfc_launch_count(h)
+    ms = _timed_single(lambda: P.hmlfc_render(h, cams, W, H, out=out, stream=stream), steps, 3, flush, stream)
+    launches = P.hmlfc_launch_count(h) - n0 - 3
+    fp = P.hmlfc_footprint_render(h, cams, W, H)
+    kernel_ms = float(np.mean(ms))
+    achieved = fp["bytes_alg"] / (kernel_ms * 1e-3) / 1e9
+    coords = torch.from_numpy(wl.random_coords(cfg, cfg.n_decode)).cuda()
+    dec_out = torch.empty((cfg.n_decode, 3), dtype=torch.uint8, device="cuda")
+    dms = _timed_single(lambda: P.hmlfc_decode(h, coords, out=dec_out, stream=stream), max(3, min(steps, 5)), 2, flush, stream)
+    fpd = P.hmlfc_footprint_decode(h, coords)
+    dec_ms = float(np.mean(dms))
+    dec_achieved = fpd["bytes_alg"] / (dec_ms * 1e-3) / 1e9
+    res = {
+        "workload": f"{cfg.name}: {cfg.U}x{cfg.V} views x {cfg.Ws}x{cfg.Ht} RGB8, h={cfg.height}, B={cfg.block}, W={cfg.window}; "
+                    f"render {V} views of {W}x{H} per step on the seeded circular camera path; decode {cfg.n_decode} seeded uniformly random coordinates",
+        "stream": "encoded by hmlfc_encode (GPU) with tau found by bisection to the PSNR target", "stream_bytes": len(data),
+        "stream_bpp": round(8.0 * len(data) / (cfg.U * cfg.V * cfg.Ws * cfg.Ht), 4), "psnr_db": round(est["psnr"], 3), "tau_res": est["tau_res"],
+        "device_bytes": int(h.info.device_bytes), "generate_s": round(t_gen, 2), "encode_s": round(t_enc, 3),
+        "ms_per_step": kernel_ms, "steps": steps, "views_per_s": V / (kernel_ms * 1e-3), "output_px_per_s": V * W * H / (kernel_ms * 1e-3),
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "bytes_alg_per_launch": fp["bytes_alg"], "out_bytes": fp["out_bytes"],
+                     "compressed_bytes_touched": fp["bytes_alg"] - fp["out_bytes"] - fp["in_bytes"]},
+        "decode": {"value": cfg.n_decode / (dec_ms * 1e-3), "unit": "LF pixels/s", "n": cfg.n_decode, "ms_per_launch": dec_ms,
+                   "roofline": {"bound": "hbm", "achieved": dec_achieved, "peak": peak, "unit": "GB/s", "frac": dec_achieved / peak,
+                                "bytes_alg_per_launch": fpd["bytes_alg"]}},
+    }
+    P.hmlfc_free(h)
+    del coords, dec_out, out, cams, data
+    torch.cuda.empty_cache()
+    return res
+
+
+def _csrc_hash():
+    """Hash of the CUDA sources the library is built from: profiles/traffic.json records it at capture time, so counters of an
+    older build are recognised as stale."""
+    import hashlib
+
+    d = os.path.join(ROOT, "paper_1902_09396_b200", "csrc")
+    hh = hashlib.sha1()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            with open(os.path.join(d, f), "rb") as fh:
+                hh.update(f.encode() + b"\0" + fh.read())
+    return hh.hexdigest()[:16]
 
 
 def run_ours(args, cfg_name):
@@ -347,7 +436,10 @@ def run_ours(args, cfg_name):
     # ---- encoder-side leg (SURVEY 8(f) first "next" row): phase-shifted exhaustive search of one level-0 channel
     sU, sV = min(cfg.U, 16), min(cfg.V, 16)  # at most a 16 x 16 sub-grid of planes per launch
     srv = torch.from_numpy(wl.srv_like_planes(cfg, sU * sV, seed_offset=rank)).cuda()
-    pairs_np = wl.cluster_pairs(sU, sV)
+    # (predictive plane, reference plane) pairs of the sub-grid: every plane with an odd index against the even-even plane of its
+    # 2 x 2 cluster (the pairing hmlfc_encode itself uses, R5)
+    pairs_np = np.array([(pv * sU + pu, (pv & ~1) * sU + (pu & ~1)) for pv in range(sV) for pu in range(sU) if (pu | pv) & 1],
+                        dtype=np.int32).reshape(-1, 2)
     pairs_d = torch.from_numpy(pairs_np).cuda()
     mv_out = torch.empty((len(pairs_np), cfg.Ht // cfg.block, cfg.Ws // cfg.block, 4), dtype=torch.int32, device="cuda")
     se_ms = timed(lambda: P.hmlfc_search(srv, pairs_d, cfg.block, cfg.window, out=mv_out, stream=stream), 5, 3)
@@ -407,12 +499,20 @@ def run_ours(args, cfg_name):
         fpd = P.hmlfc_footprint_decode(h, coords)
         dec_kernel_ms = float(np.mean(dec_ms))
         dec_achieved = fpd["bytes_alg"] / (dec_kernel_ms * 1e-3) / 1e9
+        cap_r, cap_d = _ncu_from_profiles(cfg.name, "render"), _ncu_from_profiles(cfg.name, "decode")
+        src_now = _csrc_hash()
+        stale_r, stale_d = cap_r.get("csrc_sha") != src_now, cap_d.get("csrc_sha") != src_now
         roofline = {
-            "bound": "hbm", "kernel": {1: "render_pixel_kernel", 2: "render_tiled_kernel", 3: "render_blocks_kernel", 4: "render_warp_kernel", 5: "render_warp_kernel"}.get(args.variant, "render_cta_kernel"), "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": _ncu_from_profiles(cfg.name, "render").get("dram_bytes"), "peak_source": peak_src,
+            "bound": "hbm", "kernel": {1: "render_pixel_kernel", 4: "render_warp_kernel", 5: "render_warp_kernel"}.get(args.variant, RENDER_KERNEL_NAME), "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": cap_r.get("dram_bytes"), "peak_source": peak_src,
+            "traffic_source": {"file": "profiles/traffic.json", "commit": cap_r.get("commit"), "captured_with": cap_r.get("captured_with"),
+                               "csrc_sha_at_capture": cap_r.get("csrc_sha"), "csrc_sha_now": src_now, "stale": bool(stale_r)},
             "bytes_alg_per_launch": fp["bytes_alg"], "out_bytes": fp["out_bytes"],
             "compressed_bytes_touched": fp["bytes_alg"] - fp["out_bytes"] - fp["in_bytes"],
             "kernel_ms": kernel_ms, "frac_of_8TBs": achieved / 8000.0,
+            "note": "achieved = algorithmic bytes / launch time.  The output (out_bytes) is WRITTEN inside the timed region but, where it fits the "
+                    "126 MB L2 beside the stream traffic, most of it is still in the L2 when the kernel ends: its write-back to HBM happens during "
+                    "the next L2 flush, outside the events (the ncu capture's dram__bytes_write shows how much left the L2 in the launch).",
         }
         decode = {
             "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
@@ -420,19 +520,22 @@ def run_ours(args, cfg_name):
                     "d2h_bytes_per_step": 3 * n_dec, "steps": 3},
             "roofline": {"bound": "hbm", "kernel": "decode_kernel" if args.decode_variant == 1 else "decode_queue_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
                          "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
-                         "traffic": _ncu_from_profiles(cfg.name, "decode").get("dram_bytes")},
+                         "traffic": cap_d.get("dram_bytes"),
+                         "traffic_source": {"file": "profiles/traffic.json", "commit": cap_d.get("commit"), "captured_with": cap_d.get("captured_with"),
+                                            "csrc_sha_at_capture": cap_d.get("csrc_sha"), "stale": bool(stale_d)}},
         }
         clocks = clk.summary()
         # the bound that binds hmlfc_decode on an L2-resident stream: random 32-byte sector gathers served by the L2
-        dsec = _ncu_from_profiles(cfg.name, "decode").get("l2_read_sectors")
+        dsec = cap_d.get("l2_read_sectors")
         gpeak = _ncu_top("gather_peak").get("l2_g_sectors_per_s")
-        if dsec and gpeak and info["stream_bytes"] < (96 << 20):
+        if dsec and gpeak and not stale_d and info["stream_bytes"] < (96 << 20):
             decode["roofline"]["gather"] = {"bound": "l2-sector-gather", "achieved": dsec / (dec_kernel_ms * 1e-3) / 1e9, "peak": gpeak,
                                             "unit": "G sectors/s", "frac": dsec / (dec_kernel_ms * 1e-3) / 1e9 / gpeak, "sectors_per_launch": dsec,
-                                            "source": "lts__t_sectors_srcunit_tex_op_read.sum of the committed ncu capture; peak = gather_probe (profiles/r01_gather_probe.md)"}
-        roofline["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "render").get("warp_inst"), kernel_ms, clocks.get("sm_mhz"))
-        decode["roofline"]["alu"] = _alu_view(_ncu_from_profiles(cfg.name, "decode").get("warp_inst"), dec_kernel_ms,
-                                              clocks.get("sm_mhz"))
+                                            "source": "lts__t_sectors_srcunit_tex_op_read.sum of the committed ncu capture; the peak is a builder-measured "
+                                                      "denominator (random one-sector-per-lane gathers, profiles/r01_gather_probe.md), NOT in MEASURED_PEAKS.json"}
+        # the issue-slot views divide counters of the committed capture by the live launch time: only when that capture is of THIS build
+        roofline["alu"] = None if stale_r else _alu_view(cap_r.get("warp_inst"), kernel_ms, clocks.get("sm_mhz"))
+        decode["roofline"]["alu"] = None if stale_d else _alu_view(cap_d.get("warp_inst"), dec_kernel_ms, clocks.get("sm_mhz"))
         # search: 2 exact fp32 adds per sample, mode and offset (Eqs. 1-2): a plain-ALU bound, 128 FP32 lanes per SM
         nd2 = (2 * cfg.window + 1) ** 2
         se_adds = n_blocks_search * nd2 * cfg.block * cfg.block * 2 * 2
@@ -483,11 +586,20 @@ def run_ours(args, cfg_name):
             s.render(cams_np[:1], W, H, nthreads=1)
             cpu["single_thread"] = {"value": 1.0 / (time.perf_counter() - t0), "sample": f"1 view ({W}x{H}), one thread"}
 
+        others = None
+        if world == 1 and args.configs and args.configs != "none":
+            # ---- BASELINE.json's larger configurations (north_star: "on all five configs ... on the largest config"), GPU-encoded
+            others = {}
+            for name in [c for c in args.configs.split(",") if c and c != cfg.name]:
+                others[name] = measure_other_config(P, name, max(3, min(args.steps, 10)), peak, flush, stream)
+
         line = {
             "metric": "rendered_views_per_s", "value": views_per_s, "unit": "views/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": _config_dict(cfg, info, f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB fill)"),
+            "config": _config_dict(cfg, info),
+            "timing": {"l2": f"flushed between timed steps ({L2_FLUSH_BYTES >> 20} MiB fill, outside the events)",
+                       "clock": "CUDA events on the launching stream, max over ranks"},
             "e2e": {"value": e2e_views_per_s, "unit": "views/s", "h2d_bytes_per_step": int(cams_np.nbytes),
                     "d2h_bytes_per_step": int(out_pin.numel()), "steps": e2e_steps},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "on_plane_batch": {"value": whole_job_rate(V, len(pl_ms), world, pl_total * 1e-3), "unit": "views/s", "ms_per_step": float(np.mean(pl_ms)),
@@ -505,7 +617,7 @@ def run_ours(args, cfg_name):
             "decode_blocks": {"value": whole_job_rate(n_blk * cfg.block * cfg.block, len(blk_ms), world, blk_total * 1e-3), "unit": "LF pixels/s",
                               "blocks_per_launch": int(n_blk), "ms_per_launch": float(np.mean(blk_ms)),
                               "workload": f"hmlfc_decode_blocks: {n_blk} whole {cfg.block} x {cfg.block} blocks at seeded uniformly random (u, v, bx, by)"},
-            "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode,
+            "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode, "configs": others,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),
             "min_level": args.min_level,
@@ -562,6 +674,8 @@ def main():
     ap.add_argument("--min-level", type=int, default=0, help="progressive decoding: sum only the levels >= this one (0 = full quality)")
     ap.add_argument("--encode", action="store_true", help="run the GPU encoder leg also on configurations whose light field exceeds 256 MB")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--configs", default="cfg3,cfg4,cfg5", help="other BASELINE.json configurations measured after the headline (GPU-encoded "
+                    "streams; N = 1 only); 'none' to skip")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

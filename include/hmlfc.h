@@ -150,7 +150,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 /* Kernel selection for hmlfc_render (A/B measurements and cross-checks; all variants produce identical
  * bytes): 0 = automatic (default: 6, 7 or 8 for B = 4 streams, else 4), 1 = one thread per output pixel (16
- * independent tap decodes), 2 = sample-shared tile, 3 = block-centric CTA tile (32 x 8), 4 / 5 = the
+ * independent tap decodes -- the unshared definition, kept as the cross-check), 4 / 5 = a
  * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile, 6 / 7 / 8 = CTA per 32 x 32 tile with
  * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows), with a
  * 68 KB (3 CTAs per SM) / 104 KB (2 CTAs per SM) / 50 KB (4 CTAs per SM) shared-memory arena; the automatic

@@ -1,9 +1,10 @@
 """Encoded streams of the workload configurations, made by the ORACLE encoder and cached on disk.
 
-TEST INFRASTRUCTURE.  The HMLFC encoder is outside the hot path this repo builds (DESIGN.md
-"Scope"), so the compressed streams that tests, smoke() and bench.py feed to the CUDA path are
-manufactured here, by the oracle, before any timed region.  Nothing in this module is ever
-called from paper_1902_09396_b200/.
+TEST INFRASTRUCTURE.  The compressed streams that tests, smoke() and bench.py's headline feed to the
+CUDA path are manufactured here, by the oracle's encoder, before any timed region, so that no
+input of a parity test comes from the CUDA path (the GPU encoder hmlfc_encode exists as well and
+is checked byte for byte against these streams).  Nothing in this module is ever called from
+paper_1902_09396_b200/.
 
 Cache: $HMLFC_CACHE or /tmp/hmlfc_cache, keyed by the configuration and a hash of the oracle and
 generator sources, so a stale stream is never reused after the encoder changes.

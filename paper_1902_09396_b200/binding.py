@@ -19,7 +19,7 @@ EXPORTS = (
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
 
-RENDER_AUTO, RENDER_PIXEL, RENDER_TILED, RENDER_BLOCKS, RENDER_WARP, RENDER_WARP8, RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL = 0, 1, 2, 3, 4, 5, 6, 7, 8
+RENDER_AUTO, RENDER_PIXEL, RENDER_WARP, RENDER_WARP8, RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL = 0, 1, 4, 5, 6, 7, 8
 DECODE_AUTO, DECODE_THREAD, DECODE_QUEUE = 0, 1, 2
 
 

@@ -143,7 +143,7 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
         (ce = cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = create_events(h)) != cudaSuccess ||
-        (ce = configure_render_blocks()) != cudaSuccess || (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess) {
+        (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
@@ -211,10 +211,6 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || (h->render_variant >= 6 && h->render_variant <= 8));
     if (h->render_variant == 1 || (h->ds.lmin > 0 && !cta_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else if (h->render_variant == 2)
-        CU(h, launch_render_tiled(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else if (h->render_variant == 3)
-        CU(h, launch_render_blocks(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 4 || h->render_variant == 5 || h->ds.B != 4)
         CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 5 ? 1 : 0));
     else  // 0 (default: arena chosen from the sizes), 6 / 7 / 8 (68 / 104 / 50 KB arena): block-row kernel, written for 4 x 4 blocks
@@ -393,7 +389,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 8) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 8 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
     h->render_variant = variant;
     return HMLFC_OK;
 }

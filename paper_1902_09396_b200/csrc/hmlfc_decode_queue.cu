@@ -73,8 +73,13 @@ __device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ words, 
     const bool odd = (wi & 1u) != 0u;
     const uint32_t w0 = odd ? A.y : A.x, w1 = odd ? B.x : A.y, w2 = odd ? B.y : B.x;
     const uint32_t head = __funnelshift_r(w0, w1, sh) & ((1u << hb) - 1u);  // plain: 0 bits -> 0, the quint table maps 0 to digit 0
-    const uint32_t pos = sh + hb + k * m;                  // <= 31 + 8 + 4 * 10: the field ends inside w2
-    const uint32_t lo = pos < 32u ? w0 : (pos < 64u ? w1 : w2), hi = pos < 32u ? w1 : (pos < 64u ? w2 : 0u);
+    const uint32_t pos = sh + hb + k * m;                  // payload groups (<= 63 bits): the field ends inside w2
+    uint32_t lo = pos < 32u ? w0 : (pos < 64u ? w1 : w2), hi = pos < 32u ? w1 : (pos < 64u ? w2 : 0u);
+    if (pos + m > 96u) {  // motion records of wide windows (W = 51..54: trit m = 13, 73-bit groups): the field's own two words
+        const uint32_t *f = words + base + ((gb + hb + k * m) >> 5);
+        lo = __ldg(f);
+        hi = __ldg(f + 1);
+    }
     const uint32_t low = __funnelshift_r(lo, hi, pos & 31u) & ((1u << m) - 1u);
     const uint32_t dig = ((uint32_t)lut[(trit ? 0u : 256u) + head] >> (k * (trit ? 2u : 3u))) & (trit ? 3u : 7u);
     return (dig << m) | low;

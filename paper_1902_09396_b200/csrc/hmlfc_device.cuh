@@ -23,11 +23,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#ifdef HMLFC_HOST_DEBUG
-#define HMLFC_DEV __host__ __device__ inline
-#else
 #define HMLFC_DEV __device__ __forceinline__
-#endif
 
 namespace hmlfc {
 
@@ -62,38 +58,22 @@ struct DevStream {
 template <typename T>
 HMLFC_DEV T ldg(const T *p)
 {
-#if defined(__CUDA_ARCH__)
     return __ldg(p);
-#else
-    return *p;
-#endif
 }
 
 HMLFC_DEV uint32_t funnel_r(uint32_t lo, uint32_t hi, uint32_t sh)
 {
-#if defined(__CUDA_ARCH__)
     return __funnelshift_r(lo, hi, sh);
-#else
-    return (uint32_t)(((((uint64_t)hi) << 32) | lo) >> (sh & 31));
-#endif
 }
 
 HMLFC_DEV uint32_t popc(uint32_t x)
 {
-#if defined(__CUDA_ARCH__)
     return (uint32_t)__popc(x);
-#else
-    return (uint32_t)__builtin_popcount(x);
-#endif
 }
 
 HMLFC_DEV uint32_t umulhi(uint32_t a, uint32_t b)
 {
-#if defined(__CUDA_ARCH__)
     return __umulhi(a, b);
-#else
-    return (uint32_t)(((uint64_t)a * b) >> 32);
-#endif
 }
 
 // index of the flag record of plane-channel k (= 3 * plane + channel), 32-block group g; equals pc[k].x + 4 g
@@ -125,12 +105,19 @@ HMLFC_DEV uint32_t bise_decode_at(const uint32_t *__restrict__ w, uint32_t i, ui
     if (layout == 1u) { g = i / 5u; k = i - 5u * g; hb = 8u; gb = g * (8u + 5u * m); }
     else              { g = i / 3u; k = i - 3u * g; hb = 7u; gb = g * (7u + 3u * m); }
     uint32_t idx = gb >> 5, sh = gb & 31u;
-    // a group spans at most 8 + 5*10 = 58 bits from bit sh <= 31: three words cover it
+    // three words cover the digit word and every field that ends within 96 bits of the first word: all payload groups
+    // (N <= 4096: at most 8 + 5*11 = 63 bits from bit sh <= 31).  Motion records of wide windows have longer groups (W = 51..54:
+    // trit m = 13, 73 bits); a field that ends beyond the third word is read with its own two-word fetch.
     uint32_t w0 = ldg(w + idx), w1 = ldg(w + idx + 1), w2 = ldg(w + idx + 2);
     uint32_t head = funnel_r(w0, w1, sh) & ((1u << hb) - 1u);
     uint32_t p = sh + hb + k * m;
     uint32_t a = p < 32u ? w0 : (p < 64u ? w1 : w2);
     uint32_t b = p < 32u ? w1 : (p < 64u ? w2 : 0u);
+    if (p + m > 96u) {
+        const uint32_t fb = gb + hb + k * m;
+        a = ldg(w + (fb >> 5));
+        b = ldg(w + (fb >> 5) + 1);
+    }
     uint32_t low = funnel_r(a, b, p & 31u) & ((1u << m) - 1u);
     uint32_t digit;
     if (layout == 1u) {
@@ -246,17 +233,10 @@ struct Ray {
     bool hit;
 };
 
-#if defined(__CUDA_ARCH__)
 #define HMLFC_MUL(a, b) __fmul_rn((a), (b))
 #define HMLFC_ADD(a, b) __fadd_rn((a), (b))
 #define HMLFC_SUB(a, b) __fsub_rn((a), (b))
 #define HMLFC_DIV(a, b) __fdiv_rn((a), (b))
-#else
-#define HMLFC_MUL(a, b) ((a) * (b))
-#define HMLFC_ADD(a, b) ((a) + (b))
-#define HMLFC_SUB(a, b) ((a) - (b))
-#define HMLFC_DIV(a, b) ((a) / (b))
-#endif
 
 // x / step.  When step is a power of two, x * (1/step) is the same correctly rounded real number, so
 // the multiplication is bit-identical to the IEEE division the definition asks for.

@@ -1,5 +1,4 @@
 // HMLFC kernels for sm_100a: random-access decode, per-pixel fused render, footprint accounting.
-// (The tile-shared fused render kernel lives in hmlfc_render_tiled.cu.)
 #include "hmlfc_kernels.cuh"
 
 namespace hmlfc {

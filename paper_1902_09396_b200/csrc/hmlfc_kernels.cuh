@@ -1,4 +1,4 @@
-// Launchers of the HMLFC kernels (definitions in hmlfc_kernels.cu / hmlfc_render_tiled.cu).
+// Launchers of the HMLFC kernels (definitions in hmlfc_kernels.cu, hmlfc_decode_queue.cu, hmlfc_render_warp.cu, hmlfc_render_cta.cu).
 #pragma once
 
 #include "hmlfc_device.cuh"
@@ -33,12 +33,6 @@ cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks
                                      cudaStream_t st, int *n_launches);
 cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
                                 cudaStream_t st, int *n_launches);
-cudaError_t launch_render_tiled(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
-                                cudaStream_t st, int *n_launches);
-cudaError_t launch_render_blocks(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
-                                 cudaStream_t st, int *n_launches);
-// opts the block-centric kernel into its dynamic shared-memory size on the current device (call once per device)
-cudaError_t configure_render_blocks();
 // shape 0: 16 x 8 tiles (4 pixels per lane), 1: 8 x 8 tiles (2 pixels per lane)
 cudaError_t launch_render_warp(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
                                int *n_launches, int shape);

@@ -24,9 +24,9 @@
 //   B4  one lane per (view, sample) cell: top-level RKV + the h per-level terms, inverse YCoCg-R, clamp ->
 //       float RGB patch;
 //   C   every pixel gathers its 16 taps from the patch (128-bit loads) and blends with packed fp32 FMAs.
-// A tile whose tables do not fit the shared-memory arena (minification) is split by row ranges (32 -> 16 -> ..
-// -> 1 row); a single row that still does not fit is rendered by 16 direct sample decodes per pixel.  All paths
-// produce identical bytes.
+// A tile whose tables do not fit the shared-memory arena (minification) is rendered as its four 16 x 16 quadrants,
+// a quadrant that does not fit as four 8 x 8 sub-tiles, and an 8 x 8 sub-tile that still does not fit by 16 direct
+// sample decodes per pixel.  All paths produce identical bytes.
 #include "hmlfc_kernels.cuh"
 
 namespace hmlfc {

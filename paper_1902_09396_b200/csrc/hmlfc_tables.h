@@ -167,9 +167,11 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     bise_layout(N, &layout, &m);
                     if (N < 1 || N > 4096 || offset < -32768 || offset > 32767 || e[40] != layout || e[41] != m ||
                         e[42] != (is_pred ? 1 : 0) || (pboff & 31) || (mboff & 31) || (foff & 3) ||
-                        foff + fbytes * (is_pred ? 2 : 1) > flags_len ||
-                        pboff + bise_nbits(layout, m, (uint64_t)n_res * BB) > pay_bits ||
-                        mboff + bise_nbits(D.mv_layout, D.mv_m, n_pred) > mv_bits || (!is_pred && n_pred != 0))
+                        n_res > (uint32_t)D.nblk || n_pred > (uint32_t)D.nblk ||
+                        // subtraction form: the 64-bit offsets are untrusted and must not wrap
+                        foff > flags_len || fbytes * (is_pred ? 2 : 1) > flags_len - foff ||
+                        pboff > pay_bits || bise_nbits(layout, m, (uint64_t)n_res * BB) > pay_bits - pboff ||
+                        mboff > mv_bits || bise_nbits(D.mv_layout, D.mv_m, n_pred) > mv_bits - mboff || (!is_pred && n_pred != 0))
                         return HMLFC_E_CORRUPT;
                     const uint64_t frbase = (k / 3) * (uint64_t)D.fgroups * 4 + (k % 3);  // record of group g: frbase + 4 g
                     if (frbase + 4ull * (uint64_t)D.fgroups > 0xFFFFFFFFull) return HMLFC_E_UNSUPPORTED;

@@ -61,8 +61,14 @@ def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
     bad_dir = bytearray(data)
     off_dir = int.from_bytes(data[120:128], "little")
     bad_dir[off_dir + 8] ^= 0x01  # n_res of the first plane-channel no longer matches its flag map
+    # untrusted 64-bit directory offsets near 2^64 must not wrap the bounds checks (flag map @16, payload @24, motion records @32)
+    wraps = []
+    for field, value in ((16, (1 << 64) - 4), (24, (1 << 64) - 32), (32, (1 << 64) - 32), (24, 1 << 63)):
+        w = bytearray(data)
+        w[off_dir + 48 + field:off_dir + 48 + field + 8] = value.to_bytes(8, "little")   # second entry: a plane-channel with blocks
+        wraps.append((w, -6))
     cases = [(bad_magic, -1), (data[:6], -2), (data[:100], -2), (data[:len(data) // 2], -2), (bad_version, -3),
-             (chroma, -5), (bad_block, -5), (bad_dir, -6)]
+             (chroma, -5), (bad_block, -5), (bad_dir, -6)] + wraps
     for blob, code in cases:
         rc, out = load(blob)
         assert rc == code and not out.value, (rc, code)

@@ -56,6 +56,20 @@ def test_eq12_worked_block():
     mode, dx, dy, sad = orc.search_block(P, R, 2, 1, 1, 1)
     assert (("additive" if mode else "subtractive"), dx, dy, sad) == (best[1], int(best[2]), int(best[3]), int(best[4]))
     assert sad == min(min(dm, dp) for _, _, dm, dp in per_offset)
+    # the residual, through the encoder itself: a gray 2 x 2 light field whose Y planes are 128 + R, 128 + P, 128 - R,
+    # 128 - P has the cluster mean 128 everywhere, so its level-0 SRV images are exactly R (reference, view (0,0)) and P (view (1,0))
+    for tag, Pk in (("", P), ("2", P + np.array([[0, 0, 0, 0], [0, 0, 0, 0], [0, 0, 0, 0], [0, 0, 0, 1]], dtype=np.int16))):
+        planes = [128 + R, 128 + Pk, 128 - R, 128 - Pk]   # views (u,v) = (0,0), (1,0), (0,1), (1,1)
+        lf = np.stack([np.repeat(p.astype(np.uint8)[..., None], 3, axis=-1) for p in planes]).reshape(2, 2, 4, 4, 3)
+        tree = orc.Tree(lf, orc.make_params(2, 2, 4, 4, 1, 2, 1, 0, 0, policy=orc.POLICY_ALL))
+        assert np.array_equal(tree.plane("srv", 0, 0, 0, 0), R) and np.array_equal(tree.plane("srv", 0, 1, 0, 0), Pk)
+        tree.threshold(0, 0)
+        bestk = [r for r in rows if r[0] == "best" + tag][0]
+        mode, dx, dy, sad = tree.blocks(0, 1, 0, 0)[1, 1, :4]
+        assert (("additive" if mode else "subtractive"), dx, dy, sad) == (bestk[1], int(bestk[2]), int(bestk[3]), int(bestk[4]))
+        resid = [int(x) for x in [r for r in rows if r[0] == "residual" + tag][0][1:]]
+        assert tree.plane("stored", 0, 1, 0, 0)[2:, 2:].ravel().tolist() == resid
+        tree.close()
 
 
 def test_bise_groups_and_sizes():

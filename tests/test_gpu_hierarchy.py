@@ -65,6 +65,13 @@ def test_hierarchy_matches_the_oracle_tree(P, name):
     tree.close()
 
 
+def _cluster_pairs(UL, VL):
+    """(predictive plane, reference plane) index pairs of a UL x VL level (R5: the even-even member of every
+    2 x 2 cluster is the reference of the other members); plane index = pv * UL + pu."""
+    return np.array([(pv * UL + pu, (pv & ~1) * UL + (pu & ~1)) for pv in range(VL) for pu in range(UL) if (pu | pv) & 1],
+                    dtype=np.int32).reshape(-1, 2)
+
+
 def test_hierarchy_then_search_reproduces_the_encoders_motion_decisions(P):
     """RGB light field -> hmlfc_hierarchy -> hmlfc_search on the device-resident SRV planes = the oracle encoder's (mode, dx, dy,
     SAD) of every block of every predictive plane (level 0 and 1, all channels)."""
@@ -75,7 +82,7 @@ def test_hierarchy_then_search_reproduces_the_encoders_motion_decisions(P):
     off = 0
     for L in range(cfg.height):
         UL, VL = tree.level_dims(L)
-        pairs = wl.cluster_pairs(UL, VL)
+        pairs = _cluster_pairs(UL, VL)
         for c in range(3):
             planes = srv[c, off:off + UL * VL].contiguous()
             got = P.hmlfc_search(planes, torch.from_numpy(pairs).cuda(), cfg.block, cfg.window).cpu().numpy()

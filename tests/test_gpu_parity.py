@@ -47,7 +47,10 @@ def test_decode_cfg1_every_pixel_lossless(P, enc):
     assert np.array_equal(out.reshape(lf.shape), lf)  # zero-threshold round trip reproduces the input
 
 
-@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"])
+WIDE = ["mini_w25", "mini_w37", "mini_w51", "mini_w54"]   # motion-record groups of 63 / 68 / 73 / 73 bits (trit, m = 11 / 12 / 13)
+
+
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"] + WIDE)
 def test_decode_every_pixel_matches_oracle(P, enc, name):
     cfg, lf, data, info, s = enc(name)
     h = _loaded(P, enc, name)
@@ -90,7 +93,7 @@ def test_decode_out_of_range_is_black_and_counted(P, enc):
     P.hmlfc_free(h)
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b8", "mini_h8", "mini_w64"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_b8", "mini_h8", "mini_w64"] + WIDE)
 def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
     # hmlfc_decode_views: whole views, coordinates generated in the kernel; every view of the light field (shuffled order, one repeated)
     cfg, lf, data, info, s = enc(name)
@@ -114,7 +117,7 @@ def test_decode_views_equals_the_encoder_reconstruction(P, enc, name):
     assert P.hmlfc_last_oob_count(h) - before == cfg.Ws * cfg.Ht
 
 
-@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8", "mini_h8"])
+@pytest.mark.parametrize("name", ["cfg1_lossy", "mini2", "mini3", "mini4", "mini_b2", "mini_b8", "mini_h8"] + WIDE)
 def test_decode_blocks_random_access_at_block_granularity(P, enc, name):
     # hmlfc_decode_blocks: whole B x B blocks at seeded random (u, v, bx, by), ragged counts; = the oracle's decode of their pixels
     cfg, lf, data, info, s = enc(name)
@@ -150,7 +153,7 @@ def test_decode_host_entry_point(P, enc):
 def _check_views(P, h, s, cams, W, H):
     expect = s.render(cams, W, H)
     outs = {}
-    for variant in (P.RENDER_PIXEL, P.RENDER_TILED, P.RENDER_BLOCKS, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+    for variant in (P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
         P.hmlfc_set_render_variant(h, variant)
         got = P.hmlfc_render(h, _dev(cams), W, H).cpu().numpy()
         d = np.abs(got.astype(np.int16) - expect.astype(np.int16))
@@ -158,9 +161,7 @@ def _check_views(P, h, s, cams, W, H):
         assert (d > 0).mean() < 1e-3  # rounding-boundary cases only
         outs[variant] = got
     P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_TILED])  # the kernels agree byte for byte
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_BLOCKS])
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP])
+    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP])  # the kernels agree byte for byte
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP8])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA])
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA_BIG])
@@ -168,7 +169,7 @@ def _check_views(P, h, s, cams, W, H):
     return expect
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg1_lossy", "mini2", "mini3", "mini4", "mini_h8", "mini_w64"] + WIDE)
 def test_render_matches_oracle(P, enc, name):
     cfg, lf, data, info, s = enc(name)
     h = _loaded(P, enc, name)
@@ -347,18 +348,41 @@ def _full_configs():
     return ["cfg2", "cfg3"] + [c for c in ("cfg4", "cfg5") if c in extra]
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+
+
+@pytest.mark.parametrize("name", _full_configs())
 def test_full_size_sampled_parity(P, name):
-    """Full size, in the launch configuration bench.py times: the whole view batch in one launch and the
-    configuration's whole random-coordinate list in one launch; sampled views and 2*10^6 sampled coordinates
+    """Full size, in the launch configuration bench.py times, on the ORACLE encoder's stream: the whole view batch in one launch and
+    the configuration's whole random-coordinate list in one launch; sampled views and 2*10^6 sampled coordinates
     are compared with the oracle (views within 1 LSB, decoded pixels bit-exact), both decode kernels agree on
     every coordinate and all render kernels agree on every byte of the sampled views."""
-    if name not in _full_configs():
-        pytest.skip(f"{name}: set HMLFC_FULL={name} (oracle encode takes minutes)")
-    import oracle as orc
     from oracle import streams
 
     cfg, data, info = streams.get_stream(name)
+    _full_size_checks(P, cfg, data, info["psnr"])
+
+
+@pytest.mark.parametrize("name", ["cfg4", "cfg5"])
+def test_full_size_sampled_parity_gpu_stream(P, name):
+    """BASELINE.json configs[3] and [4] (805 MB and 5.03 GB of raw light field) at full size, always run: the oracle's ENCODER needs
+    minutes on these, its DECODER and RENDERER do not.  The light field comes from `workloads`, the stream from hmlfc_encode with the
+    thresholds found by bisection to the configuration's 40 dB (byte-identical to the oracle encoder's stream wherever both were run:
+    tests/test_gpu_encode.py, and at these sizes with HMLFC_FULL).  Every EXPECTED value still comes from oracle/ alone: the oracle's
+    parser accepts any valid stream, and its decode of the stream must also be a 40 dB reconstruction of the generator's light field
+    (checked below on sampled views), so a stream that was wrong in a way both decoders agree on would not pass either."""
+    cfg = wl.CONFIGS[name]
+    lf = wl.light_field(cfg)
+    data, stats = P.hmlfc_encode(torch.from_numpy(lf).cuda(), cfg.height, cfg.block, cfg.window, geometry=wl.geometry(cfg), seed=cfg.seed,
+                                 target_psnr=cfg.target_psnr)
+    P.hmlfc_encode_release_scratch()
+    torch.cuda.empty_cache()
+    _full_size_checks(P, cfg, data, stats["psnr"], lf=lf)
+
+
+def _full_size_checks(P, cfg, data, psnr, lf=None):
+    import oracle as orc
+
+    name = cfg.name
     s = orc.Stream(data)
     h = P.hmlfc_load(data)
     del data
@@ -393,7 +417,18 @@ def test_full_size_sampled_parity(P, name):
     assert np.array_equal(P.hmlfc_decode_host(h, rc[:n_host]), out[:n_host].cpu().numpy())
     assert P.hmlfc_last_oob_count(h) == 0
     target = cfg.target_psnr
-    assert target - 2.0 < info["psnr"] < target + 2.0  # "quantisation set for ~40 dB" (45 dB for cfg3)
+    assert target - 2.0 < psnr < target + 2.0  # "quantisation set for ~40 dB" (45 dB for cfg3)
+    # whole views through hmlfc_decode_views (block-row kernel) against the oracle's decode of the same views
+    rng = np.random.default_rng(cfg.seed)
+    views = np.stack([rng.integers(0, cfg.U, 3), rng.integers(0, cfg.V, 3)], axis=1).astype(np.int32)
+    dv = P.hmlfc_decode_views(h, _dev(views)).cpu().numpy()
+    t, x = np.meshgrid(np.arange(cfg.Ht), np.arange(cfg.Ws), indexing="ij")
+    for k, (u, v) in enumerate(views):
+        vc = np.stack([np.full(t.size, u), np.full(t.size, v), x.ravel(), t.ravel()], axis=1).astype(np.int32)
+        expect = s.decode(vc).reshape(cfg.Ht, cfg.Ws, 3)
+        assert np.array_equal(dv[k], expect), (name, u, v)
+        if lf is not None:   # the stream is a ~target dB coding of the generator's light field (sampled views: within 6 dB of the mean)
+            assert orc.psnr(expect, lf[v, u]) > target - 6.0, (name, u, v)
     P.hmlfc_free(h)
 
 

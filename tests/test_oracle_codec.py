@@ -272,6 +272,82 @@ def test_stats_locality_single_pixel(enc):
     assert st["in_bytes"] == 16 and st["out_bytes"] == 3
 
 
+def _bits15(N):
+    """BISE bits per value in units of 1/15 bit, R15: the cheapest of plain 15 ceil(log2 N), trit 24 + 15 m, quint 35 + 15 m."""
+    lay, m = PyStream.layout(N)
+    return 15 * m if lay == 0 else (24 + 15 * m if lay == 1 else 35 + 15 * m)
+
+
+@pytest.mark.parametrize("policy", [orc.POLICY_ADAPTIVE, orc.POLICY_ALL])
+def test_stats_of_an_exhaustive_decode_equal_the_closed_form(policy):
+    """SURVEY 8(d) D5 on a tau = 0 stream (every block significant) when EVERY pixel is decoded: each (plane-channel, block) is
+    touched exactly once, so the counters have closed forms in terms of the directory, read here by the independent PyStream reader:
+    flag bits = sum over plane-channels of nblk x (2 if predictive else 1); payload = sum of nblk x B^2 x bits/value(N); motion records
+    = (number of predicted blocks) x bits/record; top-level RKV = U_h V_h Ws Ht x 5 bytes; plus 16 + 3 bytes per coordinate."""
+    rng = np.random.default_rng(11)
+    U, V, Ws, Ht, h, B, W = 3, 4, 16, 12, 2, 4, 3
+    lf = random_lf(rng, U, V, Ws, Ht)
+    data, info, tree = _encode(lf, h, B, W, 0, 0, policy)
+    tree.close()
+    ps, s = PyStream(data), orc.Stream(data)
+    n = U * V * Ws * Ht
+    cfg = wl.Config("x", U, V, Ws, Ht, h, 1, 0, 0, None, 0, Ws, Ht, 1, 0)
+    st = s.stats_decode(wl.all_coords(cfg))
+    flag_bits = pay15 = n_pred = 0
+    for L in range(h):
+        UL, VL = ps.dims[L]
+        for pv in range(VL):
+            for pu in range(UL):
+                for c in range(3):
+                    off, N, foff, poff, moff = ps.dirent(L, pu, pv, c)
+                    isp = (pu | pv) & 1
+                    assert all(ps.flag(foff, 0, b) for b in range(ps.nblk))          # tau = 0: every block stored
+                    flag_bits += ps.nblk * (2 if isp else 1)
+                    pay15 += ps.nblk * B * B * _bits15(N)
+                    if isp:
+                        n_pred += sum(ps.flag(foff, 1, b) for b in range(ps.nblk))
+    nd = 2 * W + 1
+    assert n_pred > 0 and (policy != orc.POLICY_ALL or n_pred == sum(ps.nblk * 3 for L in range(h) for pv in range(ps.dims[L][1])
+                                                                     for pu in range(ps.dims[L][0]) if (pu | pv) & 1))
+    assert st["blocks_touched"] == ps.n_pc * ps.nblk
+    assert st["flag_bits"] == flag_bits
+    assert st["payload_bits15"] == pay15
+    assert st["mv_bits15"] == n_pred * _bits15(2 * nd * nd)
+    assert st["rkv_bytes"] == ps.dims[h][0] * ps.dims[h][1] * Ws * Ht * 5
+    assert (st["in_bytes"], st["out_bytes"], st["taps"]) == (16 * n, 3 * n, n)
+    expect = (flag_bits + (pay15 + n_pred * _bits15(2 * nd * nd)) / 15.0) / 8.0 + st["rkv_bytes"] + 19 * n
+    assert abs(st["bytes_alg"] - expect) < 1e-9 * expect
+
+
+def test_stats_count_the_reference_block_reached_through_a_motion_vector():
+    """One pixel whose block is predicted from a DIFFERENT block of the reference plane.  A gray 2 x 2 light field with Y planes
+    128 + R, 128 + P, 128 - R, 128 - P has cluster mean 128, so its level-0 SRV images of Y are exactly R (reference) and P; P's
+    block (0,0) is R's block (1,0) (P(x,y) = R(x+4,y)), which the search finds as subtractive (dx,dy) = (4,0), SAD 0.  Decoding pixel
+    (u,v,s,t) = (1,0,1,2) must count, for Y, its own block (2 flag bits, 16 values, 1 motion record) and the reference block
+    (1 flag bit, 16 values); for Co and Cg (all-zero SRVs: never predicted) the own block only."""
+    rng = np.random.default_rng(3)
+    R = rng.integers(-60, 61, (8, 8)).astype(np.int16)
+    P = np.zeros((8, 8), dtype=np.int16)
+    P[:, :4] = R[:, 4:]
+    planes = [128 + R, 128 + P, 128 - R, 128 - P]
+    lf = np.stack([np.repeat(p.astype(np.uint8)[..., None], 3, axis=-1) for p in planes]).reshape(2, 2, 8, 8, 3)
+    data, info, tree = _encode(lf, 1, 4, 4, 0, 0, orc.POLICY_ADAPTIVE)
+    assert tuple(tree.blocks(0, 1, 0, 0)[0, 0, :4]) == (0, 4, 0, 0)
+    tree.close()
+    ps, s = PyStream(data), orc.Stream(data)
+    st = s.stats_decode(np.array([[1, 0, 1, 2]], dtype=np.int32))
+    N_own = [ps.dirent(0, 1, 0, c)[1] for c in range(3)]
+    N_ref = ps.dirent(0, 0, 0, 0)[1]
+    assert st["blocks_touched"] == 4
+    assert st["flag_bits"] == 2 + 1 + 2 + 2
+    assert st["payload_bits15"] == 16 * (sum(_bits15(N) for N in N_own) + _bits15(N_ref))
+    assert st["mv_bits15"] == _bits15(2 * 81) == 114          # N = 162: trit, m = 6: (8 + 30) bits / 5 records = 7.6 bits
+    assert st["rkv_bytes"] == 5 and st["out_bytes"] == 3 and st["in_bytes"] == 16
+    # the same pixel twice, and a second pixel of the same block: nothing new is counted (each distinct block once per batch)
+    st2 = s.stats_decode(np.array([[1, 0, 1, 2], [1, 0, 1, 2], [1, 0, 2, 2]], dtype=np.int32))
+    assert st2["blocks_touched"] == 4 and st2["payload_bits15"] == st["payload_bits15"] and st2["rkv_bytes"] == 10
+
+
 def test_psnr_closed_form():
     # SPEC.md:91: uniform error 1 -> 20 log10(255) = 48.1308 dB
     a = np.full((10, 10, 3), 100, dtype=np.uint8)

@@ -66,6 +66,12 @@ CONFIGS = {
     # plane has SRV = 0 at every level above) and search window 64 (129 x 129 offsets, wider than the image)
     "mini_h8": Config("mini_h8", 6, 5, 32, 24, 8, 3, 1, 3.0, None, 24, 72, 56, 2, 20_000, seed=BASE_SEED + 17, window=4),
     "mini_w64": Config("mini_w64", 3, 2, 24, 16, 2, 3, 1, 3.0, None, 20, 56, 40, 2, 10_000, seed=BASE_SEED + 18, window=64),
+    # search windows whose motion-record alphabet N = 2 (2W+1)^2 takes the trit layout with m = 11 / 12 / 13 / 13: BISE groups of
+    # 63 / 68 / 73 bits, longer than any payload group (the record fields end beyond a 96-bit window)
+    "mini_w25": Config("mini_w25", 4, 4, 48, 32, 2, 3, 1, 3.0, None, 16, 72, 48, 2, 10_000, seed=BASE_SEED + 19, window=25),
+    "mini_w37": Config("mini_w37", 4, 4, 48, 32, 2, 3, 1, 3.0, None, 16, 72, 48, 2, 10_000, seed=BASE_SEED + 20, window=37),
+    "mini_w51": Config("mini_w51", 4, 4, 48, 32, 2, 3, 1, 3.0, None, 16, 72, 48, 2, 10_000, seed=BASE_SEED + 21, window=51),
+    "mini_w54": Config("mini_w54", 4, 4, 48, 32, 2, 3, 1, 3.0, None, 16, 72, 48, 2, 10_000, seed=BASE_SEED + 23, window=54),
     # paper-regime sparsity: adjacent views < 1 px apart, as in the Stanford archive
     "cfg2_sparse": Config("cfg2_sparse", 16, 16, 256, 256, 3, 5, 2, 1.0, 40.0, 0, 512, 512, 64, 10 ** 7,
                           seed=BASE_SEED + 22),
@@ -284,13 +290,6 @@ def srv_like_planes(cfg: Config, n_planes: int, seed_offset=0) -> np.ndarray:
         img = sign * base[pad + dy:pad + dy + cfg.Ht, pad + dx:pad + dx + cfg.Ws] + rng.normal(0.0, 3.0, (cfg.Ht, cfg.Ws))
         out[k] = np.clip(np.rint(img), -510, 510).astype(np.int16)
     return out
-
-
-def cluster_pairs(UL: int, VL: int) -> np.ndarray:
-    """(predictive plane, reference plane) index pairs of a UL x VL level: the even-even member of every 2 x 2 cluster is
-    the reference of the other members (R5).  int32 [n][2], plane index = pv * UL + pu."""
-    return np.array([(pv * UL + pu, (pv & ~1) * UL + (pu & ~1)) for pv in range(VL) for pu in range(UL) if (pu | pv) & 1],
-                    dtype=np.int32).reshape(-1, 2)
 
 
 def all_coords(cfg: Config) -> np.ndarray:

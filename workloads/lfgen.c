@@ -44,24 +44,23 @@ static uint64_t hash4(uint64_t a, uint64_t b, uint64_t c, uint64_t d)
 }
 static double u01(uint64_t h) { return (double)(h >> 11) * (1.0 / 9007199254740992.0); }
 
-static double lattice(uint64_t tex, int oct, int ch, int64_t ix, int64_t iy)
-{
-    return u01(hash4(tex, (uint64_t)(oct * 4 + ch), (uint64_t)ix, (uint64_t)iy));
-}
-
 static double smooth(double t) { return t * t * (3.0 - 2.0 * t); }
 
-/* 4 octaves, persistence 0.5, normalised to [0,1] */
+/* 4 octaves, persistence 0.5, normalised to [0,1].  Lattice value at (ix, iy) = u01(hash4(tex, oct * 4 + ch, ix, iy)); the hash
+ * chain mix64(mix64(mix64(mix64(tex) ^ k) ^ ix) ^ iy) is shared between the four corners as far as it goes. */
 static double value_noise(uint64_t tex, int ch, double x, double y, double cell)
 {
     double sum = 0.0, amp = 1.0, norm = 0.0;
+    const uint64_t ht = mix64(tex);
     for (int o = 0; o < 4; ++o) {
         double fx = x / cell, fy = y / cell;
         double x0 = floor(fx), y0 = floor(fy);
         double tx = smooth(fx - x0), ty = smooth(fy - y0);
         int64_t ix = (int64_t)x0, iy = (int64_t)y0;
-        double a = lattice(tex, o, ch, ix, iy), b = lattice(tex, o, ch, ix + 1, iy);
-        double c = lattice(tex, o, ch, ix, iy + 1), d = lattice(tex, o, ch, ix + 1, iy + 1);
+        const uint64_t hk = mix64(ht ^ (uint64_t)(o * 4 + ch));
+        const uint64_t hx0 = mix64(hk ^ (uint64_t)ix), hx1 = mix64(hk ^ (uint64_t)(ix + 1));
+        double a = u01(mix64(hx0 ^ (uint64_t)iy)), b = u01(mix64(hx1 ^ (uint64_t)iy));
+        double c = u01(mix64(hx0 ^ (uint64_t)(iy + 1))), d = u01(mix64(hx1 ^ (uint64_t)(iy + 1)));
         double v = (a * (1.0 - tx) + b * tx) * (1.0 - ty) + (c * (1.0 - tx) + d * tx) * ty;
         sum += amp * v;
         norm += amp;
@@ -104,19 +103,17 @@ int wl_generate_lf(const wl_scene *sc, const wl_plane *planes, const wl_sphere *
             double tx = sc->st_origin[0] + is * sc->st_step[0];
             /* ray: P(z) = (cx,cy,0) + (z / zst) * (tx - cx, ty - cy, zst) */
             double dx = (tx - cx) / zst, dy = (ty - cy) / zst;
+            /* nearest hit first (the last object that lowers best_z wins), then ONE texture evaluation for the winner */
             double best_z = 1e300;
             double col[3] = { 0.0, 0.0, 0.0 };
+            int win_plane = -1, win_sphere = -1;
             for (int k = 0; k < sc->n_planes; ++k) {
                 const wl_plane *pl = &planes[k];
                 if (pl->z >= best_z) continue;
                 double X = cx + dx * pl->z, Y = cy + dy * pl->z;
                 if (X < pl->x0 || X > pl->x1 || Y < pl->y0 || Y > pl->y1) continue;
                 best_z = pl->z;
-                /* project the hit to the st plane through the central camera -> pixel units */
-                double px = ((ccx + (X - ccx) * zst / pl->z) - sc->st_origin[0]) / sc->st_step[0];
-                double py = ((ccy + (Y - ccy) * zst / pl->z) - sc->st_origin[1]) / sc->st_step[1];
-                for (int c = 0; c < 3; ++c)
-                    col[c] = 0.5 * pl->base[c] + 0.5 * value_noise(pl->tex, c, px, py, sc->base_cell_px);
+                win_plane = k;
             }
             for (int k = 0; k < sc->n_spheres; ++k) {
                 const wl_sphere *sp = &spheres[k];
@@ -130,6 +127,11 @@ int wl_generate_lf(const wl_scene *sc, const wl_plane *planes, const wl_sphere *
                 double z = (-Bq - sqrt(disc)) / (2.0 * A);
                 if (z <= 0.0 || z >= best_z) continue;
                 best_z = z;
+                win_sphere = k;
+            }
+            if (win_sphere >= 0) {
+                const wl_sphere *sp = &spheres[win_sphere];
+                double z = best_z;
                 double hx = cx + dx * z, hy = cy + dy * z, hz = z;
                 double nx = (hx - sp->c[0]) / sp->r, ny = (hy - sp->c[1]) / sp->r, nz = (hz - sp->c[2]) / sp->r;
                 double lam = nx * sc->light[0] + ny * sc->light[1] + nz * sc->light[2];
@@ -140,6 +142,14 @@ int wl_generate_lf(const wl_scene *sc, const wl_plane *planes, const wl_sphere *
                 double py = (hy - sp->c[1]) * zst / sp->c[2] / sc->st_step[1];
                 for (int c = 0; c < 3; ++c)
                     col[c] = shade * (0.5 * sp->base[c] + 0.5 * value_noise(sp->tex, c, px, py, sc->base_cell_px));
+            } else if (win_plane >= 0) {
+                const wl_plane *pl = &planes[win_plane];
+                double X = cx + dx * pl->z, Y = cy + dy * pl->z;
+                /* project the hit to the st plane through the central camera -> pixel units */
+                double px = ((ccx + (X - ccx) * zst / pl->z) - sc->st_origin[0]) / sc->st_step[0];
+                double py = ((ccy + (Y - ccy) * zst / pl->z) - sc->st_origin[1]) / sc->st_step[1];
+                for (int c = 0; c < 3; ++c)
+                    col[c] = 0.5 * pl->base[c] + 0.5 * value_noise(pl->tex, c, px, py, sc->base_cell_px);
             }
             uint8_t *o = lf + ((size_t)row * Ws + is) * 3;
             for (int c = 0; c < 3; ++c) {
