@@ -47,10 +47,15 @@ constexpr uint32_t kNone = 0xFFFFFFFFu;
 
 // debug builds (-DHMLFC_PASS_STATS) count the passes of every size and why a pass was split
 #ifdef HMLFC_PASS_STATS
-__device__ unsigned long long g_pass_stats[16];  // [0..2] passes tried at 32/16/8, [3..5] passes done, [6] direct pixels passes, [8..] fail reasons
+__device__ unsigned long long g_pass_stats[64];  // [0..2] passes tried at 32/16/8, [3..5] passes done, [6] direct pixels passes, [8..] fail reasons, [16..] cycles of thread 0 per phase
+__device__ long long g_phase_last[1 << 20];      // per CTA: clock of the previous mark
 #define PASS_STAT(i) do { if (threadIdx.x == 0) atomicAdd(&g_pass_stats[i], 1ull); } while (0)
+#define PHASE_MARK(i) do { if (threadIdx.x == 0) { const unsigned cta_ = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x; \
+        const long long now_ = clock64(); if ((i) >= 0) atomicAdd(&g_pass_stats[16 + ((i) < 0 ? 0 : (i))], (unsigned long long)(now_ - g_phase_last[cta_ & ((1u << 20) - 1u)])); \
+        g_phase_last[cta_ & ((1u << 20) - 1u)] = now_; } } while (0)
 #else
 #define PASS_STAT(i) do { } while (0)
+#define PHASE_MARK(i) do { } while (0)
 #endif
 
 
@@ -385,6 +390,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         for (int q = tid - 32; q < kSpecZero; q += kNT - 32) z[q] = make_uint4(0u, 0u, 0u, 0u);
     }
     __syncthreads();
+    PHASE_MARK(4);
     if (!ctl.fits) { PASS_STAT(10); return false; }
 
     const int nviews = ctl.nviews, ncell = ctl.ncell, nacc = ctl.nacc, nitems = ctl.nitems, reccap = ctl.reccap;
@@ -475,6 +481,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         }
     }
     __syncthreads();
+    PHASE_MARK(5);
     if (ctl.overflow != 0) { PASS_STAT(11); return false; }
     const int nrec = ctl.n_rec;
     // ------------------------------------------------ B2: motion record + reference descriptor, once per block
@@ -493,6 +500,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         }
     }
     __syncthreads();
+    PHASE_MARK(6);
     // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values
     int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
     for (int t = tid; t < 4 * nrec; t += kNT) {
@@ -546,6 +554,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
     }
     __syncthreads();
+    PHASE_MARK(7);
     // ------------------------------------------------ B4: top-level RKV + per-level terms -> float RGB patch
     for (int q = tid; q < ncell; q += kNT) {
         const int vw = ctl.chunkvw[q >> 5];
@@ -568,6 +577,7 @@ __device__ HMLFC_BP_ATTR bool build_patch(const DevStream &S, Ctl &ctl, unsigned
         patch[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
     }
     __syncthreads();
+    PHASE_MARK(8);
     return true;
 }
 
@@ -624,6 +634,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     if (tid < 4) { ctl.lo[tid] = 0x7fffffff; ctl.hi[tid] = -1; }
     if (tid == 0) { ctl.n_rec = 0; ctl.overflow = 0; ctl.fits = 0; }
     __syncthreads();
+    PHASE_MARK(1);
 
     // ------------------------------------------------------------ lane summary: common (u0, v0, du, dv) key and (s,t) box of the lane's pixels
     uint32_t key = kNone;
@@ -651,6 +662,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
         atomicMax(&ctl.hi[0], uhi); atomicMax(&ctl.hi[1], vhi); atomicMax(&ctl.hi[2], ws1); atomicMax(&ctl.hi[3], wt1);
     }
     __syncthreads();
+    PHASE_MARK(2);
     const int bu0 = ctl.lo[0], bv0 = ctl.lo[1];
     const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
     if (ctl.hi[0] < 0) return true;  // no ray of the sub-tile hits the slab: background only
@@ -700,6 +712,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
         }
     }
     __syncthreads();
+    PHASE_MARK(3);
 
     if (!build_patch<kArenaBytes>(S, ctl, arena)) return false;
 
@@ -722,6 +735,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
             }
             rgb[p] = blend16(pt[p], [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
         }
+    PHASE_MARK(9);
     return true;
 }
 
@@ -795,7 +809,9 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
             uint32_t rgb[kPPL];
 #pragma unroll
             for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
+            PHASE_MARK(-1);
             setup_rays(S, cam, W, H, sx, sy, ts, pt);
+            PHASE_MARK(0);
             PASS_STAT(ts == kTile ? 0 : ts == 16 ? 1 : 2);
             done = tile_pass<kArenaBytes>(S, ctl, arena, pt, rgb);
             if (done) PASS_STAT(ts == kTile ? 3 : ts == 16 ? 4 : 5);
@@ -809,6 +825,7 @@ render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict_
                 thread_pixel(sx, sy, ts, x0, y, npix);
                 if (q < 0) store4(out, view, W, H, x0, y, rgb, out_aligned);
                 else store1(out, view, W, H, x0, y, npix > 0, rgb[0], out_aligned);
+                PHASE_MARK(10);
             }
         }
         if (q < 0) q = done ? 4 : 0;
@@ -974,7 +991,7 @@ extern "C" int hmlfc_debug_pass_stats(unsigned long long *out, int reset)
 {
     cudaDeviceSynchronize();
     cudaMemcpyFromSymbol(out, g_pass_stats, sizeof(g_pass_stats));
-    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(g_pass_stats, z, sizeof(z)); }
+    if (reset) { unsigned long long z[64] = {}; cudaMemcpyToSymbol(g_pass_stats, z, sizeof(z)); }
     return 0;
 }
 #endif
