@@ -208,7 +208,7 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     const Camera *cams = reinterpret_cast<const Camera *>(d_cameras);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the CTA kernel
-    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || (h->render_variant >= 6 && h->render_variant <= 8));
+    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || (h->render_variant >= 6 && h->render_variant <= 10));
     if (h->render_variant == 1 || (h->ds.lmin > 0 && !cta_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (h->render_variant == 4 || h->render_variant == 5 || h->ds.B != 4)
@@ -389,7 +389,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 8 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
+    if (!h || variant < 0 || variant > 10 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
     h->render_variant = variant;
     return HMLFC_OK;
 }
