@@ -13,6 +13,10 @@
 
 using namespace hmlfc;
 
+#ifndef HMLFC_TILES_DEFAULT
+#define HMLFC_TILES_DEFAULT 0
+#endif
+
 struct hmlfc_handle {
     DevStream ds{};
     hmlfc_info_t info{};
@@ -43,6 +47,42 @@ struct hmlfc_handle {
     mutable std::atomic<long long> launches{0};
     mutable std::atomic<int> last_cuda_error{0};
 };
+
+namespace hmlfc {
+
+static cudaMemPool_t g_pool[64] = {};
+
+cudaError_t scratch_pool(cudaMemPool_t *out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!g_pool[dev]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if ((e = cudaMemPoolCreate(&g_pool[dev], &props)) != cudaSuccess) return e;
+        uint64_t keep = ~0ull;  // keep freed scratch for the next call (hmlfc_encode_release_scratch returns it)
+        if ((e = cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
+    }
+    *out = g_pool[dev];
+    return cudaSuccess;
+}
+
+cudaError_t scratch_pool_trim()
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!g_pool[dev]) return cudaSuccess;
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return e;
+    return cudaMemPoolTrimTo(g_pool[dev], 0);
+}
+
+}  // namespace hmlfc
 
 namespace {
 
@@ -143,7 +183,8 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
         (ce = cudaStreamCreateWithFlags(&h->in_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = create_events(h)) != cudaSuccess ||
-        (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess) {
+        (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess ||
+        (ce = configure_render_tiles()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
@@ -207,14 +248,31 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     int nl = 0;
     const Camera *cams = reinterpret_cast<const Camera *>(d_cameras);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the CTA kernel
-    const bool cta_ok = h->ds.B == 4 && (h->render_variant == 0 || (h->render_variant >= 6 && h->render_variant <= 10));
-    if (h->render_variant == 1 || (h->ds.lmin > 0 && !cta_ok))
+    // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the two fused kernels for 4 x 4 blocks
+    const int rv = h->render_variant;
+    const bool fused_ok = h->ds.B == 4 && (rv == 0 || (rv >= 6 && rv <= 12));
+    if (rv == 1 || (h->ds.lmin > 0 && !fused_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else if (h->render_variant == 4 || h->render_variant == 5 || h->ds.B != 4)
-        CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant == 5 ? 1 : 0));
-    else  // 0 (default: arena chosen from the sizes), 6 / 7 / 8 (68 / 104 / 50 KB arena): block-row kernel, written for 4 x 4 blocks
-        CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl, h->render_variant >= 6 ? h->render_variant - 6 : -1));
+    else if (rv == 4 || rv == 5 || h->ds.B != 4)
+        CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
+    else {
+        // 0: chosen from the sizes -- views that look at about as many light-field samples as they have pixels (or more) go to the general
+        // kernel with its largest arena, the others to the tile kernel (tables from a kernel of their own); 6 .. 10: the general kernel's five
+        // configurations; 11 / 12: the tile kernel with 3 / 4 CTAs per SM.  All give identical bytes.
+        int tiles = rv == 11 ? 0 : rv == 12 ? 1 : -1;
+        if (rv == 0 && (long long)W * H >= 2LL * h->ds.Ws * h->ds.Ht) tiles = HMLFC_TILES_DEFAULT;
+        if (tiles >= 0) {
+            void *scratch = nullptr;
+            cudaMemPool_t pool;
+            CU(h, scratch_pool(&pool));
+            CU(h, cudaMallocFromPoolAsync(&scratch, render_tiles_scratch_bytes(n_views, W, H), pool, st));
+            const cudaError_t e = launch_render_tiles(h->ds, cams, n_views, W, H, d_out, scratch, st, &nl, tiles);
+            cudaFreeAsync(scratch, st);
+            CU(h, e);
+        } else {
+            CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl, rv >= 6 ? rv - 6 : -1));
+        }
+    }
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -389,7 +447,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 10 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
+    if (!h || variant < 0 || variant > 12 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
     h->render_variant = variant;
     return HMLFC_OK;
 }

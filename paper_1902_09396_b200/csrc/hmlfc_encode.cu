@@ -27,6 +27,11 @@
 #include <cmath>
 #include <vector>
 
+namespace hmlfc {  // hmlfc_api.cu
+cudaError_t scratch_pool(cudaMemPool_t *out);
+cudaError_t scratch_pool_trim();
+}
+
 namespace {
 
 constexpr int kThreads = 256;
@@ -392,29 +397,6 @@ uint64_t up8(uint64_t x) { return (x + 7) & ~7ull; }
 
 double now_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
 
-// Device scratch from the stream-ordered pool of the device (cudaMallocAsync): after the first call the pool serves the
-// encoder's buffers without going to the driver, and frees do not synchronise the device.
-cudaMemPool_t g_pool[64] = {};
-
-cudaError_t scratch_pool(cudaMemPool_t *out)
-{
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (!g_pool[dev]) {
-        cudaMemPoolProps props{};
-        props.allocType = cudaMemAllocationTypePinned;
-        props.location.type = cudaMemLocationTypeDevice;
-        props.location.id = dev;
-        if ((e = cudaMemPoolCreate(&g_pool[dev], &props)) != cudaSuccess) return e;
-        uint64_t keep = ~0ull;  // keep freed scratch for the next call (hmlfc_encode_release_scratch returns it)
-        if ((e = cudaMemPoolSetAttribute(g_pool[dev], cudaMemPoolAttrReleaseThreshold, &keep)) != cudaSuccess) return e;
-    }
-    *out = g_pool[dev];
-    return cudaSuccess;
-}
-
 struct DevBuf {  // frees on scope exit
     void *p = nullptr;
     cudaStream_t st = nullptr;
@@ -423,7 +405,7 @@ struct DevBuf {  // frees on scope exit
     {
         st = s;
         cudaMemPool_t pool;
-        cudaError_t e = scratch_pool(&pool);
+        cudaError_t e = hmlfc::scratch_pool(&pool);
         return e != cudaSuccess ? e : cudaMallocFromPoolAsync(&p, bytes ? bytes : 16, pool, s);
     }
     template <typename T> T *as() const { return static_cast<T *>(p); }
@@ -441,10 +423,7 @@ extern "C" void hmlfc_stream_free(uint8_t *h_stream) { free(h_stream); }
 
 extern "C" int hmlfc_encode_release_scratch(void)
 {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return HMLFC_E_CUDA;
-    if (g_pool[dev] && (cudaDeviceSynchronize() != cudaSuccess || cudaMemPoolTrimTo(g_pool[dev], 0) != cudaSuccess)) return HMLFC_E_CUDA;
-    return HMLFC_OK;
+    return hmlfc::scratch_pool_trim() == cudaSuccess ? HMLFC_OK : HMLFC_E_CUDA;
 }
 
 // target_psnr < 0: encode at p's thresholds.  Otherwise ("encoding parameters are varied ... to achieve a similar

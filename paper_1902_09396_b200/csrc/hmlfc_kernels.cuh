@@ -5,6 +5,11 @@
 
 namespace hmlfc {
 
+// Device scratch from a library-owned stream-ordered pool of the current device (cudaMallocFromPoolAsync): after the first call the pool
+// serves the buffers without going to the driver, and frees do not synchronise the device.  scratch_pool_trim returns the memory.
+cudaError_t scratch_pool(cudaMemPool_t *out);
+cudaError_t scratch_pool_trim();
+
 // marks written by the footprint kernels
 struct FootprintMarks {
     uint32_t *blk;  // [n_pc * nblk] bits
@@ -37,10 +42,19 @@ cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_
 cudaError_t launch_render_warp(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
                                int *n_launches, int shape);
 cudaError_t configure_render_warp();
-// CTA per 32 x 32 tile, block-row tasks (B = 4 streams only; returns cudaErrorInvalidValue otherwise)
-// arena: 0 = 3 CTAs x 68 KB per SM, 1 = 2 CTAs x 104 KB, 2 = 4 CTAs x 50 KB, -1 = chosen from the output and light-field sizes
+// Fused render kernels for B = 4 streams (return cudaErrorInvalidValue otherwise).
+// launch_render_cta (hmlfc_render_cta.cu): tables built inside the CTA, quadtree of sub-tile passes.  config: 0 = 256 threads, 32 x 32
+// tile, 3 CTAs x 66 KB per SM, 1 = 2 CTAs x 104 KB, 2 = 4 CTAs x 47 KB, 3 = 1024 threads, 64 x 64 tile, 4 = 512 threads, 64 x 32 tile,
+// -1 = chosen from the output and light-field sizes.
 cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
-                              int *n_launches, int arena);
+                              int *n_launches, int config);
+// launch_render_tiles (hmlfc_render_tiles.cu): tile tables built by a kernel of their own from the tiles' border rays, one pass per 32 x 32
+// tile (a tile that does not fit takes the general kernel's path in its CTA).  d_scratch: render_tiles_scratch_bytes() bytes of device
+// memory for the tables (contents irrelevant before, undefined after).  config: 0 = 3 CTAs per SM, 1 = 4 CTAs per SM.
+size_t render_tiles_scratch_bytes(int n_views, int W, int H);
+cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, void *d_scratch,
+                                cudaStream_t st, int *n_launches, int config);
+cudaError_t configure_render_tiles();
 cudaError_t configure_render_cta();
 cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,
                                     FootprintMarks marks, cudaStream_t st);

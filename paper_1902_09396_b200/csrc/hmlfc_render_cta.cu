@@ -1,798 +1,41 @@
-// Fused decode + render kernel, CTA-per-tile variant with block-ROW tasks (sm_100a) -- the default of
-// hmlfc_render for B = 4 streams.
+// Fused decode + render kernel with the tile tables built inside the CTA and a quadtree of sub-tile passes (sm_100a): renders every
+// tile hmlfc_render_tiles.cu hands over and whole views at low magnification (about as many light-field samples as output pixels
+// under a tile, or more).  For B = 4 streams.
 //
-// PAPER.md:289-293 (decoding procedure): "collect the required BISE compressed SRV blocks from the top level to
-// the bottom level.  Using the block indices, we infer whether a block belongs to the predictive SRV images ...
-// The motion vector values for the corresponding block are decoded"; "As a block of pixels are
-// decoded, our method benefits any LF rendering scheme by providing fast access to neighboring pixels for
-// interpolation"; PAPER.md:73 / :409 two-plane rendering.  Definitions: DESIGN.md sections 3 and 5.
+// PAPER.md:289-293 (decoding procedure), :309 (random access), :73 / :409 (two-plane rendering); definitions: DESIGN.md sections 3
+// and 5; phases and vocabulary: hmlfc_render_common.cuh.
 //
 // One CTA of NT threads renders a TW x TH tile of one output view, 4 consecutive pixels per thread (NT = 256: 32 x 32,
-// NT = 512: 64 x 32, NT = 1024: 64 x 64).  At 40 dB only every eighth 4 x 4 block of a plane carries data, so a tile's
-// decode work is a few hundred short dependent chains (flag word -> motion record -> payload words -> reference payload
-// words): the path is bound by latency and instruction issue, not by bytes (profiles/).  The design therefore puts as
-// many pixels as possible behind every chain -- large tiles, every light-field sample a tile needs decoded exactly once --
-// and keeps the per-tile table work short:
+// NT = 512: 64 x 32, NT = 1024: 64 x 64):
 //   A   ray set-up (screen coordinates once per column / row, shared by shuffles), 16-tap footprint per pixel;
-//   SV  integer (u,v) range and (s,t) box of the tile's taps (warp reductions + 8 shared atomics per warp).  The footprint
-//       box PER VIEW needs no per-pixel work: every ray passes through the eye, so s is an affine function of u (and t
-//       of v) that depends on the camera alone; the pixels that touch view column a have u in [a-1, a+1) and hence s in
-//       the image of that interval (plus a rounding margin), intersected with the tile's box;
-//   T   warp 0 builds the view table (boxes, (view, sample) cells), warp 1 the table of SRV planes of every level under
-//       the views ("slots"; a level-L plane is shared by the 2^L x 2^L views below it and is decoded ONCE per tile) and
-//       stages their descriptors in shared memory; the other warps zero the accumulators;
-//   B1  one lane per (slot, channel, block row of the slot's box): the row's flag/rank words are loaded once
-//       (128-bit records), non-empty blocks are compacted into a record list;
-//   B2  one lane per record: the block's motion record (BISE decode_at, once per block);
-//   B3  one lane per (record, block row): the row's 4 stored values come from ONE pass over two 64-bit BISE
-//       windows (plain / trit / quint without control flow); the motion-compensated reference row (two
-//       neighbouring blocks of the reference SRV) likewise; written to the slot's int16 accumulator;
-//   B4  one lane per (view, sample) cell: top-level RKV + the h per-level terms, inverse YCoCg-R, clamp ->
-//       float RGB patch;
-//   C   every pixel gathers its 16 taps from the patch (128-bit loads) and blends with packed fp32 FMAs.
+//   SV  integer (u,v) range and (s,t) box of the tile's taps (warp reductions + 8 shared atomics per warp);
+//   T   warp 0 builds the view table, warp 1 the plane table, the other warps zero the accumulators;
+//   B1 - B4, C  as in hmlfc_render_common.cuh.
 // A tile whose tables do not fit the shared-memory arena (minification) is rendered as its four quadrants with one pixel
 // per thread, a quadrant that does not fit is split again, down to 8-pixel-wide sub-tiles; one of those that still does
 // not fit is rendered by 16 direct sample decodes per pixel.  All paths produce identical bytes.
-#include "hmlfc_kernels.cuh"
-#include "hmlfc_bise_row.cuh"
+#include "hmlfc_render_common.cuh"
 
 namespace hmlfc {
 
 namespace {
 
-constexpr int kPPL = 4;           // consecutive pixels per thread
-constexpr int kMaxV = 4;          // views per axis of one tile's footprint
-constexpr int kMaxViews = kMaxV * kMaxV;
-constexpr int kMaxSlots = 40;     // 16 + 9 + 4 * 3 planes + slack (a pass with more planes is split)
-constexpr int kMaxChunks = 512;   // 32-cell chunks of the patch
-constexpr int kMinRec = 256;      // smallest record capacity worth starting with
-constexpr uint32_t FULL = 0xffffffffu;
-constexpr uint32_t kNone = 0xFFFFFFFFu;
-
-// debug builds (-DHMLFC_PASS_STATS) count the passes of every size and why a pass was split
-#ifdef HMLFC_PASS_STATS
-__device__ unsigned long long g_pass_stats[64];  // [0..3] passes tried at quadtree level 0..3, [4..7] passes done, [8..] fail reasons, [16..] cycles of thread 0 per phase
-__device__ long long g_phase_last[1 << 20];      // per CTA: clock of the previous mark
-#define PASS_STAT(i) do { if (threadIdx.x == 0) atomicAdd(&g_pass_stats[i], 1ull); } while (0)
-#define PHASE_MARK(i) do { if (threadIdx.x == 0) { const unsigned cta_ = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x; \
-        const long long now_ = clock64(); if ((i) >= 0) atomicAdd(&g_pass_stats[16 + ((i) < 0 ? 0 : (i))], (unsigned long long)(now_ - g_phase_last[cta_ & ((1u << 20) - 1u)])); \
-        g_phase_last[cta_ & ((1u << 20) - 1u)] = now_; } } while (0)
-// the same for thread 32 (warp 1, the plane table of phase T); restarted with i < 0
-#define W1_MARK(i) do { if (threadIdx.x == 32) { const unsigned cta_ = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x; \
-        const long long now_ = clock64(); if ((i) >= 0) atomicAdd(&g_pass_stats[32 + ((i) < 0 ? 0 : (i))], (unsigned long long)(now_ - g_phase_last[(cta_ + (1u << 19)) & ((1u << 20) - 1u)])); \
-        g_phase_last[(cta_ + (1u << 19)) & ((1u << 20) - 1u)] = now_; } } while (0)
-#else
-#define PASS_STAT(i) do { } while (0)
-#define PHASE_MARK(i) do { } while (0)
-#define W1_MARK(i) do { } while (0)
-#endif
-
-// n / d for n * d < 2^32 by one multiply-high (m == 0 encodes d <= 1)
-__device__ __forceinline__ uint32_t magic_of(uint32_t d) { return d <= 1u ? 0u : 0xFFFFFFFFu / d + 1u; }
-__device__ __forceinline__ uint32_t fdiv(uint32_t n, uint32_t m) { return m ? __umulhi(n, m) : n; }
-// j / n for 0 <= j < 16, 1 <= n <= 4
-__device__ __forceinline__ int div_small(int j, int n) { return n == 1 ? j : n == 2 ? (j >> 1) : n == 4 ? (j >> 2) : ((j * 11) >> 5); }
-
-struct ViewInfo {   // view (iu, iv) of the tile's (u,v) neighbourhood, index iv * 4 + iu
-    int s0, t0, ns, nt;          // footprint box of the view (ns == 0: no pixel of the tile touches it)
-    int cellbase;                // first (view, sample) cell (a multiple of 32: a warp's cells belong to one view)
-    uint32_t m_ns;               // magic multiplier of ns
-    uint32_t rkv_lo, rkv_hi;     // index of the view's top-level RKV plane * Ht * Ws
-};
-
-struct SlotInfo {   // one SRV plane of one level under the tile's views
-    int s0, t0, ns, s1;          // sample box (union of the boxes of the views below); s1 = last column
-    int t1, bx0, by0, nbw;       // last row; block box
-    int accbase, nbh;            // first accumulator sample; block rows
-    uint32_t pred;               // plane is predictive
-    int _pad;
-};
-
-struct Ctl {
-    int lo[4], hi[4];                    // (u0, v0) range of the tile's taps [0..1], (s, t) box of all its taps [2..3]
-    float aff[2][4];                     // per axis: s = aff[0] + aff[1] u for every ray of this camera, rounding margin aff[2]
-    Camera cam;
-    ViewInfo view[kMaxViews];
-    SlotInfo slot[kMaxSlots];
-    uint4 desc[kMaxSlots][3];            // descriptors of the slot's three plane-channels ...
-    uint4 rdesc[kMaxSlots][3];           // ... and of its cluster's reference plane (predictive planes)
-    int2 voff[kMaxViews][kMaxLevels];    // accumulator offset / row stride of the view's plane at level L
-    int2 vcb[kMaxViews];                 // {cellbase - t0 * ns - s0, ns}: cell of sample (s,t) = x + t * y + s
-    uint8_t chunkvw[kMaxChunks];         // view of the 32-cell chunk
-    int lvl_base[kMaxLevels], lvl_pu0[kMaxLevels], lvl_pv0[kMaxLevels], lvl_nu[kMaxLevels];
-    int nslots, ncell, nacc, nbhmax;
-    int n_rec;
-    uint16_t lut[384];
-};
-
-struct PixTaps {  // one output pixel's 16-tap footprint
-    uint32_t uv;  // u0 | v0 << 12 | du << 24 | dv << 25   (kNone: the ray misses the slab / pixel outside the view)
-    uint32_t st;  // s0 | t0 << 14 | ds << 28 | dt << 29
-    float fu, fv, fs, ft;
-};
-
-__device__ __forceinline__ uint32_t round_rgb(float r, float g, float b)
-{
-    const uint32_t R = (uint32_t)min(max(__float2int_rd(r + 0.5f), 0), 255);
-    const uint32_t G = (uint32_t)min(max(__float2int_rd(g + 0.5f), 0), 255);
-    const uint32_t B = (uint32_t)min(max(__float2int_rd(b + 0.5f), 0), 255);
-    return R | (G << 8) | (B << 16);
-}
-
-// quadrilinear blend of 16 float RGB taps fetched by fetch(a, b): a = view (bit0 u, bit1 v), b = pixel (bit0 s, bit1 t)
-template <typename Fetch>
-__device__ __forceinline__ uint32_t blend16(const PixTaps &k, Fetch fetch)
-{
-    const float ws0 = 1.0f - k.fs, wt0 = 1.0f - k.ft, wu0 = 1.0f - k.fu, wv0 = 1.0f - k.fv;
-    const float wst[4] = {ws0 * wt0, k.fs * wt0, ws0 * k.ft, k.fs * k.ft};
-    const float wuv[4] = {wu0 * wv0, k.fu * wv0, wu0 * k.fv, k.fu * k.fv};
-    float2 accRG = make_float2(0.f, 0.f), accB = make_float2(0.f, 0.f);
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        float2 cRG = make_float2(0.f, 0.f), cB = make_float2(0.f, 0.f);
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const float4 t = fetch(a, b);
-            const float2 w2 = make_float2(wst[b], wst[b]);
-            cRG = __ffma2_rn(w2, make_float2(t.x, t.y), cRG);
-            cB = __ffma2_rn(w2, make_float2(t.z, t.w), cB);
-        }
-        const float2 w2 = make_float2(wuv[a], wuv[a]);
-        accRG = __ffma2_rn(w2, cRG, accRG);
-        accB = __ffma2_rn(w2, cB, accB);
-    }
-    return round_rgb(accRG.x, accRG.y, accB.x);
-}
-
-// the sub-tile does not fit even at the smallest size (strong minification): 16 direct sample decodes
-__device__ __noinline__ uint32_t direct_pixel(const DevStream &S, const PixTaps k)
-{
-    const int u0 = k.uv & 0xFFF, v0 = (k.uv >> 12) & 0xFFF, s0 = k.st & 0x3FFF, t0 = (k.st >> 14) & 0x3FFF;
-    const int u1 = u0 + (int)((k.uv >> 24) & 1u), v1 = v0 + (int)((k.uv >> 25) & 1u);
-    const int s1 = s0 + (int)((k.st >> 28) & 1u), t1 = t0 + (int)((k.st >> 29) & 1u);
-    uint32_t c8[16];
-#pragma unroll 1
-    for (int a = 0; a < 16; ++a) c8[a] = decode_rgb8(S, (a & 4) ? u1 : u0, (a & 8) ? v1 : v0, (a & 1) ? s1 : s0, (a & 2) ? t1 : t0);
-    return blend16(k, [&](int a, int b) {
-        const uint32_t c = c8[a * 4 + b];
-        return make_float4((float)(c & 0xFFu), (float)((c >> 8) & 0xFFu), (float)((c >> 16) & 0xFFu), 0.f);
-    });
-}
-
-// the per-pixel bodies of phases A and C exist once (calls) or four times (inlined into the 4-pixel loops)
-#ifdef HMLFC_NOINLINE_A
-#define HMLFC_A_ATTR __noinline__
-#else
-#define HMLFC_A_ATTR __forceinline__
-#endif
-#ifdef HMLFC_NOINLINE_C
-#define HMLFC_C_ATTR __noinline__
-#else
-#define HMLFC_C_ATTR __forceinline__
-#endif
-#ifndef HMLFC_EST_SLACK
-#define HMLFC_EST_SLACK 120
-#endif
-constexpr int kEstSlackPct = HMLFC_EST_SLACK;  // the full-tile pass is tried when the estimate is below this share of the arena
-
-// reset of the accumulators the next pass's SV phase writes with atomics (callers: after a barrier that every reader has passed)
-__device__ __forceinline__ void reset_ctl(Ctl &ctl)
-{
-    const int tid = threadIdx.x;
-    if (tid < 4) { ctl.lo[tid] = 0x7fffffff; ctl.hi[tid] = -1; }
-    if (tid == 32) ctl.n_rec = 0;
-}
-
-// Footprint interval along one axis of the views / planes that cover grid positions [a0, a1] of that axis: the pixels that touch
-// them have a continuous grid coordinate in [a0 - 1, a1 + 1) and, every ray passing through the eye, an image-plane coordinate
-// of aff[0] + aff[1] * (grid coordinate) up to the rounding margin aff[2]; taps are floor(.) and floor(.) + 1.  Clipped to the tile's
-// own box [lo, hi] (exact, from the pixels).  A degenerate camera (eye on the camera plane: all pixels share one grid coordinate)
-// has a non-finite map and gets the tile's box.
-__device__ __forceinline__ void axis_box(const float (&aff)[4], int a0, int a1, int lo, int hi, int &b0, int &b1)
-{
-    const float e0 = fmaf(aff[1], (float)(a0 - 1), aff[0]), e1 = fmaf(aff[1], (float)(a1 + 1), aff[0]);
-    const float x0 = fminf(e0, e1) - aff[2], x1 = fmaxf(e0, e1) + aff[2];
-    b0 = lo; b1 = hi;
-    if (x0 > (float)lo && x0 < 1e9f) b0 = (int)floorf(x0);          // NaN / infinities fail the comparisons: tile box
-    if (x1 < (float)hi && x1 > -1e9f) b1 = (int)floorf(x1) + 1;
-    b0 = max(b0, lo); b1 = min(b1, hi);
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// Phases T, B1-B4 for the sub-tile whose (u,v) range and (s,t) box (ctl.lo / ctl.hi) are set: builds the tables and, if
-// they fit the arena, the float RGB patch of every (view, sample) cell.  Returns false (CTA-uniform) when the sub-tile does
-// not fit; the caller then splits it.  Called by all threads.
-template <int kArenaBytes, int kNT>
-__device__ __forceinline__ bool build_patch(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int bu0, int bv0, int nu, int nv,
-                                            int bs0, int bs1, int bt0, int bt1)
-{
-    constexpr int kNW = kNT / 32;
-    constexpr int kSpecZero = kNT == 256 ? 1536 : (kNT == 512 ? 3072 : 6144);  // 16-byte words zeroed while warps 0 and 1 build the tables
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int h = S.h;
-
-    // -------------------------------------------------------- T: tables (warp 0: views, warp 1: planes)
-    if (warp == 0) {
-        const int iu = lane & 3, iv = (lane >> 2) & 3;
-        int vs0 = 0, vt0 = 0, vns = 0, vnt = 0;
-        if (lane < kMaxViews && iu < nu && iv < nv) {
-            int a0, a1, c0, c1;
-            axis_box(ctl.aff[0], bu0 + iu, bu0 + iu, bs0, bs1, a0, a1);
-            axis_box(ctl.aff[1], bv0 + iv, bv0 + iv, bt0, bt1, c0, c1);
-            if (a0 <= a1 && c0 <= c1) { vs0 = a0; vt0 = c0; vns = a1 - a0 + 1; vnt = c1 - c0 + 1; }
-        }
-        const int vcells = (vns * vnt + 31) & ~31;  // whole warps per view
-        int incl = vcells;
-#pragma unroll
-        for (int o = 1; o < kMaxViews; o <<= 1) {
-            const int n = __shfl_up_sync(FULL, incl, o);
-            if (lane >= o) incl += n;
-        }
-        const int ncell = __shfl_sync(FULL, incl, kMaxViews - 1);
-        if (lane < kMaxViews) {
-            ViewInfo vi;
-            vi.s0 = vs0; vi.t0 = vt0; vi.ns = vns; vi.nt = vnt;
-            vi.cellbase = incl - vcells;
-            ctl.vcb[lane] = make_int2(vi.cellbase - vt0 * vns - vs0, vns);
-            for (int c = vi.cellbase >> 5; c < min(incl >> 5, kMaxChunks); ++c) ctl.chunkvw[c] = (uint8_t)lane;
-            vi.m_ns = magic_of((uint32_t)vns);
-            const unsigned long long ro = (unsigned long long)(((bv0 + iv) >> h) * S.UH + ((bu0 + iu) >> h)) *
-                                          (unsigned long long)S.Ht * (unsigned long long)S.Ws;
-            vi.rkv_lo = (uint32_t)ro; vi.rkv_hi = (uint32_t)(ro >> 32);
-            ctl.view[lane] = vi;
-        }
-        if (lane == 0) ctl.ncell = ncell;
-        PHASE_MARK(11);
-    } else if (warp == 1) {
-        W1_MARK(-1);
-        // per level the rectangle of planes over the views; every lane walks the levels (no table, no exchange)
-        int accrun = 0, nbhmax = 0, nslots = 0;
-        for (int L = S.lmin; L < h; ++L) nslots += (((bu0 + nu - 1) >> L) - (bu0 >> L) + 1) * (((bv0 + nv - 1) >> L) - (bv0 >> L) + 1);
-        if (lane < h) {
-            int base = 0;
-            for (int L = S.lmin; L < lane; ++L) base += (((bu0 + nu - 1) >> L) - (bu0 >> L) + 1) * (((bv0 + nv - 1) >> L) - (bv0 >> L) + 1);
-            ctl.lvl_base[lane] = base; ctl.lvl_pu0[lane] = bu0 >> lane; ctl.lvl_pv0[lane] = bv0 >> lane;
-            ctl.lvl_nu[lane] = ((bu0 + nu - 1) >> lane) - (bu0 >> lane) + 1;
-        }
-        W1_MARK(0);
-        if (nslots <= kMaxSlots) {
-            for (int sb = 0; sb < nslots; sb += 32) {
-                const int s = sb + lane;
-                SlotInfo si;
-                si.pred = 0u; si._pad = 0;
-                si.s0 = si.t0 = 0; si.ns = 0; si.s1 = si.t1 = -1; si.bx0 = si.by0 = 0; si.nbw = 0; si.nbh = 0;
-                int nsamp = 0;
-                if (s < nslots) {
-                    int L = S.lmin, base = 0, n = 1;
-                    for (;;) {
-                        n = ((bu0 + nu - 1) >> L) - (bu0 >> L) + 1;
-                        const int cnt = n * ((((bv0 + nv - 1) >> L) - (bv0 >> L)) + 1);
-                        if (s < base + cnt) break;
-                        base += cnt; ++L;
-                    }
-                    const int jj = s - base, jv = div_small(jj, n);
-                    const int pv = (bv0 >> L) + jv, pu = (bu0 >> L) + (jj - jv * n);
-                    const LevelDesc lv = S.lev[L];
-                    const uint32_t pc0 = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
-                    si.pred = (uint32_t)((pu | pv) & 1);
-                    const uint32_t refpc0 = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
-                    // the plane's descriptors (and its reference plane's) go to shared memory: B1-B3 read them from there
-                    const uint4 d0 = ldg(S.pc + pc0), d1 = ldg(S.pc + pc0 + 1), d2 = ldg(S.pc + pc0 + 2);
-                    uint4 r0 = d0, r1 = d1, r2 = d2;
-                    if (si.pred) { r0 = ldg(S.pc + refpc0); r1 = ldg(S.pc + refpc0 + 1); r2 = ldg(S.pc + refpc0 + 2); }
-                    W1_MARK(1);
-                    // box of the views below this plane
-                    int a0, a1, c0, c1;
-                    axis_box(ctl.aff[0], max(pu << L, bu0), min(((pu + 1) << L) - 1, bu0 + nu - 1), bs0, bs1, a0, a1);
-                    axis_box(ctl.aff[1], max(pv << L, bv0), min(((pv + 1) << L) - 1, bv0 + nv - 1), bt0, bt1, c0, c1);
-                    if (a0 <= a1 && c0 <= c1) {
-                        si.s0 = a0; si.t0 = c0; si.s1 = a1; si.t1 = c1; si.ns = a1 - a0 + 1;
-                        si.bx0 = a0 >> 2; si.by0 = c0 >> 2;
-                        si.nbw = (a1 >> 2) - si.bx0 + 1; si.nbh = (c1 >> 2) - si.by0 + 1;
-                        nsamp = si.ns * (c1 - c0 + 1);
-                    }
-                    W1_MARK(2);
-                    ctl.desc[s][0] = d0; ctl.desc[s][1] = d1; ctl.desc[s][2] = d2;
-                    ctl.rdesc[s][0] = r0; ctl.rdesc[s][1] = r1; ctl.rdesc[s][2] = r2;
-                    W1_MARK(3);
-                }
-                int ai = nsamp;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int n1 = __shfl_up_sync(FULL, ai, o);
-                    if (lane >= o) ai += n1;
-                }
-                si.accbase = accrun + ai - nsamp;
-                if (s < nslots) ctl.slot[s] = si;
-                accrun += __shfl_sync(FULL, ai, 31);
-                nbhmax = max(nbhmax, __reduce_max_sync(FULL, si.nbh));
-            }
-        }
-        if (lane == 0) { ctl.nslots = nslots; ctl.nacc = accrun; ctl.nbhmax = nbhmax; }
-        W1_MARK(4);
-    } else {
-        // meanwhile the other warps zero the head of the accumulator region (its size is not known yet)
-        uint4 *z = reinterpret_cast<uint4 *>(arena);
-        for (int q = tid - 64; q < kSpecZero; q += kNT - 64) z[q] = make_uint4(0u, 0u, 0u, 0u);
-    }
-    __syncthreads();
-    PHASE_MARK(4);
-    const int ncell = ctl.ncell, nacc = ctl.nacc, nslots = ctl.nslots, nbhmax = ctl.nbhmax;
-    // accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by the record list (16 bytes each)
-    const long long rest = (long long)kArenaBytes - (((long long)nacc * 8 + 15) & ~15LL);
-    if (!(nslots <= kMaxSlots && ncell <= 32 * kMaxChunks && rest >= (long long)ncell * 16 && rest >= (long long)kMinRec * 16)) {
-        PASS_STAT(10);
-        return false;
-    }
-    const int reccap = (int)min(rest / 16, 0x7fffffLL);
-    uint2 *acc = reinterpret_cast<uint2 *>(arena);
-    unsigned char *region2 = arena + (((size_t)nacc * 8 + 15) & ~(size_t)15);
-    uint4 *rec = reinterpret_cast<uint4 *>(region2);      // [reccap]
-    float4 *patch = reinterpret_cast<float4 *>(region2);  // [ncell], after the records are dead
-    // ---------------------------------------------------- zero the rest of the accumulators; accumulator offsets of every (view, level)
-    {
-        uint4 *z = reinterpret_cast<uint4 *>(arena);
-        const int nz = (nacc + 1) >> 1;
-        for (int q = kSpecZero + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);
-        for (int q = tid; q < kMaxViews * h; q += kNT) {
-            const int L = q >> 4, vw = q & 15;
-            const ViewInfo &vi = ctl.view[vw];
-            if (L < S.lmin || vi.ns == 0) continue;
-            const int iu = vw & 3, iv = vw >> 2;
-            const int sidx = ctl.lvl_base[L] + (((bv0 + iv) >> L) - ctl.lvl_pv0[L]) * ctl.lvl_nu[L] + (((bu0 + iu) >> L) - ctl.lvl_pu0[L]);
-            const SlotInfo &sl = ctl.slot[sidx];
-            ctl.voff[vw][L] = make_int2(sl.accbase + (vi.t0 - sl.t0) * sl.ns + (vi.s0 - sl.s0), sl.ns);
-        }
-    }
-    // ---------------------------------------------------- B1: one lane per (slot, channel, block row): flag words -> records
-    {
-        const int per_slot = 3 * nbhmax, nitems = nslots * per_slot;
-        const uint32_t m_ps = magic_of((uint32_t)per_slot), m_nbh = magic_of((uint32_t)nbhmax);
-        for (int base = 0; base < nitems; base += kNT) {
-            const int it = base + tid;
-            bool on = it < nitems;
-            uint32_t pred = 0u, sc = 0u, frbase = 0u;
-            int b0 = 0, b1 = -1, by = 0, rowb = 0;
-            if (on) {
-                const uint32_t s = fdiv((uint32_t)it, m_ps), r = (uint32_t)it - s * (uint32_t)per_slot;
-                const uint32_t c = fdiv(r, m_nbh), jr = r - c * (uint32_t)nbhmax;
-                const SlotInfo &sl = ctl.slot[s];
-                on = (int)jr < sl.nbh;
-                if (on) {
-                    frbase = ctl.desc[s][c].x;
-                    sc = s | (c << 6);
-                    pred = sl.pred;
-                    by = sl.by0 + (int)jr;
-                    rowb = by * S.nbx;
-                    b0 = rowb + sl.bx0; b1 = b0 + sl.nbw - 1;
-                }
-            }
-            const int ng = on ? (b1 >> 5) - (b0 >> 5) + 1 : 0;
-            const int ngmax = __reduce_max_sync(FULL, ng);
-            for (int gi = 0; gi < ngmax; ++gi) {
-                uint32_t resb = 0u, prdb = 0u;
-                uint4 fr = make_uint4(0u, 0u, 0u, 0u);
-                const int g = (b0 >> 5) + gi;
-                if (gi < ng) {
-                    fr = ldg(S.flagrec + frbase + 4u * (uint32_t)g);
-                    const int lo = max(b0 - (g << 5), 0), hi = min(b1 - (g << 5), 31);
-                    const uint32_t mask = (0xFFFFFFFFu >> (31 - hi)) & (0xFFFFFFFFu << lo);
-                    resb = fr.x & mask;
-                    prdb = pred ? (fr.z & mask) : 0u;
-                }
-                uint32_t any = resb | prdb;
-                const int cnt = (int)popc(any);
-                int inc = cnt;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int n = __shfl_up_sync(FULL, inc, o);
-                    if (lane >= o) inc += n;
-                }
-                const int tot = __shfl_sync(FULL, inc, 31);
-                if (tot == 0) continue;
-                int wbase = 0;
-                if (lane == 31) wbase = atomicAdd(&ctl.n_rec, tot);
-                wbase = __shfl_sync(FULL, wbase, 31);
-                int idx = wbase + inc - cnt;
-                while (any) {
-                    const int bp = __ffs(any) - 1;
-                    const uint32_t bit = 1u << bp;
-                    any &= any - 1u;
-                    const bool hr = (resb & bit) != 0u, hp = (prdb & bit) != 0u;
-                    // rank of the block's payload * 16, rank of its motion record, slot | channel | block row | block column
-                    if (idx < reccap)
-                        rec[idx] = make_uint4(hr ? ((fr.y + popc(fr.x & (bit - 1u))) << 4) : kNone, hp ? (fr.w + popc(fr.z & (bit - 1u))) : kNone,
-                                              sc | ((uint32_t)by << 8) | ((uint32_t)((g << 5) + bp - rowb) << 20), 0u);
-                    ++idx;
-                }
-            }
-        }
-    }
-    __syncthreads();
-    PHASE_MARK(5);
-    const int nrec = ctl.n_rec;
-    if (nrec > reccap) {
-        PASS_STAT(11);
-        __syncthreads();  // every thread has read the record count (the caller resets it)
-        return false;
-    }
-    // ------------------------------------------------ B2: motion record, once per block
-    for (int rr = tid; rr < nrec; rr += kNT) {
-        const uint4 r0 = rec[rr];
-        uint32_t mvp = 0u;
-        if (r0.y != kNone) {
-            const uint32_t mr = bise_at(S.mv + ctl.desc[r0.z & 63u][(r0.z >> 6) & 3u].z, r0.y, S.mv_layout, S.mv_m, ctl.lut);
-            int md, dx, dy;
-            mv_unpack(S, mr, md, dx, dy);
-            mvp = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
-        }
-        rec[rr].y = mvp;
-    }
-    __syncthreads();
-    PHASE_MARK(6);
-    // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values (neighbouring
-    // lanes work on neighbouring blocks of one plane: their payload words share sectors and they take the same branches)
-    {
-        int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
-        for (int t = tid; t < 4 * nrec; t += kNT) {
-            const int rr = t >> 2, ky = t & 3;
-            const uint4 r0 = rec[rr];
-            const uint32_t s = r0.z & 63u, c = (r0.z >> 6) & 3u;
-            const SlotInfo &sl = ctl.slot[s];
-            const int yy = (int)(((r0.z >> 8) & 0xFFFu) << 2) + ky;
-            const int st0 = sl.t0, st1 = sl.t1;
-            if (yy < st0 || yy > st1) continue;
-            const int xx = (int)((r0.z >> 20) << 2);
-            uint2 own = make_uint2(0u, 0u);
-            if (r0.x != kNone) {
-                const uint4 d = ctl.desc[s][c];
-                own = bise_row4(S.pay + d.y, r0.x + (uint32_t)(ky << 2), d.w, ctl.lut);
-            }
-            int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
-            if (r0.y) {
-                const int rx = xx + (int)((r0.y >> 8) & 0xFFu) - S.W, ry = yy + (int)(r0.y & 0xFFu) - S.W;
-                if ((unsigned)ry < (unsigned)S.Ht) {
-                    // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
-                    const uint4 dr = ctl.rdesc[s][c];
-                    const int o = rx & 3, bxa = rx >> 2;
-                    const uint32_t i0 = (uint32_t)((ry & 3) << 2);
-                    const int rowb = (ry >> 2) * S.nbx;
-                    uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-#pragma unroll 1
-                    for (int j = 0; j < 2; ++j) {  // a loop on purpose: one instance of the row decode (instruction cache)
-                        uint2 q = make_uint2(0u, 0u);
-                        if ((j == 0 || o) && (unsigned)(bxa + j) < (unsigned)S.nbx) {
-                            const int b = rowb + bxa + j;
-                            const uint4 fr = ldg(S.flagrec + dr.x + 4u * (uint32_t)(b >> 5));
-                            const uint32_t bit = 1u << (b & 31);
-                            if (fr.x & bit) q = bise_row4(S.pay + dr.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, dr.w, ctl.lut);
-                        }
-                        if (j == 0) qa = q; else qb = q;
-                    }
-                    // samples o .. o+3 of the 8-sample string qa | qb
-                    uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
-                    if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
-                    const uint32_t sh = (uint32_t)(o & 1) << 4;
-                    const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
-                    const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
-                    // R10: subtractive P = e + R, additive P = e - R
-                    if (r0.y & 0x10000u) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
-                    else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
-                }
-            }
-            int16_t *dst = acc16 + (((sl.accbase + (yy - st0) * sl.ns + (xx - sl.s0)) << 2) + (int)c);
-            const int ss0 = sl.s0, ss1 = sl.s1;
-            if (xx >= ss0 && xx <= ss1) dst[0] = (int16_t)e0;
-            if (xx + 1 >= ss0 && xx + 1 <= ss1) dst[4] = (int16_t)e1;
-            if (xx + 2 >= ss0 && xx + 2 <= ss1) dst[8] = (int16_t)e2;
-            if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
-        }
-    }
-    __syncthreads();
-    PHASE_MARK(7);
-    // ------------------------------------------------ B4: top-level RKV + per-level terms -> float RGB patch
-    for (int q = tid; q < ncell; q += kNT) {
-        const int vw = ctl.chunkvw[q >> 5];
-        const ViewInfo vi = ctl.view[vw];
-        const uint32_t local = (uint32_t)(q - vi.cellbase);
-        const uint32_t it = fdiv(local, vi.m_ns), is = local - it * (uint32_t)vi.ns;
-        if ((int)it >= vi.nt) continue;  // padding of the view's last chunk
-        const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
-        const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
-        int a[3] = {rk.x, rk.y, rk.z};
-        for (int L = S.lmin; L < h; ++L) {
-            const int2 vo = ctl.voff[vw][L];
-            const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
-            a[0] += (int)(int16_t)(w.x & 0xFFFFu);
-            a[1] += (int)w.x >> 16;
-            a[2] += (int)(int16_t)(w.y & 0xFFFFu);
-        }
-        const uint32_t c8 = ycocg_to_rgb8(a);
-        // the patch aliases the record list: all B3 readers passed the barrier above
-        patch[q] = make_float4((float)(c8 & 0xFFu), (float)((c8 >> 8) & 0xFFu), (float)((c8 >> 16) & 0xFFu), 0.f);
-    }
-    __syncthreads();
-    PHASE_MARK(8);
-    return true;
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// Pixel mapping of a pass of pw x ph pixels at (ox, oy).  full: the whole TW x TH tile, thread (tid % (TW / 4), tid / (TW / 4)) owns 4
-// consecutive pixels.  Otherwise a sub-tile of at most NT pixels, one pixel per thread (pixel slot 0).  One code path serves both
-// (slots 1..3 are simply empty in sub-tile passes): the kernel is instruction-cache sensitive, so the phases exist once.
-template <int kTW>
-__device__ __forceinline__ void thread_pixel(int ox, int oy, bool full, int lpw, int npx, int &x0, int &y, int &npix)
-{
-    constexpr int kTPR = kTW / kPPL;
-    const int tid = threadIdx.x;
-    if (full) { x0 = ox + (tid % kTPR) * kPPL; y = oy + tid / kTPR; npix = kPPL; }
-    else { x0 = ox + (tid & ((1 << lpw) - 1)); y = oy + (tid >> lpw); npix = tid < npx ? 1 : 0; }
-}
-
-// 16-tap footprint of the pixel with screen coordinates (px, py)
-__device__ HMLFC_A_ATTR PixTaps pixel_taps(const DevStream &S, const Camera &cam, float px, float py, bool inside)
-{
-    PixTaps t;
-    t.uv = kNone; t.st = 0u;
-    t.fu = t.fv = t.fs = t.ft = 0.f;
-    if (inside) {
-        const Ray r = ray_from_screen(S, cam, px, py);
-        if (r.hit) {
-            const Taps k = tap_setup(S, r);
-            t.uv = (uint32_t)k.u0 | ((uint32_t)k.v0 << 12) | ((uint32_t)(k.u1 - k.u0) << 24) | ((uint32_t)(k.v1 - k.v0) << 25);
-            t.st = (uint32_t)k.s0 | ((uint32_t)k.t0 << 14) | ((uint32_t)(k.s1 - k.s0) << 28) | ((uint32_t)(k.t1 - k.t0) << 29);
-            t.fu = k.fu; t.fv = k.fv; t.fs = k.fs; t.ft = k.ft;
-        }
-    }
-    return t;
-}
-
-// ---------------------------------------------------------------- A: rays of the thread's pixels
-template <int kTW>
-__device__ __forceinline__ void setup_rays(const DevStream &S, const Camera &cam, int W, int H, int ox, int oy, bool full, int lpw, int npx,
-                                           PixTaps (&pt)[kPPL])
-{
-    constexpr int kTPR = kTW / kPPL, kCPL = kTW / 32, kRPW = 32 / kTPR;  // threads per tile row, tile columns per lane, tile rows per warp
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    int x0, y, npix;
-    thread_pixel<kTW>(ox, oy, full, lpw, npx, x0, y, npix);
-    // screen coordinates once per column / row of the tile, shared by shuffles (sub-tiles: each lane its own)
-    float pxl[kCPL];
-#pragma unroll
-    for (int j = 0; j < kCPL; ++j) pxl[j] = ray_screen(cam.tan_half_x, W, full ? ox + lane * kCPL + j : x0);
-    const float pyl = ray_screen(cam.tan_half_y, H, full ? oy + warp * kRPW + (lane % kRPW) : y);
-    const float py = __shfl_sync(FULL, pyl, full ? lane / kTPR : lane);
-#pragma unroll
-    for (int p = 0; p < kPPL; ++p) {
-        // pixel column (tid % kTPR) * 4 + p of the tile was computed by lane column / kCPL as its value column % kCPL
-        const float px = __shfl_sync(FULL, pxl[kCPL == 1 ? 0 : (p & (kCPL - 1))], full ? ((lane % kTPR) * kPPL + p) / kCPL : lane);
-        pt[p] = pixel_taps(S, cam, px, py, p < npix && x0 + p < W && y < H);
-    }
-}
-
-// C for one pixel: its 16 taps from the patch, blended
-__device__ HMLFC_C_ATTR uint32_t blend_pixel(const Ctl &ctl, const float4 *__restrict__ patch, const PixTaps k, int bu0, int bv0)
-{
-    const int iu = (int)(k.uv & 0xFFF) - bu0, iv = (int)((k.uv >> 12) & 0xFFF) - bv0;
-    const int s0 = (int)(k.st & 0x3FFF), t0 = (int)((k.st >> 14) & 0x3FFF);
-    const int du = (int)((k.uv >> 24) & 1u), dv = ((k.uv >> 25) & 1u) ? 4 : 0;
-    const int ds = (int)((k.st >> 28) & 1u), dt = (int)((k.st >> 29) & 1u);
-    const int vw0 = iv * 4 + iu;
-    int vb[4], vs[4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        const int2 cb = ctl.vcb[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
-#ifdef HMLFC_BOX_CHECK
-        {
-            const ViewInfo &vi = ctl.view[vw0 + ((a & 1) ? du : 0) + ((a & 2) ? dv : 0)];
-            if (s0 < vi.s0 || s0 + ds >= vi.s0 + vi.ns || t0 < vi.t0 || t0 + dt >= vi.t0 + vi.nt) atomicAdd(&g_pass_stats[12], 1ull);
-        }
-#endif
-        vb[a] = cb.x + t0 * cb.y + s0;
-        vs[a] = dt ? cb.y : 0;
-    }
-    return blend16(k, [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// One pass over a (sub-)tile whose rays are set up: ranges (SV), tables + decode (build_patch), gather + blend (C).
-// Returns true (CTA-uniform) when rgb[] holds the pass's pixels (background where the ray misses); false when the
-// tables do not fit the arena and the (sub-)tile must be split.
-template <int kArenaBytes, int kNT>
-__device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, const PixTaps (&pt)[kPPL],
-                                          uint32_t (&rgb)[kPPL])
-{
-    constexpr int PPL = kPPL;
-    const int lane = threadIdx.x & 31;
-    __syncthreads();  // the previous pass's readers of ctl / the patch are done; ctl's accumulators are reset (kernel start / end of the last pass)
-    PHASE_MARK(1);
-
-    // ------------------------------------------------------------ SV: (u,v) range and (s,t) box of the pass's taps
-    int ls0 = 0x7fffffff, lt0 = 0x7fffffff, ls1 = -1, lt1 = -1;
-    int ulo = 0x7fffffff, vlo = 0x7fffffff, uhi = -1, vhi = -1;
-#pragma unroll
-    for (int p = 0; p < PPL; ++p)
-        if (pt[p].uv != kNone) {
-            const int s0 = pt[p].st & 0x3FFF, t0 = (pt[p].st >> 14) & 0x3FFF;
-            ls0 = min(ls0, s0); ls1 = max(ls1, s0 + (int)((pt[p].st >> 28) & 1u));
-            lt0 = min(lt0, t0); lt1 = max(lt1, t0 + (int)((pt[p].st >> 29) & 1u));
-            const int u0 = pt[p].uv & 0xFFF, v0 = (pt[p].uv >> 12) & 0xFFF;
-            ulo = min(ulo, u0); uhi = max(uhi, u0 + (int)((pt[p].uv >> 24) & 1u));
-            vlo = min(vlo, v0); vhi = max(vhi, v0 + (int)((pt[p].uv >> 25) & 1u));
-        }
-    ulo = __reduce_min_sync(FULL, ulo); vlo = __reduce_min_sync(FULL, vlo);
-    uhi = __reduce_max_sync(FULL, uhi); vhi = __reduce_max_sync(FULL, vhi);
-    const int ws0 = __reduce_min_sync(FULL, ls0), wt0 = __reduce_min_sync(FULL, lt0);
-    const int ws1 = __reduce_max_sync(FULL, ls1), wt1 = __reduce_max_sync(FULL, lt1);
-    if (uhi >= 0) {
-        if (lane < 4) atomicMin(&ctl.lo[lane], lane == 0 ? ulo : lane == 1 ? vlo : lane == 2 ? ws0 : wt0);
-        else if (lane < 8) atomicMax(&ctl.hi[lane - 4], lane == 4 ? uhi : lane == 5 ? vhi : lane == 6 ? ws1 : wt1);
-    }
-    __syncthreads();
-    PHASE_MARK(3);
-    const int bu0 = ctl.lo[0], bv0 = ctl.lo[1], bs0 = ctl.lo[2], bt0 = ctl.lo[3];
-    const int bs1 = ctl.hi[2], bt1 = ctl.hi[3];
-    const int nu = ctl.hi[0] - bu0 + 1, nv = ctl.hi[1] - bv0 + 1;
-    bool go = true, done = false;
-    if (ctl.hi[0] < 0) { go = false; done = true; }  // no ray of the sub-tile hits the slab: background only
-    else if (nu > kMaxV || nv > kMaxV) { PASS_STAT(8); go = false; }
-    else {
-        // Early exit before the tables are built: from the pass's exact (u,v) range and (s,t) box, cells ~ (2 ns + nu)
-        // (2 nt + nv) (every pixel touches 2 x 2 views) and accumulator samples ~ cells (level 0) + box area x planes
-        // of every level >= 1.  Only a hint (build_patch decides): a pass that is let through and does not fit is
-        // split after the tables are built, one that is split needlessly costs some halo.
-        const int ns = bs1 - bs0 + 1, nt = bt1 - bt0 + 1;
-        const int area = ns * nt;
-        const int cells = (2 * ns + nu) * (2 * nt + nv) + 16 * nu * nv;
-        int accs = cells;
-        for (int L = 1; L < S.h; ++L)
-            accs += area * ((((bu0 + nu - 1) >> L) - (bu0 >> L) + 1) * (((bv0 + nv - 1) >> L) - (bv0 >> L) + 1));
-        if (16 * cells + 8 * accs > kArenaBytes / 100 * kEstSlackPct) { PASS_STAT(9); go = false; }
-    }
-    if (!go) {
-        __syncthreads();  // every thread has read the ranges
-        reset_ctl(ctl);
-        return done;
-    }
-
-    const bool ok = build_patch<kArenaBytes, kNT>(S, ctl, arena, bu0, bv0, nu, nv, bs0, bs1, bt0, bt1);
-    reset_ctl(ctl);  // behind build_patch's barriers: nobody reads the ranges or the record count any more
-    if (!ok) return false;
-
-    // ------------------------------------------------ C: gather + blend
-    const float4 *patch = reinterpret_cast<const float4 *>(arena + (((size_t)ctl.nacc * 8 + 15) & ~(size_t)15));
-#pragma unroll
-    for (int p = 0; p < PPL; ++p)
-        if (pt[p].uv != kNone) rgb[p] = blend_pixel(ctl, patch, pt[p], bu0, bv0);
-    PHASE_MARK(9);
-    return true;
-}
-
-// ---------------------------------------------------------------- stores
-__device__ __forceinline__ void store4(uint8_t *__restrict__ out, int view, int W, int H, int x0, int y, const uint32_t (&rgb)[4], int out_aligned)
-{
-    if (y >= H || x0 >= W) return;
-    uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x0);
-    if (out_aligned && x0 + 4 <= W) {  // 12 contiguous bytes per thread
-        uint32_t *o32 = reinterpret_cast<uint32_t *>(o);
-        o32[0] = rgb[0] | (rgb[1] << 24);
-        o32[1] = (rgb[1] >> 8) | (rgb[2] << 16);
-        o32[2] = (rgb[2] >> 16) | (rgb[3] << 8);
-    } else {
-#pragma unroll
-        for (int p = 0; p < 4; ++p)
-            if (x0 + p < W) {
-                o[3 * p + 0] = (uint8_t)(rgb[p] & 0xFF);
-                o[3 * p + 1] = (uint8_t)((rgb[p] >> 8) & 0xFF);
-                o[3 * p + 2] = (uint8_t)((rgb[p] >> 16) & 0xFF);
-            }
-    }
-}
-
-// one pixel per lane, 4 consecutive lanes = 4 consecutive pixels of a row: their 12 bytes leave as three 32-bit words
-__device__ __forceinline__ void store1(uint8_t *__restrict__ out, int view, int W, int H, int x, int y, bool active, uint32_t rgb, int out_aligned)
-{
-    const uint32_t nb = __shfl_down_sync(FULL, rgb, 1);
-    if (!active || y >= H || x >= W) return;
-    uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x);
-    if (out_aligned) {  // W % 4 == 0 and x % 4 == lane % 4: the group's 4 pixels are all inside the view
-        const int j = x & 3;
-        if (j < 3) {
-            const uint32_t w = j == 0 ? (rgb | (nb << 24)) : j == 1 ? ((rgb >> 8) | (nb << 16)) : ((rgb >> 16) | (nb << 8));
-            reinterpret_cast<uint32_t *>(o - 3 * j)[j] = w;
-        }
-    } else {
-        o[0] = (uint8_t)(rgb & 0xFF);
-        o[1] = (uint8_t)((rgb >> 8) & 0xFF);
-        o[2] = (uint8_t)((rgb >> 16) & 0xFF);
-    }
-}
-
-// s = aff[0] + aff[1] * u (index units) for every ray of the camera along one axis, and the margin aff[2] of that relation between
-// the fp32 values the ray set-up computes.  u_w = e + l0 D, s_w = e + l1 D with l0 = (0 - ez) / Dz, l1 = (z_st - ez) / Dz, so
-// s_w - e = k (u_w - e) with k = (z_st - ez) / (0 - ez) whatever D is.  The margin covers the dozen roundings of either chain (64 ulps of
-// the magnitudes involved) and the fp32 evaluation of aff[0] + aff[1] * u itself; a box that is a sample too wide costs a few decodes,
-// one that is too narrow would be wrong.
-__device__ __forceinline__ void camera_affine(const DevStream &S, const Camera &cam, int axis, float (&aff)[4])
-{
-    const float e = cam.eye[axis], ez = cam.eye[2];
-    const float uo = S.uv_origin[axis], us = S.uv_step[axis], so = S.st_origin[axis], ss = S.st_step[axis];
-    const float k = (S.z_st - ez) / (0.0f - ez), rs = 1.0f / ss;
-    const float beta = k * us * rs;
-    const float n_uv = (float)(axis == 0 ? S.U : S.V), n_st = (float)(axis == 0 ? S.Ws : S.Ht);
-    const float mw = fmaxf(fmaxf(fabsf(e), fabsf(uo) + fabsf(us) * n_uv), fmaxf(fabsf(so) + fabsf(ss) * n_st, 1.0f));
-    const float mag = (fabsf(e - so) + fabsf(k) * fabsf(uo - e)) * fabsf(rs) + fabsf(beta) * (n_uv + 2.0f);  // terms of aff[0] + aff[1] u
-    aff[0] = ((e - so) + k * (uo - e)) * rs;
-    aff[1] = beta;
-    aff[2] = 64.0f * 5.9604644775390625e-8f * (n_st + mw * fabsf(rs) + fabsf(beta) * (n_uv + mw / fabsf(us)) + mag) + 1e-5f;
-    aff[3] = 0.0f;
-}
-
 template <int kArenaBytes, int kMinBlocks, int kNT, int kTW>
 __global__ void __launch_bounds__(kNT, kMinBlocks)
 render_cta_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned)
 {
-    constexpr int kTH = kNT * kPPL / kTW;
-    constexpr int kLMax = kTW == 64 && kTH == 64 ? 3 : 2;  // quadtree levels below the tile: the smallest sub-tile is 8 pixels wide or high
     extern __shared__ __align__(16) unsigned char arena[];
     __shared__ Ctl ctl;
     const int tid = threadIdx.x;
     const int view = blockIdx.z;
-
     for (int q = tid; q < 192; q += kNT)
         reinterpret_cast<uint32_t *>(ctl.lut)[q] = reinterpret_cast<const uint32_t *>(g_cta_digit_lut.v)[q];
     reset_ctl(ctl);
     // the camera goes to shared memory (16 registers per thread otherwise, or reloads from global memory in every pass)
     if (tid < 16) reinterpret_cast<float *>(&ctl.cam)[tid] = reinterpret_cast<const float *>(cams + view)[tid];
     __syncthreads();
-    const Camera &cam = ctl.cam;
-    if (tid < 2) camera_affine(S, cam, tid, ctl.aff[tid]);
-    const uint32_t bg = (uint32_t)S.bg[0] | ((uint32_t)S.bg[1] << 8) | ((uint32_t)S.bg[2] << 16);
-
-    // ---------------------------------------------------------------- passes: the whole tile (4 pixels per thread); if it does not fit
-    // (low magnification: more light-field samples than output pixels under the tile), its four quadrants with one pixel per thread, each
-    // split again when it does not fit; a sub-tile of the last level that still does not fit (strong minification) is rendered by 16 direct
-    // sample decodes per pixel.  path = child index (2 bits) of every level on the way down.
-    int lvl = 0;
-    uint32_t path = 0u;
-    for (;;) {
-        int sx = blockIdx.x * kTW, sy = blockIdx.y * kTH;
-        for (int l = 1; l <= lvl; ++l) {
-            const uint32_t c = (path >> (2 * (l - 1))) & 3u;
-            sx += (int)(c & 1u) * (kTW >> l); sy += (int)(c >> 1) * (kTH >> l);
-        }
-        const bool full = lvl == 0;
-        const int lpw = 31 - __clz(kTW >> lvl), npx = (kTW >> lvl) * (kTH >> lvl);
-        bool done = true;
-        if (sx < W && sy < H) {
-            PixTaps pt[kPPL];
-            uint32_t rgb[kPPL];
-#pragma unroll
-            for (int p = 0; p < kPPL; ++p) rgb[p] = bg;
-            PHASE_MARK(-1);
-            setup_rays<kTW>(S, cam, W, H, sx, sy, full, lpw, npx, pt);
-            PHASE_MARK(0);
-            PASS_STAT(lvl);
-            done = tile_pass<kArenaBytes, kNT>(S, ctl, arena, pt, rgb);
-            if (done) PASS_STAT(4 + lvl);
-            if (!done && lvl == kLMax) {
-                PASS_STAT(13);
-                if (pt[0].uv != kNone) rgb[0] = direct_pixel(S, pt[0]);
-                done = true;
-            }
-            if (done) {
-                int x0, y, npix;
-                thread_pixel<kTW>(sx, sy, full, lpw, npx, x0, y, npix);
-                if (full) store4(out, view, W, H, x0, y, rgb, out_aligned);
-                else store1(out, view, W, H, x0, y, npix > 0, rgb[0], out_aligned);
-                PHASE_MARK(10);
-            }
-        }
-        if (!done) { ++lvl; path &= ~(3u << (2 * (lvl - 1))); continue; }  // descend to the first child
-        while (lvl > 0 && ((path >> (2 * (lvl - 1))) & 3u) == 3u) --lvl;       // last child done: back to the parent's level
-        if (lvl == 0) break;
-        path += 1u << (2 * (lvl - 1));
-    }
+    if (tid < 2) camera_affine(S, ctl.cam, tid, ctl.aff[tid]);
+    render_tile_general<kArenaBytes, kNT, kTW>(S, ctl, arena, W, H, out, out_aligned, view, (int)blockIdx.x, (int)blockIdx.y);
 }
 
 }  // namespace
@@ -807,9 +50,9 @@ extern "C" int hmlfc_debug_pass_stats(unsigned long long *out, int reset)
 }
 #endif
 
-// Shared memory per SM: 233,472 bytes, 1 KB reserved per resident CTA, 9.6 KB of tables (Ctl) per CTA; the rest is the arena.
-//   0: 256 threads, 32 x 32 tile, 3 CTAs x 66 KB     1: 256 threads, 32 x 32 tile, 2 CTAs x 104 KB (views that look at about as many
-//   2: 256 threads, 32 x 32 tile, 4 CTAs x 47 KB        light-field samples as they have pixels: far fewer tiles are split)
+// Shared memory per SM: 233,472 bytes, 1 KB reserved per resident CTA, 9.4 KB of tables (Ctl) per CTA; the rest is the arena.
+//   0: 256 threads, 32 x 32 tile, 3 CTAs x 65 KB     1: 256 threads, 32 x 32 tile, 2 CTAs x 103 KB (views that look at about as many
+//   2: 256 threads, 32 x 32 tile, 4 CTAs x 46 KB        light-field samples as they have pixels: far fewer tiles are split)
 //   3: 1024 threads, 64 x 64 tile, 1 CTA x 200 KB    4: 512 threads, 64 x 32 tile, 2 CTAs x 100 KB
 #ifndef HMLFC_ARENA3_KB
 #define HMLFC_ARENA3_KB 200
@@ -818,9 +61,9 @@ extern "C" int hmlfc_debug_pass_stats(unsigned long long *out, int reset)
 #define HMLFC_ARENA4_KB 100
 #endif
 #define HMLFC_CTA_CONFIGS(X) \
-    X(0, 66 * 1024, 3, 256, 32) \
-    X(1, 104 * 1024, 2, 256, 32) \
-    X(2, 47 * 1024, 4, 256, 32) \
+    X(0, 65 * 1024, 3, 256, 32) \
+    X(1, 103 * 1024, 2, 256, 32) \
+    X(2, 46 * 1024, 4, 256, 32) \
     X(3, HMLFC_ARENA3_KB * 1024, 1, 1024, 64) \
     X(4, HMLFC_ARENA4_KB * 1024, 2, 512, 64)
 
