@@ -149,13 +149,17 @@ int hmlfc_footprint_render(hmlfc_handle *h, const hmlfc_camera *d_cameras, int n
 int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, hmlfc_footprint_t *out);
 
 /* Kernel selection for hmlfc_render (A/B measurements and cross-checks; all variants produce identical
- * bytes): 0 = automatic (default: 6, 7 or 8 for B = 4 streams, else 4), 1 = one thread per output pixel (16
- * independent tap decodes -- the unshared definition, kept as the cross-check), 4 / 5 = a
- * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile, 6 / 7 / 8 = CTA per 32 x 32 tile with
- * per-view footprint boxes and block-ROW tasks (4 BISE values per lane from two 64-bit windows), with a
- * 68 KB (3 CTAs per SM) / 104 KB (2 CTAs per SM) / 50 KB (4 CTAs per SM) shared-memory arena; the automatic
- * choice takes 7 when a view has fewer than twice the pixels of a light-field image (little magnification:
- * more samples per tile), 8 when it has at least eight times as many, else 6. */
+ * bytes): 0 = automatic (default; for B = 4 streams 11, 12 or 7 as described below, else 4), 1 = one thread per
+ * output pixel (16 independent tap decodes -- the unshared definition, kept as the cross-check), 4 / 5 = a
+ * block-centric pipeline run by ONE WARP per 16 x 8 / 8 x 8 tile.  The two fused kernels for 4 x 4 blocks
+ * (per-view footprint boxes, block-ROW tasks: 4 BISE values per lane from two 64-bit windows):
+ * 6 .. 10 = the general kernel (tile tables built inside the CTA, quadtree of sub-tile passes): 256 threads per
+ * 32 x 32 tile with a 65 KB (3 CTAs per SM) / 103 KB (2) / 46 KB (4) shared-memory arena, 1024 threads per
+ * 64 x 64 tile, 512 threads per 64 x 32 tile; 11 / 12 = the tile kernel (tables of all tiles from a kernel of
+ * their own, one pass per 32 x 32 tile, 3 / 4 CTAs per SM; two launches per call and a scratch buffer from the
+ * library's stream-ordered pool).  The automatic choice takes 7 when a view has fewer than twice the pixels of
+ * a light-field image (little magnification: many samples per tile), 12 when it has at least eight times as
+ * many, else 11. */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Progressive decoding (PAPER.md:57, :183 name the property; R26): hmlfc_decode / hmlfc_render sum the top-level RKV and the

@@ -13,10 +13,6 @@
 
 using namespace hmlfc;
 
-#ifndef HMLFC_TILES_DEFAULT
-#define HMLFC_TILES_DEFAULT 0
-#endif
-
 struct hmlfc_handle {
     DevStream ds{};
     hmlfc_info_t info{};
@@ -260,7 +256,9 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
         // kernel with its largest arena, the others to the tile kernel (tables from a kernel of their own); 6 .. 10: the general kernel's five
         // configurations; 11 / 12: the tile kernel with 3 / 4 CTAs per SM.  All give identical bytes.
         int tiles = rv == 11 ? 0 : rv == 12 ? 1 : -1;
-        if (rv == 0 && (long long)W * H >= 2LL * h->ds.Ws * h->ds.Ht) tiles = HMLFC_TILES_DEFAULT;
+        // measured (ms per step, tile kernel with 3 / 4 CTAs per SM against the general kernel's best configuration): cfg2 0.67 / 0.95 /
+        // 0.81, cfg4 0.91 / 1.27 / 1.04, cfg5 1.22 / 1.10 / 1.45; cfg3 (about one sample per pixel) 1.14 / 1.37 / 0.85
+        if (rv == 0 && (long long)W * H >= 2LL * h->ds.Ws * h->ds.Ht) tiles = (long long)W * H >= 8LL * h->ds.Ws * h->ds.Ht ? 1 : 0;
         if (tiles >= 0) {
             void *scratch = nullptr;
             cudaMemPool_t pool;

@@ -255,7 +255,9 @@ HMLFC_DEV Ray ray_setup(const DevStream &S, const Camera &cam, int W, int H, int
     return ray_from_screen(S, cam, ray_screen(cam.tan_half_x, W, i), ray_screen(cam.tan_half_y, H, j));
 }
 
-HMLFC_DEV Ray ray_from_screen(const DevStream &S, const Camera &cam, float px, float py)
+// kAllPow2: all four steps are powers of two (pow2_mask == 15): the divisions by the steps are multiplications, without the test
+template <bool kAllPow2>
+HMLFC_DEV Ray ray_from_screen_t(const DevStream &S, const Camera &cam, float px, float py)
 {
     Ray r;
     r.hit = false;
@@ -270,16 +272,21 @@ HMLFC_DEV Ray ray_from_screen(const DevStream &S, const Camera &cam, float px, f
     float vw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l0, Dy));
     float sw = HMLFC_ADD(cam.eye[0], HMLFC_MUL(l1, Dx));
     float tw = HMLFC_ADD(cam.eye[1], HMLFC_MUL(l1, Dy));
-    float u = div_step(HMLFC_SUB(uw, S.uv_origin[0]), S.uv_step[0], S.uv_inv[0], S.pow2_mask & 1u);
-    float v = div_step(HMLFC_SUB(vw, S.uv_origin[1]), S.uv_step[1], S.uv_inv[1], S.pow2_mask & 2u);
-    float s = div_step(HMLFC_SUB(sw, S.st_origin[0]), S.st_step[0], S.st_inv[0], S.pow2_mask & 4u);
-    float t = div_step(HMLFC_SUB(tw, S.st_origin[1]), S.st_step[1], S.st_inv[1], S.pow2_mask & 8u);
+    float u = div_step(HMLFC_SUB(uw, S.uv_origin[0]), S.uv_step[0], S.uv_inv[0], kAllPow2 || (S.pow2_mask & 1u));
+    float v = div_step(HMLFC_SUB(vw, S.uv_origin[1]), S.uv_step[1], S.uv_inv[1], kAllPow2 || (S.pow2_mask & 2u));
+    float s = div_step(HMLFC_SUB(sw, S.st_origin[0]), S.st_step[0], S.st_inv[0], kAllPow2 || (S.pow2_mask & 4u));
+    float t = div_step(HMLFC_SUB(tw, S.st_origin[1]), S.st_step[1], S.st_inv[1], kAllPow2 || (S.pow2_mask & 8u));
     if (!(u >= 0.0f && u <= (float)(S.U - 1) && v >= 0.0f && v <= (float)(S.V - 1) && s >= 0.0f &&
           s <= (float)(S.Ws - 1) && t >= 0.0f && t <= (float)(S.Ht - 1)))
         return r;
     r.hit = true;
     r.u = u; r.v = v; r.s = s; r.t = t;
     return r;
+}
+
+HMLFC_DEV Ray ray_from_screen(const DevStream &S, const Camera &cam, float px, float py)
+{
+    return ray_from_screen_t<false>(S, cam, px, py);
 }
 
 // 16-tap enumeration: base indices, +1 neighbours clamped to the edge, fractional weights

@@ -79,7 +79,8 @@ struct TileHeader {  // 64 bytes
     int bs0, bs1, bt0, bt1;      // (s,t) box of all its taps
     int nslots, ncell, nacc, nbhmax;
     int status;                  // kTile*: what the tile's pass has to do
-    int _pad[3];
+    uint32_t m_ps, m_nbh;        // magic multipliers of 3 * nbhmax and nbhmax (B1's item -> (slot, channel, block row))
+    int _pad;
 };
 constexpr int kTileBackground = 0;  // no ray hits the slab
 constexpr int kTileTables = 1;      // tables valid
@@ -123,11 +124,11 @@ __device__ __forceinline__ uint32_t round_rgb(float r, float g, float b)
 
 // quadrilinear blend of 16 float RGB taps fetched by fetch(a, b): a = view (bit0 u, bit1 v), b = pixel (bit0 s, bit1 t)
 template <typename Fetch>
-__device__ __forceinline__ uint32_t blend16(const PixTaps &k, Fetch fetch)
+__device__ __forceinline__ uint32_t blend16(float fu, float fv, float fs, float ft, Fetch fetch)
 {
-    const float ws0 = 1.0f - k.fs, wt0 = 1.0f - k.ft, wu0 = 1.0f - k.fu, wv0 = 1.0f - k.fv;
-    const float wst[4] = {ws0 * wt0, k.fs * wt0, ws0 * k.ft, k.fs * k.ft};
-    const float wuv[4] = {wu0 * wv0, k.fu * wv0, wu0 * k.fv, k.fu * k.fv};
+    const float ws0 = 1.0f - fs, wt0 = 1.0f - ft, wu0 = 1.0f - fu, wv0 = 1.0f - fv;
+    const float wst[4] = {ws0 * wt0, fs * wt0, ws0 * ft, fs * ft};
+    const float wuv[4] = {wu0 * wv0, fu * wv0, wu0 * fv, fu * fv};
     float2 accRG = make_float2(0.f, 0.f), accB = make_float2(0.f, 0.f);
 #pragma unroll
     for (int a = 0; a < 4; ++a) {
@@ -155,10 +156,19 @@ __device__ __noinline__ uint32_t direct_pixel(const DevStream &S, const PixTaps 
     uint32_t c8[16];
 #pragma unroll 1
     for (int a = 0; a < 16; ++a) c8[a] = decode_rgb8(S, (a & 4) ? u1 : u0, (a & 8) ? v1 : v0, (a & 1) ? s1 : s0, (a & 2) ? t1 : t0);
-    return blend16(k, [&](int a, int b) {
+    return blend16(k.fu, k.fv, k.fs, k.ft, [&](int a, int b) {
         const uint32_t c = c8[a * 4 + b];
         return make_float4((float)(c & 0xFFu), (float)((c >> 8) & 0xFFu), (float)((c >> 16) & 0xFFu), 0.f);
     });
+}
+
+__device__ __forceinline__ PixTaps pack_taps(const Taps &k)
+{
+    PixTaps t;
+    t.uv = (uint32_t)k.u0 | ((uint32_t)k.v0 << 12) | ((uint32_t)(k.u1 - k.u0) << 24) | ((uint32_t)(k.v1 - k.v0) << 25);
+    t.st = (uint32_t)k.s0 | ((uint32_t)k.t0 << 14) | ((uint32_t)(k.s1 - k.s0) << 28) | ((uint32_t)(k.t1 - k.t0) << 29);
+    t.fu = k.fu; t.fv = k.fv; t.fs = k.fs; t.ft = k.ft;
+    return t;
 }
 
 // 16-tap footprint of the pixel with screen coordinates (px, py)
@@ -171,9 +181,7 @@ __device__ __forceinline__ PixTaps pixel_taps(const DevStream &S, const Camera &
         const Ray r = ray_from_screen(S, cam, px, py);
         if (r.hit) {
             const Taps k = tap_setup(S, r);
-            t.uv = (uint32_t)k.u0 | ((uint32_t)k.v0 << 12) | ((uint32_t)(k.u1 - k.u0) << 24) | ((uint32_t)(k.v1 - k.v0) << 25);
-            t.st = (uint32_t)k.s0 | ((uint32_t)k.t0 << 14) | ((uint32_t)(k.s1 - k.s0) << 28) | ((uint32_t)(k.t1 - k.t0) << 29);
-            t.fu = k.fu; t.fv = k.fv; t.fs = k.fs; t.ft = k.ft;
+            t = pack_taps(k);
         }
     }
     return t;
@@ -182,12 +190,12 @@ __device__ __forceinline__ PixTaps pixel_taps(const DevStream &S, const Camera &
 // C for one pixel: its 16 taps from the patch, blended.  kGuard: a tap outside its view's box (the tables came from a
 // conservative estimate of the tile's footprint, hmlfc_render_tiles.cu) sends the pixel to the direct decode instead.
 template <bool kGuard>
-__device__ __forceinline__ uint32_t blend_pixel(const DevStream &S, const Ctl &ctl, const float4 *__restrict__ patch, const PixTaps k, int bu0, int bv0)
+__device__ __forceinline__ uint32_t blend_taps(const DevStream &S, const Ctl &ctl, const float4 *__restrict__ patch, const Taps &k, int bu0, int bv0)
 {
-    const int iu = (int)(k.uv & 0xFFF) - bu0, iv = (int)((k.uv >> 12) & 0xFFF) - bv0;
-    const int s0 = (int)(k.st & 0x3FFF), t0 = (int)((k.st >> 14) & 0x3FFF);
-    const int du = (int)((k.uv >> 24) & 1u), dv = ((k.uv >> 25) & 1u) ? 4 : 0;
-    const int ds = (int)((k.st >> 28) & 1u), dt = (int)((k.st >> 29) & 1u);
+    const int iu = k.u0 - bu0, iv = k.v0 - bv0;
+    const int s0 = k.s0, t0 = k.t0;
+    const int du = k.u1 - k.u0, dv = (k.v1 - k.v0) << 2;
+    const int ds = k.s1 - k.s0, dt = k.t1 - k.t0;
     const int vw0 = iv * 4 + iu;
     if (kGuard) {
         // a view's box is (its column's sample columns) x (its row's sample rows): two interval tests per axis cover the four views
@@ -200,7 +208,7 @@ __device__ __forceinline__ uint32_t blend_pixel(const DevStream &S, const Ctl &c
 #ifdef HMLFC_PASS_STATS
             atomicAdd(&g_pass_stats[12], 1ull);
 #endif
-            return direct_pixel(S, k);
+            return direct_pixel(S, pack_taps(k));
         }
     }
     int vb[4], vs[4];
@@ -216,7 +224,17 @@ __device__ __forceinline__ uint32_t blend_pixel(const DevStream &S, const Ctl &c
         vb[a] = cb.x + t0 * cb.y + s0;
         vs[a] = dt ? cb.y : 0;
     }
-    return blend16(k, [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
+    return blend16(k.fu, k.fv, k.fs, k.ft, [&](int a, int b) { return patch[vb[a] + ((b & 1) ? ds : 0) + ((b & 2) ? vs[a] : 0)]; });
+}
+
+__device__ __forceinline__ uint32_t blend_pixel(const DevStream &S, const Ctl &ctl, const float4 *__restrict__ patch, const PixTaps k, int bu0, int bv0)
+{
+    Taps t;
+    t.u0 = (int)(k.uv & 0xFFF); t.v0 = (int)((k.uv >> 12) & 0xFFF); t.s0 = (int)(k.st & 0x3FFF); t.t0 = (int)((k.st >> 14) & 0x3FFF);
+    t.u1 = t.u0 + (int)((k.uv >> 24) & 1u); t.v1 = t.v0 + (int)((k.uv >> 25) & 1u);
+    t.s1 = t.s0 + (int)((k.st >> 28) & 1u); t.t1 = t.t0 + (int)((k.st >> 29) & 1u);
+    t.fu = k.fu; t.fv = k.fv; t.fs = k.fs; t.ft = k.ft;
+    return blend_taps<false>(S, ctl, patch, t, bu0, bv0);
 }
 
 // Footprint interval along one axis of the views / planes that cover grid positions [a0, a1] of that axis: the pixels that touch
@@ -358,7 +376,10 @@ __device__ __forceinline__ void build_slot_table(const DevStream &S, const float
             nbhmax = max(nbhmax, __reduce_max_sync(FULL, si.nbh));
         }
     }
-    if (lane == 0) { tab.hdr.nslots = nslots; tab.hdr.nacc = accrun; tab.hdr.nbhmax = nbhmax; }
+    if (lane == 0) {
+        tab.hdr.nslots = nslots; tab.hdr.nacc = accrun; tab.hdr.nbhmax = nbhmax;
+        tab.hdr.m_ps = magic_of((uint32_t)(3 * nbhmax)); tab.hdr.m_nbh = magic_of((uint32_t)nbhmax);
+    }
 }
 
 // do the tables fit an arena of kArenaBytes?  accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by
@@ -390,15 +411,16 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
     float4 *patch = reinterpret_cast<float4 *>(region2);  // [ncell], after the records are dead
     // ---------------------------------------------------- zero the accumulators; per-view cell offsets, chunk -> view, accumulator
     // offsets of every (view, level); the planes' descriptors (and their reference planes') go to shared memory for B2 and B3
+    static_assert(6 * kMaxSlots <= 256 && kNT >= 256, "one descriptor per thread");
+    uint4 dsc = make_uint4(0u, 0u, 0u, 0u);
     {
         uint4 *z = reinterpret_cast<uint4 *>(arena);
         const int nz = (nacc + 1) >> 1;
         for (int q = zero_from + tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);
-        for (int q = tid; q < nslots * 6; q += kNT) {
-            const uint32_t s = fdiv((uint32_t)q, 0x2AAAAAABu), j = (uint32_t)q - 6u * s;  // q / 6
+        if (tid < nslots * 6) {  // loaded now, stored behind B1 (6 * kMaxSlots <= 256 threads): B1 does not wait for them
+            const uint32_t s = fdiv((uint32_t)tid, 0x2AAAAAABu), j = (uint32_t)tid - 6u * s;  // tid / 6
             const SlotInfo &sl = ctl.tab.slot[s];
-            if (j < 3u) ctl.desc[s][j] = ldg(S.pc + sl.pc0 + j);
-            else ctl.rdesc[s][j - 3u] = ldg(S.pc + sl.refpc0 + (j - 3u));
+            dsc = ldg(S.pc + (j < 3u ? sl.pc0 + j : sl.refpc0 + (j - 3u)));
         }
         for (int q = tid; q < kMaxViews * h; q += kNT) {
             const int L = q >> 4, vw = q & 15;
@@ -422,7 +444,7 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
     // ---------------------------------------------------- B1: one lane per (slot, channel, block row): flag words -> records
     {
         const int per_slot = 3 * nbhmax, nitems = nslots * per_slot;
-        const uint32_t m_ps = magic_of((uint32_t)per_slot), m_nbh = magic_of((uint32_t)nbhmax);
+        const uint32_t m_ps = hd.m_ps, m_nbh = hd.m_nbh;
         for (int base = 0; base < nitems; base += kNT) {
             const int it = base + tid;
             bool on = it < nitems;
@@ -484,6 +506,10 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
             }
         }
     }
+    if (tid < nslots * 6) {
+        const uint32_t s = fdiv((uint32_t)tid, 0x2AAAAAABu), j = (uint32_t)tid - 6u * s;
+        if (j < 3u) ctl.desc[s][j] = dsc; else ctl.rdesc[s][j - 3u] = dsc;
+    }
     __syncthreads();
     PHASE_MARK(5);
     const int nrec = ctl.n_rec;
@@ -492,21 +518,23 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
         __syncthreads();  // every thread has read the record count (the caller resets it)
         return false;
     }
-    // ------------------------------------------------ B2: motion record, once per block
-    for (int rr = tid; rr < nrec; rr += kNT) {
-        const uint4 r0 = rec[rr];
-        uint32_t mvp = 0u;
-        if (r0.y != kNone) {
-            const uint32_t mr = bise_at(S.mv + ctl.desc[r0.z & 63u][(r0.z >> 6) & 3u].z, r0.y, S.mv_layout, S.mv_m, ctl.lut);
-            int md, dx, dy;
-            mv_unpack(S, mr, md, dx, dy);
-            mvp = 0x80000000u | ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+    // ------------------------------------------------ B2: motion record, once per block.  With few records (B3 is one or two rounds of
+    // latency) the four row lanes of a block decode it themselves in B3 -- the same loads, the same instructions: what one lane would cost,
+    // and a barrier less; with many (B3 is bound by instruction issue) one lane per record decodes it here.
+    const bool fuse_b2 = 4 * nrec <= 3 * kNT;
+    if (!fuse_b2) {
+        for (int rr = tid; rr < nrec; rr += kNT) {
+            const uint4 r0 = rec[rr];
+            if (r0.y != kNone) {
+                int md, dx, dy;
+                mv_unpack(S, bise_at(S.mv + ctl.desc[r0.z & 63u][(r0.z >> 6) & 3u].z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
+                rec[rr].y = ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+            }
         }
-        rec[rr].y = mvp;
+        __syncthreads();
     }
-    __syncthreads();
     PHASE_MARK(6);
-    // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values (neighbouring
+    // ------------------------------------------------ B2 + B3: one lane per (record, block row): 4 stored / re-compensated values (neighbouring
     // lanes work on neighbouring blocks of one plane: their payload words share sectors and they take the same branches)
     {
         int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
@@ -519,14 +547,18 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
             const int st0 = sl.t0, st1 = sl.t1;
             if (yy < st0 || yy > st1) continue;
             const int xx = (int)((r0.z >> 20) << 2);
-            uint2 own = make_uint2(0u, 0u);
-            if (r0.x != kNone) {
-                const uint4 d = ctl.desc[s][c];
-                own = bise_row4(S.pay + d.y, r0.x + (uint32_t)(ky << 2), d.w, ctl.lut);
+            const uint4 d = ctl.desc[s][c];
+            // the motion record (B2)
+            int md = 0, dx = 0, dy = 0;
+            if (r0.y != kNone) {
+                if (fuse_b2) mv_unpack(S, bise_at(S.mv + d.z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
+                else { md = (int)((r0.y >> 16) & 1u); dx = (int)((r0.y >> 8) & 0xFFu) - S.W; dy = (int)(r0.y & 0xFFu) - S.W; }
             }
+            uint2 own = make_uint2(0u, 0u);
+            if (r0.x != kNone) own = bise_row4(S.pay + d.y, r0.x + (uint32_t)(ky << 2), d.w, ctl.lut);
             int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
-            if (r0.y) {
-                const int rx = xx + (int)((r0.y >> 8) & 0xFFu) - S.W, ry = yy + (int)(r0.y & 0xFFu) - S.W;
+            if (r0.y != kNone) {
+                const int rx = xx + dx, ry = yy + dy;
                 if ((unsigned)ry < (unsigned)S.Ht) {
                     // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
                     const uint4 dr = ctl.rdesc[s][c];
@@ -534,8 +566,8 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                     const uint32_t i0 = (uint32_t)((ry & 3) << 2);
                     const int rowb = (ry >> 2) * S.nbx;
                     uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-#pragma unroll 1
-                    for (int j = 0; j < 2; ++j) {  // a loop on purpose: one instance of the row decode (instruction cache)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
                         uint2 q = make_uint2(0u, 0u);
                         if ((j == 0 || o) && (unsigned)(bxa + j) < (unsigned)S.nbx) {
                             const int b = rowb + bxa + j;
@@ -552,7 +584,7 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                     const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
                     const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
                     // R10: subtractive P = e + R, additive P = e - R
-                    if (r0.y & 0x10000u) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
+                    if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
                     else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
                 }
             }
@@ -574,14 +606,32 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
         const uint32_t it = fdiv(local, vi.m_ns), is = local - it * (uint32_t)vi.ns;
         if ((int)it >= vi.nt) continue;  // padding of the view's last chunk
         const unsigned long long ro = ((unsigned long long)vi.rkv_hi << 32) | vi.rkv_lo;
-        const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
+                const short4 rk = ldg(S.rkv + ro + (uint32_t)((vi.t0 + (int)it) * S.Ws + vi.s0 + (int)is));
         int a[3] = {rk.x, rk.y, rk.z};
-        for (int L = S.lmin; L < h; ++L) {
-            const int2 vo = ctl.voff[vw][L];
-            const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
-            a[0] += (int)(int16_t)(w.x & 0xFFFFu);
-            a[1] += (int)w.x >> 16;
-            a[2] += (int)(int16_t)(w.y & 0xFFFFu);
+        if (h <= 4) {  // the usual heights: the levels' loads issue together
+            uint2 w[4];
+#pragma unroll
+            for (int L = 0; L < 4; ++L) {
+                w[L] = make_uint2(0u, 0u);
+                if (L >= S.lmin && L < h) {
+                    const int2 vo = ctl.voff[vw][L];
+                    w[L] = acc[vo.x + (int)it * vo.y + (int)is];
+                }
+            }
+#pragma unroll
+            for (int L = 0; L < 4; ++L) {
+                a[0] += (int)(int16_t)(w[L].x & 0xFFFFu);
+                a[1] += (int)w[L].x >> 16;
+                a[2] += (int)(int16_t)(w[L].y & 0xFFFFu);
+            }
+        } else {
+            for (int L = S.lmin; L < h; ++L) {
+                const int2 vo = ctl.voff[vw][L];
+                const uint2 w = acc[vo.x + (int)it * vo.y + (int)is];
+                a[0] += (int)(int16_t)(w.x & 0xFFFFu);
+                a[1] += (int)w.x >> 16;
+                a[2] += (int)(int16_t)(w.y & 0xFFFFu);
+            }
         }
         const uint32_t c8 = ycocg_to_rgb8(a);
         // the patch aliases the record list: all B3 readers passed the barrier above
@@ -769,7 +819,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     const float4 *patch = reinterpret_cast<const float4 *>(arena + (((size_t)ctl.tab.hdr.nacc * 8 + 15) & ~(size_t)15));
 #pragma unroll
     for (int p = 0; p < PPL; ++p)
-        if (pt[p].uv != kNone) rgb[p] = blend_pixel<false>(S, ctl, patch, pt[p], bu0, bv0);
+        if (pt[p].uv != kNone) rgb[p] = blend_pixel(S, ctl, patch, pt[p], bu0, bv0);
     PHASE_MARK(9);
     return true;
 }

@@ -120,7 +120,7 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     if (status != kTileTables) {
         if (lane == 0) {
             TileHeader hd = rg;
-            hd.nslots = hd.ncell = hd.nacc = hd.nbhmax = 0; hd.status = status; hd._pad[0] = hd._pad[1] = hd._pad[2] = 0;
+            hd.nslots = hd.ncell = hd.nacc = hd.nbhmax = 0; hd.status = status; hd.m_ps = hd.m_nbh = 0u; hd._pad = 0;
             *reinterpret_cast<TileHeader *>(dst) = hd;
         }
         return;
@@ -131,7 +131,7 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     __syncwarp();
     if (lane == 0) {
         tab.hdr.status = tab.hdr.nslots <= kMaxSlots ? kTileTables : kTileGeneral;
-        tab.hdr._pad[0] = tab.hdr._pad[1] = tab.hdr._pad[2] = 0;
+        tab.hdr._pad = 0;
     }
     __syncwarp();
     const int nwords = kTableHeadWords + (tab.hdr.nslots <= kMaxSlots ? 4 * tab.hdr.nslots : 0);
@@ -139,8 +139,16 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     for (int q = lane; q < nwords; q += 32) dst[q] = src[q];
 }
 
+// the general path as a call: its registers and spills stay out of the tile kernel's own allocation (the call is rare)
+template <int kArenaBytes>
+__device__ __noinline__ void general_tile_call(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int W, int H, uint8_t *__restrict__ out,
+                                               int out_aligned, int view, int tile_x, int tile_y)
+{
+    render_tile_general<kArenaBytes, 256, kTile>(S, ctl, arena, W, H, out, out_aligned, view, tile_x, tile_y);
+}
+
 // ---------------------------------------------------------------------------------------------------------------
-template <int kArenaBytes, int kMinBlocks>
+template <int kArenaBytes, int kMinBlocks, bool kAllPow2>
 __global__ void __launch_bounds__(256, kMinBlocks)
 render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned,
                     const uint4 *__restrict__ tables)
@@ -155,7 +163,10 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
     PHASE_MARK(-1);
 
     // every thread reads the header itself (one broadcast transaction per warp); meanwhile the digit table and the camera
+    // (and, before the header says how many there are, one word of the tables per thread: a table has at most 200 words)
     TileHeader hd;
+    static_assert(kDescWords <= 256, "one table word per thread");
+    const uint4 spec = tid < kDescWords ? ldg(td + tid) : make_uint4(0u, 0u, 0u, 0u);
     {
         uint4 *h4 = reinterpret_cast<uint4 *>(&hd);
         h4[0] = ldg(td); h4[1] = ldg(td + 1); h4[2] = ldg(td + 2); h4[3] = ldg(td + 3);
@@ -175,7 +186,8 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
     if (fast) {
         const int nwords = kTableHeadWords + 4 * hd.nslots;
         uint4 *dst = reinterpret_cast<uint4 *>(&ctl.tab);
-        for (int q = tid; q < nwords; q += kNT) dst[q] = ldg(td + q);
+        if (tid < nwords) dst[tid] = spec;
+        for (int q = tid + kNT; q < nwords; q += kNT) dst[q] = ldg(td + q);
         uint4 *z = reinterpret_cast<uint4 *>(arena);
         const int nz = (hd.nacc + 1) >> 1;
         for (int q = tid; q < nz; q += kNT) z[q] = make_uint4(0u, 0u, 0u, 0u);
@@ -184,10 +196,11 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
     PHASE_MARK(4);
     if (fast) fast = decode_patch<kArenaBytes, kNT>(S, ctl, arena, 0x7fffffff - kNT);
     if (!fast) {
+        PASS_STAT(hd.status != kTileTables ? 14 : 15);
         // irregular rays, more than 4 x 4 views, or tables / records that do not fit the arena: the general path, in this CTA
         reset_ctl(ctl);
         if (tid < 2) camera_affine(S, ctl.cam, tid, ctl.aff[tid]);
-        render_tile_general<kArenaBytes, kNT, kTile>(S, ctl, arena, W, H, out, out_aligned, view, (int)blockIdx.x, (int)blockIdx.y);
+        general_tile_call<kArenaBytes>(S, ctl, arena, W, H, out, out_aligned, view, (int)blockIdx.x, (int)blockIdx.y);
         return;
     }
 
@@ -205,8 +218,11 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
 #pragma unroll
     for (int p = 0; p < kPPL; ++p) {
         const float px = __shfl_sync(FULL, pxl, tx + 8 * p);
-        const PixTaps k = pixel_taps(S, cam, px, py, ox + tx + 8 * p < W && y < H);
-        rgb[p] = k.uv != kNone ? blend_pixel<true>(S, ctl, patch, k, hd.bu0, hd.bv0) : bg;
+        rgb[p] = bg;
+        if (ox + tx + 8 * p < W && y < H) {
+            const Ray r = ray_from_screen_t<kAllPow2>(S, cam, px, py);
+            if (r.hit) rgb[p] = blend_taps<true>(S, ctl, patch, tap_setup(S, r), hd.bu0, hd.bv0);
+        }
     }
     PHASE_MARK(9);
     // ------------------------------------------------ stores.  Whole tiles of a 16-byte-aligned output: the tile's pixels are staged in
@@ -254,6 +270,16 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
 
 }  // namespace
 
+#ifdef HMLFC_PASS_STATS
+extern "C" int hmlfc_debug_pass_stats_tiles(unsigned long long *out, int reset)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, g_pass_stats, sizeof(g_pass_stats));
+    if (reset) { unsigned long long z[64] = {}; cudaMemcpyToSymbol(g_pass_stats, z, sizeof(z)); }
+    return 0;
+}
+#endif
+
 size_t render_tiles_scratch_bytes(int n_views, int W, int H)
 {
     const size_t n_tiles = (size_t)n_views * (size_t)((W + kTile - 1) / kTile) * (size_t)((H + kTile - 1) / kTile);
@@ -264,7 +290,8 @@ cudaError_t configure_render_tiles()
 {
     cudaError_t e = cudaSuccess;
 #define X(id, arena, minb) \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena);
     HMLFC_TILES_CONFIGS(X)
 #undef X
     return e;
@@ -289,7 +316,10 @@ cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)tiles_x, (unsigned)tiles_y, (unsigned)n_views);
 #define X(id, arena, minb) \
-    if (config == id) render_tiles_kernel<arena, minb><<<grid, 256, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables);
+    if (config == id) { \
+        if (S.pow2_mask == 15u) render_tiles_kernel<arena, minb, true><<<grid, 256, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
+        else render_tiles_kernel<arena, minb, false><<<grid, 256, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
+    }
     HMLFC_TILES_CONFIGS(X)
 #undef X
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

@@ -184,7 +184,7 @@ def test_degenerate_shapes(P, U, V, Ws, Ht, h, B, W):
         ref = orc.Stream(data).render(cam, 40, 24)
         assert ref.any()
         outs = []
-        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, *P.RENDER_FUSED):
             P.hmlfc_set_render_variant(hd, variant)
             outs.append(P.hmlfc_render(hd, torch.from_numpy(cam).cuda(), 40, 24).cpu().numpy())
             assert np.abs(outs[-1].astype(int) - ref.astype(int)).max() <= 1, variant
@@ -224,7 +224,7 @@ def test_more_than_65535_plane_channels(P):
     ref = s_or.render(cam, 96, 64)
     assert ref.any()
     first = None
-    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, *P.RENDER_FUSED):
         P.hmlfc_set_render_variant(h, variant)
         out = P.hmlfc_render(h, torch.from_numpy(cam).cuda(), 96, 64).cpu().numpy()
         assert np.abs(out.astype(int) - ref.astype(int)).max() <= 1, variant
@@ -283,8 +283,7 @@ def test_randomised_shapes_and_parameters(P):
         cam[0, 12:14] = (0.55 * Ws, 0.55 * Ht)   # a little wider than the image plane: the border rays miss
         ref = s.render(cam, 45, 37)
         first = None
-        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG,
-                        P.RENDER_CTA_SMALL):
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_WARP8, *P.RENDER_FUSED):
             P.hmlfc_set_render_variant(hd, variant)
             out = P.hmlfc_render(hd, torch.from_numpy(cam).cuda(), 45, 37).cpu().numpy()
             assert np.abs(out.astype(int) - ref.astype(int)).max() <= 1, (tag, variant)

@@ -153,7 +153,7 @@ def test_decode_host_entry_point(P, enc):
 def _check_views(P, h, s, cams, W, H):
     expect = s.render(cams, W, H)
     outs = {}
-    for variant in (P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_WARP8, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+    for variant in (P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_WARP8, *P.RENDER_FUSED):
         P.hmlfc_set_render_variant(h, variant)
         got = P.hmlfc_render(h, _dev(cams), W, H).cpu().numpy()
         d = np.abs(got.astype(np.int16) - expect.astype(np.int16))
@@ -163,9 +163,8 @@ def _check_views(P, h, s, cams, W, H):
     P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP])  # the kernels agree byte for byte
     assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_WARP8])
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA])
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA_BIG])
-    assert np.array_equal(outs[P.RENDER_PIXEL], outs[P.RENDER_CTA_SMALL])
+    for variant in P.RENDER_FUSED:
+        assert np.array_equal(outs[P.RENDER_PIXEL], outs[variant]), variant
     return expect
 
 
@@ -191,7 +190,7 @@ def test_other_block_sizes_and_windows(P, enc, name):
     cams = wl.camera_path(cfg)
     expect = s.render(cams, cfg.out_w, cfg.out_h)
     outs = []
-    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_CTA):
+    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_CTA, P.RENDER_TILES):
         P.hmlfc_set_render_variant(h, variant)
         got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
         assert np.abs(got.astype(np.int16) - expect.astype(np.int16)).max() <= TOL_VIEW, variant
@@ -289,7 +288,7 @@ def test_progressive_levels_match_oracle(P, enc, name):
         assert np.array_equal(P.hmlfc_decode_views(h, _dev(all_views)).cpu().numpy().reshape(-1, 3), expect), L
         ref = s.render(cams, cfg.out_w, cfg.out_h)
         outs = []
-        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):   # WARP falls back to the per-pixel kernel when L > 0
+        for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_WARP, *P.RENDER_FUSED):   # WARP falls back to the per-pixel kernel when L > 0
             P.hmlfc_set_render_variant(h, variant)
             got = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
             assert np.abs(got.astype(np.int16) - ref.astype(np.int16)).max() <= TOL_VIEW, (L, variant)
@@ -397,7 +396,7 @@ def _full_size_checks(P, cfg, data, psnr, lf=None):
     assert n_diff < 1e-3 * n_all
     P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)   # the unshared thread-per-pixel kernel on the first view
     assert np.array_equal(P.hmlfc_render(h, _dev(cams[:1]), cfg.out_w, cfg.out_h).cpu().numpy()[0], got[0])
-    for variant in (P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):   # the three shared-memory configurations of the CTA kernel (the default picks one)
+    for variant in P.RENDER_FUSED:   # every configuration of the two fused kernels (the default picks one)
         P.hmlfc_set_render_variant(h, variant)
         assert np.array_equal(P.hmlfc_render(h, _dev(cams[:2]), cfg.out_w, cfg.out_h).cpu().numpy(), got[:2])
     P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
@@ -473,7 +472,7 @@ def test_randomised_cameras_levels_and_geometries(P):
         ref = s.render(cams, Wo, Ho)
         hit.append(float(ref.reshape(-1, 3).any(1).mean()))
         outs = {}
-        for variant in (P.RENDER_PIXEL, P.RENDER_AUTO, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_CTA_SMALL):
+        for variant in (P.RENDER_PIXEL, P.RENDER_AUTO, *P.RENDER_FUSED):
             P.hmlfc_set_render_variant(hd, variant)
             outs[variant] = P.hmlfc_render(hd, _dev(cams), Wo, Ho).cpu().numpy()
             assert np.abs(outs[variant].astype(int) - ref.astype(int)).max() <= TOL_VIEW, (case, variant, L)
