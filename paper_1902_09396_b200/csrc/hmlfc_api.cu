@@ -188,6 +188,10 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
     DevStream &D = h->ds;
     D.pc = h->d_pc; D.flagrec = h->d_flagrec; D.pay = h->d_pay; D.mv = h->d_mv; D.rkv = h->d_rkv;
     h->info.device_bytes = dev_bytes;
+    // hmlfc_decode's classification: one flag sector per level and everything else fetched by the tasks pays where the L2 holds the stream
+    // (126 MB on B200; coordinates and output pass through it too) and few blocks carry data (measured: cfg2, 17% of the flags set,
+    // 12.7 -> 14.4 G px/s; cfg3, denser, 8.4 -> 7.3; cfg4 / cfg5 in HBM 6.4 -> 5.2 / 4.0 -> 3.3)
+    D.l2_resident = (dev_bytes <= (96ull << 20) && 4 * T.n_flagged <= T.n_pc * (uint64_t)D.nblk) ? 1u : 0u;
     *out = h;
     return HMLFC_OK;
 }
@@ -206,7 +210,8 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
     if (h->decode_variant == 1)
         CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
-        CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+        CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl,
+                                  h->decode_variant == 2 ? 0 : h->decode_variant == 3 ? 1 : -1));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -459,7 +464,7 @@ int hmlfc_set_min_level(hmlfc_handle *h, int min_level)
 
 int hmlfc_set_decode_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 2) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 3) return HMLFC_E_INVALID;
     h->decode_variant = variant;
     return HMLFC_OK;
 }

@@ -5,12 +5,13 @@
 //   acc = topRKV + sum_L [ stored_p(s,t)  (+|-)  stored_r(s+dx, t+dy) ].
 // For uniformly random coordinates every test of that walk (block significant? block predicted? reference
 // block significant?) is taken by a different subset of the lanes, so a thread-per-coordinate kernel runs
-// with ~8 of 32 lanes active (profiles/r01_cta_cfg2.md).  Here each lane still classifies ITS coordinate
-// (flag record + descriptor of every (level, channel): uniform control flow), but the two expensive steps
-// become tasks on two small per-warp stacks in shared memory:
-//   motion task  {MV word base, record index, reference plane-channel, destination}   -> S6 + S7 address part
-//   value task   {payload word base, value index, offset|layout|m|sign|destination}   -> S5 (BISE decode_at)
-// and are executed 32 at a time by all lanes (the stacks are drained whenever they hold >= 32 tasks, so only
+// with ~8 of 32 lanes active (profiles/r01_cta_cfg2.md).  Here each lane still classifies ITS coordinate -- ONE
+// 32-byte sector per level holds the six flag words (res / pred x Y, Co, Cg) of its block's group, uniform control
+// flow -- but everything behind a set flag becomes a task on two small per-warp stacks in shared memory:
+//   motion task  {plane-channel, group, reference plane-channel, pred blocks before | destination}   -> S6 + S7 address part
+//   value task   {plane-channel, group, position in block | res blocks before | sign | destination}  -> S4 rank + S5 (BISE decode_at)
+// A task fetches what only a significant block needs (descriptor, rank word, payload; at 40 dB seven of eight blocks are
+// empty and cost their sample nothing beyond the flag sector) and tasks are executed 32 at a time by all lanes (the stacks are drained whenever they hold >= 32 tasks, so only
 // the last batch of a warp is partial).  Values are accumulated with shared-memory atomics into the
 // destination's (Y, Co, Cg) cell; the owning lane finishes with the inverse colour transform and the staged
 // 96-byte store.  Integer arithmetic only: bit-exact by construction against the per-thread kernel and the oracle.
@@ -102,8 +103,67 @@ __device__ __forceinline__ void push(uint4 *stack, int &cnt, bool flag, uint4 ta
     cnt += __popc(m);
 }
 
-// execute the top n (<= 32) value tasks: S5 of the path
+// index of the 32-bit word with the res bits of plane-channel k's group g: Y / Co in the slot's fourth record, Cg in its own
+__device__ __forceinline__ size_t resbits_word(const DevStream &S, uint32_t k, uint32_t g)
+{
+    const uint32_t p = __umulhi(k, 0xAAAAAAABu) >> 1, c = k - 3u * p;  // k / 3, k % 3
+    return (((size_t)p * (size_t)S.fgroups + (size_t)g) * 4u + (c == 2u ? 2u : 3u)) * 4u + (c == 1u ? 1u : 0u);
+}
+
+// execute the top n (<= 32) value tasks: rank of the block (S4) and BISE decode_at of its value (S5)
 __device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+{
+    __syncwarp();
+    if (lane < n) {
+        const uint4 t = q.vq[vcnt - n + lane];
+        const uint4 d = ldg(S.pc + t.x);
+        const uint32_t rank0 = __ldg(reinterpret_cast<const uint32_t *>(S.flagrec + flag_index(S, t.x, t.y)) + 1);  // res blocks before the group
+        const uint32_t idx = ((rank0 + ((t.z >> 8) & 31u)) << (2 * S.logB)) + (t.z & 63u);
+        int val = pc_offset(d.w) + (int)bise_at(S.pay, d.y, idx, pc_layout(d.w), pc_m(d.w), lut);
+        if (t.z & kSignBit) val = -val;
+        atomicAdd(&q.acc[t.z >> 24], val);
+    }
+    vcnt -= n;
+    __syncwarp();
+}
+
+// execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
+// the reference block is significant, push its value task
+__device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
+                                             uint32_t lane_lt, const uint16_t *lut)
+{
+    __syncwarp();
+    bool has = false;
+    uint4 vt = make_uint4(0u, 0u, 0u, 0u);
+    if (lane < n) {
+        const uint4 t = q.mq[mcnt - n + lane];
+        const uint4 d = ldg(S.pc + t.x);
+        const uint32_t prank0 = __ldg(reinterpret_cast<const uint32_t *>(S.flagrec + flag_index(S, t.x, t.y)) + 3);  // pred blocks before the group
+        const uint32_t rec = bise_at(S.mv, d.z, prank0 + ((t.w >> 8) & 31u), S.mv_layout, S.mv_m, lut);
+        int mode, dx, dy;
+        mv_unpack(S, rec, mode, dx, dy);
+        const uint32_t dest = t.w & 0xFFu;
+        const uint32_t xy = q.xy[dest >> 2];
+        const int rx = (int)(xy & 0xFFFFu) + dx, ry = (int)(xy >> 16) + dy;
+        if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {  // R8: outside the image reads 0
+            const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+            const uint32_t g = (uint32_t)(b >> 5), bit = 1u << (b & 31);
+            const uint32_t bits = __ldg(reinterpret_cast<const uint32_t *>(S.flagrec) + resbits_word(S, t.z, g));
+            has = (bits & bit) != 0u;
+            const uint32_t kin = (uint32_t)(((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1)));
+            vt = make_uint4(t.z, g, kin | ((uint32_t)__popc(bits & (bit - 1u)) << 8) | (mode ? kSignBit : 0u) | (dest << 24), 0u);
+        }
+    }
+    mcnt -= n;
+    __syncwarp();
+    push(q.vq, vcnt, has, vt, lane_lt);
+}
+
+// The same two steps for tasks that carry everything the classification already fetched (eager form, below):
+//   motion task  {MV word base, record index, reference plane-channel, destination}
+//   value task   {payload word base, value index, offset|layout|m|sign|destination}
+// execute the top n (<= 32) value tasks: S5 of the path
+__device__ __forceinline__ void drain_values_eager(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
 {
     __syncwarp();
     if (lane < n) {
@@ -118,7 +178,7 @@ __device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &
 
 // execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
 // the reference block is significant, push its value task
-__device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
+__device__ __forceinline__ void drain_motion_eager(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
                                              uint32_t lane_lt, const uint16_t *lut)
 {
     __syncwarp();
@@ -147,9 +207,24 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
     push(q.vq, vcnt, has, vt, lane_lt);
 }
 
+template <bool kLazy>
+__device__ __forceinline__ void drain_v(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+{
+    if (kLazy) drain_values(S, q, vcnt, n, lane, lut); else drain_values_eager(S, q, vcnt, n, lane, lut);
+}
+
+template <bool kLazy>
+__device__ __forceinline__ void drain_m(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane, uint32_t lane_lt, const uint16_t *lut)
+{
+    if (kLazy) drain_motion(S, q, mcnt, vcnt, n, lane, lane_lt, lut); else drain_motion_eager(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
+}
+
 // kDense: the coordinates are not read but generated -- sample i is pixel i mod (Ws Ht) (row-major) of view views[i / (Ws Ht)]
 // (hmlfc_decode_views: whole views, no 16-byte coordinate per sample, neighbouring lanes in neighbouring pixels).
-template <int kDense>  // 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
+// kLazy: the classification reads one flag sector per level and the tasks fetch descriptor and rank themselves (fewest sectors per sample: for
+// streams the L2 holds, where the sector rate binds); otherwise it reads the three channels' flag records and descriptors up front and the
+// tasks carry them (one dependent load less per task: for streams in HBM, where every access is a DRAM access either way and latency binds).
+template <int kDense, bool kLazy>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
 __global__ void __launch_bounds__(kThreads)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
@@ -218,6 +293,27 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
         const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
         const uint32_t rbase = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
         const bool predictive = ((pu | pv) & 1) != 0;
+        if (kLazy) {
+        // S4, first look: the six flag words of the block's group, one 32-byte sector (the second half of the plane's 64-byte slot):
+        // a = the Cg record {res, rank, pred, rank}, bw = {res Y, res Co, pred Y, pred Co}
+        uint4 a = make_uint4(0u, 0u, 0u, 0u), bw = a;
+        if (valid) ldg256(S.flagrec + flag_index(S, base, fg) + 2, a, bw);
+        const uint32_t resw[3] = {bw.x, bw.y, a.x}, prdw[3] = {bw.z, bw.w, a.z};
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const uint32_t dest = (uint32_t)(lane * 4 + c);
+            const bool res = (resw[c] & bit) != 0u;
+            push(q.vq, vcnt, res, make_uint4(base + (uint32_t)c, fg, kin | ((uint32_t)__popc(resw[c] & (bit - 1u)) << 8) | (dest << 24), 0u), lane_lt);
+            if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
+            const bool pred = predictive && (prdw[c] & bit) != 0u;
+            push(q.mq, mcnt, pred, make_uint4(base + (uint32_t)c, fg, rbase + (uint32_t)c, dest | ((uint32_t)__popc(prdw[c] & (bit - 1u)) << 8)), lane_lt);
+            if (mcnt >= 32) {
+                drain_m<kLazy>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
+            }
+        }
+    
+        } else {
         // S4: the three channels' descriptors and flag records, six independent loads
         uint4 d[3], fr[3];
         // S4: the three channels' descriptors and their flag records; the records share one 64-byte slot: a 256-bit
@@ -237,19 +333,21 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
             const bool res = (fr[c].x & bit) != 0u;
             const uint32_t rank = fr[c].y + (uint32_t)__popc(fr[c].x & (bit - 1u));
             push(q.vq, vcnt, res, make_uint4(d[c].y, (rank << (2 * S.logB)) + kin, (d[c].w & 0x3FFFFFu) | (dest << 24), 0u), lane_lt);
-            if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
+            if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
             const bool pred = predictive && (fr[c].z & bit) != 0u;
             const uint32_t mi = fr[c].w + (uint32_t)__popc(fr[c].z & (bit - 1u));
             push(q.mq, mcnt, pred, make_uint4(d[c].z, mi, rbase + (uint32_t)c, dest), lane_lt);
             if (mcnt >= 32) {
-                drain_motion(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
-                if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
+                drain_m<kLazy>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
             }
         }
+    
+        }
     }
-    if (mcnt > 0) drain_motion(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
-    if (vcnt >= 32) drain_values(S, q, vcnt, 32, lane, lut);
-    if (vcnt > 0) drain_values(S, q, vcnt, vcnt, lane, lut);
+    if (mcnt > 0) drain_m<kLazy>(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
+    if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
+    if (vcnt > 0) drain_v<kLazy>(S, q, vcnt, vcnt, lane, lut);
     __syncwarp();
 
     // S8: inverse YCoCg-R + clamp, then the warp's 96 bytes as 24 coalesced words
@@ -281,15 +379,17 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
 }  // namespace
 
 cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
-                                unsigned long long *d_oob, cudaStream_t st, int *n_launches)
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int lazy)
 {
     if (n == 0) return cudaSuccess;
     if (S.Ws > 65536 || S.Ht > 65536) return cudaErrorInvalidValue;  // s | t << 16 packing
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<0><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
-                                                                       d_oob, aligned);
+    if (lazy < 0 ? S.l2_resident != 0u : lazy != 0)
+        decode_queue_kernel<0, true><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out, d_oob, aligned);
+    else
+        decode_queue_kernel<0, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -303,7 +403,7 @@ cudaError_t launch_decode_blocks(const DevStream &S, const int32_t *d_blocks, in
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<2><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_blocks), n, d_out, d_oob, aligned);
+    decode_queue_kernel<2, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_blocks), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -317,7 +417,7 @@ cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int6
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<1><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
+    decode_queue_kernel<1, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

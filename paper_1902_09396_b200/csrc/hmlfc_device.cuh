@@ -51,6 +51,7 @@ struct DevStream {
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
     float uv_inv[2], st_inv[2];  // 1 / step where that is exact (step a power of two), see pow2_mask
     uint32_t pow2_mask;          // bit 0..3: uv_step[0], uv_step[1], st_step[0], st_step[1] is a power of two
+    uint32_t l2_resident;        // the device form of the stream fits the L2 with room to spare and is sparse (kernel choice of hmlfc_decode)
     uint8_t bg[4];
 };
 

@@ -23,8 +23,9 @@ struct FootprintTotals {
 cudaError_t launch_decode(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
                           unsigned long long *d_oob, cudaStream_t st, int *n_launches);
 // warp-cooperative decode (hmlfc_decode_queue.cu): same result as launch_decode
+// lazy: 1 = one flag sector per level, tasks fetch descriptor and rank; 0 = flag records and descriptors up front; -1 = by S.l2_resident
 cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
-                                unsigned long long *d_oob, cudaStream_t st, int *n_launches);
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int lazy = -1);
 // whole views: d_views = int32 [n_views][2] = (u, v); d_out = uint8 [n_views][Ht][Ws][3]; coordinates are generated in the kernel
 cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
                                 cudaStream_t st, int *n_launches);

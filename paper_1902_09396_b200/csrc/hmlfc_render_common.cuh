@@ -383,12 +383,12 @@ __device__ __forceinline__ void build_slot_table(const DevStream &S, const float
 }
 
 // do the tables fit an arena of kArenaBytes?  accumulators (8 bytes per slot sample), then the patch (16 bytes per cell) aliased by
-// the record list (16 bytes each)
+// the record list (32 bytes each)
 template <int kArenaBytes>
 __device__ __forceinline__ bool tables_fit(const TileHeader &hd)
 {
     const long long rest = (long long)kArenaBytes - (((long long)hd.nacc * 8 + 15) & ~15LL);
-    return hd.nslots <= kMaxSlots && hd.ncell <= 32 * kMaxChunks && rest >= (long long)hd.ncell * 16 && rest >= (long long)kMinRec * 16;
+    return hd.nslots <= kMaxSlots && hd.ncell <= 32 * kMaxChunks && rest >= (long long)hd.ncell * 16 && rest >= (long long)kMinRec * 32;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -404,10 +404,10 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
     const int ncell = hd.ncell, nacc = hd.nacc, nslots = hd.nslots, nbhmax = hd.nbhmax;
     const int bu0 = hd.bu0, bv0 = hd.bv0, nu = hd.nu, nv = hd.nv;
     const long long rest = (long long)kArenaBytes - (((long long)nacc * 8 + 15) & ~15LL);
-    const int reccap = (int)min(rest / 16, 0x7fffffLL);
+    const int reccap = (int)min(rest / 32, 0x7fffffLL);
     uint2 *acc = reinterpret_cast<uint2 *>(arena);
     unsigned char *region2 = arena + (((size_t)nacc * 8 + 15) & ~(size_t)15);
-    uint4 *rec = reinterpret_cast<uint4 *>(region2);      // [reccap]
+    uint4 *rec = reinterpret_cast<uint4 *>(region2);      // [reccap][2]
     float4 *patch = reinterpret_cast<float4 *>(region2);  // [ncell], after the records are dead
     // ---------------------------------------------------- zero the accumulators; per-view cell offsets, chunk -> view, accumulator
     // offsets of every (view, level); the planes' descriptors (and their reference planes') go to shared memory for B2 and B3
@@ -499,7 +499,7 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                     const bool hr = (resb & bit) != 0u, hp = (prdb & bit) != 0u;
                     // rank of the block's payload * 16, rank of its motion record, slot | channel | block row | block column
                     if (idx < reccap)
-                        rec[idx] = make_uint4(hr ? ((fr.y + popc(fr.x & (bit - 1u))) << 4) : kNone, hp ? (fr.w + popc(fr.z & (bit - 1u))) : kNone,
+                        rec[2 * idx] = make_uint4(hr ? ((fr.y + popc(fr.x & (bit - 1u))) << 4) : kNone, hp ? (fr.w + popc(fr.z & (bit - 1u))) : kNone,
                                               sc | ((uint32_t)by << 8) | ((uint32_t)((g << 5) + bp - rowb) << 20), 0u);
                     ++idx;
                 }
@@ -518,65 +518,67 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
         __syncthreads();  // every thread has read the record count (the caller resets it)
         return false;
     }
-    // ------------------------------------------------ B2: motion record, once per block.  With few records (B3 is one or two rounds of
-    // latency) the four row lanes of a block decode it themselves in B3 -- the same loads, the same instructions: what one lane would cost,
-    // and a barrier less; with many (B3 is bound by instruction issue) one lane per record decodes it here.
-    const bool fuse_b2 = 4 * nrec <= 3 * kNT;
-    if (!fuse_b2) {
-        for (int rr = tid; rr < nrec; rr += kNT) {
-            const uint4 r0 = rec[rr];
-            if (r0.y != kNone) {
-                int md, dx, dy;
-                mv_unpack(S, bise_at(S.mv + ctl.desc[r0.z & 63u][(r0.z >> 6) & 3u].z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
-                rec[rr].y = ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+    // ------------------------------------------------ B2: one lane per record of a predicted block: its motion record (BISE decode_at), then
+    // the flag / rank words of the (up to 2 x 2) reference blocks its four re-compensated rows read from -> second half of the record,
+    // {significant | rank * 16} per reference block.  B3's loads then depend on nothing but the record: one round trip per task.
+    for (int rr = tid; rr < nrec; rr += kNT) {
+        const uint4 r0 = rec[2 * rr];
+        if (r0.y == kNone) continue;
+        const uint32_t s = r0.z & 63u, c = (r0.z >> 6) & 3u;
+        int md, dx, dy;
+        mv_unpack(S, bise_at(S.mv + ctl.desc[s][c].z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
+        const uint4 dr = ctl.rdesc[s][c];
+        const int rx = (int)((r0.z >> 20) << 2) + dx, ry0 = (int)(((r0.z >> 8) & 0xFFFu) << 2) + dy;  // first reference sample of the block
+        const int bxa = rx >> 2, bya = ry0 >> 2;  // arithmetic shifts: floor for positions left of / above the image
+        uint32_t e[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int bx = bxa + (j & 1), by = bya + (j >> 1);
+            e[j] = 0u;
+            // needed at all: the second column only if the row straddles two blocks, the second block row likewise
+            if ((unsigned)bx < (unsigned)S.nbx && (unsigned)by < (unsigned)S.nby && (!(j & 1) || (rx & 3)) && (!(j >> 1) || (ry0 & 3))) {
+                const int b = by * S.nbx + bx;
+                const uint2 fr = __ldg(reinterpret_cast<const uint2 *>(S.flagrec + dr.x + 4u * (uint32_t)(b >> 5)));  // {res bits, res rank}
+                const uint32_t bit = 1u << (b & 31);
+                if (fr.x & bit) e[j] = ((fr.y + popc(fr.x & (bit - 1u))) << 4) | 1u;
             }
         }
-        __syncthreads();
+        rec[2 * rr].y = ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+        rec[2 * rr + 1] = make_uint4(e[0], e[1], e[2], e[3]);
     }
+    __syncthreads();
     PHASE_MARK(6);
-    // ------------------------------------------------ B2 + B3: one lane per (record, block row): 4 stored / re-compensated values (neighbouring
+    // ------------------------------------------------ B3: one lane per (record, block row): 4 stored / re-compensated values (neighbouring
     // lanes work on neighbouring blocks of one plane: their payload words share sectors and they take the same branches)
     {
         int16_t *acc16 = reinterpret_cast<int16_t *>(arena);
         for (int t = tid; t < 4 * nrec; t += kNT) {
             const int rr = t >> 2, ky = t & 3;
-            const uint4 r0 = rec[rr];
+            const uint4 r0 = rec[2 * rr];
             const uint32_t s = r0.z & 63u, c = (r0.z >> 6) & 3u;
             const SlotInfo &sl = ctl.tab.slot[s];
-            const int yy = (int)(((r0.z >> 8) & 0xFFFu) << 2) + ky;
+            const int yy0 = (int)(((r0.z >> 8) & 0xFFFu) << 2), yy = yy0 + ky;
             const int st0 = sl.t0, st1 = sl.t1;
             if (yy < st0 || yy > st1) continue;
             const int xx = (int)((r0.z >> 20) << 2);
             const uint4 d = ctl.desc[s][c];
-            // the motion record (B2)
-            int md = 0, dx = 0, dy = 0;
-            if (r0.y != kNone) {
-                if (fuse_b2) mv_unpack(S, bise_at(S.mv + d.z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
-                else { md = (int)((r0.y >> 16) & 1u); dx = (int)((r0.y >> 8) & 0xFFu) - S.W; dy = (int)(r0.y & 0xFFu) - S.W; }
-            }
             uint2 own = make_uint2(0u, 0u);
             if (r0.x != kNone) own = bise_row4(S.pay + d.y, r0.x + (uint32_t)(ky << 2), d.w, ctl.lut);
             int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
             if (r0.y != kNone) {
+                const int md = (int)((r0.y >> 16) & 1u), dx = (int)((r0.y >> 8) & 0xFFu) - S.W, dy = (int)(r0.y & 0xFFu) - S.W;
                 const int rx = xx + dx, ry = yy + dy;
                 if ((unsigned)ry < (unsigned)S.Ht) {
-                    // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
+                    // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1: B2 looked them up
                     const uint4 dr = ctl.rdesc[s][c];
-                    const int o = rx & 3, bxa = rx >> 2;
+                    const uint4 re = rec[2 * rr + 1];
+                    const int o = rx & 3;
+                    const bool second_row = (ry >> 2) != ((yy0 + dy) >> 2);
+                    const uint32_t ea = second_row ? re.z : re.x, eb = second_row ? re.w : re.y;
                     const uint32_t i0 = (uint32_t)((ry & 3) << 2);
-                    const int rowb = (ry >> 2) * S.nbx;
                     uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        uint2 q = make_uint2(0u, 0u);
-                        if ((j == 0 || o) && (unsigned)(bxa + j) < (unsigned)S.nbx) {
-                            const int b = rowb + bxa + j;
-                            const uint4 fr = ldg(S.flagrec + dr.x + 4u * (uint32_t)(b >> 5));
-                            const uint32_t bit = 1u << (b & 31);
-                            if (fr.x & bit) q = bise_row4(S.pay + dr.y, ((fr.y + popc(fr.x & (bit - 1u))) << 4) + i0, dr.w, ctl.lut);
-                        }
-                        if (j == 0) qa = q; else qb = q;
-                    }
+                    if (ea & 1u) qa = bise_row4(S.pay + dr.y, (ea & ~15u) + i0, dr.w, ctl.lut);
+                    if (eb & 1u) qb = bise_row4(S.pay + dr.y, (eb & ~15u) + i0, dr.w, ctl.lut);
                     // samples o .. o+3 of the 8-sample string qa | qb
                     uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
                     if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }

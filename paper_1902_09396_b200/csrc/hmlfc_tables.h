@@ -16,6 +16,7 @@ struct HostTables {
     DevStream ds{};  // device pointers left null; hmlfc_load fills them after the upload
     hmlfc_info_t info{};
     std::vector<uint4> pc, flagrec;
+    uint64_t n_flagged = 0;  // set res and pred flags of the whole stream
     std::vector<uint32_t> bits15;  // per plane-channel BISE bits/value in 1/15 bit (footprint only)
     std::vector<short4> rkv;
     uint64_t n_pc = 0, off_pay = 0, off_mv = 0, total = 0;
@@ -144,7 +145,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     try {
         T.pc.resize(n_pc);
         T.bits15.resize(n_pc);
-        T.flagrec.assign((n_pc / 3) * (uint64_t)D.fgroups * 4, make_uint4(0u, 0u, 0u, 0u));  // 64-byte slot per (plane, group): Y, Co, Cg, spare
+        T.flagrec.assign((n_pc / 3) * (uint64_t)D.fgroups * 4, make_uint4(0u, 0u, 0u, 0u));  // 64-byte slot per (plane, group): Y, Co, Cg, bit words of Y and Co
         T.rkv.resize(n_top * npx);
     } catch (const std::bad_alloc &) {
         return HMLFC_E_NOMEM;
@@ -188,10 +189,17 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                             wr &= mask; wp &= mask;
                         }
                         T.flagrec[frbase + 4ull * (uint64_t)g] = make_uint4(wr, rr, wp, rp);
+                        // the slot's fourth record repeats the Y and Co bit words {res Y, res Co, pred Y, pred Co}: together with the Cg
+                        // record before it, ONE 32-byte sector holds all six bit words of the 32 blocks (a random sample's first look)
+                        if (c < 2) {
+                            uint4 &sp = T.flagrec[(k / 3) * (uint64_t)D.fgroups * 4 + 4ull * (uint64_t)g + 3];
+                            if (c == 0) { sp.x = wr; sp.z = wp; } else { sp.y = wr; sp.w = wp; }
+                        }
                         rr += popcount32(wr);
                         rp += popcount32(wp);
                     }
                     if (rr != n_res || rp != n_pred) return HMLFC_E_CORRUPT;
+                    T.n_flagged += (uint64_t)rr + (uint64_t)rp;
                 }
 
     // top-level RKVs: Y uint8 planes, then Co and Cg int16 LE planes -> short4 {Y, Co, Cg, 0} per sample
