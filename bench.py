@@ -33,7 +33,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 L2_FLUSH_BYTES = 512 << 20  # > 126 MB L2
-RENDER_KERNEL_NAME = "render_cta_kernel"
+RENDER_KERNEL_NAME = "render_tiles_kernel"
 
 
 def _peaks():
