@@ -22,7 +22,7 @@ class Params(C.Structure):
         ("tau_ref", C.c_int32), ("tau_res", C.c_int32), ("policy", C.c_int32), ("nthreads", C.c_int32),
         ("uv_origin", C.c_float * 2), ("uv_step", C.c_float * 2),
         ("st_origin", C.c_float * 2), ("st_step", C.c_float * 2), ("z_st", C.c_float),
-        ("background", C.c_uint8 * 3), ("_pad", C.c_uint8), ("seed", C.c_uint64),
+        ("background", C.c_uint8 * 3), ("chroma", C.c_uint8), ("seed", C.c_uint64),
     ]
 
 
@@ -100,9 +100,11 @@ def _ptr(a):
 
 
 def make_params(U, V, Ws, Ht, height, block=4, window=16, tau_ref=0, tau_res=0, policy=POLICY_ADAPTIVE,
-                geometry=None, background=(0, 0, 0), seed=0, nthreads=0) -> Params:
-    """geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab."""
+                geometry=None, background=(0, 0, 0), seed=0, nthreads=0, chroma=0) -> Params:
+    """geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab.
+    chroma = 1: Co / Cg planes at half resolution (R18)."""
     p = Params()
+    p.chroma = chroma
     p.U, p.V, p.Ws, p.Ht, p.height, p.block, p.window = U, V, Ws, Ht, height, block, window
     p.tau_ref, p.tau_res, p.policy, p.nthreads = tau_ref, tau_res, policy, nthreads
     g = geometry or dict(uv_origin=(0.0, 0.0), uv_step=(1.0, 1.0), st_origin=(0.0, 0.0), st_step=(1.0, 1.0), z_st=1.0)
@@ -217,7 +219,8 @@ class Tree:
     def plane(self, kind, L, pu, pv, c) -> np.ndarray:
         """kind: 'X' | 'srv' | 'stored'."""
         k = {"X": 0, "srv": 1, "stored": 2}[kind]
-        out = np.empty((self.params.Ht, self.params.Ws), dtype=np.int16)
+        sh = 1 if (self.params.chroma and c > 0) else 0   # the channel's own plane size (R18)
+        out = np.empty((self.params.Ht >> sh, self.params.Ws >> sh), dtype=np.int16)
         rc = lib().orc_tree_get_plane(self._h, k, L, pu, pv, c, _ptr(out))
         if rc:
             raise OracleError(rc, "get_plane")
@@ -226,7 +229,8 @@ class Tree:
     def blocks(self, L, pu, pv, c) -> np.ndarray:
         """[nby][nbx][6] = mode, dx, dy, sad, E, flags(bit0 res, bit1 pred)."""
         p = self.params
-        nbx, nby = p.Ws // p.block, p.Ht // p.block
+        sh = 1 if (p.chroma and c > 0) else 0
+        nbx, nby = (p.Ws >> sh) // p.block, (p.Ht >> sh) // p.block
         out = np.empty((nby, nbx, 6), dtype=np.int32)
         rc = lib().orc_tree_get_blocks(self._h, L, pu, pv, c, _ptr(out))
         if rc:

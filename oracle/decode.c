@@ -26,19 +26,22 @@ static uint64_t pc_index(const orc_stream *s, int L, int pu, int pv, int c)
     return s->level_base[L] + ((uint64_t)pv * s->UL[L] + pu) * 3 + (uint64_t)c;
 }
 
+/* top-level RKV sample of channel c at (x,y) OF THAT CHANNEL'S PLANE: Y planes uint8, then the Co planes, then the Cg planes, int16 */
 static int rkv_sample(const orc_stream *s, int c, int qu, int qv, int x, int y)
 {
     const int h = s->h;
-    const uint64_t npx = (uint64_t)s->p.Ws * s->p.Ht;
     const uint64_t n_top = (uint64_t)s->UL[h] * s->VL[h];
-    uint64_t i = ((uint64_t)qv * s->UL[h] + qu) * npx + (uint64_t)y * s->p.Ws + x;
+    const uint64_t npx = (uint64_t)s->g.W[c] * s->g.H[c];
+    uint64_t i = ((uint64_t)qv * s->UL[h] + qu) * npx + (uint64_t)y * s->g.W[c] + x;
     const uint8_t *base = s->bytes + s->off_rkv;
     if (c == 0) return base[i];
-    const uint8_t *q = base + n_top * npx + (uint64_t)(c - 1) * n_top * npx * 2 + i * 2;
+    const uint8_t *q = base + n_top * (uint64_t)s->g.W[0] * s->g.H[0];
+    if (c == 2) q += n_top * (uint64_t)s->g.W[1] * s->g.H[1] * 2;
+    q += i * 2;
     return (int16_t)((uint16_t)q[0] | ((uint16_t)q[1] << 8));
 }
 
-/* stored value of plane-channel k at pixel (x,y): 0 if the block's res flag is clear.
+/* stored value of plane-channel k at pixel (x,y) of its plane (channel k % 3): 0 if the block's res flag is clear.
  * use_rank = 1: rank directory + O(1) BISE addressing (P2).
  * use_rank = 0: linear scan of the flag map + sequential BISE decode (P3 brute force). */
 static int plane_value(const orc_stream *s, uint64_t k, int x, int y, int use_rank)
@@ -46,7 +49,7 @@ static int plane_value(const orc_stream *s, uint64_t k, int x, int y, int use_ra
     const int B = s->p.block;
     const orc_dirent *d = &s->dir[k];
     const uint8_t *fres = s->bytes + s->off_flags + d->flags_off;
-    int b = (y / B) * s->nbx + (x / B);
+    int b = (y / B) * s->g.nbx[k % 3] + (x / B);
     if (!flag_bit(fres, b)) return 0;
     const uint8_t *bits = s->bytes + s->off_payload + d->pay_bitoff / 8;
     int kk = (y % B) * B + (x % B);
@@ -67,9 +70,12 @@ static int plane_value(const orc_stream *s, uint64_t k, int x, int y, int use_ra
 static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int use_rank, uint8_t rgb[3])
 {
     const int B = s->p.block, W = s->p.window, h = s->h;
-    const uint32_t fwords = (uint32_t)((s->nblk + 31) / 32);
+    const int x0 = x, y0 = y;
     int acc[3];
     for (int c = 0; c < 3; ++c) {
+        /* the channel's sample of light-field pixel (x0, y0): with chroma subsampling (R18) Co / Cg live at half resolution */
+        const int x = x0 >> s->g.shift[c], y = y0 >> s->g.shift[c];
+        const uint32_t fwords = (uint32_t)((s->g.nblk[c] + 31) / 32);
         int a = rkv_sample(s, c, u >> h, v >> h, x, y);
         for (int L = h - 1; L >= s->min_level; --L) { /* "from the top level to the bottom level"; progressive: stop early (R26) */
             int pu = u >> L, pv = v >> L;
@@ -78,7 +84,7 @@ static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int us
             if (orc_is_predictive(pu, pv)) {
                 const orc_dirent *d = &s->dir[k];
                 const uint8_t *fpred = s->bytes + s->off_flags + d->flags_off + (size_t)fwords * 4;
-                int b = (y / B) * s->nbx + (x / B);
+                int b = (y / B) * s->g.nbx[c] + (x / B);
                 if (flag_bit(fpred, b)) {
                     uint64_t mi;
                     if (use_rank) mi = s->rank_pred[k][b];
@@ -97,7 +103,7 @@ static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int us
                     int rem = (int)(r % (uint32_t)(nd * nd));
                     int dy = rem / nd - W, dx = rem % nd - W;
                     int rx = x + dx, ry = y + dy, q = 0;
-                    if (rx >= 0 && rx < s->p.Ws && ry >= 0 && ry < s->p.Ht)
+                    if (rx >= 0 && rx < s->g.W[c] && ry >= 0 && ry < s->g.H[c])
                         q = plane_value(s, pc_index(s, L, pu & ~1, pv & ~1, c), rx, ry, use_rank);
                     e += mode ? -q : q; /* R10: sub P = e + R, add P = e - R */
                 }
@@ -187,8 +193,8 @@ int orc_decode_full(const orc_stream *s, uint8_t *lf_out, int nthreads)
  */
 typedef struct {
     const orc_stream *s;
-    uint8_t *blk_seen;  /* [n_pc * nblk] */
-    uint8_t *rkv_seen;  /* [3][n_top][npx] */
+    uint8_t *blk_seen;  /* [n_pc * nblk of channel 0] */
+    uint8_t *rkv_seen;  /* [3][n_top][npx of channel 0] */
     orc_stats st;
 } stat_ctx;
 
@@ -198,11 +204,11 @@ static int64_t bits15_per_value(uint32_t N) { return (int64_t)orc_bise_nbits(N, 
 static void touch_block(stat_ctx *cx, uint64_t k, int b, int is_pred_plane)
 {
     const orc_stream *s = cx->s;
-    uint8_t *seen = &cx->blk_seen[k * (uint64_t)s->nblk + (uint64_t)b];
+    uint8_t *seen = &cx->blk_seen[k * (uint64_t)s->g.nblk[0] + (uint64_t)b];
     if (*seen) return;
     *seen = 1;
     const orc_dirent *d = &s->dir[k];
-    const uint32_t fwords = (uint32_t)((s->nblk + 31) / 32);
+    const uint32_t fwords = (uint32_t)((s->g.nblk[k % 3] + 31) / 32);
     const uint8_t *fres = s->bytes + s->off_flags + d->flags_off;
     cx->st.blocks_touched += 1;
     cx->st.flag_bits += is_pred_plane ? 2 : 1;
@@ -214,16 +220,18 @@ static void touch_pixel(stat_ctx *cx, int u, int v, int x, int y)
 {
     const orc_stream *s = cx->s;
     const int B = s->p.block, W = s->p.window, h = s->h;
-    const uint32_t fwords = (uint32_t)((s->nblk + 31) / 32);
     const uint64_t npx = (uint64_t)s->p.Ws * s->p.Ht, n_top = (uint64_t)s->UL[h] * s->VL[h];
+    const int x0 = x, y0 = y;
     cx->st.taps += 1;
     for (int c = 0; c < 3; ++c) {
-        uint64_t ri = ((uint64_t)c * n_top + (uint64_t)(v >> h) * s->UL[h] + (u >> h)) * npx + (uint64_t)y * s->p.Ws + x;
+        const int x = x0 >> s->g.shift[c], y = y0 >> s->g.shift[c];  /* the channel's own sample (R18) */
+        const uint32_t fwords = (uint32_t)((s->g.nblk[c] + 31) / 32);
+        uint64_t ri = ((uint64_t)c * n_top + (uint64_t)(v >> h) * s->UL[h] + (u >> h)) * npx + (uint64_t)y * s->g.W[c] + x;
         if (!cx->rkv_seen[ri]) { cx->rkv_seen[ri] = 1; cx->st.rkv_bytes += (c == 0) ? 1 : 2; }
         for (int L = s->min_level; L < h; ++L) {
             int pu = u >> L, pv = v >> L;
             uint64_t k = pc_index(s, L, pu, pv, c);
-            int b = (y / B) * s->nbx + (x / B);
+            int b = (y / B) * s->g.nbx[c] + (x / B);
             int isp = orc_is_predictive(pu, pv);
             touch_block(cx, k, b, isp);
             if (!isp) continue;
@@ -234,8 +242,8 @@ static void touch_pixel(stat_ctx *cx, int u, int v, int x, int y)
             int nd = 2 * W + 1;
             int rem = (int)(r % (uint32_t)(nd * nd));
             int rx = x + rem % nd - W, ry = y + rem / nd - W;
-            if (rx >= 0 && rx < s->p.Ws && ry >= 0 && ry < s->p.Ht)
-                touch_block(cx, pc_index(s, L, pu & ~1, pv & ~1, c), (ry / B) * s->nbx + (rx / B), 0);
+            if (rx >= 0 && rx < s->g.W[c] && ry >= 0 && ry < s->g.H[c])
+                touch_block(cx, pc_index(s, L, pu & ~1, pv & ~1, c), (ry / B) * s->g.nbx[c] + (rx / B), 0);
         }
     }
 }
@@ -245,7 +253,7 @@ static int stat_begin(stat_ctx *cx, const orc_stream *s)
     memset(cx, 0, sizeof(*cx));
     cx->s = s;
     uint64_t npx = (uint64_t)s->p.Ws * s->p.Ht, n_top = (uint64_t)s->UL[s->h] * s->VL[s->h];
-    cx->blk_seen = (uint8_t *)calloc((size_t)(s->n_pc * (uint64_t)s->nblk), 1);
+    cx->blk_seen = (uint8_t *)calloc((size_t)(s->n_pc * (uint64_t)s->g.nblk[0]), 1);
     cx->rkv_seen = (uint8_t *)calloc((size_t)(3 * n_top * npx), 1);
     if (!cx->blk_seen || !cx->rkv_seen) { free(cx->blk_seen); free(cx->rkv_seen); return ORC_E_NOMEM; }
     return ORC_OK;

@@ -20,6 +20,23 @@ static int round_mean(int sum, int n)
     return -((-2 * sum + n) / (2 * n));
 }
 
+int orc__geom(const orc_params *p, orc_geom *g)
+{
+    if (p->block < 1) return ORC_E_PARAM;
+    for (int c = 0; c < 3; ++c) {
+        int sh = (p->chroma && c > 0) ? 1 : 0;
+        if (sh && ((p->Ws & 1) || (p->Ht & 1))) return ORC_E_PARAM;
+        g->shift[c] = sh;
+        g->W[c] = p->Ws >> sh;
+        g->H[c] = p->Ht >> sh;
+        if (g->W[c] < 1 || g->H[c] < 1 || (g->W[c] % p->block) || (g->H[c] % p->block)) return ORC_E_PARAM; /* R23: B must divide the plane size */
+        g->nbx[c] = g->W[c] / p->block;
+        g->nby[c] = g->H[c] / p->block;
+        g->nblk[c] = g->nbx[c] * g->nby[c];
+    }
+    return ORC_OK;
+}
+
 void orc_tree_free(orc_tree *t)
 {
     if (!t) return;
@@ -119,17 +136,19 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
     if (!err) err = &e_dummy;
     *err = ORC_OK;
     if (!lf || !p || p->U < 1 || p->V < 1 || p->Ws < 1 || p->Ht < 1 || p->height < 1 || p->height > ORC_MAX_LEVELS ||
-        p->block < 1 || p->block > 8 || p->window < 0 || p->window > 64 || (p->Ws % p->block) || (p->Ht % p->block)) {
-        *err = ORC_E_PARAM; /* R23: B must divide the image size */
+        p->block < 1 || p->block > 8 || p->window < 0 || p->window > 64 || p->chroma > 1) {
+        *err = ORC_E_PARAM;
         return NULL;
     }
+    orc_geom geom;
+    if (orc__geom(p, &geom) != ORC_OK) { *err = ORC_E_PARAM; return NULL; }
     orc_tree *t = (orc_tree *)calloc(1, sizeof(orc_tree));
     if (!t) { *err = ORC_E_NOMEM; return NULL; }
     t->p = *p;
+    t->g = geom;
     t->h = p->height;
     const int Ws = p->Ws, Ht = p->Ht, B = p->block, W = p->window, h = t->h;
     const size_t npx = (size_t)Ws * Ht;
-    t->nbx = Ws / B; t->nby = Ht / B; t->nblk = t->nbx * t->nby;
     for (int L = 0; L <= h; ++L) {
         t->UL[L] = (p->U + (1 << L) - 1) >> L; /* U_L = ceil(U / 2^L)  (R1, R3) */
         t->VL[L] = (p->V + (1 << L) - 1) >> L;
@@ -138,39 +157,60 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
     if (p->nthreads > 0) omp_set_num_threads(p->nthreads);
 #endif
     for (int c = 0; c < 3; ++c) {
+        const size_t npc = (size_t)t->g.W[c] * t->g.H[c];
         for (int L = 0; L <= h; ++L) {
             int np = t->UL[L] * t->VL[L];
             t->X[c][L] = (int16_t **)calloc((size_t)np, sizeof(int16_t *));
             if (!t->X[c][L]) goto nomem;
             for (int i = 0; i < np; ++i)
-                if (!(t->X[c][L][i] = (int16_t *)malloc(npx * sizeof(int16_t)))) goto nomem;
+                if (!(t->X[c][L][i] = (int16_t *)malloc(npc * sizeof(int16_t)))) goto nomem;
             if (L < h) {
                 t->srv[c][L] = (int16_t **)calloc((size_t)np, sizeof(int16_t *));
                 if (!t->srv[c][L]) goto nomem;
                 for (int i = 0; i < np; ++i)
-                    if (!(t->srv[c][L][i] = (int16_t *)malloc(npx * sizeof(int16_t)))) goto nomem;
-                t->blk[c][L] = (orc_block *)calloc((size_t)np * t->nblk, sizeof(orc_block));
+                    if (!(t->srv[c][L][i] = (int16_t *)malloc(npc * sizeof(int16_t)))) goto nomem;
+                t->blk[c][L] = (orc_block *)calloc((size_t)np * t->g.nblk[c], sizeof(orc_block));
                 if (!t->blk[c][L]) goto nomem;
             }
         }
     }
-    /* step 1: colour, X_0 */
+    /* step 1: colour, X_0; with p.chroma the Co / Cg planes are reduced by the 2 x 2 box mean (R18) */
     {
         int nviews = p->U * p->V;
+        int failed = 0;
 #pragma omp parallel for schedule(static)
         for (int vi = 0; vi < nviews; ++vi) {
             const uint8_t *src = lf + (size_t)vi * npx * 3;
+            int16_t *full[3] = {t->X[0][0][vi], NULL, NULL};
+            if (p->chroma) {
+                full[1] = (int16_t *)malloc(npx * sizeof(int16_t));
+                full[2] = (int16_t *)malloc(npx * sizeof(int16_t));
+                if (!full[1] || !full[2]) { free(full[1]); free(full[2]); failed = 1; continue; }
+            } else { full[1] = t->X[1][0][vi]; full[2] = t->X[2][0][vi]; }
             for (size_t i = 0; i < npx; ++i) {
                 int y, co, cg;
                 orc_rgb_to_ycocg(src[3 * i], src[3 * i + 1], src[3 * i + 2], &y, &co, &cg);
-                t->X[0][0][vi][i] = (int16_t)y;
-                t->X[1][0][vi][i] = (int16_t)co;
-                t->X[2][0][vi][i] = (int16_t)cg;
+                full[0][i] = (int16_t)y;
+                full[1][i] = (int16_t)co;
+                full[2][i] = (int16_t)cg;
+            }
+            if (p->chroma) {
+                for (int c = 1; c < 3; ++c) {
+                    const int Wc = t->g.W[c], Hc = t->g.H[c];
+                    for (int y = 0; y < Hc; ++y)
+                        for (int x = 0; x < Wc; ++x) {
+                            const int16_t *q = full[c] + (size_t)(2 * y) * Ws + 2 * x;
+                            t->X[c][0][vi][(size_t)y * Wc + x] = (int16_t)round_mean(q[0] + q[1] + q[Ws] + q[Ws + 1], 4);
+                        }
+                    free(full[c]);
+                }
             }
         }
+        if (failed) goto nomem;
     }
     /* step 2: hierarchy: RKV = filtered cluster, SRV = member - RKV, recurse */
     for (int c = 0; c < 3; ++c) {
+        const size_t npc = (size_t)t->g.W[c] * t->g.H[c];
         for (int L = 0; L < h; ++L) {
             int UL = t->UL[L], VL = t->VL[L], UP = t->UL[L + 1], VP = t->VL[L + 1];
 #pragma omp parallel for schedule(static)
@@ -185,7 +225,7 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
                         if (pu < UL && pv < VL) { mem[n] = t->X[c][L][pv * UL + pu]; srvp[n] = t->srv[c][L][pv * UL + pu]; ++n; }
                     }
                 int16_t *rk = t->X[c][L + 1][q];
-                for (size_t i = 0; i < npx; ++i) {
+                for (size_t i = 0; i < npc; ++i) {
                     int s = 0;
                     for (int k = 0; k < n; ++k) s += mem[k][i];
                     int r = round_mean(s, n);
@@ -199,30 +239,31 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
      * exhaustive phase-shifted search of every block of every predictive plane against the
      * UNTHRESHOLDED reference SRV of its cluster (R12 open loop). */
     for (int c = 0; c < 3; ++c) {
+        const int Wc = t->g.W[c], Hc = t->g.H[c], nbx = t->g.nbx[c], nby = t->g.nby[c], nblk = t->g.nblk[c];
         for (int L = 0; L < h; ++L) {
             int UL = t->UL[L], VL = t->VL[L];
             /* block energies for all planes */
 #pragma omp parallel for schedule(static)
             for (int pi = 0; pi < UL * VL; ++pi) {
-                orc_block *bk = t->blk[c][L] + (size_t)pi * t->nblk;
-                for (int by = 0; by < t->nby; ++by)
-                    for (int bx = 0; bx < t->nbx; ++bx) bk[by * t->nbx + bx].E = block_energy(t->srv[c][L][pi], Ws, B, bx, by);
+                orc_block *bk = t->blk[c][L] + (size_t)pi * nblk;
+                for (int by = 0; by < nby; ++by)
+                    for (int bx = 0; bx < nbx; ++bx) bk[by * nbx + bx].E = block_energy(t->srv[c][L][pi], Wc, B, bx, by);
             }
             for (int rv = 0; rv < VL; rv += 2)
                 for (int ru = 0; ru < UL; ru += 2) {
                     int rstride = 0;
-                    int16_t *pad = make_padded(t->srv[c][L][rv * UL + ru], Ws, Ht, W, &rstride);
+                    int16_t *pad = make_padded(t->srv[c][L][rv * UL + ru], Wc, Hc, W, &rstride);
                     if (!pad) goto nomem;
                     for (int j = 0; j < 2; ++j)
                         for (int i = 0; i < 2; ++i) {
                             int pu = ru + i, pv = rv + j;
                             if ((i | j) == 0 || pu >= UL || pv >= VL) continue;
                             const int16_t *P = t->srv[c][L][pv * UL + pu];
-                            orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->nblk;
+                            orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * nblk;
 #pragma omp parallel for schedule(dynamic, 4)
-                            for (int b = 0; b < t->nblk; ++b) {
+                            for (int b = 0; b < nblk; ++b) {
                                 int32_t r[4];
-                                search_block_padded(P, Ws, pad, rstride, B, W, b % t->nbx, b / t->nbx, r);
+                                search_block_padded(P, Wc, pad, rstride, B, W, b % nbx, b / nbx, r);
                                 bk[b].mode = r[0]; bk[b].dx = r[1]; bk[b].dy = r[2]; bk[b].sad = r[3];
                             }
                         }

@@ -59,7 +59,7 @@ typedef struct {
     int32_t nthreads;          /* OpenMP threads (<=0: all)                            */
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st; /* light slab      */
     uint8_t background[3];
-    uint8_t _pad;
+    uint8_t chroma;            /* 1: Co / Cg at half resolution (R18)    */
     uint64_t seed;             /* provenance only                                      */
 } orc_params;
 

@@ -15,15 +15,29 @@ typedef struct {
     int32_t flags; /* bit0 res, bit1 pred */
 } orc_block;
 
+/* Per-channel plane geometry.  PAPER.md:263: "the chroma channels are sub-sampled ... The hierarchy computation and motion
+ * compensation are performed separately on all the channels".  Reading R18: with p.chroma = 1 the Co and Cg planes of every input view
+ * are reduced to Ws/2 x Ht/2 by a 2 x 2 box mean rounded half away from zero right after the colour transform; every
+ * later step (hierarchy, search, thresholds, BISE, flag maps) runs on each channel at its own resolution with the same B and W; the
+ * decoder reads the chroma sample (s >> 1, t >> 1): nearest-neighbour replication back to full size.  Ws, Ht must be even and B must
+ * divide Ws/2 and Ht/2.  p.chroma = 0: all three channels at Ws x Ht. */
+typedef struct {
+    int W[3], H[3];          /* plane size of channel c        */
+    int nbx[3], nby[3], nblk[3];
+    int shift[3];            /* sample (s,t) -> (s >> shift, t >> shift) */
+} orc_geom;
+
+int orc__geom(const orc_params *p, orc_geom *g);  /* ORC_E_PARAM when the sizes do not divide */
+
 struct orc_tree {
     orc_params p;
+    orc_geom g;
     int h;
     int UL[ORC_MAX_LEVELS + 1], VL[ORC_MAX_LEVELS + 1];
-    int nbx, nby, nblk;
-    /* X[c][L][pv*UL+pu] : int16 [Ht*Ws], L = 0..h ; srv[c][L][...] : L = 0..h-1 */
+    /* X[c][L][pv*UL+pu] : int16 [g.H[c]*g.W[c]], L = 0..h ; srv[c][L][...] : L = 0..h-1 */
     int16_t **X[3][ORC_MAX_LEVELS + 1];
     int16_t **srv[3][ORC_MAX_LEVELS];
-    orc_block *blk[3][ORC_MAX_LEVELS]; /* [UL*VL][nblk] */
+    orc_block *blk[3][ORC_MAX_LEVELS]; /* [UL*VL][g.nblk[c]] */
     int thresholded;
 };
 
@@ -45,16 +59,16 @@ typedef struct {
 
 struct orc_stream {
     orc_params p;
+    orc_geom g;
     int h;
     int UL[ORC_MAX_LEVELS + 1], VL[ORC_MAX_LEVELS + 1];
-    int nbx, nby, nblk;
     uint8_t *bytes;
     size_t len;
     uint64_t off_rkv, off_dir, off_flags, off_payload, off_mv, total;
     uint64_t n_pc;
     orc_dirent *dir;            /* [n_pc] in stream order */
     uint64_t level_base[ORC_MAX_LEVELS]; /* first directory index of level L */
-    uint32_t **rank_res;        /* [n_pc][nblk+1] exclusive prefix counts (built at open) */
+    uint32_t **rank_res;        /* [n_pc][g.nblk[c]+1] exclusive prefix counts (built at open) */
     uint32_t **rank_pred;       /* same for pred maps (NULL for reference planes) */
     uint32_t mvN;               /* 2 (2W+1)^2 */
     int min_level;              /* progressive decoding (R26): the walk stops above this level; 0 = full quality */

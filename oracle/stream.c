@@ -38,9 +38,6 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
 {
     if (!t || !out || !t->thresholded) return ORC_E_PARAM;
     const int Ws = t->p.Ws, Ht = t->p.Ht, B = t->p.block, W = t->p.window, h = t->h;
-    const size_t npx = (size_t)Ws * Ht;
-    const int nblk = t->nblk;
-    const uint32_t fwords = (uint32_t)((nblk + 31) / 32);
     const uint32_t mvN = 2u * (uint32_t)(2 * W + 1) * (uint32_t)(2 * W + 1);
 
     uint64_t n_pc = 0;
@@ -54,6 +51,8 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
         for (int pv = 0; pv < t->VL[L]; ++pv)
             for (int pu = 0; pu < t->UL[L]; ++pu)
                 for (int c = 0; c < 3; ++c, ++k) {
+                    const int nblk = t->g.nblk[c];  /* every channel at its own resolution (R18) */
+                    const uint32_t fwords = (uint32_t)((nblk + 31) / 32);
                     const orc_block *bk = t->blk[c][L] + (size_t)(pv * t->UL[L] + pu) * nblk;
                     int vmin = 0, vmax = 0, first = 1;
                     uint32_t n_res = 0, n_pred = 0;
@@ -61,7 +60,7 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
                         if (bk[b].flags & 2) ++n_pred;
                         if (!(bk[b].flags & 1)) continue;
                         ++n_res;
-                        int bx = b % t->nbx, by = b / t->nbx;
+                        int bx = b % t->g.nbx[c], by = b / t->g.nbx[c];
                         for (int j = 0; j < B; ++j)
                             for (int i = 0; i < B; ++i) {
                                 int v = orc__stored_value(t, c, L, pu, pv, bx * B + i, by * B + j);
@@ -87,7 +86,8 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
                 }
 
     uint64_t n_top = (uint64_t)t->UL[h] * t->VL[h];
-    uint64_t rkv_bytes = n_top * npx * (1 + 2 + 2);
+    uint64_t rkv_bytes = 0;
+    for (int c = 0; c < 3; ++c) rkv_bytes += n_top * (uint64_t)t->g.W[c] * t->g.H[c] * (c == 0 ? 1 : 2);
     uint64_t off_rkv = ORC_HEADER_BYTES;
     uint64_t off_dir = align8(off_rkv + rkv_bytes);
     uint64_t off_flags = align8(off_dir + n_pc * ORC_DIRENT_BYTES);
@@ -106,7 +106,7 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
     wr32(s + 24, (uint32_t)h); wr32(s + 28, (uint32_t)B); wr32(s + 32, (uint32_t)W); wr32(s + 36, 3);
     wr32(s + 40, (uint32_t)t->p.tau_ref); wr32(s + 44, (uint32_t)t->p.tau_res);
     s[48] = 1; /* colour id: YCoCg-R */
-    s[49] = 0; /* chroma subsampling off (R18) */
+    s[49] = t->p.chroma ? 1 : 0; /* chroma subsampling (R18): Co / Cg planes at Ws/2 x Ht/2 */
     s[50] = 0; /* RKV codec: raw (R20) */
     s[51] = (uint8_t)t->p.policy;
     s[52] = t->p.background[0]; s[53] = t->p.background[1]; s[54] = t->p.background[2]; s[55] = 0;
@@ -125,15 +125,15 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
     {
         uint8_t *o = s + off_rkv;
         for (uint64_t i = 0; i < n_top; ++i)
-            for (size_t x = 0; x < npx; ++x) *o++ = (uint8_t)t->X[0][h][i][x];
+            for (size_t x = 0; x < (size_t)t->g.W[0] * t->g.H[0]; ++x) *o++ = (uint8_t)t->X[0][h][i][x];
         for (int c = 1; c < 3; ++c)
             for (uint64_t i = 0; i < n_top; ++i)
-                for (size_t x = 0; x < npx; ++x) { wr16(o, (uint32_t)(uint16_t)t->X[c][h][i][x]); o += 2; }
+                for (size_t x = 0; x < (size_t)t->g.W[c] * t->g.H[c]; ++x) { wr16(o, (uint32_t)(uint16_t)t->X[c][h][i][x]); o += 2; }
     }
 
     /* pass 2: directory, flag maps, payloads, motion vectors */
-    uint32_t *vals = (uint32_t *)malloc((size_t)nblk * B * B * sizeof(uint32_t));
-    uint32_t *mvs = (uint32_t *)malloc((size_t)nblk * sizeof(uint32_t));
+    uint32_t *vals = (uint32_t *)malloc((size_t)t->g.nblk[0] * B * B * sizeof(uint32_t));  /* channel 0 has the most blocks */
+    uint32_t *mvs = (uint32_t *)malloc((size_t)t->g.nblk[0] * sizeof(uint32_t));
     if (!vals || !mvs) { free(vals); free(mvs); free(dir); free(s); return ORC_E_NOMEM; }
     k = 0;
     for (int L = h - 1; L >= 0; --L)
@@ -141,6 +141,8 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
             for (int pu = 0; pu < t->UL[L]; ++pu)
                 for (int c = 0; c < 3; ++c, ++k) {
                     const orc_dirent *d = &dir[k];
+                    const int nblk = t->g.nblk[c];
+                    const uint32_t fwords = (uint32_t)((nblk + 31) / 32);
                     const orc_block *bk = t->blk[c][L] + (size_t)(pv * t->UL[L] + pu) * nblk;
                     int is_pred = orc_is_predictive(pu, pv);
                     uint8_t *e = s + off_dir + k * ORC_DIRENT_BYTES;
@@ -158,7 +160,7 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
                         }
                         if (!(bk[b].flags & 1)) continue;
                         fres[b >> 3] |= (uint8_t)(1u << (b & 7));
-                        int bx = b % t->nbx, by = b / t->nbx;
+                        int bx = b % t->g.nbx[c], by = b / t->g.nbx[c];
                         for (int j = 0; j < B; ++j)
                             for (int i = 0; i < B; ++i)
                                 vals[nv++] = (uint32_t)(orc__stored_value(t, c, L, pu, pv, bx * B + i, by * B + j) - d->offset);
@@ -214,22 +216,23 @@ orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err)
     s->off_rkv = rd64(bytes + 112); s->off_dir = rd64(bytes + 120); s->off_flags = rd64(bytes + 128);
     s->off_payload = rd64(bytes + 136); s->off_mv = rd64(bytes + 144); s->total = rd64(bytes + 152);
     const orc_params *p = &s->p;
-    if (rd16(bytes + 6) != ORC_HEADER_BYTES || nch != 3 || bytes[48] != 1 || bytes[49] != 0 || bytes[50] != 0 ||
+    s->p.chroma = bytes[49];
+    if (rd16(bytes + 6) != ORC_HEADER_BYTES || nch != 3 || bytes[48] != 1 || bytes[49] > 1 || bytes[50] != 0 ||
         p->U < 1 || p->V < 1 || p->Ws < 1 || p->Ht < 1 || p->height < 1 || p->height > ORC_MAX_LEVELS || p->block < 1 ||
-        p->block > 8 || p->window < 0 || p->window > 64 || (p->Ws % p->block) || (p->Ht % p->block)) {
+        p->block > 8 || p->window < 0 || p->window > 64 || orc__geom(p, &s->g) != ORC_OK) {
         free(s); *err = ORC_E_PARAM; return NULL;
     }
     if (len < s->total) { free(s); *err = ORC_E_TRUNCATED; return NULL; }
     s->h = p->height;
-    s->nbx = p->Ws / p->block; s->nby = p->Ht / p->block; s->nblk = s->nbx * s->nby;
     uint64_t n_pc = 0;
     for (int L = 0; L <= s->h; ++L) {
         s->UL[L] = (p->U + (1 << L) - 1) >> L;
         s->VL[L] = (p->V + (1 << L) - 1) >> L;
     }
     for (int L = s->h - 1; L >= 0; --L) { s->level_base[L] = n_pc; n_pc += (uint64_t)s->UL[L] * s->VL[L] * 3; }
-    uint64_t npx = (uint64_t)p->Ws * p->Ht;
-    if (n_pc != s->n_pc || s->off_rkv != ORC_HEADER_BYTES || s->off_dir < s->off_rkv + (uint64_t)s->UL[s->h] * s->VL[s->h] * npx * 5 ||
+    uint64_t rkv_bytes = 0;
+    for (int c = 0; c < 3; ++c) rkv_bytes += (uint64_t)s->UL[s->h] * s->VL[s->h] * (uint64_t)s->g.W[c] * s->g.H[c] * (c == 0 ? 1 : 2);
+    if (n_pc != s->n_pc || s->off_rkv != ORC_HEADER_BYTES || s->off_dir < s->off_rkv + rkv_bytes ||
         s->off_flags < s->off_dir + n_pc * ORC_DIRENT_BYTES || s->off_payload < s->off_flags || s->off_mv < s->off_payload ||
         s->total < s->off_mv) {
         free(s); *err = ORC_E_CORRUPT; return NULL;
@@ -242,8 +245,9 @@ orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err)
     s->rank_pred = (uint32_t **)calloc((size_t)n_pc, sizeof(uint32_t *));
     if (!s->bytes || !s->dir || !s->rank_res || !s->rank_pred) { orc_close(s); *err = ORC_E_NOMEM; return NULL; }
     memcpy(s->bytes, bytes, s->len);
-    const uint32_t fwords = (uint32_t)((s->nblk + 31) / 32);
     for (uint64_t k = 0; k < n_pc; ++k) {
+        const int nblk = s->g.nblk[k % 3];  /* channel = k % 3 (level bases are multiples of 3) */
+        const uint32_t fwords = (uint32_t)((nblk + 31) / 32);
         const uint8_t *e = s->bytes + s->off_dir + k * ORC_DIRENT_BYTES;
         orc_dirent *d = &s->dir[k];
         d->offset = (int32_t)rd32(e); d->N = rd32(e + 4); d->n_res = rd32(e + 8); d->n_pred = rd32(e + 12);
@@ -260,21 +264,21 @@ orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err)
         }
         /* rank directory: exclusive prefix popcounts of the flag maps */
         const uint8_t *fres = s->bytes + s->off_flags + d->flags_off;
-        uint32_t *rr = (uint32_t *)malloc((size_t)(s->nblk + 1) * sizeof(uint32_t));
+        uint32_t *rr = (uint32_t *)malloc((size_t)(nblk + 1) * sizeof(uint32_t));
         if (!rr) { orc_close(s); *err = ORC_E_NOMEM; return NULL; }
         s->rank_res[k] = rr;
         uint32_t acc = 0;
-        for (int b = 0; b < s->nblk; ++b) { rr[b] = acc; acc += (fres[b >> 3] >> (b & 7)) & 1u; }
-        rr[s->nblk] = acc;
+        for (int b = 0; b < nblk; ++b) { rr[b] = acc; acc += (fres[b >> 3] >> (b & 7)) & 1u; }
+        rr[nblk] = acc;
         if (acc != d->n_res) { orc_close(s); *err = ORC_E_CORRUPT; return NULL; }
         if (is_pred) {
             const uint8_t *fpred = fres + (size_t)fwords * 4;
-            uint32_t *rp = (uint32_t *)malloc((size_t)(s->nblk + 1) * sizeof(uint32_t));
+            uint32_t *rp = (uint32_t *)malloc((size_t)(nblk + 1) * sizeof(uint32_t));
             if (!rp) { orc_close(s); *err = ORC_E_NOMEM; return NULL; }
             s->rank_pred[k] = rp;
             acc = 0;
-            for (int b = 0; b < s->nblk; ++b) { rp[b] = acc; acc += (fpred[b >> 3] >> (b & 7)) & 1u; }
-            rp[s->nblk] = acc;
+            for (int b = 0; b < nblk; ++b) { rp[b] = acc; acc += (fpred[b >> 3] >> (b & 7)) & 1u; }
+            rp[nblk] = acc;
             if (acc != d->n_pred) { orc_close(s); *err = ORC_E_CORRUPT; return NULL; }
         } else if (d->n_pred != 0) { orc_close(s); *err = ORC_E_CORRUPT; return NULL; }
     }

@@ -23,8 +23,8 @@ int orc_tree_threshold(orc_tree *t, int tau_ref, int tau_res, int policy)
             int UL = t->UL[L], VL = t->VL[L];
             for (int pv = 0; pv < VL; ++pv)
                 for (int pu = 0; pu < UL; ++pu) {
-                    orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->nblk;
-                    for (int b = 0; b < t->nblk; ++b) {
+                    orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->g.nblk[c];
+                    for (int b = 0; b < t->g.nblk[c]; ++b) {
                         int res, pred = 0;
                         if (!orc_is_predictive(pu, pv)) {
                             res = bk[b].E >= tau_ref;
@@ -48,21 +48,22 @@ int orc_tree_threshold(orc_tree *t, int tau_ref, int tau_res, int policy)
     return ORC_OK;
 }
 
-/* value of plane (L,pu,pv,c) as STORED in the HMLFC tree at pixel (x,y), ignoring the res flag:
+/* value of plane (L,pu,pv,c) as STORED in the HMLFC tree at pixel (x,y) of that channel's plane, ignoring the res flag:
  * reference plane: the SRV sample; predictive plane: e = P - (pred ? +-R(x+dx,y+dy) : 0) with the
  * unthresholded reference R (R12), R = 0 outside the image (R8).  R10: sub: e = P - R; add: e = P + R. */
 static int stored_value(const orc_tree *t, int c, int L, int pu, int pv, int x, int y)
 {
     int UL = t->UL[L];
     int B = t->p.block;
-    int v = t->srv[c][L][pv * UL + pu][(size_t)y * t->p.Ws + x];
+    const int Wc = t->g.W[c], Hc = t->g.H[c];
+    int v = t->srv[c][L][pv * UL + pu][(size_t)y * Wc + x];
     if (!orc_is_predictive(pu, pv)) return v;
-    const orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->nblk + (y / B) * t->nbx + (x / B);
+    const orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->g.nblk[c] + (y / B) * t->g.nbx[c] + (x / B);
     if (bk->flags & 2) {
         int rx = x + bk->dx, ry = y + bk->dy;
         int r = 0;
-        if (rx >= 0 && rx < t->p.Ws && ry >= 0 && ry < t->p.Ht)
-            r = t->srv[c][L][(pv & ~1) * UL + (pu & ~1)][(size_t)ry * t->p.Ws + rx];
+        if (rx >= 0 && rx < Wc && ry >= 0 && ry < Hc)
+            r = t->srv[c][L][(pv & ~1) * UL + (pu & ~1)][(size_t)ry * Wc + rx];
         v = bk->mode ? v + r : v - r;
     }
     return v;
@@ -80,12 +81,12 @@ int orc_tree_get_plane(const orc_tree *t, int kind, int L, int pu, int pv, int c
 {
     if (!t || c < 0 || c > 2 || L < 0 || L > t->h || (kind != 0 && L >= t->h)) return ORC_E_PARAM;
     if (pu < 0 || pv < 0 || pu >= t->UL[L] || pv >= t->VL[L]) return ORC_E_PARAM;
-    size_t npx = (size_t)t->p.Ws * t->p.Ht;
+    size_t npx = (size_t)t->g.W[c] * t->g.H[c];  /* the channel's own plane size (R18) */
     if (kind == 0) memcpy(out, t->X[c][L][pv * t->UL[L] + pu], npx * sizeof(int16_t));
     else if (kind == 1) memcpy(out, t->srv[c][L][pv * t->UL[L] + pu], npx * sizeof(int16_t));
     else if (kind == 2) {
-        for (int y = 0; y < t->p.Ht; ++y)
-            for (int x = 0; x < t->p.Ws; ++x) out[(size_t)y * t->p.Ws + x] = (int16_t)stored_value(t, c, L, pu, pv, x, y);
+        for (int y = 0; y < t->g.H[c]; ++y)
+            for (int x = 0; x < t->g.W[c]; ++x) out[(size_t)y * t->g.W[c] + x] = (int16_t)stored_value(t, c, L, pu, pv, x, y);
     } else return ORC_E_PARAM;
     return ORC_OK;
 }
@@ -94,8 +95,8 @@ int orc_tree_get_blocks(const orc_tree *t, int L, int pu, int pv, int c, int32_t
 {
     if (!t || c < 0 || c > 2 || L < 0 || L >= t->h) return ORC_E_PARAM;
     if (pu < 0 || pv < 0 || pu >= t->UL[L] || pv >= t->VL[L]) return ORC_E_PARAM;
-    const orc_block *bk = t->blk[c][L] + (size_t)(pv * t->UL[L] + pu) * t->nblk;
-    for (int b = 0; b < t->nblk; ++b) {
+    const orc_block *bk = t->blk[c][L] + (size_t)(pv * t->UL[L] + pu) * t->g.nblk[c];
+    for (int b = 0; b < t->g.nblk[c]; ++b) {
         out[6 * b + 0] = bk[b].mode; out[6 * b + 1] = bk[b].dx; out[6 * b + 2] = bk[b].dy;
         out[6 * b + 3] = bk[b].sad;  out[6 * b + 4] = bk[b].E;  out[6 * b + 5] = bk[b].flags;
     }
@@ -117,12 +118,14 @@ int orc__stored_value(const orc_tree *t, int c, int L, int pu, int pv, int x, in
 int orc_tree_reconstruct(const orc_tree *t, uint8_t *lf_out)
 {
     if (!t || !lf_out || !t->thresholded) return ORC_E_PARAM;
-    const int Ws = t->p.Ws, Ht = t->p.Ht, B = t->p.block, h = t->h;
-    const size_t npx = (size_t)Ws * Ht;
+    const int B = t->p.block, h = t->h;
     const int nviews = t->p.U * t->p.V;
     int16_t *Y0[3];
     for (int c = 0; c < 3; ++c) Y0[c] = NULL;
     for (int c = 0; c < 3; ++c) {
+        /* every channel at its own resolution (R18) */
+        const int Ws = t->g.W[c], Ht = t->g.H[c], nbx = t->g.nbx[c], nblk = t->g.nblk[c];
+        const size_t npx = (size_t)Ws * Ht;
         /* Y[L] arrays of planes, built top-down */
         int16_t *above = (int16_t *)malloc((size_t)t->UL[h] * t->VL[h] * npx * sizeof(int16_t));
         if (!above) return ORC_E_NOMEM;
@@ -135,24 +138,24 @@ int orc_tree_reconstruct(const orc_tree *t, uint8_t *lf_out)
             for (int rv = 0; rv < VL; rv += 2)
                 for (int ru = 0; ru < UL; ru += 2) {
                     /* stored reference R' */
-                    const orc_block *rb = t->blk[c][L] + (size_t)(rv * UL + ru) * t->nblk;
+                    const orc_block *rb = t->blk[c][L] + (size_t)(rv * UL + ru) * nblk;
                     const int16_t *rs = t->srv[c][L][rv * UL + ru];
                     for (int y = 0; y < Ht; ++y)
                         for (int x = 0; x < Ws; ++x)
-                            Rp[(size_t)y * Ws + x] = (rb[(y / B) * t->nbx + (x / B)].flags & 1) ? rs[(size_t)y * Ws + x] : 0;
+                            Rp[(size_t)y * Ws + x] = (rb[(y / B) * nbx + (x / B)].flags & 1) ? rs[(size_t)y * Ws + x] : 0;
                     for (int j = 0; j < 2; ++j)
                         for (int i = 0; i < 2; ++i) {
                             int pu = ru + i, pv = rv + j;
                             if (pu >= UL || pv >= VL) continue;
                             const int16_t *par = above + (size_t)((pv >> 1) * UP + (pu >> 1)) * npx;
                             int16_t *dst = cur + (size_t)(pv * UL + pu) * npx;
-                            const orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->nblk;
+                            const orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * nblk;
                             for (int y = 0; y < Ht; ++y)
                                 for (int x = 0; x < Ws; ++x) {
                                     int s;
                                     if ((i | j) == 0) s = Rp[(size_t)y * Ws + x];
                                     else {
-                                        const orc_block *b = bk + (y / B) * t->nbx + (x / B);
+                                        const orc_block *b = bk + (y / B) * nbx + (x / B);
                                         s = (b->flags & 1) ? stored_value(t, c, L, pu, pv, x, y) : 0;
                                         if (b->flags & 2) {
                                             int rx = x + b->dx, ry = y + b->dy, q = 0;
@@ -170,11 +173,16 @@ int orc_tree_reconstruct(const orc_tree *t, uint8_t *lf_out)
         }
         Y0[c] = above;
     }
+    /* inverse colour at full resolution; a subsampled chroma plane is replicated (nearest neighbour, R18) */
+    const int Wf = t->p.Ws, Hf = t->p.Ht;
     for (int vi = 0; vi < nviews; ++vi)
-        for (size_t i = 0; i < npx; ++i) {
-            int r, g, b;
-            orc_ycocg_to_rgb(Y0[0][(size_t)vi * npx + i], Y0[1][(size_t)vi * npx + i], Y0[2][(size_t)vi * npx + i], &r, &g, &b);
-            uint8_t *o = lf_out + ((size_t)vi * npx + i) * 3;
+        for (int y = 0; y < Hf; ++y)
+          for (int x = 0; x < Wf; ++x) {
+            int r, g, b, a[3];
+            for (int c = 0; c < 3; ++c)
+                a[c] = Y0[c][(size_t)vi * t->g.W[c] * t->g.H[c] + (size_t)(y >> t->g.shift[c]) * t->g.W[c] + (x >> t->g.shift[c])];
+            orc_ycocg_to_rgb(a[0], a[1], a[2], &r, &g, &b);
+            uint8_t *o = lf_out + (((size_t)vi * Hf + y) * Wf + x) * 3;
             o[0] = (uint8_t)(r < 0 ? 0 : (r > 255 ? 255 : r));
             o[1] = (uint8_t)(g < 0 ? 0 : (g > 255 ? 255 : g));
             o[2] = (uint8_t)(b < 0 ? 0 : (b > 255 ? 255 : b));
