@@ -207,7 +207,7 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
 {
     if (!h || n < 0 || (n > 0 && (!d_coords || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->decode_variant == 1)
+    if (h->decode_variant == 1 || h->ds.cs)  // chroma-subsampled streams (R18): the per-sample kernels read them
         CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl,
@@ -221,7 +221,9 @@ int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_
     if (!h || n_views < 0 || (n_views > 0 && (!d_views || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
     // B = 4 streams: one lane per block-row segment; other block sizes (and decode variant 1 / 2, for cross-checks): one lane per pixel
-    if (h->ds.B == 4 && h->decode_variant == 0)
+    if (h->ds.cs)
+        CU(h, launch_decode_dense(h->ds, d_views, n_views, false, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_rows(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_views(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
@@ -233,7 +235,9 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
 {
     if (!h || n_blocks < 0 || (n_blocks > 0 && (!d_blocks || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->ds.B == 4 && h->decode_variant == 0)
+    if (h->ds.cs)
+        CU(h, launch_decode_dense(h->ds, d_blocks, n_blocks, true, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
+    else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_block_rows(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_blocks(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
@@ -252,7 +256,7 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the two fused kernels for 4 x 4 blocks
     const int rv = h->render_variant;
     const bool fused_ok = h->ds.B == 4 && (rv == 0 || (rv >= 6 && rv <= 12));
-    if (rv == 1 || (h->ds.lmin > 0 && !fused_ok))
+    if (rv == 1 || h->ds.cs || (h->ds.lmin > 0 && !fused_ok))
         CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
     else if (rv == 4 || rv == 5 || h->ds.B != 4)
         CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
@@ -406,6 +410,7 @@ static int footprint_common(hmlfc_handle *h, const hmlfc_camera *d_cameras, int 
                             int64_t n, hmlfc_footprint_t *out)
 {
     const DevStream &D = h->ds;
+    if (D.cs) return HMLFC_E_UNSUPPORTED;  // the counting kernels (a measurement aid) assume one block grid for the three channels
     const size_t blk_words = ((size_t)h->n_pc * (size_t)D.nblk + 31) / 32 + 1;
     const size_t rkv_words = ((size_t)D.UH * D.VH * D.Ht * D.Ws + 31) / 32 + 1;
     FootprintMarks mk{nullptr, nullptr};

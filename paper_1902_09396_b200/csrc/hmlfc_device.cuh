@@ -39,6 +39,10 @@ struct DevStream {
     int32_t U, V, Ws, Ht, h, B, logB, W;
     int32_t nbx, nby, nblk, fgroups;  // blocks per row / column / plane; 32-block groups per plane-channel
     int32_t UH, VH;                   // top-level RKV grid
+    // chroma subsampling (R18): cs = 1: the Co / Cg planes of every level are Ws/2 x Ht/2 (sample (s >> 1, t >> 1));
+    // their block grid is nbx_c x nby_c.  cs = 0: the chroma fields repeat the luma ones.  (The top-level RKVs are stored at full
+    // resolution on the device either way: hmlfc_load replicates subsampled chroma.)
+    int32_t cs, nbx_c, nby_c, nblk_c;
     uint32_t nd, nd2, nd_magic;       // 2W+1, (2W+1)^2, ceil(2^32 / nd)
     uint32_t mv_layout, mv_m;         // BISE layout of the motion records, N = 2 (2W+1)^2
     int32_t lmin;                     // progressive decoding (R26): levels below lmin are not summed; 0 = full quality
@@ -144,10 +148,10 @@ HMLFC_DEV int stored_value(const DevStream &S, uint4 d, uint4 fr, uint32_t bit, 
 }
 
 // reference-plane sample at (rx,ry): 0 outside the image (R8) or in an insignificant block
-HMLFC_DEV int reference_value(const DevStream &S, uint4 d, int rx, int ry)
+HMLFC_DEV int reference_value(const DevStream &S, uint4 d, int rx, int ry, int Wc, int Hc, int nbx)
 {
-    if ((unsigned)rx >= (unsigned)S.Ws || (unsigned)ry >= (unsigned)S.Ht) return 0;
-    int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+    if ((unsigned)rx >= (unsigned)Wc || (unsigned)ry >= (unsigned)Hc) return 0;
+    int b = (ry >> S.logB) * nbx + (rx >> S.logB);
     uint4 fr = ldg(S.flagrec + d.x + 4u * (uint32_t)(b >> 5));
     int kin = ((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1));
     return stored_value(S, d, fr, 1u << (b & 31), kin);
@@ -170,10 +174,10 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
     size_t ri = ((size_t)((v >> h) * S.UH + (u >> h)) * (size_t)S.Ht + (size_t)y) * (size_t)S.Ws + (size_t)x;
     short4 r = ldg(S.rkv + ri);
     acc[0] = r.x; acc[1] = r.y; acc[2] = r.z;
-    const int b = (y >> S.logB) * S.nbx + (x >> S.logB);
-    const uint32_t bit = 1u << (b & 31);
-    const uint32_t fg = (uint32_t)(b >> 5);
-    const int kin = ((y & (S.B - 1)) << S.logB) + (x & (S.B - 1));
+    // block, flag bit and position in the block for luma [0] and for chroma [1] (the chroma sample of (x,y) is (x >> cs, y >> cs), R18)
+    const int xc = x >> S.cs, yc = y >> S.cs;
+    const int b2[2] = {(y >> S.logB) * S.nbx + (x >> S.logB), (yc >> S.logB) * S.nbx_c + (xc >> S.logB)};
+    const int kin2[2] = {((y & (S.B - 1)) << S.logB) + (x & (S.B - 1)), ((yc & (S.B - 1)) << S.logB) + (xc & (S.B - 1))};
 #pragma unroll 1
     for (int L = S.lmin; L < h; ++L) {
         const int pu = u >> L, pv = v >> L;
@@ -183,6 +187,8 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
         const bool predictive = ((pu | pv) & 1) != 0;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
+            const int b = b2[c > 0], kin = kin2[c > 0];
+            const uint32_t bit = 1u << (b & 31), fg = (uint32_t)(b >> 5);
             uint4 d = ldg(S.pc + base + c);
             // the flag record's index follows from the plane-channel index (= d.x + 4 fg): both loads issue at once
             uint4 fr = ldg(S.flagrec + flag_index(S, base + (uint32_t)c, fg));
@@ -192,7 +198,8 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
                 uint32_t rec = bise_decode_at(S.mv + d.z, mi, S.mv_layout, S.mv_m);
                 int mode, dx, dy;
                 mv_unpack(S, rec, mode, dx, dy);
-                int q = reference_value(S, ldg(S.pc + rbase + c), x + dx, y + dy);
+                int q = c > 0 ? reference_value(S, ldg(S.pc + rbase + c), xc + dx, yc + dy, S.Ws >> S.cs, S.Ht >> S.cs, S.nbx_c)
+                              : reference_value(S, ldg(S.pc + rbase + c), x + dx, y + dy, S.Ws, S.Ht, S.nbx);
                 e += mode ? -q : q;  // R10: subtractive P = e + R, additive P = e - R
             }
             acc[c] += e;

@@ -52,6 +52,43 @@ decode_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, u
     store_rgb_warp(out + 3 * wbase, out_aligned && (wbase + 32 <= n), valid, rgb, stage[threadIdx.x >> 5]);
 }
 
+// hmlfc_decode_views / hmlfc_decode_blocks with one thread per pixel, the coordinates generated here (kBlocks: sample i is pixel
+// i mod B^2 of block blocks[i / B^2] = (u, v, bx, by); else pixel i mod (Ws Ht) of view views[i / (Ws Ht)] = (u, v)).  The path of
+// chroma-subsampled streams (R18), which the block-row and warp-cooperative kernels do not read.
+template <bool kBlocks>
+__global__ void __launch_bounds__(kDecodeThreads)
+decode_dense_kernel(const DevStream S, const int32_t *__restrict__ list, long long n, uint8_t *__restrict__ out, unsigned long long *oob,
+                    int out_aligned)
+{
+    __shared__ uint32_t stage[kDecodeThreads / 32][24];
+    const long long i = (long long)blockIdx.x * kDecodeThreads + threadIdx.x;
+    const bool valid = i < n;
+    uint32_t rgb = 0;
+    if (valid) {
+        int u, v, x, y;
+        bool ok;
+        if (kBlocks) {
+            const int bb = S.B * S.B;
+            const long long blk = i / bb;
+            const int k = (int)(i - blk * bb), ky = k >> S.logB;
+            const int4 q = __ldg(reinterpret_cast<const int4 *>(list) + blk);
+            u = q.x; v = q.y; x = q.z * S.B + (k - (ky << S.logB)); y = q.w * S.B + ky;
+            ok = (unsigned)q.z < (unsigned)S.nbx && (unsigned)q.w < (unsigned)S.nby;
+        } else {
+            const long long npx = (long long)S.Ws * S.Ht;
+            const long long view = i / npx;
+            const int pix = (int)(i - view * npx);
+            const int2 uv = __ldg(reinterpret_cast<const int2 *>(list) + view);
+            u = uv.x; v = uv.y; y = pix / S.Ws; x = pix - y * S.Ws;
+            ok = true;
+        }
+        if (ok && (unsigned)u < (unsigned)S.U && (unsigned)v < (unsigned)S.V) rgb = decode_rgb8(S, u, v, x, y);
+        else atomicAdd(oob, 1ull);
+    }
+    const long long wbase = i - (threadIdx.x & 31);
+    store_rgb_warp(out + 3 * wbase, out_aligned && (wbase + 32 <= n), valid, rgb, stage[threadIdx.x >> 5]);
+}
+
 // ---------------------------------------------------------------- hmlfc_render, one thread per output pixel
 // Ray set-up -> 16 taps -> 16 independent sample decodes -> quadrilinear blend -> RGB8 store.
 constexpr int kPixTx = 32, kPixTy = 8;
@@ -233,6 +270,20 @@ cudaError_t launch_decode(const DevStream &S, const int32_t *d_coords, int64_t n
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
     decode_kernel<<<(unsigned)blocks, kDecodeThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out,
                                                                 d_oob, aligned);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode_dense(const DevStream &S, const int32_t *d_list, int64_t n_items, bool blocks, uint8_t *d_out,
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches)
+{
+    if (n_items == 0) return cudaSuccess;
+    const long long n = (long long)n_items * (blocks ? (long long)S.B * S.B : (long long)S.Ws * S.Ht);
+    const long long ctas = (n + kDecodeThreads - 1) / kDecodeThreads;
+    if (ctas > 0x7fffffffLL) return cudaErrorInvalidValue;
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
+    if (blocks) decode_dense_kernel<true><<<(unsigned)ctas, kDecodeThreads, 0, st>>>(S, d_list, n, d_out, d_oob, aligned);
+    else decode_dense_kernel<false><<<(unsigned)ctas, kDecodeThreads, 0, st>>>(S, d_list, n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

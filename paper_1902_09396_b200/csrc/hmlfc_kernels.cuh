@@ -37,6 +37,9 @@ cudaError_t launch_decode_blocks(const DevStream &S, const int32_t *d_blocks, in
                                  cudaStream_t st, int *n_launches);
 cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks, int64_t n_blocks, uint8_t *d_out, unsigned long long *d_oob,
                                      cudaStream_t st, int *n_launches);
+// one thread per pixel of whole views (d_list = int32 [n][2]) or whole blocks (int32 [n][4]): any stream, incl. chroma-subsampled ones
+cudaError_t launch_decode_dense(const DevStream &S, const int32_t *d_list, int64_t n_items, bool blocks, uint8_t *d_out,
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches);
 cudaError_t launch_render_pixel(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out,
                                 cudaStream_t st, int *n_launches);
 // shape 0: 16 x 8 tiles (4 pixels per lane), 1: 8 x 8 tiles (2 pixels per lane)

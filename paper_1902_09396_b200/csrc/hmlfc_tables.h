@@ -91,9 +91,11 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
 
     if (rd16(s + 6) != kHeaderBytes) return HMLFC_E_CORRUPT;
     if (I.U < 1 || I.V < 1 || I.Ws < 1 || I.Ht < 1 || I.height < 1 || I.window < 0) return HMLFC_E_CORRUPT;
-    if (n_channels != 3 || colour_id != 1 || chroma != 0 || rkv_codec != 0) return HMLFC_E_UNSUPPORTED;
+    if (n_channels != 3 || colour_id != 1 || chroma > 1 || rkv_codec != 0) return HMLFC_E_UNSUPPORTED;
     if (I.height > kMaxLevels || I.window > 64) return HMLFC_E_UNSUPPORTED;
     if (!(I.block == 2 || I.block == 4 || I.block == 8) || (I.Ws % I.block) || (I.Ht % I.block)) return HMLFC_E_UNSUPPORTED;
+    // chroma subsampling (R18): Co / Cg planes at Ws/2 x Ht/2, which the blocks must tile as well
+    if (chroma && ((I.Ws & 1) || (I.Ht & 1) || ((I.Ws / 2) % I.block) || ((I.Ht / 2) % I.block))) return HMLFC_E_UNSUPPORTED;
     if ((uint64_t)I.U * I.V > (1u << 24) || (uint64_t)I.Ws * I.Ht > (1u << 26)) return HMLFC_E_UNSUPPORTED;
     if (I.U > 4096 || I.V > 4096 || I.Ws > 16384 || I.Ht > 16384) return HMLFC_E_UNSUPPORTED;  // packed tap indices
     if (len < total) return HMLFC_E_TRUNCATED;
@@ -102,6 +104,8 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     D.U = I.U; D.V = I.V; D.Ws = I.Ws; D.Ht = I.Ht; D.h = I.height; D.B = I.block; D.W = I.window;
     D.logB = I.block == 2 ? 1 : I.block == 4 ? 2 : 3;
     D.nbx = I.Ws / I.block; D.nby = I.Ht / I.block; D.nblk = D.nbx * D.nby; D.fgroups = (D.nblk + 31) / 32;
+    D.cs = chroma ? 1 : 0;
+    D.nbx_c = (I.Ws >> D.cs) / I.block; D.nby_c = (I.Ht >> D.cs) / I.block; D.nblk_c = D.nbx_c * D.nby_c;
     D.nd = 2u * I.window + 1u; D.nd2 = D.nd * D.nd;
     D.nd_magic = D.nd == 1 ? 0xFFFFFFFFu : (uint32_t)((0x100000000ull + D.nd - 1) / D.nd);
     bise_layout(2u * D.nd2, &D.mv_layout, &D.mv_m);
@@ -132,8 +136,9 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     D.UH = (I.U + (1 << I.height) - 1) >> I.height;
     D.VH = (I.V + (1 << I.height) - 1) >> I.height;
     const uint64_t npx = (uint64_t)I.Ws * I.Ht, n_top = (uint64_t)D.UH * D.VH;
+    const uint64_t npx_c = (uint64_t)(I.Ws >> D.cs) * (uint64_t)(I.Ht >> D.cs);  // samples of a chroma plane
     if (n_pc != n_pc_hdr || n_pc * (uint64_t)D.fgroups > 0xFFFFFFFFull) return HMLFC_E_CORRUPT;
-    if (off_rkv != kHeaderBytes || off_dir < off_rkv + n_top * npx * 5 || off_flags < off_dir + n_pc * kDirentBytes ||
+    if (off_rkv != kHeaderBytes || off_dir < off_rkv + n_top * (npx + 4 * npx_c) || off_flags < off_dir + n_pc * kDirentBytes ||
         off_pay < off_flags || off_mv < off_pay || total < off_mv)
         return HMLFC_E_CORRUPT;
     const uint64_t flags_len = off_pay - off_flags, pay_bits = (off_mv - off_pay) * 8, mv_bits = (total - off_mv) * 8;
@@ -152,7 +157,6 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     }
 
     // descriptors + flag/rank records
-    const uint64_t fbytes = (uint64_t)D.fgroups * 4;
     const uint32_t BB = (uint32_t)(I.block * I.block);
     uint64_t k = 0;
     for (int L = I.height - 1; L >= 0; --L)
@@ -164,11 +168,13 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     const uint32_t N = rd32(e + 4), n_res = rd32(e + 8), n_pred = rd32(e + 12);
                     const uint64_t foff = rd64(e + 16), pboff = rd64(e + 24), mboff = rd64(e + 32);
                     const bool is_pred = ((pu | pv) & 1) != 0;
+                    const int nblk_k = c == 0 ? D.nblk : D.nblk_c, fgroups_k = (nblk_k + 31) / 32;  // the channel's own block grid
+                    const uint64_t fbytes = (uint64_t)fgroups_k * 4;
                     uint32_t layout, m;
                     bise_layout(N, &layout, &m);
                     if (N < 1 || N > 4096 || offset < -32768 || offset > 32767 || e[40] != layout || e[41] != m ||
                         e[42] != (is_pred ? 1 : 0) || (pboff & 31) || (mboff & 31) || (foff & 3) ||
-                        n_res > (uint32_t)D.nblk || n_pred > (uint32_t)D.nblk ||
+                        n_res > (uint32_t)nblk_k || n_pred > (uint32_t)nblk_k ||
                         // subtraction form: the 64-bit offsets are untrusted and must not wrap
                         foff > flags_len || fbytes * (is_pred ? 2 : 1) > flags_len - foff ||
                         pboff > pay_bits || bise_nbits(layout, m, (uint64_t)n_res * BB) > pay_bits - pboff ||
@@ -182,10 +188,10 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     const uint8_t *fres = s + off_flags + foff;
                     const uint8_t *fprd = fres + fbytes;
                     uint32_t rr = 0, rp = 0;
-                    for (int g = 0; g < D.fgroups; ++g) {
+                    for (int g = 0; g < fgroups_k; ++g) {  // (a subsampled channel leaves the records of the plane's later groups empty)
                         uint32_t wr = rd32(fres + 4 * g), wp = is_pred ? rd32(fprd + 4 * g) : 0u;
-                        if (g == D.fgroups - 1 && (D.nblk & 31)) {  // ignore padding bits
-                            const uint32_t mask = (1u << (D.nblk & 31)) - 1u;
+                        if (g == fgroups_k - 1 && (nblk_k & 31)) {  // ignore padding bits
+                            const uint32_t mask = (1u << (nblk_k & 31)) - 1u;
                             wr &= mask; wp &= mask;
                         }
                         T.flagrec[frbase + 4ull * (uint64_t)g] = make_uint4(wr, rr, wp, rp);
@@ -202,10 +208,16 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     T.n_flagged += (uint64_t)rr + (uint64_t)rp;
                 }
 
-    // top-level RKVs: Y uint8 planes, then Co and Cg int16 LE planes -> short4 {Y, Co, Cg, 0} per sample
-    const uint8_t *py = s + off_rkv, *pco = py + n_top * npx, *pcg = pco + n_top * npx * 2;
-    for (uint64_t i = 0; i < n_top * npx; ++i)
-        T.rkv[i] = make_short4((short)py[i], (short)(int16_t)rd16(pco + 2 * i), (short)(int16_t)rd16(pcg + 2 * i), 0);
+    // top-level RKVs: Y uint8 planes, then Co and Cg int16 LE planes -> short4 {Y, Co, Cg, 0} per full-resolution sample (subsampled
+    // chroma is replicated here, once: nearest neighbour, R18)
+    const uint8_t *py = s + off_rkv, *pco = py + n_top * npx, *pcg = pco + n_top * npx_c * 2;
+    const uint64_t Wc = (uint64_t)(I.Ws >> D.cs);
+    for (uint64_t q = 0; q < n_top; ++q)
+        for (uint64_t y = 0; y < (uint64_t)I.Ht; ++y)
+            for (uint64_t x = 0; x < (uint64_t)I.Ws; ++x) {
+                const uint64_t i = q * npx + y * (uint64_t)I.Ws + x, ic = q * npx_c + (y >> D.cs) * Wc + (x >> D.cs);
+                T.rkv[i] = make_short4((short)py[i], (short)(int16_t)rd16(pco + 2 * ic), (short)(int16_t)rd16(pcg + 2 * ic), 0);
+            }
     return HMLFC_OK;
 }
 

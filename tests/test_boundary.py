@@ -55,7 +55,9 @@ def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
     bad_version = bytearray(data)
     bad_version[4] = 9
     chroma = bytearray(data)
-    chroma[49] = 1
+    chroma[49] = 2       # 0 = off, 1 = Co / Cg at half resolution (R18); anything else is not a layout this library reads
+    chroma_flip = bytearray(data)
+    chroma_flip[49] = 1  # a full-resolution stream that claims subsampled chroma: its directory no longer matches its flag maps
     bad_block = bytearray(data)
     bad_block[28] = 3
     bad_dir = bytearray(data)
@@ -68,7 +70,7 @@ def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
         w[off_dir + 48 + field:off_dir + 48 + field + 8] = value.to_bytes(8, "little")   # second entry: a plane-channel with blocks
         wraps.append((w, -6))
     cases = [(bad_magic, -1), (data[:6], -2), (data[:100], -2), (data[:len(data) // 2], -2), (bad_version, -3),
-             (chroma, -5), (bad_block, -5), (bad_dir, -6)] + wraps
+             (chroma, -5), (chroma_flip, -6), (bad_block, -5), (bad_dir, -6)] + wraps
     for blob, code in cases:
         rc, out = load(blob)
         assert rc == code and not out.value, (rc, code)
