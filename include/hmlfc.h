@@ -127,6 +127,19 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
 int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
                  void *cuda_stream);
 
+/* hmlfc_render_lod -- level of detail per view ("progressive decoding"; R26, R27): view k is rendered as by
+ * hmlfc_render with the tree walk stopped above level max(h_levels[k], the handle's min_level), i.e. from the representative key views of
+ * its level-h_levels[k] clusters: fewer lookups and bytes per sample for views that need less angular detail.
+ *   h_levels : HOST, int32 [n_views], each in [0, height]; the other arguments as for hmlfc_render.
+ * One kernel sequence per run of consecutive views with equal level, on `cuda_stream`; asynchronous.  HMLFC_E_INVALID for a level
+ * outside [0, height].
+ * hmlfc_lod_levels -- the distance rule that fills such an array (host arithmetic only): a viewer at distance d = |z_st - eye.z| from the
+ * image plane gets floor(log2(d / d0)) clamped to [0, height] (every doubling of the distance beyond d0 goes one level up); d0 <= 0
+ * gives level 0 everywhere.   h_cameras : HOST, hmlfc_camera [n_views];  h_levels : HOST, int32 [n_views] (out). */
+int hmlfc_render_lod(const hmlfc_handle *h, const hmlfc_camera *d_cameras, const int32_t *h_levels, int n_views, int W, int H,
+                     uint8_t *d_out, void *cuda_stream);
+int hmlfc_lod_levels(const hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, float d0, int32_t *h_levels);
+
 /* End-to-end variants with HOST buffers: copy the inputs to the device, run the same kernels,
  * copy the result back, synchronise.  Scratch device buffers live in the handle and grow on
  * demand (so these calls are not re-entrant on one handle).  The work is pipelined in
@@ -207,7 +220,8 @@ int hmlfc_hierarchy(const uint8_t *d_lf, int U, int V, int Ws, int Ht, int heigh
 /* Encoder, complete: RGB8 light field on the device -> compressed stream in host memory, every
  * arithmetic step in CUDA kernels: hmlfc_hierarchy, hmlfc_search for every predictive SRV image of every
  * level and channel, the replacement step and the two block thresholds (reference block
- * kept iff sum|block| >= tau_ref; predictive block per `policy`, R13: 0 adaptive, 1 all, 2 literal), BISE packing of
+ * kept iff sum|block| >= tau_ref; predictive block per `policy`, R13: 0 adaptive, 1 all, 2 literal, 3 no motion
+ * compensation at all = the RLFC hierarchy alone), BISE packing of
  * the stored blocks and of the joint motion records, in the BFS order of PAPER.md:276.  The host writes the
  * header, the raw top-level RKVs and the directory around the device-built sections ("Stream format v1").
  *   d_lf      device, uint8 [V][U][Ht][Ws][3] RGB8, 4-byte aligned (not modified)

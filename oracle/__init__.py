@@ -10,7 +10,7 @@ import numpy as np
 
 from . import build as _build
 
-POLICY_ADAPTIVE, POLICY_ALL, POLICY_LITERAL = 0, 1, 2
+POLICY_ADAPTIVE, POLICY_ALL, POLICY_LITERAL, POLICY_NOMOTION = 0, 1, 2, 3
 BISE_PLAIN, BISE_TRIT, BISE_QUINT = 0, 1, 2
 E_MAGIC, E_TRUNCATED, E_VERSION, E_PARAM, E_NOMEM, E_CORRUPT = -1, -2, -3, -4, -5, -6
 
@@ -76,6 +76,8 @@ def lib():
         "orc_decode_full": (C.c_int, [vp, vp, C.c_int]),
         "orc_render": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]),
         "orc_render_dense": (C.c_int, [vp, C.POINTER(Params), vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]),
+        "orc_render_lod": (C.c_int, [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, C.c_int]),
+        "orc_lod_level": (C.c_int, [C.POINTER(Params), vp, C.c_float]),
         "orc_ray_setup": (C.c_int, [C.POINTER(Params), vp, C.c_int, C.c_int, vp]),
         "orc_stats_decode": (C.c_int, [vp, vp, i64, C.POINTER(Stats)]),
         "orc_stats_render": (C.c_int, [vp, vp, C.c_int, C.c_int, C.c_int, C.POINTER(Stats)]),
@@ -312,6 +314,23 @@ class Stream:
         if rc:
             raise OracleError(rc, "render")
         return out
+
+    def render_lod(self, cams, levels, W, H, nthreads=0):
+        """Per-view level of detail (R27): view k is rendered with the walk stopped above levels[k]."""
+        cams = np.ascontiguousarray(cams, dtype=np.float32).reshape(-1, 16)
+        levels = np.ascontiguousarray(levels, dtype=np.int32)
+        assert levels.shape == (cams.shape[0],)
+        out = np.empty((cams.shape[0], H, W, 3), dtype=np.uint8)
+        rc = lib().orc_render_lod(self._h, _ptr(cams), _ptr(levels), cams.shape[0], W, H, _ptr(out), nthreads)
+        if rc:
+            raise OracleError(rc, "render_lod")
+        return out
+
+    def lod_levels(self, cams, d0):
+        """floor(log2(|z_st - eye.z| / d0)) clamped to [0, height], per camera."""
+        cams = np.ascontiguousarray(cams, dtype=np.float32).reshape(-1, 16)
+        p = self.params
+        return np.array([lib().orc_lod_level(C.byref(p), _ptr(cams[k]), C.c_float(d0)) for k in range(cams.shape[0])], dtype=np.int32)
 
     def stats_decode(self, coords):
         c = np.ascontiguousarray(coords, dtype=np.int32).reshape(-1, 4)

@@ -44,7 +44,9 @@ enum {
 };
 
 /* encoder policies for the per-block (pred,res) decision: DESIGN.md reading R13 */
-enum { ORC_POLICY_ADAPTIVE = 0, ORC_POLICY_ALL = 1, ORC_POLICY_LITERAL = 2 };
+/* ORC_POLICY_NOMOTION: no block is ever predicted -- the RLFC hierarchy without the motion compensation this paper adds (PAPER.md:183,
+ * "RLFC"; :375 compares HMLFC against it).  Same stream format, same decoder: a stream without motion records. */
+enum { ORC_POLICY_ADAPTIVE = 0, ORC_POLICY_ALL = 1, ORC_POLICY_LITERAL = 2, ORC_POLICY_NOMOTION = 3 };
 
 /* BISE layouts (section 4.6) */
 enum { ORC_BISE_PLAIN = 0, ORC_BISE_TRIT = 1, ORC_BISE_QUINT = 2 };
@@ -132,6 +134,9 @@ int orc_decode_full(const orc_stream *s, uint8_t *lf_out, int nthreads);
 /* ------------------------------------------------------------------ renderer */
 /* camera: 16 floats = eye[3], right[3], down[3], fwd[3], tan_half_x, tan_half_y, pad[2] */
 int orc_render(const orc_stream *s, const float *cams, int n_views, int W, int H, uint8_t *out, int nthreads);
+/* per-view level of detail (R27): view k stops the walk above levels[k]; orc_lod_level = floor(log2(|z_st - eye.z| / d0)) in [0, h] */
+int orc_render_lod(const orc_stream *s, const float *cams, const int32_t *levels, int n_views, int W, int H, uint8_t *out, int nthreads);
+int orc_lod_level(const orc_params *p, const float *cam, float d0);
 /* same sampling path, pixels taken from a dense RGB8 light field (pin: render-from-stream = render-from-LF) */
 int orc_render_dense(const uint8_t *lf, const orc_params *p, const float *cams, int n_views, int W, int H,
                      uint8_t *out, int nthreads);

@@ -14,7 +14,7 @@
  */
 int orc_tree_threshold(orc_tree *t, int tau_ref, int tau_res, int policy)
 {
-    if (!t || tau_ref < 0 || tau_res < 0 || policy < 0 || policy > 2) return ORC_E_PARAM;
+    if (!t || tau_ref < 0 || tau_res < 0 || policy < 0 || policy > 3) return ORC_E_PARAM;
     t->p.tau_ref = tau_ref;
     t->p.tau_res = tau_res;
     t->p.policy = policy;
@@ -36,9 +36,11 @@ int orc_tree_threshold(orc_tree *t, int tau_ref, int tau_res, int policy)
                         } else if (policy == ORC_POLICY_ALL) {
                             pred = 1;
                             res = bk[b].sad >= tau_res;
-                        } else {
+                        } else if (policy == ORC_POLICY_LITERAL) {
                             res = bk[b].sad >= tau_res;
                             pred = res;
+                        } else { /* ORC_POLICY_NOMOTION: the hierarchy alone (RLFC): predictive planes are coded intra */
+                            res = bk[b].E >= tau_res;
                         }
                         bk[b].flags = (res ? 1 : 0) | (pred ? 2 : 0);
                     }

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 
 # every symbol include/hmlfc.h declares
 EXPORTS = (
-    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_decode_blocks", "hmlfc_render", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_decode_blocks", "hmlfc_render", "hmlfc_render_lod", "hmlfc_lod_levels", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
     "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
@@ -74,6 +74,8 @@ def lib():
     L.hmlfc_decode_views.argtypes, L.hmlfc_decode_views.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_decode_blocks.argtypes, L.hmlfc_decode_blocks.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
+    L.hmlfc_render_lod.argtypes, L.hmlfc_render_lod.restype = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
+    L.hmlfc_lod_levels.argtypes, L.hmlfc_lod_levels.restype = [vp, vp, C.c_int, C.c_float, vp], C.c_int
     L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
     L.hmlfc_decode_views_host.argtypes, L.hmlfc_decode_views_host.restype = [vp, vp, i64, vp], C.c_int
     L.hmlfc_render_host.argtypes, L.hmlfc_render_host.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp], C.c_int
@@ -205,6 +207,30 @@ def hmlfc_render(h: Handle, cameras, W: int, H: int, out=None, stream=None):
     assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * H * W * 3
     _check(lib().hmlfc_render(h._h, C.c_void_p(cameras.data_ptr()), n, W, H, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
            "hmlfc_render", h._h)
+    return out
+
+
+def hmlfc_render_lod(h: Handle, cameras, levels: np.ndarray, W: int, H: int, out=None, stream=None):
+    """Per-view level of detail: cameras as for hmlfc_render, levels = HOST int32 [n_views] (numpy)."""
+    torch = _require_cuda()
+    assert cameras.is_cuda and cameras.dtype == torch.float32 and cameras.is_contiguous() and cameras.shape[-1] == 16
+    n = cameras.numel() // 16
+    levels = np.ascontiguousarray(levels, dtype=np.int32)
+    assert levels.shape == (n,)
+    if out is None:
+        out = torch.empty((n, H, W, 3), dtype=torch.uint8, device=cameras.device)
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * H * W * 3
+    _check(lib().hmlfc_render_lod(h._h, C.c_void_p(cameras.data_ptr()), levels.ctypes.data_as(C.c_void_p), n, W, H,
+                                  C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "hmlfc_render_lod", h._h)
+    return out
+
+
+def hmlfc_lod_levels(h: Handle, cameras: np.ndarray, d0: float) -> np.ndarray:
+    """The distance rule: HOST float32 [n_views][16] -> int32 [n_views] = floor(log2(|z_st - eye.z| / d0)) in [0, height]."""
+    cameras = np.ascontiguousarray(cameras, dtype=np.float32).reshape(-1, 16)
+    out = np.empty(cameras.shape[0], dtype=np.int32)
+    _check(lib().hmlfc_lod_levels(h._h, cameras.ctypes.data_as(C.c_void_p), cameras.shape[0], C.c_float(d0), out.ctypes.data_as(C.c_void_p)),
+           "hmlfc_lod_levels", h._h)
     return out
 
 

@@ -6,6 +6,7 @@
 #include "hmlfc_tables.h"
 
 #include <atomic>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -245,8 +246,9 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
     return HMLFC_OK;
 }
 
-int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
-                 void *cuda_stream)
+// hmlfc_render with the stream view D (= D, or D with another lmin: per-view level of detail)
+static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                       void *cuda_stream)
 {
     if (!h || n_views < 0 || W <= 0 || H <= 0 || n_views > 65535 || (n_views > 0 && (!d_cameras || !d_out))) return HMLFC_E_INVALID;
     static_assert(sizeof(hmlfc_camera) == sizeof(Camera) && sizeof(Camera) == 64, "camera layout");
@@ -255,11 +257,11 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the two fused kernels for 4 x 4 blocks
     const int rv = h->render_variant;
-    const bool fused_ok = h->ds.B == 4 && (rv == 0 || (rv >= 6 && rv <= 12));
-    if (rv == 1 || h->ds.cs || (h->ds.lmin > 0 && !fused_ok))
-        CU(h, launch_render_pixel(h->ds, cams, n_views, W, H, d_out, st, &nl));
-    else if (rv == 4 || rv == 5 || h->ds.B != 4)
-        CU(h, launch_render_warp(h->ds, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
+    const bool fused_ok = D.B == 4 && (rv == 0 || (rv >= 6 && rv <= 12));
+    if (rv == 1 || D.cs || (D.lmin > 0 && !fused_ok))
+        CU(h, launch_render_pixel(D, cams, n_views, W, H, d_out, st, &nl));
+    else if (rv == 4 || rv == 5 || D.B != 4)
+        CU(h, launch_render_warp(D, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
     else {
         // 0: chosen from the sizes -- views that look at about as many light-field samples as they have pixels (or more) go to the general
         // kernel with its largest arena, the others to the tile kernel (tables from a kernel of their own); 6 .. 10: the general kernel's five
@@ -267,20 +269,59 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
         int tiles = rv == 11 ? 0 : rv == 12 ? 1 : -1;
         // measured (ms per step, tile kernel with 3 / 4 CTAs per SM against the general kernel's best configuration): cfg2 0.67 / 0.95 /
         // 0.81, cfg4 0.91 / 1.27 / 1.04, cfg5 1.22 / 1.10 / 1.45; cfg3 (about one sample per pixel) 1.14 / 1.37 / 0.85
-        if (rv == 0 && (long long)W * H >= 2LL * h->ds.Ws * h->ds.Ht) tiles = (long long)W * H >= 8LL * h->ds.Ws * h->ds.Ht ? 1 : 0;
+        if (rv == 0 && (long long)W * H >= 2LL * D.Ws * D.Ht) tiles = (long long)W * H >= 8LL * D.Ws * D.Ht ? 1 : 0;
         if (tiles >= 0) {
             void *scratch = nullptr;
             cudaMemPool_t pool;
             CU(h, scratch_pool(&pool));
             CU(h, cudaMallocFromPoolAsync(&scratch, render_tiles_scratch_bytes(n_views, W, H), pool, st));
-            const cudaError_t e = launch_render_tiles(h->ds, cams, n_views, W, H, d_out, scratch, st, &nl, tiles);
+            const cudaError_t e = launch_render_tiles(D, cams, n_views, W, H, d_out, scratch, st, &nl, tiles);
             cudaFreeAsync(scratch, st);
             CU(h, e);
         } else {
-            CU(h, launch_render_cta(h->ds, cams, n_views, W, H, d_out, st, &nl, rv >= 6 ? rv - 6 : -1));
+            CU(h, launch_render_cta(D, cams, n_views, W, H, d_out, st, &nl, rv >= 6 ? rv - 6 : -1));
         }
     }
     h->launches += nl;
+    return HMLFC_OK;
+}
+
+int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                 void *cuda_stream)
+{
+    if (!h) return HMLFC_E_INVALID;
+    return render_impl(h, h->ds, d_cameras, n_views, W, H, d_out, cuda_stream);
+}
+
+int hmlfc_render_lod(const hmlfc_handle *h, const hmlfc_camera *d_cameras, const int32_t *h_levels, int n_views, int W, int H,
+                     uint8_t *d_out, void *cuda_stream)
+{
+    if (!h || n_views < 0 || W <= 0 || H <= 0 || (n_views > 0 && (!d_cameras || !d_out || !h_levels))) return HMLFC_E_INVALID;
+    for (int k = 0; k < n_views; ++k)
+        if (h_levels[k] < 0 || h_levels[k] > h->ds.h) return HMLFC_E_INVALID;
+    // one launch per run of consecutive views with the same level: the kernels take the level from the stream view
+    for (int k0 = 0; k0 < n_views;) {
+        int k1 = k0 + 1;
+        while (k1 < n_views && h_levels[k1] == h_levels[k0]) ++k1;
+        DevStream D = h->ds;
+        D.lmin = h_levels[k0] > D.lmin ? h_levels[k0] : D.lmin;
+        const int rc = render_impl(h, D, d_cameras + k0, k1 - k0, W, H, d_out + (size_t)k0 * (size_t)W * (size_t)H * 3u, cuda_stream);
+        if (rc != HMLFC_OK) return rc;
+        k0 = k1;
+    }
+    return HMLFC_OK;
+}
+
+int hmlfc_lod_levels(const hmlfc_handle *h, const hmlfc_camera *h_cameras, int n_views, float d0, int32_t *h_levels)
+{
+    if (!h || n_views < 0 || (n_views > 0 && (!h_cameras || !h_levels))) return HMLFC_E_INVALID;
+    for (int k = 0; k < n_views; ++k) {
+        const float d = std::fabs(h->ds.z_st - h_cameras[k].eye[2]);
+        int L = 0;
+        if (d0 > 0.0f)
+            while (L < h->ds.h && d >= d0 * (float)(2 << L)) ++L;
+        h_levels[k] = L;
+    }
     return HMLFC_OK;
 }
 

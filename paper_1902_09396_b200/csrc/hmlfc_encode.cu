@@ -129,9 +129,11 @@ classify_kernel(const int16_t *__restrict__ srv, const int4 *__restrict__ rec, c
             } else if (policy == 1) {
                 pred = true;
                 res = r.w >= tau_res;
-            } else {
+            } else if (policy == 2) {
                 res = r.w >= tau_res;
                 pred = res;
+            } else {  // 3: no motion compensation (the RLFC hierarchy alone): predictive planes coded intra
+                res = E >= tau_res;
             }
             if (pred) {
                 const int16_t *R = srv + pc.ref_off;
@@ -439,7 +441,7 @@ static int encode_impl(const uint8_t *d_lf, const hmlfc_encode_params_t *p_in, d
     hmlfc_encode_params_t prm = *p_in;
     hmlfc_encode_params_t *p = &prm;
     const int U = p->U, V = p->V, Ws = p->Ws, Ht = p->Ht, h = p->height, B = p->block, W = p->window;
-    if (U < 1 || V < 1 || Ws < 1 || Ht < 1 || h < 1 || p->tau_ref < 0 || p->tau_res < 0 || p->policy < 0 || p->policy > 2) return HMLFC_E_INVALID;
+    if (U < 1 || V < 1 || Ws < 1 || Ht < 1 || h < 1 || p->tau_ref < 0 || p->tau_res < 0 || p->policy < 0 || p->policy > 3) return HMLFC_E_INVALID;
     if (h > 8 || (B != 2 && B != 4 && B != 8) || W < 0 || W > 64 || Ws % B || Ht % B || Ws % 4 || (long long)U * V > (1 << 24))
         return HMLFC_E_UNSUPPORTED;  // what hmlfc_load accepts and hmlfc_hierarchy needs
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);

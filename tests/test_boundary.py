@@ -101,7 +101,7 @@ def test_entry_points_validate_arguments(P):
     assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -5    # B not in {2, 4, 8}
     p.block, p.Ws = 4, 18
     assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -5    # B does not divide Ws
-    p.Ws, p.policy = 16, 3
+    p.Ws, p.policy = 16, 4
     assert L.hmlfc_encode(dummy, C.byref(p), C.byref(out), C.byref(n), None, None) == -4    # unknown policy
     L.hmlfc_stream_free(None)  # no-op
 

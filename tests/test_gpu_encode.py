@@ -64,7 +64,7 @@ def test_encoded_stream_equals_the_oracle_stream(P, enc, name):
     assert stats["psnr"] == info["psnr"] or abs(stats["psnr"] - info["psnr"]) < 1e-9
 
 
-@pytest.mark.parametrize("policy", [orc.POLICY_ALL, orc.POLICY_LITERAL])
+@pytest.mark.parametrize("policy", [orc.POLICY_ALL, orc.POLICY_LITERAL, orc.POLICY_NOMOTION])
 @pytest.mark.parametrize("tau", [0, 37, 100000])
 def test_other_policies_and_degenerate_thresholds(P, policy, tau):
     # tau = 100000: no block survives (empty payload and, under `literal`, empty motion-vector strings)
@@ -246,7 +246,7 @@ def test_randomised_shapes_and_parameters(P):
         Ws, Ht = B * int(rng.integers(1, 7)), B * int(rng.integers(1, 6))
         if Ws % 4:
             Ws *= 2  # hmlfc_hierarchy needs Ws % 4 == 0
-        h, W, tau, policy = int(rng.integers(1, 5)), int(rng.integers(0, 10)), int(rng.integers(0, 121)), int(rng.integers(0, 3))
+        h, W, tau, policy = int(rng.integers(1, 5)), int(rng.integers(0, 10)), int(rng.integers(0, 121)), int(rng.integers(0, 4))
         tag = (case, U, V, Ws, Ht, h, B, W, tau, policy)
         lf = random_lf(rng, U, V, Ws, Ht, smooth=bool(case & 1))
         p = orc.make_params(U, V, Ws, Ht, h, B, W, tau // 2, tau, policy=policy, seed=case)

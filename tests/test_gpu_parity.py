@@ -479,3 +479,27 @@ def test_randomised_cameras_levels_and_geometries(P):
             assert np.array_equal(outs[variant], outs[P.RENDER_PIXEL]), (case, variant, L)
         P.hmlfc_free(hd)
     assert np.mean(hit) > 0.2 and np.mean(np.array(hit) < 0.98) > 0.5   # the cameras see the light field, and most frames also have misses
+
+
+@pytest.mark.parametrize("name", ["mini2", "mini4", "mini_b8", "cfg1_lossy"])
+def test_per_view_level_of_detail_matches_oracle(P, enc, name):
+    # DESIGN.md R27: view k at level levels[k]; the distance rule equals the oracle's (floor(log2(d / d0)) clamped to [0, h])
+    cfg, lf, data, info, s = enc(name)
+    h = _loaded(P, enc, name)
+    cams = wl.camera_path(cfg)
+    n = cams.shape[0]
+    rng = np.random.Generator(np.random.PCG64(cfg.seed + 5))
+    levels = rng.integers(0, cfg.height + 1, n).astype(np.int32)
+    levels[: min(3, n)] = [0, cfg.height, 0][: min(3, n)]
+    ref = s.render_lod(cams, levels, cfg.out_w, cfg.out_h)
+    for variant in (P.RENDER_AUTO, P.RENDER_PIXEL, P.RENDER_CTA, P.RENDER_TILES):
+        P.hmlfc_set_render_variant(h, variant)
+        got = P.hmlfc_render_lod(h, _dev(cams), levels, cfg.out_w, cfg.out_h).cpu().numpy()
+        assert np.abs(got.astype(np.int16) - ref.astype(np.int16)).max() <= TOL_VIEW, variant
+    P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+    moved = cams.copy().reshape(-1, 16)
+    moved[:, 2] -= np.linspace(0.0, 40.0, n, dtype=np.float32)   # viewers further and further from the image plane
+    for d0 in (0.5, 2.0, 7.0):
+        assert np.array_equal(P.hmlfc_lod_levels(h, moved, d0), s.lod_levels(moved, d0)), d0
+    with pytest.raises(P.HmlfcError):
+        P.hmlfc_render_lod(h, _dev(cams), np.full(n, cfg.height + 1, dtype=np.int32), cfg.out_w, cfg.out_h)

@@ -187,3 +187,31 @@ def test_cameras_coords_and_sharding_are_seeded():
     spans = [wl.shard(64, r, 3) for r in range(3)]
     assert spans == [(0, 22), (22, 43), (43, 64)]
     assert wl.all_coords(wl.CONFIGS["cfg1"]).shape == (262144, 4)
+
+
+def test_per_view_level_of_detail_is_the_progressive_decoder_view_by_view():
+    # R27: view k rendered at level levels[k] = the R26 decoder at that level on that view alone (R26 is pinned by the hierarchy itself:
+    # level L of a lossless stream is the cluster key view X_L); the distance rule is floor(log2(d / d0)) clamped to [0, h]
+    import workloads as wl
+
+    cfg = wl.CONFIGS["mini3"]
+    lf = wl.light_field(cfg)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, cfg.window, 10, 20, geometry=wl.geometry(cfg))
+    t = orc.Tree(lf, p)
+    s = orc.Stream(t.serialize())
+    t.close()
+    cams = wl.camera_path(cfg)
+    n = cams.shape[0]
+    levels = np.arange(n, dtype=np.int32) % (cfg.height + 1)
+    got = s.render_lod(cams, levels, 40, 28)
+    for k in range(n):
+        s.set_min_level(int(levels[k]))
+        assert np.array_equal(got[k], s.render(cams[k:k + 1], 40, 28)[0])
+    s.set_min_level(0)
+    # the rule, against its closed form: distance = |z_st - eye.z|
+    z_st = wl.geometry(cfg)["z_st"]
+    cam = np.array(cams[0], dtype=np.float32).reshape(16).copy()
+    for d, want in ((0.5, 0), (1.0, 0), (1.99, 0), (2.0, 1), (3.9, 1), (4.0, 2), (8.0, 3), (1000.0, cfg.height)):
+        cam[2] = z_st - d
+        assert s.lod_levels(cam[None], 1.0)[0] == min(want, cfg.height), d
+    assert s.lod_levels(cam[None], 0.0)[0] == 0
