@@ -168,11 +168,12 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
  * (per-view footprint boxes, block-ROW tasks: 4 BISE values per lane from two 64-bit windows):
  * 6 .. 10 = the general kernel (tile tables built inside the CTA, quadtree of sub-tile passes): 256 threads per
  * 32 x 32 tile with a 65 KB (3 CTAs per SM) / 103 KB (2) / 46 KB (4) shared-memory arena, 1024 threads per
- * 64 x 64 tile, 512 threads per 64 x 32 tile; 11 / 12 = the tile kernel (tables of all tiles from a kernel of
- * their own, one pass per 32 x 32 tile, 3 / 4 CTAs per SM; two launches per call and a scratch buffer from the
- * library's stream-ordered pool).  The automatic choice takes 7 when a view has fewer than twice the pixels of
- * a light-field image (little magnification: many samples per tile), 12 when it has at least eight times as
- * many, else 11. */
+ * 64 x 64 tile, 512 threads per 64 x 32 tile; 11 .. 15 = the tile kernel (tables of all tiles from a kernel of
+ * their own, one pass per tile; two launches per call and a scratch buffer from the library's stream-ordered
+ * pool): 32 x 32 tile with 3 / 4 CTAs per SM, 64 x 32 tile with 512 threads, 64 x 32 tile with 256 threads (8
+ * pixels per thread) and 2 / 3 CTAs per SM.  The automatic choice takes 7 when a view has fewer than twice the
+ * pixels of a light-field image (little magnification: many samples per tile), 15 when it has at least eight
+ * times as many, else 11. */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Progressive decoding (PAPER.md:57, :183 name the property; R26): hmlfc_decode / hmlfc_render sum the top-level RKV and the

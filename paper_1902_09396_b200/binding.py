@@ -20,9 +20,10 @@ EXPORTS = (
 )
 
 RENDER_AUTO, RENDER_PIXEL, RENDER_WARP, RENDER_WARP8, RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL = 0, 1, 4, 5, 6, 7, 8
-RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4 = 9, 10, 11, 12
+RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4, RENDER_TILES_W512, RENDER_TILES_W256, RENDER_TILES_W256X3 = 9, 10, 11, 12, 13, 14, 15
 # every configuration of the two fused kernels for 4 x 4 blocks (all give the same bytes; hmlfc_set_render_variant forces one)
-RENDER_FUSED = (RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL, RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4)
+RENDER_FUSED = (RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL, RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4,
+                RENDER_TILES_W512, RENDER_TILES_W256, RENDER_TILES_W256X3)
 DECODE_AUTO, DECODE_THREAD, DECODE_QUEUE, DECODE_QUEUE_LAZY = 0, 1, 2, 3
 
 

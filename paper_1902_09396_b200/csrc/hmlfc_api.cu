@@ -257,7 +257,7 @@ static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_ca
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the two fused kernels for 4 x 4 blocks
     const int rv = h->render_variant;
-    const bool fused_ok = D.B == 4 && (rv == 0 || (rv >= 6 && rv <= 12));
+    const bool fused_ok = D.B == 4 && (rv == 0 || (rv >= 6 && rv <= 15));
     if (rv == 1 || D.cs || (D.lmin > 0 && !fused_ok))
         CU(h, launch_render_pixel(D, cams, n_views, W, H, d_out, st, &nl));
     else if (rv == 4 || rv == 5 || D.B != 4)
@@ -266,10 +266,12 @@ static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_ca
         // 0: chosen from the sizes -- views that look at about as many light-field samples as they have pixels (or more) go to the general
         // kernel with its largest arena, the others to the tile kernel (tables from a kernel of their own); 6 .. 10: the general kernel's five
         // configurations; 11 / 12: the tile kernel with 3 / 4 CTAs per SM.  All give identical bytes.
-        int tiles = rv == 11 ? 0 : rv == 12 ? 1 : -1;
-        // measured (ms per step, tile kernel with 3 / 4 CTAs per SM against the general kernel's best configuration): cfg2 0.67 / 0.95 /
-        // 0.81, cfg4 0.91 / 1.27 / 1.04, cfg5 1.22 / 1.10 / 1.45; cfg3 (about one sample per pixel) 1.14 / 1.37 / 0.85
-        if (rv == 0 && (long long)W * H >= 2LL * D.Ws * D.Ht) tiles = (long long)W * H >= 8LL * D.Ws * D.Ht ? 1 : 0;
+        int tiles = rv >= 11 && rv <= 15 ? rv - 11 : -1;
+        // measured, ms per step (tile kernel 32 x 32 x 3 CTAs / 32 x 32 x 4 CTAs / 64 x 32 with 512 threads / 64 x 32 with 256 threads x 2 CTAs /
+        // 64 x 32 with 256 threads x 3 CTAs, against the general kernel's best configuration): cfg2 0.66 / 0.93 / 0.67 / 0.70 / 1.09 (0.81),
+        // cfg4 0.88 / 1.26 / 0.90 / 0.97 / 1.39 (1.00), cfg5 1.18 / 1.07 / 1.05 / 1.18 / 0.97 (1.50); cfg3 (about one sample per pixel) 1.06 / 1.28 /
+        // 1.12 / 1.44 / 1.50 (0.84)
+        if (rv == 0 && (long long)W * H >= 2LL * D.Ws * D.Ht) tiles = (long long)W * H >= 8LL * D.Ws * D.Ht ? 4 : 0;
         if (tiles >= 0) {
             void *scratch = nullptr;
             cudaMemPool_t pool;
@@ -496,7 +498,7 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
 
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 12 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
+    if (!h || variant < 0 || variant > 15 || variant == 2 || variant == 3) return HMLFC_E_INVALID;  // 2, 3: removed kernels
     h->render_variant = variant;
     return HMLFC_OK;
 }

@@ -54,7 +54,8 @@ cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_vi
                               int *n_launches, int config);
 // launch_render_tiles (hmlfc_render_tiles.cu): tile tables built by a kernel of their own from the tiles' border rays, one pass per 32 x 32
 // tile (a tile that does not fit takes the general kernel's path in its CTA).  d_scratch: render_tiles_scratch_bytes() bytes of device
-// memory for the tables (contents irrelevant before, undefined after).  config: 0 = 3 CTAs per SM, 1 = 4 CTAs per SM.
+// memory for the tables (contents irrelevant before, undefined after).  config: 0 / 1 = 32 x 32 tiles, 3 / 4 CTAs per SM; 2 = 64 x 32 tiles, 512 threads;
+// 3 / 4 = 64 x 32 tiles, 256 threads (8 pixels per thread), 2 / 3 CTAs per SM.
 size_t render_tiles_scratch_bytes(int n_views, int W, int H);
 cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, void *d_scratch,
                                 cudaStream_t st, int *n_launches, int config);

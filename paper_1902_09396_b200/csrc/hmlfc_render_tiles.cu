@@ -25,7 +25,7 @@ namespace hmlfc {
 
 namespace {
 
-constexpr int kTile = 32;
+constexpr int kTile = 32;        // tile height; the width is 32 or 64 (template parameter kTW)
 constexpr int kTablesWarps = 4;  // tiles per CTA of tile_tables_kernel
 constexpr int kDescWords = (int)(sizeof(TileTables) / 16);
 static_assert(sizeof(TileTables) % 16 == 0 && sizeof(TileHeader) == 64 && sizeof(ViewInfo) == 32 && sizeof(SlotInfo) == 64 &&
@@ -58,8 +58,8 @@ __device__ __forceinline__ float ray_uvst(const DevStream &S, const Camera &cam,
 // ---------------------------------------------------------------------------------------------------------------
 // One warp per 32 x 32 tile: footprint ranges from the border pixels, then the tile's tables -> tables[tile].
 __global__ void __launch_bounds__(kTablesWarps * 32)
-tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, int tiles_x, int tiles_y, int n_tiles,
-                   uint4 *__restrict__ tables)
+tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, int tile_w, int tiles_x, int tiles_y,
+                   int n_tiles, uint4 *__restrict__ tables)
 {
     __shared__ TileTables stage[kTablesWarps];
     __shared__ Camera s_cam[kTablesWarps];
@@ -76,8 +76,8 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
     if (lane < 2) camera_affine(S, cam, lane, s_aff[warp][lane]);
 
     // ---- corner pixels, one per lane
-    const int x0 = tx * kTile, y0 = ty * kTile;
-    const int pw = min(kTile, W - x0), ph = min(kTile, H - y0);
+    const int x0 = tx * tile_w, y0 = ty * kTile;
+    const int pw = min(tile_w, W - x0), ph = min(kTile, H - y0);
     int kmin[4] = {0x7fffffff, 0x7fffffff, 0x7fffffff, 0x7fffffff}, kmax[4] = {(int)0x80000000, (int)0x80000000, (int)0x80000000, (int)0x80000000};
     bool regular = true;
     if (lane < 4) {
@@ -140,25 +140,33 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
 }
 
 // the general path as a call: its registers and spills stay out of the tile kernel's own allocation (the call is rare)
-template <int kArenaBytes>
+template <int kArenaBytes, int kNT, int kTW>
 __device__ __noinline__ void general_tile_call(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int W, int H, uint8_t *__restrict__ out,
                                                int out_aligned, int view, int tile_x, int tile_y)
 {
-    render_tile_general<kArenaBytes, 256, kTile>(S, ctl, arena, W, H, out, out_aligned, view, tile_x, tile_y);
+    // the general path's tile is kTW x (4 kNT / kTW) pixels: one call, or two for the 64 x 32 tile of 256 threads (64 x 16 each)
+    constexpr int kGenTH = kNT * kPPL / kTW;
+    for (int part = 0; part < kTile / kGenTH; ++part)
+        render_tile_general<kArenaBytes, kNT, kTW>(S, ctl, arena, W, H, out, out_aligned, view, tile_x, tile_y * (kTile / kGenTH) + part);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-template <int kArenaBytes, int kMinBlocks, bool kAllPow2>
-__global__ void __launch_bounds__(256, kMinBlocks)
+// kTW x 32 pixels per CTA of kNT threads: 32 x 32 / 256 (4 pixels per thread), 64 x 32 / 512 (4), 64 x 32 / 256 (8)
+template <int kArenaBytes, int kMinBlocks, bool kAllPow2, int kNT, int kTW>
+__global__ void __launch_bounds__(kNT, kMinBlocks)
 render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned,
                     const uint4 *__restrict__ tables)
 {
-    constexpr int kNT = 256;
+    constexpr int kTPR = kNT / kTile;        // threads per pixel row: thread (tid % kTPR, tid / kTPR) owns pixels x = tid % kTPR + kTPR p of its row
+    constexpr int kPPT = kTW / kTPR;         // pixels per thread
+    constexpr int kCPL = kTW / 32;           // tile columns per lane (screen x computed once per column)
+    constexpr int kRPW = 32 / kTPR;          // pixel rows per warp
+    static_assert(kTPR == 8 || kTPR == 16, "quarter warps gather for 8 neighbouring pixels");
     extern __shared__ __align__(16) unsigned char arena[];
     __shared__ Ctl ctl;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int view = blockIdx.z;
-    const int ox = blockIdx.x * kTile, oy = blockIdx.y * kTile;
+    const int ox = blockIdx.x * kTW, oy = blockIdx.y * kTile;
     const uint4 *td = tables + (size_t)((view * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * kDescWords;
     PHASE_MARK(-1);
 
@@ -179,7 +187,8 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
 
     if (hd.status == kTileBackground) {
         const uint32_t rgb[4] = {bg, bg, bg, bg};
-        store4(out, view, W, H, ox + (tid & 7) * kPPL, oy + (tid >> 3), rgb, out_aligned);
+        for (int q = tid; q < kTW / kPPL * kTile; q += kNT)
+            store4(out, view, W, H, ox + (q % (kTW / kPPL)) * kPPL, oy + q / (kTW / kPPL), rgb, out_aligned ? 1 : 0);
         return;
     }
     bool fast = hd.status == kTileTables && tables_fit<kArenaBytes>(hd);
@@ -200,49 +209,53 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
         // irregular rays, more than 4 x 4 views, or tables / records that do not fit the arena: the general path, in this CTA
         reset_ctl(ctl);
         if (tid < 2) camera_affine(S, ctl.cam, tid, ctl.aff[tid]);
-        general_tile_call<kArenaBytes>(S, ctl, arena, W, H, out, out_aligned, view, (int)blockIdx.x, (int)blockIdx.y);
+        general_tile_call<kArenaBytes, kNT, kTW>(S, ctl, arena, W, H, out, out_aligned ? 1 : 0, view, (int)blockIdx.x, (int)blockIdx.y);
         return;
     }
 
-    // ------------------------------------------------ A + C: per pixel, ray -> 16 taps -> gather + blend.  Thread (tid & 7, tid >> 3) owns
-    // pixels x = (tid & 7) + 8 p of row tid >> 3: the 8 lanes of a quarter warp gather for 8 NEIGHBOURING pixels at a time, whose taps are the
+    // ------------------------------------------------ A + C: per pixel, ray -> 16 taps -> gather + blend.  Thread (tid % kTPR, tid / kTPR) owns
+    // pixels x = tid % kTPR + kTPR p of its row: the 8 lanes of a quarter warp gather for 8 NEIGHBOURING pixels at a time, whose taps are the
     // same few patch cells (one shared-memory wavefront per 128-bit load, where pixels 4 apart spread over 13 cells and collide)
     const Camera &cam = ctl.cam;
     const float4 *patch = reinterpret_cast<const float4 *>(arena + (((size_t)hd.nacc * 8 + 15) & ~(size_t)15));
     // screen coordinates once per column / row of the tile, shared by shuffles
-    const float pxl = ray_screen(cam.tan_half_x, W, ox + lane);
-    const float pyl = ray_screen(cam.tan_half_y, H, oy + warp * 4 + (lane & 3));
-    const float py = __shfl_sync(FULL, pyl, lane >> 3);
-    const int tx = tid & 7, y = oy + (tid >> 3);
-    uint32_t rgb[kPPL];
+    float pxl[kCPL];
 #pragma unroll
-    for (int p = 0; p < kPPL; ++p) {
-        const float px = __shfl_sync(FULL, pxl, tx + 8 * p);
+    for (int j = 0; j < kCPL; ++j) pxl[j] = ray_screen(cam.tan_half_x, W, ox + 32 * j + lane);
+    const float pyl = ray_screen(cam.tan_half_y, H, oy + warp * kRPW + (lane % kRPW));
+    const float py = __shfl_sync(FULL, pyl, lane / kTPR);
+    const int tx = tid % kTPR, y = oy + tid / kTPR;
+    uint32_t rgb[kPPT];
+#pragma unroll
+    for (int p = 0; p < kPPT; ++p) {
+        const int xr = tx + kTPR * p;  // column of the tile: computed by lane xr % 32 as its value xr / 32
+        const float px = __shfl_sync(FULL, pxl[xr / 32 < kCPL ? xr / 32 : 0], xr & 31);
         rgb[p] = bg;
-        if (ox + tx + 8 * p < W && y < H) {
+        if (ox + xr < W && y < H) {
             const Ray r = ray_from_screen_t<kAllPow2>(S, cam, px, py);
             if (r.hit) rgb[p] = blend_taps<true>(S, ctl, patch, tap_setup(S, r), hd.bu0, hd.bv0);
         }
     }
     PHASE_MARK(9);
     // ------------------------------------------------ stores.  Whole tiles of a 16-byte-aligned output: the tile's pixels are staged in
-    // shared memory (the accumulators are dead) and leave as 16-byte stores, 6 per 96-byte row, every sector written once.
-    if (out_aligned == 2 && ox + kTile <= W && oy + kTile <= H) {
-        constexpr int kStride = 40;  // words per staged row: the 4 rows x 8 columns a warp writes per step fall into 32 different banks
+    // shared memory (the accumulators are dead) and leave as 16-byte stores, 6 per 96 bytes of a row, every sector written once.
+    if (out_aligned == 2 && ox + kTW <= W && oy + kTile <= H) {
+        constexpr int kStride = kTW + 8;  // words per staged row: the rows x columns a warp writes per step fall into 32 different banks
+        constexpr int kChunks = 3 * kTW / 16;   // 16-byte chunks per row
         uint32_t *stage = reinterpret_cast<uint32_t *>(arena);
         if (hd.nacc * 8 < kTile * kStride * 4) __syncthreads();  // (CTA-uniform) the stage reaches into the patch: every pixel has gathered
 #pragma unroll
-        for (int p = 0; p < kPPL; ++p) stage[(tid >> 3) * kStride + tx + 8 * p] = rgb[p];
+        for (int p = 0; p < kPPT; ++p) stage[(tid / kTPR) * kStride + tx + kTPR * p] = rgb[p];
         __syncthreads();
-        if (tid < 6 * kTile) {
-            const int row = tid / 6, k = tid - row * 6;
+        for (int q = tid; q < kChunks * kTile; q += kNT) {
+            const int row = q / kChunks, k = q - row * kChunks;
             const uint32_t *src = stage + row * kStride;
             uint32_t w[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 // output word at byte b of the row's RGB stream: pixel b / 3 from its byte b % 3 on, then the next pixel
                 const int b = 16 * k + 4 * j, a = (b * 21846) >> 16, r = b - 3 * a;
-                const uint32_t lo = src[a], hi = a + 1 < kTile ? src[a + 1] : 0u;
+                const uint32_t lo = src[a], hi = a + 1 < kTW ? src[a + 1] : 0u;
                 w[j] = (lo >> (8 * r)) | (hi << (24 - 8 * r));
             }
             uint8_t *o = out + 3 * (((size_t)view * H + (size_t)(oy + row)) * (size_t)W + (size_t)ox) + 16 * k;
@@ -250,8 +263,8 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
         }
     } else {
 #pragma unroll
-        for (int p = 0; p < kPPL; ++p) {
-            const int x = ox + tx + 8 * p;
+        for (int p = 0; p < kPPT; ++p) {
+            const int x = ox + tx + kTPR * p;
             if (x < W && y < H) {
                 uint8_t *o = out + 3 * (((size_t)view * H + (size_t)y) * (size_t)W + (size_t)x);
                 o[0] = (uint8_t)(rgb[p] & 0xFF);
@@ -263,10 +276,16 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
     PHASE_MARK(10);
 }
 
-// 3 CTAs x 65 KB or 4 CTAs x 46 KB per SM (233,472 bytes of shared memory per SM, 1 KB reserved and 9.4 KB of tables per CTA)
+// 233,472 bytes of shared memory per SM, 1 KB reserved and 9.4 KB of tables per CTA
+//   0: 32 x 32 tile, 256 threads, 3 CTAs x 65 KB     1: 32 x 32, 256 threads, 4 CTAs x 46 KB
+//   2: 64 x 32 tile, 512 threads, 2 CTAs x 103 KB    3: 64 x 32, 256 threads (8 pixels per thread), 2 CTAs x 103 KB
+//   4: 64 x 32 tile, 256 threads, 3 CTAs x 65 KB
 #define HMLFC_TILES_CONFIGS(X) \
-    X(0, 65 * 1024, 3) \
-    X(1, 46 * 1024, 4)
+    X(0, 65 * 1024, 3, 256, 32) \
+    X(1, 46 * 1024, 4, 256, 32) \
+    X(2, 103 * 1024, 2, 512, 64) \
+    X(3, 103 * 1024, 2, 256, 64) \
+    X(4, 65 * 1024, 3, 256, 64)
 
 }  // namespace
 
@@ -282,16 +301,16 @@ extern "C" int hmlfc_debug_pass_stats_tiles(unsigned long long *out, int reset)
 
 size_t render_tiles_scratch_bytes(int n_views, int W, int H)
 {
-    const size_t n_tiles = (size_t)n_views * (size_t)((W + kTile - 1) / kTile) * (size_t)((H + kTile - 1) / kTile);
+    const size_t n_tiles = (size_t)n_views * (size_t)((W + kTile - 1) / kTile) * (size_t)((H + kTile - 1) / kTile);  // enough for either width
     return n_tiles * sizeof(TileTables);
 }
 
 cudaError_t configure_render_tiles()
 {
     cudaError_t e = cudaSuccess;
-#define X(id, arena, minb) \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena);
+#define X(id, arena, minb, nt, tw) \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, false, nt, tw>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<arena, minb, true, nt, tw>, cudaFuncAttributeMaxDynamicSharedMemorySize, arena);
     HMLFC_TILES_CONFIGS(X)
 #undef X
     return e;
@@ -302,7 +321,8 @@ cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_
 {
     if (n_views == 0) return cudaSuccess;
     if (S.B != 4 || !d_scratch) return cudaErrorInvalidValue;
-    const int tiles_x = (W + kTile - 1) / kTile, tiles_y = (H + kTile - 1) / kTile;
+    const int tile_w = config >= 2 ? 64 : 32;
+    const int tiles_x = (W + tile_w - 1) / tile_w, tiles_y = (H + kTile - 1) / kTile;
     const long long n_tiles_ll = (long long)n_views * tiles_x * tiles_y;
     if (tiles_y > 65535 || tiles_x > 65535 || n_tiles_ll > 0x3fffffffLL) return cudaErrorInvalidValue;
     const int n_tiles = (int)n_tiles_ll;
@@ -310,15 +330,15 @@ cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_
     // 2: rows of tiles start at 16-byte boundaries (staged 16-byte stores), 1: 4-pixel groups at 4-byte boundaries, 0: byte stores
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 15u) == 0 && (W % 16) == 0) ? 2 :
                         ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0 && (W % 4) == 0) ? 1 : 0;
-    tile_tables_kernel<<<(unsigned)((n_tiles + kTablesWarps - 1) / kTablesWarps), kTablesWarps * 32, 0, st>>>(S, d_cams, W, H, tiles_x, tiles_y, n_tiles,
-                                                                                                          tables);
+    tile_tables_kernel<<<(unsigned)((n_tiles + kTablesWarps - 1) / kTablesWarps), kTablesWarps * 32, 0, st>>>(S, d_cams, W, H, tile_w, tiles_x, tiles_y,
+                                                                                                          n_tiles, tables);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)tiles_x, (unsigned)tiles_y, (unsigned)n_views);
-#define X(id, arena, minb) \
+#define X(id, arena, minb, nt, tw) \
     if (config == id) { \
-        if (S.pow2_mask == 15u) render_tiles_kernel<arena, minb, true><<<grid, 256, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
-        else render_tiles_kernel<arena, minb, false><<<grid, 256, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
+        if (S.pow2_mask == 15u) render_tiles_kernel<arena, minb, true, nt, tw><<<grid, nt, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
+        else render_tiles_kernel<arena, minb, false, nt, tw><<<grid, nt, arena, st>>>(S, d_cams, W, H, d_out, aligned, tables); \
     }
     HMLFC_TILES_CONFIGS(X)
 #undef X
