@@ -182,12 +182,16 @@ int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
  * bytes per sample.  Takes effect for launches enqueued afterwards; HMLFC_E_INVALID outside [0, height]. */
 int hmlfc_set_min_level(hmlfc_handle *h, int min_level);
 
-/* Kernel selection for hmlfc_decode (identical bytes): 0 = automatic (default: 2 or 3), 1 = one thread per
- * coordinate walks the tree on its own, 2 / 3 = warp-cooperative (each lane classifies its coordinate, the
- * motion-record and BISE value decodes run as 32-wide batches from per-warp task stacks): 2 reads the three
+/* Kernel selection for hmlfc_decode (identical bytes): 0 = automatic (default), 1 = one thread per
+ * coordinate walks the tree on its own, 2 / 3 / 4 = warp-cooperative (each lane classifies its coordinate, the
+ * motion-record and value decodes run as 32-wide batches from per-warp task stacks): 2 reads the three
  * channels' flag records and descriptors of every level up front, 3 reads ONE 32-byte sector of flag words per
- * level and lets the tasks of significant blocks fetch the rest.  The automatic choice takes 3 for streams whose
- * device form fits the L2 cache and where at most a quarter of the block flags are set, else 2. */
+ * level and lets the tasks of significant blocks fetch the rest; 4 reads the BLOCK RECORDS hmlfc_load builds for
+ * streams with full-resolution chroma (every stored value and motion record once more, as plain binary fields
+ * grouped per block: one sector per level says what a plane holds for a sample and where, one or two more hold
+ * all three channels of it; counted in device_bytes).  The automatic choice is 4 where the stream has block
+ * records (subsampled streams have none and run the per-sample kernel whatever the variant); otherwise 3 for streams whose device form fits the
+ * L2 cache and where at most a quarter of the block flags are set, else 2. */
 int hmlfc_set_decode_variant(hmlfc_handle *h, int variant);
 
 /* Encoder side (first "next" row): phase-shifted exhaustive block motion search, PAPER.md:227-248,

@@ -24,7 +24,7 @@ RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4, RENDER_TILES_W512,
 # every configuration of the two fused kernels for 4 x 4 blocks (all give the same bytes; hmlfc_set_render_variant forces one)
 RENDER_FUSED = (RENDER_CTA, RENDER_CTA_BIG, RENDER_CTA_SMALL, RENDER_CTA_1024, RENDER_CTA_512, RENDER_TILES, RENDER_TILES4,
                 RENDER_TILES_W512, RENDER_TILES_W256, RENDER_TILES_W256X3)
-DECODE_AUTO, DECODE_THREAD, DECODE_QUEUE, DECODE_QUEUE_LAZY = 0, 1, 2, 3
+DECODE_AUTO, DECODE_THREAD, DECODE_QUEUE, DECODE_QUEUE_LAZY, DECODE_QUEUE_BLOCKREC = 0, 1, 2, 3, 4
 
 
 class HmlfcError(RuntimeError):

@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJ = os.path.join(HERE, "build")
 SOURCES = ["hmlfc_api.cu", "hmlfc_kernels.cu", "hmlfc_decode_queue.cu", "hmlfc_search.cu", "hmlfc_hierarchy.cu", "hmlfc_encode.cu",
-           "hmlfc_render_warp.cu", "hmlfc_render_cta.cu", "hmlfc_render_tiles.cu", "hmlfc_decode_rows.cu"]
+           "hmlfc_render_warp.cu", "hmlfc_render_cta.cu", "hmlfc_render_tiles.cu", "hmlfc_decode_rows.cu", "hmlfc_repack.cu"]
 HEADERS = ["hmlfc_device.cuh", "hmlfc_kernels.cuh", "hmlfc_tables.h", "hmlfc_bise_row.cuh", "hmlfc_render_common.cuh"]
 LIB = os.path.join(HERE, "libhmlfc_b200.so")
 

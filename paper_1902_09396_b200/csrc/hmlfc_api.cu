@@ -21,6 +21,9 @@ struct hmlfc_handle {
     // device allocations
     uint4 *d_pc = nullptr;
     uint4 *d_flagrec = nullptr;
+    uint4 *d_bslot = nullptr;
+    uint4 *d_pb = nullptr;              // block records (hmlfc_device.cuh): per-plane descriptors and the records
+    uint32_t *d_brec = nullptr;
     uint32_t *d_pay = nullptr;
     uint32_t *d_mv = nullptr;
     short4 *d_rkv = nullptr;
@@ -98,7 +101,7 @@ int cuda_fail(const hmlfc_handle *h, cudaError_t e)
 void release(hmlfc_handle *h)
 {
     if (!h) return;
-    cudaFree(h->d_pc); cudaFree(h->d_flagrec); cudaFree(h->d_pay); cudaFree(h->d_mv); cudaFree(h->d_rkv);
+    cudaFree(h->d_pc); cudaFree(h->d_flagrec); cudaFree(h->d_pb); cudaFree(h->d_bslot); cudaFree(h->d_brec); cudaFree(h->d_pay); cudaFree(h->d_mv); cudaFree(h->d_rkv);
     cudaFree(h->d_bits15); cudaFree(h->d_oob); cudaFree(h->d_in); cudaFree(h->d_outbuf);
     if (h->host_stream) cudaStreamDestroy(h->host_stream);
     if (h->in_stream) cudaStreamDestroy(h->in_stream);
@@ -181,13 +184,34 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
         (ce = cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = create_events(h)) != cudaSuccess ||
         (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess ||
-        (ce = configure_render_tiles()) != cudaSuccess) {
+        (ce = configure_render_tiles()) != cudaSuccess || (ce = configure_decode_queue()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
     }
     DevStream &D = h->ds;
     D.pc = h->d_pc; D.flagrec = h->d_flagrec; D.pay = h->d_pay; D.mv = h->d_mv; D.rkv = h->d_rkv;
+    D.pb = nullptr; D.bslot = nullptr; D.brec = nullptr;
+    if (!T.pb.empty()) {
+        // block records: every stored value and motion record once more, regrouped per block (one kernel over the uploaded stream)
+        const size_t bytes = (size_t)T.brec_words * 4;
+        if ((ce = upload(&h->d_pb, T.pb.data(), T.pb.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
+            (ce = upload(&h->d_bslot, T.bslot.data(), T.bslot.size() * sizeof(uint4), 0, &dev_bytes)) != cudaSuccess ||
+            (ce = cudaMalloc(reinterpret_cast<void **>(&h->d_brec), bytes)) != cudaSuccess ||
+            (ce = cudaMemsetAsync(h->d_brec, 0, bytes, h->host_stream)) != cudaSuccess) {
+            const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
+            release(h);
+            return code;
+        }
+        D.pb = h->d_pb; D.bslot = h->d_bslot;
+        if ((ce = launch_repack(D, T.pb.size(), h->d_brec, h->host_stream)) != cudaSuccess ||
+            (ce = cudaStreamSynchronize(h->host_stream)) != cudaSuccess) {
+            release(h);
+            return HMLFC_E_CUDA;
+        }
+        D.brec = h->d_brec;
+        dev_bytes += bytes;
+    }
     h->info.device_bytes = dev_bytes;
     // hmlfc_decode's classification: one flag sector per level and everything else fetched by the tasks pays where the L2 holds the stream
     // (126 MB on B200; coordinates and output pass through it too) and few blocks carry data (measured: cfg2, 17% of the flags set,
@@ -212,7 +236,7 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
         CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl,
-                                  h->decode_variant == 2 ? 0 : h->decode_variant == 3 ? 1 : -1));
+                                  h->decode_variant == 2 ? 0 : h->decode_variant == 3 ? 1 : h->decode_variant == 4 ? 2 : -1));
     h->launches += nl;
     return HMLFC_OK;
 }
@@ -512,7 +536,7 @@ int hmlfc_set_min_level(hmlfc_handle *h, int min_level)
 
 int hmlfc_set_decode_variant(hmlfc_handle *h, int variant)
 {
-    if (!h || variant < 0 || variant > 3) return HMLFC_E_INVALID;
+    if (!h || variant < 0 || variant > 4) return HMLFC_E_INVALID;
     h->decode_variant = variant;
     return HMLFC_OK;
 }

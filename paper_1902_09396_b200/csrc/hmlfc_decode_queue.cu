@@ -17,6 +17,8 @@
 // 96-byte store.  Integer arithmetic only: bit-exact by construction against the per-thread kernel and the oracle.
 #include "hmlfc_kernels.cuh"
 
+#include <type_traits>
+
 namespace hmlfc {
 
 namespace {
@@ -47,13 +49,17 @@ constexpr DigitLut make_digit_lut()
 
 __device__ const DigitLut g_dq_digit_lut = make_digit_lut();
 
-struct WarpQ {
+// (shared memory is L1 taken away: this kernel's loads live on L1 hits of descriptors, slots and neighbouring fields, so the stacks stay small)
+template <int kLookups>
+struct WarpQT {
     uint4 vq[kCap];      // value tasks
     uint4 mq[kCap];      // motion tasks
+    uint4 rq[kLookups];  // reference lookups (block records only)
     int acc[32 * 4];     // {Y, Co, Cg, -} per coordinate of the warp
     uint32_t xy[32];     // s | t << 16 of the warp's coordinates
-    uint32_t stage[24];  // the warp's 96 output bytes
 };
+using WarpQ = WarpQT<1>;
+using WarpQB = WarpQT<kCap>;
 
 // BISE decode_at (bit layout in DESIGN.md section 4) of value i of the string that starts at word `base`
 // of `words`, without control flow: plain = groups of one value with an empty digit word, so lanes holding tasks of
@@ -111,7 +117,8 @@ __device__ __forceinline__ size_t resbits_word(const DevStream &S, uint32_t k, u
 }
 
 // execute the top n (<= 32) value tasks: rank of the block (S4) and BISE decode_at of its value (S5)
-__device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+template <typename Q>
+__device__ __forceinline__ void drain_values(const DevStream &S, Q &q, int &vcnt, int n, int lane, const uint16_t *lut)
 {
     __syncwarp();
     if (lane < n) {
@@ -129,7 +136,8 @@ __device__ __forceinline__ void drain_values(const DevStream &S, WarpQ &q, int &
 
 // execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
 // the reference block is significant, push its value task
-__device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
+template <typename Q>
+__device__ __forceinline__ void drain_motion(const DevStream &S, Q &q, int &mcnt, int &vcnt, int n, int lane,
                                              uint32_t lane_lt, const uint16_t *lut)
 {
     __syncwarp();
@@ -163,7 +171,8 @@ __device__ __forceinline__ void drain_motion(const DevStream &S, WarpQ &q, int &
 //   motion task  {MV word base, record index, reference plane-channel, destination}
 //   value task   {payload word base, value index, offset|layout|m|sign|destination}
 // execute the top n (<= 32) value tasks: S5 of the path
-__device__ __forceinline__ void drain_values_eager(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+template <typename Q>
+__device__ __forceinline__ void drain_values_eager(const DevStream &S, Q &q, int &vcnt, int n, int lane, const uint16_t *lut)
 {
     __syncwarp();
     if (lane < n) {
@@ -178,7 +187,8 @@ __device__ __forceinline__ void drain_values_eager(const DevStream &S, WarpQ &q,
 
 // execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
 // the reference block is significant, push its value task
-__device__ __forceinline__ void drain_motion_eager(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane,
+template <typename Q>
+__device__ __forceinline__ void drain_motion_eager(const DevStream &S, Q &q, int &mcnt, int &vcnt, int n, int lane,
                                              uint32_t lane_lt, const uint16_t *lut)
 {
     __syncwarp();
@@ -207,16 +217,123 @@ __device__ __forceinline__ void drain_motion_eager(const DevStream &S, WarpQ &q,
     push(q.vq, vcnt, has, vt, lane_lt);
 }
 
-template <bool kLazy>
-__device__ __forceinline__ void drain_v(const DevStream &S, WarpQ &q, int &vcnt, int n, int lane, const uint16_t *lut)
+// The same steps on the block records (hmlfc_device.cuh; kMode 2).  One task covers the three channels:
+//   value task   {word of the sample's first field, what (below), offset Y | offset Co << 16, offset Cg}
+//                what = bit | present << 5 | wanted << 8 | subtract << 11 | wY << 14 | wCo << 18 | wCg << 22 | destination lane << 26
+//                (present: the channels whose fields follow each other from that bit on; wanted: those to accumulate)
+//   motion task  {word of the block's first motion record, bit | pred mask << 5 | destination lane << 8, reference plane}
+//   lookup task  {reference plane, rx | ry << 16, channels | subtract << 3 | destination lane << 8}: channels whose motion records point at
+//                the same reference sample share the lookup and, where the reference block holds them, the value task
+__device__ __forceinline__ uint32_t value_what(uint32_t bit, uint32_t present, uint32_t wanted, uint32_t sub, uint4 pb, uint32_t lane)
 {
-    if (kLazy) drain_values(S, q, vcnt, n, lane, lut); else drain_values_eager(S, q, vcnt, n, lane, lut);
+    return bit | (present << 5) | (wanted << 8) | (sub << 11) | ((pb.y & 0xFu) << 14) | (((pb.y >> 8) & 0xFu) << 18) | (((pb.y >> 16) & 0xFu) << 22) | (lane << 26);
 }
 
-template <bool kLazy>
-__device__ __forceinline__ void drain_m(const DevStream &S, WarpQ &q, int &mcnt, int &vcnt, int n, int lane, uint32_t lane_lt, const uint16_t *lut)
+template <typename Q>
+__device__ __forceinline__ void drain_values_brec(const DevStream &S, Q &q, int &vcnt, int n, int lane)
 {
-    if (kLazy) drain_motion(S, q, mcnt, vcnt, n, lane, lane_lt, lut); else drain_motion_eager(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
+    __syncwarp();
+    if (lane < n) {
+        const uint4 t = q.vq[vcnt - n + lane];
+        const uint32_t sh = t.y & 31u, present = (t.y >> 5) & 7u, wanted = (t.y >> 8) & 7u, sub = (t.y >> 11) & 7u;
+        const uint32_t w[3] = {(t.y >> 14) & 15u, (t.y >> 18) & 15u, (t.y >> 22) & 15u};
+        const int off[3] = {(int)(int16_t)(t.z & 0xFFFFu), (int)(int16_t)(t.z >> 16), (int)(int16_t)(t.w & 0xFFFFu)};
+        const uint32_t span = ((present & 1u) ? w[0] : 0u) + ((present & 2u) ? w[1] : 0u) + ((present & 4u) ? w[2] : 0u);
+        const BrecWindow win = brec_window(S.brec, ((unsigned long long)t.x << 5) | sh, span);
+        int *acc = q.acc + (t.y >> 26) * 4;
+        uint32_t pos = sh;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if (!((present >> c) & 1u)) continue;
+            if ((wanted >> c) & 1u) {
+                const int val = off[c] + (int)brec_window_field(win, pos, w[c]);
+                atomicAdd(acc + c, ((sub >> c) & 1u) ? -val : val);
+            }
+            pos += w[c];
+        }
+    }
+    vcnt -= n;
+    __syncwarp();
+}
+
+// reference lookups: slot and descriptor of the reference plane -> value task for the channels its block holds
+template <typename Q>
+__device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int &rcnt, int &vcnt, int n, int lane, uint32_t lane_lt)
+{
+    __syncwarp();
+    bool has = false;
+    uint4 vt = make_uint4(0u, 0u, 0u, 0u);
+    if (lane < n) {
+        const uint4 t = q.rq[rcnt - n + lane];
+        const int rx = (int)(t.y & 0xFFFFu), ry = (int)(t.y >> 16);
+        const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+        uint4 sa, sb;
+        ldg256(S.bslot + ((size_t)t.x * (size_t)S.fgroups + (size_t)(b >> 5)) * 2u, sa, sb);
+        const uint4 pb = ldg(S.pb + t.x);
+        const BrecPos r = brec_locate(S, sa, sb, 1u << (b & 31), pb);
+        const uint32_t wanted = (t.z & 7u) & r.res;
+        has = wanted != 0u;
+        const uint32_t kin = (uint32_t)(((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1)));
+        const unsigned long long pos = r.bit + brec_sample_offset(r, pb, kin);
+        vt = make_uint4((uint32_t)(pos >> 5), value_what((uint32_t)pos & 31u, r.res, wanted, (t.z >> 3) & 7u, pb, (t.z >> 8) & 31u), pb.z, pb.w);
+    }
+    rcnt -= n;
+    __syncwarp();
+    push(q.vq, vcnt, has, vt, lane_lt);
+}
+
+// motion records of a block (S6), reference sample of every predicted channel (S7) -> lookup tasks
+template <typename Q>
+__device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int &mcnt, int &rcnt, int n, int lane, uint32_t lane_lt)
+{
+    __syncwarp();
+    uint32_t rem = 0u, sub = 0u;
+    int px[3] = {0, 0, 0}, py[3] = {0, 0, 0};
+    uint4 t = make_uint4(0u, 0u, 0u, 0u);
+    if (lane < n) {
+        t = q.mq[mcnt - n + lane];
+        const uint32_t sh = t.y & 31u, pred = (t.y >> 5) & 7u, todo = t.w & 7u;  // todo: the channels this pass still has to look up
+        const BrecWindow win = brec_window(S.brec, ((unsigned long long)t.x << 5) | sh, popc(pred) * S.mv_w);
+        const uint32_t xy = q.xy[(t.y >> 8) & 31u];
+        uint32_t pos = sh;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            if (!((pred >> c) & 1u)) continue;
+            int mode, dx, dy;
+            mv_unpack(S, brec_window_field(win, pos, S.mv_w), mode, dx, dy);
+            pos += S.mv_w;
+            px[c] = (int)(xy & 0xFFFFu) + dx; py[c] = (int)(xy >> 16) + dy;
+            if (mode) sub |= 1u << c;
+            if (((todo >> c) & 1u) && (unsigned)px[c] < (unsigned)S.Ws && (unsigned)py[c] < (unsigned)S.Ht) rem |= 1u << c;  // R8: outside the image reads 0
+        }
+    }
+    mcnt -= n;
+    __syncwarp();
+    // one lookup for the first channel and every channel whose motion record points at the same reference sample (usually all: the
+    // channels of a block move together); the others come back as a motion task of their own
+    const int c0 = (rem & 1u) ? 0 : (rem & 2u) ? 1 : 2;
+    const int x0 = c0 == 0 ? px[0] : c0 == 1 ? px[1] : px[2], y0 = c0 == 0 ? py[0] : c0 == 1 ? py[1] : py[2];
+    uint32_t grp = 0u;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        if (((rem >> c) & 1u) && px[c] == x0 && py[c] == y0) grp |= 1u << c;
+    push(q.rq, rcnt, rem != 0u, make_uint4(t.z, (uint32_t)x0 | ((uint32_t)y0 << 16), grp | (sub << 3) | (((t.y >> 8) & 31u) << 8), 0u), lane_lt);
+    rem &= ~grp;
+    push(q.mq, mcnt, rem != 0u, make_uint4(t.x, t.y, t.z, rem), lane_lt);
+}
+
+template <int kMode, typename Q>
+__device__ __forceinline__ void drain_v(const DevStream &S, Q &q, int &vcnt, int n, int lane, const uint16_t *lut)
+{
+    if (kMode == 1) drain_values(S, q, vcnt, n, lane, lut);
+    else drain_values_eager(S, q, vcnt, n, lane, lut);
+}
+
+template <int kMode, typename Q>
+__device__ __forceinline__ void drain_m(const DevStream &S, Q &q, int &mcnt, int &vcnt, int n, int lane, uint32_t lane_lt, const uint16_t *lut)
+{
+    if (kMode == 1) drain_motion(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
+    else drain_motion_eager(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
 }
 
 // kDense: the coordinates are not read but generated -- sample i is pixel i mod (Ws Ht) (row-major) of view views[i / (Ws Ht)]
@@ -224,19 +341,21 @@ __device__ __forceinline__ void drain_m(const DevStream &S, WarpQ &q, int &mcnt,
 // kLazy: the classification reads one flag sector per level and the tasks fetch descriptor and rank themselves (fewest sectors per sample: for
 // streams the L2 holds, where the sector rate binds); otherwise it reads the three channels' flag records and descriptors up front and the
 // tasks carry them (one dependent load less per task: for streams in HBM, where every access is a DRAM access either way and latency binds).
-template <int kDense, bool kLazy>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
+template <int kDense, int kMode>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
 __global__ void __launch_bounds__(kThreads)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
 {
-    __shared__ WarpQ wq[kWarps];
+    __shared__ typename std::conditional<kMode >= 2, WarpQB, WarpQ>::type wq[kWarps];
     __shared__ uint16_t lut[384];
-    for (int k = threadIdx.x; k < 384; k += kThreads) lut[k] = g_dq_digit_lut.v[k];
-    __syncthreads();
+    if (kMode < 2) {  // (the block records are plain binary)
+        for (int k = threadIdx.x; k < 384; k += kThreads) lut[k] = g_dq_digit_lut.v[k];
+        __syncthreads();
+    }
 
     const int lane = threadIdx.x & 31;
     const uint32_t lane_lt = (1u << lane) - 1u;
-    WarpQ &q = wq[threadIdx.x >> 5];
+    auto &q = wq[threadIdx.x >> 5];
     const long long i = (long long)blockIdx.x * kThreads + threadIdx.x;
     const bool present = i < n;
     int4 c4 = make_int4(0, 0, 0, 0);
@@ -286,6 +405,113 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const uint32_t kin = (uint32_t)(((y & (S.B - 1)) << S.logB) + (x & (S.B - 1)));
     int vcnt = 0, mcnt = 0;
 
+    constexpr bool kLazy = kMode == 1;
+    if (kMode >= 2) {
+        // S4 on the block records: per level ONE sector (the slot of the block's group in the level's plane) says what the plane holds for
+        // the sample and where; the plane's descriptor (16 bytes, a few hundred KB in all) gives widths and offsets
+        // Every batch of 32 tasks is executed by ONE copy of its code (the kernel is instruction-cache bound otherwise): the level loop runs
+        // one extra round that only flushes.  Order: values while 32 wait, then lookups (they push <= 32 values), then motion tasks
+        // (<= 32 lookups); the flush drains producers first.
+        int rcnt = 0;
+#pragma unroll 1
+        for (int L = S.lmin; L <= h; ++L) {
+            const bool flush = L == h;
+            if (!flush) {
+                const int pu = u >> L, pv = v >> L;
+                const LevelDesc lv = S.lev[L];
+                const uint32_t plane0 = umulhi(lv.pc_base, 0xAAAAAAABu) >> 1;  // pc_base / 3
+                const uint32_t plane = plane0 + (uint32_t)(pv * lv.UL + pu), rplane = plane0 + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1));
+                const bool predictive = ((pu | pv) & 1) != 0;
+                uint4 sa = make_uint4(0u, 0u, 0u, 0u), sb = sa, pb = sa;
+                if (valid) {
+                    ldg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
+                    pb = ldg(S.pb + plane);
+                }
+                const BrecPos r = brec_locate(S, sa, sb, bit, pb);
+                const unsigned long long vpos = r.bit + brec_sample_offset(r, pb, kin);
+                push(q.vq, vcnt, r.res != 0u,
+                     make_uint4((uint32_t)(vpos >> 5), value_what((uint32_t)vpos & 31u, r.res, r.res, 0u, pb, (uint32_t)lane), pb.z, pb.w), lane_lt);
+                push(q.mq, mcnt, predictive && r.pred != 0u,
+                     make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | ((uint32_t)lane << 8), rplane, r.pred), lane_lt);
+            }
+            if (!flush) {  // (in the level loop the usual order, inline: 4% faster than going through the loop below)
+                if (vcnt >= 32) drain_values_brec(S, q, vcnt, 32, lane);
+                while (mcnt >= 32) {
+                    drain_motion_brec(S, q, mcnt, rcnt, 32, lane, lane_lt);
+                    if (rcnt >= 32) {
+                        drain_lookups_brec(S, q, rcnt, vcnt, 32, lane, lane_lt);
+                        if (vcnt >= 32) drain_values_brec(S, q, vcnt, 32, lane);
+                    }
+                }
+                continue;
+            }
+#pragma unroll 1
+            while (true) {
+                const int which = vcnt >= 32 ? 0 : rcnt >= 32 ? 1 : (mcnt >= 32 || (flush && mcnt > 0)) ? 2 : (flush && rcnt > 0) ? 1 : (flush && vcnt > 0) ? 0 : -1;
+                if (which < 0) break;
+                if (which == 0) drain_values_brec(S, q, vcnt, min(vcnt, 32), lane);
+                else if (which == 1) drain_lookups_brec(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
+                else drain_motion_brec(S, q, mcnt, rcnt, min(mcnt, 32), lane, lane_lt);
+            }
+        }
+    } else if (kLazy) {
+        // S4, first look, for (up to) four levels at a time: the six flag words of the block's group in each level's plane, one 32-byte
+        // sector per level (the second half of the plane's 64-byte slot: the Cg record {res, rank, pred, rank} and {res Y, res Co, pred Y,
+        // pred Co}).  The addresses depend on the coordinate alone, so the levels' loads are in flight together: one memory round trip
+        // where a level-by-level walk takes h.  What a level contributes is then packed into two words (flags, in-group ranks).
+#pragma unroll 1
+        for (int L0 = S.lmin; L0 < h; L0 += 4) {
+            uint32_t fl[4], pr[4];
+            {
+                uint4 a[4], bw[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    a[j] = bw[j] = make_uint4(0u, 0u, 0u, 0u);
+                    const int L = L0 + j;
+                    if (valid && L < h) {
+                        const LevelDesc lv = S.lev[L];
+                        ldg256(S.flagrec + flag_index(S, lv.pc_base + (uint32_t)((v >> L) * lv.UL + (u >> L)) * 3u, fg) + 2, a[j], bw[j]);
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t resw[3] = {bw[j].x, bw[j].y, a[j].x}, prdw[3] = {bw[j].z, bw[j].w, a[j].z};
+                    fl[j] = pr[j] = 0u;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        fl[j] |= ((resw[c] & bit) ? 1u << c : 0u) | ((prdw[c] & bit) ? 8u << c : 0u) | ((uint32_t)__popc(resw[c] & (bit - 1u)) << (8 + 5 * c));
+                        pr[j] |= (uint32_t)__popc(prdw[c] & (bit - 1u)) << (5 * c);
+                    }
+                }
+            }
+#pragma unroll 1  // (the drains are large: one copy of them)
+            for (int j = 0; j < 4; ++j) {
+                const int L = L0 + j;
+                if (L < h) {  // warp-uniform
+                const uint32_t flj = j == 0 ? fl[0] : j == 1 ? fl[1] : j == 2 ? fl[2] : fl[3];
+                const uint32_t prj = j == 0 ? pr[0] : j == 1 ? pr[1] : j == 2 ? pr[2] : pr[3];
+                const int pu = u >> L, pv = v >> L;
+                const LevelDesc lv = S.lev[L];
+                const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
+                const uint32_t rbase = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
+                const bool predictive = ((pu | pv) & 1) != 0;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const uint32_t dest = (uint32_t)(lane * 4 + c);
+                    const bool res = (flj >> c) & 1u;
+                    push(q.vq, vcnt, res, make_uint4(base + (uint32_t)c, fg, kin | (((flj >> (8 + 5 * c)) & 31u) << 8) | (dest << 24), 0u), lane_lt);
+                    if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
+                    const bool pred = predictive && ((flj >> (3 + c)) & 1u);
+                    push(q.mq, mcnt, pred, make_uint4(base + (uint32_t)c, fg, rbase + (uint32_t)c, dest | (((prj >> (5 * c)) & 31u) << 8)), lane_lt);
+                    if (mcnt >= 32) {
+                        drain_m<kMode>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                        if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
+                    }
+                }
+                }
+            }
+        }
+    } else {
 #pragma unroll 1
     for (int L = S.lmin; L < h; ++L) {
         const int pu = u >> L, pv = v >> L;
@@ -293,27 +519,6 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
         const uint32_t base = lv.pc_base + (uint32_t)(pv * lv.UL + pu) * 3u;
         const uint32_t rbase = lv.pc_base + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1)) * 3u;
         const bool predictive = ((pu | pv) & 1) != 0;
-        if (kLazy) {
-        // S4, first look: the six flag words of the block's group, one 32-byte sector (the second half of the plane's 64-byte slot):
-        // a = the Cg record {res, rank, pred, rank}, bw = {res Y, res Co, pred Y, pred Co}
-        uint4 a = make_uint4(0u, 0u, 0u, 0u), bw = a;
-        if (valid) ldg256(S.flagrec + flag_index(S, base, fg) + 2, a, bw);
-        const uint32_t resw[3] = {bw.x, bw.y, a.x}, prdw[3] = {bw.z, bw.w, a.z};
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const uint32_t dest = (uint32_t)(lane * 4 + c);
-            const bool res = (resw[c] & bit) != 0u;
-            push(q.vq, vcnt, res, make_uint4(base + (uint32_t)c, fg, kin | ((uint32_t)__popc(resw[c] & (bit - 1u)) << 8) | (dest << 24), 0u), lane_lt);
-            if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
-            const bool pred = predictive && (prdw[c] & bit) != 0u;
-            push(q.mq, mcnt, pred, make_uint4(base + (uint32_t)c, fg, rbase + (uint32_t)c, dest | ((uint32_t)__popc(prdw[c] & (bit - 1u)) << 8)), lane_lt);
-            if (mcnt >= 32) {
-                drain_m<kLazy>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
-                if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
-            }
-        }
-    
-        } else {
         // S4: the three channels' descriptors and flag records, six independent loads
         uint4 d[3], fr[3];
         // S4: the three channels' descriptors and their flag records; the records share one 64-byte slot: a 256-bit
@@ -333,21 +538,21 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
             const bool res = (fr[c].x & bit) != 0u;
             const uint32_t rank = fr[c].y + (uint32_t)__popc(fr[c].x & (bit - 1u));
             push(q.vq, vcnt, res, make_uint4(d[c].y, (rank << (2 * S.logB)) + kin, (d[c].w & 0x3FFFFFu) | (dest << 24), 0u), lane_lt);
-            if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
+            if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
             const bool pred = predictive && (fr[c].z & bit) != 0u;
             const uint32_t mi = fr[c].w + (uint32_t)__popc(fr[c].z & (bit - 1u));
             push(q.mq, mcnt, pred, make_uint4(d[c].z, mi, rbase + (uint32_t)c, dest), lane_lt);
             if (mcnt >= 32) {
-                drain_m<kLazy>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
-                if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
+                drain_m<kMode>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
             }
         }
     
-        }
     }
-    if (mcnt > 0) drain_m<kLazy>(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
-    if (vcnt >= 32) drain_v<kLazy>(S, q, vcnt, 32, lane, lut);
-    if (vcnt > 0) drain_v<kLazy>(S, q, vcnt, vcnt, lane, lut);
+    }
+    if (mcnt > 0) drain_m<kMode>(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
+    if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
+    if (vcnt > 0) drain_v<kMode>(S, q, vcnt, vcnt, lane, lut);
     __syncwarp();
 
     // S8: inverse YCoCg-R + clamp, then the warp's 96 bytes as 24 coalesced words
@@ -359,15 +564,16 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const long long wbase = i - lane;
     uint8_t *o = out + 3 * wbase;
     if (out_aligned && wbase + 32 <= n) {
-        uint8_t *sb = reinterpret_cast<uint8_t *>(q.stage);
+        uint32_t *stage = reinterpret_cast<uint32_t *>(q.vq);  // the warp's 96 output bytes (its stacks are empty)
+        uint8_t *sb = reinterpret_cast<uint8_t *>(stage);
         sb[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
         sb[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
         sb[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
         __syncwarp();
 #ifdef HMLFC_DECODE_CS
-        if (lane < 24) __stcs(reinterpret_cast<uint32_t *>(o) + lane, q.stage[lane]);
+        if (lane < 24) __stcs(reinterpret_cast<uint32_t *>(o) + lane, stage[lane]);
 #else
-        if (lane < 24) reinterpret_cast<uint32_t *>(o)[lane] = q.stage[lane];
+        if (lane < 24) reinterpret_cast<uint32_t *>(o)[lane] = stage[lane];
 #endif
     } else if (present) {
         o[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
@@ -378,18 +584,34 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
 
 }  // namespace
 
+// The block-record kernel lives on L1 hits (plane descriptors, neighbouring fields) as much as on occupancy: 6 CTAs per SM leave 60 KB of
+// L1, 5 leave 92 KB.  Measured (G px/s, 6 / 5 CTAs): cfg2 (stream in the L2) 14.8 / 14.4, cfg4 (in HBM) 6.0 / 7.3 -- instantiation 3 is the
+// kernel with a shared-memory carve-out that fits 5 CTAs, used for streams the L2 does not hold.
+cudaError_t configure_decode_queue()
+{
+    return cudaFuncSetAttribute(decode_queue_kernel<0, 3>, cudaFuncAttributePreferredSharedMemoryCarveout, 65);
+}
+
 cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
-                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int lazy)
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int mode)
 {
     if (n == 0) return cudaSuccess;
     if (S.Ws > 65536 || S.Ht > 65536) return cudaErrorInvalidValue;  // s | t << 16 packing
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    if (lazy < 0 ? S.l2_resident != 0u : lazy != 0)
-        decode_queue_kernel<0, true><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out, d_oob, aligned);
+    // mode: 0 eager, 1 lazy, 2 block records (needs S.brec); < 0: chosen here
+    if (mode < 0) mode = S.brec ? 2 : (S.l2_resident ? 1 : 0);
+    if (mode == 2 && !S.brec) return cudaErrorInvalidValue;
+    const int4 *c4 = reinterpret_cast<const int4 *>(d_coords);
+    if (mode == 1)
+        decode_queue_kernel<0, 1><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
+    else if (mode == 2 && S.l2_resident)
+        decode_queue_kernel<0, 2><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
+    else if (mode == 2)  // the same kernel with a larger L1 (configure_decode_queue)
+        decode_queue_kernel<0, 3><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     else
-        decode_queue_kernel<0, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_coords), (long long)n, d_out, d_oob, aligned);
+        decode_queue_kernel<0, 0><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -403,7 +625,7 @@ cudaError_t launch_decode_blocks(const DevStream &S, const int32_t *d_blocks, in
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<2, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_blocks), n, d_out, d_oob, aligned);
+    decode_queue_kernel<2, 0><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_blocks), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -417,7 +639,7 @@ cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int6
     const long long blocks = (n + kThreads - 1) / kThreads;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_queue_kernel<1, false><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
+    decode_queue_kernel<1, 0><<<(unsigned)blocks, kThreads, 0, st>>>(S, reinterpret_cast<const int4 *>(d_views), n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

@@ -52,6 +52,12 @@ struct DevStream {
     const uint32_t *pay;
     const uint32_t *mv;
     const short4 *rkv;
+    // block records (full-resolution chroma only; null otherwise): the stored values and motion records of a plane once more, regrouped
+    // per BLOCK so that what one sample needs from a plane lies in one or two sectors -- see brec_locate below
+    const uint4 *pb;       // per plane {first word of the plane in brec[], wY | wCo << 8 | wCg << 16 | wMV << 24, offY | offCo << 16, offCg}
+    const uint4 *bslot;    // two per (plane, 32-block group): the group's slot
+    const uint32_t *brec;
+    uint32_t mv_w;         // bits of a motion record as a plain binary field
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st;
     float uv_inv[2], st_inv[2];  // 1 / step where that is exact (step a power of two), see pow2_mask
     uint32_t pow2_mask;          // bit 0..3: uv_step[0], uv_step[1], st_step[0], st_step[1] is a power of two
@@ -155,6 +161,71 @@ HMLFC_DEV int reference_value(const DevStream &S, uint4 d, int rx, int ry, int W
     uint4 fr = ldg(S.flagrec + d.x + 4u * (uint32_t)(b >> 5));
     int kin = ((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1));
     return stored_value(S, d, fr, 1u << (b & 31), kin);
+}
+
+// ---------------------------------------------------------------- block records (device form, hmlfc_load)
+// The serialized stream keeps one BISE string per plane-channel, so the (up to) three stored values and three motion records one
+// sample needs from a plane lie in six unrelated places, behind three flag records and three descriptors.  hmlfc_load re-packs them
+// per plane as plain binary fields, block after block in raster order, every block that carries anything as ONE record:
+//     [motion record of Y, Co, Cg where the pred flag is set : wMV bits each]
+//     [sample 0: value of Y, Co, Cg where the res flag is set : wY, wCo, wCg bits][sample 1: ...] ... [sample B^2 - 1]
+// (value = code, without the channel's offset; w = bits of the channel's alphabet), and keeps one 32-byte SLOT per 32 blocks of a plane:
+//     bslot = {res bits Y, Co, Cg, pred bits Y, Co, Cg, first bit of the group's first record (from the plane's start), 0}
+// The record of block b starts where the group starts plus the sizes of the group's records before b: popcounts of the six words.
+// One sector says whether a plane holds anything for a sample and where; one or two more hold all of it.
+struct BrecPos {
+    unsigned long long bit;  // first bit of the block's record in brec[]
+    uint32_t res, pred;      // 3-bit masks of the block's set flags
+    uint32_t stride;         // bits per sample
+};
+
+// a, b = the two halves of the slot of the block's group, bit = 1 << (block & 31), pb = the plane's record descriptor
+HMLFC_DEV BrecPos brec_locate(const DevStream &S, uint4 a, uint4 b, uint32_t bit, uint4 pb)
+{
+    const uint32_t below = bit - 1u;
+    const uint32_t wY = pb.y & 0xFFu, wCo = (pb.y >> 8) & 0xFFu, wCg = (pb.y >> 16) & 0xFFu, wMV = pb.y >> 24;
+    BrecPos r;
+    r.res = ((a.x & bit) ? 1u : 0u) | ((a.y & bit) ? 2u : 0u) | ((a.z & bit) ? 4u : 0u);
+    r.pred = ((a.w & bit) ? 1u : 0u) | ((b.x & bit) ? 2u : 0u) | ((b.y & bit) ? 4u : 0u);
+    r.stride = ((r.res & 1u) ? wY : 0u) + ((r.res & 2u) ? wCo : 0u) + ((r.res & 4u) ? wCg : 0u);
+    const uint32_t before = ((popc(a.x & below) * wY + popc(a.y & below) * wCo + popc(a.z & below) * wCg) << (2 * S.logB)) +
+                            (popc(a.w & below) + popc(b.x & below) + popc(b.y & below)) * wMV;
+    r.bit = (unsigned long long)pb.x * 32ull + (unsigned long long)b.z + (unsigned long long)before;
+    return r;
+}
+
+// bit offset (from the record's start) of the motion record of channel c / of sample kin's first value / of channel c within a sample
+HMLFC_DEV uint32_t brec_mv_offset(const BrecPos &r, uint4 pb, int c) { return popc(r.pred & ((1u << c) - 1u)) * (pb.y >> 24); }
+HMLFC_DEV uint32_t brec_sample_offset(const BrecPos &r, uint4 pb, uint32_t kin) { return popc(r.pred) * (pb.y >> 24) + kin * r.stride; }
+HMLFC_DEV uint32_t brec_channel_offset(const BrecPos &r, uint4 pb, int c)
+{
+    uint32_t before = 0u;
+    if (c > 0 && (r.res & 1u)) before += pb.y & 0xFFu;
+    if (c > 1 && (r.res & 2u)) before += (pb.y >> 8) & 0xFFu;
+    return before;
+}
+HMLFC_DEV int brec_offset_of(uint4 pb, int c) { return (int)(int16_t)(c == 0 ? pb.z & 0xFFFFu : c == 1 ? pb.z >> 16 : pb.w & 0xFFFFu); }
+
+// 96-bit window of brec[] from the word that holds bit `bit`: an aligned 64-bit load, the next pair only when `span` bits from `bit`
+// leave the first (at most 96 - 31 = 65 bits are needed by any caller)
+struct BrecWindow { uint32_t w0, w1, w2; };
+HMLFC_DEV BrecWindow brec_window(const uint32_t *__restrict__ brec, unsigned long long bit, uint32_t span)
+{
+    const unsigned long long wi = bit >> 5;
+    const uint32_t odd = (uint32_t)wi & 1u, sh = (uint32_t)bit & 31u;
+    const uint2 *p2 = reinterpret_cast<const uint2 *>(brec + (wi & ~1ull));
+    const uint2 A = __ldg(p2);
+    uint2 B = make_uint2(0u, 0u);
+    if (odd * 32u + sh + span > 64u) B = __ldg(p2 + 1);
+    BrecWindow r;
+    r.w0 = odd ? A.y : A.x; r.w1 = odd ? B.x : A.y; r.w2 = odd ? B.y : B.x;
+    return r;
+}
+// the w-bit field (w <= 16) at bit `pos` (< 80) of the window
+HMLFC_DEV uint32_t brec_window_field(const BrecWindow &q, uint32_t pos, uint32_t w)
+{
+    const uint32_t lo = pos < 32u ? q.w0 : (pos < 64u ? q.w1 : q.w2), hi = pos < 32u ? q.w1 : (pos < 64u ? q.w2 : 0u);
+    return funnel_r(lo, hi, pos & 31u) & ((1u << w) - 1u);
 }
 
 // motion record r = mode*nd^2 + (dy+W)*nd + (dx+W)  (R16)

@@ -23,9 +23,11 @@ struct FootprintTotals {
 cudaError_t launch_decode(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
                           unsigned long long *d_oob, cudaStream_t st, int *n_launches);
 // warp-cooperative decode (hmlfc_decode_queue.cu): same result as launch_decode
-// lazy: 1 = one flag sector per level, tasks fetch descriptor and rank; 0 = flag records and descriptors up front; -1 = by S.l2_resident
+// mode: 0 = flag records and descriptors up front (eager); 1 = one flag sector per level, tasks fetch descriptor and rank (lazy); 2 = the
+// block records (S.brec); -1 = block records where the stream has them, else lazy / eager by S.l2_resident
 cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
-                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int lazy = -1);
+                                unsigned long long *d_oob, cudaStream_t st, int *n_launches, int mode = -1);
+cudaError_t configure_decode_queue();
 // whole views: d_views = int32 [n_views][2] = (u, v); d_out = uint8 [n_views][Ht][Ws][3]; coordinates are generated in the kernel
 cudaError_t launch_decode_views(const DevStream &S, const int32_t *d_views, int64_t n_views, uint8_t *d_out, unsigned long long *d_oob,
                                 cudaStream_t st, int *n_launches);
@@ -57,6 +59,9 @@ cudaError_t launch_render_cta(const DevStream &S, const Camera *d_cams, int n_vi
 // memory for the tables (contents irrelevant before, undefined after).  config: 0 / 1 = 32 x 32 tiles, 3 / 4 CTAs per SM; 2 = 64 x 32 tiles, 512 threads;
 // 3 / 4 = 64 x 32 tiles, 256 threads (8 pixels per thread), 2 / 3 CTAs per SM.
 size_t render_tiles_scratch_bytes(int n_views, int W, int H);
+
+// hmlfc_load: block records of the uploaded stream S (S.pb set) -> d_brec (zeroed), hmlfc_repack.cu
+cudaError_t launch_repack(const DevStream &S, uint64_t n_planes, uint32_t *d_brec, cudaStream_t st);
 cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, void *d_scratch,
                                 cudaStream_t st, int *n_launches, int config);
 cudaError_t configure_render_tiles();

@@ -16,6 +16,9 @@ struct HostTables {
     DevStream ds{};  // device pointers left null; hmlfc_load fills them after the upload
     hmlfc_info_t info{};
     std::vector<uint4> pc, flagrec;
+    std::vector<uint4> bslot;  // block records: 32-byte slot per (plane, 32-block group)
+    std::vector<uint4> pb;     // per plane: block-record descriptor (hmlfc_device.cuh, "block records"); empty for subsampled streams
+    uint64_t brec_words = 0;   // 32-bit words of the block-record array (with its read slack)
     uint64_t n_flagged = 0;  // set res and pred flags of the whole stream
     std::vector<uint32_t> bits15;  // per plane-channel BISE bits/value in 1/15 bit (footprint only)
     std::vector<short4> rkv;
@@ -109,6 +112,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     D.nd = 2u * I.window + 1u; D.nd2 = D.nd * D.nd;
     D.nd_magic = D.nd == 1 ? 0xFFFFFFFFu : (uint32_t)((0x100000000ull + D.nd - 1) / D.nd);
     bise_layout(2u * D.nd2, &D.mv_layout, &D.mv_m);
+    D.mv_w = D.mv_m + (D.mv_layout == 0 ? 0u : D.mv_layout == 1 ? 2u : 3u);
     T.mv_bits15 = bise_bits15(D.mv_layout, D.mv_m);
     for (int i = 0; i < 2; ++i) {
         D.uv_origin[i] = I.uv_origin[i]; D.uv_step[i] = I.uv_step[i];
@@ -152,6 +156,10 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
         T.bits15.resize(n_pc);
         T.flagrec.assign((n_pc / 3) * (uint64_t)D.fgroups * 4, make_uint4(0u, 0u, 0u, 0u));  // 64-byte slot per (plane, group): Y, Co, Cg, bit words of Y and Co
         T.rkv.resize(n_top * npx);
+        if (!D.cs) {
+            T.pb.assign(n_pc / 3, make_uint4(0u, 0u, 0u, 0u));
+            T.bslot.assign((n_pc / 3) * (uint64_t)D.fgroups * 2, make_uint4(0u, 0u, 0u, 0u));
+        }
     } catch (const std::bad_alloc &) {
         return HMLFC_E_NOMEM;
     }
@@ -206,7 +214,44 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     }
                     if (rr != n_res || rp != n_pred) return HMLFC_E_CORRUPT;
                     T.n_flagged += (uint64_t)rr + (uint64_t)rp;
+                    if (!D.cs) {
+                        // block records (hmlfc_device.cuh): field widths and offsets of the plane's channels; .x counts the plane's bits
+                        // until the prefix sum below turns it into the plane's first word
+                        uint4 &pb = T.pb[k / 3];
+                        const uint32_t w = m + (layout == 0 ? 0u : layout == 1 ? 2u : 3u);  // values < 2^m, 3 2^m, 5 2^m
+                        pb.y |= w << (8 * c);
+                        if (c == 0) pb.y |= D.mv_w << 24;
+                        if (c < 2) pb.z |= ((uint32_t)offset & 0xFFFFu) << (16 * c); else pb.w = (uint32_t)offset & 0xFFFFu;
+                        const uint64_t bits = (uint64_t)pb.x + (uint64_t)n_res * BB * w + (uint64_t)n_pred * D.mv_w;
+                        if (bits > 0xFFFFFF00ull) return HMLFC_E_UNSUPPORTED;
+                        pb.x = (uint32_t)bits;
+                    }
                 }
+    if (!D.cs) {
+        // slots: the six bit words of every group and the position of the group's first record in its plane
+        for (uint64_t p = 0; p < n_pc / 3; ++p) {
+            const uint4 pb = T.pb[p];
+            const uint32_t w[3] = {pb.y & 0xFFu, (pb.y >> 8) & 0xFFu, (pb.y >> 16) & 0xFFu};
+            uint64_t base = 0;
+            for (int g = 0; g < D.fgroups; ++g) {
+                const uint4 *fr = &T.flagrec[(p * (uint64_t)D.fgroups + (uint64_t)g) * 4];
+                T.bslot[(p * (uint64_t)D.fgroups + (uint64_t)g) * 2] = make_uint4(fr[0].x, fr[1].x, fr[2].x, fr[0].z);
+                T.bslot[(p * (uint64_t)D.fgroups + (uint64_t)g) * 2 + 1] = make_uint4(fr[1].z, fr[2].z, (uint32_t)base, 0u);
+                for (int c = 0; c < 3; ++c)
+                    base += (uint64_t)popcount32(fr[c].x) * BB * w[c] + (uint64_t)popcount32(fr[c].z) * D.mv_w;
+            }
+            if (base != (uint64_t)pb.x) return HMLFC_E_CORRUPT;  // (cannot happen: both count the same flags)
+        }
+        uint64_t word = 0;
+        for (uint4 &pb : T.pb) {  // planes start at 32-byte boundaries
+            const uint64_t words = ((uint64_t)pb.x + 31) / 32;
+            if (word > 0xFFFFFF00ull) return HMLFC_E_UNSUPPORTED;
+            pb.x = (uint32_t)word;
+            word += (words + 7) & ~7ull;
+        }
+        T.brec_words = word + 8;  // fields are read as aligned 64-bit pairs plus one word
+        if (T.brec_words > 0xFFFFFF00ull) return HMLFC_E_UNSUPPORTED;
+    }
 
     // top-level RKVs: Y uint8 planes, then Co and Cg int16 LE planes -> short4 {Y, Co, Cg, 0} per full-resolution sample (subsampled
     // chroma is replicated here, once: nearest neighbour, R18)

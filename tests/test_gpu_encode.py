@@ -258,20 +258,20 @@ def test_randomised_shapes_and_parameters(P):
         full = s.decode_full()
         hd = P.hmlfc_load(got)
         views = np.array([[u, v] for v in range(V) for u in range(U)], dtype=np.int32)
-        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
             P.hmlfc_set_decode_variant(hd, variant)
             dec = P.hmlfc_decode_views(hd, torch.from_numpy(views).cuda()).cpu().numpy().reshape(V, U, Ht, Ws, 3)
             assert np.array_equal(dec, full), tag
         coords = np.stack([a.ravel() for a in np.meshgrid(np.arange(U), np.arange(V), np.arange(Ws), np.arange(Ht), indexing="ij")], 1).astype(np.int32)
         coords = coords[rng.permutation(len(coords))]
         expect = full[coords[:, 1], coords[:, 0], coords[:, 3], coords[:, 2]]
-        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
             P.hmlfc_set_decode_variant(hd, variant)
             assert np.array_equal(P.hmlfc_decode(hd, torch.from_numpy(coords).cuda()).cpu().numpy(), expect), tag
         blocks = np.stack([a.ravel() for a in np.meshgrid(np.arange(U), np.arange(V), np.arange(Ws // B), np.arange(Ht // B), indexing="ij")], 1).astype(np.int32)
         blocks = blocks[rng.permutation(len(blocks))]
         bexp = np.stack([full[b[1], b[0], b[3] * B:(b[3] + 1) * B, b[2] * B:(b[2] + 1) * B] for b in blocks])
-        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
             P.hmlfc_set_decode_variant(hd, variant)
             assert np.array_equal(P.hmlfc_decode_blocks(hd, torch.from_numpy(blocks).cuda()).cpu().numpy(), bexp), tag
         P.hmlfc_set_decode_variant(hd, P.DECODE_AUTO)

@@ -56,7 +56,7 @@ def test_decode_every_pixel_matches_oracle(P, enc, name):
     h = _loaded(P, enc, name)
     coords = wl.all_coords(cfg)
     rc = wl.random_coords(cfg, 100_003)                           # ragged: not a multiple of the block size
-    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_AUTO):
+    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC, P.DECODE_AUTO):
         P.hmlfc_set_decode_variant(h, variant)
         out = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
         assert np.array_equal(out.reshape(lf.shape), info["p1"])  # = the encoder's own reconstruction
@@ -69,7 +69,7 @@ def test_decode_ragged_sizes_and_unaligned_output(P, enc, n):
     h = _loaded(P, enc, "mini3")
     rc = wl.random_coords(cfg, max(n, 1), seed_offset=n)[:n]
     expect = s.decode(rc) if n else np.zeros((0, 3), np.uint8)
-    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
         P.hmlfc_set_decode_variant(h, variant)
         assert np.array_equal(P.hmlfc_decode(h, _dev(rc).reshape(-1, 4)).cpu().numpy(), expect)
         if n:
@@ -86,7 +86,7 @@ def test_decode_out_of_range_is_black_and_counted(P, enc):
     h = P.hmlfc_load(data)
     coords = np.array([[0, 0, 0, 0], [8, 0, 0, 0], [0, -1, 0, 0], [0, 0, 64, 0], [0, 0, 0, 64], [7, 7, 63, 63]], dtype=np.int32)
     exp, oob = s.decode(coords, return_oob=True)
-    for k, variant in enumerate((P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY)):
+    for k, variant in enumerate((P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC)):
         P.hmlfc_set_decode_variant(h, variant)
         out = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
         assert np.array_equal(out, exp) and oob == 4 and P.hmlfc_last_oob_count(h) == (k + 1) * oob
@@ -131,7 +131,7 @@ def test_decode_blocks_random_access_at_block_granularity(P, enc, name):
         coords = np.stack([np.repeat(blocks[:, 0], B * B), np.repeat(blocks[:, 1], B * B),
                            (blocks[:, 2:3] * B + ii.ravel()[None]).ravel(), (blocks[:, 3:4] * B + jj.ravel()[None]).ravel()], axis=1).astype(np.int32)
         expect = s.decode(coords).reshape(n, B, B, 3)
-        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+        for variant in (P.DECODE_AUTO, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
             P.hmlfc_set_decode_variant(h, variant)
             assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy(), expect), (name, n, variant)
     P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
@@ -183,7 +183,7 @@ def test_other_block_sizes_and_windows(P, enc, name):
     h = _loaded(P, enc, name)
     assert (h.info.block, h.info.window) == (cfg.block, cfg.window)
     coords = wl.all_coords(cfg)
-    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+    for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
         P.hmlfc_set_decode_variant(h, variant)
         assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy().reshape(lf.shape), info["p1"])
     P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
@@ -279,7 +279,7 @@ def test_progressive_levels_match_oracle(P, enc, name):
         s.set_min_level(L)
         P.hmlfc_set_min_level(h, L)
         expect = s.decode(coords)
-        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY):
+        for variant in (P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):
             P.hmlfc_set_decode_variant(h, variant)
             assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), (L, variant)
         # whole views at this level: the block-row kernel (B = 4) / the lane-per-pixel kernel; all_coords is in [V][U][Ht][Ws] order
