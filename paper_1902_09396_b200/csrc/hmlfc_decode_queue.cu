@@ -92,13 +92,6 @@ __device__ __forceinline__ uint32_t bise_at(const uint32_t *__restrict__ words, 
     return (dig << m) | low;
 }
 
-// 256-bit load (LDG.E.ENL2.256, sm_100a): two adjacent 16-byte records of a 32-byte aligned pair in one request
-__device__ __forceinline__ void ldg256(const uint4 *__restrict__ p, uint4 &a, uint4 &b)
-{
-    asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
-}
-
 constexpr uint32_t kSignBit = 1u << 23;  // value task: subtract (additive / "phase-shifted" mode, R10)
 
 // push one task per flagged lane on a warp stack; cnt is warp-uniform

@@ -72,6 +72,13 @@ HMLFC_DEV T ldg(const T *p)
     return __ldg(p);
 }
 
+// 256-bit load (LDG.E.ENL2.256, sm_100a): two adjacent 16-byte records of a 32-byte aligned pair in one request
+HMLFC_DEV void ldg256(const uint4 *__restrict__ p, uint4 &a, uint4 &b)
+{
+    asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+}
+
 HMLFC_DEV uint32_t funnel_r(uint32_t lo, uint32_t hi, uint32_t sh)
 {
     return __funnelshift_r(lo, hi, sh);
