@@ -222,7 +222,7 @@ __device__ __forceinline__ uint32_t value_what(uint32_t bit, uint32_t present, u
     return bit | (present << 5) | (wanted << 8) | (sub << 11) | ((pb.y & 0xFu) << 14) | (((pb.y >> 8) & 0xFu) << 18) | (((pb.y >> 16) & 0xFu) << 22) | (lane << 26);
 }
 
-template <typename Q>
+template <bool kCg, typename Q>
 __device__ __forceinline__ void drain_values_brec(const DevStream &S, Q &q, int &vcnt, int n, int lane)
 {
     __syncwarp();
@@ -232,7 +232,7 @@ __device__ __forceinline__ void drain_values_brec(const DevStream &S, Q &q, int 
         const uint32_t w[3] = {(t.y >> 14) & 15u, (t.y >> 18) & 15u, (t.y >> 22) & 15u};
         const int off[3] = {(int)(int16_t)(t.z & 0xFFFFu), (int)(int16_t)(t.z >> 16), (int)(int16_t)(t.w & 0xFFFFu)};
         const uint32_t span = ((present & 1u) ? w[0] : 0u) + ((present & 2u) ? w[1] : 0u) + ((present & 4u) ? w[2] : 0u);
-        const BrecWindow win = brec_window(S.brec, ((unsigned long long)t.x << 5) | sh, span);
+        const BrecWindow win = brec_window<kCg>(S.brec, ((unsigned long long)t.x << 5) | sh, span);
         int *acc = q.acc + (t.y >> 26) * 4;
         uint32_t pos = sh;
 #pragma unroll
@@ -250,7 +250,7 @@ __device__ __forceinline__ void drain_values_brec(const DevStream &S, Q &q, int 
 }
 
 // reference lookups: slot and descriptor of the reference plane -> value task for the channels its block holds
-template <typename Q>
+template <bool kCg, typename Q>
 __device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int &rcnt, int &vcnt, int n, int lane, uint32_t lane_lt)
 {
     __syncwarp();
@@ -261,7 +261,8 @@ __device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int
         const int rx = (int)(t.y & 0xFFFFu), ry = (int)(t.y >> 16);
         const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
         uint4 sa, sb;
-        ldg256(S.bslot + ((size_t)t.x * (size_t)S.fgroups + (size_t)(b >> 5)) * 2u, sa, sb);
+        if (kCg) ldcg256(S.bslot + ((size_t)t.x * (size_t)S.fgroups + (size_t)(b >> 5)) * 2u, sa, sb);
+        else ldg256(S.bslot + ((size_t)t.x * (size_t)S.fgroups + (size_t)(b >> 5)) * 2u, sa, sb);
         const uint4 pb = ldg(S.pb + t.x);
         const BrecPos r = brec_locate(S, sa, sb, 1u << (b & 31), pb);
         const uint32_t wanted = (t.z & 7u) & r.res;
@@ -276,7 +277,7 @@ __device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int
 }
 
 // motion records of a block (S6), reference sample of every predicted channel (S7) -> lookup tasks
-template <typename Q>
+template <bool kCg, typename Q>
 __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int &mcnt, int &rcnt, int n, int lane, uint32_t lane_lt)
 {
     __syncwarp();
@@ -286,7 +287,7 @@ __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int 
     if (lane < n) {
         t = q.mq[mcnt - n + lane];
         const uint32_t sh = t.y & 31u, pred = (t.y >> 5) & 7u, todo = t.w & 7u;  // todo: the channels this pass still has to look up
-        const BrecWindow win = brec_window(S.brec, ((unsigned long long)t.x << 5) | sh, popc(pred) * S.mv_w);
+        const BrecWindow win = brec_window<kCg>(S.brec, ((unsigned long long)t.x << 5) | sh, popc(pred) * S.mv_w);
         const uint32_t xy = q.xy[(t.y >> 8) & 31u];
         uint32_t pos = sh;
 #pragma unroll
@@ -399,6 +400,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     int vcnt = 0, mcnt = 0;
 
     constexpr bool kLazy = kMode == 1;
+    constexpr bool kCg = kMode == 3;  // streams in HBM: the random sectors go through the L2 only
     if (kMode >= 2) {
         // S4 on the block records: per level ONE sector (the slot of the block's group in the level's plane) says what the plane holds for
         // the sample and where; the plane's descriptor (16 bytes, a few hundred KB in all) gives widths and offsets
@@ -417,7 +419,8 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
                 const bool predictive = ((pu | pv) & 1) != 0;
                 uint4 sa = make_uint4(0u, 0u, 0u, 0u), sb = sa, pb = sa;
                 if (valid) {
-                    ldg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
+                    if (kCg) ldcg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
+                    else ldg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
                     pb = ldg(S.pb + plane);
                 }
                 const BrecPos r = brec_locate(S, sa, sb, bit, pb);
@@ -428,12 +431,12 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
                      make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | ((uint32_t)lane << 8), rplane, r.pred), lane_lt);
             }
             if (!flush) {  // (in the level loop the usual order, inline: 4% faster than going through the loop below)
-                if (vcnt >= 32) drain_values_brec(S, q, vcnt, 32, lane);
+                if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
                 while (mcnt >= 32) {
-                    drain_motion_brec(S, q, mcnt, rcnt, 32, lane, lane_lt);
+                    drain_motion_brec<kCg>(S, q, mcnt, rcnt, 32, lane, lane_lt);
                     if (rcnt >= 32) {
-                        drain_lookups_brec(S, q, rcnt, vcnt, 32, lane, lane_lt);
-                        if (vcnt >= 32) drain_values_brec(S, q, vcnt, 32, lane);
+                        drain_lookups_brec<kCg>(S, q, rcnt, vcnt, 32, lane, lane_lt);
+                        if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
                     }
                 }
                 continue;
@@ -442,9 +445,9 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
             while (true) {
                 const int which = vcnt >= 32 ? 0 : rcnt >= 32 ? 1 : (mcnt >= 32 || (flush && mcnt > 0)) ? 2 : (flush && rcnt > 0) ? 1 : (flush && vcnt > 0) ? 0 : -1;
                 if (which < 0) break;
-                if (which == 0) drain_values_brec(S, q, vcnt, min(vcnt, 32), lane);
-                else if (which == 1) drain_lookups_brec(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
-                else drain_motion_brec(S, q, mcnt, rcnt, min(mcnt, 32), lane, lane_lt);
+                if (which == 0) drain_values_brec<kCg>(S, q, vcnt, min(vcnt, 32), lane);
+                else if (which == 1) drain_lookups_brec<kCg>(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
+                else drain_motion_brec<kCg>(S, q, mcnt, rcnt, min(mcnt, 32), lane, lane_lt);
             }
         }
     } else if (kLazy) {

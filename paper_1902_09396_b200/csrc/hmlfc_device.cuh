@@ -79,6 +79,13 @@ HMLFC_DEV void ldg256(const uint4 *__restrict__ p, uint4 &a, uint4 &b)
                  : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
 }
 
+// the same through the L2 only (ld.global.cg): a random sector that the L1 would not see again anyway
+HMLFC_DEV void ldcg256(const uint4 *__restrict__ p, uint4 &a, uint4 &b)
+{
+    asm volatile("ld.global.cg.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+}
+
 HMLFC_DEV uint32_t funnel_r(uint32_t lo, uint32_t hi, uint32_t sh)
 {
     return __funnelshift_r(lo, hi, sh);
@@ -216,14 +223,15 @@ HMLFC_DEV int brec_offset_of(uint4 pb, int c) { return (int)(int16_t)(c == 0 ? p
 // 96-bit window of brec[] from the word that holds bit `bit`: an aligned 64-bit load, the next pair only when `span` bits from `bit`
 // leave the first (at most 96 - 31 = 65 bits are needed by any caller)
 struct BrecWindow { uint32_t w0, w1, w2; };
+template <bool kCg = false>
 HMLFC_DEV BrecWindow brec_window(const uint32_t *__restrict__ brec, unsigned long long bit, uint32_t span)
 {
     const unsigned long long wi = bit >> 5;
     const uint32_t odd = (uint32_t)wi & 1u, sh = (uint32_t)bit & 31u;
     const uint2 *p2 = reinterpret_cast<const uint2 *>(brec + (wi & ~1ull));
-    const uint2 A = __ldg(p2);
+    const uint2 A = kCg ? __ldcg(p2) : __ldg(p2);
     uint2 B = make_uint2(0u, 0u);
-    if (odd * 32u + sh + span > 64u) B = __ldg(p2 + 1);
+    if (odd * 32u + sh + span > 64u) B = kCg ? __ldcg(p2 + 1) : __ldg(p2 + 1);
     BrecWindow r;
     r.w0 = odd ? A.y : A.x; r.w1 = odd ? B.x : A.y; r.w2 = odd ? B.y : B.x;
     return r;
