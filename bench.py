@@ -200,6 +200,8 @@ def _config_dict(cfg, info):
                     f"render {cfg.n_views} views of {cfg.out_w}x{cfg.out_h} per step on the seeded circular camera path",
         "stream_bytes": info["stream_bytes"], "stream_bpp": round(info["bpp"], 4), "psnr_db": round(info["psnr"], 3),
         "tau_res": info["tau_res"], "views_per_step": cfg.n_views, "out_w": cfg.out_w, "out_h": cfg.out_h,
+        "encoder_policy": "adaptive (DESIGN.md R13: a predictive block below tau_res is dropped whole and pred is kept only where it lowers the "
+                          "energy; SPEC.md's default stores a motion record for every predictive block = policy 'all')",
     }
 
 
