@@ -278,7 +278,7 @@ __device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int
 
 // motion records of a block (S6), reference sample of every predicted channel (S7) -> lookup tasks
 template <bool kCg, typename Q>
-__device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int &mcnt, int &rcnt, int n, int lane, uint32_t lane_lt)
+__device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int &mcnt, int &rcnt, int &vcnt, int n, int lane, uint32_t lane_lt)
 {
     __syncwarp();
     uint32_t rem = 0u, sub = 0u;
@@ -286,7 +286,7 @@ __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int 
     uint4 t = make_uint4(0u, 0u, 0u, 0u);
     if (lane < n) {
         t = q.mq[mcnt - n + lane];
-        const uint32_t sh = t.y & 31u, pred = (t.y >> 5) & 7u, todo = t.w & 7u;  // todo: the channels this pass still has to look up
+        const uint32_t sh = t.y & 31u, pred = (t.y >> 5) & 7u;
         const BrecWindow win = brec_window<kCg>(S.brec, ((unsigned long long)t.x << 5) | sh, popc(pred) * S.mv_w);
         const uint32_t xy = q.xy[(t.y >> 8) & 31u];
         uint32_t pos = sh;
@@ -298,22 +298,30 @@ __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int 
             pos += S.mv_w;
             px[c] = (int)(xy & 0xFFFFu) + dx; py[c] = (int)(xy >> 16) + dy;
             if (mode) sub |= 1u << c;
-            if (((todo >> c) & 1u) && (unsigned)px[c] < (unsigned)S.Ws && (unsigned)py[c] < (unsigned)S.Ht) rem |= 1u << c;  // R8: outside the image reads 0
+            if ((unsigned)px[c] < (unsigned)S.Ws && (unsigned)py[c] < (unsigned)S.Ht) rem |= 1u << c;  // R8: outside the image reads 0
         }
     }
     mcnt -= n;
     __syncwarp();
-    // one lookup for the first channel and every channel whose motion record points at the same reference sample (usually all: the
-    // channels of a block move together); the others come back as a motion task of their own
-    const int c0 = (rem & 1u) ? 0 : (rem & 2u) ? 1 : 2;
-    const int x0 = c0 == 0 ? px[0] : c0 == 1 ? px[1] : px[2], y0 = c0 == 0 ? py[0] : c0 == 1 ? py[1] : py[2];
-    uint32_t grp = 0u;
+    // one lookup per distinct reference sample: the first channel and every channel whose motion record points at the same sample (usually
+    // all: the channels of a block move together), then the same for what is left (a pass through the motion stack for the few stragglers
+    // would run whole 32-lane batches for a handful of tasks)
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
-        if (((rem >> c) & 1u) && px[c] == x0 && py[c] == y0) grp |= 1u << c;
-    push(q.rq, rcnt, rem != 0u, make_uint4(t.z, (uint32_t)x0 | ((uint32_t)y0 << 16), grp | (sub << 3) | (((t.y >> 8) & 31u) << 8), 0u), lane_lt);
-    rem &= ~grp;
-    push(q.mq, mcnt, rem != 0u, make_uint4(t.x, t.y, t.z, rem), lane_lt);
+    for (int round = 0; round < 3; ++round) {
+        if (!__any_sync(0xffffffffu, rem != 0u)) break;
+        const int c0 = (rem & 1u) ? 0 : (rem & 2u) ? 1 : 2;
+        const int x0 = c0 == 0 ? px[0] : c0 == 1 ? px[1] : px[2], y0 = c0 == 0 ? py[0] : c0 == 1 ? py[1] : py[2];
+        uint32_t grp = 0u;
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            if (((rem >> c) & 1u) && px[c] == x0 && py[c] == y0) grp |= 1u << c;
+        push(q.rq, rcnt, rem != 0u, make_uint4(t.z, (uint32_t)x0 | ((uint32_t)y0 << 16), grp | (sub << 3) | (((t.y >> 8) & 31u) << 8), 0u), lane_lt);
+        rem &= ~grp;
+        if (rcnt >= 32) {
+            drain_lookups_brec<kCg>(S, q, rcnt, vcnt, 32, lane, lane_lt);
+            if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
+        }
+    }
 }
 
 template <int kMode, typename Q>
@@ -336,7 +344,7 @@ __device__ __forceinline__ void drain_m(const DevStream &S, Q &q, int &mcnt, int
 // streams the L2 holds, where the sector rate binds); otherwise it reads the three channels' flag records and descriptors up front and the
 // tasks carry them (one dependent load less per task: for streams in HBM, where every access is a DRAM access either way and latency binds).
 template <int kDense, int kMode>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, kMode == 2 ? 6 : 5)  // (the L2-resident block-record case runs best with 6 CTAs per SM, the others with 5)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
 {
@@ -428,17 +436,11 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
                 push(q.vq, vcnt, r.res != 0u,
                      make_uint4((uint32_t)(vpos >> 5), value_what((uint32_t)vpos & 31u, r.res, r.res, 0u, pb, (uint32_t)lane), pb.z, pb.w), lane_lt);
                 push(q.mq, mcnt, predictive && r.pred != 0u,
-                     make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | ((uint32_t)lane << 8), rplane, r.pred), lane_lt);
+                     make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | ((uint32_t)lane << 8), rplane, 0u), lane_lt);
             }
             if (!flush) {  // (in the level loop the usual order, inline: 4% faster than going through the loop below)
                 if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
-                while (mcnt >= 32) {
-                    drain_motion_brec<kCg>(S, q, mcnt, rcnt, 32, lane, lane_lt);
-                    if (rcnt >= 32) {
-                        drain_lookups_brec<kCg>(S, q, rcnt, vcnt, 32, lane, lane_lt);
-                        if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
-                    }
-                }
+                if (mcnt >= 32) drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, 32, lane, lane_lt);
                 continue;
             }
 #pragma unroll 1
@@ -447,7 +449,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
                 if (which < 0) break;
                 if (which == 0) drain_values_brec<kCg>(S, q, vcnt, min(vcnt, 32), lane);
                 else if (which == 1) drain_lookups_brec<kCg>(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
-                else drain_motion_brec<kCg>(S, q, mcnt, rcnt, min(mcnt, 32), lane, lane_lt);
+                else drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, min(mcnt, 32), lane, lane_lt);
             }
         }
     } else if (kLazy) {
