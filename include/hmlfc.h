@@ -85,7 +85,11 @@ typedef struct {
  * PAPER.md:296 "the reference SRV images at all the levels are ... loaded into the memory".
  * Parses the serialized stream (layout: DESIGN.md "Stream format v1"), re-packs it into the
  * device structure-of-arrays form (flag + rank records, bit-packed BISE payloads and motion
- * vectors, packed top-level RKVs) and uploads it to the current CUDA device.
+ * vectors, packed top-level RKVs) and uploads it to the current CUDA device.  For streams with
+ * full-resolution chroma one kernel then writes the BLOCK RECORDS on the device (every stored value
+ * and motion record once more, grouped per block for random access: DESIGN.md section 8); the call
+ * returns when they are complete.  hmlfc_info().device_bytes counts everything that stays resident
+ * (about 2.2 x the stream).  HMLFC_E_NOMEM if the device cannot hold it.
  *   h_stream_bytes : host, read only during the call; the caller may free it afterwards.
  *   out            : receives the handle; untouched on error.                              */
 int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out);
