@@ -25,6 +25,10 @@ namespace {
 
 constexpr int kThreads = 256, kWarps = kThreads / 32;
 constexpr int kCap = 64;  // per stack: < 32 left over + <= 32 pushed per round
+// runs of 32 coordinates per warp of the block-record kernel.  Two runs sharing the stacks (the last, partial batches paid once per 64
+// coordinates) measured SLOWER: cfg2 11.8 against 16.9 G px/s -- 5 KB more shared memory per CTA is L1 taken away, and the second run's
+// slot loads wait behind the first run's pushes.
+constexpr int kBrecSets = 1;
 
 struct DigitLut {
     uint16_t v[384];
@@ -50,16 +54,15 @@ constexpr DigitLut make_digit_lut()
 __device__ const DigitLut g_dq_digit_lut = make_digit_lut();
 
 // (shared memory is L1 taken away: this kernel's loads live on L1 hits of descriptors, slots and neighbouring fields, so the stacks stay small)
-template <int kLookups>
+template <int kLookups, int kSets>
 struct WarpQT {
-    uint4 vq[kCap];      // value tasks
-    uint4 mq[kCap];      // motion tasks
-    uint4 rq[kLookups];  // reference lookups (block records only)
-    int acc[32 * 4];     // {Y, Co, Cg, -} per coordinate of the warp
-    uint32_t xy[32];     // s | t << 16 of the warp's coordinates
+    uint4 vq[kCap];              // value tasks
+    uint4 mq[kCap];              // motion tasks
+    uint4 rq[kLookups];          // reference lookups (block records only)
+    int acc[kSets * 32 * 4];     // {Y, Co, Cg, -} per coordinate of the warp
+    uint32_t xy[kSets * 32];     // s | t << 16 of the warp's coordinates
 };
-using WarpQ = WarpQT<1>;
-using WarpQB = WarpQT<kCap>;
+using WarpQ = WarpQT<1, 1>;
 
 // BISE decode_at (bit layout in DESIGN.md section 4) of value i of the string that starts at word `base`
 // of `words`, without control flow: plain = groups of one value with an empty digit word, so lanes holding tasks of
@@ -118,7 +121,7 @@ __device__ __forceinline__ void drain_values(const DevStream &S, Q &q, int &vcnt
         const uint4 t = q.vq[vcnt - n + lane];
         const uint4 d = ldg(S.pc + t.x);
         const uint32_t rank0 = __ldg(reinterpret_cast<const uint32_t *>(S.flagrec + flag_index(S, t.x, t.y)) + 1);  // res blocks before the group
-        const uint32_t idx = ((rank0 + ((t.z >> 8) & 31u)) << (2 * S.logB)) + (t.z & 63u);
+        const uint32_t idx = ((rank0 + ((t.z >> 8) & 63u)) << (2 * S.logB)) + (t.z & 63u);
         int val = pc_offset(d.w) + (int)bise_at(S.pay, d.y, idx, pc_layout(d.w), pc_m(d.w), lut);
         if (t.z & kSignBit) val = -val;
         atomicAdd(&q.acc[t.z >> 24], val);
@@ -269,7 +272,7 @@ __device__ __forceinline__ void drain_lookups_brec(const DevStream &S, Q &q, int
         has = wanted != 0u;
         const uint32_t kin = (uint32_t)(((ry & (S.B - 1)) << S.logB) + (rx & (S.B - 1)));
         const unsigned long long pos = r.bit + brec_sample_offset(r, pb, kin);
-        vt = make_uint4((uint32_t)(pos >> 5), value_what((uint32_t)pos & 31u, r.res, wanted, (t.z >> 3) & 7u, pb, (t.z >> 8) & 31u), pb.z, pb.w);
+        vt = make_uint4((uint32_t)(pos >> 5), value_what((uint32_t)pos & 31u, r.res, wanted, (t.z >> 3) & 7u, pb, (t.z >> 8) & 63u), pb.z, pb.w);
     }
     rcnt -= n;
     __syncwarp();
@@ -288,7 +291,7 @@ __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int 
         t = q.mq[mcnt - n + lane];
         const uint32_t sh = t.y & 31u, pred = (t.y >> 5) & 7u;
         const BrecWindow win = brec_window<kCg>(S.brec, ((unsigned long long)t.x << 5) | sh, popc(pred) * S.mv_w);
-        const uint32_t xy = q.xy[(t.y >> 8) & 31u];
+        const uint32_t xy = q.xy[(t.y >> 8) & 63u];
         uint32_t pos = sh;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -315,7 +318,7 @@ __device__ __forceinline__ void drain_motion_brec(const DevStream &S, Q &q, int 
 #pragma unroll
         for (int c = 0; c < 3; ++c)
             if (((rem >> c) & 1u) && px[c] == x0 && py[c] == y0) grp |= 1u << c;
-        push(q.rq, rcnt, rem != 0u, make_uint4(t.z, (uint32_t)x0 | ((uint32_t)y0 << 16), grp | (sub << 3) | (((t.y >> 8) & 31u) << 8), 0u), lane_lt);
+        push(q.rq, rcnt, rem != 0u, make_uint4(t.z, (uint32_t)x0 | ((uint32_t)y0 << 16), grp | (sub << 3) | (((t.y >> 8) & 63u) << 8), 0u), lane_lt);
         rem &= ~grp;
         if (rcnt >= 32) {
             drain_lookups_brec<kCg>(S, q, rcnt, vcnt, 32, lane, lane_lt);
@@ -344,16 +347,14 @@ __device__ __forceinline__ void drain_m(const DevStream &S, Q &q, int &mcnt, int
 // streams the L2 holds, where the sector rate binds); otherwise it reads the three channels' flag records and descriptors up front and the
 // tasks carry them (one dependent load less per task: for streams in HBM, where every access is a DRAM access either way and latency binds).
 template <int kDense, int kMode>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
-__global__ void __launch_bounds__(kThreads, kMode == 2 ? 6 : 5)  // (the L2-resident block-record case runs best with 6 CTAs per SM, the others with 5)
+__global__ void __launch_bounds__(kThreads, 5)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
 {
-    __shared__ typename std::conditional<kMode >= 2, WarpQB, WarpQ>::type wq[kWarps];
+    __shared__ WarpQ wq[kWarps];
     __shared__ uint16_t lut[384];
-    if (kMode < 2) {  // (the block records are plain binary)
-        for (int k = threadIdx.x; k < 384; k += kThreads) lut[k] = g_dq_digit_lut.v[k];
-        __syncthreads();
-    }
+    for (int k = threadIdx.x; k < 384; k += kThreads) lut[k] = g_dq_digit_lut.v[k];
+    __syncthreads();
 
     const int lane = threadIdx.x & 31;
     const uint32_t lane_lt = (1u << lane) - 1u;
@@ -408,51 +409,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     int vcnt = 0, mcnt = 0;
 
     constexpr bool kLazy = kMode == 1;
-    constexpr bool kCg = kMode == 3;  // streams in HBM: the random sectors go through the L2 only
-    if (kMode >= 2) {
-        // S4 on the block records: per level ONE sector (the slot of the block's group in the level's plane) says what the plane holds for
-        // the sample and where; the plane's descriptor (16 bytes, a few hundred KB in all) gives widths and offsets
-        // Every batch of 32 tasks is executed by ONE copy of its code (the kernel is instruction-cache bound otherwise): the level loop runs
-        // one extra round that only flushes.  Order: values while 32 wait, then lookups (they push <= 32 values), then motion tasks
-        // (<= 32 lookups); the flush drains producers first.
-        int rcnt = 0;
-#pragma unroll 1
-        for (int L = S.lmin; L <= h; ++L) {
-            const bool flush = L == h;
-            if (!flush) {
-                const int pu = u >> L, pv = v >> L;
-                const LevelDesc lv = S.lev[L];
-                const uint32_t plane0 = umulhi(lv.pc_base, 0xAAAAAAABu) >> 1;  // pc_base / 3
-                const uint32_t plane = plane0 + (uint32_t)(pv * lv.UL + pu), rplane = plane0 + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1));
-                const bool predictive = ((pu | pv) & 1) != 0;
-                uint4 sa = make_uint4(0u, 0u, 0u, 0u), sb = sa, pb = sa;
-                if (valid) {
-                    if (kCg) ldcg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
-                    else ldg256(S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)fg) * 2u, sa, sb);
-                    pb = ldg(S.pb + plane);
-                }
-                const BrecPos r = brec_locate(S, sa, sb, bit, pb);
-                const unsigned long long vpos = r.bit + brec_sample_offset(r, pb, kin);
-                push(q.vq, vcnt, r.res != 0u,
-                     make_uint4((uint32_t)(vpos >> 5), value_what((uint32_t)vpos & 31u, r.res, r.res, 0u, pb, (uint32_t)lane), pb.z, pb.w), lane_lt);
-                push(q.mq, mcnt, predictive && r.pred != 0u,
-                     make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | ((uint32_t)lane << 8), rplane, 0u), lane_lt);
-            }
-            if (!flush) {  // (in the level loop the usual order, inline: 4% faster than going through the loop below)
-                if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
-                if (mcnt >= 32) drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, 32, lane, lane_lt);
-                continue;
-            }
-#pragma unroll 1
-            while (true) {
-                const int which = vcnt >= 32 ? 0 : rcnt >= 32 ? 1 : (mcnt >= 32 || (flush && mcnt > 0)) ? 2 : (flush && rcnt > 0) ? 1 : (flush && vcnt > 0) ? 0 : -1;
-                if (which < 0) break;
-                if (which == 0) drain_values_brec<kCg>(S, q, vcnt, min(vcnt, 32), lane);
-                else if (which == 1) drain_lookups_brec<kCg>(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
-                else drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, min(mcnt, 32), lane, lane_lt);
-            }
-        }
-    } else if (kLazy) {
+    if (kLazy) {
         // S4, first look, for (up to) four levels at a time: the six flag words of the block's group in each level's plane, one 32-byte
         // sector per level (the second half of the plane's 64-byte slot: the Cg record {res, rank, pred, rank} and {res Y, res Co, pred Y,
         // pred Co}).  The addresses depend on the coordinate alone, so the levels' loads are in flight together: one memory round trip
@@ -580,6 +537,117 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// hmlfc_decode on the block records (hmlfc_device.cuh): a warp walks kSets x 32 coordinates through the levels and shares its task
+// stacks between them (kSets = 1 is what runs, see kBrecSets).  kCg: streams in HBM: the random sectors go through the L2 only.
+template <bool kCg, int kSets, int kMinBlocks>
+__global__ void __launch_bounds__(kThreads, kMinBlocks)
+decode_brec_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
+                   unsigned long long *oob, int out_aligned)
+{
+    __shared__ WarpQT<kCap, kSets> wq[kWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t lane_lt = (1u << lane) - 1u;
+    auto &q = wq[warp];
+    const int h = S.h;
+    // coordinate of set k: the warp's k-th run of 32 consecutive coordinates
+    long long idx[kSets];
+    int4 c4[kSets];
+    bool valid[kSets];
+#pragma unroll
+    for (int k = 0; k < kSets; ++k) {
+        idx[k] = ((long long)blockIdx.x * kWarps + warp) * (kSets * 32) + k * 32 + lane;
+        c4[k] = make_int4(0, 0, 0, 0);
+        if (idx[k] < n) c4[k] = __ldg(coords + idx[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < kSets; ++k) {
+        valid[k] = idx[k] < n && (unsigned)c4[k].x < (unsigned)S.U && (unsigned)c4[k].y < (unsigned)S.V &&
+                   (unsigned)c4[k].z < (unsigned)S.Ws && (unsigned)c4[k].w < (unsigned)S.Ht;
+        if (idx[k] < n && !valid[k]) atomicAdd(oob, 1ull);
+        // S3 root term: one 64-bit load; the cell starts at the top-level RKV sample
+        short4 root = make_short4(0, 0, 0, 0);
+        if (valid[k])
+            root = ldg(S.rkv + ((size_t)((c4[k].y >> h) * S.UH + (c4[k].x >> h)) * (size_t)S.Ht + (size_t)c4[k].w) * (size_t)S.Ws + (size_t)c4[k].z);
+        const int cell = k * 32 + lane;
+        q.acc[cell * 4 + 0] = root.x;
+        q.acc[cell * 4 + 1] = root.y;
+        q.acc[cell * 4 + 2] = root.z;
+        q.xy[cell] = (uint32_t)c4[k].z | ((uint32_t)c4[k].w << 16);
+    }
+    int vcnt = 0, mcnt = 0, rcnt = 0;
+    // S4 on the block records: per level ONE sector (the slot of the block's group in the level's plane) says what the plane holds for
+    // the sample and where; the plane's descriptor (16 bytes, a few hundred KB in all) gives widths and offsets.  The level loop runs
+    // one extra round that only flushes (one copy of the flush code).
+#pragma unroll 1
+    for (int L = S.lmin; L <= h; ++L) {
+        const bool flush = L == h;
+        if (!flush) {
+            const LevelDesc lv = S.lev[L];
+            const uint32_t plane0 = umulhi(lv.pc_base, 0xAAAAAAABu) >> 1;  // pc_base / 3
+#pragma unroll
+            for (int k = 0; k < kSets; ++k) {
+                const int pu = c4[k].x >> L, pv = c4[k].y >> L;
+                const uint32_t plane = plane0 + (uint32_t)(pv * lv.UL + pu), rplane = plane0 + (uint32_t)((pv & ~1) * lv.UL + (pu & ~1));
+                const bool predictive = ((pu | pv) & 1) != 0;
+                const int b = valid[k] ? (c4[k].w >> S.logB) * S.nbx + (c4[k].z >> S.logB) : 0;
+                const uint32_t kin = (uint32_t)(((c4[k].w & (S.B - 1)) << S.logB) + (c4[k].z & (S.B - 1)));
+                uint4 sa = make_uint4(0u, 0u, 0u, 0u), sb = sa, pb = sa;
+                if (valid[k]) {
+                    const uint4 *slot = S.bslot + ((size_t)plane * (size_t)S.fgroups + (size_t)(b >> 5)) * 2u;
+                    if (kCg) ldcg256(slot, sa, sb); else ldg256(slot, sa, sb);
+                    pb = ldg(S.pb + plane);
+                }
+                const BrecPos r = brec_locate(S, sa, sb, 1u << (b & 31), pb);
+                const unsigned long long vpos = r.bit + brec_sample_offset(r, pb, kin);
+                const uint32_t cell = (uint32_t)(k * 32 + lane);
+                push(q.vq, vcnt, r.res != 0u, make_uint4((uint32_t)(vpos >> 5), value_what((uint32_t)vpos & 31u, r.res, r.res, 0u, pb, cell), pb.z, pb.w), lane_lt);
+                push(q.mq, mcnt, predictive && r.pred != 0u,
+                     make_uint4((uint32_t)(r.bit >> 5), ((uint32_t)r.bit & 31u) | (r.pred << 5) | (cell << 8), rplane, 0u), lane_lt);
+                // the usual order, inline (4% faster than going through the loop below)
+                if (vcnt >= 32) drain_values_brec<kCg>(S, q, vcnt, 32, lane);
+                if (mcnt >= 32) drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, 32, lane, lane_lt);
+            }
+            continue;
+        }
+#pragma unroll 1
+        while (true) {
+            const int which = vcnt >= 32 ? 0 : rcnt >= 32 ? 1 : mcnt > 0 ? 2 : rcnt > 0 ? 1 : vcnt > 0 ? 0 : -1;
+            if (which < 0) break;
+            if (which == 0) drain_values_brec<kCg>(S, q, vcnt, min(vcnt, 32), lane);
+            else if (which == 1) drain_lookups_brec<kCg>(S, q, rcnt, vcnt, min(rcnt, 32), lane, lane_lt);
+            else drain_motion_brec<kCg>(S, q, mcnt, rcnt, vcnt, min(mcnt, 32), lane, lane_lt);
+        }
+    }
+    __syncwarp();
+    // S8: inverse YCoCg-R + clamp, then each set's 96 bytes as 24 coalesced words (staged in the empty value stack)
+    uint32_t *stage = reinterpret_cast<uint32_t *>(q.vq);
+#pragma unroll
+    for (int k = 0; k < kSets; ++k) {
+        uint32_t rgb = 0u;
+        if (valid[k]) {
+            const int cell = k * 32 + lane;
+            const int acc[3] = {q.acc[cell * 4 + 0], q.acc[cell * 4 + 1], q.acc[cell * 4 + 2]};
+            rgb = ycocg_to_rgb8(acc);
+        }
+        const long long wbase = idx[k] - lane;
+        uint8_t *o = out + 3 * wbase;
+        if (out_aligned && wbase + 32 <= n) {
+            uint8_t *sb = reinterpret_cast<uint8_t *>(stage + 24 * k);
+            sb[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
+            sb[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
+            sb[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
+            __syncwarp();
+            if (lane < 24) reinterpret_cast<uint32_t *>(o)[lane] = stage[24 * k + lane];
+        } else if (idx[k] < n) {
+            o[3 * lane + 0] = (uint8_t)(rgb & 0xFF);
+            o[3 * lane + 1] = (uint8_t)((rgb >> 8) & 0xFF);
+            o[3 * lane + 2] = (uint8_t)((rgb >> 16) & 0xFF);
+        }
+    }
+}
+
 }  // namespace
 
 // The block-record kernel lives on L1 hits (plane descriptors, neighbouring fields) as much as on occupancy: 6 CTAs per SM leave 60 KB of
@@ -587,7 +655,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
 // kernel with a shared-memory carve-out that fits 5 CTAs, used for streams the L2 does not hold.
 cudaError_t configure_decode_queue()
 {
-    return cudaFuncSetAttribute(decode_queue_kernel<0, 3>, cudaFuncAttributePreferredSharedMemoryCarveout, 65);
+    return cudaFuncSetAttribute(decode_brec_kernel<true, kBrecSets, 5>, cudaFuncAttributePreferredSharedMemoryCarveout, 65);
 }
 
 cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int64_t n, uint8_t *d_out,
@@ -602,12 +670,12 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
     if (mode < 0) mode = S.brec ? 2 : (S.l2_resident ? 1 : 0);
     if (mode == 2 && !S.brec) return cudaErrorInvalidValue;
     const int4 *c4 = reinterpret_cast<const int4 *>(d_coords);
-    if (mode == 1)
+    if (mode == 2) {
+        const long long per_cta = (long long)kThreads * kBrecSets, cb = (n + per_cta - 1) / per_cta;
+        if (S.l2_resident) decode_brec_kernel<false, kBrecSets, 6><<<(unsigned)cb, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
+        else decode_brec_kernel<true, kBrecSets, 5><<<(unsigned)cb, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);  // larger L1: configure_decode_queue
+    } else if (mode == 1)
         decode_queue_kernel<0, 1><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
-    else if (mode == 2 && S.l2_resident)
-        decode_queue_kernel<0, 2><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
-    else if (mode == 2)  // the same kernel with a larger L1 (configure_decode_queue)
-        decode_queue_kernel<0, 3><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     else
         decode_queue_kernel<0, 0><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
