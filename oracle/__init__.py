@@ -22,7 +22,7 @@ class Params(C.Structure):
         ("tau_ref", C.c_int32), ("tau_res", C.c_int32), ("policy", C.c_int32), ("nthreads", C.c_int32),
         ("uv_origin", C.c_float * 2), ("uv_step", C.c_float * 2),
         ("st_origin", C.c_float * 2), ("st_step", C.c_float * 2), ("z_st", C.c_float),
-        ("background", C.c_uint8 * 3), ("chroma", C.c_uint8), ("seed", C.c_uint64),
+        ("background", C.c_uint8 * 3), ("chroma", C.c_uint8), ("subpel", C.c_uint8), ("seed", C.c_uint64),
     ]
 
 
@@ -67,6 +67,7 @@ def lib():
         "orc_tree_get_plane": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp]),
         "orc_tree_get_blocks": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]),
         "orc_search_block": (None, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp]),
+        "orc_search_block_halfpel": (None, [vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, vp]),
         "orc_open": (vp, [vp, C.c_size_t, C.POINTER(C.c_int)]),
         "orc_close": (None, [vp]),
         "orc_stream_params": (C.c_int, [vp, C.POINTER(Params)]),
@@ -102,11 +103,13 @@ def _ptr(a):
 
 
 def make_params(U, V, Ws, Ht, height, block=4, window=16, tau_ref=0, tau_res=0, policy=POLICY_ADAPTIVE,
-                geometry=None, background=(0, 0, 0), seed=0, nthreads=0, chroma=0) -> Params:
+                geometry=None, background=(0, 0, 0), seed=0, nthreads=0, chroma=0, subpel=0) -> Params:
     """geometry: dict(uv_origin, uv_step, st_origin, st_step, z_st) or None for the unit slab.
-    chroma = 1: Co / Cg planes at half resolution (R18)."""
+    chroma = 1: Co / Cg planes at half resolution (R18); subpel = 1: half-pel motion compensation
+    (R28)."""
     p = Params()
     p.chroma = chroma
+    p.subpel = subpel
     p.U, p.V, p.Ws, p.Ht, p.height, p.block, p.window = U, V, Ws, Ht, height, block, window
     p.tau_ref, p.tau_res, p.policy, p.nthreads = tau_ref, tau_res, policy, nthreads
     g = geometry or dict(uv_origin=(0.0, 0.0), uv_step=(1.0, 1.0), st_origin=(0.0, 0.0), st_step=(1.0, 1.0), z_st=1.0)
@@ -246,6 +249,15 @@ def search_block(P, R, B, W, bx, by):
     out = np.zeros(4, dtype=np.int32)
     lib().orc_search_block(_ptr(P), _ptr(R), P.shape[1], P.shape[0], B, W, bx, by, _ptr(out))
     return tuple(int(x) for x in out)  # mode, dx, dy, sad
+
+
+def search_block_halfpel(P, R, B, W, bx, by):
+    """The search on the half-pel grid (R28): (mode, dx2, dy2, sad), offsets in half pixels."""
+    P = np.ascontiguousarray(P, dtype=np.int16)
+    R = np.ascontiguousarray(R, dtype=np.int16)
+    out = np.zeros(4, dtype=np.int32)
+    lib().orc_search_block_halfpel(_ptr(P), _ptr(R), P.shape[1], P.shape[0], B, W, bx, by, _ptr(out))
+    return tuple(int(x) for x in out)
 
 
 def psnr(a, b) -> float:

@@ -67,9 +67,18 @@ static int plane_value(const orc_stream *s, uint64_t k, int x, int y, int use_ra
     return v;
 }
 
+/* stored sample of the reference plane k (channel c) at an integer position: 0 outside the image (R8) or in an insignificant block */
+typedef struct { const orc_stream *s; uint64_t k; int c, use_rank; } ref_ctx;
+static int ref_at(const void *ctx, int rx, int ry)
+{
+    const ref_ctx *r = (const ref_ctx *)ctx;
+    if (rx < 0 || rx >= r->s->g.W[r->c] || ry < 0 || ry >= r->s->g.H[r->c]) return 0;
+    return plane_value(r->s, r->k, rx, ry, r->use_rank);
+}
+
 static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int use_rank, uint8_t rgb[3])
 {
-    const int B = s->p.block, W = s->p.window, h = s->h;
+    const int B = s->p.block, h = s->h;
     const int x0 = x, y0 = y;
     int acc[3];
     for (int c = 0; c < 3; ++c) {
@@ -98,13 +107,13 @@ static void decode_pixel(const orc_stream *s, int u, int v, int x, int y, int us
                         r = tmp[mi];
                         free(tmp);
                     }
-                    int nd = 2 * W + 1;
+                    const int off = orc_mv_off(&s->p), nd = 2 * off + 1;
                     int mode = (int)(r / (uint32_t)(nd * nd));
                     int rem = (int)(r % (uint32_t)(nd * nd));
-                    int dy = rem / nd - W, dx = rem % nd - W;
-                    int rx = x + dx, ry = y + dy, q = 0;
-                    if (rx >= 0 && rx < s->g.W[c] && ry >= 0 && ry < s->g.H[c])
-                        q = plane_value(s, pc_index(s, L, pu & ~1, pv & ~1, c), rx, ry, use_rank);
+                    int dy = rem / nd - off, dx = rem % nd - off;
+                    ref_ctx rc = {s, pc_index(s, L, pu & ~1, pv & ~1, c), c, use_rank};
+                    /* R28: half-pel offsets read the bilinear mean of 1, 2 or 4 stored reference samples */
+                    int q = s->p.subpel ? orc_halfpel(ref_at, &rc, 2 * x + dx, 2 * y + dy) : ref_at(&rc, x + dx, y + dy);
                     e += mode ? -q : q; /* R10: sub P = e + R, add P = e - R */
                 }
             }
@@ -219,7 +228,7 @@ static void touch_block(stat_ctx *cx, uint64_t k, int b, int is_pred_plane)
 static void touch_pixel(stat_ctx *cx, int u, int v, int x, int y)
 {
     const orc_stream *s = cx->s;
-    const int B = s->p.block, W = s->p.window, h = s->h;
+    const int B = s->p.block, h = s->h;
     const uint64_t npx = (uint64_t)s->p.Ws * s->p.Ht, n_top = (uint64_t)s->UL[h] * s->VL[h];
     const int x0 = x, y0 = y;
     cx->st.taps += 1;
@@ -239,11 +248,18 @@ static void touch_pixel(stat_ctx *cx, int u, int v, int x, int y)
             const uint8_t *fpred = s->bytes + s->off_flags + d->flags_off + (size_t)fwords * 4;
             if (!flag_bit(fpred, b)) continue;
             uint32_t r = orc_bise_decode_at(s->bytes + s->off_mv + d->mv_bitoff / 8, s->mvN, s->rank_pred[k][b]);
-            int nd = 2 * W + 1;
+            const int off = orc_mv_off(&s->p), nd = 2 * off + 1;
             int rem = (int)(r % (uint32_t)(nd * nd));
-            int rx = x + rem % nd - W, ry = y + rem / nd - W;
-            if (rx >= 0 && rx < s->g.W[c] && ry >= 0 && ry < s->g.H[c])
-                touch_block(cx, pc_index(s, L, pu & ~1, pv & ~1, c), (ry / B) * s->g.nbx[c] + (rx / B), 0);
+            const int dx = rem % nd - off, dy = rem / nd - off;
+            /* the integer samples the reference value is made of: one, or the 2 / 4 around a half-pel position (R28) */
+            const int x2 = s->p.subpel ? 2 * x + dx : 2 * (x + dx), y2 = s->p.subpel ? 2 * y + dy : 2 * (y + dy);
+            const int rx0 = orc_floor_div(x2, 2), ry0 = orc_floor_div(y2, 2);
+            for (int jy = 0; jy <= (y2 - 2 * ry0); ++jy)
+                for (int jx = 0; jx <= (x2 - 2 * rx0); ++jx) {
+                    const int rx = rx0 + jx, ry = ry0 + jy;
+                    if (rx >= 0 && rx < s->g.W[c] && ry >= 0 && ry < s->g.H[c])
+                        touch_block(cx, pc_index(s, L, pu & ~1, pv & ~1, c), (ry / B) * s->g.nbx[c] + (rx / B), 0);
+                }
         }
     }
 }

@@ -101,6 +101,36 @@ static void search_block_padded(const int16_t *P, int Ws, const int16_t *Rpad, i
     else { out[0] = 1; out[1] = pdx; out[2] = pdy; out[3] = best_p; }
 }
 
+/* The same search on the half-pel grid (R28): offsets (dx2, dy2) in [-2W, 2W]^2 half pixels, the reference block interpolated
+ * bilinearly (orc_halfpel).  Ties as above, on the half-pel offsets.  The integer-pel candidates are the even offsets, so the
+ * minimum is never above the integer-pel minimum. */
+static void search_block_halfpel(const int16_t *P, const int16_t *R, int Ws, int Ht, int B, int W, int bx, int by, int32_t out[4])
+{
+    const orc_plane_src src = {R, Ws, Ht};
+    int best_m = 0x7fffffff, best_p = 0x7fffffff;
+    int mdx = 0, mdy = 0, pdx = 0, pdy = 0;
+    for (int dy = -2 * W; dy <= 2 * W; ++dy)
+        for (int dx = -2 * W; dx <= 2 * W; ++dx) {
+            int sm = 0, sp = 0;
+            for (int j = 0; j < B; ++j)
+                for (int i = 0; i < B; ++i) {
+                    const int x = bx * B + i, y = by * B + j;
+                    const int pv = P[(size_t)y * Ws + x], r = orc_halfpel(orc_plane_at, &src, 2 * x + dx, 2 * y + dy);
+                    sm += iabs(pv - r);
+                    sp += iabs(pv + r);
+                }
+            if (sm < best_m) { best_m = sm; mdx = dx; mdy = dy; }
+            if (sp < best_p) { best_p = sp; pdx = dx; pdy = dy; }
+        }
+    if (best_m <= best_p) { out[0] = 0; out[1] = mdx; out[2] = mdy; out[3] = best_m; }
+    else { out[0] = 1; out[1] = pdx; out[2] = pdy; out[3] = best_p; }
+}
+
+void orc_search_block_halfpel(const int16_t *P, const int16_t *R, int Ws, int Ht, int B, int W, int bx, int by, int32_t out[4])
+{
+    search_block_halfpel(P, R, Ws, Ht, B, W, bx, by, out);
+}
+
 static int16_t *make_padded(const int16_t *R, int Ws, int Ht, int W, int *rstride)
 {
     int stride = Ws + 2 * W;
@@ -136,7 +166,7 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
     if (!err) err = &e_dummy;
     *err = ORC_OK;
     if (!lf || !p || p->U < 1 || p->V < 1 || p->Ws < 1 || p->Ht < 1 || p->height < 1 || p->height > ORC_MAX_LEVELS ||
-        p->block < 1 || p->block > 8 || p->window < 0 || p->window > 64 || p->chroma > 1) {
+        p->block < 1 || p->block > 8 || p->window < 0 || p->window > 64 || p->chroma > 1 || p->subpel > 1) {
         *err = ORC_E_PARAM;
         return NULL;
     }
@@ -263,7 +293,8 @@ orc_tree *orc_encode_begin(const uint8_t *lf, const orc_params *p, int *err)
 #pragma omp parallel for schedule(dynamic, 4)
                             for (int b = 0; b < nblk; ++b) {
                                 int32_t r[4];
-                                search_block_padded(P, Wc, pad, rstride, B, W, b % nbx, b / nbx, r);
+                                if (p->subpel) search_block_halfpel(P, t->srv[c][L][rv * UL + ru], Wc, Hc, B, W, b % nbx, b / nbx, r);
+                                else search_block_padded(P, Wc, pad, rstride, B, W, b % nbx, b / nbx, r);
                                 bk[b].mode = r[0]; bk[b].dx = r[1]; bk[b].dy = r[2]; bk[b].sad = r[3];
                             }
                         }

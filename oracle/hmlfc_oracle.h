@@ -62,6 +62,7 @@ typedef struct {
     float uv_origin[2], uv_step[2], st_origin[2], st_step[2], z_st; /* light slab      */
     uint8_t background[3];
     uint8_t chroma;            /* 1: Co / Cg at half resolution (R18)    */
+    uint8_t subpel;            /* 1: half-pel motion compensation (R28)   */
     uint64_t seed;             /* provenance only                                      */
 } orc_params;
 
@@ -112,6 +113,8 @@ int orc_tree_get_blocks(const orc_tree *t, int L, int pu, int pv, int c, int32_t
 /* search one block directly (pin): P,R int16 planes [Ht][Ws]; writes mode,dx,dy,sad */
 void orc_search_block(const int16_t *P, const int16_t *R, int Ws, int Ht, int B, int W, int bx, int by,
                       int32_t out[4]);
+/* the same on the half-pel grid (R28): out = {mode, dx2, dy2, Delta}, offsets in half pixels, range [-2W, 2W] */
+void orc_search_block_halfpel(const int16_t *P, const int16_t *R, int Ws, int Ht, int B, int W, int bx, int by, int32_t out[4]);
 
 /* ------------------------------------------------------------------ decoder */
 typedef struct orc_stream orc_stream;

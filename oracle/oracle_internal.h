@@ -76,4 +76,34 @@ struct orc_stream {
 
 static inline int orc_is_predictive(int pu, int pv) { return ((pu | pv) & 1) != 0; }
 
+/* ---- half-pel motion compensation (section 6: "sub-pel motion compensation, i.e., sub-pixel level motion compensation
+ * to search for a matching block using bi-linear interpolation methods"; reading R28).  With p.subpel = 1 the
+ * motion offsets (dx, dy) of a block are counted in HALF pixels, range [-2W, 2W]^2.  The reference value at the half-pel position
+ * (x2 / 2, y2 / 2) is the bilinear interpolation there: the mean of the 1, 2 or 4 integer samples around it, rounded half up
+ * (floor((sum + n/2) / n)); a sample outside the image reads 0 (R8).  Even offsets are the integer-pel case. */
+static inline int orc_floor_div(int a, int n)  /* n > 0 */
+{
+    int q = a / n;
+    return (a % n != 0 && a < 0) ? q - 1 : q;
+}
+typedef int (*orc_sample_fn)(const void *ctx, int x, int y);  /* reference sample at an integer position, 0 outside the image */
+static inline int orc_halfpel(orc_sample_fn at, const void *ctx, int x2, int y2)
+{
+    const int x0 = orc_floor_div(x2, 2), y0 = orc_floor_div(y2, 2);
+    const int fx = x2 - 2 * x0, fy = y2 - 2 * y0;
+    int s = at(ctx, x0, y0), n = 1;
+    if (fx) { s += at(ctx, x0 + 1, y0); n = 2; }
+    if (fy) { s += at(ctx, x0, y0 + 1); if (fx) s += at(ctx, x0 + 1, y0 + 1); n *= 2; }
+    return n == 1 ? s : orc_floor_div(s + n / 2, n);
+}
+/* a dense int16 plane as the sample source */
+typedef struct { const int16_t *R; int W, H; } orc_plane_src;
+static inline int orc_plane_at(const void *ctx, int x, int y)
+{
+    const orc_plane_src *p = (const orc_plane_src *)ctx;
+    return (x >= 0 && x < p->W && y >= 0 && y < p->H) ? p->R[(size_t)y * p->W + x] : 0;
+}
+/* motion-record alphabet (R16): offsets in [-off, off], nd = 2 off + 1 values per axis, off = W (integer-pel) or 2W (half-pel) */
+static inline int orc_mv_off(const orc_params *p) { return p->subpel ? 2 * p->window : p->window; }
+
 #endif

@@ -27,18 +27,18 @@ static void wrf(uint8_t *p, float f) { uint32_t u; memcpy(&u, &f, 4); wr32(p, u)
 static float rdf(const uint8_t *p) { uint32_t u = rd32(p); float f; memcpy(&f, &u, 4); return f; }
 static uint64_t align8(uint64_t x) { return (x + 7) & ~(uint64_t)7; }
 
-/* joint motion record (R16): r = mode (2W+1)^2 + (dy+W)(2W+1) + (dx+W) */
-static uint32_t mv_pack(int mode, int dx, int dy, int W)
+/* joint motion record (R16): r = mode nd^2 + (dy + off) nd + (dx + off), nd = 2 off + 1; off = W, or 2W with half-pel offsets (R28) */
+static uint32_t mv_pack(int mode, int dx, int dy, int off)
 {
-    uint32_t nd = (uint32_t)(2 * W + 1);
-    return (uint32_t)mode * nd * nd + (uint32_t)(dy + W) * nd + (uint32_t)(dx + W);
+    uint32_t nd = (uint32_t)(2 * off + 1);
+    return (uint32_t)mode * nd * nd + (uint32_t)(dy + off) * nd + (uint32_t)(dx + off);
 }
 
 int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
 {
     if (!t || !out || !t->thresholded) return ORC_E_PARAM;
     const int Ws = t->p.Ws, Ht = t->p.Ht, B = t->p.block, W = t->p.window, h = t->h;
-    const uint32_t mvN = 2u * (uint32_t)(2 * W + 1) * (uint32_t)(2 * W + 1);
+    const uint32_t mvN = 2u * (uint32_t)(2 * orc_mv_off(&t->p) + 1) * (uint32_t)(2 * orc_mv_off(&t->p) + 1);
 
     uint64_t n_pc = 0;
     for (int L = 0; L < h; ++L) n_pc += (uint64_t)t->UL[L] * t->VL[L] * 3;
@@ -109,7 +109,8 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
     s[49] = t->p.chroma ? 1 : 0; /* chroma subsampling (R18): Co / Cg planes at Ws/2 x Ht/2 */
     s[50] = 0; /* RKV codec: raw (R20) */
     s[51] = (uint8_t)t->p.policy;
-    s[52] = t->p.background[0]; s[53] = t->p.background[1]; s[54] = t->p.background[2]; s[55] = 0;
+    s[52] = t->p.background[0]; s[53] = t->p.background[1]; s[54] = t->p.background[2];
+    s[55] = t->p.subpel ? 1 : 0; /* motion offsets in half pixels (R28) */
     wrf(s + 56, t->p.uv_origin[0]); wrf(s + 60, t->p.uv_origin[1]);
     wrf(s + 64, t->p.uv_step[0]);   wrf(s + 68, t->p.uv_step[1]);
     wrf(s + 72, t->p.st_origin[0]); wrf(s + 76, t->p.st_origin[1]);
@@ -156,7 +157,7 @@ int64_t orc_tree_serialize(const orc_tree *t, uint8_t **out)
                     for (int b = 0; b < nblk; ++b) {
                         if (bk[b].flags & 2) {
                             fpred[b >> 3] |= (uint8_t)(1u << (b & 7));
-                            mvs[nm++] = mv_pack(bk[b].mode, bk[b].dx, bk[b].dy, W);
+                            mvs[nm++] = mv_pack(bk[b].mode, bk[b].dx, bk[b].dy, orc_mv_off(&t->p));
                         }
                         if (!(bk[b].flags & 1)) continue;
                         fres[b >> 3] |= (uint8_t)(1u << (b & 7));
@@ -217,7 +218,8 @@ orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err)
     s->off_payload = rd64(bytes + 136); s->off_mv = rd64(bytes + 144); s->total = rd64(bytes + 152);
     const orc_params *p = &s->p;
     s->p.chroma = bytes[49];
-    if (rd16(bytes + 6) != ORC_HEADER_BYTES || nch != 3 || bytes[48] != 1 || bytes[49] > 1 || bytes[50] != 0 ||
+    s->p.subpel = bytes[55];
+    if (rd16(bytes + 6) != ORC_HEADER_BYTES || nch != 3 || bytes[48] != 1 || bytes[49] > 1 || bytes[50] != 0 || bytes[55] > 1 ||
         p->U < 1 || p->V < 1 || p->Ws < 1 || p->Ht < 1 || p->height < 1 || p->height > ORC_MAX_LEVELS || p->block < 1 ||
         p->block > 8 || p->window < 0 || p->window > 64 || orc__geom(p, &s->g) != ORC_OK) {
         free(s); *err = ORC_E_PARAM; return NULL;
@@ -237,7 +239,7 @@ orc_stream *orc_open(const uint8_t *bytes, size_t len, int *err)
         s->total < s->off_mv) {
         free(s); *err = ORC_E_CORRUPT; return NULL;
     }
-    s->mvN = 2u * (uint32_t)(2 * p->window + 1) * (uint32_t)(2 * p->window + 1);
+    s->mvN = 2u * (uint32_t)(2 * orc_mv_off(p) + 1) * (uint32_t)(2 * orc_mv_off(p) + 1);
     s->len = (size_t)s->total;
     s->bytes = (uint8_t *)malloc(s->len);
     s->dir = (orc_dirent *)calloc((size_t)n_pc, sizeof(orc_dirent));

@@ -62,10 +62,9 @@ static int stored_value(const orc_tree *t, int c, int L, int pu, int pv, int x, 
     if (!orc_is_predictive(pu, pv)) return v;
     const orc_block *bk = t->blk[c][L] + (size_t)(pv * UL + pu) * t->g.nblk[c] + (y / B) * t->g.nbx[c] + (x / B);
     if (bk->flags & 2) {
-        int rx = x + bk->dx, ry = y + bk->dy;
-        int r = 0;
-        if (rx >= 0 && rx < Wc && ry >= 0 && ry < Hc)
-            r = t->srv[c][L][(pv & ~1) * UL + (pu & ~1)][(size_t)ry * Wc + rx];
+        const orc_plane_src src = {t->srv[c][L][(pv & ~1) * UL + (pu & ~1)], Wc, Hc};
+        const int r = t->p.subpel ? orc_halfpel(orc_plane_at, &src, 2 * x + bk->dx, 2 * y + bk->dy)  /* R28: offsets in half pixels */
+                                  : orc_plane_at(&src, x + bk->dx, y + bk->dy);
         v = bk->mode ? v + r : v - r;
     }
     return v;
@@ -160,8 +159,9 @@ int orc_tree_reconstruct(const orc_tree *t, uint8_t *lf_out)
                                         const orc_block *b = bk + (y / B) * nbx + (x / B);
                                         s = (b->flags & 1) ? stored_value(t, c, L, pu, pv, x, y) : 0;
                                         if (b->flags & 2) {
-                                            int rx = x + b->dx, ry = y + b->dy, q = 0;
-                                            if (rx >= 0 && rx < Ws && ry >= 0 && ry < Ht) q = Rp[(size_t)ry * Ws + rx];
+                                            const orc_plane_src src = {Rp, Ws, Ht};
+                                            const int q = t->p.subpel ? orc_halfpel(orc_plane_at, &src, 2 * x + b->dx, 2 * y + b->dy)
+                                                                      : orc_plane_at(&src, x + b->dx, y + b->dy);
                                             s += b->mode ? -q : q;
                                         }
                                     }
