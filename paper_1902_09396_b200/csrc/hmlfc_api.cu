@@ -232,7 +232,7 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
 {
     if (!h || n < 0 || (n > 0 && (!d_coords || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->decode_variant == 1 || h->ds.cs)  // chroma-subsampled streams (R18): the per-sample kernels read them
+    if (h->decode_variant == 1 || h->ds.cs || h->ds.sp)  // chroma-subsampled and half-pel streams (R18, R28): the per-sample kernels read them
         CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl,
@@ -246,7 +246,7 @@ int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_
     if (!h || n_views < 0 || (n_views > 0 && (!d_views || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
     // B = 4 streams: one lane per block-row segment; other block sizes (and decode variant 1 / 2, for cross-checks): one lane per pixel
-    if (h->ds.cs)
+    if (h->ds.cs || h->ds.sp)
         CU(h, launch_decode_dense(h->ds, d_views, n_views, false, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_rows(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
@@ -260,7 +260,7 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
 {
     if (!h || n_blocks < 0 || (n_blocks > 0 && (!d_blocks || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->ds.cs)
+    if (h->ds.cs || h->ds.sp)
         CU(h, launch_decode_dense(h->ds, d_blocks, n_blocks, true, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_block_rows(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
@@ -282,7 +282,7 @@ static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_ca
     // progressive decoding (lmin > 0) is implemented by the thread-per-pixel kernel and the two fused kernels for 4 x 4 blocks
     const int rv = h->render_variant;
     const bool fused_ok = D.B == 4 && (rv == 0 || (rv >= 6 && rv <= 15));
-    if (rv == 1 || D.cs || (D.lmin > 0 && !fused_ok))
+    if (rv == 1 || D.cs || D.sp || (D.lmin > 0 && !fused_ok))
         CU(h, launch_render_pixel(D, cams, n_views, W, H, d_out, st, &nl));
     else if (rv == 4 || rv == 5 || D.B != 4)
         CU(h, launch_render_warp(D, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
@@ -477,7 +477,7 @@ static int footprint_common(hmlfc_handle *h, const hmlfc_camera *d_cameras, int 
                             int64_t n, hmlfc_footprint_t *out)
 {
     const DevStream &D = h->ds;
-    if (D.cs) return HMLFC_E_UNSUPPORTED;  // the counting kernels (a measurement aid) assume one block grid for the three channels
+    if (D.cs || D.sp) return HMLFC_E_UNSUPPORTED;  // the counting kernels (a measurement aid) assume one block grid for the three channels and one reference sample per tap
     const size_t blk_words = ((size_t)h->n_pc * (size_t)D.nblk + 31) / 32 + 1;
     const size_t rkv_words = ((size_t)D.UH * D.VH * D.Ht * D.Ws + 31) / 32 + 1;
     FootprintMarks mk{nullptr, nullptr};

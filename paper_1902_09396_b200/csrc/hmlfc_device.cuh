@@ -43,6 +43,9 @@ struct DevStream {
     // their block grid is nbx_c x nby_c.  cs = 0: the chroma fields repeat the luma ones.  (The top-level RKVs are stored at full
     // resolution on the device either way: hmlfc_load replicates subsampled chroma.)
     int32_t cs, nbx_c, nby_c, nblk_c;
+    // half-pel motion compensation (R28): sp = 1: motion offsets count half pixels; mv_off = the largest offset
+    // (W, or 2W), nd = 2 mv_off + 1
+    int32_t sp, mv_off;
     uint32_t nd, nd2, nd_magic;       // 2W+1, (2W+1)^2, ceil(2^32 / nd)
     uint32_t mv_layout, mv_m;         // BISE layout of the motion records, N = 2 (2W+1)^2
     int32_t lmin;                     // progressive decoding (R26): levels below lmin are not summed; 0 = full quality
@@ -243,14 +246,29 @@ HMLFC_DEV uint32_t brec_window_field(const BrecWindow &q, uint32_t pos, uint32_t
     return funnel_r(lo, hi, pos & 31u) & ((1u << w) - 1u);
 }
 
-// motion record r = mode*nd^2 + (dy+W)*nd + (dx+W)  (R16)
+// reference value at the half-pel position (x2 / 2, y2 / 2) (R28): the mean of the 1, 2 or 4 stored reference samples around
+// it, rounded half up (arithmetic shifts = floor), each sample 0 outside the image or in an insignificant block
+HMLFC_DEV int reference_halfpel(const DevStream &S, uint4 d, int x2, int y2, int Wc, int Hc, int nbx)
+{
+    const int x0 = x2 >> 1, y0 = y2 >> 1, fx = x2 & 1, fy = y2 & 1;
+    int s = reference_value(S, d, x0, y0, Wc, Hc, nbx);
+    if (fx) s += reference_value(S, d, x0 + 1, y0, Wc, Hc, nbx);
+    if (fy) {
+        s += reference_value(S, d, x0, y0 + 1, Wc, Hc, nbx);
+        if (fx) s += reference_value(S, d, x0 + 1, y0 + 1, Wc, Hc, nbx);
+    }
+    const int k = fx + fy;  // log2 of the number of samples; the rounding term n / 2 = 0, 1, 2 = k
+    return (s + k) >> k;
+}
+
+// motion record r = mode*nd^2 + (dy+off)*nd + (dx+off), off = mv_off  (R16, R28)
 HMLFC_DEV void mv_unpack(const DevStream &S, uint32_t r, int &mode, int &dx, int &dy)
 {
     mode = r >= S.nd2;
     uint32_t rem = r - (mode ? S.nd2 : 0u);
     uint32_t q = umulhi(rem, S.nd_magic);  // exact floor(rem / nd) for rem < 2^16
-    dy = (int)q - S.W;
-    dx = (int)(rem - q * S.nd) - S.W;
+    dy = (int)q - S.mv_off;
+    dx = (int)(rem - q * S.nd) - S.mv_off;
 }
 
 // (Y, Co, Cg) of light-field sample (u,v,s=x,t=y); coordinates must be in range
@@ -284,8 +302,11 @@ HMLFC_DEV void decode_ycocg(const DevStream &S, int u, int v, int x, int y, int 
                 uint32_t rec = bise_decode_at(S.mv + d.z, mi, S.mv_layout, S.mv_m);
                 int mode, dx, dy;
                 mv_unpack(S, rec, mode, dx, dy);
-                int q = c > 0 ? reference_value(S, ldg(S.pc + rbase + c), xc + dx, yc + dy, S.Ws >> S.cs, S.Ht >> S.cs, S.nbx_c)
-                              : reference_value(S, ldg(S.pc + rbase + c), x + dx, y + dy, S.Ws, S.Ht, S.nbx);
+                const uint4 rd = ldg(S.pc + rbase + c);
+                const int px = c > 0 ? xc : x, py = c > 0 ? yc : y;
+                const int Wc = c > 0 ? (S.Ws >> S.cs) : S.Ws, Hc = c > 0 ? (S.Ht >> S.cs) : S.Ht, nbxc = c > 0 ? S.nbx_c : S.nbx;
+                const int q = S.sp ? reference_halfpel(S, rd, 2 * px + dx, 2 * py + dy, Wc, Hc, nbxc)
+                                   : reference_value(S, rd, px + dx, py + dy, Wc, Hc, nbxc);
                 e += mode ? -q : q;  // R10: subtractive P = e + R, additive P = e - R
             }
             acc[c] += e;

@@ -83,7 +83,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     I.height = (int32_t)rd32(s + 24); I.block = (int32_t)rd32(s + 28); I.window = (int32_t)rd32(s + 32);
     const uint32_t n_channels = rd32(s + 36);
     I.tau_ref = (int32_t)rd32(s + 40); I.tau_res = (int32_t)rd32(s + 44);
-    const uint8_t colour_id = s[48], chroma = s[49], rkv_codec = s[50];
+    const uint8_t colour_id = s[48], chroma = s[49], rkv_codec = s[50], subpel = s[55];
     I.background[0] = s[52]; I.background[1] = s[53]; I.background[2] = s[54];
     I.uv_origin[0] = rdf(s + 56); I.uv_origin[1] = rdf(s + 60); I.uv_step[0] = rdf(s + 64); I.uv_step[1] = rdf(s + 68);
     I.st_origin[0] = rdf(s + 72); I.st_origin[1] = rdf(s + 76); I.st_step[0] = rdf(s + 80); I.st_step[1] = rdf(s + 84);
@@ -94,7 +94,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
 
     if (rd16(s + 6) != kHeaderBytes) return HMLFC_E_CORRUPT;
     if (I.U < 1 || I.V < 1 || I.Ws < 1 || I.Ht < 1 || I.height < 1 || I.window < 0) return HMLFC_E_CORRUPT;
-    if (n_channels != 3 || colour_id != 1 || chroma > 1 || rkv_codec != 0) return HMLFC_E_UNSUPPORTED;
+    if (n_channels != 3 || colour_id != 1 || chroma > 1 || rkv_codec != 0 || subpel > 1) return HMLFC_E_UNSUPPORTED;
     if (I.height > kMaxLevels || I.window > 64) return HMLFC_E_UNSUPPORTED;
     if (!(I.block == 2 || I.block == 4 || I.block == 8) || (I.Ws % I.block) || (I.Ht % I.block)) return HMLFC_E_UNSUPPORTED;
     // chroma subsampling (R18): Co / Cg planes at Ws/2 x Ht/2, which the blocks must tile as well
@@ -109,7 +109,10 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
     D.nbx = I.Ws / I.block; D.nby = I.Ht / I.block; D.nblk = D.nbx * D.nby; D.fgroups = (D.nblk + 31) / 32;
     D.cs = chroma ? 1 : 0;
     D.nbx_c = (I.Ws >> D.cs) / I.block; D.nby_c = (I.Ht >> D.cs) / I.block; D.nblk_c = D.nbx_c * D.nby_c;
-    D.nd = 2u * I.window + 1u; D.nd2 = D.nd * D.nd;
+    // half-pel motion compensation (R28): offsets in half pixels, range [-2W, 2W]
+    D.sp = subpel ? 1 : 0;
+    D.mv_off = (subpel ? 2 : 1) * I.window;
+    D.nd = 2u * (uint32_t)D.mv_off + 1u; D.nd2 = D.nd * D.nd;
     D.nd_magic = D.nd == 1 ? 0xFFFFFFFFu : (uint32_t)((0x100000000ull + D.nd - 1) / D.nd);
     bise_layout(2u * D.nd2, &D.mv_layout, &D.mv_m);
     D.mv_w = D.mv_m + (D.mv_layout == 0 ? 0u : D.mv_layout == 1 ? 2u : 3u);
@@ -156,7 +159,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
         T.bits15.resize(n_pc);
         T.flagrec.assign((n_pc / 3) * (uint64_t)D.fgroups * 4, make_uint4(0u, 0u, 0u, 0u));  // 64-byte slot per (plane, group): Y, Co, Cg, bit words of Y and Co
         T.rkv.resize(n_top * npx);
-        if (!D.cs) {
+        if (!D.cs && !D.sp) {
             T.pb.assign(n_pc / 3, make_uint4(0u, 0u, 0u, 0u));
             T.bslot.assign((n_pc / 3) * (uint64_t)D.fgroups * 2, make_uint4(0u, 0u, 0u, 0u));
         }
@@ -214,7 +217,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                     }
                     if (rr != n_res || rp != n_pred) return HMLFC_E_CORRUPT;
                     T.n_flagged += (uint64_t)rr + (uint64_t)rp;
-                    if (!D.cs) {
+                    if (!T.pb.empty()) {
                         // block records (hmlfc_device.cuh): field widths and offsets of the plane's channels; .x counts the plane's bits
                         // until the prefix sum below turns it into the plane's first word
                         uint4 &pb = T.pb[k / 3];
@@ -227,7 +230,7 @@ inline int build_tables(const void *h_stream_bytes, size_t len, HostTables &T)
                         pb.x = (uint32_t)bits;
                     }
                 }
-    if (!D.cs) {
+    if (!T.pb.empty()) {
         // slots: the six bit words of every group and the position of the group's first record in its plane
         for (uint64_t p = 0; p < n_pc / 3; ++p) {
             const uint4 pb = T.pb[p];

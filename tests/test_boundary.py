@@ -56,6 +56,10 @@ def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
     bad_version[4] = 9
     chroma = bytearray(data)
     chroma[49] = 2       # 0 = off, 1 = Co / Cg at half resolution (R18); anything else is not a layout this library reads
+    subpel = bytearray(data)
+    subpel[55] = 2       # 0 = whole-pixel motion offsets, 1 = half pixels (R28)
+    subpel_flip = bytearray(data)
+    subpel_flip[55] = 1  # an integer-pel stream that claims half-pel offsets: the motion strings no longer have the directory's sizes
     chroma_flip = bytearray(data)
     chroma_flip[49] = 1  # a full-resolution stream that claims subsampled chroma: its directory no longer matches its flag maps
     bad_block = bytearray(data)
@@ -70,7 +74,7 @@ def test_load_rejects_malformed_streams_with_distinct_codes(P, enc):
         w[off_dir + 48 + field:off_dir + 48 + field + 8] = value.to_bytes(8, "little")   # second entry: a plane-channel with blocks
         wraps.append((w, -6))
     cases = [(bad_magic, -1), (data[:6], -2), (data[:100], -2), (data[:len(data) // 2], -2), (bad_version, -3),
-             (chroma, -5), (chroma_flip, -6), (bad_block, -5), (bad_dir, -6)] + wraps
+             (chroma, -5), (chroma_flip, -6), (subpel, -5), (subpel_flip, -6), (bad_block, -5), (bad_dir, -6)] + wraps
     for blob, code in cases:
         rc, out = load(blob)
         assert rc == code and not out.value, (rc, code)
