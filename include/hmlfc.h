@@ -38,7 +38,8 @@ enum {
                                /* subsampling set, RKV codec != raw, height > 8              */
     HMLFC_E_CORRUPT = -6,      /* directory inconsistent with the section sizes              */
     HMLFC_E_NOMEM = -7,        /* host or device allocation failed                           */
-    HMLFC_E_CUDA = -8          /* a CUDA runtime call failed (see hmlfc_last_cuda_error)     */
+    HMLFC_E_CUDA = -8,         /* a CUDA runtime call failed (see hmlfc_last_cuda_error)     */
+    HMLFC_E_LIMIT = -9         /* the request exceeds a fixed capacity (hmlfc_render_noalloc) */
 };
 
 typedef struct hmlfc_handle hmlfc_handle; /* opaque; owns every device allocation */
@@ -132,6 +133,21 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
  *   d_out     : device, uint8 [n_views][H][W][3], row-major, no padding.                    */
 int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
                  void *cuda_stream);
+
+/* hmlfc_render_noalloc -- hmlfc_render for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same views, byte for byte, from the tile kernels (tile_tables_kernel + render_tiles_kernel)
+ * with the tile tables -- the scratch memory hmlfc_render takes from a stream-ordered pool -- in a static device buffer of the library.
+ * The call launches two kernels on cuda_stream and calls no cudaMalloc, cudaFree or other allocating routine.
+ *   Limit: n_views x ceil(W / w) x ceil(H / 32) <= HMLFC_NOALLOC_MAX_TILES tiles per call (w = 64 where W x H >= 8 x Ws x Ht, else 32),
+ *   e.g. 16 views of 512 x 512; beyond it HMLFC_E_LIMIT and nothing is launched -- render the views in several calls.  The buffer
+ *   (HMLFC_NOALLOC_MAX_TILES x 3,200 bytes = 13.1 MB) is held by every GPU that loads the library until the process exits.
+ *   Streams: 4 x 4 blocks, full-resolution chroma, whole-pixel motion (the streams whose hmlfc_render uses scratch memory at all);
+ *   others HMLFC_E_UNSUPPORTED.  The current device must be the handle's (hmlfc_load sets the buffer up for its device).
+ *   All calls on a device share the buffer: calls that may OVERLAP on the GPU (different streams without a dependency) race on it
+ *   and give undefined pixels; calls on one stream, or ordered by events, are safe.  Progressive decoding applies. */
+#define HMLFC_NOALLOC_MAX_TILES 4096
+int hmlfc_render_noalloc(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                         void *cuda_stream);
 
 /* hmlfc_render_lod -- level of detail per view ("progressive decoding"; R26, R27): view k is rendered as by
  * hmlfc_render with the tree walk stopped above level max(h_levels[k], the handle's min_level), i.e. from the representative key views of

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libhmlfc_b200.so")
 
 # every symbol include/hmlfc.h declares
 EXPORTS = (
-    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_decode_blocks", "hmlfc_render", "hmlfc_render_lod", "hmlfc_lod_levels", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
+    "hmlfc_load", "hmlfc_info", "hmlfc_decode", "hmlfc_decode_views", "hmlfc_decode_blocks", "hmlfc_render", "hmlfc_render_noalloc", "hmlfc_render_lod", "hmlfc_lod_levels", "hmlfc_decode_host", "hmlfc_decode_views_host", "hmlfc_render_host",
     "hmlfc_last_oob_count", "hmlfc_footprint_render", "hmlfc_footprint_decode", "hmlfc_set_render_variant", "hmlfc_set_decode_variant", "hmlfc_search", "hmlfc_hierarchy", "hmlfc_hierarchy_sizes", "hmlfc_set_min_level", "hmlfc_encode", "hmlfc_encode_psnr", "hmlfc_stream_free", "hmlfc_encode_release_scratch",
     "hmlfc_launch_count", "hmlfc_free", "hmlfc_strerror", "hmlfc_last_cuda_error",
 )
@@ -75,6 +75,7 @@ def lib():
     L.hmlfc_decode_views.argtypes, L.hmlfc_decode_views.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_decode_blocks.argtypes, L.hmlfc_decode_blocks.restype = [vp, vp, i64, vp, vp], C.c_int
     L.hmlfc_render.argtypes, L.hmlfc_render.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
+    L.hmlfc_render_noalloc.argtypes, L.hmlfc_render_noalloc.restype = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
     L.hmlfc_render_lod.argtypes, L.hmlfc_render_lod.restype = [vp, vp, vp, C.c_int, C.c_int, C.c_int, vp, vp], C.c_int
     L.hmlfc_lod_levels.argtypes, L.hmlfc_lod_levels.restype = [vp, vp, C.c_int, C.c_float, vp], C.c_int
     L.hmlfc_decode_host.argtypes, L.hmlfc_decode_host.restype = [vp, vp, i64, vp], C.c_int
@@ -208,6 +209,21 @@ def hmlfc_render(h: Handle, cameras, W: int, H: int, out=None, stream=None):
     assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * H * W * 3
     _check(lib().hmlfc_render(h._h, C.c_void_p(cameras.data_ptr()), n, W, H, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
            "hmlfc_render", h._h)
+    return out
+
+
+NOALLOC_MAX_TILES = 4096   # include/hmlfc.h: HMLFC_NOALLOC_MAX_TILES
+
+
+def hmlfc_render_noalloc(h: Handle, cameras, W: int, H: int, out, stream=None):
+    """hmlfc_render with the tile tables in the library's static device buffer: the call allocates nothing (the caller passes `out`).
+    At most NOALLOC_MAX_TILES tiles per call (HmlfcError -9 beyond); calls that overlap on the GPU race on the buffer."""
+    torch = _require_cuda()
+    assert cameras.is_cuda and cameras.dtype == torch.float32 and cameras.is_contiguous() and cameras.shape[-1] == 16
+    n = cameras.numel() // 16
+    assert out.is_cuda and out.dtype == torch.uint8 and out.is_contiguous() and out.numel() == n * H * W * 3
+    _check(lib().hmlfc_render_noalloc(h._h, C.c_void_p(cameras.data_ptr()), n, W, H, C.c_void_p(out.data_ptr()), _stream_ptr(stream)),
+           "hmlfc_render_noalloc", h._h)
     return out
 
 

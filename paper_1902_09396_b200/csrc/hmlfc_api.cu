@@ -150,6 +150,7 @@ const char *hmlfc_strerror(int code)
     case HMLFC_E_CORRUPT: return "corrupt stream directory";
     case HMLFC_E_NOMEM: return "out of memory";
     case HMLFC_E_CUDA: return "CUDA runtime error";
+    case HMLFC_E_LIMIT: return "request exceeds a fixed capacity of this entry point";
     default: return "unknown error";
     }
 }
@@ -184,7 +185,8 @@ int hmlfc_load(const void *h_stream_bytes, size_t len, hmlfc_handle **out)
         (ce = cudaStreamCreateWithFlags(&h->out_stream, cudaStreamNonBlocking)) != cudaSuccess ||
         (ce = create_events(h)) != cudaSuccess ||
         (ce = configure_render_warp()) != cudaSuccess || (ce = configure_render_cta()) != cudaSuccess ||
-        (ce = configure_render_tiles()) != cudaSuccess || (ce = configure_decode_queue()) != cudaSuccess) {
+        (ce = configure_render_tiles()) != cudaSuccess || (ce = configure_decode_queue()) != cudaSuccess ||
+        (ce = configure_render_tiles_noalloc()) != cudaSuccess) {
         const int code = (ce == cudaErrorMemoryAllocation) ? HMLFC_E_NOMEM : HMLFC_E_CUDA;
         release(h);
         return code;
@@ -317,6 +319,23 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
 {
     if (!h) return HMLFC_E_INVALID;
     return render_impl(h, h->ds, d_cameras, n_views, W, H, d_out, cuda_stream);
+}
+
+int hmlfc_render_noalloc(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_views, int W, int H, uint8_t *d_out,
+                         void *cuda_stream)
+{
+    if (!h || n_views < 0 || W <= 0 || H <= 0 || n_views > 65535 || (n_views > 0 && (!d_cameras || !d_out))) return HMLFC_E_INVALID;
+    const DevStream &D = h->ds;
+    if (D.B != 4 || D.cs || D.sp) return HMLFC_E_UNSUPPORTED;  // streams whose render path has no scratch memory to begin with
+    int nl = 0;
+    bool too_large = false;
+    // tile shape as the automatic choice of hmlfc_render makes it where it takes the tile kernels
+    const int config = (long long)W * H >= 8LL * D.Ws * D.Ht ? 4 : 0;
+    CU(h, launch_render_tiles_noalloc(D, reinterpret_cast<const Camera *>(d_cameras), n_views, W, H, d_out,
+                                      static_cast<cudaStream_t>(cuda_stream), &nl, config, &too_large));
+    if (too_large) return HMLFC_E_LIMIT;
+    h->launches += nl;
+    return HMLFC_OK;
 }
 
 int hmlfc_render_lod(const hmlfc_handle *h, const hmlfc_camera *d_cameras, const int32_t *h_levels, int n_views, int W, int H,

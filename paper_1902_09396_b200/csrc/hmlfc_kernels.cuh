@@ -64,6 +64,11 @@ size_t render_tiles_scratch_bytes(int n_views, int W, int H);
 cudaError_t launch_repack(const DevStream &S, uint64_t n_planes, uint32_t *d_brec, cudaStream_t st);
 cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, void *d_scratch,
                                 cudaStream_t st, int *n_launches, int config);
+// the same with the tables in the library's static device buffer (hmlfc_render_noalloc; at most HMLFC_NOALLOC_MAX_TILES tiles per call):
+// set-up once per device (by hmlfc_load), then launches that allocate nothing
+cudaError_t configure_render_tiles_noalloc();
+cudaError_t launch_render_tiles_noalloc(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
+                                        int *n_launches, int config, bool *too_large);
 cudaError_t configure_render_tiles();
 cudaError_t configure_render_cta();
 cudaError_t launch_footprint_render(const DevStream &S, const Camera *d_cams, int n_views, int W, int H,

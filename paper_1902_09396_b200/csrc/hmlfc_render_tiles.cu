@@ -20,6 +20,9 @@
 // rendered by 16 direct sample decodes -- the result is the definition's in every case.  A tile whose tables do not fit the arena takes the
 // general path (quadtree of sub-tile passes) in the same CTA.
 #include "hmlfc_render_common.cuh"
+#include "../../include/hmlfc.h"  // HMLFC_NOALLOC_MAX_TILES
+
+#include <mutex>
 
 namespace hmlfc {
 
@@ -346,5 +349,56 @@ cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_
     if (n_launches) *n_launches += 2;
     return cudaSuccess;
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// hmlfc_render_noalloc: the tile path with its tables in a buffer that exists from the moment the library is loaded, for callers that
+// cannot allocate (CUDA graph capture, tight serving loops).  The buffer is a file-scope __device__ array: every GPU that loads the
+// library holds its kNoAllocMaxTiles x 3,200 bytes (13.1 MB) until the process exits.  In host code the array's NAME is a host-side
+// stand-in, not a device address; the device address comes from cudaGetSymbolAddress, asked for once per device at set-up
+// (configure_render_tiles_noalloc, called by hmlfc_load with its device current) and passed to the kernels.
+// Every call on a device shares the array.  Nothing in it has to start at zero (tile_tables_kernel writes every word the render kernel
+// reads: the header of every tile, the slot words the header counts), so a call leaves the previous call's contents to be overwritten;
+// two calls that overlap on the GPU (different streams, no dependency) RACE on it.
+constexpr int kNoAllocMaxTiles = HMLFC_NOALLOC_MAX_TILES;
+constexpr int kNoAllocMaxDevices = 64;
+static __device__ __align__(256) unsigned char g_noalloc_tables[(size_t)kNoAllocMaxTiles * sizeof(TileTables)];
+static void *g_noalloc_ptr[kNoAllocMaxDevices];  // device address of g_noalloc_tables on device i (null: not set up there)
+static std::mutex g_noalloc_mutex;
+
+cudaError_t configure_render_tiles_noalloc()
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return cudaSuccess;  // the entry point will say that this device was not set up
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (g_noalloc_ptr[dev]) return cudaSuccess;
+    void *ptr = nullptr;
+    if ((e = cudaGetSymbolAddress(&ptr, g_noalloc_tables)) != cudaSuccess) return e;
+    g_noalloc_ptr[dev] = ptr;
+    return cudaSuccess;
+}
+
+// *too_large: the batch has more tiles than the buffer holds (nothing was launched).  Calls no allocating routine.
+cudaError_t launch_render_tiles_noalloc(const DevStream &S, const Camera *d_cams, int n_views, int W, int H, uint8_t *d_out, cudaStream_t st,
+                                        int *n_launches, int config, bool *too_large)
+{
+    *too_large = false;
+    if (n_views == 0) return cudaSuccess;
+    const int tile_w = config >= 2 ? 64 : 32;
+    const long long n_tiles = (long long)n_views * ((W + tile_w - 1) / tile_w) * ((H + kTile - 1) / kTile);
+    if (n_tiles > kNoAllocMaxTiles) { *too_large = true; return cudaSuccess; }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    void *ptr = nullptr;
+    if (dev >= 0 && dev < kNoAllocMaxDevices) {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        ptr = g_noalloc_ptr[dev];
+    }
+    if (!ptr) return cudaErrorInvalidDevice;  // no hmlfc_load ran with this device current
+    return launch_render_tiles(S, d_cams, n_views, W, H, d_out, ptr, st, n_launches, config);
+}
+
 
 }  // namespace hmlfc
