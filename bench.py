@@ -520,7 +520,7 @@ def run_ours(args, cfg_name):
             "value": dec_px_per_s, "unit": "LF pixels/s", "n": n_dec, "ms_per_launch": dec_kernel_ms,
             "e2e": {"value": whole_job_rate(n_dec, 3, world, dec_e2e_s), "unit": "LF pixels/s", "h2d_bytes_per_step": 16 * n_dec,
                     "d2h_bytes_per_step": 3 * n_dec, "steps": 3},
-            "roofline": {"bound": "hbm", "kernel": "decode_kernel" if args.decode_variant == 1 else "decode_queue_kernel", "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": {1: "decode_kernel", 2: "decode_queue_kernel", 3: "decode_queue_kernel"}.get(args.decode_variant, "decode_brec_kernel"), "achieved": dec_achieved, "peak": peak, "unit": "GB/s",
                          "frac": dec_achieved / peak, "bytes_alg_per_launch": fpd["bytes_alg"],
                          "traffic": cap_d.get("dram_bytes"),
                          "traffic_source": {"file": "profiles/traffic.json", "commit": cap_d.get("commit"), "captured_with": cap_d.get("captured_with"),
