@@ -278,6 +278,61 @@ def measure_other_config(P, name, steps, peak, flush, stream):
     return res
 
 
+def measure_extra_stream(P, cfg_name, kind, tau_res, steps, flush, stream):
+    """The rows of SURVEY 8(f) that have an oracle and a correct (per-sample) CUDA path but no fast one: a chroma-subsampled (R18) or a
+    half-pel motion-compensated (R28) stream of the headline configuration's light field, encoded by the ORACLE (hmlfc_encode does
+    neither) at the headline stream's threshold; the same timed legs, and a parity spot check against the oracle."""
+    import torch
+
+    import oracle as orc
+    import workloads as wl
+
+    cfg = wl.CONFIGS[cfg_name]
+    lf = wl.light_field(cfg)
+    window = min(cfg.window, 4) if kind == "halfpel" else cfg.window  # the oracle's half-pel search is exhaustive over (4W + 1)^2 interpolated candidates
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, window, tau_res // 2, tau_res, geometry=wl.geometry(cfg),
+                        seed=cfg.seed, chroma=1 if kind == "chroma" else 0, subpel=1 if kind == "halfpel" else 0)
+    t0 = time.perf_counter()
+    tree = orc.Tree(lf, p)
+    data = tree.serialize()
+    tree.close()
+    t_enc = time.perf_counter() - t0
+    s = orc.Stream(data)
+    h = P.hmlfc_load(data)
+    W, H, V = cfg.out_w, cfg.out_h, cfg.n_views
+    cams_np = wl.camera_path(cfg)
+    cams = torch.from_numpy(cams_np).cuda()
+    out = torch.empty((V, H, W, 3), dtype=torch.uint8, device="cuda")
+    ms = _timed_single(lambda: P.hmlfc_render(h, cams, W, H, out=out, stream=stream), steps, 2, flush, stream)
+    n = min(cfg.n_decode, 2_000_000)
+    coords_np = wl.random_coords(cfg, n)
+    coords = torch.from_numpy(coords_np).cuda()
+    dec_out = torch.empty((n, 3), dtype=torch.uint8, device="cuda")
+    dms = _timed_single(lambda: P.hmlfc_decode(h, coords, out=dec_out, stream=stream), steps, 2, flush, stream)
+    views = torch.from_numpy(np.array([(u, v) for v in range(cfg.V) for u in range(cfg.U)], dtype=np.int32)).cuda()
+    vms = _timed_single(lambda: P.hmlfc_decode_views(h, views, stream=stream), max(2, steps // 2), 1, flush, stream)
+    # parity: sampled coordinates bit-exact, one rendered view within 1 LSB
+    k = 20_000
+    exact = bool(np.array_equal(dec_out[:k].cpu().numpy(), s.decode(coords_np[:k])))
+    ref = s.render(cams_np[:1], W, H)
+    d = np.abs(out[:1].cpu().numpy().astype(np.int16) - ref.astype(np.int16))
+    res = {
+        "workload": f"{cfg.name} light field, oracle-encoded with {'Co / Cg at half resolution' if kind == 'chroma' else 'half-pel motion offsets'}, "
+                    f"tau_res = {tau_res}, window {window}; render {V} views of {W}x{H}; decode {n} random coordinates; decode all {cfg.U * cfg.V} views",
+        "kernels": "render_pixel_kernel, decode_kernel, decode_dense_kernel (the per-sample definition: correct, no fast path yet)",
+        "stream_bytes": len(data), "stream_bpp": round(8.0 * len(data) / (cfg.U * cfg.V * cfg.Ws * cfg.Ht), 4),
+        "psnr_db": round(float(orc.psnr(lf, s.decode_full())), 3), "oracle_encode_s": round(t_enc, 1),
+        "render_ms_per_step": float(np.mean(ms)), "views_per_s": V / (float(np.mean(ms)) * 1e-3),
+        "decode": {"value": n / (float(np.mean(dms)) * 1e-3), "unit": "LF pixels/s", "n": n},
+        "decode_views": {"value": cfg.U * cfg.V * cfg.Ws * cfg.Ht / (float(np.mean(vms)) * 1e-3), "unit": "LF pixels/s"},
+        "parity": {"decode_bit_exact_on_sample": exact, "render_max_abs_diff": int(d.max()), "render_frac_diff": float((d > 0).mean())},
+    }
+    P.hmlfc_free(h)
+    del coords, dec_out, out, cams, views
+    torch.cuda.empty_cache()
+    return res
+
+
 def _csrc_hash():
     """Hash of the CUDA sources the library is built from: profiles/traffic.json records it at capture time, so counters of an
     older build are recognised as stale."""
@@ -595,6 +650,12 @@ def run_ours(args, cfg_name):
             for name in [c for c in args.configs.split(",") if c and c != cfg.name]:
                 others[name] = measure_other_config(P, name, max(3, min(args.steps, 10)), peak, flush, stream)
 
+        extras = None
+        if world == 1 and args.extras and args.extras != "none":
+            # ---- optional (minutes of oracle encoding): the 8(f) rows that so far have only the per-sample CUDA path
+            extras = {kind: measure_extra_stream(P, cfg.name, kind, int(info["tau_res"]), max(3, min(args.steps, 5)), flush, stream)
+                      for kind in args.extras.split(",") if kind in ("chroma", "halfpel")}
+
         line = {
             "metric": "rendered_views_per_s", "value": views_per_s, "unit": "views/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -619,7 +680,7 @@ def run_ours(args, cfg_name):
             "decode_blocks": {"value": whole_job_rate(n_blk * cfg.block * cfg.block, len(blk_ms), world, blk_total * 1e-3), "unit": "LF pixels/s",
                               "blocks_per_launch": int(n_blk), "ms_per_launch": float(np.mean(blk_ms)),
                               "workload": f"hmlfc_decode_blocks: {n_blk} whole {cfg.block} x {cfg.block} blocks at seeded uniformly random (u, v, bx, by)"},
-            "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode, "configs": others,
+            "decode": decode, "search": search, "hierarchy": hierarchy, "encode": encode, "configs": others, "extras": extras,
             "output_px_per_s": views_per_s * W * H, "clocks": clocks,
             "device_bytes": int(h.info.device_bytes),
             "min_level": args.min_level,
@@ -676,6 +737,8 @@ def main():
     ap.add_argument("--min-level", type=int, default=0, help="progressive decoding: sum only the levels >= this one (0 = full quality)")
     ap.add_argument("--encode", action="store_true", help="run the GPU encoder leg also on configurations whose light field exceeds 256 MB")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--extras", default="none", help="comma list of chroma, halfpel: also measure an oracle-encoded chroma-subsampled / half-pel stream "
+                                                       "of the headline light field (per-sample kernels; adds minutes of CPU encoding; off by default)")
     ap.add_argument("--configs", default="cfg3,cfg4,cfg5", help="other BASELINE.json configurations measured after the headline (GPU-encoded "
                     "streams; N = 1 only); 'none' to skip")
     args = ap.parse_args()
