@@ -395,7 +395,7 @@ __device__ __forceinline__ bool tables_fit(const TileHeader &hd)
 // Phases B1-B4 for the tile whose tables are in ctl.tab (visible to all threads; they fit the arena): the float RGB patch of every
 // (view, sample) cell.  kZeroFrom: the first 16-byte word of the accumulator region this function still has to zero (the caller zeroed
 // the words before it and ctl.n_rec).  Returns false (CTA-uniform) when the record list does not fit; ends with a barrier either way.
-template <int kArenaBytes, int kNT>
+template <int kArenaBytes, int kNT, bool kSubpel = false>
 __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int zero_from)
 {
     const int tid = threadIdx.x, lane = tid & 31;
@@ -528,7 +528,10 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
         int md, dx, dy;
         mv_unpack(S, bise_at(S.mv + ctl.desc[s][c].z, r0.y, S.mv_layout, S.mv_m, ctl.lut), md, dx, dy);
         const uint4 dr = ctl.rdesc[s][c];
-        const int rx = (int)((r0.z >> 20) << 2) + dx, ry0 = (int)(((r0.z >> 8) & 0xFFFu) << 2) + dy;  // first reference sample of the block
+        // first reference sample of the block; kSubpel (R28): the offsets count half pixels, a reference value is the mean of the
+        // 1 / 2 / 4 samples from (rx, ry0) on, so a block reads one more column (fx) and one more row (fy)
+        const int fx = kSubpel ? (dx & 1) : 0, fy = kSubpel ? (dy & 1) : 0;
+        const int rx = (int)((r0.z >> 20) << 2) + (kSubpel ? (dx >> 1) : dx), ry0 = (int)(((r0.z >> 8) & 0xFFFu) << 2) + (kSubpel ? (dy >> 1) : dy);
         const int bxa = rx >> 2, bya = ry0 >> 2;  // arithmetic shifts: floor for positions left of / above the image
         uint32_t e[4];
 #pragma unroll
@@ -536,14 +539,14 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
             const int bx = bxa + (j & 1), by = bya + (j >> 1);
             e[j] = 0u;
             // needed at all: the second column only if the row straddles two blocks, the second block row likewise
-            if ((unsigned)bx < (unsigned)S.nbx && (unsigned)by < (unsigned)S.nby && (!(j & 1) || (rx & 3)) && (!(j >> 1) || (ry0 & 3))) {
+            if ((unsigned)bx < (unsigned)S.nbx && (unsigned)by < (unsigned)S.nby && (!(j & 1) || (rx & 3) || fx) && (!(j >> 1) || (ry0 & 3) || fy)) {
                 const int b = by * S.nbx + bx;
                 const uint2 fr = __ldg(reinterpret_cast<const uint2 *>(S.flagrec + dr.x + 4u * (uint32_t)(b >> 5)));  // {res bits, res rank}
                 const uint32_t bit = 1u << (b & 31);
                 if (fr.x & bit) e[j] = ((fr.y + popc(fr.x & (bit - 1u))) << 4) | 1u;
             }
         }
-        rec[2 * rr].y = ((uint32_t)md << 16) | ((uint32_t)(dx + S.W) << 8) | (uint32_t)(dy + S.W);
+        rec[2 * rr].y = ((uint32_t)md << 16) | ((uint32_t)(dx + S.mv_off) << 8) | (uint32_t)(dy + S.mv_off);  // (mv_off <= 127: the caller's condition)
         rec[2 * rr + 1] = make_uint4(e[0], e[1], e[2], e[3]);
     }
     __syncthreads();
@@ -566,26 +569,57 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
             if (r0.x != kNone) own = bise_row4(S.pay + d.y, r0.x + (uint32_t)(ky << 2), d.w, ctl.lut);
             int e0 = (int)(int16_t)(own.x & 0xFFFFu), e1 = (int)own.x >> 16, e2 = (int)(int16_t)(own.y & 0xFFFFu), e3 = (int)own.y >> 16;
             if (r0.y != kNone) {
-                const int md = (int)((r0.y >> 16) & 1u), dx = (int)((r0.y >> 8) & 0xFFu) - S.W, dy = (int)(r0.y & 0xFFu) - S.W;
-                const int rx = xx + dx, ry = yy + dy;
-                if ((unsigned)ry < (unsigned)S.Ht) {
-                    // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1: B2 looked them up
-                    const uint4 dr = ctl.rdesc[s][c];
-                    const uint4 re = rec[2 * rr + 1];
-                    const int o = rx & 3;
-                    const bool second_row = (ry >> 2) != ((yy0 + dy) >> 2);
-                    const uint32_t ea = second_row ? re.z : re.x, eb = second_row ? re.w : re.y;
-                    const uint32_t i0 = (uint32_t)((ry & 3) << 2);
-                    uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-                    if (ea & 1u) qa = bise_row4(S.pay + dr.y, (ea & ~15u) + i0, dr.w, ctl.lut);
-                    if (eb & 1u) qb = bise_row4(S.pay + dr.y, (eb & ~15u) + i0, dr.w, ctl.lut);
-                    // samples o .. o+3 of the 8-sample string qa | qb
-                    uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
-                    if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
-                    const uint32_t sh = (uint32_t)(o & 1) << 4;
-                    const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
-                    const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
-                    // R10: subtractive P = e + R, additive P = e - R
+                const int md = (int)((r0.y >> 16) & 1u), dx = (int)((r0.y >> 8) & 0xFFu) - S.mv_off, dy = (int)(r0.y & 0xFFu) - S.mv_off;
+                const uint4 dr = ctl.rdesc[s][c];
+                const uint4 re = rec[2 * rr + 1];
+                if (!kSubpel) {
+                    const int rx = xx + dx, ry = yy + dy;
+                    if ((unsigned)ry < (unsigned)S.Ht) {
+                        // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1: B2 looked them up
+                        const int o = rx & 3;
+                        const bool second_row = (ry >> 2) != ((yy0 + dy) >> 2);
+                        const uint32_t ea = second_row ? re.z : re.x, eb = second_row ? re.w : re.y;
+                        const uint32_t i0 = (uint32_t)((ry & 3) << 2);
+                        uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
+                        if (ea & 1u) qa = bise_row4(S.pay + dr.y, (ea & ~15u) + i0, dr.w, ctl.lut);
+                        if (eb & 1u) qb = bise_row4(S.pay + dr.y, (eb & ~15u) + i0, dr.w, ctl.lut);
+                        // samples o .. o+3 of the 8-sample string qa | qb
+                        uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
+                        if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
+                        const uint32_t sh = (uint32_t)(o & 1) << 4;
+                        const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
+                        const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
+                        // R10: subtractive P = e + R, additive P = e - R
+                        if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
+                        else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
+                    }
+                } else {
+                    // half-pel (R28): samples (rx .. rx+3+fx) of the rows ry and, if fy, ry + 1, summed and rounded half up; a row outside
+                    // the image and a sample in an insignificant block contribute 0 to the sum
+                    const int fx = dx & 1, fy = dy & 1;
+                    const int rx = xx + (dx >> 1), ry = yy + (dy >> 1), o = rx & 3, bya = (yy0 + (dy >> 1)) >> 2;
+                    int h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+#pragma unroll
+                    for (int jr = 0; jr < 2; ++jr) {
+                        const int r = ry + jr;
+                        if ((jr && !fy) || (unsigned)r >= (unsigned)S.Ht) continue;
+                        const bool second_row = (r >> 2) != bya;
+                        const uint32_t ea = second_row ? re.z : re.x, eb = second_row ? re.w : re.y;
+                        const uint32_t i0 = (uint32_t)((r & 3) << 2);
+                        uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
+                        if (ea & 1u) qa = bise_row4(S.pay + dr.y, (ea & ~15u) + i0, dr.w, ctl.lut);
+                        if (eb & 1u) qb = bise_row4(S.pay + dr.y, (eb & ~15u) + i0, dr.w, ctl.lut);
+                        // samples o .. o+4 of the 8-sample string qa | qb (o + 4 <= 7)
+                        uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
+                        if (o & 2) { w0 = w1; w1 = w2; w2 = w3; w3 = 0u; }
+                        const uint32_t sh = (uint32_t)(o & 1) << 4;
+                        const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh), q45 = __funnelshift_r(w2, w3, sh);
+                        const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
+                        const int q4 = (int)(int16_t)(q45 & 0xFFFFu);
+                        h0 += q0 + (fx ? q1 : 0); h1 += q1 + (fx ? q2 : 0); h2 += q2 + (fx ? q3 : 0); h3 += q3 + (fx ? q4 : 0);
+                    }
+                    const int k = fx + fy;  // log2 of the number of samples; the rounding term n / 2 = 0, 1, 2 = k
+                    const int q0 = (h0 + k) >> k, q1 = (h1 + k) >> k, q2 = (h2 + k) >> k, q3 = (h3 + k) >> k;
                     if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
                     else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
                 }
@@ -738,7 +772,7 @@ __device__ __forceinline__ void setup_rays(const DevStream &S, const Camera &cam
 // One pass over a (sub-)tile whose rays are set up: ranges (SV), tables (T), decode (decode_patch), gather + blend (C).
 // Returns true (CTA-uniform) when rgb[] holds the pass's pixels (background where the ray misses); false when the
 // tables do not fit the arena and the (sub-)tile must be split.
-template <int kArenaBytes, int kNT>
+template <int kArenaBytes, int kNT, bool kSubpel = false>
 __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, const PixTaps (&pt)[kPPL],
                                           uint32_t (&rgb)[kPPL])
 {
@@ -813,7 +847,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     PHASE_MARK(4);
     bool ok = tables_fit<kArenaBytes>(ctl.tab.hdr);
     if (!ok) PASS_STAT(10);
-    else ok = decode_patch<kArenaBytes, kNT>(S, ctl, arena, kSpecZero);
+    else ok = decode_patch<kArenaBytes, kNT, kSubpel>(S, ctl, arena, kSpecZero);
     reset_ctl(ctl);  // behind a barrier that followed every read of the ranges and of the record count
     if (!ok) return false;
 
@@ -832,7 +866,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
 // than output pixels under the tile), its four quadrants with one pixel per thread, each split again when it does not fit; a sub-tile of
 // the last level that still does not fit (strong minification) is rendered by 16 direct sample decodes per pixel.  ctl.cam, ctl.aff and
 // ctl.lut are set and visible, the accumulators of ctl are reset (reset_ctl).  path = child index (2 bits) of every level on the way down.
-template <int kArenaBytes, int kNT, int kTW>
+template <int kArenaBytes, int kNT, int kTW, bool kSubpel = false>
 __device__ __forceinline__ void render_tile_general(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int W, int H, uint8_t *__restrict__ out,
                                                     int out_aligned, int view, int tile_x, int tile_y)
 {
@@ -860,7 +894,7 @@ __device__ __forceinline__ void render_tile_general(const DevStream &S, Ctl &ctl
             setup_rays<kTW>(S, cam, W, H, sx, sy, full, lpw, npx, pt);
             PHASE_MARK(0);
             PASS_STAT(lvl);
-            done = tile_pass<kArenaBytes, kNT>(S, ctl, arena, pt, rgb);
+            done = tile_pass<kArenaBytes, kNT, kSubpel>(S, ctl, arena, pt, rgb);
             if (done) PASS_STAT(4 + lvl);
             if (!done && lvl == kLMax) {
                 PASS_STAT(13);

@@ -65,11 +65,25 @@ def test_halfpel_stream_decode_and_render(P, name, tau):
     assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy().reshape(-1, 3), s.decode(bc))
     cams = wl.camera_path(cfg)
     ref = s.render(cams, cfg.out_w, cfg.out_h)
-    for variant in (P.RENDER_AUTO, P.RENDER_TILES, P.RENDER_CTA, P.RENDER_WARP):   # likewise: the thread-per-pixel kernel
+    P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)
+    unshared = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
+    # 4 x 4 blocks: the tile kernel's half-pel instantiation (whatever fused variant is asked for); otherwise the thread-per-pixel kernel
+    for variant in (P.RENDER_AUTO, P.RENDER_TILES, P.RENDER_TILES_W256X3, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_WARP):
         P.hmlfc_set_render_variant(h, variant)
         out = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
         d = np.abs(out.astype(np.int16) - ref.astype(np.int16))
         assert d.max() <= 1 and (d > 0).mean() < 1e-3, (variant, int(d.max()))
+        assert np.array_equal(out, unshared), variant
+    # a magnified, rotated batch (several tiles per view, ragged edges) and every progressive level
+    cams2 = wl.camera_path(cfg, n_views=3, out_w=200, out_h=136, seed_offset=3)
+    for level in range(cfg.height + 1):
+        P.hmlfc_set_min_level(h, level)
+        P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)
+        a = P.hmlfc_render(h, _dev(cams2), 200, 136)
+        P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+        b = P.hmlfc_render(h, _dev(cams2), 200, 136)
+        assert torch.equal(a, b), level
+    P.hmlfc_set_min_level(h, 0)
     with pytest.raises(P.HmlfcError):   # the counting aid does not read these streams and says so
         P.hmlfc_footprint_decode(h, _dev(coords[:16]))
     P.hmlfc_free(h)
