@@ -17,7 +17,8 @@ constexpr int kNT = 256;  // threads per CTA
 // the shared-memory tables of the render kernel: whole views need no footprint.  PAPER.md:289-293; DESIGN.md section 3.
 // kBlocks (hmlfc_decode_blocks): the segments are the 4 rows of arbitrary 4 x 4 blocks (u, v, bx, by) = blocks[g / 4] -- random access at
 // the granularity the paper decodes at ("As a block of pixels are decoded ...") -- written as [n][4][4][3].
-template <bool kBlocks>
+// kSubpel: streams with half-pel motion offsets (R28): the reference row is the rounded mean of 1 / 2 / 4 samples of up to two rows.
+template <bool kBlocks, bool kSubpel = false>
 __global__ void __launch_bounds__(kNT)
 decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__ views, long long n_seg, uint8_t *__restrict__ out,
                    unsigned long long *__restrict__ oob, int out_aligned)
@@ -75,33 +76,72 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
                     const uint32_t mr = bise_at(S.mv + d.z, fr.w + popc(fr.z & (bit - 1u)), S.mv_layout, S.mv_m, lut);
                     int md, dx, dy;
                     mv_unpack(S, mr, md, dx, dy);
-                    const int rx = s0 + dx, ry = t + dy;
-                    if ((unsigned)ry < (unsigned)S.Ht) {
+                    if (!kSubpel) {
+                        const int rx = s0 + dx, ry = t + dy;
+                        if ((unsigned)ry < (unsigned)S.Ht) {
+                            const uint4 dr = ldg(S.pc + refpc0 + c);
+                            // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
+                            const int o = rx & 3, bxa = rx >> 2;
+                            const uint32_t j0 = (uint32_t)((ry & 3) << 2);
+                            const int rowb = (ry >> 2) * S.nbx;
+                            uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
+                            if ((unsigned)bxa < (unsigned)S.nbx) {
+                                const int rb = rowb + bxa;
+                                const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
+                                const uint32_t rbit = 1u << (rb & 31);
+                                if (rf.x & rbit) qa = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
+                            }
+                            if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
+                                const int rb = rowb + bxa + 1;
+                                const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
+                                const uint32_t rbit = 1u << (rb & 31);
+                                if (rf.x & rbit) qb = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
+                            }
+                            uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
+                            if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
+                            const uint32_t sh = (uint32_t)(o & 1) << 4;
+                            const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
+                            const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
+                            if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }   // R10: additive P = e - R
+                            else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }      //      subtractive P = e + R
+                        }
+                    } else {
+                        const int fx = dx & 1, fy = dy & 1;
+                        const int rx = s0 + (dx >> 1), ry = t + (dy >> 1), o = rx & 3, bxa = rx >> 2;
                         const uint4 dr = ldg(S.pc + refpc0 + c);
-                        // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
-                        const int o = rx & 3, bxa = rx >> 2;
-                        const uint32_t j0 = (uint32_t)((ry & 3) << 2);
-                        const int rowb = (ry >> 2) * S.nbx;
-                        uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-                        if ((unsigned)bxa < (unsigned)S.nbx) {
-                            const int rb = rowb + bxa;
-                            const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
-                            const uint32_t rbit = 1u << (rb & 31);
-                            if (rf.x & rbit) qa = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
+                        int h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+#pragma unroll
+                        for (int jr = 0; jr < 2; ++jr) {
+                            const int r = ry + jr;
+                            if ((jr && !fy) || (unsigned)r >= (unsigned)S.Ht) continue;
+                            const uint32_t j0 = (uint32_t)((r & 3) << 2);
+                            const int rowb = (r >> 2) * S.nbx;
+                            uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
+                            if ((unsigned)bxa < (unsigned)S.nbx) {
+                                const int rb = rowb + bxa;
+                                const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
+                                const uint32_t rbit = 1u << (rb & 31);
+                                if (rf.x & rbit) qa = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
+                            }
+                            if ((o || fx) && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
+                                const int rb = rowb + bxa + 1;
+                                const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
+                                const uint32_t rbit = 1u << (rb & 31);
+                                if (rf.x & rbit) qb = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
+                            }
+                            // samples o .. o+4 of the 8-sample string qa | qb
+                            uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
+                            if (o & 2) { w0 = w1; w1 = w2; w2 = w3; w3 = 0u; }
+                            const uint32_t sh = (uint32_t)(o & 1) << 4;
+                            const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh), q45 = __funnelshift_r(w2, w3, sh);
+                            const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
+                            const int q4 = (int)(int16_t)(q45 & 0xFFFFu);
+                            h0 += q0 + (fx ? q1 : 0); h1 += q1 + (fx ? q2 : 0); h2 += q2 + (fx ? q3 : 0); h3 += q3 + (fx ? q4 : 0);
                         }
-                        if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
-                            const int rb = rowb + bxa + 1;
-                            const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
-                            const uint32_t rbit = 1u << (rb & 31);
-                            if (rf.x & rbit) qb = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
-                        }
-                        uint32_t w0 = qa.x, w1 = qa.y, w2 = qb.x, w3 = qb.y;
-                        if (o & 2) { w0 = w1; w1 = w2; w2 = w3; }
-                        const uint32_t sh = (uint32_t)(o & 1) << 4;
-                        const uint32_t q01 = __funnelshift_r(w0, w1, sh), q23 = __funnelshift_r(w1, w2, sh);
-                        const int q0 = (int)(int16_t)(q01 & 0xFFFFu), q1 = (int)q01 >> 16, q2 = (int)(int16_t)(q23 & 0xFFFFu), q3 = (int)q23 >> 16;
-                        if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }   // R10: additive P = e - R
-                        else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }      //      subtractive P = e + R
+                        const int k = fx + fy;  // log2 of the number of samples; rounding term n / 2 = 0, 1, 2 = k
+                        const int q0 = (h0 + k) >> k, q1 = (h1 + k) >> k, q2 = (h2 + k) >> k, q3 = (h3 + k) >> k;
+                        if (md) { e0 -= q0; e1 -= q1; e2 -= q2; e3 -= q3; }
+                        else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
                     }
                 }
                 a[c][0] += e0; a[c][1] += e1; a[c][2] += e2; a[c][3] += e3;
@@ -142,7 +182,8 @@ cudaError_t launch_decode_rows(const DevStream &S, const int32_t *d_views, int64
     const long long blocks = (n_seg + kNT - 1) / kNT;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_rows_kernel<false><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    if (S.sp) decode_rows_kernel<false, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    else decode_rows_kernel<false><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
@@ -156,7 +197,8 @@ cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks
     const long long blocks = (n_seg + kNT - 1) / kNT;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    decode_rows_kernel<true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
+    if (S.sp) decode_rows_kernel<true, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
+    else decode_rows_kernel<true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }

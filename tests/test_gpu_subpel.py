@@ -63,6 +63,10 @@ def test_halfpel_stream_decode_and_render(P, name, tau):
     B = cfg.block
     bc = np.array([(u, v, bx * B + i, by * B + j) for (u, v, bx, by) in blocks for j in range(B) for i in range(B)], dtype=np.int32)
     assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy().reshape(-1, 3), s.decode(bc))
+    P.hmlfc_set_decode_variant(h, P.DECODE_THREAD)   # whole views and blocks once more through the per-sample kernel (4 x 4 blocks: above ran the block-row kernel)
+    assert np.array_equal(P.hmlfc_decode_views(h, _dev(views)).cpu().numpy().reshape(-1, 3), expect)
+    assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy().reshape(-1, 3), s.decode(bc))
+    P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
     cams = wl.camera_path(cfg)
     ref = s.render(cams, cfg.out_w, cfg.out_h)
     P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)
