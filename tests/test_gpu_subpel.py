@@ -50,7 +50,7 @@ def test_halfpel_stream_decode_and_render(P, name, tau):
     expect = s.decode(coords)
     if tau == 0:
         assert np.array_equal(expect.reshape(lf.shape), lf)
-    for variant in (P.DECODE_AUTO, P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):   # all land on the per-sample kernel
+    for variant in (P.DECODE_AUTO, P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):   # thread per coordinate, or the queue kernel's half-pel instantiation
         P.hmlfc_set_decode_variant(h, variant)
         assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), variant
     P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
