@@ -287,7 +287,9 @@ static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_ca
     const bool fused_ok = D.B == 4 && (rv == 0 || (rv >= 6 && rv <= 15));
     // half-pel streams (R28): the tile kernel's half-pel instantiation (32 x 32 tiles) for 4 x 4 blocks and windows up to 63, else per sample
     const bool sp_tiles = D.sp && !D.cs && D.B == 4 && D.mv_off <= 127 && (rv == 0 || rv >= 6);
-    if (rv == 1 || D.cs || (D.sp && !sp_tiles) || (D.lmin > 0 && !fused_ok))
+    // chroma-subsampled streams (R18): likewise its chroma instantiation (not both at once)
+    const bool cs_tiles = D.cs && !D.sp && D.B == 4 && (rv == 0 || rv >= 6);
+    if (rv == 1 || (D.cs && !cs_tiles) || (D.sp && !sp_tiles) || (D.lmin > 0 && !fused_ok))
         CU(h, launch_render_pixel(D, cams, n_views, W, H, d_out, st, &nl));
     else if (rv == 4 || rv == 5 || D.B != 4)
         CU(h, launch_render_warp(D, cams, n_views, W, H, d_out, st, &nl, rv == 5 ? 1 : 0));
@@ -301,7 +303,7 @@ static int render_impl(const hmlfc_handle *h, const DevStream &D, const hmlfc_ca
         // cfg4 0.88 / 1.26 / 0.90 / 0.97 / 1.39 (1.00), cfg5 1.18 / 1.07 / 1.05 / 1.18 / 0.97 (1.50); cfg3 (about one sample per pixel) 1.06 / 1.28 /
         // 1.12 / 1.44 / 1.50 (0.84)
         if (rv == 0 && (long long)W * H >= 2LL * D.Ws * D.Ht) tiles = (long long)W * H >= 8LL * D.Ws * D.Ht ? 4 : 0;
-        if (sp_tiles) tiles = 0;
+        if (sp_tiles || cs_tiles) tiles = 0;
         if (tiles >= 0) {
             void *scratch = nullptr;
             cudaMemPool_t pool;

@@ -395,7 +395,9 @@ __device__ __forceinline__ bool tables_fit(const TileHeader &hd)
 // Phases B1-B4 for the tile whose tables are in ctl.tab (visible to all threads; they fit the arena): the float RGB patch of every
 // (view, sample) cell.  kZeroFrom: the first 16-byte word of the accumulator region this function still has to zero (the caller zeroed
 // the words before it and ctl.n_rec).  Returns false (CTA-uniform) when the record list does not fit; ends with a barrier either way.
-template <int kArenaBytes, int kNT, bool kSubpel = false>
+// kCs: chroma-subsampled streams (R18): the Co / Cg plane-channels have their own (half-resolution) block grid in B1 - B3; the
+// accumulators stay at luma resolution (a chroma sample is written to the up to 2 x 2 cells it covers), so B4 and the tables do not change.
+template <int kArenaBytes, int kNT, bool kSubpel = false, bool kCs = false>
 __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int zero_from)
 {
     const int tid = threadIdx.x, lane = tid & 31;
@@ -455,14 +457,20 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                 const uint32_t s = fdiv((uint32_t)it, m_ps), r = (uint32_t)it - s * (uint32_t)per_slot;
                 const uint32_t c = fdiv(r, m_nbh), jr = r - c * (uint32_t)nbhmax;
                 const SlotInfo &sl = ctl.tab.slot[s];
-                on = (int)jr < sl.nbh;
+                // the channel's block box: the slot's, or (kCs, chroma) the blocks of the half-resolution plane under the slot's sample box
+                int cbx0 = sl.bx0, cby0 = sl.by0, cnbw = sl.nbw, cnbh = sl.nbh, cnbx = S.nbx;
+                if (kCs && c > 0u) {
+                    cbx0 = sl.s0 >> 3; cby0 = sl.t0 >> 3; cnbw = (sl.s1 >> 3) - cbx0 + 1; cnbh = (sl.t1 >> 3) - cby0 + 1; cnbx = S.nbx_c;
+                    if (sl.ns == 0) cnbh = 0;
+                }
+                on = (int)jr < cnbh;
                 if (on) {
                     frbase = flag_index(S, sl.pc0 + c, 0u);  // = the descriptor's flag record base, without waiting for it
                     sc = s | (c << 6);
                     pred = sl.pred;
-                    by = sl.by0 + (int)jr;
-                    rowb = by * S.nbx;
-                    b0 = rowb + sl.bx0; b1 = b0 + sl.nbw - 1;
+                    by = cby0 + (int)jr;
+                    rowb = by * cnbx;
+                    b0 = rowb + cbx0; b1 = b0 + cnbw - 1;
                 }
             }
             const int ng = on ? (b1 >> 5) - (b0 >> 5) + 1 : 0;
@@ -533,14 +541,15 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
         const int fx = kSubpel ? (dx & 1) : 0, fy = kSubpel ? (dy & 1) : 0;
         const int rx = (int)((r0.z >> 20) << 2) + (kSubpel ? (dx >> 1) : dx), ry0 = (int)(((r0.z >> 8) & 0xFFFu) << 2) + (kSubpel ? (dy >> 1) : dy);
         const int bxa = rx >> 2, bya = ry0 >> 2;  // arithmetic shifts: floor for positions left of / above the image
+        const int cnbx = (kCs && c > 0u) ? S.nbx_c : S.nbx, cnby = (kCs && c > 0u) ? S.nby_c : S.nby;  // the channel's block grid
         uint32_t e[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int bx = bxa + (j & 1), by = bya + (j >> 1);
             e[j] = 0u;
             // needed at all: the second column only if the row straddles two blocks, the second block row likewise
-            if ((unsigned)bx < (unsigned)S.nbx && (unsigned)by < (unsigned)S.nby && (!(j & 1) || (rx & 3) || fx) && (!(j >> 1) || (ry0 & 3) || fy)) {
-                const int b = by * S.nbx + bx;
+            if ((unsigned)bx < (unsigned)cnbx && (unsigned)by < (unsigned)cnby && (!(j & 1) || (rx & 3) || fx) && (!(j >> 1) || (ry0 & 3) || fy)) {
+                const int b = by * cnbx + bx;
                 const uint2 fr = __ldg(reinterpret_cast<const uint2 *>(S.flagrec + dr.x + 4u * (uint32_t)(b >> 5)));  // {res bits, res rank}
                 const uint32_t bit = 1u << (b & 31);
                 if (fr.x & bit) e[j] = ((fr.y + popc(fr.x & (bit - 1u))) << 4) | 1u;
@@ -562,7 +571,9 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
             const SlotInfo &sl = ctl.tab.slot[s];
             const int yy0 = (int)(((r0.z >> 8) & 0xFFFu) << 2), yy = yy0 + ky;
             const int st0 = sl.t0, st1 = sl.t1;
-            if (yy < st0 || yy > st1) continue;
+            const int csh = (kCs && c > 0u) ? 1 : 0;  // the channel's samples are (s >> csh, t >> csh); its image has Ht >> csh rows
+            if (yy < (st0 >> csh) || yy > (st1 >> csh)) continue;
+            const int cHt = S.Ht >> csh;
             const int xx = (int)((r0.z >> 20) << 2);
             const uint4 d = ctl.desc[s][c];
             uint2 own = make_uint2(0u, 0u);
@@ -574,7 +585,7 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                 const uint4 re = rec[2 * rr + 1];
                 if (!kSubpel) {
                     const int rx = xx + dx, ry = yy + dy;
-                    if ((unsigned)ry < (unsigned)S.Ht) {
+                    if ((unsigned)ry < (unsigned)cHt) {
                         // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1: B2 looked them up
                         const int o = rx & 3;
                         const bool second_row = (ry >> 2) != ((yy0 + dy) >> 2);
@@ -602,7 +613,7 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
 #pragma unroll
                     for (int jr = 0; jr < 2; ++jr) {
                         const int r = ry + jr;
-                        if ((jr && !fy) || (unsigned)r >= (unsigned)S.Ht) continue;
+                        if ((jr && !fy) || (unsigned)r >= (unsigned)cHt) continue;
                         const bool second_row = (r >> 2) != bya;
                         const uint32_t ea = second_row ? re.z : re.x, eb = second_row ? re.w : re.y;
                         const uint32_t i0 = (uint32_t)((r & 3) << 2);
@@ -624,12 +635,28 @@ __device__ __forceinline__ bool decode_patch(const DevStream &S, Ctl &ctl, unsig
                     else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
                 }
             }
-            int16_t *dst = acc16 + (((sl.accbase + (yy - st0) * sl.ns + (xx - sl.s0)) << 2) + (int)c);
             const int ss0 = sl.s0, ss1 = sl.s1;
-            if (xx >= ss0 && xx <= ss1) dst[0] = (int16_t)e0;
-            if (xx + 1 >= ss0 && xx + 1 <= ss1) dst[4] = (int16_t)e1;
-            if (xx + 2 >= ss0 && xx + 2 <= ss1) dst[8] = (int16_t)e2;
-            if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
+            if (!csh) {
+                int16_t *dst = acc16 + (((sl.accbase + (yy - st0) * sl.ns + (xx - sl.s0)) << 2) + (int)c);
+                if (xx >= ss0 && xx <= ss1) dst[0] = (int16_t)e0;
+                if (xx + 1 >= ss0 && xx + 1 <= ss1) dst[4] = (int16_t)e1;
+                if (xx + 2 >= ss0 && xx + 2 <= ss1) dst[8] = (int16_t)e2;
+                if (xx + 3 >= ss0 && xx + 3 <= ss1) dst[12] = (int16_t)e3;
+            } else {
+                // a chroma sample (x, y) is the value of the luma-resolution cells (2x .. 2x+1, 2y .. 2y+1) (R18: nearest-neighbour replication)
+                const int ev[4] = {e0, e1, e2, e3};
+#pragma unroll
+                for (int jy = 0; jy < 2; ++jy) {
+                    const int ly = 2 * yy + jy;
+                    if (ly < st0 || ly > st1) continue;
+                    int16_t *row = acc16 + (((sl.accbase + (ly - st0) * sl.ns - ss0) << 2) + (int)c);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int lx = 2 * xx + i;
+                        if (lx >= ss0 && lx <= ss1) row[lx << 2] = (int16_t)ev[i >> 1];
+                    }
+                }
+            }
         }
     }
     __syncthreads();
@@ -772,7 +799,7 @@ __device__ __forceinline__ void setup_rays(const DevStream &S, const Camera &cam
 // One pass over a (sub-)tile whose rays are set up: ranges (SV), tables (T), decode (decode_patch), gather + blend (C).
 // Returns true (CTA-uniform) when rgb[] holds the pass's pixels (background where the ray misses); false when the
 // tables do not fit the arena and the (sub-)tile must be split.
-template <int kArenaBytes, int kNT, bool kSubpel = false>
+template <int kArenaBytes, int kNT, bool kSubpel = false, bool kCs = false>
 __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, const PixTaps (&pt)[kPPL],
                                           uint32_t (&rgb)[kPPL])
 {
@@ -847,7 +874,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
     PHASE_MARK(4);
     bool ok = tables_fit<kArenaBytes>(ctl.tab.hdr);
     if (!ok) PASS_STAT(10);
-    else ok = decode_patch<kArenaBytes, kNT, kSubpel>(S, ctl, arena, kSpecZero);
+    else ok = decode_patch<kArenaBytes, kNT, kSubpel, kCs>(S, ctl, arena, kSpecZero);
     reset_ctl(ctl);  // behind a barrier that followed every read of the ranges and of the record count
     if (!ok) return false;
 
@@ -866,7 +893,7 @@ __device__ __forceinline__ bool tile_pass(const DevStream &S, Ctl &ctl, unsigned
 // than output pixels under the tile), its four quadrants with one pixel per thread, each split again when it does not fit; a sub-tile of
 // the last level that still does not fit (strong minification) is rendered by 16 direct sample decodes per pixel.  ctl.cam, ctl.aff and
 // ctl.lut are set and visible, the accumulators of ctl are reset (reset_ctl).  path = child index (2 bits) of every level on the way down.
-template <int kArenaBytes, int kNT, int kTW, bool kSubpel = false>
+template <int kArenaBytes, int kNT, int kTW, bool kSubpel = false, bool kCs = false>
 __device__ __forceinline__ void render_tile_general(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int W, int H, uint8_t *__restrict__ out,
                                                     int out_aligned, int view, int tile_x, int tile_y)
 {
@@ -894,7 +921,7 @@ __device__ __forceinline__ void render_tile_general(const DevStream &S, Ctl &ctl
             setup_rays<kTW>(S, cam, W, H, sx, sy, full, lpw, npx, pt);
             PHASE_MARK(0);
             PASS_STAT(lvl);
-            done = tile_pass<kArenaBytes, kNT, kSubpel>(S, ctl, arena, pt, rgb);
+            done = tile_pass<kArenaBytes, kNT, kSubpel, kCs>(S, ctl, arena, pt, rgb);
             if (done) PASS_STAT(4 + lvl);
             if (!done && lvl == kLMax) {
                 PASS_STAT(13);

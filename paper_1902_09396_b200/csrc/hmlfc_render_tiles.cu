@@ -143,20 +143,20 @@ tile_tables_kernel(const __grid_constant__ DevStream S, const Camera *__restrict
 }
 
 // the general path as a call: its registers and spills stay out of the tile kernel's own allocation (the call is rare)
-template <int kArenaBytes, int kNT, int kTW, bool kSubpel = false>
+template <int kArenaBytes, int kNT, int kTW, bool kSubpel = false, bool kCs = false>
 __device__ __noinline__ void general_tile_call(const DevStream &S, Ctl &ctl, unsigned char *__restrict__ arena, int W, int H, uint8_t *__restrict__ out,
                                                int out_aligned, int view, int tile_x, int tile_y)
 {
     // the general path's tile is kTW x (4 kNT / kTW) pixels: one call, or two for the 64 x 32 tile of 256 threads (64 x 16 each)
     constexpr int kGenTH = kNT * kPPL / kTW;
     for (int part = 0; part < kTile / kGenTH; ++part)
-        render_tile_general<kArenaBytes, kNT, kTW, kSubpel>(S, ctl, arena, W, H, out, out_aligned, view, tile_x, tile_y * (kTile / kGenTH) + part);
+        render_tile_general<kArenaBytes, kNT, kTW, kSubpel, kCs>(S, ctl, arena, W, H, out, out_aligned, view, tile_x, tile_y * (kTile / kGenTH) + part);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // kTW x 32 pixels per CTA of kNT threads: 32 x 32 / 256 (4 pixels per thread), 64 x 32 / 512 (4), 64 x 32 / 256 (8)
-// kSubpel: streams with half-pel motion offsets (R28; phases B2 / B3 of decode_patch)
-template <int kArenaBytes, int kMinBlocks, bool kAllPow2, int kNT, int kTW, bool kSubpel = false>
+// kSubpel: streams with half-pel motion offsets (R28; phases B2 / B3 of decode_patch); kCs: chroma-subsampled streams (R18; B1 - B3)
+template <int kArenaBytes, int kMinBlocks, bool kAllPow2, int kNT, int kTW, bool kSubpel = false, bool kCs = false>
 __global__ void __launch_bounds__(kNT, kMinBlocks)
 render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restrict__ cams, int W, int H, uint8_t *__restrict__ out, int out_aligned,
                     const uint4 *__restrict__ tables)
@@ -207,13 +207,13 @@ render_tiles_kernel(const __grid_constant__ DevStream S, const Camera *__restric
     }
     __syncthreads();
     PHASE_MARK(4);
-    if (fast) fast = decode_patch<kArenaBytes, kNT, kSubpel>(S, ctl, arena, 0x7fffffff - kNT);
+    if (fast) fast = decode_patch<kArenaBytes, kNT, kSubpel, kCs>(S, ctl, arena, 0x7fffffff - kNT);
     if (!fast) {
         PASS_STAT(hd.status != kTileTables ? 14 : 15);
         // irregular rays, more than 4 x 4 views, or tables / records that do not fit the arena: the general path, in this CTA
         reset_ctl(ctl);
         if (tid < 2) camera_affine(S, ctl.cam, tid, ctl.aff[tid]);
-        general_tile_call<kArenaBytes, kNT, kTW, kSubpel>(S, ctl, arena, W, H, out, out_aligned ? 1 : 0, view, (int)blockIdx.x, (int)blockIdx.y);
+        general_tile_call<kArenaBytes, kNT, kTW, kSubpel, kCs>(S, ctl, arena, W, H, out, out_aligned ? 1 : 0, view, (int)blockIdx.x, (int)blockIdx.y);
         return;
     }
 
@@ -321,6 +321,8 @@ cudaError_t configure_render_tiles()
     // half-pel streams: configuration 0 only
     if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<kSubpelArena, 3, false, 256, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubpelArena);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<kSubpelArena, 3, true, 256, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubpelArena);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<kSubpelArena, 3, false, 256, 32, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubpelArena);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(render_tiles_kernel<kSubpelArena, 3, true, 256, 32, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubpelArena);
     return e;
 }
 
@@ -343,7 +345,11 @@ cudaError_t launch_render_tiles(const DevStream &S, const Camera *d_cams, int n_
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)tiles_x, (unsigned)tiles_y, (unsigned)n_views);
-    if (S.sp) {  // half-pel streams: 32 x 32 tiles, 3 CTAs per SM whatever the configuration asked for
+    if (S.cs) {  // chroma-subsampled streams: 32 x 32 tiles, 3 CTAs per SM whatever the configuration asked for
+        if (S.sp || config >= 2) return cudaErrorInvalidValue;  // (both at once: the caller routes to the per-sample kernel)
+        if (S.pow2_mask == 15u) render_tiles_kernel<kSubpelArena, 3, true, 256, 32, false, true><<<grid, 256, kSubpelArena, st>>>(S, d_cams, W, H, d_out, aligned, tables);
+        else render_tiles_kernel<kSubpelArena, 3, false, 256, 32, false, true><<<grid, 256, kSubpelArena, st>>>(S, d_cams, W, H, d_out, aligned, tables);
+    } else if (S.sp) {  // half-pel streams: likewise
         if (S.mv_off > 127 || config >= 2) return cudaErrorInvalidValue;  // (the records pack an offset in 8 bits; the caller routes)
         if (S.pow2_mask == 15u) render_tiles_kernel<kSubpelArena, 3, true, 256, 32, true><<<grid, 256, kSubpelArena, st>>>(S, d_cams, W, H, d_out, aligned, tables);
         else render_tiles_kernel<kSubpelArena, 3, false, 256, 32, true><<<grid, 256, kSubpelArena, st>>>(S, d_cams, W, H, d_out, aligned, tables);

@@ -1,7 +1,7 @@
 """GPU parity on chroma-subsampled streams (R18): the CUDA path through the C ABI against the oracle.
 
 The streams come from the oracle's encoder (hmlfc_encode does not subsample); decoded pixels bit-exact, views within 1 LSB.
-On these streams hmlfc_decode / _views / _blocks and hmlfc_render run the per-sample kernels."""
+On these streams hmlfc_decode / _views / _blocks run the per-sample kernels; hmlfc_render the tile kernel's chroma instantiation (4 x 4 blocks)."""
 import numpy as np
 import pytest
 
@@ -67,11 +67,25 @@ def test_subsampled_stream_decode_and_render(P, name, tau):
     # views
     cams = wl.camera_path(cfg)
     ref = s.render(cams, cfg.out_w, cfg.out_h)
-    for variant in (P.RENDER_AUTO, P.RENDER_TILES, P.RENDER_CTA):         # likewise: the thread-per-pixel kernel
+    P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)
+    unshared = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
+    # 4 x 4 blocks: the tile kernel's chroma instantiation (whatever fused variant is asked for); otherwise the thread-per-pixel kernel
+    for variant in (P.RENDER_AUTO, P.RENDER_TILES, P.RENDER_TILES_W256X3, P.RENDER_CTA, P.RENDER_CTA_BIG, P.RENDER_WARP):
         P.hmlfc_set_render_variant(h, variant)
         out = P.hmlfc_render(h, _dev(cams), cfg.out_w, cfg.out_h).cpu().numpy()
         d = np.abs(out.astype(np.int16) - ref.astype(np.int16))
         assert d.max() <= 1 and (d > 0).mean() < 1e-3, (variant, int(d.max()))
+        assert np.array_equal(out, unshared), variant
+    # a magnified, rotated batch (several tiles per view, ragged edges) and every progressive level
+    cams2 = wl.camera_path(cfg, n_views=3, out_w=200, out_h=136, seed_offset=3)
+    for level in range(cfg.height + 1):
+        P.hmlfc_set_min_level(h, level)
+        P.hmlfc_set_render_variant(h, P.RENDER_PIXEL)
+        a = P.hmlfc_render(h, _dev(cams2), 200, 136)
+        P.hmlfc_set_render_variant(h, P.RENDER_AUTO)
+        b = P.hmlfc_render(h, _dev(cams2), 200, 136)
+        assert torch.equal(a, b), level
+    P.hmlfc_set_min_level(h, 0)
     # the counting aid does not read these streams and says so
     with pytest.raises(P.HmlfcError):
         P.hmlfc_footprint_decode(h, _dev(coords[:16]))
