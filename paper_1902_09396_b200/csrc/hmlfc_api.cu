@@ -234,7 +234,7 @@ int hmlfc_decode(const hmlfc_handle *h, const int32_t *d_coords, int64_t n, uint
 {
     if (!h || n < 0 || (n > 0 && (!d_coords || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->decode_variant == 1 || h->ds.cs)  // chroma-subsampled streams (R18): the per-sample kernel reads them
+    if (h->decode_variant == 1)  // the per-sample kernel (cross-check)
         CU(h, launch_decode(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else
         CU(h, launch_decode_queue(h->ds, d_coords, n, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl,

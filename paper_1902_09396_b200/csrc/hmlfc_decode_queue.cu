@@ -183,7 +183,7 @@ __device__ __forceinline__ void drain_values_eager(const DevStream &S, Q &q, int
 
 // execute the top n (<= 32) motion tasks: decode the record (S6), locate the reference sample (S7) and, where
 // the reference block is significant, push its value task
-template <bool kSubpel, typename Q>
+template <bool kSubpel, bool kCs, typename Q>
 __device__ __forceinline__ void drain_motion_eager(const DevStream &S, Q &q, int &mcnt, int &vcnt, int n, int lane,
                                              uint32_t lane_lt, const uint16_t *lut)
 {
@@ -196,10 +196,13 @@ __device__ __forceinline__ void drain_motion_eager(const DevStream &S, Q &q, int
         int mode, dx, dy;
         mv_unpack(S, rec, mode, dx, dy);
         const uint32_t xy = q.xy[t.w >> 2];
+        // the channel's own geometry: (kCs, R18) Co / Cg live at half resolution, sample (s >> 1, t >> 1)
+        const int csh = (kCs && (t.w & 3u) != 0u) ? 1 : 0;
+        const int px = (int)(xy & 0xFFFFu) >> csh, py = (int)(xy >> 16) >> csh, cW = S.Ws >> csh, cH = S.Ht >> csh, cnbx = csh ? S.nbx_c : S.nbx;
         if (kSubpel) {
             // half-pel offsets (R28): the reference value is the mean of the 1 / 2 / 4 stored samples around the position, rounded
             // half up -- the sum has to be complete before it is rounded, so the lane looks the samples up itself (no value tasks)
-            const int x2 = 2 * (int)(xy & 0xFFFFu) + dx, y2 = 2 * (int)(xy >> 16) + dy;
+            const int x2 = 2 * px + dx, y2 = 2 * py + dy;
             const int x0 = x2 >> 1, y0 = y2 >> 1, fx = x2 & 1, fy = y2 & 1;
             const uint4 rd = ldg(S.pc + t.z);
             int sum = 0;
@@ -207,8 +210,8 @@ __device__ __forceinline__ void drain_motion_eager(const DevStream &S, Q &q, int
             for (int j = 0; j < 4; ++j) {
                 if (((j & 1) && !fx) || ((j >> 1) && !fy)) continue;
                 const int rx = x0 + (j & 1), ry = y0 + (j >> 1);
-                if ((unsigned)rx >= (unsigned)S.Ws || (unsigned)ry >= (unsigned)S.Ht) continue;  // R8
-                const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+                if ((unsigned)rx >= (unsigned)cW || (unsigned)ry >= (unsigned)cH) continue;  // R8
+                const int b = (ry >> S.logB) * cnbx + (rx >> S.logB);
                 const uint4 fr = ldg(S.flagrec + flag_index(S, t.z, (uint32_t)(b >> 5)));
                 const uint32_t bit = 1u << (b & 31);
                 if (!(fr.x & bit)) continue;
@@ -219,9 +222,9 @@ __device__ __forceinline__ void drain_motion_eager(const DevStream &S, Q &q, int
             const int k = fx + fy, qv = (sum + k) >> k;  // rounding term n / 2 = 0, 1, 2 = k
             atomicAdd(&q.acc[t.w], mode ? -qv : qv);
         } else {
-            const int rx = (int)(xy & 0xFFFFu) + dx, ry = (int)(xy >> 16) + dy;
-            if ((unsigned)rx < (unsigned)S.Ws && (unsigned)ry < (unsigned)S.Ht) {  // R8: outside the image reads 0
-                const int b = (ry >> S.logB) * S.nbx + (rx >> S.logB);
+            const int rx = px + dx, ry = py + dy;
+            if ((unsigned)rx < (unsigned)cW && (unsigned)ry < (unsigned)cH) {  // R8: outside the image reads 0
+                const int b = (ry >> S.logB) * cnbx + (rx >> S.logB);
                 const uint4 rd = ldg(S.pc + t.z);
                 const uint4 fr = ldg(S.flagrec + flag_index(S, t.z, (uint32_t)(b >> 5)));
                 const uint32_t bit = 1u << (b & 31);
@@ -358,11 +361,11 @@ __device__ __forceinline__ void drain_v(const DevStream &S, Q &q, int &vcnt, int
     else drain_values_eager(S, q, vcnt, n, lane, lut);
 }
 
-template <int kMode, bool kSubpel, typename Q>
+template <int kMode, bool kSubpel, bool kCs, typename Q>
 __device__ __forceinline__ void drain_m(const DevStream &S, Q &q, int &mcnt, int &vcnt, int n, int lane, uint32_t lane_lt, const uint16_t *lut)
 {
     if (kMode == 1) drain_motion(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
-    else drain_motion_eager<kSubpel>(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
+    else drain_motion_eager<kSubpel, kCs>(S, q, mcnt, vcnt, n, lane, lane_lt, lut);
 }
 
 // kDense: the coordinates are not read but generated -- sample i is pixel i mod (Ws Ht) (row-major) of view views[i / (Ws Ht)]
@@ -371,7 +374,8 @@ __device__ __forceinline__ void drain_m(const DevStream &S, Q &q, int &mcnt, int
 // streams the L2 holds, where the sector rate binds); otherwise it reads the three channels' flag records and descriptors up front and the
 // tasks carry them (one dependent load less per task: for streams in HBM, where every access is a DRAM access either way and latency binds).
 // kSubpel (eager form only): streams with half-pel motion offsets, see drain_motion_eager.
-template <int kDense, int kMode, bool kSubpel = false>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
+// kCs (eager form only): chroma-subsampled streams -- the Co / Cg channels of a sample are classified on their own block grid.
+template <int kDense, int kMode, bool kSubpel = false, bool kCs = false>  // kDense 0: coordinates read; 1: whole views; 2: whole B x B blocks (u, v, bx, by) = blocks[i / B^2], written [n][B][B][3]
 __global__ void __launch_bounds__(kThreads, 5)
 decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long long n, uint8_t *__restrict__ out,
                     unsigned long long *oob, int out_aligned)
@@ -431,6 +435,12 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
     const uint32_t bit = 1u << (b & 31);
     const uint32_t fg = (uint32_t)(b >> 5);
     const uint32_t kin = (uint32_t)(((y & (S.B - 1)) << S.logB) + (x & (S.B - 1)));
+    // (kCs) the same for the sample's chroma position (x >> 1, y >> 1) on the chroma block grid
+    const int xc = x >> 1, yc = y >> 1;
+    const int b_c = (kCs && valid) ? (yc >> S.logB) * S.nbx_c + (xc >> S.logB) : 0;
+    const uint32_t bit_c = kCs ? 1u << (b_c & 31) : bit, fg_c = kCs ? (uint32_t)(b_c >> 5) : fg;
+    const uint32_t kin_c = kCs ? (uint32_t)(((yc & (S.B - 1)) << S.logB) + (xc & (S.B - 1))) : kin;
+    const uint32_t bit0 = bit, kin0 = kin;
     int vcnt = 0, mcnt = 0;
 
     constexpr bool kLazy = kMode == 1;
@@ -484,7 +494,7 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
                     const bool pred = predictive && ((flj >> (3 + c)) & 1u);
                     push(q.mq, mcnt, pred, make_uint4(base + (uint32_t)c, fg, rbase + (uint32_t)c, dest | (((prj >> (5 * c)) & 31u) << 8)), lane_lt);
                     if (mcnt >= 32) {
-                        drain_m<kMode, kSubpel>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                        drain_m<kMode, kSubpel, kCs>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
                         if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
                     }
                 }
@@ -507,14 +517,22 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
         for (int c = 0; c < 3; ++c) d[c] = fr[c] = make_uint4(0u, 0u, 0u, 0u);
         if (valid) {
             const uint4 *slot = S.flagrec + flag_index(S, base, fg);
-            ldg256(slot, fr[0], fr[1]);
-            fr[2] = ldg(slot + 2);
+            if (kCs) {  // the chroma records of the plane's slot of group fg_c
+                const uint4 *slot_c = S.flagrec + flag_index(S, base, fg_c);
+                fr[0] = ldg(slot);
+                fr[1] = ldg(slot_c + 1);
+                fr[2] = ldg(slot_c + 2);
+            } else {
+                ldg256(slot, fr[0], fr[1]);
+                fr[2] = ldg(slot + 2);
+            }
 #pragma unroll
             for (int c = 0; c < 3; ++c) d[c] = ldg(S.pc + base + c);
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const uint32_t dest = (uint32_t)(lane * 4 + c);
+            const uint32_t bit = c ? bit_c : bit0, kin = c ? kin_c : kin0;
             const bool res = (fr[c].x & bit) != 0u;
             const uint32_t rank = fr[c].y + (uint32_t)__popc(fr[c].x & (bit - 1u));
             push(q.vq, vcnt, res, make_uint4(d[c].y, (rank << (2 * S.logB)) + kin, (d[c].w & 0x3FFFFFu) | (dest << 24), 0u), lane_lt);
@@ -523,14 +541,14 @@ decode_queue_kernel(const DevStream S, const int4 *__restrict__ coords, long lon
             const uint32_t mi = fr[c].w + (uint32_t)__popc(fr[c].z & (bit - 1u));
             push(q.mq, mcnt, pred, make_uint4(d[c].z, mi, rbase + (uint32_t)c, dest), lane_lt);
             if (mcnt >= 32) {
-                drain_m<kMode, kSubpel>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
+                drain_m<kMode, kSubpel, kCs>(S, q, mcnt, vcnt, 32, lane, lane_lt, lut);
                 if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
             }
         }
     
     }
     }
-    if (mcnt > 0) drain_m<kMode, kSubpel>(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
+    if (mcnt > 0) drain_m<kMode, kSubpel, kCs>(S, q, mcnt, vcnt, mcnt, lane, lane_lt, lut);
     if (vcnt >= 32) drain_v<kMode>(S, q, vcnt, 32, lane, lut);
     if (vcnt > 0) drain_v<kMode>(S, q, vcnt, vcnt, lane, lut);
     __syncwarp();
@@ -693,7 +711,7 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
     // mode: 0 eager, 1 lazy, 2 block records (needs S.brec); < 0: chosen here
     if (mode < 0) mode = S.brec ? 2 : (S.l2_resident ? 1 : 0);
-    if (S.sp) mode = 0;  // half-pel streams: the eager form has the half-pel instantiation (and they have no block records)
+    if (S.sp || S.cs) mode = 0;  // half-pel / chroma-subsampled streams: the eager form has their instantiations (and they have no block records)
     if (mode == 2 && !S.brec) return cudaErrorInvalidValue;
     const int4 *c4 = reinterpret_cast<const int4 *>(d_coords);
     if (mode == 2) {
@@ -702,6 +720,10 @@ cudaError_t launch_decode_queue(const DevStream &S, const int32_t *d_coords, int
         else decode_brec_kernel<true, kBrecSets, 5><<<(unsigned)cb, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);  // larger L1: configure_decode_queue
     } else if (mode == 1)
         decode_queue_kernel<0, 1><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
+    else if (S.cs && S.sp)
+        decode_queue_kernel<0, 0, true, true><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
+    else if (S.cs)
+        decode_queue_kernel<0, 0, false, true><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     else if (S.sp)
         decode_queue_kernel<0, 0, true><<<(unsigned)blocks, kThreads, 0, st>>>(S, c4, (long long)n, d_out, d_oob, aligned);
     else

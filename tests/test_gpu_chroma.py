@@ -1,7 +1,8 @@
 """GPU parity on chroma-subsampled streams (R18): the CUDA path through the C ABI against the oracle.
 
 The streams come from the oracle's encoder (hmlfc_encode does not subsample); decoded pixels bit-exact, views within 1 LSB.
-On these streams hmlfc_decode / _views / _blocks run the per-sample kernels; hmlfc_render the tile kernel's chroma instantiation (4 x 4 blocks)."""
+On these streams hmlfc_decode_views / _blocks run the per-sample kernel; hmlfc_decode the queue kernel's and hmlfc_render (4 x 4 blocks) the tile
+kernel's chroma instantiation."""
 import numpy as np
 import pytest
 
@@ -49,7 +50,7 @@ def test_subsampled_stream_decode_and_render(P, name, tau):
     h = P.hmlfc_load(data)
     coords = wl.all_coords(cfg)
     expect = s.decode(coords)
-    for variant in (P.DECODE_AUTO, P.DECODE_THREAD, P.DECODE_QUEUE_LAZY):   # every choice lands on the per-sample kernel
+    for variant in (P.DECODE_AUTO, P.DECODE_THREAD, P.DECODE_QUEUE, P.DECODE_QUEUE_LAZY, P.DECODE_QUEUE_BLOCKREC):   # thread per coordinate, or the queue kernel's chroma instantiation
         P.hmlfc_set_decode_variant(h, variant)
         assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), expect), variant
     P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
