@@ -279,8 +279,8 @@ def measure_other_config(P, name, steps, peak, flush, stream):
 
 
 def measure_extra_stream(P, cfg_name, kind, tau_res, steps, flush, stream):
-    """The rows of SURVEY 8(f) beyond the headline stream: a chroma-subsampled (R18: per-sample CUDA path only) or a half-pel
-    motion-compensated (R28: half-pel instantiations of the fast kernels, no block records) stream of the headline configuration's light field, encoded by the ORACLE (hmlfc_encode does
+    """The rows of SURVEY 8(f) beyond the headline stream: a chroma-subsampled (R18) or a half-pel motion-compensated (R28)
+    stream (both: instantiations of the fast kernels, no block records) of the headline configuration's light field, encoded by the ORACLE (hmlfc_encode does
     neither) at the headline stream's threshold; the same timed legs, and a parity spot check against the oracle."""
     import torch
 
@@ -319,7 +319,7 @@ def measure_extra_stream(P, cfg_name, kind, tau_res, steps, flush, stream):
     res = {
         "workload": f"{cfg.name} light field, oracle-encoded with {'Co / Cg at half resolution' if kind == 'chroma' else 'half-pel motion offsets'}, "
                     f"tau_res = {tau_res}, window {window}; render {V} views of {W}x{H}; decode {n} random coordinates; decode all {cfg.U * cfg.V} views",
-        "kernels": ("render_pixel_kernel, decode_kernel, decode_dense_kernel (the per-sample definition: correct, no fast path yet)" if kind == "chroma" else
+        "kernels": ("render_tiles_kernel<kCs>, decode_rows_kernel<kCs>, decode_queue_kernel<kCs> (no block records)" if kind == "chroma" else
                     "render_tiles_kernel<kSubpel>, decode_rows_kernel<kSubpel>, decode_queue_kernel<kSubpel> (no block records)"),
         "stream_bytes": len(data), "stream_bpp": round(8.0 * len(data) / (cfg.U * cfg.V * cfg.Ws * cfg.Ht), 4),
         "psnr_db": round(float(orc.psnr(lf, s.decode_full())), 3), "oracle_encode_s": round(t_enc, 1),

@@ -89,11 +89,11 @@ typedef struct {
  * vectors, packed top-level RKVs) and uploads it to the current CUDA device.  For streams with
  * full-resolution chroma one kernel then writes the BLOCK RECORDS on the device (every stored value
  * and motion record once more, grouped per block for random access: DESIGN.md section 8); the call
- * returns when they are complete.  Streams with subsampled chroma (header byte 49, R18) are read by the
- * per-sample kernels of every entry point (correct, not fast) and get no block records.  Streams with half-pel motion offsets (byte 55;
- * PAPER.md:464, R28) get no block records either, but every entry point has a half-pel instantiation of a fast kernel: hmlfc_decode the
- * warp-cooperative kernel on the stream's strings (any block size), hmlfc_render and hmlfc_decode_views / _blocks the tile and block-row
- * kernels for 4 x 4 blocks (hmlfc_render: windows up to 63); other cases run per sample.  hmlfc_info().device_bytes counts everything that stays resident
+ * returns when they are complete.  Streams with subsampled chroma (header byte 49, R18) and with half-pel
+ * motion offsets (byte 55, R28) get no block records, but every entry point has an instantiation of a fast kernel for
+ * them: hmlfc_decode the warp-cooperative kernel on the stream's strings (any block size), hmlfc_render and hmlfc_decode_views / _blocks
+ * the tile and block-row kernels for 4 x 4 blocks (hmlfc_render: not both flags at once, half-pel windows up to 63); other cases run
+ * per sample -- identical bytes.  hmlfc_info().device_bytes counts everything that stays resident
  * (about 2.2 x the stream).  HMLFC_E_NOMEM if the device cannot hold it.
  *   h_stream_bytes : host, read only during the call; the caller may free it afterwards.
  *   out            : receives the handle; untouched on error.                              */

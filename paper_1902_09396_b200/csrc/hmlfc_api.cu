@@ -248,8 +248,8 @@ int hmlfc_decode_views(const hmlfc_handle *h, const int32_t *d_views, int64_t n_
     if (!h || n_views < 0 || (n_views > 0 && (!d_views || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
     // B = 4 streams: one lane per block-row segment; other block sizes (and decode variant 1 / 2, for cross-checks): one lane per pixel
-    // (half-pel streams, R28: the block-row kernel's half-pel instantiation; per sample for other block sizes and as a cross-check)
-    if (h->ds.cs || (h->ds.sp && !(h->ds.B == 4 && h->decode_variant == 0)))
+    // (half-pel and chroma-subsampled streams, R28 / R18: the block-row kernel's instantiations; per sample for other block sizes and as a cross-check)
+    if ((h->ds.cs || h->ds.sp) && !(h->ds.B == 4 && h->decode_variant == 0))
         CU(h, launch_decode_dense(h->ds, d_views, n_views, false, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_rows(h->ds, d_views, n_views, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
@@ -263,7 +263,7 @@ int hmlfc_decode_blocks(const hmlfc_handle *h, const int32_t *d_blocks, int64_t 
 {
     if (!h || n_blocks < 0 || (n_blocks > 0 && (!d_blocks || !d_out))) return HMLFC_E_INVALID;
     int nl = 0;
-    if (h->ds.cs || (h->ds.sp && !(h->ds.B == 4 && h->decode_variant == 0)))
+    if ((h->ds.cs || h->ds.sp) && !(h->ds.B == 4 && h->decode_variant == 0))
         CU(h, launch_decode_dense(h->ds, d_blocks, n_blocks, true, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));
     else if (h->ds.B == 4 && h->decode_variant == 0)
         CU(h, launch_decode_block_rows(h->ds, d_blocks, n_blocks, d_out, h->d_oob, static_cast<cudaStream_t>(cuda_stream), &nl));

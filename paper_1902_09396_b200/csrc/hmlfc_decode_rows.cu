@@ -18,7 +18,9 @@ constexpr int kNT = 256;  // threads per CTA
 // kBlocks (hmlfc_decode_blocks): the segments are the 4 rows of arbitrary 4 x 4 blocks (u, v, bx, by) = blocks[g / 4] -- random access at
 // the granularity the paper decodes at ("As a block of pixels are decoded ...") -- written as [n][4][4][3].
 // kSubpel: streams with half-pel motion offsets (R28): the reference row is the rounded mean of 1 / 2 / 4 samples of up to two rows.
-template <bool kBlocks, bool kSubpel = false>
+// kCs: chroma-subsampled streams (R18): for Co / Cg the lane decodes the row of the CHROMA block that holds its two chroma samples
+// ((s0 >> 1) .. (s0 >> 1) + 1 of row t >> 1) with the channel's own geometry and takes those two (each serves two of its four pixels).
+template <bool kBlocks, bool kSubpel = false, bool kCs = false>
 __global__ void __launch_bounds__(kNT)
 decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__ views, long long n_seg, uint8_t *__restrict__ out,
                    unsigned long long *__restrict__ oob, int out_aligned)
@@ -57,8 +59,6 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
                 a[0][i] = k.x; a[1][i] = k.y; a[2][i] = k.z;
             }
         }
-        const int b = (t >> 2) * S.nbx + bx;
-        const uint32_t g32 = (uint32_t)(b >> 5), bit = 1u << (b & 31), i0 = (uint32_t)((t & 3) << 2);
         for (int L = S.lmin; L < h; ++L) {
             const LevelDesc lv = S.lev[L];
             const int pu = u >> L, pv = v >> L;
@@ -67,6 +67,11 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
             const bool predictive = ((pu | pv) & 1) != 0;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
+                // the channel's geometry: row tc of its plane, first sample sc0 of the block row segment, block grid, image height
+                const int csh = (kCs && c > 0) ? 1 : 0;
+                const int tc = t >> csh, sc0 = csh ? ((s0 >> 1) & ~3) : s0, cnbx = csh ? S.nbx_c : S.nbx, cHt = S.Ht >> csh;
+                const int b = (tc >> 2) * cnbx + (sc0 >> 2);
+                const uint32_t g32 = (uint32_t)(b >> 5), bit = 1u << (b & 31), i0 = (uint32_t)((tc & 3) << 2);
                 const uint4 d = ldg(S.pc + pc0 + c);
                 const uint4 fr = ldg(S.flagrec + d.x + 4u * g32);
                 uint2 own = make_uint2(0u, 0u);
@@ -77,21 +82,21 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
                     int md, dx, dy;
                     mv_unpack(S, mr, md, dx, dy);
                     if (!kSubpel) {
-                        const int rx = s0 + dx, ry = t + dy;
-                        if ((unsigned)ry < (unsigned)S.Ht) {
+                        const int rx = sc0 + dx, ry = tc + dy;
+                        if ((unsigned)ry < (unsigned)cHt) {
                             const uint4 dr = ldg(S.pc + refpc0 + c);
                             // the 4 reference samples (rx .. rx+3, ry) lie in the block row ry>>2, blocks rx>>2 and (rx>>2)+1
                             const int o = rx & 3, bxa = rx >> 2;
                             const uint32_t j0 = (uint32_t)((ry & 3) << 2);
-                            const int rowb = (ry >> 2) * S.nbx;
+                            const int rowb = (ry >> 2) * cnbx;
                             uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-                            if ((unsigned)bxa < (unsigned)S.nbx) {
+                            if ((unsigned)bxa < (unsigned)cnbx) {
                                 const int rb = rowb + bxa;
                                 const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
                                 const uint32_t rbit = 1u << (rb & 31);
                                 if (rf.x & rbit) qa = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
                             }
-                            if (o && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
+                            if (o && (unsigned)(bxa + 1) < (unsigned)cnbx) {
                                 const int rb = rowb + bxa + 1;
                                 const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
                                 const uint32_t rbit = 1u << (rb & 31);
@@ -107,23 +112,23 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
                         }
                     } else {
                         const int fx = dx & 1, fy = dy & 1;
-                        const int rx = s0 + (dx >> 1), ry = t + (dy >> 1), o = rx & 3, bxa = rx >> 2;
+                        const int rx = sc0 + (dx >> 1), ry = tc + (dy >> 1), o = rx & 3, bxa = rx >> 2;
                         const uint4 dr = ldg(S.pc + refpc0 + c);
                         int h0 = 0, h1 = 0, h2 = 0, h3 = 0;
 #pragma unroll
                         for (int jr = 0; jr < 2; ++jr) {
                             const int r = ry + jr;
-                            if ((jr && !fy) || (unsigned)r >= (unsigned)S.Ht) continue;
+                            if ((jr && !fy) || (unsigned)r >= (unsigned)cHt) continue;
                             const uint32_t j0 = (uint32_t)((r & 3) << 2);
-                            const int rowb = (r >> 2) * S.nbx;
+                            const int rowb = (r >> 2) * cnbx;
                             uint2 qa = make_uint2(0u, 0u), qb = make_uint2(0u, 0u);
-                            if ((unsigned)bxa < (unsigned)S.nbx) {
+                            if ((unsigned)bxa < (unsigned)cnbx) {
                                 const int rb = rowb + bxa;
                                 const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
                                 const uint32_t rbit = 1u << (rb & 31);
                                 if (rf.x & rbit) qa = bise_row4(S.pay + dr.y, ((rf.y + popc(rf.x & (rbit - 1u))) << 4) + j0, dr.w, lut);
                             }
-                            if ((o || fx) && (unsigned)(bxa + 1) < (unsigned)S.nbx) {
+                            if ((o || fx) && (unsigned)(bxa + 1) < (unsigned)cnbx) {
                                 const int rb = rowb + bxa + 1;
                                 const uint4 rf = ldg(S.flagrec + dr.x + 4u * (uint32_t)(rb >> 5));
                                 const uint32_t rbit = 1u << (rb & 31);
@@ -144,7 +149,12 @@ decode_rows_kernel(const __grid_constant__ DevStream S, const int2 *__restrict__
                         else { e0 += q0; e1 += q1; e2 += q2; e3 += q3; }
                     }
                 }
-                a[c][0] += e0; a[c][1] += e1; a[c][2] += e2; a[c][3] += e3;
+                if (!csh) { a[c][0] += e0; a[c][1] += e1; a[c][2] += e2; a[c][3] += e3; }
+                else {  // chroma samples (s0 >> 1) and (s0 >> 1) + 1: elements 0, 1 or 2, 3 of the decoded row
+                    const bool hi = ((s0 >> 1) & 2) != 0;
+                    const int ea = hi ? e2 : e0, eb = hi ? e3 : e1;
+                    a[c][0] += ea; a[c][1] += ea; a[c][2] += eb; a[c][3] += eb;
+                }
             }
         }
 #pragma unroll
@@ -182,7 +192,9 @@ cudaError_t launch_decode_rows(const DevStream &S, const int32_t *d_views, int64
     const long long blocks = (n_seg + kNT - 1) / kNT;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    if (S.sp) decode_rows_kernel<false, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    if (S.cs && S.sp) decode_rows_kernel<false, true, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    else if (S.cs) decode_rows_kernel<false, false, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
+    else if (S.sp) decode_rows_kernel<false, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
     else decode_rows_kernel<false><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_views), n_seg, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
@@ -197,7 +209,9 @@ cudaError_t launch_decode_block_rows(const DevStream &S, const int32_t *d_blocks
     const long long blocks = (n_seg + kNT - 1) / kNT;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     const int aligned = ((reinterpret_cast<uintptr_t>(d_out) & 3u) == 0) ? 1 : 0;
-    if (S.sp) decode_rows_kernel<true, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
+    if (S.cs && S.sp) decode_rows_kernel<true, true, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
+    else if (S.cs) decode_rows_kernel<true, false, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
+    else if (S.sp) decode_rows_kernel<true, true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
     else decode_rows_kernel<true><<<(unsigned)blocks, kNT, 0, st>>>(S, reinterpret_cast<const int2 *>(d_blocks), n_seg, d_out, d_oob, aligned);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();

@@ -1,8 +1,8 @@
 """GPU parity on chroma-subsampled streams (R18): the CUDA path through the C ABI against the oracle.
 
 The streams come from the oracle's encoder (hmlfc_encode does not subsample); decoded pixels bit-exact, views within 1 LSB.
-On these streams hmlfc_decode_views / _blocks run the per-sample kernel; hmlfc_decode the queue kernel's and hmlfc_render (4 x 4 blocks) the tile
-kernel's chroma instantiation."""
+On these streams every entry point runs the chroma instantiation of its fast kernel (hmlfc_render, hmlfc_decode_views / _blocks: 4 x 4 blocks),
+cross-checked against the per-sample kernels."""
 import numpy as np
 import pytest
 
@@ -65,6 +65,10 @@ def test_subsampled_stream_decode_and_render(P, name, tau):
     B = cfg.block
     bc = np.array([(u, v, bx * B + i, by * B + j) for (u, v, bx, by) in blocks for j in range(B) for i in range(B)], dtype=np.int32)
     assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy().reshape(-1, 3), s.decode(bc))
+    P.hmlfc_set_decode_variant(h, P.DECODE_THREAD)   # whole views and blocks once more through the per-sample kernel (4 x 4 blocks: above ran the block-row kernel)
+    assert np.array_equal(P.hmlfc_decode_views(h, _dev(views)).cpu().numpy().reshape(-1, 3), expect)
+    assert np.array_equal(P.hmlfc_decode_blocks(h, _dev(blocks)).cpu().numpy().reshape(-1, 3), s.decode(bc))
+    P.hmlfc_set_decode_variant(h, P.DECODE_AUTO)
     # views
     cams = wl.camera_path(cfg)
     ref = s.render(cams, cfg.out_w, cfg.out_h)

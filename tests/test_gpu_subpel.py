@@ -97,10 +97,14 @@ def test_halfpel_with_subsampled_chroma_and_progressive_levels(P):
     cfg, lf, data, s = _halfpel_stream("mini3", 30, chroma=1)
     h = P.hmlfc_load(data)
     coords = wl.random_coords(cfg, 20_001)
+    views = np.array([(u, v) for v in range(cfg.V) for u in range(cfg.U)], dtype=np.int32)
+    allc = wl.all_coords(cfg)
     for level in range(cfg.height + 1):
         s.set_min_level(level)
         P.hmlfc_set_min_level(h, level)
         assert np.array_equal(P.hmlfc_decode(h, _dev(coords)).cpu().numpy(), s.decode(coords)), level
+        # whole views: the block-row kernel's instantiation for both flags at once
+        assert np.array_equal(P.hmlfc_decode_views(h, _dev(views)).cpu().numpy().reshape(-1, 3), s.decode(allc)), level
     s.set_min_level(0)
     P.hmlfc_free(h)
 
