@@ -5,16 +5,20 @@
 //   acc = topRKV + sum_L [ stored_p(s,t)  (+|-)  stored_r(s+dx, t+dy) ].
 // For uniformly random coordinates every test of that walk (block significant? block predicted? reference
 // block significant?) is taken by a different subset of the lanes, so a thread-per-coordinate kernel runs
-// with ~8 of 32 lanes active (profiles/r01_cta_cfg2.md).  Here each lane still classifies ITS coordinate -- ONE
-// 32-byte sector per level holds the six flag words (res / pred x Y, Co, Cg) of its block's group, uniform control
-// flow -- but everything behind a set flag becomes a task on two small per-warp stacks in shared memory:
-//   motion task  {plane-channel, group, reference plane-channel, pred blocks before | destination}   -> S6 + S7 address part
-//   value task   {plane-channel, group, position in block | res blocks before | sign | destination}  -> S4 rank + S5 (BISE decode_at)
-// A task fetches what only a significant block needs (descriptor, rank word, payload; at 40 dB seven of eight blocks are
-// empty and cost their sample nothing beyond the flag sector) and tasks are executed 32 at a time by all lanes (the stacks are drained whenever they hold >= 32 tasks, so only
-// the last batch of a warp is partial).  Values are accumulated with shared-memory atomics into the
-// destination's (Y, Co, Cg) cell; the owning lane finishes with the inverse colour transform and the staged
-// 96-byte store.  Integer arithmetic only: bit-exact by construction against the per-thread kernel and the oracle.
+// with ~8 of 32 lanes active (profiles/r01c_final.md).  Here each lane still classifies ITS coordinate with uniform control
+// flow, but everything behind a set flag becomes a task on small per-warp stacks in shared memory; tasks are executed 32 at a time by
+// all lanes (a stack is drained whenever it holds >= 32 tasks, so only the last batch of a warp is partial).  Values are
+// accumulated with shared-memory atomics into the destination's (Y, Co, Cg) cell; the owning lane finishes with the inverse
+// colour transform and the staged 96-byte store.  Integer arithmetic only: bit-exact by construction against the per-thread
+// kernel and the oracle.
+//
+// Two kernels:
+//   decode_brec_kernel   on the BLOCK RECORDS hmlfc_load builds (hmlfc_device.cuh): one 32-byte slot per level says what the plane
+//                        holds for the sample and where; value / motion / lookup tasks cover the three channels.  The default.
+//   decode_queue_kernel  on the stream's own BISE strings: kMode 0 (eager: flag records and descriptors of the three channels up front,
+//                        tasks carry them) and 1 (lazy: one flag sector per level, tasks fetch descriptor and rank); its kSubpel / kCs
+//                        instantiations read half-pel (R28) and chroma-subsampled (R18) streams, which have no block records; kDense
+//                        1 / 2 generate whole views / blocks for block sizes other than 4.
 #include "hmlfc_kernels.cuh"
 
 #include <type_traits>
