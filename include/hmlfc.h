@@ -140,11 +140,12 @@ int hmlfc_render(const hmlfc_handle *h, const hmlfc_camera *d_cameras, int n_vie
  * harnesses that forbid cudaMalloc): the same views, byte for byte, from the tile kernels (tile_tables_kernel + render_tiles_kernel)
  * with the tile tables -- the scratch memory hmlfc_render takes from a stream-ordered pool -- in a static device buffer of the library.
  * The call launches two kernels on cuda_stream and calls no cudaMalloc, cudaFree or other allocating routine.
- *   Limit: n_views x ceil(W / w) x ceil(H / 32) <= HMLFC_NOALLOC_MAX_TILES tiles per call (w = 64 where W x H >= 8 x Ws x Ht, else 32),
+ *   Limit: n_views x ceil(W / w) x ceil(H / 32) <= HMLFC_NOALLOC_MAX_TILES tiles per call (w = 64 where W x H >= 8 x Ws x Ht on streams
+ *   with full-resolution chroma and whole-pixel motion, else 32),
  *   e.g. 16 views of 512 x 512; beyond it HMLFC_E_LIMIT and nothing is launched -- render the views in several calls.  The buffer
  *   (HMLFC_NOALLOC_MAX_TILES x 3,200 bytes = 13.1 MB) is held by every GPU that loads the library until the process exits.
- *   Streams: 4 x 4 blocks, full-resolution chroma, whole-pixel motion (the streams whose hmlfc_render uses scratch memory at all);
- *   others HMLFC_E_UNSUPPORTED.  The current device must be the handle's (hmlfc_load sets the buffer up for its device).
+ *   Streams: 4 x 4 blocks (the streams whose hmlfc_render uses scratch memory at all), chroma-subsampled or half-pel ones included
+ *   (not both at once; half-pel windows up to 63); others HMLFC_E_UNSUPPORTED.  The current device must be the handle's (hmlfc_load sets the buffer up for its device).
  *   All calls on a device share the buffer: calls that may OVERLAP on the GPU (different streams without a dependency) race on it
  *   and give undefined pixels; calls on one stream, or ordered by events, are safe.  Progressive decoding applies. */
 #define HMLFC_NOALLOC_MAX_TILES 4096

@@ -332,11 +332,12 @@ int hmlfc_render_noalloc(const hmlfc_handle *h, const hmlfc_camera *d_cameras, i
 {
     if (!h || n_views < 0 || W <= 0 || H <= 0 || n_views > 65535 || (n_views > 0 && (!d_cameras || !d_out))) return HMLFC_E_INVALID;
     const DevStream &D = h->ds;
-    if (D.B != 4 || D.cs || D.sp) return HMLFC_E_UNSUPPORTED;  // streams whose render path has no scratch memory to begin with
+    // streams whose hmlfc_render takes the tile kernels: 4 x 4 blocks; chroma-subsampled or half-pel (not both, windows up to 63) included
+    if (D.B != 4 || (D.cs && D.sp) || (D.sp && D.mv_off > 127)) return HMLFC_E_UNSUPPORTED;
     int nl = 0;
     bool too_large = false;
-    // tile shape as the automatic choice of hmlfc_render makes it where it takes the tile kernels
-    const int config = (long long)W * H >= 8LL * D.Ws * D.Ht ? 4 : 0;
+    // tile shape as the automatic choice of hmlfc_render makes it where it takes the tile kernels (32 x 32 for chroma / half-pel streams)
+    const int config = (!D.cs && !D.sp && (long long)W * H >= 8LL * D.Ws * D.Ht) ? 4 : 0;
     CU(h, launch_render_tiles_noalloc(D, reinterpret_cast<const Camera *>(d_cameras), n_views, W, H, d_out,
                                       static_cast<cudaStream_t>(cuda_stream), &nl, config, &too_large));
     if (too_large) return HMLFC_E_LIMIT;

@@ -94,3 +94,25 @@ def test_render_noalloc_limit_and_arguments(P, enc):
     # an empty batch is a no-op
     P.hmlfc_render_noalloc(h, cams[:0], W, H, out=out[:0])
     P.hmlfc_free(h)
+
+
+@pytest.mark.parametrize("kind", ["chroma", "halfpel"])
+def test_render_noalloc_on_chroma_and_halfpel_streams(P, kind):
+    import oracle as orc
+
+    cfg = wl.CONFIGS["mini3"]
+    lf = wl.light_field(cfg)
+    p = orc.make_params(cfg.U, cfg.V, cfg.Ws, cfg.Ht, cfg.height, cfg.block, min(cfg.window, 4), 15, 30, geometry=wl.geometry(cfg), seed=cfg.seed,
+                        chroma=1 if kind == "chroma" else 0, subpel=1 if kind == "halfpel" else 0)
+    tree = orc.Tree(lf, p)
+    data = tree.serialize()
+    tree.close()
+    h = P.hmlfc_load(data)
+    cams = _dev(wl.camera_path(cfg, n_views=4, out_w=320, out_h=200))   # > 8x the light-field image: still 32 x 32 tiles on these streams
+    ref = _existing(P, h, cams, 320, 200)
+    out = torch.full_like(ref, 0xAB)
+    for _ in range(2):
+        out.fill_(0xAB)
+        P.hmlfc_render_noalloc(h, cams, 320, 200, out=out)
+        assert torch.equal(out, ref)
+    P.hmlfc_free(h)
