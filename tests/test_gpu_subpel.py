@@ -123,3 +123,74 @@ def test_halfpel_offsets_at_the_image_border(P):
     got = P.hmlfc_decode(h, _dev(coords)).cpu().numpy()
     assert np.array_equal(got, s.decode(coords)) and np.array_equal(got.reshape(lf.shape), lf)
     P.hmlfc_free(h)
+
+
+def test_randomised_chroma_and_halfpel_streams(P):
+    """48 seeded random cases: small light fields (2..6 x 2..6 views of 16..48-pixel images, B in {2, 4, 8}, h 1..3, W 1..4, thresholds
+    0..60, three policies) with the chroma flag, the half-pel flag or both, a random slab geometry, a random progressive level and two
+    rotated cameras: every decode entry point bit-exact against the oracle (fast and per-sample kernels), every render variant within
+    1 LSB of the oracle and byte-identical to the thread-per-pixel kernel."""
+    from conftest import random_lf
+
+    rng = np.random.default_rng(19020939)
+    n_fast = 0
+    for case in range(48):
+        B = int(rng.choice([4, 4, 4, 2, 8]))
+        chroma, subpel = [(1, 0), (0, 1), (1, 1)][case % 3]
+        U, V = int(rng.integers(2, 7)), int(rng.integers(2, 7))
+        unit = 2 * B if chroma else B
+        Ws, Ht = unit * int(rng.integers(max(1, 16 // unit), 48 // unit + 1)), unit * int(rng.integers(max(1, 16 // unit), 48 // unit + 1))
+        h, W, tau = int(rng.integers(1, 4)), int(rng.integers(1, 5)), int(rng.integers(0, 60))
+        policy = int(rng.choice([orc.POLICY_ADAPTIVE, orc.POLICY_ALL, orc.POLICY_LITERAL]))
+        step_u, step_v = float(rng.uniform(0.2, 1.0)) * Ws / (2 * U), float(rng.uniform(0.2, 1.0)) * Ht / (2 * V)
+        z_st = float(rng.uniform(0.3, 2.0)) * Ws
+        geo = dict(uv_origin=(float(rng.uniform(-3, 3)), float(rng.uniform(-3, 3))), uv_step=(step_u, step_v),
+                   st_origin=(float(rng.uniform(-5, 5)), float(rng.uniform(-5, 5))), st_step=(float(rng.uniform(0.5, 2.0)), float(rng.uniform(0.5, 2.0))),
+                   z_st=z_st)
+        lf = random_lf(rng, U, V, Ws, Ht)
+        p = orc.make_params(U, V, Ws, Ht, h, B, W, tau // 2, tau, policy, geometry=geo, seed=case, chroma=chroma, subpel=subpel)
+        tree = orc.Tree(lf, p)
+        data = tree.serialize()
+        tree.close()
+        s = orc.Stream(data)
+        hd = P.hmlfc_load(data)
+        L = int(rng.integers(0, h + 1))
+        s.set_min_level(L)
+        P.hmlfc_set_min_level(hd, L)
+        tag = (case, B, chroma, subpel, h, W, tau, policy, L)
+        # decode: every coordinate, whole views, random blocks -- default (fast) kernels and the per-sample ones
+        coords = np.array([(u, v, x, y) for v in range(V) for u in range(U) for y in range(Ht) for x in range(Ws)], dtype=np.int32)
+        expect = s.decode(coords)
+        views = np.array([(u, v) for v in range(V) for u in range(U)], dtype=np.int32)
+        nb = 64
+        blocks = np.stack([rng.integers(0, U, nb), rng.integers(0, V, nb), rng.integers(0, Ws // B, nb), rng.integers(0, Ht // B, nb)], axis=1).astype(np.int32)
+        bc = np.array([(u, v, bx * B + i, by * B + j) for (u, v, bx, by) in blocks for j in range(B) for i in range(B)], dtype=np.int32)
+        bexp = s.decode(bc)
+        for variant in (P.DECODE_AUTO, P.DECODE_THREAD):
+            P.hmlfc_set_decode_variant(hd, variant)
+            assert np.array_equal(P.hmlfc_decode(hd, _dev(coords)).cpu().numpy(), expect), tag + (variant, "decode")
+            assert np.array_equal(P.hmlfc_decode_views(hd, _dev(views)).cpu().numpy().reshape(-1, 3), expect), tag + (variant, "views")
+            assert np.array_equal(P.hmlfc_decode_blocks(hd, _dev(blocks)).cpu().numpy().reshape(-1, 3), bexp), tag + (variant, "blocks")
+        P.hmlfc_set_decode_variant(hd, P.DECODE_AUTO)
+        # render: two rotated off-plane cameras
+        uc = (geo["uv_origin"][0] + 0.5 * (U - 1) * step_u, geo["uv_origin"][1] + 0.5 * (V - 1) * step_v)
+        sc = (geo["st_origin"][0] + 0.5 * (Ws - 1) * geo["st_step"][0], geo["st_origin"][1] + 0.5 * (Ht - 1) * geo["st_step"][1])
+        cams = []
+        for _ in range(2):
+            eye = (uc[0] + rng.uniform(-0.35, 0.35) * U * step_u, uc[1] + rng.uniform(-0.35, 0.35) * V * step_v, -float(rng.uniform(0.0, 0.8)) * z_st)
+            look = (sc[0] + rng.uniform(-0.3, 0.3) * Ws * geo["st_step"][0], sc[1] + rng.uniform(-0.3, 0.3) * Ht * geo["st_step"][1], z_st)
+            d = float(np.linalg.norm(np.array(look) - np.array(eye)))
+            th = float(rng.uniform(0.1, 0.5)) * Ws * geo["st_step"][0] / d
+            cams.append(wl._camera(eye, look, th, th * float(rng.uniform(0.6, 1.4))))
+        cams = np.stack(cams)
+        Wo, Ho = int(rng.integers(20, 100)), int(rng.integers(20, 80))
+        ref = s.render(cams, Wo, Ho)
+        P.hmlfc_set_render_variant(hd, P.RENDER_PIXEL)
+        unshared = P.hmlfc_render(hd, _dev(cams), Wo, Ho).cpu().numpy()
+        assert np.abs(unshared.astype(int) - ref.astype(int)).max() <= 1, tag
+        for variant in (P.RENDER_AUTO, P.RENDER_TILES, P.RENDER_CTA_SMALL, P.RENDER_WARP):
+            P.hmlfc_set_render_variant(hd, variant)
+            assert np.array_equal(P.hmlfc_render(hd, _dev(cams), Wo, Ho).cpu().numpy(), unshared), tag + (variant,)
+        n_fast += int(B == 4)
+        P.hmlfc_free(hd)
+    assert n_fast >= 20   # most cases ran the instantiations of the fast kernels (4 x 4 blocks)
