@@ -198,7 +198,8 @@ int hmlfc_footprint_decode(hmlfc_handle *h, const int32_t *d_coords, int64_t n, 
  * pool): 32 x 32 tile with 3 / 4 CTAs per SM, 64 x 32 tile with 512 threads, 64 x 32 tile with 256 threads (8
  * pixels per thread) and 2 / 3 CTAs per SM.  The automatic choice takes 7 when a view has fewer than twice the
  * pixels of a light-field image (little magnification: many samples per tile), 15 when it has at least eight
- * times as many, else 11. */
+ * times as many, else 11.  On streams with subsampled chroma or half-pel motion offsets (4 x 4 blocks) 0 and 6 .. 15 all run the
+ * tile kernel's instantiation for that kind of stream (32 x 32 tiles, 3 CTAs per SM); 4 / 5 and other block sizes run per pixel. */
 int hmlfc_set_render_variant(hmlfc_handle *h, int variant);
 
 /* Progressive decoding (PAPER.md:57, :183 name the property; R26): hmlfc_decode / hmlfc_render sum the top-level RKV and the
@@ -212,11 +213,12 @@ int hmlfc_set_min_level(hmlfc_handle *h, int min_level);
  * motion-record and value decodes run as 32-wide batches from per-warp task stacks): 2 reads the three
  * channels' flag records and descriptors of every level up front, 3 reads ONE 32-byte sector of flag words per
  * level and lets the tasks of significant blocks fetch the rest; 4 reads the BLOCK RECORDS hmlfc_load builds for
- * streams with full-resolution chroma (every stored value and motion record once more, as plain binary fields
+ * streams with full-resolution chroma and whole-pixel motion (every stored value and motion record once more, as plain binary fields
  * grouped per block: one sector per level says what a plane holds for a sample and where, one or two more hold
  * all three channels of it; counted in device_bytes).  The automatic choice is 4 where the stream has block
- * records (subsampled streams have none and run the per-sample kernel whatever the variant); otherwise 3 for streams whose device form fits the
- * L2 cache and where at most a quarter of the block flags are set, else 2. */
+ * records; chroma-subsampled and half-pel streams have none and run, for 0 and 2 .. 4 alike, the instantiation of kernel 2 for that kind of
+ * stream; otherwise 3 for streams whose device form fits the L2 cache and where at most a quarter of the block flags are set, else 2.
+ * hmlfc_decode_views / _blocks: 0 = the block-row kernel (4 x 4 blocks), anything else their lane-per-pixel kernels. */
 int hmlfc_set_decode_variant(hmlfc_handle *h, int variant);
 
 /* Encoder side (first "next" row): phase-shifted exhaustive block motion search, PAPER.md:227-248,
